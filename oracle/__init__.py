@@ -1,0 +1,122 @@
+"""ctypes front end of the CPU float64 oracle (`oracle/cp_oracle.c`).
+
+TEST INFRASTRUCTURE ONLY: importable from tests/, `__graft_entry__.smoke()` and
+`bench.py`'s cpu_baseline / `--impl reference` legs.  Nothing under
+`paper_2606_24506_b200/` may import it, and it imports nothing from there.
+This file only marshals arguments; all arithmetic is in the C file.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "cp_oracle.c")
+_LIB = os.path.join(_HERE, "libcp_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (plain C, no fast-math, no FMA contraction)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+                               "-Wall", "-Wextra", _SRC, "-o", tmp, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_LIB)
+        u16p = ctypes.POINTER(ctypes.c_uint16)
+        i32p = ctypes.POINTER(ctypes.c_int32)
+        f64p = ctypes.POINTER(ctypes.c_double)
+        L.cpo_num_threads.restype = ctypes.c_int
+        L.cpo_gather.restype = ctypes.c_int
+        L.cpo_gather.argtypes = [u16p, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32,
+                                 ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                 i32p, ctypes.c_int, ctypes.c_int, u16p, u16p]
+        L.cpo_attention.restype = ctypes.c_int
+        L.cpo_attention.argtypes = [u16p, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32,
+                                    ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                    ctypes.c_int, ctypes.c_float,
+                                    i32p, ctypes.c_int, ctypes.c_int,
+                                    u16p, i32p, ctypes.c_int, ctypes.c_int, f64p, f64p]
+        _lib = L
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().cpo_num_threads())
+
+
+def _p(a: np.ndarray, ty):
+    return a.ctypes.data_as(ctypes.POINTER(ty))
+
+
+def gather(arena: np.ndarray, page_tokens: int, page_bytes: int, num_pages: int, kind: int,
+           n_kv_heads: int, d_k: int, d_v: int, page_ids: np.ndarray, context_len: int):
+    """-> (K uint16 [T,Hkv,d_k], V uint16 [T,Hkv,d_v]) bit patterns."""
+    arena = np.ascontiguousarray(arena, dtype=np.uint16)
+    page_ids = np.ascontiguousarray(page_ids, dtype=np.int32)
+    k = np.empty((context_len, n_kv_heads, d_k), dtype=np.uint16)
+    v = np.empty((context_len, n_kv_heads, d_v), dtype=np.uint16)
+    rc = lib().cpo_gather(_p(arena, ctypes.c_uint16), page_tokens, page_bytes, num_pages, kind,
+                          n_kv_heads, d_k, d_v, _p(page_ids, ctypes.c_int32), page_ids.size,
+                          context_len, _p(k, ctypes.c_uint16), _p(v, ctypes.c_uint16))
+    if rc != 0:
+        raise ValueError("cpo_gather failed: %d" % rc)
+    return k, v
+
+
+def attention(arena: np.ndarray, page_tokens: int, page_bytes: int, num_pages: int, kind: int,
+              n_q_heads: int, n_kv_heads: int, d_k: int, d_v: int, softmax_scale: float,
+              page_ids: np.ndarray, context_len: int, q: np.ndarray,
+              heads: Optional[Sequence[int]] = None, n_splits: int = 1):
+    """-> (O float64 [n_sel, d_v], LSE float64 [n_sel]) for one request."""
+    arena = np.ascontiguousarray(arena, dtype=np.uint16)
+    page_ids = np.ascontiguousarray(page_ids, dtype=np.int32)
+    q = np.ascontiguousarray(q, dtype=np.uint16)
+    assert q.size == n_q_heads * d_k
+    if heads is None:
+        n_sel, hp = n_q_heads, None
+    else:
+        h = np.ascontiguousarray(heads, dtype=np.int32)
+        n_sel, hp = h.size, _p(h, ctypes.c_int32)
+    out = np.empty((n_sel, d_v), dtype=np.float64)
+    lse = np.empty((n_sel,), dtype=np.float64)
+    rc = lib().cpo_attention(_p(arena, ctypes.c_uint16), page_tokens, page_bytes, num_pages, kind,
+                             n_q_heads, n_kv_heads, d_k, d_v, ctypes.c_float(softmax_scale),
+                             _p(page_ids, ctypes.c_int32), page_ids.size, context_len,
+                             _p(q, ctypes.c_uint16), hp, n_sel, n_splits,
+                             _p(out, ctypes.c_double), _p(lse, ctypes.c_double))
+    if rc != 0:
+        raise ValueError("cpo_attention failed: %d" % rc)
+    return out, lse
+
+
+def decode_workload(w, heads_per_request: Optional[Sequence[Optional[Sequence[int]]]] = None,
+                    request_indices: Optional[Sequence[int]] = None, n_splits: int = 1):
+    """Run the oracle over (a subset of) a `workloads.Workload`, request by request.
+
+    Returns a list of (O, LSE) per selected request.  `w` is duck-typed so that this
+    module need not import the generator.
+    """
+    res = []
+    idx = range(len(w.requests)) if request_indices is None else request_indices
+    for n, i in enumerate(idx):
+        r = w.requests[i]
+        m = w.models[r.model_id]
+        heads = None if heads_per_request is None else heads_per_request[n]
+        res.append(attention(w.arena, w.page_tokens, w.page_bytes, w.num_pages, m.kind,
+                             m.n_q_heads, m.n_kv_heads, m.head_dim_qk, m.head_dim_v,
+                             m.softmax_scale, r.page_ids, r.context_len, w.q[i],
+                             heads=heads, n_splits=n_splits))
+    return res
