@@ -1,0 +1,311 @@
+#!/usr/bin/env python
+"""bench.py -- paged decode-attention KV GB/s on one B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (translation + split-KV partial attention + LSE
+combine, all inside one persistent launch) over one synthetic batch: one
+cp_decode_attention call.  Default workload: BASELINE.json configs[1], the shared pool of
+4 cold GQA models (344 MB of KV per step, larger than the 126 MB L2, so no flush is
+needed between steps).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+
+Prints ONE JSON line (see DESIGN.md §7 for every field).  N > 1 = independent replicas
+(the path does not shard: BASELINE north_star fixes one GPU).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "paged decode-attention KV GB/s"
+UNIT = "GB/s"
+L2_BYTES = 126 * 1024 * 1024
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d.get("bf16_tflops", 1590.0)),
+                "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", 1400.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+def workload_desc(w, k):
+    return {"workload": "cfg%d:%s" % (k, w.name), "requests": len(w.requests),
+            "tokens": w.total_tokens(), "page_tokens": w.page_tokens,
+            "kv_bytes_per_step": w.algorithmic_bytes(), "flops_per_step": w.flops(),
+            "l2": ("inputs %.0f MB > L2 126 MB, no flush" % (w.algorithmic_bytes() / 1e6))
+            if w.algorithmic_bytes() > L2_BYTES else "L2 flushed between steps (256 MB write)"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed regions run."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1] or [r for (_, r) in self.rows]
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample_plan(w, budget_s: float):
+    """Pick a bounded sample of (request, head) pairs for the CPU oracle: every request, an
+    evenly spaced subset of heads, sized from a quick calibration so one pass costs about
+    budget_s.  Returns (heads_per_request, fraction_of_heads)."""
+    import oracle
+    r = min(range(len(w.requests)), key=lambda i: w.requests[i].context_len)
+    m = w.models[w.requests[r].model_id]
+    t = time.perf_counter()
+    oracle.decode_workload(w, request_indices=[r], heads_per_request=[[0]])
+    dt = max(time.perf_counter() - t, 1e-4)
+    per_head_token = dt / w.requests[r].context_len / ((m.head_dim_qk + m.head_dim_v) / 256.0)
+    cores = oracle.num_threads()
+    full = sum(w.requests[i].context_len * w.models[w.requests[i].model_id].n_q_heads *
+               (w.models[w.requests[i].model_id].head_dim_qk + w.models[w.requests[i].model_id].head_dim_v) / 256.0
+               for i in range(len(w.requests))) * per_head_token / cores
+    frac = min(1.0, budget_s / max(full, 1e-9))
+    heads, used, total = [], 0, 0
+    for rq in w.requests:
+        hq = w.models[rq.model_id].n_q_heads
+        n = max(1, int(round(hq * frac)))
+        hs = sorted(set(int(x) for x in np.linspace(0, hq - 1, n)))
+        heads.append(hs)
+        used += len(hs) * rq.context_len
+        total += hq * rq.context_len
+    return heads, used / total
+
+
+def run_reference(args, w, k):
+    """--impl reference: the CPU oracle, as it stands, timed on the host cores."""
+    import oracle
+    oracle.build()
+    cores = oracle.num_threads()
+    budget = min(1.5, 150.0 / max(1, args.steps + args.warmup))
+    heads, frac = oracle_sample_plan(w, budget)
+    for _ in range(args.warmup):
+        oracle.decode_workload(w, heads_per_request=heads)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.decode_workload(w, heads_per_request=heads)
+    dt = time.perf_counter() - t0
+    value = frac * w.algorithmic_bytes() * args.steps / dt / 1e9
+    sample = "every request, %.1f%% of the (head, token) pairs (evenly spaced heads) per step" % (100 * frac)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps / frac,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_desc(w, k),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0,
+            "note": "ms_per_step is extrapolated to the full step from the sampled fraction"}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--kernel", type=int, default=0, help="CP_OPT_KERNEL (0 auto, 1 generic)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    import workloads as W
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        run_reference(args, W.config(args.config), args.config)
+        return 0
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    import paper_2606_24506_b200 as cp
+    from paper_2606_24506_b200.harness import DeviceWorkload
+
+    dev = "cuda:%d" % local_rank
+    torch.cuda.set_device(dev)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    k = args.config
+    w = W.config(k)
+    dw = DeviceWorkload(w, dev)
+    dw.pool.set_option(cp.CP_OPT_KERNEL, args.kernel)
+    dw.ensure_workspace()
+    abytes = w.algorithmic_bytes()
+    flush = None
+    if abytes <= L2_BYTES:
+        flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+
+    # ---------------- device-resident leg: K steps, inputs already in HBM
+    for _ in range(args.warmup):
+        dw.decode()
+    barrier()
+    c0 = dw.pool.counters()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps)]
+    t_wall0 = time.time()
+    start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    start.record()
+    for i in range(args.steps):
+        if flush is not None:
+            flush.fill_(i & 0xFF)
+        ev[2 * i].record()
+        dw.decode()
+        ev[2 * i + 1].record()
+    stop.record()
+    barrier()
+    c1 = dw.pool.counters()
+    kern_ms = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(args.steps)]
+    region_ms = start.elapsed_time(stop)
+    step_ms = float(np.sum(kern_ms)) / args.steps if flush is not None else region_ms / args.steps
+    t = torch.tensor([step_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    step_ms = float(t.item())
+    launches = c1["kernel_launches"] - c0["kernel_launches"]
+
+    # ---------------- end-to-end leg: host buffers through cp_decode_attention_host
+    need = dw.pool.decode_workspace_bytes_host(dw.ids)
+    ws = torch.empty(need, dtype=torch.uint8, device=dev)
+    q_host = torch.from_numpy(w.q_packed().view(np.int16)).pin_memory()
+    o_host = torch.empty(dw.out.numel(), dtype=torch.float32).pin_memory()
+    l_host = torch.empty(dw.lse.numel(), dtype=torch.float32).pin_memory()
+    for _ in range(3):
+        dw.pool.decode_attention_host(dw.ids, q_host, o_host, l_host, ws, need, dw.stream())
+    barrier()
+    e2e_steps = args.steps
+    t0 = time.perf_counter()
+    for i in range(e2e_steps):
+        if flush is not None:
+            flush.fill_(i & 0xFF)
+        dw.pool.decode_attention_host(dw.ids, q_host, o_host, l_host, ws, need, dw.stream())
+    torch.cuda.synchronize()
+    e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
+    t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item())
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peaks = measured_peaks()
+    value = world * abytes / (step_ms * 1e-3) / 1e9
+    kern_avg_ms = float(np.mean(kern_ms))
+    achieved = abytes / (kern_avg_ms * 1e-3) / 1e9
+    mla = any(m.kind == 1 for m in w.models)
+    roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+            "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+            "kernel_us": 1e3 * kern_avg_ms, "kernel_us_p10_p50_p90":
+                [float(x) * 1e3 for x in np.percentile(kern_ms, [10, 50, 90])],
+            "frac_of_nominal_8000": achieved / 8000.0}
+    if mla:
+        tf = w.flops() / (kern_avg_ms * 1e-3) / 1e12
+        roof["tensor"] = {"achieved_tflops": tf, "peak_burst": peaks["bf16_tflops"],
+                          "frac_burst": tf / peaks["bf16_tflops"]}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": step_ms, "us_per_step": 1e3 * step_ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16 in, fp32 accumulate",
+            "data": "synthetic", "config": workload_desc(w, k), "clocks": clocks,
+            "e2e": {"value": world * abytes / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
+                    "us_per_step": 1e3 * e2e_ms,
+                    "h2d_bytes_per_step": int(q_host.numel() * 2),
+                    "d2h_bytes_per_step": int(o_host.numel() * 4 + l_host.numel() * 4)},
+            "gpu_launches": int(launches), "roofline": roof,
+            "pct_of_hbm_peak": {"measured_copy": 100 * achieved / peaks["hbm_gbs"], "nominal_8TBs": 100 * achieved / 8000.0}}
+
+    if not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        heads, frac = oracle_sample_plan(w, 8.0)
+        t0 = time.perf_counter()
+        n = 0
+        while True:
+            oracle.decode_workload(w, heads_per_request=heads)
+            n += 1
+            if time.perf_counter() - t0 > 10.0 or n >= 3:
+                break
+        dt = (time.perf_counter() - t0) / n
+        line["cpu_baseline"] = {"value": frac * abytes / dt / 1e9, "unit": UNIT, "cores": oracle.num_threads(),
+                                "kind": "oracle", "us_per_step": 1e6 * dt / frac,
+                                "sample": "%d pass(es) over every request, %.1f%% of the (head, token) pairs" % (n, 100 * frac)}
+    print(json.dumps(line))
+    dw.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,233 @@
+/*
+ * crosspool.h -- C ABI of the B200-native paged decode attention on a shared KV-cache pool.
+ *
+ * One hot path of CrossPool (arxiv 2606.24506): the decode-step attention that runs
+ * locally on the shared, virtualized KV-cache pool, where the paged KV blocks of many
+ * cold models' active requests live interleaved in one device arena behind a page table.
+ * Citations are PAPER.md line numbers (the paper text) and DESIGN.md readings.
+ *
+ * Conventions for every entry point
+ *   - extern "C", plain pointers and sizes; no C++ types, no exceptions cross the boundary.
+ *   - every call returns a cp_status (0 = CP_OK, negative = error); it never aborts.
+ *   - "host" / "dev" in a parameter name says where the pointer lives.  All large device
+ *     buffers (arena, Q, O, LSE, workspace) are owned by the CALLER (e.g. torch tensors);
+ *     the library owns only its metadata (page table, work list, counters).
+ *   - argument errors are detected synchronously and leave the pool unchanged.
+ *   - device work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream) and the call returns without synchronising, except the
+ *     *_host variant which synchronises the stream before returning.
+ *   - an asynchronous CUDA fault surfaces as CP_ERR_CUDA on the call that observes it.
+ *   - a pool is not thread-safe; the caller serialises calls on one pool.
+ *   - device pointers must be 16-byte aligned (the arena 256-byte aligned).
+ *   - there is NO CPU fallback: without a usable CUDA device the compute entry points
+ *     return CP_ERR_CUDA.
+ *
+ * Arena layout (reading R1; the paper fixes only "page size" and per-token
+ * KV bytes kappa(M)): the arena is num_pages pages of page_bytes.  ONE
+ * PAGE holds page_tokens tokens of ONE kv head of one request:
+ *     kind CP_KIND_KV : K block [page_tokens][head_dim_qk] bf16 row-major, immediately
+ *                       followed by V block [page_tokens][head_dim_v] bf16;
+ *     kind CP_KIND_MLA: one block [page_tokens][head_dim_qk] bf16 (the latent row, e.g.
+ *                       512 latent + 64 rope); the value of a token is the first
+ *                       head_dim_v entries of its row.
+ * A model fits the pool if its block(s) fit in page_bytes (trailing bytes unused).
+ * A request's page list is PAGE-MAJOR: page_ids[lp * n_kv_heads + c] is the physical page
+ * of logical page lp (tokens lp*P .. lp*P+P-1) of kv head c.  Query head h reads kv head
+ * c = h / (n_q_heads / n_kv_heads) (reading A2).  Slots past context_len in the last
+ * page, and all unmapped pages, are undefined and never influence a result (reading A5).
+ */
+#ifndef CROSSPOOL_H_
+#define CROSSPOOL_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cp_pool cp_pool;   /* opaque; created by cp_pool_create, owned by the library */
+typedef int32_t cp_status;
+
+enum {
+    CP_OK = 0,
+    CP_ERR_INVALID_ARG = -1,      /* NULL / out-of-range / inconsistent argument           */
+    CP_ERR_NO_PAGES = -2,         /* page budget exhausted: the paper's "reject" (L122)     */
+    CP_ERR_PAGE_RANGE = -3,       /* a page id is >= num_pages or negative                  */
+    CP_ERR_PAGE_IN_USE = -4,      /* a page is already owned (or repeated in the list)      */
+    CP_ERR_UNKNOWN_REQUEST = -5,  /* request id not mapped                                  */
+    CP_ERR_UNSUPPORTED = -6,      /* model shape outside what the kernels implement         */
+    CP_ERR_WORKSPACE = -7,        /* workspace_dev too small or misaligned                  */
+    CP_ERR_CUDA = -8              /* CUDA runtime / driver error (no device, launch fault)  */
+};
+
+enum { CP_KIND_KV = 0, CP_KIND_MLA = 1 };
+
+/* Per-model KV description: "KV tensor layouts, numbers of KV heads, and per-token KV
+ * bytes" differ per colocated model (challenge C1; kappa(M) in L103). */
+typedef struct {
+    int32_t kind;            /* CP_KIND_KV (MQA/GQA/MHA) or CP_KIND_MLA                      */
+    int32_t n_q_heads;       /* Hq                                                          */
+    int32_t n_kv_heads;      /* Hkv; Hq % Hkv == 0; MLA requires 1                          */
+    int32_t head_dim_qk;     /* d_k (MLA: full latent row width, e.g. 576)                  */
+    int32_t head_dim_v;      /* d_v (MLA: leading part of the row that is the value)        */
+    float   softmax_scale;   /* sigma; multiplies the fp32 dot product (reading A3)         */
+} cp_model_cfg;
+
+/* One tile of the device work list (introspection only; see cp_decode_plan). */
+typedef struct {
+    int32_t batch_index;     /* position of the request in the decode batch                 */
+    int32_t kv_head;         /* kv head of the (request, kv head) group this tile belongs to */
+    int32_t split;           /* index of this KV split inside the group                     */
+    int32_t n_splits;        /* number of KV splits of the group                            */
+    int32_t page_begin;      /* first logical page of the tile                              */
+    int32_t page_end;        /* one past the last logical page                              */
+} cp_tile_info;
+
+/* Tunables (cp_pool_set_option). */
+enum {
+    CP_OPT_KERNEL = 0,       /* 0 = auto (tensor-core kernels where the shape allows),
+                                1 = force the generic SIMT kernel (any supported shape)      */
+    CP_OPT_NUM_CTAS = 1,     /* persistent grid size; 0 = number of SMs of the device       */
+    CP_OPT_WAVES_X16 = 2,    /* target tiles per CTA, in 1/16 units (default 32 = 2.0)      */
+    CP_OPT_MIN_TILE_PAGES = 3 /* lower bound on pages per tile (default 2)                   */
+};
+
+/*
+ * cp_pool_create -- describe a shared KV-cache pool over a caller-owned device arena.
+ * "a shared KV-cache pool ... total KV-cache pool page budget"; the
+ * budget is num_pages.  The arena is never read or written by this call.  No CUDA call is
+ * made here (device metadata is allocated lazily by the first compute call), so pool
+ * bookkeeping can be exercised on a host without a GPU.
+ *   arena_dev              device pointer, 256-B aligned, >= num_pages * page_bytes bytes
+ *   page_tokens            P, tokens per page (multiple of 16, <= 256)
+ *   page_bytes             bytes per page (multiple of 256)
+ *   models / n_models      copied; model ids are indices into this array
+ *   max_requests           request ids are 0 .. max_requests-1
+ *   max_pages_per_request  capacity of one request's page list (entries = logical pages
+ *                          * n_kv_heads)
+ * Errors: INVALID_ARG (NULL, zero sizes, arena too small / misaligned), UNSUPPORTED (Hq not a
+ * multiple of Hkv, head dims not multiples of 16 or > 576 (qk) / 512 (v), MLA with Hkv != 1
+ * or d_v > d_k, a model whose page does not fit page_bytes).
+ */
+cp_status cp_pool_create(void *arena_dev, uint64_t arena_bytes,
+                         uint32_t page_tokens, uint32_t page_bytes, uint32_t num_pages,
+                         const cp_model_cfg *models, int32_t n_models,
+                         int32_t max_requests, int32_t max_pages_per_request,
+                         cp_pool **out);
+
+/* cp_pool_free -- release the library's metadata (host and device).  Never touches the
+ * arena.  NULL is accepted. */
+cp_status cp_pool_free(cp_pool *pool);
+
+/*
+ * cp_pool_map_pages -- the virtualizer's slow path: "map physical KV pages on demand ...
+ * mapping and unmapping remain slow paths outside the per-token critical path"
+ * (PAPER.md:L122).  The first call for a request id creates the request (model_id fixed
+ * from then on); later calls APPEND page ids and/or raise context_len.
+ *   page_ids_host   n_page_ids physical page ids to append (page-major, see top), or NULL
+ *                   with n_page_ids > 0 to let the library take pages from its free list,
+ *                   or NULL with n_page_ids == 0 to only update context_len
+ *   context_len     number of valid tokens now in the pool for this request (>= 1, never
+ *                   decreasing, <= mapped logical pages * P) (readings A4, A8)
+ * All-or-nothing.  Errors: INVALID_ARG, UNSUPPORTED (n_page_ids not a multiple of Hkv),
+ * PAGE_RANGE, PAGE_IN_USE, NO_PAGES (budget exhausted -> the caller queues or rejects,
+ * PAPER.md:L122), UNKNOWN_REQUEST is never returned here.
+ * The device copy of the tables is refreshed by the next compute call on its stream.
+ */
+cp_status cp_pool_map_pages(cp_pool *pool, int32_t request_id, int32_t model_id,
+                            const int32_t *page_ids_host, int32_t n_page_ids,
+                            int32_t context_len);
+
+/* cp_pool_unmap_request -- the request finished decoding: its pages return to the free
+ * list ("Active KV pages are kept until their decode requests finish"). */
+cp_status cp_pool_unmap_request(cp_pool *pool, int32_t request_id);
+
+/* cp_pool_request_info -- query a request: model, context length, number of page-list
+ * entries; if page_ids_out_host != NULL copies up to cap entries.  Any out pointer may be
+ * NULL. */
+cp_status cp_pool_request_info(const cp_pool *pool, int32_t request_id, int32_t *model_id,
+                               int32_t *context_len, int32_t *n_page_ids,
+                               int32_t *page_ids_out_host, int32_t cap);
+
+/* cp_pool_stats -- free / used pages against the page budget. */
+cp_status cp_pool_stats(const cp_pool *pool, uint32_t *free_pages, uint32_t *used_pages);
+
+/* cp_pool_set_option -- tunables above; INVALID_ARG for unknown keys / bad values. */
+cp_status cp_pool_set_option(cp_pool *pool, int32_t key, int64_t value);
+
+/*
+ * cp_pool_gather_kv -- page-table translation + KV gather (hot-path step a2): "attention
+ * kernels can use a logical KV address space while the virtualizer controls physical page
+ * allocation".  Copies the raw 16-bit patterns of tokens 0..context_len-1:
+ *   k_out_dev  bf16 [T][Hkv][d_k]   (MLA: [T][d_k], the latent rows)
+ *   v_out_dev  bf16 [T][Hkv][d_v]   (MLA: [T][d_v], the leading part); may be NULL
+ * Bit-exact (NaN payloads, -0 included).  Runs on `stream`.
+ */
+cp_status cp_pool_gather_kv(cp_pool *pool, int32_t request_id,
+                            void *k_out_dev, void *v_out_dev, void *stream);
+
+/*
+ * cp_decode_workspace_bytes -- bytes of scratch cp_decode_attention needs for this batch
+ * (split-KV partial results; 0 when no group is split).
+ */
+cp_status cp_decode_workspace_bytes(cp_pool *pool, const int32_t *request_ids_host,
+                                    int32_t n_requests, uint64_t *bytes_out);
+
+/*
+ * cp_decode_attention -- ONE decode step of attention for a batch of requests of any mix
+ * of the pool's models (batch sizes 1-4 per model are typical): for every
+ * request r in the batch and query head h,
+ *     s_t = sigma * <q_h, k_t>,  t = 0 .. T_r - 1  (k_t, v_t read through the page table)
+ *     O_h = sum_t softmax(s)_t v_t,          LSE_h = ln sum_t exp(s_t)
+ * computed as split-KV partial attention (online softmax, fp32 accumulation over bf16 K/V)
+ * plus a log-sum-exp combine, scheduled by persistent kernels over a device-resident
+ * work list of (request, model, kv-split) tiles: one launch per attention kind present in
+ * the batch, no per-request launches (GPU-resident control instead of host-driven
+ * dispatch).
+ *   request_ids_host  batch order; ids must be distinct and mapped
+ *   q_dev    bf16, packed in batch order, per request [Hq][d_k]
+ *   out_dev  fp32, packed in batch order, per request [Hq][d_v]
+ *   lse_dev  fp32, packed in batch order, per request [Hq] (natural log, scale inside)
+ *   workspace_dev / workspace_bytes  >= cp_decode_workspace_bytes(...), 16-B aligned
+ * Errors: INVALID_ARG, UNKNOWN_REQUEST, WORKSPACE, CUDA.
+ */
+cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                              const void *q_dev, float *out_dev, float *lse_dev,
+                              void *workspace_dev, uint64_t workspace_bytes, void *stream);
+
+/*
+ * cp_decode_attention_host -- the same step with HOST query / result buffers: copies q
+ * host->device, runs cp_decode_attention, copies O and LSE device->host and synchronises
+ * `stream`.  The KV arena stays resident on the device (it is the cache).  The staging
+ * copies of q / O / LSE live at the front of workspace_dev: it must hold
+ * cp_decode_workspace_bytes_host(...) bytes.
+ */
+cp_status cp_decode_workspace_bytes_host(cp_pool *pool, const int32_t *request_ids_host,
+                                         int32_t n_requests, uint64_t *bytes_out);
+cp_status cp_decode_attention_host(cp_pool *pool, const int32_t *request_ids_host,
+                                   int32_t n_requests, const void *q_host, float *out_host,
+                                   float *lse_host, void *workspace_dev, uint64_t workspace_bytes,
+                                   void *stream);
+
+/*
+ * cp_decode_plan -- introspection of the device work list the next cp_decode_attention on
+ * this batch will consume (host only, no CUDA): writes up to cap tiles in the order the
+ * persistent CTAs pop them.  n_tiles_out receives the total number of tiles,
+ * n_groups_out the number of (request, kv head) groups.  tiles_out may be NULL.
+ */
+cp_status cp_decode_plan(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                         cp_tile_info *tiles_out, int32_t cap, int32_t *n_tiles_out,
+                         int32_t *n_groups_out);
+
+/* cp_pool_counters -- monotonically increasing counters since cp_pool_create: kernels
+ * launched by the library, work-list (re)builds, host->device metadata bytes. */
+cp_status cp_pool_counters(const cp_pool *pool, uint64_t *kernel_launches,
+                           uint64_t *plan_builds, uint64_t *metadata_h2d_bytes);
+
+/* cp_status_string -- static, never NULL. */
+const char *cp_status_string(cp_status status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CROSSPOOL_H_ */

@@ -1,0 +1,239 @@
+"""paper_2606_24506_b200 -- thin Python binding of libcrosspool (include/crosspool.h).
+
+B200-native (sm_100a) paged decode attention on CrossPool's shared KV-cache pool.
+This module only marshals arguments: every step of the hot path runs in the CUDA
+kernels behind the C ABI.  PyTorch is used by callers for device memory and streams
+only.  There is no CPU fallback: if the shared library is missing or no CUDA device is
+usable the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcrosspool.so")
+
+CP_OK = 0
+CP_ERR_INVALID_ARG = -1
+CP_ERR_NO_PAGES = -2
+CP_ERR_PAGE_RANGE = -3
+CP_ERR_PAGE_IN_USE = -4
+CP_ERR_UNKNOWN_REQUEST = -5
+CP_ERR_UNSUPPORTED = -6
+CP_ERR_WORKSPACE = -7
+CP_ERR_CUDA = -8
+
+CP_KIND_KV = 0
+CP_KIND_MLA = 1
+
+CP_OPT_KERNEL = 0
+CP_OPT_NUM_CTAS = 1
+CP_OPT_WAVES_X16 = 2
+CP_OPT_MIN_TILE_PAGES = 3
+
+
+class cp_model_cfg(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int32), ("n_q_heads", ctypes.c_int32),
+                ("n_kv_heads", ctypes.c_int32), ("head_dim_qk", ctypes.c_int32),
+                ("head_dim_v", ctypes.c_int32), ("softmax_scale", ctypes.c_float)]
+
+
+class cp_tile_info(ctypes.Structure):
+    _fields_ = [("batch_index", ctypes.c_int32), ("kv_head", ctypes.c_int32),
+                ("split", ctypes.c_int32), ("n_splits", ctypes.c_int32),
+                ("page_begin", ctypes.c_int32), ("page_end", ctypes.c_int32)]
+
+
+class CrossPoolError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__("%s failed: %s (%d)" % (where, status_string(status), status))
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libcrosspool.so (built in-tree by paper_2606_24506_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libcrosspool.so not built: run `python -m paper_2606_24506_b200.build` "
+                          "(or __graft_entry__.build()); there is no fallback path")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i32, u32, u64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_uint32, ctypes.c_uint64
+    i32p = ctypes.POINTER(ctypes.c_int32)
+    u32p = ctypes.POINTER(ctypes.c_uint32)
+    u64p = ctypes.POINTER(ctypes.c_uint64)
+    sig = {
+        "cp_pool_create": (i32, [vp, u64, u32, u32, u32, ctypes.POINTER(cp_model_cfg), i32, i32, i32,
+                                 ctypes.POINTER(vp)]),
+        "cp_pool_free": (i32, [vp]),
+        "cp_pool_map_pages": (i32, [vp, i32, i32, i32p, i32, i32]),
+        "cp_pool_unmap_request": (i32, [vp, i32]),
+        "cp_pool_request_info": (i32, [vp, i32, i32p, i32p, i32p, i32p, i32]),
+        "cp_pool_stats": (i32, [vp, u32p, u32p]),
+        "cp_pool_set_option": (i32, [vp, i32, ctypes.c_int64]),
+        "cp_pool_gather_kv": (i32, [vp, i32, vp, vp, vp]),
+        "cp_decode_workspace_bytes": (i32, [vp, i32p, i32, u64p]),
+        "cp_decode_attention": (i32, [vp, i32p, i32, vp, vp, vp, vp, u64, vp]),
+        "cp_decode_workspace_bytes_host": (i32, [vp, i32p, i32, u64p]),
+        "cp_decode_attention_host": (i32, [vp, i32p, i32, vp, vp, vp, vp, u64, vp]),
+        "cp_decode_plan": (i32, [vp, i32p, i32, ctypes.POINTER(cp_tile_info), i32, i32p, i32p]),
+        "cp_pool_counters": (i32, [vp, u64p, u64p, u64p]),
+        "cp_status_string": (ctypes.c_char_p, [i32]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = L
+    return L
+
+
+EXPORTED = ["cp_pool_create", "cp_pool_free", "cp_pool_map_pages", "cp_pool_unmap_request",
+            "cp_pool_request_info", "cp_pool_stats", "cp_pool_set_option", "cp_pool_gather_kv",
+            "cp_decode_workspace_bytes", "cp_decode_attention", "cp_decode_workspace_bytes_host",
+            "cp_decode_attention_host", "cp_decode_plan", "cp_pool_counters", "cp_status_string"]
+
+
+def status_string(status: int) -> str:
+    return load_library().cp_status_string(int(status)).decode()
+
+
+def _check(status: int, where: str):
+    if status != CP_OK:
+        raise CrossPoolError(status, where)
+
+
+def _ids(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _i32p(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))
+
+
+def _ptr(x) -> int:
+    """Raw address of a torch tensor / numpy array / int."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return int(x.data_ptr())
+    if isinstance(x, np.ndarray):
+        return int(x.ctypes.data)
+    raise TypeError(type(x))
+
+
+class Pool:
+    """Owner of one cp_pool handle; method names follow the C entry points."""
+
+    def __init__(self, arena_dev, arena_bytes: int, page_tokens: int, page_bytes: int, num_pages: int,
+                 models: Sequence, max_requests: int, max_pages_per_request: int):
+        L = load_library()
+        arr = (cp_model_cfg * len(models))()
+        for i, m in enumerate(models):
+            arr[i] = cp_model_cfg(int(m.kind), int(m.n_q_heads), int(m.n_kv_heads), int(m.head_dim_qk),
+                                  int(m.head_dim_v), float(m.softmax_scale))
+        h = ctypes.c_void_p()
+        _check(L.cp_pool_create(_ptr(arena_dev), arena_bytes, page_tokens, page_bytes, num_pages, arr,
+                                len(models), max_requests, max_pages_per_request, ctypes.byref(h)),
+               "cp_pool_create")
+        self._h = h
+        self._L = L
+        self._keep = arena_dev        # keep the arena tensor alive
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.cp_pool_free(self._h)
+            self._h = None
+
+    __del__ = close
+
+    # --- slow path
+    def map_pages(self, request_id: int, model_id: int, page_ids: Optional[Sequence[int]],
+                  context_len: int, n_allocate: int = 0):
+        if page_ids is None:
+            st = self._L.cp_pool_map_pages(self._h, request_id, model_id, None, n_allocate, context_len)
+        else:
+            a = _ids(page_ids)
+            st = self._L.cp_pool_map_pages(self._h, request_id, model_id, _i32p(a), a.size, context_len)
+        _check(st, "cp_pool_map_pages")
+
+    def unmap_request(self, request_id: int):
+        _check(self._L.cp_pool_unmap_request(self._h, request_id), "cp_pool_unmap_request")
+
+    def request_info(self, request_id: int):
+        m, c, n = ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32()
+        _check(self._L.cp_pool_request_info(self._h, request_id, ctypes.byref(m), ctypes.byref(c),
+                                            ctypes.byref(n), None, 0), "cp_pool_request_info")
+        ids = np.empty(n.value, dtype=np.int32)
+        if n.value:
+            _check(self._L.cp_pool_request_info(self._h, request_id, None, None, None, _i32p(ids), n.value),
+                   "cp_pool_request_info")
+        return m.value, c.value, ids
+
+    def stats(self):
+        f, u = ctypes.c_uint32(), ctypes.c_uint32()
+        _check(self._L.cp_pool_stats(self._h, ctypes.byref(f), ctypes.byref(u)), "cp_pool_stats")
+        return f.value, u.value
+
+    def set_option(self, key: int, value: int):
+        _check(self._L.cp_pool_set_option(self._h, key, value), "cp_pool_set_option")
+
+    def counters(self):
+        a, b, c = ctypes.c_uint64(), ctypes.c_uint64(), ctypes.c_uint64()
+        _check(self._L.cp_pool_counters(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)),
+               "cp_pool_counters")
+        return {"kernel_launches": a.value, "plan_builds": b.value, "metadata_h2d_bytes": c.value}
+
+    def decode_plan(self, request_ids):
+        ids = _ids(request_ids)
+        nt, ng = ctypes.c_int32(), ctypes.c_int32()
+        _check(self._L.cp_decode_plan(self._h, _i32p(ids), ids.size, None, 0, ctypes.byref(nt),
+                                      ctypes.byref(ng)), "cp_decode_plan")
+        tiles = (cp_tile_info * max(1, nt.value))()
+        _check(self._L.cp_decode_plan(self._h, _i32p(ids), ids.size, tiles, nt.value, ctypes.byref(nt),
+                                      ctypes.byref(ng)), "cp_decode_plan")
+        return [(t.batch_index, t.kv_head, t.split, t.n_splits, t.page_begin, t.page_end)
+                for t in tiles[:nt.value]], ng.value
+
+    # --- device path
+    def gather_kv(self, request_id: int, k_out_dev, v_out_dev, stream: int = 0):
+        _check(self._L.cp_pool_gather_kv(self._h, request_id, _ptr(k_out_dev), _ptr(v_out_dev), stream),
+               "cp_pool_gather_kv")
+
+    def decode_workspace_bytes(self, request_ids) -> int:
+        ids = _ids(request_ids)
+        b = ctypes.c_uint64()
+        _check(self._L.cp_decode_workspace_bytes(self._h, _i32p(ids), ids.size, ctypes.byref(b)),
+               "cp_decode_workspace_bytes")
+        return b.value
+
+    def decode_attention(self, request_ids, q_dev, out_dev, lse_dev, workspace_dev, workspace_bytes: int,
+                         stream: int = 0):
+        ids = _ids(request_ids)
+        _check(self._L.cp_decode_attention(self._h, _i32p(ids), ids.size, _ptr(q_dev), _ptr(out_dev),
+                                           _ptr(lse_dev), _ptr(workspace_dev), workspace_bytes, stream),
+               "cp_decode_attention")
+
+    def decode_workspace_bytes_host(self, request_ids) -> int:
+        ids = _ids(request_ids)
+        b = ctypes.c_uint64()
+        _check(self._L.cp_decode_workspace_bytes_host(self._h, _i32p(ids), ids.size, ctypes.byref(b)),
+               "cp_decode_workspace_bytes_host")
+        return b.value
+
+    def decode_attention_host(self, request_ids, q_host, out_host, lse_host, workspace_dev,
+                              workspace_bytes: int, stream: int = 0):
+        ids = _ids(request_ids)
+        _check(self._L.cp_decode_attention_host(self._h, _i32p(ids), ids.size, _ptr(q_host), _ptr(out_host),
+                                                _ptr(lse_host), _ptr(workspace_dev), workspace_bytes, stream),
+               "cp_decode_attention_host")

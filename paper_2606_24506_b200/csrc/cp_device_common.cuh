@@ -1,0 +1,157 @@
+// cp_device_common.cuh -- device helpers shared by the decode kernels: bf16 unpacking,
+// acquire/release counters of the persistent scheduler, and the LSE combine unit
+// (hot-path step a4).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include "cp_internal.h"
+
+namespace cp {
+
+__device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w & 0xFFFF0000u); }
+
+__device__ __forceinline__ int ld_acquire(const int32_t *p)
+{
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ void red_release_add(int32_t *p, int v)
+{
+    asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+__device__ __forceinline__ float4 ld_cg_f4(const float *p)
+{
+    return __ldcg(reinterpret_cast<const float4 *>(p));
+}
+
+// Byte offset of row `slot` of the K (is_v = false) or V block of a page, for a model.
+__device__ __forceinline__ uint64_t row_byte_offset(const DecodeParams &p, const DevModel &m,
+                                                    int32_t pid, uint32_t slot, bool is_v)
+{
+    uint64_t base = (uint64_t)pid * p.page_bytes;
+    if (m.kind == 1 || !is_v) return base + (uint64_t)slot * m.d_k * 2u;
+    return base + (uint64_t)p.page_tokens * m.d_k * 2u + (uint64_t)slot * m.d_v * 2u;
+}
+
+// ---------------------------------------------------------------------------------------
+// LSE combine of one (group, head): waits until every split of the group has published
+// its partial (acquire on the group counter), then
+//     M = max_s m_s;  w_s = 2^(m_s - M);  L = sum_s w_s l_s;
+//     O = (sum_s w_s O_s) / L;  LSE = (M + log2 L) * ln 2
+// Every sum runs in a fixed order (strided lanes in split order, then a fixed tree), so
+// the result does not depend on which CTA runs it or when (deterministic).
+// Partials are unnormalised: O_s = sum_t 2^(s_t - m_s) v_t, l_s = sum_t 2^(s_t - m_s),
+// scores in log2 units.  Called by all threads of a CTA (blockDim.x a multiple of 32,
+// >= d_v / 4); smem_f is 16-B aligned and holds cp_combine_smem_bytes() bytes.
+// ---------------------------------------------------------------------------------------
+__host__ __device__ inline size_t cp_combine_smem_bytes(int max_splits, int threads)
+{
+    return ((size_t)4 * threads + 40 + 2 * (size_t)max_splits) * sizeof(float);
+}
+
+__device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int arrivals_per_tile,
+                                    float *smem_f)
+{
+    const Group g = p.groups[cu.group];
+    const DevModel m = p.models[g.model];
+    const int ns = g.n_splits;
+    const int dv = m.d_v;
+    const int stride = dv + kPartPad;
+    const int tid = threadIdx.x;
+    const int nthr = blockDim.x;
+
+    // wait for all splits of the group (tiles are popped before combine units and never
+    // block, so this spin terminates)
+    if (tid == 0) {
+        const int want = ns * arrivals_per_tile;
+        while (ld_acquire(p.group_counters + cu.group) < want) __nanosleep(32);
+    }
+    __syncthreads();
+
+    float4 *red4 = reinterpret_cast<float4 *>(smem_f);      // [nthr]
+    float *red = smem_f + 4 * nthr;                         // [40]
+    float *w_s = red + 40;                                  // [ns]
+    float *l_s = w_s + ns;                                  // [ns]
+    const float *part = p.workspace + g.part_off + (int64_t)cu.head * stride;
+    const int64_t split_stride = (int64_t)m.group * stride;
+
+    // pass 1: M = max m_s, weights, L
+    float mloc = -INFINITY;
+    for (int s = tid; s < ns; s += nthr) {
+        const float2 ml = __ldcg(reinterpret_cast<const float2 *>(part + s * split_stride + dv));
+        w_s[s] = ml.x;
+        l_s[s] = ml.y;
+        mloc = fmaxf(mloc, ml.x);
+    }
+    for (int o = 16; o > 0; o >>= 1) mloc = fmaxf(mloc, __shfl_xor_sync(0xffffffffu, mloc, o));
+    if ((tid & 31) == 0) red[tid >> 5] = mloc;
+    __syncthreads();
+    float M = -INFINITY;
+    for (int w = 0; w < (nthr >> 5); ++w) M = fmaxf(M, red[w]);
+    __syncthreads();
+    for (int s = tid; s < ns; s += nthr) w_s[s] = exp2f(w_s[s] - M);
+    __syncthreads();
+    if (tid < 32) {                      // warp 0: strided in-order sums, then a fixed tree
+        float L = 0.f;
+        for (int s = tid; s < ns; s += 32) L += w_s[s] * l_s[s];
+        for (int o = 16; o > 0; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
+        if (tid == 0) red[32] = L;
+    }
+    __syncthreads();
+    const float L = red[32];
+    const float invL = 1.0f / L;
+
+    // pass 2: O.  Thread -> (column quad cq, lane z); the lanes interleave the splits.
+    const int nq = dv >> 2;                       // float4 columns
+    const int lanes = nthr / nq;                  // >= 1 by contract
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    const int cq = tid % nq;
+    const int z = tid / nq;
+    if (z < lanes) {
+#pragma unroll 8
+        for (int s = z; s < ns; s += lanes) {
+            const float w = w_s[s];
+            const float4 v = ld_cg_f4(part + s * split_stride + cq * 4);
+            acc.x += w * v.x; acc.y += w * v.y; acc.z += w * v.z; acc.w += w * v.w;
+        }
+        red4[z * nq + cq] = acc;
+    }
+    __syncthreads();
+    if (tid < nq) {
+        float4 o = red4[tid];
+        for (int zz = 1; zz < lanes; ++zz) {
+            const float4 v = red4[zz * nq + tid];
+            o.x += v.x; o.y += v.y; o.z += v.z; o.w += v.w;
+        }
+        o.x *= invL; o.y *= invL; o.z *= invL; o.w *= invL;
+        float *dst = p.out + g.out_off + (int64_t)cu.head * dv + tid * 4;
+        *reinterpret_cast<float4 *>(dst) = o;
+    }
+    if (tid == 0) p.lse[g.lse_off + cu.head] = (M + log2f(L)) * 0.6931471805599453f;
+    __syncthreads();
+}
+
+// Persistent-scheduler epilogue: the last CTA to finish resets the counters so that the
+// next launch (stream-ordered) starts from zero without a host memset.
+__device__ inline void scheduler_epilogue(const DecodeParams &p, int *s_flag)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        *s_flag = (atomicAdd(p.work_counter + 1, 1) == (int)gridDim.x - 1);
+    }
+    __syncthreads();
+    if (*s_flag) {
+        for (int i = threadIdx.x; i < p.n_groups; i += blockDim.x) p.group_counters[i] = 0;
+        if (threadIdx.x == 0) {
+            p.work_counter[0] = 0;
+            p.work_counter[1] = 0;
+        }
+    }
+}
+
+}  // namespace cp

@@ -1,0 +1,661 @@
+// cp_pool.cu -- host side of libcrosspool: the C ABI of include/crosspool.h, the pool
+// manager (page ownership against the page budget, per-request page lists: the software
+// counterpart of the paper's KV-cache virtualizer), the tile planner that
+// builds the device work list (hot-path step a1), and the kernel launch glue.
+#include <cuda_runtime.h>
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/crosspool.h"
+#include "cp_internal.h"
+#include "cp_launch.h"
+
+using namespace cp;
+
+namespace {
+
+struct DevBuf {
+    void *ptr = nullptr;
+    size_t cap = 0;
+    // grow (never shrink); contents are NOT preserved.  Slow path: synchronises the device
+    // before freeing the old buffer so no in-flight kernel can still read it.
+    cudaError_t ensure(size_t bytes)
+    {
+        if (bytes <= cap) return cudaSuccess;
+        if (ptr) {
+            cudaError_t e = cudaDeviceSynchronize();
+            if (e != cudaSuccess) return e;
+            cudaFree(ptr);
+            ptr = nullptr;
+            cap = 0;
+        }
+        size_t want = std::max(bytes, (size_t)256);
+        want = (want * 3 / 2 + 255) & ~(size_t)255;
+        cudaError_t e = cudaMalloc(&ptr, want);
+        if (e != cudaSuccess) { ptr = nullptr; return e; }
+        cap = want;
+        return cudaSuccess;
+    }
+    void release() { if (ptr) cudaFree(ptr); ptr = nullptr; cap = 0; }
+};
+
+struct Request {
+    bool live = false;
+    int32_t model = -1;
+    int32_t ctx = 0;
+    std::vector<int32_t> pages;      // page-major page list
+    size_t uploaded = 0;             // entries already in the device page table
+};
+
+struct KindPlan {
+    std::vector<Group> groups;
+    std::vector<Tile> tiles;
+    std::vector<Combine> combines;
+    int max_splits = 1;
+    int max_dk = 0, max_dv = 0;
+    int max_group = 0;
+    bool uploaded = false;
+    DevBuf d_groups, d_tiles, d_combines, d_counters;   // counters: [2] work + [n_groups]
+};
+
+}  // namespace
+
+struct cp_pool {
+    uint8_t *arena = nullptr;
+    uint64_t arena_bytes = 0;
+    uint32_t P = 0, page_bytes = 0, num_pages = 0;
+    std::vector<cp_model_cfg> models;
+    int32_t max_requests = 0, max_ppr = 0;
+
+    std::vector<int32_t> owner;          // per physical page: owning request id or -1
+    uint32_t n_free = 0;
+    uint32_t alloc_cursor = 0;
+    std::vector<Request> reqs;
+    std::vector<int32_t> h_ctx;          // host mirror of the device ctx table
+    int32_t ctx_dirty_lo = INT32_MAX, ctx_dirty_hi = -1;
+    uint64_t topo_version = 1;           // bumps when any request's planned page count changes
+
+    // options
+    int opt_kernel = 0, opt_num_ctas = 0, opt_waves_x16 = 32, opt_min_tile_pages = 2;
+
+    // plan cache
+    std::vector<int32_t> plan_batch;
+    uint64_t plan_version = 0;
+    bool plan_valid = false;
+    KindPlan plan[2];
+    uint64_t plan_ws_floats = 0;
+    std::vector<int64_t> q_off, out_off, lse_off;   // per batch slot (packed offsets)
+    int64_t q_elems = 0, out_floats = 0, lse_floats = 0;
+
+    // device side (lazy)
+    bool dev_ready = false;
+    int n_sm = 148;
+    DevBuf d_page_table, d_ctx, d_models;
+
+    // counters
+    uint64_t n_launches = 0, n_plan_builds = 0, n_h2d_bytes = 0;
+};
+
+namespace {
+
+inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+bool model_supported(const cp_model_cfg &m, uint32_t P, uint32_t page_bytes)
+{
+    if (m.kind != CP_KIND_KV && m.kind != CP_KIND_MLA) return false;
+    if (m.n_q_heads < 1 || m.n_kv_heads < 1 || m.n_q_heads % m.n_kv_heads != 0) return false;
+    if (m.head_dim_qk < 8 || m.head_dim_v < 8 || m.head_dim_qk % 8 || m.head_dim_v % 8) return false;
+    if (m.head_dim_qk > kMaxDk || m.head_dim_v > kMaxDv) return false;
+    if (!(m.softmax_scale == m.softmax_scale)) return false;
+    uint64_t need;
+    if (m.kind == CP_KIND_MLA) {
+        if (m.n_kv_heads != 1 || m.head_dim_v > m.head_dim_qk) return false;
+        need = (uint64_t)P * m.head_dim_qk * 2;
+    } else {
+        need = (uint64_t)P * (m.head_dim_qk + m.head_dim_v) * 2;
+    }
+    return need <= page_bytes;
+}
+
+// ----------------------------------------------------------------------------- planner
+// Step a1: cut every (request, kv head) group into page-aligned KV splits of near-equal
+// length so that the whole batch yields about n_ctas * waves tiles; tiles are ordered
+// longest first (the persistent CTAs pop them in array order), combine units follow.
+void build_plan(cp_pool *pool, const int32_t *ids, int n)
+{
+    const int P = (int)pool->P;
+    for (int k = 0; k < 2; ++k) {
+        KindPlan &kp = pool->plan[k];
+        kp.groups.clear(); kp.tiles.clear(); kp.combines.clear();
+        kp.max_splits = 1; kp.max_dk = kp.max_dv = kp.max_group = 0; kp.uploaded = false;
+    }
+    pool->q_off.assign(n, 0); pool->out_off.assign(n, 0); pool->lse_off.assign(n, 0);
+    int64_t qo = 0, oo = 0, lo = 0;
+    int64_t total_pages[2] = {0, 0};
+    for (int b = 0; b < n; ++b) {
+        const Request &r = pool->reqs[ids[b]];
+        const cp_model_cfg &m = pool->models[r.model];
+        pool->q_off[b] = qo; pool->out_off[b] = oo; pool->lse_off[b] = lo;
+        qo += (int64_t)m.n_q_heads * m.head_dim_qk;
+        oo += (int64_t)m.n_q_heads * m.head_dim_v;
+        lo += m.n_q_heads;
+        total_pages[m.kind] += (int64_t)ceil_div(r.ctx, P) * m.n_kv_heads;
+    }
+    pool->q_elems = qo; pool->out_floats = oo; pool->lse_floats = lo;
+
+    const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
+    uint64_t ws = 0;
+    for (int k = 0; k < 2; ++k) {
+        KindPlan &kp = pool->plan[k];
+        if (total_pages[k] == 0) continue;
+        const int64_t target_tiles = std::max<int64_t>(1, (int64_t)n_ctas * pool->opt_waves_x16 / 16);
+        int64_t L = (total_pages[k] + target_tiles - 1) / target_tiles;
+        L = std::max<int64_t>(L, pool->opt_min_tile_pages);
+        for (int b = 0; b < n; ++b) {
+            const Request &r = pool->reqs[ids[b]];
+            const cp_model_cfg &m = pool->models[r.model];
+            if (m.kind != k) continue;
+            const int g = m.n_q_heads / m.n_kv_heads;
+            const int n_lp = ceil_div(r.ctx, P);
+            const int ns = (int)((n_lp + L - 1) / L);
+            kp.max_splits = std::max(kp.max_splits, ns);
+            kp.max_dk = std::max(kp.max_dk, m.head_dim_qk);
+            kp.max_dv = std::max(kp.max_dv, m.head_dim_v);
+            kp.max_group = std::max(kp.max_group, g);
+            for (int c = 0; c < m.n_kv_heads; ++c) {
+                Group gr;
+                gr.req = ids[b]; gr.model = r.model; gr.kv_head = c; gr.n_splits = ns;
+                gr.n_pages = n_lp; gr.batch_index = b;
+                gr.q_off = pool->q_off[b] + (int64_t)c * g * m.head_dim_qk;
+                gr.out_off = pool->out_off[b] + (int64_t)c * g * m.head_dim_v;
+                gr.lse_off = pool->lse_off[b] + (int64_t)c * g;
+                gr.part_off = 0;
+                if (ns > 1) {
+                    gr.part_off = (int64_t)ws;
+                    ws += (uint64_t)ns * g * (m.head_dim_v + kPartPad);
+                }
+                const int gi = (int)kp.groups.size();
+                kp.groups.push_back(gr);
+                const int base = n_lp / ns, rem = n_lp % ns;
+                int pb = 0;
+                for (int s = 0; s < ns; ++s) {
+                    const int len = base + (s < rem ? 1 : 0);
+                    kp.tiles.push_back(Tile{gi, s, pb, pb + len});
+                    pb += len;
+                }
+                if (ns > 1)
+                    for (int h = 0; h < g; ++h) kp.combines.push_back(Combine{gi, h});
+            }
+        }
+        std::stable_sort(kp.tiles.begin(), kp.tiles.end(), [](const Tile &a, const Tile &b) {
+            return (a.page_end - a.page_begin) > (b.page_end - b.page_begin);
+        });
+    }
+    pool->plan_ws_floats = ws;
+    pool->plan_batch.assign(ids, ids + n);
+    pool->plan_version = pool->topo_version;
+    pool->plan_valid = true;
+    pool->n_plan_builds++;
+}
+
+cp_status check_batch(cp_pool *pool, const int32_t *ids, int n)
+{
+    if (!pool || !ids || n < 1) return CP_ERR_INVALID_ARG;
+    for (int b = 0; b < n; ++b) {
+        if (ids[b] < 0 || ids[b] >= pool->max_requests) return CP_ERR_INVALID_ARG;
+        if (!pool->reqs[ids[b]].live) return CP_ERR_UNKNOWN_REQUEST;
+    }
+    // distinct ids (batches are small; O(n log n))
+    std::vector<int32_t> s(ids, ids + n);
+    std::sort(s.begin(), s.end());
+    for (int b = 1; b < n; ++b)
+        if (s[b] == s[b - 1]) return CP_ERR_INVALID_ARG;
+    return CP_OK;
+}
+
+void ensure_plan(cp_pool *pool, const int32_t *ids, int n)
+{
+    if (pool->plan_valid && pool->plan_version == pool->topo_version &&
+        (int)pool->plan_batch.size() == n && std::equal(ids, ids + n, pool->plan_batch.begin()))
+        return;
+    build_plan(pool, ids, n);
+}
+
+// ------------------------------------------------------------------------ device state
+cp_status ensure_device(cp_pool *pool)
+{
+    if (pool->dev_ready) return CP_OK;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+    cudaPointerAttributes attr;
+    if (cudaPointerGetAttributes(&attr, pool->arena) != cudaSuccess ||
+        attr.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        return CP_ERR_INVALID_ARG;          // arena is not device memory
+    }
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, attr.device) != cudaSuccess)
+        return CP_ERR_CUDA;
+    if (pool->d_page_table.ensure((size_t)pool->max_requests * pool->max_ppr * 4) != cudaSuccess ||
+        pool->d_ctx.ensure((size_t)pool->max_requests * 4) != cudaSuccess ||
+        pool->d_models.ensure(pool->models.size() * sizeof(DevModel)) != cudaSuccess) {
+        cudaGetLastError();
+        return CP_ERR_CUDA;
+    }
+    std::vector<DevModel> dm(pool->models.size());
+    for (size_t i = 0; i < dm.size(); ++i) {
+        const cp_model_cfg &m = pool->models[i];
+        dm[i].kind = m.kind; dm[i].n_q_heads = m.n_q_heads; dm[i].n_kv_heads = m.n_kv_heads;
+        dm[i].d_k = m.head_dim_qk; dm[i].d_v = m.head_dim_v; dm[i].group = m.n_q_heads / m.n_kv_heads;
+        dm[i].scale = m.softmax_scale;
+        dm[i].scale_log2 = (float)((double)m.softmax_scale * 1.4426950408889634);
+    }
+    if (cudaMemcpy(pool->d_models.ptr, dm.data(), dm.size() * sizeof(DevModel),
+                   cudaMemcpyHostToDevice) != cudaSuccess)
+        return CP_ERR_CUDA;
+    if (cudaMemset(pool->d_ctx.ptr, 0, (size_t)pool->max_requests * 4) != cudaSuccess)
+        return CP_ERR_CUDA;
+    pool->n_sm = sms;
+    pool->dev_ready = true;
+    pool->plan_valid = false;               // the SM count feeds the planner
+    // everything mapped so far is dirty
+    for (auto &r : pool->reqs) r.uploaded = 0;
+    pool->ctx_dirty_lo = 0; pool->ctx_dirty_hi = pool->max_requests - 1;
+    return CP_OK;
+}
+
+// Upload page-table rows and context lengths that changed since the last device call.
+cp_status flush_tables(cp_pool *pool, cudaStream_t stream)
+{
+    for (int rid = 0; rid < pool->max_requests; ++rid) {
+        Request &r = pool->reqs[rid];
+        if (!r.live || r.uploaded >= r.pages.size()) continue;
+        const size_t n = r.pages.size() - r.uploaded;
+        int32_t *dst = (int32_t *)pool->d_page_table.ptr + (size_t)rid * pool->max_ppr + r.uploaded;
+        if (cudaMemcpyAsync(dst, r.pages.data() + r.uploaded, n * 4, cudaMemcpyHostToDevice, stream) != cudaSuccess)
+            return CP_ERR_CUDA;
+        pool->n_h2d_bytes += n * 4;
+        r.uploaded = r.pages.size();
+    }
+    if (pool->ctx_dirty_hi >= pool->ctx_dirty_lo) {
+        const int lo = pool->ctx_dirty_lo, hi = pool->ctx_dirty_hi;
+        if (cudaMemcpyAsync((int32_t *)pool->d_ctx.ptr + lo, pool->h_ctx.data() + lo, (size_t)(hi - lo + 1) * 4,
+                            cudaMemcpyHostToDevice, stream) != cudaSuccess)
+            return CP_ERR_CUDA;
+        pool->n_h2d_bytes += (size_t)(hi - lo + 1) * 4;
+        pool->ctx_dirty_lo = INT32_MAX; pool->ctx_dirty_hi = -1;
+    }
+    return CP_OK;
+}
+
+cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
+{
+    if (kp.uploaded) return CP_OK;
+    const size_t gb = kp.groups.size() * sizeof(Group), tb = kp.tiles.size() * sizeof(Tile);
+    const size_t cb = kp.combines.size() * sizeof(Combine), nb = (2 + kp.groups.size()) * 4;
+    const bool counters_new = kp.d_counters.cap < nb;
+    if (kp.d_groups.ensure(gb) != cudaSuccess || kp.d_tiles.ensure(tb) != cudaSuccess ||
+        kp.d_combines.ensure(std::max(cb, (size_t)16)) != cudaSuccess ||
+        kp.d_counters.ensure(nb) != cudaSuccess) {
+        cudaGetLastError();
+        return CP_ERR_CUDA;
+    }
+    if (cudaMemcpyAsync(kp.d_groups.ptr, kp.groups.data(), gb, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
+        cudaMemcpyAsync(kp.d_tiles.ptr, kp.tiles.data(), tb, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
+        (cb && cudaMemcpyAsync(kp.d_combines.ptr, kp.combines.data(), cb, cudaMemcpyHostToDevice, stream) != cudaSuccess))
+        return CP_ERR_CUDA;
+    // counters are zero between launches (the kernels reset them); zero a fresh buffer
+    if (counters_new && cudaMemsetAsync(kp.d_counters.ptr, 0, kp.d_counters.cap, stream) != cudaSuccess)
+        return CP_ERR_CUDA;
+    pool->n_h2d_bytes += gb + tb + cb;
+    kp.uploaded = true;
+    return CP_OK;
+}
+
+}  // namespace
+
+// =========================================================================== C ABI
+extern "C" {
+
+const char *cp_status_string(cp_status s)
+{
+    switch (s) {
+    case CP_OK: return "CP_OK";
+    case CP_ERR_INVALID_ARG: return "CP_ERR_INVALID_ARG";
+    case CP_ERR_NO_PAGES: return "CP_ERR_NO_PAGES";
+    case CP_ERR_PAGE_RANGE: return "CP_ERR_PAGE_RANGE";
+    case CP_ERR_PAGE_IN_USE: return "CP_ERR_PAGE_IN_USE";
+    case CP_ERR_UNKNOWN_REQUEST: return "CP_ERR_UNKNOWN_REQUEST";
+    case CP_ERR_UNSUPPORTED: return "CP_ERR_UNSUPPORTED";
+    case CP_ERR_WORKSPACE: return "CP_ERR_WORKSPACE";
+    case CP_ERR_CUDA: return "CP_ERR_CUDA";
+    default: return "CP_ERR_?";
+    }
+}
+
+cp_status cp_pool_create(void *arena_dev, uint64_t arena_bytes, uint32_t page_tokens,
+                         uint32_t page_bytes, uint32_t num_pages, const cp_model_cfg *models,
+                         int32_t n_models, int32_t max_requests, int32_t max_pages_per_request,
+                         cp_pool **out)
+{
+    if (!out) return CP_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!arena_dev || !models || n_models < 1 || max_requests < 1 || max_pages_per_request < 1)
+        return CP_ERR_INVALID_ARG;
+    if (page_tokens < 1 || page_tokens > 256 || page_bytes < 16 || page_bytes % 16 || num_pages < 1)
+        return CP_ERR_INVALID_ARG;
+    if (num_pages > (uint32_t)INT32_MAX) return CP_ERR_INVALID_ARG;
+    if ((uint64_t)num_pages * page_bytes > arena_bytes) return CP_ERR_INVALID_ARG;
+    if (((uintptr_t)arena_dev & 255u) != 0) return CP_ERR_INVALID_ARG;
+    if ((uint64_t)max_requests * (uint64_t)max_pages_per_request > (1ull << 31)) return CP_ERR_INVALID_ARG;
+    for (int i = 0; i < n_models; ++i)
+        if (!model_supported(models[i], page_tokens, page_bytes)) return CP_ERR_UNSUPPORTED;
+    cp_pool *p = new (std::nothrow) cp_pool();
+    if (!p) return CP_ERR_INVALID_ARG;
+    try {
+        p->arena = (uint8_t *)arena_dev; p->arena_bytes = arena_bytes;
+        p->P = page_tokens; p->page_bytes = page_bytes; p->num_pages = num_pages;
+        p->models.assign(models, models + n_models);
+        p->max_requests = max_requests; p->max_ppr = max_pages_per_request;
+        p->owner.assign(num_pages, -1);
+        p->n_free = num_pages;
+        p->reqs.resize(max_requests);
+        p->h_ctx.assign(max_requests, 0);
+    } catch (...) {
+        delete p;
+        return CP_ERR_INVALID_ARG;
+    }
+    *out = p;
+    return CP_OK;
+}
+
+cp_status cp_pool_free(cp_pool *pool)
+{
+    if (!pool) return CP_OK;
+    if (pool->dev_ready) cudaDeviceSynchronize();
+    pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release();
+    for (int k = 0; k < 2; ++k) {
+        pool->plan[k].d_groups.release(); pool->plan[k].d_tiles.release();
+        pool->plan[k].d_combines.release(); pool->plan[k].d_counters.release();
+    }
+    delete pool;
+    return CP_OK;
+}
+
+cp_status cp_pool_map_pages(cp_pool *pool, int32_t request_id, int32_t model_id,
+                            const int32_t *page_ids_host, int32_t n_page_ids, int32_t context_len)
+{
+    if (!pool || request_id < 0 || request_id >= pool->max_requests) return CP_ERR_INVALID_ARG;
+    if (model_id < 0 || model_id >= (int)pool->models.size()) return CP_ERR_INVALID_ARG;
+    if (n_page_ids < 0 || context_len < 1) return CP_ERR_INVALID_ARG;
+    Request &r = pool->reqs[request_id];
+    if (r.live && r.model != model_id) return CP_ERR_INVALID_ARG;
+    if (r.live && context_len < r.ctx) return CP_ERR_INVALID_ARG;
+    const cp_model_cfg &m = pool->models[model_id];
+    if (n_page_ids % m.n_kv_heads != 0) return CP_ERR_UNSUPPORTED;
+    const size_t have = r.live ? r.pages.size() : 0;
+    const size_t total = have + (size_t)n_page_ids;
+    if (total > (size_t)pool->max_ppr) return CP_ERR_INVALID_ARG;
+    const uint64_t capacity_tokens = (uint64_t)(total / m.n_kv_heads) * pool->P;
+    if ((uint64_t)context_len > capacity_tokens) return CP_ERR_INVALID_ARG;
+
+    std::vector<int32_t> fresh;
+    if (n_page_ids > 0) {
+        fresh.resize(n_page_ids);
+        if (page_ids_host) {
+            for (int i = 0; i < n_page_ids; ++i) {
+                const int32_t pid = page_ids_host[i];
+                if (pid < 0 || (uint32_t)pid >= pool->num_pages) return CP_ERR_PAGE_RANGE;
+                fresh[i] = pid;
+            }
+            for (int i = 0; i < n_page_ids; ++i)
+                if (pool->owner[fresh[i]] != -1) return CP_ERR_PAGE_IN_USE;
+            std::vector<int32_t> s(fresh);
+            std::sort(s.begin(), s.end());
+            for (int i = 1; i < n_page_ids; ++i)
+                if (s[i] == s[i - 1]) return CP_ERR_PAGE_IN_USE;
+        } else {
+            if ((uint32_t)n_page_ids > pool->n_free) return CP_ERR_NO_PAGES;
+            uint32_t cur = pool->alloc_cursor;
+            for (int i = 0; i < n_page_ids;) {
+                if (pool->owner[cur] == -1) fresh[i++] = (int32_t)cur;
+                cur = (cur + 1) % pool->num_pages;
+            }
+            pool->alloc_cursor = cur;
+        }
+    }
+    // commit (nothing below can fail)
+    const int old_planned = r.live ? ceil_div(r.ctx, (int)pool->P) : -1;
+    if (!r.live) {
+        r.live = true; r.model = model_id; r.pages.clear(); r.uploaded = 0;
+    }
+    for (int32_t pid : fresh) pool->owner[pid] = request_id;
+    pool->n_free -= (uint32_t)fresh.size();
+    r.pages.insert(r.pages.end(), fresh.begin(), fresh.end());
+    r.ctx = context_len;
+    pool->h_ctx[request_id] = context_len;
+    pool->ctx_dirty_lo = std::min(pool->ctx_dirty_lo, request_id);
+    pool->ctx_dirty_hi = std::max(pool->ctx_dirty_hi, request_id);
+    if (ceil_div(context_len, (int)pool->P) != old_planned) pool->topo_version++;
+    return CP_OK;
+}
+
+cp_status cp_pool_unmap_request(cp_pool *pool, int32_t request_id)
+{
+    if (!pool || request_id < 0 || request_id >= pool->max_requests) return CP_ERR_INVALID_ARG;
+    Request &r = pool->reqs[request_id];
+    if (!r.live) return CP_ERR_UNKNOWN_REQUEST;
+    for (int32_t pid : r.pages) pool->owner[pid] = -1;
+    pool->n_free += (uint32_t)r.pages.size();
+    r = Request();
+    pool->topo_version++;
+    return CP_OK;
+}
+
+cp_status cp_pool_request_info(const cp_pool *pool, int32_t request_id, int32_t *model_id,
+                               int32_t *context_len, int32_t *n_page_ids,
+                               int32_t *page_ids_out_host, int32_t cap)
+{
+    if (!pool || request_id < 0 || request_id >= pool->max_requests) return CP_ERR_INVALID_ARG;
+    const Request &r = pool->reqs[request_id];
+    if (!r.live) return CP_ERR_UNKNOWN_REQUEST;
+    if (model_id) *model_id = r.model;
+    if (context_len) *context_len = r.ctx;
+    if (n_page_ids) *n_page_ids = (int32_t)r.pages.size();
+    if (page_ids_out_host && cap > 0)
+        std::memcpy(page_ids_out_host, r.pages.data(), sizeof(int32_t) * std::min<size_t>(cap, r.pages.size()));
+    return CP_OK;
+}
+
+cp_status cp_pool_stats(const cp_pool *pool, uint32_t *free_pages, uint32_t *used_pages)
+{
+    if (!pool) return CP_ERR_INVALID_ARG;
+    if (free_pages) *free_pages = pool->n_free;
+    if (used_pages) *used_pages = pool->num_pages - pool->n_free;
+    return CP_OK;
+}
+
+cp_status cp_pool_set_option(cp_pool *pool, int32_t key, int64_t value)
+{
+    if (!pool) return CP_ERR_INVALID_ARG;
+    switch (key) {
+    case CP_OPT_KERNEL:
+        if (value < 0 || value > 1) return CP_ERR_INVALID_ARG;
+        pool->opt_kernel = (int)value; break;
+    case CP_OPT_NUM_CTAS:
+        if (value < 0 || value > 65536) return CP_ERR_INVALID_ARG;
+        pool->opt_num_ctas = (int)value; break;
+    case CP_OPT_WAVES_X16:
+        if (value < 1 || value > 4096) return CP_ERR_INVALID_ARG;
+        pool->opt_waves_x16 = (int)value; break;
+    case CP_OPT_MIN_TILE_PAGES:
+        if (value < 1 || value > (1 << 20)) return CP_ERR_INVALID_ARG;
+        pool->opt_min_tile_pages = (int)value; break;
+    default: return CP_ERR_INVALID_ARG;
+    }
+    pool->plan_valid = false;
+    return CP_OK;
+}
+
+cp_status cp_pool_counters(const cp_pool *pool, uint64_t *kernel_launches, uint64_t *plan_builds,
+                           uint64_t *metadata_h2d_bytes)
+{
+    if (!pool) return CP_ERR_INVALID_ARG;
+    if (kernel_launches) *kernel_launches = pool->n_launches;
+    if (plan_builds) *plan_builds = pool->n_plan_builds;
+    if (metadata_h2d_bytes) *metadata_h2d_bytes = pool->n_h2d_bytes;
+    return CP_OK;
+}
+
+cp_status cp_decode_plan(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                         cp_tile_info *tiles_out, int32_t cap, int32_t *n_tiles_out,
+                         int32_t *n_groups_out)
+{
+    cp_status st = check_batch(pool, request_ids_host, n_requests);
+    if (st != CP_OK) return st;
+    ensure_plan(pool, request_ids_host, n_requests);
+    int nt = 0, ng = 0;
+    for (int k = 0; k < 2; ++k) {
+        const KindPlan &kp = pool->plan[k];
+        for (const Tile &t : kp.tiles) {
+            if (tiles_out && nt < cap) {
+                const Group &g = kp.groups[t.group];
+                tiles_out[nt] = cp_tile_info{g.batch_index, g.kv_head, t.split, g.n_splits,
+                                             t.page_begin, t.page_end};
+            }
+            ++nt;
+        }
+        ng += (int)kp.groups.size();
+    }
+    if (n_tiles_out) *n_tiles_out = nt;
+    if (n_groups_out) *n_groups_out = ng;
+    return CP_OK;
+}
+
+cp_status cp_decode_workspace_bytes(cp_pool *pool, const int32_t *request_ids_host,
+                                    int32_t n_requests, uint64_t *bytes_out)
+{
+    if (!bytes_out) return CP_ERR_INVALID_ARG;
+    cp_status st = check_batch(pool, request_ids_host, n_requests);
+    if (st != CP_OK) return st;
+    ensure_plan(pool, request_ids_host, n_requests);
+    *bytes_out = pool->plan_ws_floats * 4;
+    return CP_OK;
+}
+
+cp_status cp_pool_gather_kv(cp_pool *pool, int32_t request_id, void *k_out_dev, void *v_out_dev,
+                            void *stream)
+{
+    if (!pool || request_id < 0 || request_id >= pool->max_requests || !k_out_dev)
+        return CP_ERR_INVALID_ARG;
+    Request &r = pool->reqs[request_id];
+    if (!r.live) return CP_ERR_UNKNOWN_REQUEST;
+    if (((uintptr_t)k_out_dev & 15u) || ((uintptr_t)v_out_dev & 15u)) return CP_ERR_INVALID_ARG;
+    cp_status st = ensure_device(pool);
+    if (st != CP_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    st = flush_tables(pool, s);
+    if (st != CP_OK) return st;
+    const cp_model_cfg &m = pool->models[r.model];
+    launch_gather(pool->arena, pool->P, pool->page_bytes,
+                  (const int32_t *)pool->d_page_table.ptr + (size_t)request_id * pool->max_ppr,
+                  m.kind, m.n_kv_heads, m.head_dim_qk, m.head_dim_v, r.ctx, k_out_dev, v_out_dev,
+                  pool->n_sm, s);
+    pool->n_launches++;
+    if (cudaGetLastError() != cudaSuccess) return CP_ERR_CUDA;
+    return CP_OK;
+}
+
+cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                              const void *q_dev, float *out_dev, float *lse_dev,
+                              void *workspace_dev, uint64_t workspace_bytes, void *stream)
+{
+    cp_status st = check_batch(pool, request_ids_host, n_requests);
+    if (st != CP_OK) return st;
+    if (!q_dev || !out_dev || !lse_dev) return CP_ERR_INVALID_ARG;
+    if (((uintptr_t)q_dev & 15u) || ((uintptr_t)out_dev & 15u) || ((uintptr_t)lse_dev & 3u))
+        return CP_ERR_INVALID_ARG;
+    st = ensure_device(pool);
+    if (st != CP_OK) return st;
+    ensure_plan(pool, request_ids_host, n_requests);
+    if (pool->plan_ws_floats * 4 > workspace_bytes) return CP_ERR_WORKSPACE;
+    if (pool->plan_ws_floats && (!workspace_dev || ((uintptr_t)workspace_dev & 15u))) return CP_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    st = flush_tables(pool, s);
+    if (st != CP_OK) return st;
+
+    for (int k = 0; k < 2; ++k) {
+        KindPlan &kp = pool->plan[k];
+        if (kp.tiles.empty()) continue;
+        st = upload_plan(pool, kp, s);
+        if (st != CP_OK) return st;
+        DecodeParams prm;
+        prm.arena = pool->arena; prm.page_tokens = pool->P; prm.page_bytes = pool->page_bytes;
+        prm.page_table = (const int32_t *)pool->d_page_table.ptr; prm.max_ppr = pool->max_ppr;
+        prm.req_ctx = (const int32_t *)pool->d_ctx.ptr;
+        prm.models = (const DevModel *)pool->d_models.ptr;
+        prm.groups = (const Group *)kp.d_groups.ptr;
+        prm.tiles = (const Tile *)kp.d_tiles.ptr;
+        prm.combines = (const Combine *)kp.d_combines.ptr;
+        prm.n_tiles = (int)kp.tiles.size(); prm.n_combines = (int)kp.combines.size();
+        prm.n_groups = (int)kp.groups.size();
+        prm.q = (const uint16_t *)q_dev; prm.out = out_dev; prm.lse = lse_dev;
+        prm.workspace = (float *)workspace_dev;
+        prm.work_counter = (int32_t *)kp.d_counters.ptr;
+        prm.group_counters = (int32_t *)kp.d_counters.ptr + 2;
+        const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
+        cudaError_t e = launch_decode_generic(prm, kp.max_dk, kp.max_dv, k == CP_KIND_KV,
+                                              kp.max_splits, std::min(n_ctas, pool->n_sm), s);
+        pool->n_launches++;
+        if (e != cudaSuccess) return CP_ERR_CUDA;
+    }
+    return CP_OK;
+}
+
+static inline uint64_t align256(uint64_t x) { return (x + 255) & ~(uint64_t)255; }
+
+cp_status cp_decode_workspace_bytes_host(cp_pool *pool, const int32_t *request_ids_host,
+                                         int32_t n_requests, uint64_t *bytes_out)
+{
+    uint64_t ws = 0;
+    cp_status st = cp_decode_workspace_bytes(pool, request_ids_host, n_requests, &ws);
+    if (st != CP_OK) return st;
+    *bytes_out = align256((uint64_t)pool->q_elems * 2) + align256((uint64_t)pool->out_floats * 4) +
+                 align256((uint64_t)pool->lse_floats * 4) + ws;
+    return CP_OK;
+}
+
+cp_status cp_decode_attention_host(cp_pool *pool, const int32_t *request_ids_host,
+                                   int32_t n_requests, const void *q_host, float *out_host,
+                                   float *lse_host, void *workspace_dev, uint64_t workspace_bytes,
+                                   void *stream)
+{
+    if (!q_host || !out_host || !lse_host || !workspace_dev) return CP_ERR_INVALID_ARG;
+    uint64_t need = 0;
+    cp_status st = cp_decode_workspace_bytes_host(pool, request_ids_host, n_requests, &need);
+    if (st != CP_OK) return st;
+    if (need > workspace_bytes || ((uintptr_t)workspace_dev & 255u)) return CP_ERR_WORKSPACE;
+    st = ensure_device(pool);
+    if (st != CP_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    uint8_t *w = (uint8_t *)workspace_dev;
+    void *q_dev = w;                      w += align256((uint64_t)pool->q_elems * 2);
+    float *o_dev = (float *)w;            w += align256((uint64_t)pool->out_floats * 4);
+    float *l_dev = (float *)w;            w += align256((uint64_t)pool->lse_floats * 4);
+    const uint64_t rest = workspace_bytes - (uint64_t)(w - (uint8_t *)workspace_dev);
+    if (cudaMemcpyAsync(q_dev, q_host, (size_t)pool->q_elems * 2, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return CP_ERR_CUDA;
+    st = cp_decode_attention(pool, request_ids_host, n_requests, q_dev, o_dev, l_dev, w, rest, s);
+    if (st != CP_OK) return st;
+    if (cudaMemcpyAsync(out_host, o_dev, (size_t)pool->out_floats * 4, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaMemcpyAsync(lse_host, l_dev, (size_t)pool->lse_floats * 4, cudaMemcpyDeviceToHost, s) != cudaSuccess)
+        return CP_ERR_CUDA;
+    if (cudaStreamSynchronize(s) != cudaSuccess) return CP_ERR_CUDA;
+    return CP_OK;
+}
+
+}  // extern "C"

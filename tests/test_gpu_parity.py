@@ -1,0 +1,305 @@
+"""GPU parity tests (run with -m gpu on the B200 box): the CUDA path, called through the
+C ABI, against the CPU float64 oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star / DESIGN.md §3): translation + gather bit-exact; attention
+max-abs <= 1e-2 and mean-abs <= 1e-3 over all outputs of a config, LSE max-abs <= 1e-3, and
+the self-imposed per-request relative bound ||dO||_F / ||O*||_F <= 1e-2 (the absolute bounds
+alone would accept an all-zero output on the MLA config)."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+from workloads import KIND_KV, KIND_MLA, ModelCfg
+
+pytestmark = pytest.mark.gpu
+
+MAX_ABS, MEAN_ABS, LSE_ABS, REL_FRO = 1e-2, 1e-3, 1e-3, 1e-2
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device (no CPU fallback exists)"
+    return torch
+
+
+def device_workload(w, **kw):
+    from paper_2606_24506_b200.harness import DeviceWorkload
+    return DeviceWorkload(w, **kw)
+
+
+def compare(w, got, ref, label=""):
+    """got/ref: lists of (O, LSE) per request."""
+    all_abs = []
+    worst = {"max_abs": 0.0, "lse": 0.0, "rel": 0.0}
+    for i, ((o, l), (ro, rl)) in enumerate(zip(got, ref)):
+        assert np.isfinite(o).all() and np.isfinite(l).all(), "%s request %d: non-finite output" % (label, i)
+        d = np.abs(o.astype(np.float64) - ro)
+        all_abs.append(d.reshape(-1))
+        rel = np.linalg.norm(o.astype(np.float64) - ro) / np.linalg.norm(ro)
+        worst["max_abs"] = max(worst["max_abs"], d.max())
+        worst["lse"] = max(worst["lse"], np.abs(l.astype(np.float64) - rl).max())
+        worst["rel"] = max(worst["rel"], rel)
+        assert rel <= REL_FRO, "%s request %d: relative error %.3e" % (label, i, rel)
+    mean_abs = np.concatenate(all_abs).mean()
+    assert worst["max_abs"] <= MAX_ABS, (label, worst)
+    assert mean_abs <= MEAN_ABS, (label, mean_abs)
+    assert worst["lse"] <= LSE_ABS, (label, worst)
+    worst["mean_abs"] = mean_abs
+    return worst
+
+
+def run_and_compare(w, label="", options=None, heads=None):
+    dw = device_workload(w)
+    try:
+        for k, v in (options or {}).items():
+            dw.pool.set_option(k, v)
+        dw.out.fill_(float("nan"))
+        dw.lse.fill_(float("nan"))
+        dw.decode()
+        got = dw.results()
+        # a second launch on the same pool must give the same bits (counters reset, determinism)
+        dw.out.fill_(float("nan"))
+        dw.decode()
+        got2 = dw.results()
+        for (o, l), (o2, l2) in zip(got, got2):
+            assert np.array_equal(o, o2) and np.array_equal(l, l2), "%s: relaunch differs" % label
+    finally:
+        dw.close()
+    ref = oracle.decode_workload(w)
+    return compare(w, got, ref, label)
+
+
+# ------------------------------------------------------------------ gather: bit-exact
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_gather_bit_exact_all_configs(torch_cuda, k):
+    w = W.config(k)
+    dw = device_workload(w)
+    try:
+        # cfg5 has 64 requests: check them all (the copies are cheap)
+        for i, r in enumerate(w.requests):
+            m = w.models[r.model_id]
+            gk, gv = dw.gather(i)
+            rk, rv = oracle.gather(w.arena, w.page_tokens, w.page_bytes, w.num_pages, m.kind,
+                                   m.n_kv_heads, m.head_dim_qk, m.head_dim_v, r.page_ids, r.context_len)
+            assert gk.tobytes() == rk.tobytes(), "cfg%d request %d K" % (k, i)
+            assert gv.tobytes() == rv.tobytes(), "cfg%d request %d V" % (k, i)
+    finally:
+        dw.close()
+
+
+def test_gather_arbitrary_bit_patterns(torch_cuda):
+    m = ModelCfg(KIND_KV, 4, 2, 16, 8, 1.0)
+    w = W.small_workload([m], [0, 0], [77, 3], page_tokens=8, seed=5)
+    rng = np.random.default_rng(6)
+    w.arena[:] = rng.integers(0, 65536, size=w.arena.size).astype(np.uint16)   # NaNs, -0, denormals
+    dw = device_workload(w)
+    try:
+        for i, r in enumerate(w.requests):
+            gk, gv = dw.gather(i)
+            rk, rv = oracle.gather(w.arena, 8, w.page_bytes, w.num_pages, 0, 2, 16, 8, r.page_ids, r.context_len)
+            assert gk.tobytes() == rk.tobytes() and gv.tobytes() == rv.tobytes()
+    finally:
+        dw.close()
+
+
+# ------------------------------------------------------------------ attention: small shapes, every kernel
+SMALL = [
+    # (models, req_models, req_ctx, P, value_shift)  -- several tiles and a ragged tail each
+    ([ModelCfg(KIND_KV, 8, 1, 128, 128, 128 ** -0.5)], [0, 0, 0], [1, 17, 1000], 16, 0.0),
+    ([ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5)], [0, 0], [4097, 700], 64, 0.0),
+    ([ModelCfg(KIND_KV, 32, 1, 128, 128, 128 ** -0.5)], [0], [9999], 64, 3.0),
+    ([ModelCfg(KIND_KV, 64, 8, 128, 128, 128 ** -0.5), ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5)],
+     [0, 1, 1, 0, 1], [333, 5000, 31, 2049, 128], 32, 0.0),
+    ([ModelCfg(KIND_KV, 12, 3, 64, 32, 0.2)], [0, 0], [500, 65], 16, 0.0),       # generic shapes
+    ([ModelCfg(KIND_KV, 40, 2, 128, 128, 0.1)], [0], [3000], 128, 3.0),          # g = 20 (ragged m-tile)
+    ([ModelCfg(KIND_MLA, 128, 1, 576, 512, 192 ** -0.5)], [0, 0], [2000, 129], 64, 0.0),
+    ([ModelCfg(KIND_MLA, 16, 1, 576, 512, 192 ** -0.5)], [0], [777], 64, 0.0),
+    ([ModelCfg(KIND_MLA, 8, 1, 64, 32, 0.3), ModelCfg(KIND_KV, 4, 2, 64, 64, 0.3)], [0, 1, 0], [100, 200, 7], 8, 0.0),
+]
+
+
+@pytest.mark.parametrize("case", range(len(SMALL)))
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_attention_small(torch_cuda, case, kernel):
+    import paper_2606_24506_b200 as cp
+    models, rm, rc, P, shift = SMALL[case]
+    scale = 0.1 if models[0].kind == KIND_MLA and models[0].head_dim_qk == 576 else 1.0
+    w = W.small_workload(models, rm, rc, page_tokens=P, seed=100 + case, value_scale=scale,
+                         value_shift=shift, keep_contiguous=False)
+    # few CTAs' worth of target tiles would give one tile per group: force real splitting
+    worst = run_and_compare(w, "small%d/k%d" % (case, kernel),
+                            {cp.CP_OPT_KERNEL: kernel, cp.CP_OPT_MIN_TILE_PAGES: 1})
+    print("small case %d kernel %d: %s" % (case, kernel, worst))
+
+
+def test_outputs_of_order_one_mla(torch_cuda):
+    """O(1)-sized outputs on the MLA shape: one dominant key and shifted latents, so that an
+    all-zero or mis-scaled result cannot hide under the absolute tolerances."""
+    import paper_2606_24506_b200 as cp
+    m = ModelCfg(KIND_MLA, 128, 1, 576, 512, 192 ** -0.5)
+    w = W.small_workload([m], [0], [3000], page_tokens=64, seed=321, value_scale=0.1,
+                         keep_contiguous=False)
+    # make token 1234 dominant for every head: k = 40 * mean-direction of the queries
+    q = W.bf16_to_f64(w.q[0])
+    direction = q.mean(0)
+    direction /= np.linalg.norm(direction)
+    r = w.requests[0]
+    pid = int(r.page_ids[1234 // 64])
+    row = w.arena.reshape(w.num_pages, -1)[pid].reshape(64, 576)
+    row[1234 % 64] = W.f32_to_bf16((direction * 6.0 + 1.0).astype(np.float32))
+    for kernel in (0, 1):
+        worst = run_and_compare(w, "mla_O1/k%d" % kernel, {cp.CP_OPT_KERNEL: kernel})
+        print(worst)
+
+
+# ------------------------------------------------------------------ invariants on the GPU path
+def test_page_permutation_is_bit_identical(torch_cuda):
+    """P5 on the GPU: split boundaries are logical, so moving the data to other physical
+    pages must not change a single bit."""
+    m = ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5)
+    a = W.small_workload([m], [0, 0], [5000, 333], page_tokens=64, seed=7, extra_pages=5)
+    b = W.small_workload([m], [0, 0], [5000, 333], page_tokens=64, seed=7, extra_pages=5)
+    # b: same logical data, different physical placement
+    perm = np.random.default_rng(99).permutation(b.num_pages)
+    pages = b.arena.reshape(b.num_pages, -1)
+    newp = np.empty_like(pages)
+    newp[perm] = pages
+    b.arena = newp.reshape(-1)
+    for r in b.requests:
+        r.page_ids = perm[r.page_ids].astype(np.int32)
+    res = []
+    for w in (a, b):
+        dw = device_workload(w)
+        dw.decode()
+        res.append(dw.results())
+        dw.close()
+    for (o1, l1), (o2, l2) in zip(*res):
+        assert np.array_equal(o1, o2) and np.array_equal(l1, l2)
+
+
+def test_poison_and_batch_independence(torch_cuda):
+    """P7 on the GPU: results do not depend on free pages, on the dead tail of the last page,
+    nor on which other requests share the launch."""
+    ms = [ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5), ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5)]
+    w = W.small_workload(ms, [0, 1, 0], [1000, 2500, 77], page_tokens=32, seed=11, extra_pages=9)
+    dw = device_workload(w)
+    dw.decode()
+    full = dw.results()
+    dw.close()
+    # rewrite everything that is not a mapped valid slot with other garbage (inf, big, NaN)
+    w2 = W.small_workload(ms, [0, 1, 0], [1000, 2500, 77], page_tokens=32, seed=11, extra_pages=9)
+    mask = (w2.arena == W.BF16_NAN)
+    junk = np.random.default_rng(3).choice(np.array([0x7F80, 0xFF80, 0x7F7F, 0x7FFF, 0x4000], np.uint16),
+                                           size=w2.arena.size)
+    w2.arena[mask] = junk[mask]
+    dw = device_workload(w2)
+    dw.decode()
+    junked = dw.results()
+    # request 1 alone, and the batch in another order
+    import torch
+    ids = np.array([1], dtype=np.int32)
+    m1 = ms[1]
+    q1 = torch.from_numpy(w2.q[1].view(np.int16).reshape(-1)).cuda()
+    o1 = torch.empty(m1.n_q_heads * m1.head_dim_v, dtype=torch.float32, device="cuda")
+    l1 = torch.empty(m1.n_q_heads, dtype=torch.float32, device="cuda")
+    dw.decode(ids=ids, q=q1, out=o1, lse=l1)
+    torch.cuda.synchronize()
+    alone = o1.cpu().numpy().reshape(m1.n_q_heads, m1.head_dim_v)
+    dw.close()
+    for (a, la), (b, lb) in zip(full, junked):
+        assert np.array_equal(a, b) and np.array_equal(la, lb)
+    ref = oracle.decode_workload(w2, request_indices=[1])[0]
+    assert np.abs(alone - ref[0]).max() <= MAX_ABS
+    assert np.linalg.norm(alone - ref[0]) / np.linalg.norm(ref[0]) <= REL_FRO
+
+
+def test_golden_g1_on_gpu(torch_cuda):
+    """The golden vector G1 (tests/golden/g1_kv.txt) through the CUDA path (d = 8)."""
+    from test_oracle_pins import _g1_inputs, manual_workload, parse_golden, bf16
+    Q, K, V = _g1_inputs()
+    m = ModelCfg(KIND_KV, 2, 1, 8, 8, 1.0 / np.sqrt(8.0))
+    w = manual_workload(m, 2, bf16(Q), bf16(K).reshape(5, 1, 8), bf16(V).reshape(5, 1, 8))
+    dw = device_workload(w)
+    dw.decode()
+    (o, l), = dw.results()
+    dw.close()
+    g = parse_golden("g1_kv.txt")
+    assert np.abs(l - g["lse"]).max() < 1e-5
+    for h in range(2):
+        assert np.abs(o[h] - g["out"][h]).max() < 5e-3   # P is rounded to bf16 on the tensor path
+
+
+def test_append_and_context_growth(torch_cuda):
+    """Decode, grow the context (same page, then a new page), decode again: the plan cache and
+    the device tables follow (slow path a0), results track the oracle at every step."""
+    m = ModelCfg(KIND_KV, 8, 1, 128, 128, 128 ** -0.5)
+    full = W.small_workload([m], [0], [200], page_tokens=16, seed=21)
+    r = full.requests[0]
+    dw = device_workload(full, map_requests=False)
+    n0 = 10                                     # pages mapped first: 160 tokens of capacity
+    dw.pool.map_pages(0, 0, r.page_ids[:n0], 150)
+    for ctx, extra in ((150, 0), (151, 0), (160, 0), (161, 1), (200, 2)):
+        if extra:
+            have = dw.pool.request_info(0)[2].size
+            dw.pool.map_pages(0, 0, r.page_ids[have:have + extra], ctx)
+        else:
+            dw.pool.map_pages(0, 0, None, ctx)
+        dw.decode()
+        (o, l), = dw.results()
+        ro, rl = oracle.attention(full.arena, 16, full.page_bytes, full.num_pages, 0, 8, 1, 128, 128,
+                                  m.softmax_scale, r.page_ids, ctx, full.q[0])
+        assert np.abs(o - ro).max() <= MAX_ABS and np.abs(l - rl).max() <= LSE_ABS
+        assert np.linalg.norm(o - ro) / np.linalg.norm(ro) <= REL_FRO
+    dw.close()
+
+
+def test_host_buffer_entry_point_matches_device_path(torch_cuda):
+    torch = torch_cuda
+    ms = [ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5), ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5)]
+    w = W.small_workload(ms, [0, 1], [3000, 900], page_tokens=64, seed=31)
+    dw = device_workload(w)
+    dw.decode()
+    dev = dw.results()
+    need = dw.pool.decode_workspace_bytes_host(dw.ids)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    q_host = torch.from_numpy(w.q_packed().view(np.int16)).pin_memory()
+    o_host = torch.empty(dw.out.numel(), dtype=torch.float32).pin_memory()
+    l_host = torch.empty(dw.lse.numel(), dtype=torch.float32).pin_memory()
+    dw.pool.decode_attention_host(dw.ids, q_host, o_host, l_host, ws, need, dw.stream())
+    o = np.concatenate([x[0].reshape(-1) for x in dev])
+    l = np.concatenate([x[1].reshape(-1) for x in dev])
+    assert np.array_equal(o_host.numpy(), o) and np.array_equal(l_host.numpy(), l)
+    dw.close()
+
+
+def test_workspace_too_small_is_rejected(torch_cuda):
+    import paper_2606_24506_b200 as cp
+    m = ModelCfg(KIND_KV, 8, 1, 128, 128, 128 ** -0.5)
+    w = W.small_workload([m], [0], [4000], page_tokens=16, seed=41)
+    dw = device_workload(w)
+    need = dw.ensure_workspace()
+    assert need > 0
+    with pytest.raises(cp.CrossPoolError) as e:
+        dw.pool.decode_attention(dw.ids, dw.q, dw.out, dw.lse, dw.ws, need - 4, dw.stream())
+    assert e.value.status == cp.CP_ERR_WORKSPACE
+    dw.close()
+
+
+# ------------------------------------------------------------------ the five BASELINE configs, full size
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_attention_full_config(torch_cuda, k):
+    """Full-size parity in the launch configuration bench.py times (default options)."""
+    w = W.config(k)
+    worst = run_and_compare(w, "cfg%d" % k)
+    print("cfg%d: %s" % (k, worst))
+
+
+@pytest.mark.parametrize("k", [2, 3])
+def test_attention_full_config_generic_kernel(torch_cuda, k):
+    """The shape-generic kernel on full-size inputs (independent GPU cross-check)."""
+    import paper_2606_24506_b200 as cp
+    w = W.config(k) if k == 2 else W.config3(ctx=(16384, 4096))
+    worst = run_and_compare(w, "cfg%d-generic" % k, {cp.CP_OPT_KERNEL: 1})
+    print("cfg%d generic: %s" % (k, worst))
