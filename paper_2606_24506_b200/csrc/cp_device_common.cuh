@@ -53,24 +53,36 @@ __host__ __device__ inline size_t cp_combine_smem_bytes(int max_splits, int thre
     return ((size_t)4 * threads + 40 + 2 * (size_t)max_splits) * sizeof(float);
 }
 
-__device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int arrivals_per_tile,
-                                    float *smem_f)
+__host__ __device__ inline int mtiles_pow2(int g)    // 16-head M tiles rounded up to a power of two
+{
+    int mt = (g + 15) / 16, q = 1;
+    while (q < mt) q <<= 1;
+    return q;
+}
+
+struct BlockSync {
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+
+// arrival_mode 0: one counter arrival per tile; 1: one per 16-head M tile (tensor-core KV path).
+// tid / nthr / sync: the participating threads (a whole CTA, or the consumer warps only).
+template <class Sync>
+__device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int arrival_mode,
+                                    float *smem_f, const int tid, const int nthr, Sync sync)
 {
     const Group g = p.groups[cu.group];
     const DevModel m = p.models[g.model];
     const int ns = g.n_splits;
     const int dv = m.d_v;
     const int stride = dv + kPartPad;
-    const int tid = threadIdx.x;
-    const int nthr = blockDim.x;
 
     // wait for all splits of the group (tiles are popped before combine units and never
     // block, so this spin terminates)
     if (tid == 0) {
-        const int want = ns * arrivals_per_tile;
+        const int want = ns * (arrival_mode ? mtiles_pow2(m.group) : 1);
         while (ld_acquire(p.group_counters + cu.group) < want) __nanosleep(32);
     }
-    __syncthreads();
+    sync();
 
     float4 *red4 = reinterpret_cast<float4 *>(smem_f);      // [nthr]
     float *red = smem_f + 4 * nthr;                         // [40]
@@ -89,19 +101,19 @@ __device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int
     }
     for (int o = 16; o > 0; o >>= 1) mloc = fmaxf(mloc, __shfl_xor_sync(0xffffffffu, mloc, o));
     if ((tid & 31) == 0) red[tid >> 5] = mloc;
-    __syncthreads();
+    sync();
     float M = -INFINITY;
     for (int w = 0; w < (nthr >> 5); ++w) M = fmaxf(M, red[w]);
-    __syncthreads();
+    sync();
     for (int s = tid; s < ns; s += nthr) w_s[s] = exp2f(w_s[s] - M);
-    __syncthreads();
+    sync();
     if (tid < 32) {                      // warp 0: strided in-order sums, then a fixed tree
         float L = 0.f;
         for (int s = tid; s < ns; s += 32) L += w_s[s] * l_s[s];
         for (int o = 16; o > 0; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
         if (tid == 0) red[32] = L;
     }
-    __syncthreads();
+    sync();
     const float L = red[32];
     const float invL = 1.0f / L;
 
@@ -120,7 +132,7 @@ __device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int
         }
         red4[z * nq + cq] = acc;
     }
-    __syncthreads();
+    sync();
     if (tid < nq) {
         float4 o = red4[tid];
         for (int zz = 1; zz < lanes; ++zz) {
@@ -132,7 +144,7 @@ __device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int
         *reinterpret_cast<float4 *>(dst) = o;
     }
     if (tid == 0) p.lse[g.lse_off + cu.head] = (M + log2f(L)) * 0.6931471805599453f;
-    __syncthreads();
+    sync();
 }
 
 // Persistent-scheduler epilogue: the last CTA to finish resets the counters so that the

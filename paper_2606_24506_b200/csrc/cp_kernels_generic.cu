@@ -122,7 +122,7 @@ cp_decode_generic_kernel(const DecodeParams p, int max_dk, int max_dv, int any_k
         if (work >= n_work) break;
 
         if (work >= p.n_tiles) {        // ---- LSE combine unit (step a4)
-            combine_unit(p, p.combines[work - p.n_tiles], 1, reinterpret_cast<float *>(smem_raw));
+            combine_unit(p, p.combines[work - p.n_tiles], 0, reinterpret_cast<float *>(smem_raw), tid, GEN_THREADS, BlockSync());
             continue;
         }
 

@@ -1,0 +1,561 @@
+// cp_kernels_kv.cu -- the MQA / GQA fast path of libcrosspool (hot-path steps a2-a6 for
+// kind CP_KIND_KV with d_k = d_v = 128): ONE persistent launch per decode step.
+//
+//   * 1 producer warp: pops work items (tiles, then combine units) from the device work
+//     list with a global atomic, translates logical pages through the page table and
+//     streams the pages into a ring of shared-memory stages with TMA
+//     (cp.async.bulk.tensor, SWIZZLE_128B boxes, mbarrier complete_tx, L2 evict-first).
+//   * 8 consumer warps: each page is consumed by one warp per 16-query-head M tile:
+//     S = Q K^T and O += P V on warp-level tensor-core MMA (mma.sync m16n8k16, bf16 in,
+//     fp32 accumulate; operands via conflict-free ldmatrix from the swizzled stage),
+//     online softmax in fp32 in log2 units.  North-star keeps tcgen05/TMEM for the MLA
+//     path; this path is HBM-bound and the MMA only keeps the FP32 ALUs off the critical
+//     path.
+//   * page lanes merge their running (m, l, O) through shared memory at the end of a
+//     tile (fixed tree => deterministic), then publish the split partial (or the final
+//     result when the group has a single split) and bump the group's counter; combine
+//     units (LSE combine, step a4) are popped from the same work list.
+//
+// Paper anchors: paged KV interface PAPER.md:L101,L122; KV-head-limited attention under
+// low concurrency PAPER.md:L21,L57; GPU-resident persistent control PAPER.md:L146.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdint>
+#include "cp_device_common.cuh"
+#include "cp_launch.h"
+
+namespace cp {
+
+constexpr int KV_CWARPS = 8;                       // consumer warps
+constexpr int KV_CTHREADS = KV_CWARPS * 32;        // 256
+constexpr int KV_THREADS = KV_CTHREADS + 32;       // + producer warp
+constexpr int KV_D = 128;                          // head dim (qk and v)
+constexpr int KV_TQ = 4;                           // tile-queue depth
+constexpr int KV_MERGE_SLOT_FLOATS = 68 * 32;      // per sender warp: 64 O + m0,m1,l0,l1 per lane
+constexpr int KV_MERGE_BYTES = 4 * KV_MERGE_SLOT_FLOATS * 4;
+constexpr int KV_MAX_STAGES = 16;
+constexpr int KV_SMEM_LIMIT = 232448;              // 227 KB opt-in maximum per CTA
+
+__host__ __device__ inline int kv_stage_bytes(int P) { return P * 4 * KV_D; }   // K + V blocks
+__host__ __device__ inline int kv_num_stages(int P)
+{
+    int n = (KV_SMEM_LIMIT - KV_MERGE_BYTES - 1024) / kv_stage_bytes(P);
+    return n > KV_MAX_STAGES ? KV_MAX_STAGES : n;
+}
+__host__ __device__ inline int kv_smem_bytes(int P)
+{
+    return kv_num_stages(P) * kv_stage_bytes(P) + KV_MERGE_BYTES + 1024;
+}
+__host__ __device__ inline int kv_mtiles(int g)     // 16-head M tiles, rounded to a power of two
+{
+    int mt = (g + 15) / 16, p = 1;
+    while (p < mt) p <<= 1;
+    return p;
+}
+
+// What the producer hands to the consumers for one work item (shared-memory tile queue), so
+// that no consumer warp chases tile -> group -> model pointers through global memory.
+struct TileDesc {
+    int32_t item;            // work index; < 0: no more work
+    int32_t group_idx;
+    int32_t page_begin;
+    int32_t npg;
+    int32_t split;
+    int32_t n_splits;
+    int32_t ctx;
+    int32_t gsize;           // query heads per kv head
+    int32_t mt;              // 16-head M tiles (power of two)
+    float scale_log2;
+    int64_t q_off, out_off, lse_off, part_off;
+};
+
+// ----------------------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                 "selp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    while (!mbar_try_wait(bar, parity)) { }
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, int c0, int c1,
+                                            uint32_t bar, uint64_t policy)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+                 " [%0], [%1, {%2, %3}], [%4], %5;"
+                 ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(bar), "l"(policy)
+                 : "memory");
+}
+__device__ __forceinline__ void ldmatrix_x4(uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3, uint32_t addr)
+{
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3, uint32_t addr)
+{
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+__device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
+{
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+__device__ __forceinline__ void consumer_bar()      // the 256 consumer threads only
+{
+    asm volatile("bar.sync 1, %0;" ::"n"(KV_CTHREADS) : "memory");
+}
+
+struct ConsumerSync {
+    __device__ __forceinline__ void operator()() const { consumer_bar(); }
+};
+
+// ----------------------------------------------------------------------------- the kernel
+template <int P>
+__global__ void __launch_bounds__(KV_THREADS, 1)
+cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap, int rows_per_page)
+{
+    constexpr int STAGE_BYTES = P * 4 * KV_D;
+    constexpr int SUB = P * 128;                    // one swizzled sub-tile: P rows x 128 B
+    constexpr int CH = P < 64 ? P : 64;             // tokens per softmax chunk
+    constexpr int NCH = P / CH;                     // chunks per page
+    constexpr int NT = CH / 8;                      // S n-tiles per chunk
+    const int NS = kv_num_stages(P);
+
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t *stage_base = smem;
+    float *merge = reinterpret_cast<float *>(smem + (size_t)NS * STAGE_BYTES);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + (size_t)NS * STAGE_BYTES + KV_MERGE_BYTES);
+    // bars: full[NS], empty[NS], tq_full[TQ], tq_empty[TQ]; then the tile queue, flag
+    uint64_t *full_b = bars, *empty_b = bars + NS, *tqf_b = bars + 2 * NS, *tqe_b = bars + 2 * NS + KV_TQ;
+    TileDesc *tq = reinterpret_cast<TileDesc *>(bars + 2 * NS + 2 * KV_TQ);
+    int *s_flag = reinterpret_cast<int *>(tq + KV_TQ);
+    // pages issued so far by the producer.  A slot's consecutive uses are consumed by DIFFERENT
+    // warps, so a consumer could otherwise wait on full[slot] two phases ahead of the barrier,
+    // where a parity wait is ambiguous; it first waits until its page has been issued (which
+    // implies the slot's previous use was released, i.e. the barrier is in the right phase).
+    uint32_t *s_issued = reinterpret_cast<uint32_t *>(s_flag + 1);
+
+    const int tid = threadIdx.x;
+    const int warp = tid >> 5;
+    const int lane = tid & 31;
+
+    if (tid == 0) {
+        // full[s]: one arrive.expect_tx by the producer + the TMA transaction bytes.
+        // empty[s]: a page is consumed by `mt` warps (one per 16-head M tile), which differs per
+        // model; the barrier counts all 8 consumer warps and the producer arrives on behalf of
+        // the (8 - mt) warps that do not touch the page when it refills the slot.
+        for (int i = 0; i < NS; ++i) { mbar_init(smem_u32(full_b + i), 1); mbar_init(smem_u32(empty_b + i), KV_CWARPS); }
+        for (int i = 0; i < KV_TQ; ++i) { mbar_init(smem_u32(tqf_b + i), 1); mbar_init(smem_u32(tqe_b + i), KV_CWARPS); }
+        *s_issued = 0;
+        asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap)) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    const int n_work = p.n_tiles + p.n_combines;
+
+    if (warp == KV_CWARPS) {
+        // =========================================================== producer warp
+        uint64_t policy;
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+        uint32_t pc = 0;          // pages issued by this CTA (ring position)
+        uint32_t qi = 0;          // work items pushed
+        for (;;) {
+            int work = 0;
+            if (lane == 0) work = atomicAdd(p.work_counter, 1);
+            work = __shfl_sync(0xffffffffu, work, 0);
+            const int item = work < n_work ? work : -1;
+            Tile tile = Tile{0, 0, 0, 0};
+            Group g;
+            g.req = 0; g.model = 0; g.kv_head = 0; g.n_splits = 1; g.n_pages = 0; g.batch_index = 0;
+            g.q_off = g.out_off = g.lse_off = g.part_off = 0;
+            int hkv = 1, mt = 1, gsize = 1, ctx = 0;
+            float scale_log2 = 0.f;
+            const bool is_tile = item >= 0 && item < p.n_tiles;
+            if (is_tile) {
+                tile = p.tiles[item];
+                g = p.groups[tile.group];
+                const DevModel m = p.models[g.model];
+                hkv = m.n_kv_heads; gsize = m.group; mt = kv_mtiles(m.group); scale_log2 = m.scale_log2;
+                ctx = __ldg(p.req_ctx + g.req);
+            }
+            // push the descriptor to the tile queue
+            const uint32_t qs = qi % KV_TQ;
+            mbar_wait(smem_u32(tqe_b + qs), ((qi / KV_TQ) & 1) ^ 1);
+            if (lane == 0) {
+                TileDesc d;
+                d.item = item; d.group_idx = tile.group; d.page_begin = tile.page_begin;
+                d.npg = tile.page_end - tile.page_begin; d.split = tile.split; d.n_splits = g.n_splits;
+                d.ctx = ctx; d.gsize = gsize; d.mt = mt; d.scale_log2 = scale_log2;
+                d.q_off = g.q_off; d.out_off = g.out_off; d.lse_off = g.lse_off; d.part_off = g.part_off;
+                tq[qs] = d;
+                mbar_arrive(smem_u32(tqf_b + qs));     // release: consumers acquire via try_wait
+            }
+            ++qi;
+            if (item < 0) break;
+            if (!is_tile) continue;                    // combine unit: nothing to load
+
+            const int32_t *pt = p.page_table + (int64_t)g.req * p.max_ppr + g.kv_head;
+            const int npg = tile.page_end - tile.page_begin;
+            for (int j0 = 0; j0 < npg; j0 += 32) {
+                // translate up to 32 logical pages at once (one coalesced-ish load per lane)
+                int32_t pid = 0;
+                if (j0 + lane < npg) pid = __ldg(pt + (int64_t)(tile.page_begin + j0 + lane) * hkv);
+                const int nj = min(32, npg - j0);
+                for (int j = 0; j < nj; ++j) {
+                    const int32_t my = __shfl_sync(0xffffffffu, pid, j);
+                    const uint32_t slot = pc % NS;
+                    const uint32_t par = ((pc / NS) & 1) ^ 1;
+                    mbar_wait(smem_u32(empty_b + slot), par);
+                    if (lane == 0) {
+                        // the (8 - mt) warps that do not consume this page: arrive on their behalf
+                        for (int x = mt; x < KV_CWARPS; ++x) mbar_arrive(smem_u32(empty_b + slot));
+                        const uint32_t fb = smem_u32(full_b + slot);
+                        mbar_arrive_expect_tx(fb, STAGE_BYTES);
+                        const uint32_t dst = smem_u32(stage_base + (size_t)slot * STAGE_BYTES);
+                        const int row = my * rows_per_page;
+                        tma_load_2d(dst, &tmap, 0, row, fb, policy);               // K, d 0..63
+                        tma_load_2d(dst + SUB, &tmap, 64, row, fb, policy);        // K, d 64..127
+                        tma_load_2d(dst + 2 * SUB, &tmap, 0, row + P, fb, policy); // V, d 0..63
+                        tma_load_2d(dst + 3 * SUB, &tmap, 64, row + P, fb, policy);// V, d 64..127
+                        asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(smem_u32(s_issued)), "r"(pc + 1) : "memory");
+                    }
+                    ++pc;
+                }
+            }
+        }
+    } else {
+        // =========================================================== consumer warps
+        uint32_t pc = 0;          // pages consumed by this CTA so far (ring position of tile start)
+        uint32_t qi = 0;
+        const int r0 = lane >> 2;             // fragment row (query head in the M tile), and r0 + 8
+        const int cq = (lane & 3) * 2;        // fragment column pair
+        for (;;) {
+            const uint32_t qs = qi % KV_TQ;
+            mbar_wait(smem_u32(tqf_b + qs), (qi / KV_TQ) & 1);
+            const TileDesc d = tq[qs];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(tqe_b + qs));
+            ++qi;
+            if (d.item < 0) break;
+            if (d.item >= p.n_tiles) {
+                combine_unit(p, p.combines[d.item - p.n_tiles], /*arrival_mode=*/1, merge, tid, KV_CTHREADS,
+                             ConsumerSync());
+                continue;
+            }
+            const int mt = d.mt;
+            const int NL = KV_CWARPS / mt;            // page lanes
+            const int mtile = warp % mt;
+            const int plane = warp / mt;
+            const int ctx = d.ctx;
+            const int npg = d.npg;
+            const int gsize = d.gsize;
+            const float scale_log2 = d.scale_log2;
+            const int h0 = mtile * 16 + r0, h1 = h0 + 8;     // heads (inside the group) of my two rows
+
+            // ---- Q fragments (A operand, 16 heads x 128), rows beyond the group are zero
+            uint32_t qf[8][4];
+            {
+                const uint16_t *q0 = p.q + d.q_off + (int64_t)h0 * KV_D;
+                const uint16_t *q1 = p.q + d.q_off + (int64_t)h1 * KV_D;
+#pragma unroll
+                for (int ks = 0; ks < 8; ++ks) {
+                    const int k = ks * 16 + cq;
+                    qf[ks][0] = h0 < gsize ? __ldg(reinterpret_cast<const uint32_t *>(q0 + k)) : 0u;
+                    qf[ks][1] = h1 < gsize ? __ldg(reinterpret_cast<const uint32_t *>(q1 + k)) : 0u;
+                    qf[ks][2] = h0 < gsize ? __ldg(reinterpret_cast<const uint32_t *>(q0 + k + 8)) : 0u;
+                    qf[ks][3] = h1 < gsize ? __ldg(reinterpret_cast<const uint32_t *>(q1 + k + 8)) : 0u;
+                }
+            }
+            float o[16][4];
+#pragma unroll
+            for (int i = 0; i < 16; ++i) { o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f; }
+            float m_run[2] = {-INFINITY, -INFINITY};
+            float l_run[2] = {0.f, 0.f};              // per-thread partial row sums
+
+            for (int j = plane; j < npg; j += NL) {
+                const uint32_t pidx = pc + (uint32_t)j;
+                const uint32_t slot = pidx % NS;
+                {
+                    uint32_t issued;
+                    do {
+                        asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(issued) : "r"(smem_u32(s_issued)) : "memory");
+                    } while ((int32_t)(issued - pidx) <= 0);
+                }
+                mbar_wait(smem_u32(full_b + slot), (pidx / NS) & 1);
+                const uint32_t sb = smem_u32(stage_base + (size_t)slot * STAGE_BYTES);
+                const int lp = d.page_begin + j;
+                const int valid = ctx - lp * P;                 // >= 1; < P only on the request's last page
+                if (valid < P) {
+                    // zero the V rows of dead slots (they may hold NaN; 0 * NaN would poison O)
+                    for (int i = lane; i < (P - valid) * 16; i += 32) {
+                        const int row = valid + (i >> 4), ch = i & 15;
+                        const uint32_t a = sb + 2 * SUB + (ch >> 3) * SUB + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
+                        asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
+                    }
+                    __syncwarp();
+                }
+#pragma unroll
+                for (int c = 0; c < NCH; ++c) {
+                    const int tok0 = c * CH;
+                    // ---- S = Q K^T for CH tokens
+                    float s[NT][4];
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) { s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f; }
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) {
+                        const int row = tok0 + nt * 8 + (lane & 7);
+                        const uint32_t rbase = sb + row * 128;
+#pragma unroll
+                        for (int kp = 0; kp < 4; ++kp) {       // pairs of k-steps (32 d values)
+                            const int ch = kp * 4 + (lane >> 3);          // 16-B chunk 0..15
+                            const uint32_t a = rbase + (ch >> 3) * SUB + (((ch & 7) ^ (row & 7)) << 4);
+                            uint32_t b0, b1, b2, b3;
+                            ldmatrix_x4(b0, b1, b2, b3, a);
+                            mma_bf16(s[nt], qf[2 * kp], b0, b1);
+                            mma_bf16(s[nt], qf[2 * kp + 1], b2, b3);
+                        }
+                    }
+                    // ---- online softmax (log2 units), rows r0 and r0 + 8
+                    float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) {
+                        const int t = tok0 + nt * 8 + cq;
+                        s[nt][0] = (t < valid) ? s[nt][0] * scale_log2 : -INFINITY;
+                        s[nt][1] = (t + 1 < valid) ? s[nt][1] * scale_log2 : -INFINITY;
+                        s[nt][2] = (t < valid) ? s[nt][2] * scale_log2 : -INFINITY;
+                        s[nt][3] = (t + 1 < valid) ? s[nt][3] * scale_log2 : -INFINITY;
+                        mx0 = fmaxf(mx0, fmaxf(s[nt][0], s[nt][1]));
+                        mx1 = fmaxf(mx1, fmaxf(s[nt][2], s[nt][3]));
+                    }
+                    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
+                    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+                    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+                    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+                    if (tok0 >= valid) continue;               // whole chunk dead (P = 128 tail)
+                    const float mn0 = fmaxf(m_run[0], mx0), mn1 = fmaxf(m_run[1], mx1);
+                    const float a0 = exp2f(m_run[0] - mn0), a1 = exp2f(m_run[1] - mn1);
+                    m_run[0] = mn0; m_run[1] = mn1;
+                    float sum0 = 0.f, sum1 = 0.f;
+                    uint32_t pf[NT / 2][4];
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) {
+                        const float p0 = exp2f(s[nt][0] - mn0), p1 = exp2f(s[nt][1] - mn0);
+                        const float p2 = exp2f(s[nt][2] - mn1), p3 = exp2f(s[nt][3] - mn1);
+                        sum0 += p0 + p1; sum1 += p2 + p3;
+                        pf[nt >> 1][(nt & 1) * 2 + 0] = pack_bf16(p0, p1);
+                        pf[nt >> 1][(nt & 1) * 2 + 1] = pack_bf16(p2, p3);
+                    }
+                    l_run[0] = l_run[0] * a0 + sum0;
+                    l_run[1] = l_run[1] * a1 + sum1;
+                    if (__any_sync(0xffffffffu, (a0 != 1.f) || (a1 != 1.f))) {
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) { o[i][0] *= a0; o[i][1] *= a0; o[i][2] *= a1; o[i][3] *= a1; }
+                    }
+                    // ---- O += P V
+#pragma unroll
+                    for (int kk = 0; kk < NT / 2; ++kk) {
+                        const int row = tok0 + kk * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+                        const uint32_t rbase = sb + 2 * SUB + row * 128;
+#pragma unroll
+                        for (int np = 0; np < 8; ++np) {       // pairs of d n-tiles
+                            const int ch = np * 2 + (lane >> 4);          // 16-B chunk of d
+                            const uint32_t a = rbase + (ch >> 3) * SUB + (((ch & 7) ^ (row & 7)) << 4);
+                            uint32_t b0, b1, b2, b3;
+                            ldmatrix_x4_trans(b0, b1, b2, b3, a);
+                            mma_bf16(o[2 * np], pf[kk], b0, b1);
+                            mma_bf16(o[2 * np + 1], pf[kk], b2, b3);
+                        }
+                    }
+                }
+                // release the stage (generic-proxy accesses ordered before the next TMA write)
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(empty_b + slot));
+            }
+            pc += (uint32_t)npg;
+
+            // ---- quad-reduce the row sums, then merge the page lanes (fixed tree)
+            l_run[0] += __shfl_xor_sync(0xffffffffu, l_run[0], 1);
+            l_run[0] += __shfl_xor_sync(0xffffffffu, l_run[0], 2);
+            l_run[1] += __shfl_xor_sync(0xffffffffu, l_run[1], 1);
+            l_run[1] += __shfl_xor_sync(0xffffffffu, l_run[1], 2);
+            for (int r = 1; r < NL; r <<= 1) {
+                const bool sender = (plane % (2 * r)) == r;
+                const bool receiver = (plane % (2 * r)) == 0 && plane + r < NL;
+                // slot of a (sender lane, m-tile): senders in this round are lanes r, 3r, 5r, ...
+                const int pair = plane / (2 * r);
+                float *slotp = merge + (size_t)((pair * mt + mtile) % 4) * KV_MERGE_SLOT_FLOATS;
+                if (sender) {
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        slotp[(i * 4 + 0) * 32 + lane] = o[i][0];
+                        slotp[(i * 4 + 1) * 32 + lane] = o[i][1];
+                        slotp[(i * 4 + 2) * 32 + lane] = o[i][2];
+                        slotp[(i * 4 + 3) * 32 + lane] = o[i][3];
+                    }
+                    slotp[64 * 32 + lane] = m_run[0];
+                    slotp[65 * 32 + lane] = m_run[1];
+                    slotp[66 * 32 + lane] = l_run[0];
+                    slotp[67 * 32 + lane] = l_run[1];
+                }
+                consumer_bar();
+                if (receiver) {
+                    const float om0 = slotp[64 * 32 + lane], om1 = slotp[65 * 32 + lane];
+                    const float ol0 = slotp[66 * 32 + lane], ol1 = slotp[67 * 32 + lane];
+                    const float M0 = fmaxf(m_run[0], om0), M1 = fmaxf(m_run[1], om1);
+                    // a lane that saw no page has m = -inf, l = 0, O = 0: weight 0
+                    const float wa0 = (m_run[0] == -INFINITY) ? 0.f : exp2f(m_run[0] - M0);
+                    const float wa1 = (m_run[1] == -INFINITY) ? 0.f : exp2f(m_run[1] - M1);
+                    const float wb0 = (om0 == -INFINITY) ? 0.f : exp2f(om0 - M0);
+                    const float wb1 = (om1 == -INFINITY) ? 0.f : exp2f(om1 - M1);
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        o[i][0] = o[i][0] * wa0 + slotp[(i * 4 + 0) * 32 + lane] * wb0;
+                        o[i][1] = o[i][1] * wa0 + slotp[(i * 4 + 1) * 32 + lane] * wb0;
+                        o[i][2] = o[i][2] * wa1 + slotp[(i * 4 + 2) * 32 + lane] * wb1;
+                        o[i][3] = o[i][3] * wa1 + slotp[(i * 4 + 3) * 32 + lane] * wb1;
+                    }
+                    l_run[0] = l_run[0] * wa0 + ol0 * wb0;
+                    l_run[1] = l_run[1] * wa1 + ol1 * wb1;
+                    m_run[0] = M0; m_run[1] = M1;
+                }
+                consumer_bar();
+            }
+
+            // ---- publish (page lane 0 of every M tile)
+            if (plane == 0) {
+                if (d.n_splits == 1) {
+                    const float i0 = 1.f / l_run[0], i1 = 1.f / l_run[1];
+                    float *d0 = p.out + d.out_off + (int64_t)h0 * KV_D + cq;
+                    float *d1 = p.out + d.out_off + (int64_t)h1 * KV_D + cq;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        if (h0 < gsize) *reinterpret_cast<float2 *>(d0 + i * 8) = make_float2(o[i][0] * i0, o[i][1] * i0);
+                        if (h1 < gsize) *reinterpret_cast<float2 *>(d1 + i * 8) = make_float2(o[i][2] * i1, o[i][3] * i1);
+                    }
+                    if ((lane & 3) == 0) {
+                        if (h0 < gsize) p.lse[d.lse_off + h0] = (m_run[0] + log2f(l_run[0])) * 0.6931471805599453f;
+                        if (h1 < gsize) p.lse[d.lse_off + h1] = (m_run[1] + log2f(l_run[1])) * 0.6931471805599453f;
+                    }
+                } else {
+                    constexpr int stride = KV_D + kPartPad;
+                    float *base = p.workspace + d.part_off + (int64_t)d.split * gsize * stride;
+                    float *d0 = base + (int64_t)h0 * stride + cq;
+                    float *d1 = base + (int64_t)h1 * stride + cq;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        if (h0 < gsize) __stcg(reinterpret_cast<float2 *>(d0 + i * 8), make_float2(o[i][0], o[i][1]));
+                        if (h1 < gsize) __stcg(reinterpret_cast<float2 *>(d1 + i * 8), make_float2(o[i][2], o[i][3]));
+                    }
+                    if ((lane & 3) == 0) {
+                        if (h0 < gsize) __stcg(reinterpret_cast<float2 *>(base + (int64_t)h0 * stride + KV_D), make_float2(m_run[0], l_run[0]));
+                        if (h1 < gsize) __stcg(reinterpret_cast<float2 *>(base + (int64_t)h1 * stride + KV_D), make_float2(m_run[1], l_run[1]));
+                    }
+                    __threadfence();
+                    __syncwarp();
+                    if (lane == 0) red_release_add(p.group_counters + d.group_idx, 1);
+                }
+            }
+        }
+    }
+    scheduler_epilogue(p, s_flag);
+}
+
+// ----------------------------------------------------------------------------- host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (fn) return fn;
+    void *ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+        return nullptr;
+    fn = reinterpret_cast<EncodeTiledFn>(ptr);
+    return fn;
+}
+
+// 2-D view of the arena as rows of `row_elems` bf16; box = box_cols x box_rows, SWIZZLE_128B.
+bool make_arena_tensor_map(void *out_map, const void *arena, uint64_t total_rows, uint32_t row_elems,
+                           uint32_t box_cols, uint32_t box_rows)
+{
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[2] = {row_elems, total_rows};
+    cuuint64_t strides[1] = {(cuuint64_t)row_elems * 2};
+    cuuint32_t box[2] = {box_cols, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(reinterpret_cast<CUtensorMap *>(out_map), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+                    const_cast<void *>(arena), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+bool kv_fast_supported(int P) { return P == 16 || P == 32 || P == 64 || P == 128; }
+
+template <int P>
+static cudaError_t launch_kv_t(const DecodeParams &p, const CUtensorMap &tmap, int rows_per_page, int grid,
+                               cudaStream_t stream)
+{
+    const int smem = kv_smem_bytes(P);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(cp_decode_kv_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    cp_decode_kv_kernel<P><<<grid, KV_THREADS, smem, stream>>>(p, tmap, rows_per_page);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_decode_kv(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas,
+                             cudaStream_t stream)
+{
+    const CUtensorMap &tm = *reinterpret_cast<const CUtensorMap *>(tmap);
+    int grid = p.n_tiles + p.n_combines;
+    if (grid > n_ctas) grid = n_ctas;
+    if (grid < 1) grid = 1;
+    switch (p.page_tokens) {
+    case 16: return launch_kv_t<16>(p, tm, rows_per_page, grid, stream);
+    case 32: return launch_kv_t<32>(p, tm, rows_per_page, grid, stream);
+    case 64: return launch_kv_t<64>(p, tm, rows_per_page, grid, stream);
+    case 128: return launch_kv_t<128>(p, tm, rows_per_page, grid, stream);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace cp

@@ -14,4 +14,11 @@ size_t generic_smem_bytes(int max_dk, int max_dv, bool any_kv_kind, int max_spli
 cudaError_t launch_decode_generic(const DecodeParams &p, int max_dk, int max_dv, bool any_kv_kind,
                                   int max_splits, int n_ctas, cudaStream_t stream);
 
+// tensor-core MQA/GQA path (cp_kernels_kv.cu)
+bool kv_fast_supported(int page_tokens);
+bool make_arena_tensor_map(void *out_map, const void *arena, uint64_t total_rows, uint32_t row_elems,
+                           uint32_t box_cols, uint32_t box_rows);
+cudaError_t launch_decode_kv(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas,
+                             cudaStream_t stream);
+
 }  // namespace cp

@@ -58,6 +58,7 @@ struct KindPlan {
     int max_splits = 1;
     int max_dk = 0, max_dv = 0;
     int max_group = 0;
+    bool all_fast = false;           // every group of this kind runs on the tensor-core kernel
     bool uploaded = false;
     DevBuf d_groups, d_tiles, d_combines, d_counters;   // counters: [2] work + [n_groups]
 };
@@ -95,6 +96,8 @@ struct cp_pool {
     bool dev_ready = false;
     int n_sm = 148;
     DevBuf d_page_table, d_ctx, d_models;
+    alignas(64) unsigned char kv_tmap[128];   // CUtensorMap of the arena for the MQA/GQA kernel
+    bool kv_tmap_ok = false;
 
     // counters
     uint64_t n_launches = 0, n_plan_builds = 0, n_h2d_bytes = 0;
@@ -155,13 +158,17 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         const int64_t target_tiles = std::max<int64_t>(1, (int64_t)n_ctas * pool->opt_waves_x16 / 16);
         int64_t L = (total_pages[k] + target_tiles - 1) / target_tiles;
         L = std::max<int64_t>(L, pool->opt_min_tile_pages);
+        kp.all_fast = true;
         for (int b = 0; b < n; ++b) {
             const Request &r = pool->reqs[ids[b]];
             const cp_model_cfg &m = pool->models[r.model];
             if (m.kind != k) continue;
             const int g = m.n_q_heads / m.n_kv_heads;
             const int n_lp = ceil_div(r.ctx, P);
-            const int ns = (int)((n_lp + L - 1) / L);
+            int ns = (int)((n_lp + L - 1) / L);
+            ns = std::min(ns, 1024);                      // bounds the combine's shared memory
+            if (k == CP_KIND_KV && !(m.head_dim_qk == 128 && m.head_dim_v == 128 && g <= 128))
+                kp.all_fast = false;
             kp.max_splits = std::max(kp.max_splits, ns);
             kp.max_dk = std::max(kp.max_dk, m.head_dim_qk);
             kp.max_dv = std::max(kp.max_dv, m.head_dim_v);
@@ -259,6 +266,13 @@ cp_status ensure_device(cp_pool *pool)
         return CP_ERR_CUDA;
     if (cudaMemset(pool->d_ctx.ptr, 0, (size_t)pool->max_requests * 4) != cudaSuccess)
         return CP_ERR_CUDA;
+    pool->kv_tmap_ok = false;
+    if (kv_fast_supported((int)pool->P) && pool->page_bytes % 256 == 0 &&
+        pool->page_bytes >= pool->P * 512u) {
+        const uint64_t rows = (uint64_t)pool->num_pages * (pool->page_bytes / 256);
+        pool->kv_tmap_ok = rows < (1ull << 32) &&
+                           make_arena_tensor_map(pool->kv_tmap, pool->arena, rows, 128, 64, pool->P);
+    }
     pool->n_sm = sms;
     pool->dev_ready = true;
     pool->plan_valid = false;               // the SM count feeds the planner
@@ -608,8 +622,13 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.work_counter = (int32_t *)kp.d_counters.ptr;
         prm.group_counters = (int32_t *)kp.d_counters.ptr + 2;
         const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
-        cudaError_t e = launch_decode_generic(prm, kp.max_dk, kp.max_dv, k == CP_KIND_KV,
-                                              kp.max_splits, std::min(n_ctas, pool->n_sm), s);
+        cudaError_t e;
+        if (k == CP_KIND_KV && pool->opt_kernel == 0 && kp.all_fast && pool->kv_tmap_ok)
+            e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256),
+                                 std::min(n_ctas, pool->n_sm), s);
+        else
+            e = launch_decode_generic(prm, kp.max_dk, kp.max_dv, k == CP_KIND_KV, kp.max_splits,
+                                      std::min(n_ctas, pool->n_sm), s);
         pool->n_launches++;
         if (e != cudaSuccess) return CP_ERR_CUDA;
     }
