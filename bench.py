@@ -160,7 +160,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--kernel", type=int, default=0, help="CP_OPT_KERNEL (0 auto, 1 generic)")
+    ap.add_argument("--waves-x16", type=int, default=0, help="CP_OPT_WAVES_X16 (0 = library default)")
+    ap.add_argument("--min-tile-pages", type=int, default=0, help="CP_OPT_MIN_TILE_PAGES (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (tuning sweeps only)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -191,6 +194,10 @@ def main():
     w = W.config(k)
     dw = DeviceWorkload(w, dev)
     dw.pool.set_option(cp.CP_OPT_KERNEL, args.kernel)
+    if args.waves_x16 > 0:
+        dw.pool.set_option(cp.CP_OPT_WAVES_X16, args.waves_x16)
+    if args.min_tile_pages > 0:
+        dw.pool.set_option(cp.CP_OPT_MIN_TILE_PAGES, args.min_tile_pages)
     dw.ensure_workspace()
     abytes = w.algorithmic_bytes()
     flush = None
@@ -237,10 +244,10 @@ def main():
     q_host = torch.from_numpy(w.q_packed().view(np.int16)).pin_memory()
     o_host = torch.empty(dw.out.numel(), dtype=torch.float32).pin_memory()
     l_host = torch.empty(dw.lse.numel(), dtype=torch.float32).pin_memory()
-    for _ in range(3):
+    e2e_steps = 1 if args.no_e2e else args.steps
+    for _ in range(1 if args.no_e2e else 3):
         dw.pool.decode_attention_host(dw.ids, q_host, o_host, l_host, ws, need, dw.stream())
     barrier()
-    e2e_steps = args.steps
     t0 = time.perf_counter()
     for i in range(e2e_steps):
         if flush is not None:

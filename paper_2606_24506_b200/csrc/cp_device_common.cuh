@@ -147,6 +147,72 @@ __device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int
     sync();
 }
 
+// ---------------------------------------------------------------------------------------
+// Warp-sized LSE combine unit (tensor-core KV path): ONE warp combines 32 output columns
+// (`chunk`) of one (group, head); no CTA barrier, so the 8 consumer warps of a CTA run 8
+// units at once and the tail after the last tile stays a few microseconds even for
+// hundreds of splits.  Same arithmetic and the same fixed summation order per output
+// element as combine_unit (lane-strided in split order, then a fixed shuffle tree).
+// The group counter receives one arrival per (split, 16-head M tile).  wsm: this warp's
+// shared-memory scratch, >= n_splits floats.
+// ---------------------------------------------------------------------------------------
+__device__ inline void combine_warp_unit(const DecodeParams &p, const Combine cu, const int chunk,
+                                         float *wsm, const int lane)
+{
+    const Group g = p.groups[cu.group];
+    const DevModel m = p.models[g.model];
+    const int ns = g.n_splits;
+    const int dv = m.d_v;
+    const int stride = dv + kPartPad;
+    if (lane == 0) {
+        const int want = ns * mtiles_pow2(m.group);
+        while (ld_acquire(p.group_counters + cu.group) < want) __nanosleep(32);
+    }
+    __syncwarp();
+    const float *part = p.workspace + g.part_off + (int64_t)cu.head * stride;
+    const int64_t ss = (int64_t)m.group * stride;
+
+    float mloc = -INFINITY;
+    for (int s = lane; s < ns; s += 32)
+        mloc = fmaxf(mloc, __ldcg(reinterpret_cast<const float2 *>(part + s * ss + dv)).x);
+    for (int o = 16; o > 0; o >>= 1) mloc = fmaxf(mloc, __shfl_xor_sync(0xffffffffu, mloc, o));
+    const float M = mloc;
+    float L = 0.f;
+    for (int s = lane; s < ns; s += 32) {
+        const float2 ml = __ldcg(reinterpret_cast<const float2 *>(part + s * ss + dv));
+        const float w = exp2f(ml.x - M);
+        wsm[s] = w;
+        L += w * ml.y;
+    }
+    for (int o = 16; o > 0; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
+    __syncwarp();
+
+    // lane -> (split lane z of 4, column quad cq of 8)
+    const int cq = lane & 7, z = lane >> 3;
+    const float *src = part + chunk * 32 + cq * 4;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 8
+    for (int s = z; s < ns; s += 4) {
+        const float w = wsm[s];
+        const float4 v = ld_cg_f4(src + s * ss);
+        acc.x += w * v.x; acc.y += w * v.y; acc.z += w * v.z; acc.w += w * v.w;
+    }
+#pragma unroll
+    for (int o = 8; o <= 16; o <<= 1) {
+        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
+        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
+        acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
+    }
+    if (z == 0) {
+        const float invL = 1.0f / L;
+        float *dst = p.out + g.out_off + (int64_t)cu.head * dv + chunk * 32 + cq * 4;
+        *reinterpret_cast<float4 *>(dst) = make_float4(acc.x * invL, acc.y * invL, acc.z * invL, acc.w * invL);
+    }
+    if (chunk == 0 && lane == 0) p.lse[g.lse_off + cu.head] = (M + log2f(L)) * 0.6931471805599453f;
+    __syncwarp();               // wsm is reused by this warp's next unit
+}
+
 // Persistent-scheduler epilogue: the last CTA to finish resets the counters so that the
 // next launch (stream-ordered) starts from zero without a host memset.
 __device__ inline void scheduler_epilogue(const DecodeParams &p, int *s_flag)

@@ -8,6 +8,7 @@ namespace cp {
 constexpr int kPartPad = 4;          // partial row = d_v floats of O, then m, l, 2 pad floats
 constexpr int kMaxDk = 576;
 constexpr int kMaxDv = 512;
+constexpr int kMaxSplits = 512;      // KV splits per group (bounds the combine's shared memory)
 
 // Device copy of a model description (cp_model_cfg plus derived values).
 struct DevModel {
@@ -63,7 +64,8 @@ struct DecodeParams {
     const Tile *tiles;
     const Combine *combines;
     int32_t n_tiles;
-    int32_t n_combines;
+    int32_t n_combines;            // work items after the tiles (CTA-sized combine items)
+    int32_t n_combine_units;       // tensor-core kernels: warp-sized combine units; else = n_combines
     int32_t n_groups;
     const uint16_t *q;             // bf16 packed
     float *out;

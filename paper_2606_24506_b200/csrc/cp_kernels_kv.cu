@@ -5,16 +5,18 @@
 //     list with a global atomic, translates logical pages through the page table and
 //     streams the pages into a ring of shared-memory stages with TMA
 //     (cp.async.bulk.tensor, SWIZZLE_128B boxes, mbarrier complete_tx, L2 evict-first).
-//   * 8 consumer warps: each page is consumed by one warp per 16-query-head M tile:
-//     S = Q K^T and O += P V on warp-level tensor-core MMA (mma.sync m16n8k16, bf16 in,
-//     fp32 accumulate; operands via conflict-free ldmatrix from the swizzled stage),
-//     online softmax in fp32 in log2 units.  North-star keeps tcgen05/TMEM for the MLA
+//   * 8 consumer warps: a page is cut into 16-token slices; (slice, 16-query-head M tile)
+//     units are dealt round-robin to the warps, so all warps work on the oldest page of
+//     the ring at once.  S = Q K^T and O += P V on warp-level tensor-core MMA (mma.sync
+//     m16n8k16, bf16 in, fp32 accumulate; operands via conflict-free ldmatrix from the
+//     swizzled stage), online softmax in fp32 in log2 units.  North-star keeps tcgen05/TMEM for the MLA
 //     path; this path is HBM-bound and the MMA only keeps the FP32 ALUs off the critical
 //     path.
-//   * page lanes merge their running (m, l, O) through shared memory at the end of a
+//   * slice lanes merge their running (m, l, O) through shared memory at the end of a
 //     tile (fixed tree => deterministic), then publish the split partial (or the final
 //     result when the group has a single split) and bump the group's counter; combine
-//     units (LSE combine, step a4) are popped from the same work list.
+//     items (LSE combine, step a4: one warp per (group, head, 32 columns)) are popped
+//     from the same work list.
 //
 // Paper anchors: paged KV interface PAPER.md:L101,L122; KV-head-limited attention under
 // low concurrency PAPER.md:L21,L57; GPU-resident persistent control PAPER.md:L146.
@@ -36,13 +38,17 @@ constexpr int KV_MERGE_BYTES = 4 * KV_MERGE_SLOT_FLOATS * 4;
 constexpr int KV_MAX_STAGES = 16;
 constexpr int KV_SMEM_LIMIT = 232448;              // 227 KB opt-in maximum per CTA
 
-__host__ __device__ inline int kv_stage_bytes(int P) { return P * 4 * KV_D; }   // K + V blocks
-__host__ __device__ inline int kv_num_stages(int P)
+constexpr int KV_COMBINE_WARP_FLOATS = kMaxSplits;  // per-warp split weights of the LSE combine
+static_assert(KV_CWARPS * KV_COMBINE_WARP_FLOATS * 4 <= KV_MERGE_BYTES, "combine scratch must fit the merge area");
+
+__host__ __device__ constexpr int kv_stage_bytes(int P) { return P * 4 * KV_D; }   // K + V blocks
+__host__ __device__ constexpr int kv_num_stages(int P)
 {
-    int n = (KV_SMEM_LIMIT - KV_MERGE_BYTES - 1024) / kv_stage_bytes(P);
-    return n > KV_MAX_STAGES ? KV_MAX_STAGES : n;
+    return (KV_SMEM_LIMIT - KV_MERGE_BYTES - 1024) / kv_stage_bytes(P) > KV_MAX_STAGES
+               ? KV_MAX_STAGES
+               : (KV_SMEM_LIMIT - KV_MERGE_BYTES - 1024) / kv_stage_bytes(P);
 }
-__host__ __device__ inline int kv_smem_bytes(int P)
+__host__ __device__ constexpr int kv_smem_bytes(int P)
 {
     return kv_num_stages(P) * kv_stage_bytes(P) + KV_MERGE_BYTES + 1024;
 }
@@ -136,16 +142,93 @@ struct ConsumerSync {
 };
 
 // ----------------------------------------------------------------------------- the kernel
+// One work unit of a consumer warp: a 16-token slice of the page in stage `sb` against the
+// warp's 16-head M tile.  S (16 x 16) = Q K^T, online softmax (log2 units), O (16 x 128) += P V.
+template <int P>
+__device__ __forceinline__ void kv_slice_unit(const uint32_t sb, const int tok0, const int valid,
+                                              const uint32_t (&qf)[8][4], const float scale_log2,
+                                              float (&o)[16][4], float (&m_run)[2], float (&l_run)[2],
+                                              const int lane)
+{
+    constexpr int SUB = P * 128;                    // one swizzled sub-tile: P rows x 128 B
+    const int cq = (lane & 3) * 2;
+    // ---- S = Q K^T for 16 tokens (two 8-token n-tiles)
+    float s[2][4];
+#pragma unroll
+    for (int nt = 0; nt < 2; ++nt) { s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f; }
+#pragma unroll
+    for (int kp = 0; kp < 4; ++kp) {                // pairs of k-steps (32 d values)
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt) {
+            const int row = tok0 + nt * 8 + (lane & 7);
+            const int ch = kp * 4 + (lane >> 3);    // 16-B chunk 0..15 of the K row
+            const uint32_t a = sb + row * 128 + (ch >> 3) * SUB + (((ch & 7) ^ (row & 7)) << 4);
+            uint32_t b0, b1, b2, b3;
+            ldmatrix_x4(b0, b1, b2, b3, a);
+            mma_bf16(s[nt], qf[2 * kp], b0, b1);
+            mma_bf16(s[nt], qf[2 * kp + 1], b2, b3);
+        }
+    }
+    // ---- online softmax, rows r0 = lane / 4 and r0 + 8
+    float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+    for (int nt = 0; nt < 2; ++nt) {
+        const int t = tok0 + nt * 8 + cq;
+        s[nt][0] = (t < valid) ? s[nt][0] * scale_log2 : -INFINITY;
+        s[nt][1] = (t + 1 < valid) ? s[nt][1] * scale_log2 : -INFINITY;
+        s[nt][2] = (t < valid) ? s[nt][2] * scale_log2 : -INFINITY;
+        s[nt][3] = (t + 1 < valid) ? s[nt][3] * scale_log2 : -INFINITY;
+        mx0 = fmaxf(mx0, fmaxf(s[nt][0], s[nt][1]));
+        mx1 = fmaxf(mx1, fmaxf(s[nt][2], s[nt][3]));
+    }
+    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
+    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+    // token tok0 is valid (the caller skips dead slices), so mn0 / mn1 are finite
+    const float mn0 = fmaxf(m_run[0], mx0), mn1 = fmaxf(m_run[1], mx1);
+    const float a0 = exp2f(m_run[0] - mn0), a1 = exp2f(m_run[1] - mn1);
+    m_run[0] = mn0; m_run[1] = mn1;
+    uint32_t pf[4];
+    float sum0 = 0.f, sum1 = 0.f;
+#pragma unroll
+    for (int nt = 0; nt < 2; ++nt) {
+        const float p0 = exp2f(s[nt][0] - mn0), p1 = exp2f(s[nt][1] - mn0);
+        const float p2 = exp2f(s[nt][2] - mn1), p3 = exp2f(s[nt][3] - mn1);
+        sum0 += p0 + p1; sum1 += p2 + p3;
+        pf[nt * 2 + 0] = pack_bf16(p0, p1);
+        pf[nt * 2 + 1] = pack_bf16(p2, p3);
+    }
+    l_run[0] = l_run[0] * a0 + sum0;
+    l_run[1] = l_run[1] * a1 + sum1;
+    if (__any_sync(0xffffffffu, (a0 != 1.f) || (a1 != 1.f))) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) { o[i][0] *= a0; o[i][1] *= a0; o[i][2] *= a1; o[i][3] *= a1; }
+    }
+    // ---- O += P V (one 16-token k-step, 16 d n-tiles)
+    {
+        const int row = tok0 + (lane & 7) + ((lane >> 3) & 1) * 8;
+        const uint32_t rbase = sb + 2 * SUB + row * 128;
+#pragma unroll
+        for (int np = 0; np < 8; ++np) {            // pairs of d n-tiles
+            const int ch = np * 2 + (lane >> 4);    // 16-B chunk of d
+            const uint32_t a = rbase + (ch >> 3) * SUB + (((ch & 7) ^ (row & 7)) << 4);
+            uint32_t b0, b1, b2, b3;
+            ldmatrix_x4_trans(b0, b1, b2, b3, a);
+            mma_bf16(o[2 * np], pf, b0, b1);
+            mma_bf16(o[2 * np + 1], pf, b2, b3);
+        }
+    }
+}
+
 template <int P>
 __global__ void __launch_bounds__(KV_THREADS, 1)
 cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap, int rows_per_page)
 {
     constexpr int STAGE_BYTES = P * 4 * KV_D;
     constexpr int SUB = P * 128;                    // one swizzled sub-tile: P rows x 128 B
-    constexpr int CH = P < 64 ? P : 64;             // tokens per softmax chunk
-    constexpr int NCH = P / CH;                     // chunks per page
-    constexpr int NT = CH / 8;                      // S n-tiles per chunk
-    const int NS = kv_num_stages(P);
+    constexpr int SPP = P / 16;                     // 16-token slices per page
+    constexpr int NS = kv_num_stages(P);
 
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t *stage_base = smem;
@@ -155,11 +238,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
     uint64_t *full_b = bars, *empty_b = bars + NS, *tqf_b = bars + 2 * NS, *tqe_b = bars + 2 * NS + KV_TQ;
     TileDesc *tq = reinterpret_cast<TileDesc *>(bars + 2 * NS + 2 * KV_TQ);
     int *s_flag = reinterpret_cast<int *>(tq + KV_TQ);
-    // pages issued so far by the producer.  A slot's consecutive uses are consumed by DIFFERENT
-    // warps, so a consumer could otherwise wait on full[slot] two phases ahead of the barrier,
-    // where a parity wait is ambiguous; it first waits until its page has been issued (which
-    // implies the slot's previous use was released, i.e. the barrier is in the right phase).
-    uint32_t *s_issued = reinterpret_cast<uint32_t *>(s_flag + 1);
 
     const int tid = threadIdx.x;
     const int warp = tid >> 5;
@@ -167,19 +245,18 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
 
     if (tid == 0) {
         // full[s]: one arrive.expect_tx by the producer + the TMA transaction bytes.
-        // empty[s]: a page is consumed by `mt` warps (one per 16-head M tile), which differs per
-        // model; the barrier counts all 8 consumer warps and the producer arrives on behalf of
-        // the (8 - mt) warps that do not touch the page when it refills the slot.
+        // empty[s]: EVERY consumer warp waits for every page in ring order and arrives on its
+        // release, whether or not it owns a slice of the page: the barrier count is a constant
+        // and no warp can run a phase ahead of a stage.
         for (int i = 0; i < NS; ++i) { mbar_init(smem_u32(full_b + i), 1); mbar_init(smem_u32(empty_b + i), KV_CWARPS); }
         for (int i = 0; i < KV_TQ; ++i) { mbar_init(smem_u32(tqf_b + i), 1); mbar_init(smem_u32(tqe_b + i), KV_CWARPS); }
-        *s_issued = 0;
         asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap)) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
 
-    const int n_work = p.n_tiles + p.n_combines;
+    const int n_work = p.n_tiles + p.n_combines;     // n_combines = CTA-sized combine items here
 
     if (warp == KV_CWARPS) {
         // =========================================================== producer warp
@@ -220,12 +297,12 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             }
             ++qi;
             if (item < 0) break;
-            if (!is_tile) continue;                    // combine unit: nothing to load
+            if (!is_tile) continue;                    // combine item: nothing to load
 
             const int32_t *pt = p.page_table + (int64_t)g.req * p.max_ppr + g.kv_head;
             const int npg = tile.page_end - tile.page_begin;
             for (int j0 = 0; j0 < npg; j0 += 32) {
-                // translate up to 32 logical pages at once (one coalesced-ish load per lane)
+                // translate up to 32 logical pages at once (step a2: one page-table entry per lane)
                 int32_t pid = 0;
                 if (j0 + lane < npg) pid = __ldg(pt + (int64_t)(tile.page_begin + j0 + lane) * hkv);
                 const int nj = min(32, npg - j0);
@@ -235,8 +312,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                     const uint32_t par = ((pc / NS) & 1) ^ 1;
                     mbar_wait(smem_u32(empty_b + slot), par);
                     if (lane == 0) {
-                        // the (8 - mt) warps that do not consume this page: arrive on their behalf
-                        for (int x = mt; x < KV_CWARPS; ++x) mbar_arrive(smem_u32(empty_b + slot));
                         const uint32_t fb = smem_u32(full_b + slot);
                         mbar_arrive_expect_tx(fb, STAGE_BYTES);
                         const uint32_t dst = smem_u32(stage_base + (size_t)slot * STAGE_BYTES);
@@ -245,7 +320,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                         tma_load_2d(dst + SUB, &tmap, 64, row, fb, policy);        // K, d 64..127
                         tma_load_2d(dst + 2 * SUB, &tmap, 0, row + P, fb, policy); // V, d 0..63
                         tma_load_2d(dst + 3 * SUB, &tmap, 64, row + P, fb, policy);// V, d 64..127
-                        asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(smem_u32(s_issued)), "r"(pc + 1) : "memory");
                     }
                     ++pc;
                 }
@@ -266,12 +340,15 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             ++qi;
             if (d.item < 0) break;
             if (d.item >= p.n_tiles) {
-                combine_unit(p, p.combines[d.item - p.n_tiles], /*arrival_mode=*/1, merge, tid, KV_CTHREADS,
-                             ConsumerSync());
+                // LSE combine (step a4): each warp takes one (group, head, 32-column) unit
+                const int u = (d.item - p.n_tiles) * KV_CWARPS + warp;
+                if (u < p.n_combine_units)
+                    combine_warp_unit(p, p.combines[u / (KV_D / 32)], u % (KV_D / 32),
+                                      merge + warp * KV_COMBINE_WARP_FLOATS, lane);
                 continue;
             }
             const int mt = d.mt;
-            const int NL = KV_CWARPS / mt;            // page lanes
+            const int NL = KV_CWARPS / mt;            // slice lanes per M tile
             const int mtile = warp % mt;
             const int plane = warp / mt;
             const int ctx = d.ctx;
@@ -300,109 +377,41 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             float m_run[2] = {-INFINITY, -INFINITY};
             float l_run[2] = {0.f, 0.f};              // per-thread partial row sums
 
-            for (int j = plane; j < npg; j += NL) {
+            // Slices are dealt round-robin over the NL slice lanes in logical token order, so all
+            // warps work on the oldest page(s) of the ring at once and a stage is released after a
+            // fraction of the time one warp would need for a whole page.
+            for (int j = 0; j < npg; ++j) {
                 const uint32_t pidx = pc + (uint32_t)j;
                 const uint32_t slot = pidx % NS;
-                {
-                    uint32_t issued;
-                    do {
-                        asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(issued) : "r"(smem_u32(s_issued)) : "memory");
-                    } while ((int32_t)(issued - pidx) <= 0);
-                }
                 mbar_wait(smem_u32(full_b + slot), (pidx / NS) & 1);
                 const uint32_t sb = smem_u32(stage_base + (size_t)slot * STAGE_BYTES);
-                const int lp = d.page_begin + j;
-                const int valid = ctx - lp * P;                 // >= 1; < P only on the request's last page
-                if (valid < P) {
-                    // zero the V rows of dead slots (they may hold NaN; 0 * NaN would poison O)
-                    for (int i = lane; i < (P - valid) * 16; i += 32) {
-                        const int row = valid + (i >> 4), ch = i & 15;
-                        const uint32_t a = sb + 2 * SUB + (ch >> 3) * SUB + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
-                        asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
-                    }
-                    __syncwarp();
-                }
+                const int valid = ctx - (d.page_begin + j) * P;     // >= 1; < P only on the request's last page
+#ifndef CP_KV_PROBE_NO_COMPUTE
 #pragma unroll
-                for (int c = 0; c < NCH; ++c) {
-                    const int tok0 = c * CH;
-                    // ---- S = Q K^T for CH tokens
-                    float s[NT][4];
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) { s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f; }
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) {
-                        const int row = tok0 + nt * 8 + (lane & 7);
-                        const uint32_t rbase = sb + row * 128;
-#pragma unroll
-                        for (int kp = 0; kp < 4; ++kp) {       // pairs of k-steps (32 d values)
-                            const int ch = kp * 4 + (lane >> 3);          // 16-B chunk 0..15
-                            const uint32_t a = rbase + (ch >> 3) * SUB + (((ch & 7) ^ (row & 7)) << 4);
-                            uint32_t b0, b1, b2, b3;
-                            ldmatrix_x4(b0, b1, b2, b3, a);
-                            mma_bf16(s[nt], qf[2 * kp], b0, b1);
-                            mma_bf16(s[nt], qf[2 * kp + 1], b2, b3);
+                for (int s = 0; s < SPP; ++s) {
+                    if (((j * SPP + s) & (NL - 1)) != plane) continue;
+                    const int tok0 = s * 16;
+                    if (tok0 >= valid) continue;                     // dead slice of the last page
+                    if (valid < tok0 + 16) {
+                        // zero the V rows of dead slots (they may hold NaN; 0 * NaN would poison O)
+                        for (int i = lane; i < (tok0 + 16 - valid) * 16; i += 32) {
+                            const int row = valid + (i >> 4), ch = i & 15;
+                            const uint32_t a = sb + 2 * SUB + (ch >> 3) * SUB + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
+                            asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
                         }
+                        // generic-proxy writes ordered before the next TMA write into this stage
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                        __syncwarp();
                     }
-                    // ---- online softmax (log2 units), rows r0 and r0 + 8
-                    float mx0 = -INFINITY, mx1 = -INFINITY;
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) {
-                        const int t = tok0 + nt * 8 + cq;
-                        s[nt][0] = (t < valid) ? s[nt][0] * scale_log2 : -INFINITY;
-                        s[nt][1] = (t + 1 < valid) ? s[nt][1] * scale_log2 : -INFINITY;
-                        s[nt][2] = (t < valid) ? s[nt][2] * scale_log2 : -INFINITY;
-                        s[nt][3] = (t + 1 < valid) ? s[nt][3] * scale_log2 : -INFINITY;
-                        mx0 = fmaxf(mx0, fmaxf(s[nt][0], s[nt][1]));
-                        mx1 = fmaxf(mx1, fmaxf(s[nt][2], s[nt][3]));
-                    }
-                    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
-                    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
-                    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
-                    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
-                    if (tok0 >= valid) continue;               // whole chunk dead (P = 128 tail)
-                    const float mn0 = fmaxf(m_run[0], mx0), mn1 = fmaxf(m_run[1], mx1);
-                    const float a0 = exp2f(m_run[0] - mn0), a1 = exp2f(m_run[1] - mn1);
-                    m_run[0] = mn0; m_run[1] = mn1;
-                    float sum0 = 0.f, sum1 = 0.f;
-                    uint32_t pf[NT / 2][4];
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) {
-                        const float p0 = exp2f(s[nt][0] - mn0), p1 = exp2f(s[nt][1] - mn0);
-                        const float p2 = exp2f(s[nt][2] - mn1), p3 = exp2f(s[nt][3] - mn1);
-                        sum0 += p0 + p1; sum1 += p2 + p3;
-                        pf[nt >> 1][(nt & 1) * 2 + 0] = pack_bf16(p0, p1);
-                        pf[nt >> 1][(nt & 1) * 2 + 1] = pack_bf16(p2, p3);
-                    }
-                    l_run[0] = l_run[0] * a0 + sum0;
-                    l_run[1] = l_run[1] * a1 + sum1;
-                    if (__any_sync(0xffffffffu, (a0 != 1.f) || (a1 != 1.f))) {
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) { o[i][0] *= a0; o[i][1] *= a0; o[i][2] *= a1; o[i][3] *= a1; }
-                    }
-                    // ---- O += P V
-#pragma unroll
-                    for (int kk = 0; kk < NT / 2; ++kk) {
-                        const int row = tok0 + kk * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
-                        const uint32_t rbase = sb + 2 * SUB + row * 128;
-#pragma unroll
-                        for (int np = 0; np < 8; ++np) {       // pairs of d n-tiles
-                            const int ch = np * 2 + (lane >> 4);          // 16-B chunk of d
-                            const uint32_t a = rbase + (ch >> 3) * SUB + (((ch & 7) ^ (row & 7)) << 4);
-                            uint32_t b0, b1, b2, b3;
-                            ldmatrix_x4_trans(b0, b1, b2, b3, a);
-                            mma_bf16(o[2 * np], pf[kk], b0, b1);
-                            mma_bf16(o[2 * np + 1], pf[kk], b2, b3);
-                        }
-                    }
+                    kv_slice_unit<P>(sb, tok0, valid, qf, scale_log2, o, m_run, l_run, lane);
                 }
-                // release the stage (generic-proxy accesses ordered before the next TMA write)
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+#endif
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(empty_b + slot));
             }
             pc += (uint32_t)npg;
 
-            // ---- quad-reduce the row sums, then merge the page lanes (fixed tree)
+            // ---- quad-reduce the row sums, then merge the slice lanes (fixed tree)
             l_run[0] += __shfl_xor_sync(0xffffffffu, l_run[0], 1);
             l_run[0] += __shfl_xor_sync(0xffffffffu, l_run[0], 2);
             l_run[1] += __shfl_xor_sync(0xffffffffu, l_run[1], 1);
@@ -431,7 +440,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                     const float om0 = slotp[64 * 32 + lane], om1 = slotp[65 * 32 + lane];
                     const float ol0 = slotp[66 * 32 + lane], ol1 = slotp[67 * 32 + lane];
                     const float M0 = fmaxf(m_run[0], om0), M1 = fmaxf(m_run[1], om1);
-                    // a lane that saw no page has m = -inf, l = 0, O = 0: weight 0
+                    // a lane that saw no slice has m = -inf, l = 0, O = 0: weight 0
                     const float wa0 = (m_run[0] == -INFINITY) ? 0.f : exp2f(m_run[0] - M0);
                     const float wa1 = (m_run[1] == -INFINITY) ? 0.f : exp2f(m_run[1] - M1);
                     const float wb0 = (om0 == -INFINITY) ? 0.f : exp2f(om0 - M0);
@@ -450,7 +459,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 consumer_bar();
             }
 
-            // ---- publish (page lane 0 of every M tile)
+            // ---- publish (slice lane 0 of every M tile)
             if (plane == 0) {
                 if (d.n_splits == 1) {
                     const float i0 = 1.f / l_run[0], i1 = 1.f / l_run[1];

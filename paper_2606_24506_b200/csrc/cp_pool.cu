@@ -166,7 +166,7 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             const int g = m.n_q_heads / m.n_kv_heads;
             const int n_lp = ceil_div(r.ctx, P);
             int ns = (int)((n_lp + L - 1) / L);
-            ns = std::min(ns, 1024);                      // bounds the combine's shared memory
+            ns = std::min(ns, kMaxSplits);                // bounds the combine's shared memory
             if (k == CP_KIND_KV && !(m.head_dim_qk == 128 && m.head_dim_v == 128 && g <= 128))
                 kp.all_fast = false;
             kp.max_splits = std::max(kp.max_splits, ns);
@@ -200,6 +200,13 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         }
         std::stable_sort(kp.tiles.begin(), kp.tiles.end(), [](const Tile &a, const Tile &b) {
             return (a.page_end - a.page_begin) > (b.page_end - b.page_begin);
+        });
+        // combine units in the order in which their groups' last tiles are popped, so a CTA
+        // that runs out of tiles first combines the groups that finish first
+        std::vector<int> last_pos(kp.groups.size(), 0);
+        for (size_t i = 0; i < kp.tiles.size(); ++i) last_pos[kp.tiles[i].group] = (int)i;
+        std::stable_sort(kp.combines.begin(), kp.combines.end(), [&](const Combine &a, const Combine &b) {
+            return last_pos[a.group] < last_pos[b.group];
         });
     }
     pool->plan_ws_floats = ws;
@@ -616,6 +623,7 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.tiles = (const Tile *)kp.d_tiles.ptr;
         prm.combines = (const Combine *)kp.d_combines.ptr;
         prm.n_tiles = (int)kp.tiles.size(); prm.n_combines = (int)kp.combines.size();
+        prm.n_combine_units = prm.n_combines;
         prm.n_groups = (int)kp.groups.size();
         prm.q = (const uint16_t *)q_dev; prm.out = out_dev; prm.lse = lse_dev;
         prm.workspace = (float *)workspace_dev;
@@ -623,10 +631,13 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.group_counters = (int32_t *)kp.d_counters.ptr + 2;
         const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
         cudaError_t e;
-        if (k == CP_KIND_KV && pool->opt_kernel == 0 && kp.all_fast && pool->kv_tmap_ok)
+        if (k == CP_KIND_KV && pool->opt_kernel == 0 && kp.all_fast && pool->kv_tmap_ok) {
+            // warp-sized combine units: (group, head, 32 columns); 8 per CTA-sized work item
+            prm.n_combine_units = prm.n_combines * (128 / 32);
+            prm.n_combines = (prm.n_combine_units + 7) / 8;
             e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256),
                                  std::min(n_ctas, pool->n_sm), s);
-        else
+        } else
             e = launch_decode_generic(prm, kp.max_dk, kp.max_dv, k == CP_KIND_KV, kp.max_splits,
                                       std::min(n_ctas, pool->n_sm), s);
         pool->n_launches++;
