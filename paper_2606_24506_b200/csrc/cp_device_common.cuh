@@ -6,6 +6,10 @@
 #include <cstdint>
 #include "cp_internal.h"
 
+#ifndef KV_STAMP
+#define KV_STAMP(k, cond) do { } while (0)
+#endif
+
 namespace cp {
 
 __device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
@@ -16,6 +20,19 @@ __device__ __forceinline__ int ld_acquire(const int32_t *p)
     int v;
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
+}
+
+// Wait until group counter `gi` has reached `want` (called by one lane).  Polls with exponential
+// back-off: hundreds of warps polling one L2 line every few dozen ns would saturate its slice
+// and delay the very arrivals they wait for.
+__device__ __forceinline__ void wait_group(const int32_t *counters, int gi, int want)
+{
+    const int32_t *c = counters + (size_t)gi * kCounterStride;
+    unsigned ns = 128;
+    while (ld_acquire(c) < want) {
+        __nanosleep(ns);
+        if (ns < 1024) ns <<= 1;
+    }
 }
 
 __device__ __forceinline__ void red_release_add(int32_t *p, int v)
@@ -74,13 +91,12 @@ __device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int
     const DevModel m = p.models[g.model];
     const int ns = g.n_splits;
     const int dv = m.d_v;
-    const int stride = dv + kPartPad;
 
     // wait for all splits of the group (tiles are popped before combine units and never
     // block, so this spin terminates)
     if (tid == 0) {
         const int want = ns * (arrival_mode ? mtiles_pow2(m.group) : 1);
-        while (ld_acquire(p.group_counters + cu.group) < want) __nanosleep(32);
+        wait_group(p.group_counters, cu.group, want);
     }
     sync();
 
@@ -88,13 +104,14 @@ __device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int
     float *red = smem_f + 4 * nthr;                         // [40]
     float *w_s = red + 40;                                  // [ns]
     float *l_s = w_s + ns;                                  // [ns]
-    const float *part = p.workspace + g.part_off + (int64_t)cu.head * stride;
-    const int64_t split_stride = (int64_t)m.group * stride;
+    const float *part = p.workspace + g.part_off + part_o_off(cu.head, 0, ns, dv);
+    const float *mlp = p.workspace + g.part_off + part_ml_off(m.group, cu.head, 0, ns, dv);
+    const int64_t split_stride = dv;
 
     // pass 1: M = max m_s, weights, L
     float mloc = -INFINITY;
     for (int s = tid; s < ns; s += nthr) {
-        const float2 ml = __ldcg(reinterpret_cast<const float2 *>(part + s * split_stride + dv));
+        const float2 ml = __ldcg(reinterpret_cast<const float2 *>(mlp + 2 * s));
         w_s[s] = ml.x;
         l_s[s] = ml.y;
         mloc = fmaxf(mloc, ml.x);
@@ -148,57 +165,72 @@ __device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int
 }
 
 // ---------------------------------------------------------------------------------------
-// Warp-sized LSE combine unit (tensor-core KV path): ONE warp combines 32 output columns
-// (`chunk`) of one (group, head); no CTA barrier, so the 8 consumer warps of a CTA run 8
-// units at once and the tail after the last tile stays a few microseconds even for
-// hundreds of splits.  Same arithmetic and the same fixed summation order per output
-// element as combine_unit (lane-strided in split order, then a fixed shuffle tree).
-// The group counter receives one arrival per (split, 16-head M tile).  wsm: this warp's
-// shared-memory scratch, >= n_splits floats.
+// Warp-sized LSE combine unit (tensor-core kernels): ONE warp combines (128 >> zl) output
+// columns of one (group, head) described by a CombineUnit record; units are popped warp by
+// warp from a device counter, no CTA barrier.  The warp's lanes are (split lane z of
+// ZL = 2^zl) x (column quad cq of 32 / ZL): every lane fetches all its (<= 16) partial
+// vectors and (m, l) pairs in ONE batch of independent loads, so a unit costs two L2 round
+// trips (descriptor, data) whatever the split count.  Same arithmetic as combine_unit; all
+// sums run in a fixed order (k ascending per lane, then a fixed shuffle tree) => deterministic.
+// wsm: this warp's shared-memory scratch, >= n_splits floats.  n_splits <= kMaxSplits = 16 * 32
+// and n_splits <= 16 * ZL (the planner picks zl accordingly).
 // ---------------------------------------------------------------------------------------
-__device__ inline void combine_warp_unit(const DecodeParams &p, const Combine cu, const int chunk,
-                                         float *wsm, const int lane)
+__device__ __forceinline__ float ex2_ftz(float x)     // 2^x; ex2(-inf) = 0
 {
-    const Group g = p.groups[cu.group];
-    const DevModel m = p.models[g.model];
-    const int ns = g.n_splits;
-    const int dv = m.d_v;
-    const int stride = dv + kPartPad;
-    if (lane == 0) {
-        const int want = ns * mtiles_pow2(m.group);
-        while (ld_acquire(p.group_counters + cu.group) < want) __nanosleep(32);
-    }
-    __syncwarp();
-    const float *part = p.workspace + g.part_off + (int64_t)cu.head * stride;
-    const int64_t ss = (int64_t)m.group * stride;
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
 
-    float mloc = -INFINITY;
-    for (int s = lane; s < ns; s += 32)
-        mloc = fmaxf(mloc, __ldcg(reinterpret_cast<const float2 *>(part + s * ss + dv)).x);
-    for (int o = 16; o > 0; o >>= 1) mloc = fmaxf(mloc, __shfl_xor_sync(0xffffffffu, mloc, o));
-    const float M = mloc;
+// Deliberately compact (short loops unrolled by 4, 32-bit offsets): the code runs once per
+// launch per warp, so its cost is dominated by cold instruction-cache misses, not by issue slots.
+static __device__ __noinline__ void combine_warp_unit(const DecodeParams &p, const int u, float *wsm, const int lane)
+{
+    CombineUnit cu;
+    {
+        const uint4 *src = reinterpret_cast<const uint4 *>(p.cunits + u);
+        uint4 *dst = reinterpret_cast<uint4 *>(&cu);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) dst[i] = __ldg(src + i);
+    }
+    KV_STAMP(8, threadIdx.x == 0);
+    const int ns = cu.n_splits;
+    const int zl = cu.zl_log2;
+    const int ZL = 1 << zl, CQ = 32 >> zl;
+    const int z = lane >> (5 - zl), cq = lane & (CQ - 1);
+    if (lane == 0) wait_group(p.group_counters, cu.group, cu.want);
+    __syncwarp();
+    KV_STAMP(9, threadIdx.x == 0);
+    const float2 *mlp = reinterpret_cast<const float2 *>(p.workspace + cu.ml_off);
+    const float *src = p.workspace + cu.part_off + cq * 4;
+    const int ss = cu.split_stride;
+
+    // pass 1: M = max_s m_s (lane-strided, then a fixed tree)
+    float M = -INFINITY;
+#pragma unroll 4
+    for (int s = lane; s < ns; s += 32) M = fmaxf(M, __ldcg(mlp + s).x);
+    for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+    // pass 2: weights w_s = 2^(m_s - M) to shared memory, L = sum_s w_s l_s
     float L = 0.f;
+#pragma unroll 4
     for (int s = lane; s < ns; s += 32) {
-        const float2 ml = __ldcg(reinterpret_cast<const float2 *>(part + s * ss + dv));
-        const float w = exp2f(ml.x - M);
+        const float2 ml = __ldcg(mlp + s);
+        const float w = ex2_ftz(ml.x - M);
         wsm[s] = w;
         L += w * ml.y;
     }
     for (int o = 16; o > 0; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
     __syncwarp();
-
-    // lane -> (split lane z of 4, column quad cq of 8)
-    const int cq = lane & 7, z = lane >> 3;
-    const float *src = part + chunk * 32 + cq * 4;
+    KV_STAMP(10, threadIdx.x == 0);
+    // pass 3: O = sum_s w_s O_s over this lane's splits z, z + ZL, ... (in order), then the tree
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll 8
-    for (int s = z; s < ns; s += 4) {
-        const float w = wsm[s];
+#pragma unroll 4
+    for (int s = z; s < ns; s += ZL) {
         const float4 v = ld_cg_f4(src + s * ss);
+        const float w = wsm[s];
         acc.x += w * v.x; acc.y += w * v.y; acc.z += w * v.z; acc.w += w * v.w;
     }
-#pragma unroll
-    for (int o = 8; o <= 16; o <<= 1) {
+    for (int o = CQ; o < 32; o <<= 1) {               // warp-uniform trip count
         acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
         acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
         acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
@@ -206,11 +238,12 @@ __device__ inline void combine_warp_unit(const DecodeParams &p, const Combine cu
     }
     if (z == 0) {
         const float invL = 1.0f / L;
-        float *dst = p.out + g.out_off + (int64_t)cu.head * dv + chunk * 32 + cq * 4;
-        *reinterpret_cast<float4 *>(dst) = make_float4(acc.x * invL, acc.y * invL, acc.z * invL, acc.w * invL);
+        *reinterpret_cast<float4 *>(p.out + cu.out_off + cq * 4) =
+            make_float4(acc.x * invL, acc.y * invL, acc.z * invL, acc.w * invL);
     }
-    if (chunk == 0 && lane == 0) p.lse[g.lse_off + cu.head] = (M + log2f(L)) * 0.6931471805599453f;
+    if (cu.lse_off >= 0 && lane == 0) p.lse[cu.lse_off] = (M + log2f(L)) * 0.6931471805599453f;
     __syncwarp();               // wsm is reused by this warp's next unit
+    KV_STAMP(11, threadIdx.x == 0);
 }
 
 // Persistent-scheduler epilogue: the last CTA to finish resets the counters so that the
@@ -224,10 +257,11 @@ __device__ inline void scheduler_epilogue(const DecodeParams &p, int *s_flag)
     }
     __syncthreads();
     if (*s_flag) {
-        for (int i = threadIdx.x; i < p.n_groups; i += blockDim.x) p.group_counters[i] = 0;
+        for (int i = threadIdx.x; i < p.n_groups; i += blockDim.x) p.group_counters[(size_t)i * kCounterStride] = 0;
         if (threadIdx.x == 0) {
             p.work_counter[0] = 0;
             p.work_counter[1] = 0;
+            p.work_counter[2] = 0;
         }
     }
 }

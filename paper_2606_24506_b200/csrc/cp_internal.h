@@ -2,13 +2,29 @@
 // libcrosspool.  Private to paper_2606_24506_b200/csrc (the oracle shares nothing with it).
 #pragma once
 #include <cstdint>
+#ifndef __CUDACC__
+#define __host__
+#define __device__
+#endif
 
 namespace cp {
 
-constexpr int kPartPad = 4;          // partial row = d_v floats of O, then m, l, 2 pad floats
+// Split partials of one group in the workspace (float offsets from Group::part_off), g = heads of
+// the group, ns = its splits:  O[h][s][d_v] (unnormalised), then ML[h][s] = (m in log2 units, l).
+// Head-major, so the LSE combine of one head reads contiguous rows and a contiguous (m, l) vector.
+__host__ __device__ inline int64_t part_o_off(int h, int s, int ns, int dv) { return ((int64_t)h * ns + s) * dv; }
+__host__ __device__ inline int64_t part_ml_off(int g, int h, int s, int ns, int dv)
+{
+    return (int64_t)g * ns * dv + ((int64_t)h * ns + s) * 2;
+}
+__host__ __device__ inline int64_t part_group_floats(int g, int ns, int dv)
+{
+    return (((int64_t)g * ns * (dv + 2)) + 3) & ~(int64_t)3;
+}
 constexpr int kMaxDk = 576;
 constexpr int kMaxDv = 512;
-constexpr int kMaxSplits = 512;      // KV splits per group (bounds the combine's shared memory)
+constexpr int kMaxSplits = 512;
+constexpr int kCounterStride = 32;   // ints between group counters: one 128-byte line each (no false sharing under polling)      // KV splits per group (bounds the combine's shared memory)
 
 // Device copy of a model description (cp_model_cfg plus derived values).
 struct DevModel {
@@ -51,6 +67,22 @@ struct Combine {
     int32_t head;           // head index inside the group (0 .. g-1)
 };
 
+// One warp-sized unit of the LSE combine (tensor-core kernels): 128 >> zl_log2 output columns of
+// one (group, head), with everything the warp needs in one 64-byte record (no pointer chasing).
+struct CombineUnit {
+    int64_t part_off;       // float offset in the workspace of (split 0, this head, first column)
+    int64_t ml_off;         // float offset in the workspace of (m, l) of (split 0, this head); splits contiguous
+    int64_t out_off;        // float offset in packed O of (this head, first column)
+    int64_t lse_off;        // index in packed LSE of this head, or -1 if another unit writes it
+    int32_t split_stride;   // floats between consecutive splits of this head's O rows (= d_v)
+    int32_t n_splits;
+    int32_t zl_log2;        // split lanes of the warp = 1 << zl_log2 (1, 8 or 32)
+    int32_t want;           // arrivals on the group counter that mean "all splits published"
+    int32_t group;          // index of the group counter
+    int32_t pad[3];
+};
+static_assert(sizeof(CombineUnit) == 64, "CombineUnit is loaded as four 16-byte vectors");
+
 // Kernel arguments common to all decode kernels (passed by value).
 struct DecodeParams {
     const uint8_t *arena;
@@ -63,6 +95,7 @@ struct DecodeParams {
     const Group *groups;
     const Tile *tiles;
     const Combine *combines;
+    const CombineUnit *cunits;     // [n_combine_units] (tensor-core kernels)
     int32_t n_tiles;
     int32_t n_combines;            // work items after the tiles (CTA-sized combine items)
     int32_t n_combine_units;       // tensor-core kernels: warp-sized combine units; else = n_combines
@@ -71,8 +104,9 @@ struct DecodeParams {
     float *out;
     float *lse;
     float *workspace;              // split partials
-    int32_t *work_counter;         // [0] next work item, [1] CTAs that finished
-    int32_t *group_counters;       // [n_groups] tile arrivals
+    int32_t *work_counter;         // [0] next work item (tile), [1] CTAs that finished,
+                                   // [2] next warp-sized combine unit, [3] pad
+    int32_t *group_counters;       // [n_groups * kCounterStride] tile arrivals, counter g at g * kCounterStride
 };
 
 }  // namespace cp

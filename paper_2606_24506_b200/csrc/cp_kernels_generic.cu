@@ -259,17 +259,17 @@ cp_decode_generic_kernel(const DecodeParams p, int max_dk, int max_dv, int any_k
                 if (tid < nh)
                     p.lse[g.lse_off + h0 + tid] = (sm.m[tid] + log2f(sm.l[tid])) * 0.6931471805599453f;
             } else {
-                const int stride = dv + kPartPad;
-                float *part = p.workspace + g.part_off + ((int64_t)tile.split * m.group + h0) * stride;
+                float *ws = p.workspace + g.part_off;
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
                     const int c = tid + j * GEN_THREADS;
                     if (j < ncol && c < dv)
-                        for (int h = 0; h < nh; ++h) part[(int64_t)h * stride + c] = acc[j][h];
+                        for (int h = 0; h < nh; ++h) ws[part_o_off(h0 + h, tile.split, g.n_splits, dv) + c] = acc[j][h];
                 }
                 if (tid < nh) {
-                    part[(int64_t)tid * stride + dv] = sm.m[tid];
-                    part[(int64_t)tid * stride + dv + 1] = sm.l[tid];
+                    float *mlp = ws + part_ml_off(m.group, h0 + tid, tile.split, g.n_splits, dv);
+                    mlp[0] = sm.m[tid];
+                    mlp[1] = sm.l[tid];
                 }
             }
             __syncthreads();
@@ -278,7 +278,7 @@ cp_decode_generic_kernel(const DecodeParams p, int max_dk, int max_dv, int any_k
             // all partial stores of this CTA happen-before the release increment
             __threadfence();
             __syncthreads();
-            if (tid == 0) red_release_add(p.group_counters + tile.group, 1);
+            if (tid == 0) red_release_add(p.group_counters + (size_t)tile.group * kCounterStride, 1);
         }
     }
     scheduler_epilogue(p, &s_flag);

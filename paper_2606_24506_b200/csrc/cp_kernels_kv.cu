@@ -5,7 +5,7 @@
 //     list with a global atomic, translates logical pages through the page table and
 //     streams the pages into a ring of shared-memory stages with TMA
 //     (cp.async.bulk.tensor, SWIZZLE_128B boxes, mbarrier complete_tx, L2 evict-first).
-//   * 8 consumer warps: a page is cut into 16-token slices; (slice, 16-query-head M tile)
+//   * 8 consumer warps: a page is cut into 16/32-token slices; (slice, 16-query-head M tile)
 //     units are dealt round-robin to the warps, so all warps work on the oldest page of
 //     the ring at once.  S = Q K^T and O += P V on warp-level tensor-core MMA (mma.sync
 //     m16n8k16, bf16 in, fp32 accumulate; operands via conflict-free ldmatrix from the
@@ -23,6 +23,21 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstdint>
+namespace cp {
+#ifdef CP_KV_PROBE_TIMING        /* probe builds only: per-CTA globaltimer stamps */
+__device__ unsigned long long cp_kv_probe_ts[160 * 16];
+__device__ __forceinline__ void probe_stamp(int k)
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    cp_kv_probe_ts[blockIdx.x * 16 + k] = t;
+}
+#define KV_STAMP(k, cond) do { if (cond) probe_stamp(k); } while (0)
+#else
+#define KV_STAMP(k, cond) do { } while (0)
+#endif
+
+}  // namespace cp
 #include "cp_device_common.cuh"
 #include "cp_launch.h"
 
@@ -36,6 +51,8 @@ constexpr int KV_TQ = 4;                           // tile-queue depth
 constexpr int KV_MERGE_SLOT_FLOATS = 68 * 32;      // per sender warp: 64 O + m0,m1,l0,l1 per lane
 constexpr int KV_MERGE_BYTES = 4 * KV_MERGE_SLOT_FLOATS * 4;
 constexpr int KV_MAX_STAGES = 16;
+constexpr int KV_LDSM_DEPTH = 4;                   // ldmatrix prefetch distance (register ring)
+constexpr float KV_LAZY_LOG2 = 8.0f;               // lazy-rescale threshold (log2 units)
 constexpr int KV_SMEM_LIMIT = 232448;              // 227 KB opt-in maximum per CTA
 
 constexpr int KV_COMBINE_WARP_FLOATS = kMaxSplits;  // per-warp split weights of the LSE combine
@@ -122,9 +139,16 @@ __device__ __forceinline__ void ldmatrix_x4_trans(uint32_t &r0, uint32_t &r1, ui
 }
 __device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
 {
-    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+    // not volatile: the compiler may schedule it freely after the (ordered) ldmatrix that feeds it
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                  : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
                  : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ float ex2(float x)        // 2^x, flush-to-zero; ex2(-inf) = 0
+{
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
 }
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
 {
@@ -142,37 +166,50 @@ struct ConsumerSync {
 };
 
 // ----------------------------------------------------------------------------- the kernel
-// One work unit of a consumer warp: a 16-token slice of the page in stage `sb` against the
-// warp's 16-head M tile.  S (16 x 16) = Q K^T, online softmax (log2 units), O (16 x 128) += P V.
-template <int P>
+// One work unit of a consumer warp: a slice of 8*NT tokens of the page in stage `sb` against the
+// warp's 16-head M tile.  S (16 x 8NT) = Q K^T as NT independent accumulator chains (ILP for the
+// tensor pipe), one online-softmax update per unit (log2 units), O (16 x 128) += P V.
+// koff / vbase: per-lane swizzle constants (see the caller).
+template <int P, int NT>
 __device__ __forceinline__ void kv_slice_unit(const uint32_t sb, const int tok0, const int valid,
                                               const uint32_t (&qf)[8][4], const float scale_log2,
                                               float (&o)[16][4], float (&m_run)[2], float (&l_run)[2],
-                                              const int lane)
+                                              const int lane, const uint32_t (&koff)[2], const uint32_t vrow,
+                                              const uint32_t vbase)
 {
     constexpr int SUB = P * 128;                    // one swizzled sub-tile: P rows x 128 B
     const int cq = (lane & 3) * 2;
-    // ---- S = Q K^T for 16 tokens (two 8-token n-tiles)
-    float s[2][4];
+    // ---- S = Q K^T for 8*NT tokens
+    float s[NT][4];
 #pragma unroll
-    for (int nt = 0; nt < 2; ++nt) { s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f; }
+    for (int nt = 0; nt < NT; ++nt) { s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f; }
+    const uint32_t kb = sb + tok0 * 128;
+    {
+        // 4*NT ldmatrix.x4, each feeding 2 MMAs.  The loads are issued KV_LDSM_DEPTH steps ahead of
+        // their use through a small register ring (ldmatrix is asm volatile, i.e. kept in program
+        // order: without the explicit prefetch every MMA pair would wait a full shared-memory latency).
+        constexpr int L = 4 * NT;
+        uint32_t fr[KV_LDSM_DEPTH][4];
+        // load i -> (kp = i / NT, nt = i % NT): row = tok0 + nt*8 + (lane & 7); 16-B chunk kp*4 + (lane >> 3)
+#define KV_K_ADDR(i) (kb + ((i) % NT) * 8 * 128 + (((i) / NT) >> 1) * SUB + koff[((i) / NT) & 1])
 #pragma unroll
-    for (int kp = 0; kp < 4; ++kp) {                // pairs of k-steps (32 d values)
+        for (int i = 0; i < KV_LDSM_DEPTH; ++i)
+            ldmatrix_x4(fr[i][0], fr[i][1], fr[i][2], fr[i][3], KV_K_ADDR(i));
 #pragma unroll
-        for (int nt = 0; nt < 2; ++nt) {
-            const int row = tok0 + nt * 8 + (lane & 7);
-            const int ch = kp * 4 + (lane >> 3);    // 16-B chunk 0..15 of the K row
-            const uint32_t a = sb + row * 128 + (ch >> 3) * SUB + (((ch & 7) ^ (row & 7)) << 4);
-            uint32_t b0, b1, b2, b3;
-            ldmatrix_x4(b0, b1, b2, b3, a);
-            mma_bf16(s[nt], qf[2 * kp], b0, b1);
-            mma_bf16(s[nt], qf[2 * kp + 1], b2, b3);
+        for (int i = 0; i < L; ++i) {
+            const int kp = i / NT, nt = i % NT;
+            mma_bf16(s[nt], qf[2 * kp], fr[i % KV_LDSM_DEPTH][0], fr[i % KV_LDSM_DEPTH][1]);
+            mma_bf16(s[nt], qf[2 * kp + 1], fr[i % KV_LDSM_DEPTH][2], fr[i % KV_LDSM_DEPTH][3]);
+            if (i + KV_LDSM_DEPTH < L)
+                ldmatrix_x4(fr[i % KV_LDSM_DEPTH][0], fr[i % KV_LDSM_DEPTH][1], fr[i % KV_LDSM_DEPTH][2],
+                            fr[i % KV_LDSM_DEPTH][3], KV_K_ADDR(i + KV_LDSM_DEPTH));
         }
+#undef KV_K_ADDR
     }
     // ---- online softmax, rows r0 = lane / 4 and r0 + 8
     float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
-    for (int nt = 0; nt < 2; ++nt) {
+    for (int nt = 0; nt < NT; ++nt) {
         const int t = tok0 + nt * 8 + cq;
         s[nt][0] = (t < valid) ? s[nt][0] * scale_log2 : -INFINITY;
         s[nt][1] = (t + 1 < valid) ? s[nt][1] * scale_log2 : -INFINITY;
@@ -182,42 +219,57 @@ __device__ __forceinline__ void kv_slice_unit(const uint32_t sb, const int tok0,
         mx1 = fmaxf(mx1, fmaxf(s[nt][2], s[nt][3]));
     }
     mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
-    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
     mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
     mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+    // Lazy reference update: the running reference m only moves when the slice maximum exceeds
+    // it by more than 2^KV_LAZY_LOG2 (p <= 2^KV_LAZY_LOG2 stays exact enough in bf16/fp32 and cannot
+    // overflow), so the O rescale below is rare instead of once per slice.  (m, l, O) stay
+    // mutually consistent: any reference gives the same O / l and LSE = m + log2 l.
     // token tok0 is valid (the caller skips dead slices), so mn0 / mn1 are finite
-    const float mn0 = fmaxf(m_run[0], mx0), mn1 = fmaxf(m_run[1], mx1);
-    const float a0 = exp2f(m_run[0] - mn0), a1 = exp2f(m_run[1] - mn1);
-    m_run[0] = mn0; m_run[1] = mn1;
-    uint32_t pf[4];
+    const float mn0 = (mx0 > m_run[0] + KV_LAZY_LOG2) ? mx0 : m_run[0];
+    const float mn1 = (mx1 > m_run[1] + KV_LAZY_LOG2) ? mx1 : m_run[1];
+    if (__any_sync(0xffffffffu, (mn0 != m_run[0]) || (mn1 != m_run[1]))) {
+        const float a0 = ex2(m_run[0] - mn0), a1 = ex2(m_run[1] - mn1);
+        l_run[0] *= a0; l_run[1] *= a1;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) { o[i][0] *= a0; o[i][1] *= a0; o[i][2] *= a1; o[i][3] *= a1; }
+        m_run[0] = mn0; m_run[1] = mn1;
+    }
+    uint32_t pf[NT * 2];
     float sum0 = 0.f, sum1 = 0.f;
 #pragma unroll
-    for (int nt = 0; nt < 2; ++nt) {
-        const float p0 = exp2f(s[nt][0] - mn0), p1 = exp2f(s[nt][1] - mn0);
-        const float p2 = exp2f(s[nt][2] - mn1), p3 = exp2f(s[nt][3] - mn1);
+    for (int nt = 0; nt < NT; ++nt) {
+        const float p0 = ex2(s[nt][0] - mn0), p1 = ex2(s[nt][1] - mn0);
+        const float p2 = ex2(s[nt][2] - mn1), p3 = ex2(s[nt][3] - mn1);
         sum0 += p0 + p1; sum1 += p2 + p3;
         pf[nt * 2 + 0] = pack_bf16(p0, p1);
         pf[nt * 2 + 1] = pack_bf16(p2, p3);
     }
-    l_run[0] = l_run[0] * a0 + sum0;
-    l_run[1] = l_run[1] * a1 + sum1;
-    if (__any_sync(0xffffffffu, (a0 != 1.f) || (a1 != 1.f))) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) { o[i][0] *= a0; o[i][1] *= a0; o[i][2] *= a1; o[i][3] *= a1; }
-    }
-    // ---- O += P V (one 16-token k-step, 16 d n-tiles)
+    l_run[0] += sum0;
+    l_run[1] += sum1;
+    // ---- O += P V (NT/2 k-steps of 16 tokens, 16 d n-tiles): 4*NT ldmatrix.x4.trans, same ring
     {
-        const int row = tok0 + (lane & 7) + ((lane >> 3) & 1) * 8;
-        const uint32_t rbase = sb + 2 * SUB + row * 128;
+        constexpr int L = 4 * NT;
+        uint32_t fr[KV_LDSM_DEPTH][4];
+        // load i -> (kk = i / 8, np = i % 8): row = tok0 + kk*16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+        // 16-B chunk np*2 + (lane >> 4)
+        const uint32_t vb = sb + 2 * SUB + tok0 * 128 + vrow;
+#define KV_V_ADDR(i) (vb + ((i) / 8) * 16 * 128 + ((((i) % 8)) >> 2) * SUB + ((vbase ^ (uint32_t)(2 * (((i) % 8) & 3))) << 4))
 #pragma unroll
-        for (int np = 0; np < 8; ++np) {            // pairs of d n-tiles
-            const int ch = np * 2 + (lane >> 4);    // 16-B chunk of d
-            const uint32_t a = rbase + (ch >> 3) * SUB + (((ch & 7) ^ (row & 7)) << 4);
-            uint32_t b0, b1, b2, b3;
-            ldmatrix_x4_trans(b0, b1, b2, b3, a);
-            mma_bf16(o[2 * np], pf, b0, b1);
-            mma_bf16(o[2 * np + 1], pf, b2, b3);
+        for (int i = 0; i < KV_LDSM_DEPTH; ++i)
+            ldmatrix_x4_trans(fr[i][0], fr[i][1], fr[i][2], fr[i][3], KV_V_ADDR(i));
+#pragma unroll
+        for (int i = 0; i < L; ++i) {
+            const int kk = i / 8, np = i % 8;
+            const uint32_t (&pa)[4] = *reinterpret_cast<const uint32_t (*)[4]>(&pf[kk * 4]);
+            mma_bf16(o[2 * np], pa, fr[i % KV_LDSM_DEPTH][0], fr[i % KV_LDSM_DEPTH][1]);
+            mma_bf16(o[2 * np + 1], pa, fr[i % KV_LDSM_DEPTH][2], fr[i % KV_LDSM_DEPTH][3]);
+            if (i + KV_LDSM_DEPTH < L)
+                ldmatrix_x4_trans(fr[i % KV_LDSM_DEPTH][0], fr[i % KV_LDSM_DEPTH][1], fr[i % KV_LDSM_DEPTH][2],
+                                  fr[i % KV_LDSM_DEPTH][3], KV_V_ADDR(i + KV_LDSM_DEPTH));
         }
+#undef KV_V_ADDR
     }
 }
 
@@ -227,7 +279,9 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
 {
     constexpr int STAGE_BYTES = P * 4 * KV_D;
     constexpr int SUB = P * 128;                    // one swizzled sub-tile: P rows x 128 B
-    constexpr int SPP = P / 16;                     // 16-token slices per page
+    constexpr int NT = P >= 32 ? 4 : 2;             // 8-token n-tiles per work unit
+    constexpr int TU = 8 * NT;                      // tokens per work unit (slice)
+    constexpr int SPP = P / TU;                     // slices per page
     constexpr int NS = kv_num_stages(P);
 
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -242,6 +296,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
     const int tid = threadIdx.x;
     const int warp = tid >> 5;
     const int lane = tid & 31;
+    KV_STAMP(0, tid == 0);
 
     if (tid == 0) {
         // full[s]: one arrive.expect_tx by the producer + the TMA transaction bytes.
@@ -256,7 +311,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
     }
     __syncthreads();
 
-    const int n_work = p.n_tiles + p.n_combines;     // n_combines = CTA-sized combine items here
 
     if (warp == KV_CWARPS) {
         // =========================================================== producer warp
@@ -268,14 +322,14 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             int work = 0;
             if (lane == 0) work = atomicAdd(p.work_counter, 1);
             work = __shfl_sync(0xffffffffu, work, 0);
-            const int item = work < n_work ? work : -1;
+            const int item = work < p.n_tiles ? work : -1;      // tiles only; combine units are popped by the consumer warps
             Tile tile = Tile{0, 0, 0, 0};
             Group g;
             g.req = 0; g.model = 0; g.kv_head = 0; g.n_splits = 1; g.n_pages = 0; g.batch_index = 0;
             g.q_off = g.out_off = g.lse_off = g.part_off = 0;
             int hkv = 1, mt = 1, gsize = 1, ctx = 0;
             float scale_log2 = 0.f;
-            const bool is_tile = item >= 0 && item < p.n_tiles;
+            const bool is_tile = item >= 0;
             if (is_tile) {
                 tile = p.tiles[item];
                 g = p.groups[tile.group];
@@ -297,7 +351,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             }
             ++qi;
             if (item < 0) break;
-            if (!is_tile) continue;                    // combine item: nothing to load
 
             const int32_t *pt = p.page_table + (int64_t)g.req * p.max_ppr + g.kv_head;
             const int npg = tile.page_end - tile.page_begin;
@@ -313,6 +366,9 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                     mbar_wait(smem_u32(empty_b + slot), par);
                     if (lane == 0) {
                         const uint32_t fb = smem_u32(full_b + slot);
+#ifdef CP_KV_PROBE_NO_LOAD      /* probe builds only: consumer capacity without memory traffic */
+                        mbar_arrive(fb);
+#else
                         mbar_arrive_expect_tx(fb, STAGE_BYTES);
                         const uint32_t dst = smem_u32(stage_base + (size_t)slot * STAGE_BYTES);
                         const int row = my * rows_per_page;
@@ -320,6 +376,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                         tma_load_2d(dst + SUB, &tmap, 64, row, fb, policy);        // K, d 64..127
                         tma_load_2d(dst + 2 * SUB, &tmap, 0, row + P, fb, policy); // V, d 0..63
                         tma_load_2d(dst + 3 * SUB, &tmap, 64, row + P, fb, policy);// V, d 64..127
+#endif
                     }
                     ++pc;
                 }
@@ -331,6 +388,11 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
         uint32_t qi = 0;
         const int r0 = lane >> 2;             // fragment row (query head in the M tile), and r0 + 8
         const int cq = (lane & 3) * 2;        // fragment column pair
+        // per-lane constants of the SWIZZLE_128B addressing (16-B chunk index ^ (row & 7), row & 7 = lane & 7)
+        const uint32_t koff[2] = {(uint32_t)((lane & 7) * 128 + ((((lane >> 3)) ^ (lane & 7)) << 4)),
+                                  (uint32_t)((lane & 7) * 128 + (((4 + (lane >> 3)) ^ (lane & 7)) << 4))};
+        const uint32_t vrow = (uint32_t)(((lane & 7) + ((lane >> 3) & 1) * 8) * 128);
+        const uint32_t vbase = (uint32_t)((lane >> 4) ^ (lane & 7));
         for (;;) {
             const uint32_t qs = qi % KV_TQ;
             mbar_wait(smem_u32(tqf_b + qs), (qi / KV_TQ) & 1);
@@ -339,14 +401,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             if (lane == 0) mbar_arrive(smem_u32(tqe_b + qs));
             ++qi;
             if (d.item < 0) break;
-            if (d.item >= p.n_tiles) {
-                // LSE combine (step a4): each warp takes one (group, head, 32-column) unit
-                const int u = (d.item - p.n_tiles) * KV_CWARPS + warp;
-                if (u < p.n_combine_units)
-                    combine_warp_unit(p, p.combines[u / (KV_D / 32)], u % (KV_D / 32),
-                                      merge + warp * KV_COMBINE_WARP_FLOATS, lane);
-                continue;
-            }
+            KV_STAMP(1, tid == 0 && qi == 1);
             const int mt = d.mt;
             const int NL = KV_CWARPS / mt;            // slice lanes per M tile
             const int mtile = warp % mt;
@@ -384,17 +439,18 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 const uint32_t pidx = pc + (uint32_t)j;
                 const uint32_t slot = pidx % NS;
                 mbar_wait(smem_u32(full_b + slot), (pidx / NS) & 1);
+                KV_STAMP(2, tid == 0 && qi == 1 && j == 0);
                 const uint32_t sb = smem_u32(stage_base + (size_t)slot * STAGE_BYTES);
                 const int valid = ctx - (d.page_begin + j) * P;     // >= 1; < P only on the request's last page
 #ifndef CP_KV_PROBE_NO_COMPUTE
 #pragma unroll
                 for (int s = 0; s < SPP; ++s) {
                     if (((j * SPP + s) & (NL - 1)) != plane) continue;
-                    const int tok0 = s * 16;
+                    const int tok0 = s * TU;
                     if (tok0 >= valid) continue;                     // dead slice of the last page
-                    if (valid < tok0 + 16) {
+                    if (valid < tok0 + TU) {
                         // zero the V rows of dead slots (they may hold NaN; 0 * NaN would poison O)
-                        for (int i = lane; i < (tok0 + 16 - valid) * 16; i += 32) {
+                        for (int i = lane; i < (tok0 + TU - valid) * 16; i += 32) {
                             const int row = valid + (i >> 4), ch = i & 15;
                             const uint32_t a = sb + 2 * SUB + (ch >> 3) * SUB + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
                             asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
@@ -403,13 +459,14 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                         __syncwarp();
                     }
-                    kv_slice_unit<P>(sb, tok0, valid, qf, scale_log2, o, m_run, l_run, lane);
+                    kv_slice_unit<P, NT>(sb, tok0, valid, qf, scale_log2, o, m_run, l_run, lane, koff, vrow, vbase);
                 }
 #endif
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(empty_b + slot));
             }
             pc += (uint32_t)npg;
+            KV_STAMP(3, tid == 0);
 
             // ---- quad-reduce the row sums, then merge the slice lanes (fixed tree)
             l_run[0] += __shfl_xor_sync(0xffffffffu, l_run[0], 1);
@@ -459,6 +516,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 consumer_bar();
             }
 
+            KV_STAMP(4, tid == 0);
             // ---- publish (slice lane 0 of every M tile)
             if (plane == 0) {
                 if (d.n_splits == 1) {
@@ -475,27 +533,39 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                         if (h1 < gsize) p.lse[d.lse_off + h1] = (m_run[1] + log2f(l_run[1])) * 0.6931471805599453f;
                     }
                 } else {
-                    constexpr int stride = KV_D + kPartPad;
-                    float *base = p.workspace + d.part_off + (int64_t)d.split * gsize * stride;
-                    float *d0 = base + (int64_t)h0 * stride + cq;
-                    float *d1 = base + (int64_t)h1 * stride + cq;
+                    float *ws = p.workspace + d.part_off;
+                    float *d0 = ws + part_o_off(h0, d.split, d.n_splits, KV_D) + cq;
+                    float *d1 = ws + part_o_off(h1, d.split, d.n_splits, KV_D) + cq;
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
                         if (h0 < gsize) __stcg(reinterpret_cast<float2 *>(d0 + i * 8), make_float2(o[i][0], o[i][1]));
                         if (h1 < gsize) __stcg(reinterpret_cast<float2 *>(d1 + i * 8), make_float2(o[i][2], o[i][3]));
                     }
                     if ((lane & 3) == 0) {
-                        if (h0 < gsize) __stcg(reinterpret_cast<float2 *>(base + (int64_t)h0 * stride + KV_D), make_float2(m_run[0], l_run[0]));
-                        if (h1 < gsize) __stcg(reinterpret_cast<float2 *>(base + (int64_t)h1 * stride + KV_D), make_float2(m_run[1], l_run[1]));
+                        if (h0 < gsize) __stcg(reinterpret_cast<float2 *>(ws + part_ml_off(gsize, h0, d.split, d.n_splits, KV_D)), make_float2(m_run[0], l_run[0]));
+                        if (h1 < gsize) __stcg(reinterpret_cast<float2 *>(ws + part_ml_off(gsize, h1, d.split, d.n_splits, KV_D)), make_float2(m_run[1], l_run[1]));
                     }
-                    __threadfence();
+                    // the warp's partial stores happen-before lane 0's gpu-scope release (cumulative
+                    // over the __syncwarp), which the combine units acquire: no membar needed
                     __syncwarp();
-                    if (lane == 0) red_release_add(p.group_counters + d.group_idx, 1);
+                    if (lane == 0) red_release_add(p.group_counters + (size_t)d.group_idx * kCounterStride, 1);
                 }
             }
         }
+        KV_STAMP(5, tid == 0);
+#ifndef CP_KV_PROBE_NO_COMBINE
+        // ---- LSE combine (step a4): no tile is left to pop; every consumer warp runs its
+        // warp-sized units.  A unit only waits for tiles that are already running on some SM, so
+        // the spin inside terminates.
+        // Units are assigned statically (unit u -> consumer warp u mod #warps of the grid): popping
+        // them from one counter would serialise thousands of same-address atomics at the L2.
+        for (int u = blockIdx.x * KV_CWARPS + warp; u < p.n_combine_units; u += gridDim.x * KV_CWARPS)
+            combine_warp_unit(p, u, merge + warp * KV_COMBINE_WARP_FLOATS, lane);
+#endif
+        KV_STAMP(6, tid == 0);
     }
     scheduler_epilogue(p, s_flag);
+    KV_STAMP(7, tid == 0);
 }
 
 // ----------------------------------------------------------------------------- host side
@@ -534,6 +604,13 @@ bool make_arena_tensor_map(void *out_map, const void *arena, uint64_t total_rows
     return r == CUDA_SUCCESS;
 }
 
+#ifdef CP_KV_PROBE_TIMING
+extern "C" int cp_kv_probe_read(unsigned long long *out_host)
+{
+    return (int)cudaMemcpyFromSymbol(out_host, cp_kv_probe_ts, sizeof(cp_kv_probe_ts));
+}
+#endif
+
 bool kv_fast_supported(int P) { return P == 16 || P == 32 || P == 64 || P == 128; }
 
 template <int P>
@@ -555,7 +632,8 @@ cudaError_t launch_decode_kv(const DecodeParams &p, const void *tmap, int rows_p
                              cudaStream_t stream)
 {
     const CUtensorMap &tm = *reinterpret_cast<const CUtensorMap *>(tmap);
-    int grid = p.n_tiles + p.n_combines;
+    int grid = p.n_tiles > (p.n_combine_units + KV_CWARPS - 1) / KV_CWARPS
+                   ? p.n_tiles : (p.n_combine_units + KV_CWARPS - 1) / KV_CWARPS;
     if (grid > n_ctas) grid = n_ctas;
     if (grid < 1) grid = 1;
     switch (p.page_tokens) {

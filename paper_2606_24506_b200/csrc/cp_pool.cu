@@ -54,13 +54,14 @@ struct Request {
 struct KindPlan {
     std::vector<Group> groups;
     std::vector<Tile> tiles;
-    std::vector<Combine> combines;
+    std::vector<Combine> combines;       // CTA-sized combine units (generic kernel)
+    std::vector<CombineUnit> cunits;     // warp-sized combine units (tensor-core kernels)
     int max_splits = 1;
     int max_dk = 0, max_dv = 0;
     int max_group = 0;
     bool all_fast = false;           // every group of this kind runs on the tensor-core kernel
     bool uploaded = false;
-    DevBuf d_groups, d_tiles, d_combines, d_counters;   // counters: [2] work + [n_groups]
+    DevBuf d_groups, d_tiles, d_combines, d_cunits, d_counters;   // counters: [32] scheduler + [n_groups * kCounterStride]
 };
 
 }  // namespace
@@ -81,7 +82,7 @@ struct cp_pool {
     uint64_t topo_version = 1;           // bumps when any request's planned page count changes
 
     // options
-    int opt_kernel = 0, opt_num_ctas = 0, opt_waves_x16 = 32, opt_min_tile_pages = 2;
+    int opt_kernel = 0, opt_num_ctas = 0, opt_waves_x16 = 16, opt_min_tile_pages = 2;
 
     // plan cache
     std::vector<int32_t> plan_batch;
@@ -133,7 +134,7 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
     const int P = (int)pool->P;
     for (int k = 0; k < 2; ++k) {
         KindPlan &kp = pool->plan[k];
-        kp.groups.clear(); kp.tiles.clear(); kp.combines.clear();
+        kp.groups.clear(); kp.tiles.clear(); kp.combines.clear(); kp.cunits.clear();
         kp.max_splits = 1; kp.max_dk = kp.max_dv = kp.max_group = 0; kp.uploaded = false;
     }
     pool->q_off.assign(n, 0); pool->out_off.assign(n, 0); pool->lse_off.assign(n, 0);
@@ -155,9 +156,32 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
     for (int k = 0; k < 2; ++k) {
         KindPlan &kp = pool->plan[k];
         if (total_pages[k] == 0) continue;
+        // smallest tile length L (pages) for which the batch yields at most target_tiles tiles, so
+        // that with waves = w every persistent CTA gets exactly w near-equal tiles (one tile more
+        // on a few CTAs would cost a whole extra tile time at the end)
         const int64_t target_tiles = std::max<int64_t>(1, (int64_t)n_ctas * pool->opt_waves_x16 / 16);
-        int64_t L = (total_pages[k] + target_tiles - 1) / target_tiles;
-        L = std::max<int64_t>(L, pool->opt_min_tile_pages);
+        auto tiles_for = [&](int64_t len) {
+            int64_t t = 0;
+            for (int b = 0; b < n; ++b) {
+                const Request &r = pool->reqs[ids[b]];
+                const cp_model_cfg &m = pool->models[r.model];
+                if (m.kind == k) t += (int64_t)m.n_kv_heads * ((ceil_div(r.ctx, P) + len - 1) / len);
+            }
+            return t;
+        };
+        // (searched in [L_bal, 2 L_bal]; a batch of many short requests cannot meet the target at
+        // all -- every group is at least one tile -- and then keeps the balanced length L_bal)
+        const int64_t L_bal = std::max<int64_t>((total_pages[k] + target_tiles - 1) / target_tiles,
+                                                pool->opt_min_tile_pages);
+        int64_t L = L_bal;
+        if (tiles_for(2 * L_bal) <= target_tiles) {
+            int64_t lo = L_bal, hi = 2 * L_bal;
+            while (lo < hi) {
+                const int64_t mid = (lo + hi) / 2;
+                if (tiles_for(mid) <= target_tiles) hi = mid; else lo = mid + 1;
+            }
+            L = lo;
+        }
         kp.all_fast = true;
         for (int b = 0; b < n; ++b) {
             const Request &r = pool->reqs[ids[b]];
@@ -183,7 +207,7 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
                 gr.part_off = 0;
                 if (ns > 1) {
                     gr.part_off = (int64_t)ws;
-                    ws += (uint64_t)ns * g * (m.head_dim_v + kPartPad);
+                    ws += (uint64_t)part_group_floats(g, ns, m.head_dim_v);
                 }
                 const int gi = (int)kp.groups.size();
                 kp.groups.push_back(gr);
@@ -194,8 +218,30 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
                     kp.tiles.push_back(Tile{gi, s, pb, pb + len});
                     pb += len;
                 }
-                if (ns > 1)
+                if (ns > 1) {
                     for (int h = 0; h < g; ++h) kp.combines.push_back(Combine{gi, h});
+                    // warp-sized units: split lanes ZL so that a lane holds <= 16 splits (8 for ZL = 1, 8)
+                    const int zl = ns <= 8 ? 0 : (ns <= 64 ? 3 : (ns <= 256 ? 4 : 5));
+                    const int cols = 128 >> zl;
+                    const int mt = (g + 15) / 16;
+                    int mtp = 1;
+                    while (mtp < mt) mtp <<= 1;
+                    for (int h = 0; h < g; ++h)
+                        for (int c0 = 0; c0 < m.head_dim_v; c0 += cols) {
+                            CombineUnit cu;
+                            std::memset(&cu, 0, sizeof(cu));
+                            cu.part_off = gr.part_off + part_o_off(h, 0, ns, m.head_dim_v) + c0;
+                            cu.ml_off = gr.part_off + part_ml_off(g, h, 0, ns, m.head_dim_v);
+                            cu.out_off = gr.out_off + (int64_t)h * m.head_dim_v + c0;
+                            cu.lse_off = c0 == 0 ? gr.lse_off + h : -1;
+                            cu.split_stride = m.head_dim_v;
+                            cu.n_splits = ns;
+                            cu.zl_log2 = zl;
+                            cu.want = ns * (k == CP_KIND_KV ? mtp : 1);
+                            cu.group = gi;
+                            kp.cunits.push_back(cu);
+                        }
+                }
             }
         }
         std::stable_sort(kp.tiles.begin(), kp.tiles.end(), [](const Tile &a, const Tile &b) {
@@ -206,6 +252,9 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         std::vector<int> last_pos(kp.groups.size(), 0);
         for (size_t i = 0; i < kp.tiles.size(); ++i) last_pos[kp.tiles[i].group] = (int)i;
         std::stable_sort(kp.combines.begin(), kp.combines.end(), [&](const Combine &a, const Combine &b) {
+            return last_pos[a.group] < last_pos[b.group];
+        });
+        std::stable_sort(kp.cunits.begin(), kp.cunits.end(), [&](const CombineUnit &a, const CombineUnit &b) {
             return last_pos[a.group] < last_pos[b.group];
         });
     }
@@ -317,22 +366,25 @@ cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
 {
     if (kp.uploaded) return CP_OK;
     const size_t gb = kp.groups.size() * sizeof(Group), tb = kp.tiles.size() * sizeof(Tile);
-    const size_t cb = kp.combines.size() * sizeof(Combine), nb = (2 + kp.groups.size()) * 4;
+    const size_t cb = kp.combines.size() * sizeof(Combine), nb = (32 + kp.groups.size() * (size_t)kCounterStride) * 4;
+    const size_t ub = kp.cunits.size() * sizeof(CombineUnit);
     const bool counters_new = kp.d_counters.cap < nb;
     if (kp.d_groups.ensure(gb) != cudaSuccess || kp.d_tiles.ensure(tb) != cudaSuccess ||
         kp.d_combines.ensure(std::max(cb, (size_t)16)) != cudaSuccess ||
+        kp.d_cunits.ensure(std::max(ub, (size_t)64)) != cudaSuccess ||
         kp.d_counters.ensure(nb) != cudaSuccess) {
         cudaGetLastError();
         return CP_ERR_CUDA;
     }
     if (cudaMemcpyAsync(kp.d_groups.ptr, kp.groups.data(), gb, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
         cudaMemcpyAsync(kp.d_tiles.ptr, kp.tiles.data(), tb, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
-        (cb && cudaMemcpyAsync(kp.d_combines.ptr, kp.combines.data(), cb, cudaMemcpyHostToDevice, stream) != cudaSuccess))
+        (cb && cudaMemcpyAsync(kp.d_combines.ptr, kp.combines.data(), cb, cudaMemcpyHostToDevice, stream) != cudaSuccess) ||
+        (ub && cudaMemcpyAsync(kp.d_cunits.ptr, kp.cunits.data(), ub, cudaMemcpyHostToDevice, stream) != cudaSuccess))
         return CP_ERR_CUDA;
     // counters are zero between launches (the kernels reset them); zero a fresh buffer
     if (counters_new && cudaMemsetAsync(kp.d_counters.ptr, 0, kp.d_counters.cap, stream) != cudaSuccess)
         return CP_ERR_CUDA;
-    pool->n_h2d_bytes += gb + tb + cb;
+    pool->n_h2d_bytes += gb + tb + cb + ub;
     kp.uploaded = true;
     return CP_OK;
 }
@@ -401,7 +453,8 @@ cp_status cp_pool_free(cp_pool *pool)
     pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release();
     for (int k = 0; k < 2; ++k) {
         pool->plan[k].d_groups.release(); pool->plan[k].d_tiles.release();
-        pool->plan[k].d_combines.release(); pool->plan[k].d_counters.release();
+        pool->plan[k].d_combines.release(); pool->plan[k].d_cunits.release();
+        pool->plan[k].d_counters.release();
     }
     delete pool;
     return CP_OK;
@@ -622,19 +675,19 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.groups = (const Group *)kp.d_groups.ptr;
         prm.tiles = (const Tile *)kp.d_tiles.ptr;
         prm.combines = (const Combine *)kp.d_combines.ptr;
+        prm.cunits = (const CombineUnit *)kp.d_cunits.ptr;
         prm.n_tiles = (int)kp.tiles.size(); prm.n_combines = (int)kp.combines.size();
         prm.n_combine_units = prm.n_combines;
         prm.n_groups = (int)kp.groups.size();
         prm.q = (const uint16_t *)q_dev; prm.out = out_dev; prm.lse = lse_dev;
         prm.workspace = (float *)workspace_dev;
         prm.work_counter = (int32_t *)kp.d_counters.ptr;
-        prm.group_counters = (int32_t *)kp.d_counters.ptr + 2;
+        prm.group_counters = (int32_t *)kp.d_counters.ptr + 32;
         const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
         cudaError_t e;
         if (k == CP_KIND_KV && pool->opt_kernel == 0 && kp.all_fast && pool->kv_tmap_ok) {
-            // warp-sized combine units: (group, head, 32 columns); 8 per CTA-sized work item
-            prm.n_combine_units = prm.n_combines * (128 / 32);
-            prm.n_combines = (prm.n_combine_units + 7) / 8;
+            // warp-sized combine units, popped warp by warp after the tiles
+            prm.n_combine_units = (int)kp.cunits.size();
             e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256),
                                  std::min(n_ctas, pool->n_sm), s);
         } else

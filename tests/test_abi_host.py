@@ -144,8 +144,14 @@ def test_tile_plan_covers_every_page_once_and_balances():
     lens = [t[5] - t[4] for t in tiles]
     assert lens == sorted(lens, reverse=True)        # longest first
     total = sum(lens)
-    assert 148 <= len(tiles) <= 148 * 2 + n_groups   # about two waves on 148 CTAs
-    assert max(lens) <= -(-total // (148 * 2)) + 1
+    # one wave on 148 CTAs: at most one tile per CTA when the groups allow it, tile length within
+    # [L_bal, 2 L_bal] of the balanced length L_bal = ceil(total / 148)
+    assert 148 // 2 <= len(tiles) <= 148
+    assert max(lens) <= 2 * -(-total // 148)
+    p.set_option(cp.CP_OPT_WAVES_X16, 32)            # two waves
+    tiles_w2, _ = p.decode_plan(ids)
+    _coverage(tiles_w2, n_groups, pages_of)
+    assert 148 < len(tiles_w2) <= 148 * 2
     # plan options
     p.set_option(cp.CP_OPT_NUM_CTAS, 4)
     p.set_option(cp.CP_OPT_WAVES_X16, 16)
@@ -175,8 +181,9 @@ def test_workspace_bytes_formula():
     p.map_pages(0, 0, None, 4096 * 64, n_allocate=4096)
     tiles, ng = p.decode_plan([0])
     ns = tiles[0][3]
-    assert ng == 1 and ns == len(tiles) and 148 <= ns <= 300
-    assert p.decode_workspace_bytes([0]) == ns * 32 * (128 + 4) * 4
+    assert ng == 1 and ns == len(tiles) and 74 <= ns <= 148     # one wave on 148 CTAs
+    # per group: O[g][ns][d_v] + (m, l)[g][ns] floats (head-major partial layout)
+    assert p.decode_workspace_bytes([0]) == ns * 32 * (128 + 2) * 4
     p.map_pages(1, 0, None, 64, n_allocate=1)       # single-tile request adds no workspace
     assert p.decode_workspace_bytes([1]) == 0
     p.close()
