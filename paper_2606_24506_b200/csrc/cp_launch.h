@@ -21,4 +21,10 @@ bool make_arena_tensor_map(void *out_map, const void *arena, uint64_t total_rows
 cudaError_t launch_decode_kv(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas,
                              cudaStream_t stream);
 
+// tcgen05 MLA path (cp_kernels_mla.cu)
+bool mla_fast_supported(int page_tokens, uint32_t page_bytes);
+bool make_mla_tensor_map(void *out_map, const void *arena, uint64_t total_rows);
+cudaError_t launch_decode_mla(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas,
+                              cudaStream_t stream);
+
 }  // namespace cp

@@ -99,6 +99,8 @@ struct cp_pool {
     DevBuf d_page_table, d_ctx, d_models;
     alignas(64) unsigned char kv_tmap[128];   // CUtensorMap of the arena for the MQA/GQA kernel
     bool kv_tmap_ok = false;
+    alignas(64) unsigned char mla_tmap[128];  // CUtensorMap of the arena for the MLA kernel
+    bool mla_tmap_ok = false;
 
     // counters
     uint64_t n_launches = 0, n_plan_builds = 0, n_h2d_bytes = 0;
@@ -159,7 +161,16 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         // smallest tile length L (pages) for which the batch yields at most target_tiles tiles, so
         // that with waves = w every persistent CTA gets exactly w near-equal tiles (one tile more
         // on a few CTAs would cost a whole extra tile time at the end)
-        const int64_t target_tiles = std::max<int64_t>(1, (int64_t)n_ctas * pool->opt_waves_x16 / 16);
+        // the tcgen05 MLA kernel runs every tile as two work items (value halves)
+        bool mla_fast = k == CP_KIND_MLA && pool->opt_kernel == 0 && mla_fast_supported(P, pool->page_bytes);
+        if (mla_fast)
+            for (int b = 0; b < n; ++b) {
+                const cp_model_cfg &m = pool->models[pool->reqs[ids[b]].model];
+                if (m.kind == CP_KIND_MLA && !(m.head_dim_qk == 576 && m.head_dim_v == 512 && m.n_q_heads <= 128))
+                    mla_fast = false;
+            }
+        const int64_t target_tiles =
+            std::max<int64_t>(1, (int64_t)n_ctas * pool->opt_waves_x16 / 16 / (mla_fast ? 2 : 1));
         auto tiles_for = [&](int64_t len) {
             int64_t t = 0;
             for (int b = 0; b < n; ++b) {
@@ -182,7 +193,7 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             }
             L = lo;
         }
-        kp.all_fast = true;
+        kp.all_fast = k == CP_KIND_KV ? true : mla_fast;
         for (int b = 0; b < n; ++b) {
             const Request &r = pool->reqs[ids[b]];
             const cp_model_cfg &m = pool->models[r.model];
@@ -237,7 +248,7 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
                             cu.split_stride = m.head_dim_v;
                             cu.n_splits = ns;
                             cu.zl_log2 = zl;
-                            cu.want = ns * (k == CP_KIND_KV ? mtp : 1);
+                            cu.want = ns * (k == CP_KIND_KV ? mtp : 8);   // MLA: 4 softmax warps x 2 value halves
                             cu.group = gi;
                             kp.cunits.push_back(cu);
                         }
@@ -328,6 +339,11 @@ cp_status ensure_device(cp_pool *pool)
         const uint64_t rows = (uint64_t)pool->num_pages * (pool->page_bytes / 256);
         pool->kv_tmap_ok = rows < (1ull << 32) &&
                            make_arena_tensor_map(pool->kv_tmap, pool->arena, rows, 128, 64, pool->P);
+    }
+    pool->mla_tmap_ok = false;
+    if (mla_fast_supported((int)pool->P, pool->page_bytes)) {
+        const uint64_t rows = (uint64_t)pool->num_pages * (pool->page_bytes / 1152);
+        pool->mla_tmap_ok = rows < (1ull << 32) && make_mla_tensor_map(pool->mla_tmap, pool->arena, rows);
     }
     pool->n_sm = sms;
     pool->dev_ready = true;
@@ -690,6 +706,10 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
             prm.n_combine_units = (int)kp.cunits.size();
             e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256),
                                  std::min(n_ctas, pool->n_sm), s);
+        } else if (k == CP_KIND_MLA && pool->opt_kernel == 0 && kp.all_fast && pool->mla_tmap_ok) {
+            prm.n_combine_units = (int)kp.cunits.size();
+            e = launch_decode_mla(prm, pool->mla_tmap, (int)(pool->page_bytes / 1152),
+                                  std::min(n_ctas, pool->n_sm), s);
         } else
             e = launch_decode_generic(prm, kp.max_dk, kp.max_dv, k == CP_KIND_KV, kp.max_splits,
                                       std::min(n_ctas, pool->n_sm), s);
