@@ -4,9 +4,10 @@
 //
 // 128 query heads against one shared latent row per token is a real dense contraction
 // (241 flop per KV byte), so here -- and only here -- the 5th-generation tensor cores are used:
-//     S[128 x 16]   = Q[128 x 576] . C_slice^T      36 x tcgen05.mma M128 N16  K16 (A, B K-major)
-//     O[128 x 256] += P[128 x 16]  . C_slice[:, half]  1 x tcgen05.mma M128 N256 K16 (B MN-major)
-// per 16-token slice of a page.  TMEM holds 512 fp32 columns per SM; O[128 x 512] alone would
+//     S[128 x 32]   = Q[128 x 576] . C_slice^T      36 x tcgen05.mma M128 N32  K16 (A, B K-major)
+//     O[128 x 256] += P[128 x 32]  . C_slice[:, half]  2 x tcgen05.mma M128 N256 K16 (B MN-major)
+// per 32-token slice of a page (measured: an SS-mode MMA costs ~64 cycles of shared-memory operand
+// reads for the 4 KB A tile whatever N is, so the slice is as long as shared memory allows).  TMEM holds 512 fp32 columns per SM; O[128 x 512] alone would
 // fill it, so one work item is (tile, value half): it accumulates 256 of the 512 value columns
 // (TMEM columns 0..255) and keeps two S buffers (columns 256.., 288..).  The two halves of a
 // tile are adjacent work items, popped by different CTAs at about the same time, so the second
@@ -14,8 +15,8 @@
 //
 // Warp roles (192 threads, 1 CTA/SM):
 //   warp 0      producer: pops work items, translates logical pages through the page table
-//               (step a2) and streams 16-token slices into a 4-stage ring with one 3-D TMA
-//               box each (9 swizzled [16 x 64] tiles), mbarrier complete_tx.
+//               (step a2) and streams 32-token slices into a 2-stage ring with one 3-D TMA
+//               box each (9 swizzled [32 x 64] tiles), mbarrier complete_tx.
 //   warp 1      MMA issuer (one elected lane): S_{i+1} is issued before P_i V_i so the tensor
 //               pipe computes the next scores while the softmax warps work on the current ones.
 //   warps 2..5  softmax: thread = one query head = one TMEM lane, so the row maximum and row
@@ -35,36 +36,53 @@
 
 namespace cp {
 
+#ifdef CP_KV_PROBE_TIMING        /* probe builds only */
+__device__ unsigned long long cp_mla_probe_ts[160 * 16];
+__device__ __forceinline__ void mla_stamp(int k)
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    cp_mla_probe_ts[blockIdx.x * 16 + k] = t;
+}
+#define MLA_STAMP(k, cond) do { if (cond) mla_stamp(k); } while (0)
+extern "C" int cp_mla_probe_read(unsigned long long *out_host)
+{
+    return (int)cudaMemcpyFromSymbol(out_host, cp_mla_probe_ts, sizeof(cp_mla_probe_ts));
+}
+#else
+#define MLA_STAMP(k, cond) do { } while (0)
+#endif
+
 constexpr int MLA_DK = 576;                         // latent row width (512 latent + 64 rope)
 constexpr int MLA_DV = 512;                         // value = first 512 entries of the row
 constexpr int MLA_HALF = 256;                       // value columns per work item
 constexpr int MLA_M = 128;                          // query heads = MMA M = TMEM lanes
-constexpr int MLA_TS = 16;                          // tokens per slice = MMA N of the score MMA
+constexpr int MLA_TS = 32;                          // tokens per slice = MMA N of the score MMA
 constexpr int MLA_KB = MLA_DK / 64;                 // 9 column blocks of 64 (128 B, one swizzle row)
-constexpr int MLA_STAGES = 4;
-constexpr int MLA_STAGE_BYTES = MLA_TS * MLA_DK * 2;        // 18432
-constexpr int MLA_BLK_BYTES = MLA_TS * 128;                 // one [16 x 64] swizzled tile: 2048
+constexpr int MLA_STAGES = 2;
+constexpr int MLA_STAGE_BYTES = MLA_TS * MLA_DK * 2;        // 36864
+constexpr int MLA_BLK_BYTES = MLA_TS * 128;                 // one [32 x 64] swizzled tile: 4096
 constexpr int MLA_Q_BYTES = MLA_M * MLA_DK * 2;             // 147456: 9 blocks of [128 x 64]
 constexpr int MLA_QBLK_BYTES = MLA_M * 128;                 // 16384
-constexpr int MLA_P_BYTES = MLA_M * MLA_TS * 2;             // 4096 per P buffer
+constexpr int MLA_P_BYTES = MLA_M * MLA_TS * 2;             // 8192, one P buffer
 constexpr int MLA_THREADS = 192;
 constexpr int MLA_TQ = 2;                           // work-item queue depth
 constexpr int MLA_SMEM_Q = 0;
 constexpr int MLA_SMEM_STAGE = MLA_Q_BYTES;
 constexpr int MLA_SMEM_P = MLA_SMEM_STAGE + MLA_STAGES * MLA_STAGE_BYTES;
-constexpr int MLA_SMEM_MISC = MLA_SMEM_P + 2 * MLA_P_BYTES;         // barriers, queue, tmem address
+constexpr int MLA_SMEM_MISC = MLA_SMEM_P + MLA_P_BYTES;         // barriers, queue, tmem address
 constexpr int MLA_SMEM_BYTES = MLA_SMEM_MISC + 1024;
 static_assert(MLA_SMEM_BYTES <= 232448, "MLA kernel exceeds the 227 KB shared-memory limit");
 constexpr uint32_t MLA_TMEM_COLS = 512;
-constexpr uint32_t MLA_TMEM_S0 = 256, MLA_TMEM_S1 = 288;
+constexpr uint32_t MLA_TMEM_S0 = 256, MLA_TMEM_S1 = 288;       // two score buffers of MLA_TS columns
 constexpr float MLA_LAZY_LOG2 = 8.0f;
 
 // What the producer hands to the other warps for one work item.
 struct MlaDesc {
     int32_t item;            // work index; < 0: no more work
     int32_t group_idx;
-    int32_t n_slices;        // 16-token slices of the tile
-    int32_t valid_last;      // valid tokens of the last slice (1..16)
+    int32_t n_slices;        // MLA_TS-token slices of the tile
+    int32_t valid_last;      // valid tokens of the last slice (1..MLA_TS)
     int32_t split, n_splits;
     int32_t half;            // value half (0: columns 0..255, 1: 256..511)
     int32_t n_heads;         // Hq
@@ -77,7 +95,7 @@ struct MlaDesc {
 struct MlaMisc {
     uint64_t full[MLA_STAGES], empty[MLA_STAGES];       // slice ring: TMA -> MMA, MMA -> TMA
     uint64_t s_full[2], s_empty[2];                     // score buffers in TMEM: MMA -> softmax -> MMA
-    uint64_t p_full[2], p_done[2];                      // P buffers in smem: softmax -> MMA; MMA done reading
+    uint64_t p_full, p_done;                            // P buffer in smem: softmax -> MMA; MMA done reading
     uint64_t q_full;                                    // query block staged (softmax warps -> MMA)
     uint64_t tq_full[MLA_TQ], tq_empty[MLA_TQ];         // work-item queue
     MlaDesc tq[MLA_TQ];
@@ -102,8 +120,8 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
         for (int i = 0; i < MLA_STAGES; ++i) { mbar_init(smem_u32(&mi->full[i]), 1); mbar_init(smem_u32(&mi->empty[i]), 1); }
         for (int i = 0; i < 2; ++i) {
             mbar_init(smem_u32(&mi->s_full[i]), 1); mbar_init(smem_u32(&mi->s_empty[i]), 4);
-            mbar_init(smem_u32(&mi->p_full[i]), 4); mbar_init(smem_u32(&mi->p_done[i]), 1);
         }
+        mbar_init(smem_u32(&mi->p_full), 4); mbar_init(smem_u32(&mi->p_done), 1);
         mbar_init(smem_u32(&mi->q_full), 4);
         for (int i = 0; i < MLA_TQ; ++i) { mbar_init(smem_u32(&mi->tq_full[i]), 1); mbar_init(smem_u32(&mi->tq_empty[i]), 5); }
         asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap)) : "memory");
@@ -179,7 +197,7 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                         const uint32_t fb = smem_u32(&mi->full[slot]);
                         mbar_arrive_expect_tx(fb, MLA_STAGE_BYTES);
                         const int row = my * rows_per_page + ((s0 + j) % spp) * MLA_TS;
-                        // one 3-D box {64 columns, 16 rows, 9 column blocks} -> 9 swizzled [16 x 64] tiles
+                        // one 3-D box {64 columns, 32 rows, 9 column blocks} -> 9 swizzled [32 x 64] tiles
                         tma_load_3d(st_base + slot * MLA_STAGE_BYTES, &tmap, 0, row, 0, fb, policy);
                     }
                     ++gs;
@@ -205,8 +223,11 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 if (i < n) {
                     // ---- S_i = Q C_i^T into score buffer (g & 1)
                     const uint32_t g = gs + (uint32_t)i, slot = g % MLA_STAGES, b = g & 1;
+                    MLA_STAMP(0, lane == 0 && i == 50);
                     mbar_wait(smem_u32(&mi->full[slot]), (g / MLA_STAGES) & 1);
+                    MLA_STAMP(1, lane == 0 && i == 50);
                     mbar_wait(smem_u32(&mi->s_empty[b]), ((g >> 1) & 1) ^ 1);
+                    MLA_STAMP(2, lane == 0 && i == 50);
                     tc_fence_after();
                     if (lane == 0) {
                         const uint32_t c0 = st_base + slot * MLA_STAGE_BYTES;
@@ -223,23 +244,30 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                         umma_commit(smem_u32(&mi->s_full[b]));
                     }
                     __syncwarp();
+                    MLA_STAMP(3, lane == 0 && i == 50);
                 }
                 if (i >= 1) {
                     // ---- O += P_{i-1} V_{i-1} (value half of the work item)
-                    const uint32_t g = gs + (uint32_t)i - 1, slot = g % MLA_STAGES, b = g & 1;
-                    mbar_wait(smem_u32(&mi->p_full[b]), (g >> 1) & 1);
+                    const uint32_t g = gs + (uint32_t)i - 1, slot = g % MLA_STAGES;
+                    mbar_wait(smem_u32(&mi->p_full), g & 1);
+                    MLA_STAMP(4, lane == 0 && i == 50);
                     tc_fence_after();
                     if (lane == 0) {
-                        // P: no swizzle, core matrices of 8 rows x 16 B; K halves 2048 B apart, 8-row groups 128 B apart
-                        const uint64_t ad = umma_smem_desc(p_base + b * MLA_P_BYTES, 2048, 128, 0);
-                        // V: MN-major, 128-byte swizzle: 64-column blocks 2048 B apart, 8-token groups 1024 B apart
-                        const uint64_t bd = umma_smem_desc(st_base + slot * MLA_STAGE_BYTES + d.half * 4 * MLA_BLK_BYTES,
-                                                           MLA_BLK_BYTES, 1024, 2);
-                        umma_bf16_ss(tmem, ad, bd, IDESC_PV, i > 1);
+#pragma unroll
+                        for (int kk = 0; kk < MLA_TS / 16; ++kk) {    // K = 16 tokens per MMA
+                            // P: no swizzle, core matrices of 8 rows x 16 B: 8-token chunks 2048 B apart, 8-row groups 128 B apart
+                            const uint64_t ad = umma_smem_desc(p_base + kk * 4096, 2048, 128, 0);
+                            // V: MN-major, 128-byte swizzle: 64-column blocks MLA_BLK_BYTES apart, 8-token groups 1024 B apart
+                            const uint64_t bd = umma_smem_desc(st_base + slot * MLA_STAGE_BYTES + d.half * 4 * MLA_BLK_BYTES + kk * 2048,
+                                                               MLA_BLK_BYTES, 1024, 2);
+                            umma_bf16_ss(tmem, ad, bd, IDESC_PV, (i > 1) || (kk > 0));
+                        }
                         umma_commit(smem_u32(&mi->empty[slot]));      // slice consumed: the stage is free
-                        umma_commit(smem_u32(&mi->p_done[b]));        // P buffer free, O updated
+                        umma_commit(smem_u32(&mi->p_done));           // P buffer free, O updated
                     }
                     __syncwarp();
+                    MLA_STAMP(5, lane == 0 && i == 50);
+                    MLA_STAMP(6, lane == 0 && i == 51);
                 }
             }
             gs += (uint32_t)n;
@@ -280,31 +308,49 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             const int n = d.n_slices;
             for (int i = 0; i < n; ++i) {
                 const uint32_t g = gs + (uint32_t)i, b = g & 1, k = g >> 1;
+                MLA_STAMP(8, tid == 64 && i == 50);
                 mbar_wait(smem_u32(&mi->s_full[b]), k & 1);
+                MLA_STAMP(9, tid == 64 && i == 50);
                 tc_fence_after();
-                uint32_t sr[16];
-                tmem_ld16(tl + (b ? MLA_TMEM_S1 : MLA_TMEM_S0), sr);
+                uint32_t sr[MLA_TS];
+#pragma unroll
+                for (int c = 0; c < MLA_TS; c += 16)
+                    tmem_ld16(tl + (b ? MLA_TMEM_S1 : MLA_TMEM_S0) + c, *reinterpret_cast<uint32_t (*)[16]>(&sr[c]));
                 tmem_wait_ld();
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&mi->s_empty[b]));       // score buffer free
+                MLA_STAMP(10, tid == 64 && i == 50);
                 const int valid = (i == n - 1) ? d.valid_last : MLA_TS;
-                float s[16];
                 float mx = -INFINITY;
 #pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    s[j] = j < valid ? __uint_as_float(sr[j]) * d.scale_log2 : -INFINITY;
-                    mx = fmaxf(mx, s[j]);
+                for (int j = 0; j < MLA_TS; ++j) {
+                    const float v = j < valid ? __uint_as_float(sr[j]) * d.scale_log2 : -INFINITY;
+                    sr[j] = __float_as_uint(v);
+                    mx = fmaxf(mx, v);
                 }
                 // lazy reference update (see the MQA/GQA kernel): m only moves when it must
                 const float m_new = (mx > m_run + MLA_LAZY_LOG2) ? mx : m_run;
                 const bool need = (m_new != m_run) && i > 0;     // at i == 0 the MMA overwrites O
+                const float a_resc = ex2_ftz(m_run - m_new);      // 1 when the reference stays
+                if (m_new != m_run) { l_run *= a_resc; m_run = m_new; }
+                uint32_t pw[MLA_TS / 2];
+                float sum = 0.f;
+#pragma unroll
+                for (int j = 0; j < MLA_TS / 2; ++j) {
+                    const float p0 = ex2_ftz(__uint_as_float(sr[2 * j]) - m_run), p1 = ex2_ftz(__uint_as_float(sr[2 * j + 1]) - m_run);
+                    sum += p0 + p1;
+                    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pw[j]) : "f"(p1), "f"(p0));
+                }
+                l_run += sum;
+                // the P buffer (and O, if it must be rescaled) is free once P_{i-1} V_{i-1} has completed
+                MLA_STAMP(11, tid == 64 && i == 50);
+                mbar_wait(smem_u32(&mi->p_done), (g & 1) ^ 1);
+                MLA_STAMP(12, tid == 64 && i == 50);
                 if (__any_sync(0xffffffffu, need)) {
-                    // rescale this warp's O rows in TMEM; P_{i-1} V_{i-1} must have completed
-                    const uint32_t gp = g - 1;
-                    mbar_wait(smem_u32(&mi->p_done[gp & 1]), (gp >> 1) & 1);
+                    // rescale this warp's O rows in TMEM
                     tc_fence_after();
-                    const float a = need ? ex2_ftz(m_run - m_new) : 1.f;
+                    const float a = need ? a_resc : 1.f;
                     for (int c = 0; c < MLA_HALF; c += 16) {
                         uint32_t o[16];
                         tmem_ld16(tl + c, o);
@@ -315,21 +361,11 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                     }
                     tmem_wait_st();
                 }
-                if (m_new != m_run) { l_run *= ex2_ftz(m_run - m_new); m_run = m_new; }
-                uint32_t pw[8];
-                float sum = 0.f;
+                // P[row][token] as 8-token chunks: chunk c of row r at c * 2048 + r * 16
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const float p0 = ex2_ftz(s[2 * j] - m_run), p1 = ex2_ftz(s[2 * j + 1] - m_run);
-                    sum += p0 + p1;
-                    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pw[j]) : "f"(p1), "f"(p0));
-                }
-                l_run += sum;
-                // P buffer b: the MMA that read its previous contents must be done
-                mbar_wait(smem_u32(&mi->p_done[b]), (k & 1) ^ 1);
-                const uint32_t pa = p_base + b * MLA_P_BYTES + row * 16;
-                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(pa), "r"(pw[0]), "r"(pw[1]), "r"(pw[2]), "r"(pw[3]) : "memory");
-                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(pa + 2048), "r"(pw[4]), "r"(pw[5]), "r"(pw[6]), "r"(pw[7]) : "memory");
+                for (int c = 0; c < MLA_TS / 8; ++c)
+                    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p_base + c * 2048 + row * 16), "r"(pw[4 * c]),
+                                 "r"(pw[4 * c + 1]), "r"(pw[4 * c + 2]), "r"(pw[4 * c + 3]) : "memory");
                 if (valid < MLA_TS) {
                     // dead slots of the request's last slice may hold NaN: zero their value rows (0 * NaN);
                     // warp q4 clears column block half*4 + q4 of the stage
@@ -342,14 +378,16 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 fence_proxy_async();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&mi->p_full[b]));
+                if (lane == 0) mbar_arrive(smem_u32(&mi->p_full));
+                MLA_STAMP(13, tid == 64 && i == 50);
+                MLA_STAMP(14, tid == 64 && i == 51);
             }
             gs += (uint32_t)n;
 
             // ---- end of tile: O (this value half) from TMEM, publish
             {
                 const uint32_t gl = gs - 1;
-                mbar_wait(smem_u32(&mi->p_done[gl & 1]), (gl >> 1) & 1);
+                mbar_wait(smem_u32(&mi->p_done), gl & 1);
                 tc_fence_after();
                 const bool final_out = d.n_splits == 1;
                 const float inv = final_out ? 1.f / l_run : 1.f;
@@ -401,7 +439,7 @@ bool mla_fast_supported(int page_tokens, uint32_t page_bytes)
 }
 
 // 3-D view of the arena: {64 columns, rows of 576 bf16 (1152 B apart), 9 column blocks (128 B apart)};
-// one box = a 16-token slice as 9 consecutive 128-byte-swizzled [16 x 64] tiles in shared memory.
+// one box = a 32-token slice as 9 consecutive 128-byte-swizzled [32 x 64] tiles in shared memory.
 bool make_mla_tensor_map(void *out_map, const void *arena, uint64_t total_rows)
 {
     typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
