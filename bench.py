@@ -4,7 +4,8 @@
 A "step" is one pass of the whole hot path (translation + split-KV partial attention + LSE
 combine, all inside one persistent launch) over one synthetic batch: one
 cp_decode_attention call.  Default workload: BASELINE.json configs[1], the shared pool of
-4 cold GQA models (344 MB of KV per step).  L2 is flushed between steps.
+4 cold GQA models (344 MB of KV per step, larger than the 126 MB L2: no flush needed; smaller
+configs flush L2 with a 256 MB write between steps).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
 
@@ -27,6 +28,11 @@ if ROOT not in sys.path:
 
 import numpy as np
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the decode kernel, from the committed
+# `ncu --set full` captures (profiles/r1_ncu_full_cfg{2,4}_kv_v3.txt, r1_ncu_full_cfg3_mla_v1.txt)
+NCU_TRAFFIC_BYTES = {2: 344.64e6 + 7.86e6, 3: 285.27e6 + 7.97e6, 4: 134.33e6 + 6.31e6}
+NCU_TENSOR_PIPE_PCT = {3: 13.4}       # sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active
+
 METRIC = "paged decode-attention KV GB/s"
 UNIT = "GB/s"
 L2_BYTES = 126 * 1024 * 1024
@@ -46,8 +52,8 @@ def workload_desc(w, k):
     return {"workload": "cfg%d:%s" % (k, w.name), "requests": len(w.requests),
             "tokens": w.total_tokens(), "page_tokens": w.page_tokens,
             "kv_bytes_per_step": w.algorithmic_bytes(), "flops_per_step": w.flops(),
-            "l2": "L2 flushed between steps (256 MB write, outside the per-step CUDA events); "
-                  "inputs %.0f MB vs L2 126 MB" % (w.algorithmic_bytes() / 1e6)}
+            "l2": ("inputs %.0f MB > L2 126 MB, no flush" % (w.algorithmic_bytes() / 1e6))
+            if w.algorithmic_bytes() > L2_BYTES else "L2 flushed between steps (256 MB write, outside the per-step events)"}
 
 
 class ClockSampler:
@@ -62,7 +68,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                 "--format=csv,noheader,nounits", "-lms", "50"],
+                 "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -199,9 +205,15 @@ def main():
         dw.pool.set_option(cp.CP_OPT_MIN_TILE_PAGES, args.min_tile_pages)
     dw.ensure_workspace()
     abytes = w.algorithmic_bytes()
-    # Always flush: it defeats L2 residency of the smaller configs and keeps the GPU busy while
-    # the host enqueues the next step, so the per-step events never include host launch latency.
-    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    # Inputs smaller than L2 are flushed out of it between steps (256 MB write).  Before every
+    # timed step a short device-side spin (no memory traffic) keeps the GPU busy while the host
+    # enqueues the step, so the per-step events never include host launch latency.
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev) if abytes <= L2_BYTES else None
+
+    def spacer(i):
+        if flush is not None:
+            flush.fill_(i & 0xFF)
+        torch.cuda._sleep(100000)       # ~50 us at 1.9 GHz
 
     def barrier():
         if world > 1:
@@ -220,8 +232,7 @@ def main():
     start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     start.record()
     for i in range(args.steps):
-        if flush is not None:
-            flush.fill_(i & 0xFF)
+        spacer(i)
         ev[2 * i].record()
         dw.decode()
         ev[2 * i + 1].record()
@@ -230,7 +241,7 @@ def main():
     c1 = dw.pool.counters()
     kern_ms = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(args.steps)]
     region_ms = start.elapsed_time(stop)
-    step_ms = float(np.sum(kern_ms)) / args.steps if flush is not None else region_ms / args.steps
+    step_ms = float(np.sum(kern_ms)) / args.steps     # one launch per step: step = the event-bracketed launch
     t = torch.tensor([step_ms], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -249,7 +260,8 @@ def main():
     barrier()
     e2e_s = 0.0
     for i in range(e2e_steps):
-        flush.fill_(i & 0xFF)
+        if flush is not None:
+            flush.fill_(i & 0xFF)
         torch.cuda.synchronize()
         t0 = time.perf_counter()       # the call copies q H2D, runs the step, copies O/LSE D2H and syncs
         dw.pool.decode_attention_host(dw.ids, q_host, o_host, l_host, ws, need, dw.stream())
@@ -273,14 +285,15 @@ def main():
     achieved = abytes / (kern_avg_ms * 1e-3) / 1e9
     mla = any(m.kind == 1 for m in w.models)
     roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-            "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+            "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(k), "peak_source": peaks["source"],
             "kernel_us": 1e3 * kern_avg_ms, "kernel_us_p10_p50_p90":
                 [float(x) * 1e3 for x in np.percentile(kern_ms, [10, 50, 90])],
             "frac_of_nominal_8000": achieved / 8000.0}
     if mla:
         tf = w.flops() / (kern_avg_ms * 1e-3) / 1e12
         roof["tensor"] = {"achieved_tflops": tf, "peak_burst": peaks["bf16_tflops"],
-                          "frac_burst": tf / peaks["bf16_tflops"]}
+                          "frac_burst": tf / peaks["bf16_tflops"],
+                          "tensor_pipe_pct_ncu": NCU_TENSOR_PIPE_PCT.get(k)}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": step_ms, "us_per_step": 1e3 * step_ms,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16 in, fp32 accumulate",
