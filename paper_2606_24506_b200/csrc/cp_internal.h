@@ -61,6 +61,18 @@ struct Tile {
     int32_t page_end;
 };
 
+// Everything a producer warp needs to start a tile, in one 80-byte record (one level of loads
+// after the pop instead of tile -> group -> model): same order as Tile[].
+struct TileRec {
+    int32_t group, req, kv_head, n_kv_heads;
+    int32_t page_begin, n_pages, split, n_splits;
+    int32_t gsize, n_q_heads;
+    float scale_log2;
+    int32_t pad;
+    int64_t q_off, out_off, lse_off, part_off;
+};
+static_assert(sizeof(TileRec) == 80, "TileRec is loaded as five 16-byte vectors");
+
 // One unit of the LSE combine: one query head of a split group.
 struct Combine {
     int32_t group;
@@ -94,6 +106,7 @@ struct DecodeParams {
     const DevModel *models;
     const Group *groups;
     const Tile *tiles;
+    const TileRec *tile_recs;      // [n_tiles], same order as tiles
     const Combine *combines;
     const CombineUnit *cunits;     // [n_combine_units] (tensor-core kernels)
     int32_t n_tiles;

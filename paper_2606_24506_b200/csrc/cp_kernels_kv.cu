@@ -286,45 +286,50 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
         uint32_t pc = 0;          // pages issued by this CTA (ring position)
         uint32_t qi = 0;          // work items pushed
         for (;;) {
+            // the first tile of a CTA is static (its block index): no atomic round trip at start-up
             int work = 0;
-            if (lane == 0) work = atomicAdd(p.work_counter, 1);
-            work = __shfl_sync(0xffffffffu, work, 0);
-            const int item = work < p.n_tiles ? work : -1;      // tiles only; combine units are popped by the consumer warps
-            Tile tile = Tile{0, 0, 0, 0};
-            Group g;
-            g.req = 0; g.model = 0; g.kv_head = 0; g.n_splits = 1; g.n_pages = 0; g.batch_index = 0;
-            g.q_off = g.out_off = g.lse_off = g.part_off = 0;
-            int hkv = 1, mt = 1, gsize = 1, ctx = 0;
-            float scale_log2 = 0.f;
-            const bool is_tile = item >= 0;
-            if (is_tile) {
-                tile = p.tiles[item];
-                g = p.groups[tile.group];
-                const DevModel m = p.models[g.model];
-                hkv = m.n_kv_heads; gsize = m.group; mt = kv_mtiles(m.group); scale_log2 = m.scale_log2;
-                ctx = __ldg(p.req_ctx + g.req);
+            if (qi == 0) work = blockIdx.x;
+            else {
+                if (lane == 0) work = atomicAdd(p.work_counter, 1) + (int)gridDim.x;
+                work = __shfl_sync(0xffffffffu, work, 0);
+            }
+            const int item = work < p.n_tiles ? work : -1;      // tiles only; combine units are static
+            TileRec r;
+            int ctx = 0, mt = 1;
+            if (item >= 0) {
+                const uint4 *src = reinterpret_cast<const uint4 *>(p.tile_recs + item);
+                uint4 *dst = reinterpret_cast<uint4 *>(&r);
+#pragma unroll
+                for (int i = 0; i < 5; ++i) dst[i] = __ldg(src + i);
+                ctx = __ldg(p.req_ctx + r.req);
+                mt = kv_mtiles(r.gsize);
+            } else {
+                r.group = 0; r.req = 0; r.kv_head = 0; r.n_kv_heads = 1; r.page_begin = 0; r.n_pages = 0;
+                r.split = 0; r.n_splits = 1; r.gsize = 1; r.n_q_heads = 1; r.scale_log2 = 0.f;
+                r.q_off = r.out_off = r.lse_off = r.part_off = 0;
             }
             // push the descriptor to the tile queue
             const uint32_t qs = qi % KV_TQ;
             mbar_wait(smem_u32(tqe_b + qs), ((qi / KV_TQ) & 1) ^ 1);
             if (lane == 0) {
                 TileDesc d;
-                d.item = item; d.group_idx = tile.group; d.page_begin = tile.page_begin;
-                d.npg = tile.page_end - tile.page_begin; d.split = tile.split; d.n_splits = g.n_splits;
-                d.ctx = ctx; d.gsize = gsize; d.mt = mt; d.scale_log2 = scale_log2;
-                d.q_off = g.q_off; d.out_off = g.out_off; d.lse_off = g.lse_off; d.part_off = g.part_off;
+                d.item = item; d.group_idx = r.group; d.page_begin = r.page_begin;
+                d.npg = r.n_pages; d.split = r.split; d.n_splits = r.n_splits;
+                d.ctx = ctx; d.gsize = r.gsize; d.mt = mt; d.scale_log2 = r.scale_log2;
+                d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
                 tq[qs] = d;
                 mbar_arrive(smem_u32(tqf_b + qs));     // release: consumers acquire via try_wait
             }
             ++qi;
             if (item < 0) break;
 
-            const int32_t *pt = p.page_table + (int64_t)g.req * p.max_ppr + g.kv_head;
-            const int npg = tile.page_end - tile.page_begin;
+            const int32_t *pt = p.page_table + (int64_t)r.req * p.max_ppr + r.kv_head;
+            const int npg = r.n_pages;
+            const int hkv = r.n_kv_heads;
             for (int j0 = 0; j0 < npg; j0 += 32) {
                 // translate up to 32 logical pages at once (step a2: one page-table entry per lane)
                 int32_t pid = 0;
-                if (j0 + lane < npg) pid = __ldg(pt + (int64_t)(tile.page_begin + j0 + lane) * hkv);
+                if (j0 + lane < npg) pid = __ldg(pt + (int64_t)(r.page_begin + j0 + lane) * hkv);
                 const int nj = min(32, npg - j0);
                 for (int j = 0; j < nj; ++j) {
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);

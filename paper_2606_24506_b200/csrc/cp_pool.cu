@@ -54,6 +54,7 @@ struct Request {
 struct KindPlan {
     std::vector<Group> groups;
     std::vector<Tile> tiles;
+    std::vector<TileRec> tile_recs;
     std::vector<Combine> combines;       // CTA-sized combine units (generic kernel)
     std::vector<CombineUnit> cunits;     // warp-sized combine units (tensor-core kernels)
     int max_splits = 1;
@@ -61,7 +62,7 @@ struct KindPlan {
     int max_group = 0;
     bool all_fast = false;           // every group of this kind runs on the tensor-core kernel
     bool uploaded = false;
-    DevBuf d_groups, d_tiles, d_combines, d_cunits, d_counters;   // counters: [32] scheduler + [n_groups * kCounterStride]
+    DevBuf d_groups, d_tiles, d_tile_recs, d_combines, d_cunits, d_counters;   // counters: [32] scheduler + [n_groups * kCounterStride]
 };
 
 }  // namespace
@@ -260,6 +261,19 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         });
         // combine units in the order in which their groups' last tiles are popped, so a CTA
         // that runs out of tiles first combines the groups that finish first
+        kp.tile_recs.resize(kp.tiles.size());
+        for (size_t i = 0; i < kp.tiles.size(); ++i) {
+            const Tile &t = kp.tiles[i];
+            const Group &gr = kp.groups[t.group];
+            const cp_model_cfg &m = pool->models[gr.model];
+            TileRec &r = kp.tile_recs[i];
+            std::memset(&r, 0, sizeof(r));
+            r.group = t.group; r.req = gr.req; r.kv_head = gr.kv_head; r.n_kv_heads = m.n_kv_heads;
+            r.page_begin = t.page_begin; r.n_pages = t.page_end - t.page_begin; r.split = t.split;
+            r.n_splits = gr.n_splits; r.gsize = m.n_q_heads / m.n_kv_heads; r.n_q_heads = m.n_q_heads;
+            r.scale_log2 = (float)((double)m.softmax_scale * 1.4426950408889634);
+            r.q_off = gr.q_off; r.out_off = gr.out_off; r.lse_off = gr.lse_off; r.part_off = gr.part_off;
+        }
         std::vector<int> last_pos(kp.groups.size(), 0);
         for (size_t i = 0; i < kp.tiles.size(); ++i) last_pos[kp.tiles[i].group] = (int)i;
         std::stable_sort(kp.combines.begin(), kp.combines.end(), [&](const Combine &a, const Combine &b) {
@@ -384,10 +398,12 @@ cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
     const size_t gb = kp.groups.size() * sizeof(Group), tb = kp.tiles.size() * sizeof(Tile);
     const size_t cb = kp.combines.size() * sizeof(Combine), nb = (32 + kp.groups.size() * (size_t)kCounterStride) * 4;
     const size_t ub = kp.cunits.size() * sizeof(CombineUnit);
+    const size_t rb = kp.tile_recs.size() * sizeof(TileRec);
     const bool counters_new = kp.d_counters.cap < nb;
     if (kp.d_groups.ensure(gb) != cudaSuccess || kp.d_tiles.ensure(tb) != cudaSuccess ||
         kp.d_combines.ensure(std::max(cb, (size_t)16)) != cudaSuccess ||
         kp.d_cunits.ensure(std::max(ub, (size_t)64)) != cudaSuccess ||
+        kp.d_tile_recs.ensure(std::max(rb, (size_t)80)) != cudaSuccess ||
         kp.d_counters.ensure(nb) != cudaSuccess) {
         cudaGetLastError();
         return CP_ERR_CUDA;
@@ -395,12 +411,13 @@ cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
     if (cudaMemcpyAsync(kp.d_groups.ptr, kp.groups.data(), gb, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
         cudaMemcpyAsync(kp.d_tiles.ptr, kp.tiles.data(), tb, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
         (cb && cudaMemcpyAsync(kp.d_combines.ptr, kp.combines.data(), cb, cudaMemcpyHostToDevice, stream) != cudaSuccess) ||
+        (rb && cudaMemcpyAsync(kp.d_tile_recs.ptr, kp.tile_recs.data(), rb, cudaMemcpyHostToDevice, stream) != cudaSuccess) ||
         (ub && cudaMemcpyAsync(kp.d_cunits.ptr, kp.cunits.data(), ub, cudaMemcpyHostToDevice, stream) != cudaSuccess))
         return CP_ERR_CUDA;
     // counters are zero between launches (the kernels reset them); zero a fresh buffer
     if (counters_new && cudaMemsetAsync(kp.d_counters.ptr, 0, kp.d_counters.cap, stream) != cudaSuccess)
         return CP_ERR_CUDA;
-    pool->n_h2d_bytes += gb + tb + cb + ub;
+    pool->n_h2d_bytes += gb + tb + cb + ub + rb;
     kp.uploaded = true;
     return CP_OK;
 }
@@ -469,7 +486,7 @@ cp_status cp_pool_free(cp_pool *pool)
     pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release();
     for (int k = 0; k < 2; ++k) {
         pool->plan[k].d_groups.release(); pool->plan[k].d_tiles.release();
-        pool->plan[k].d_combines.release(); pool->plan[k].d_cunits.release();
+        pool->plan[k].d_combines.release(); pool->plan[k].d_cunits.release(); pool->plan[k].d_tile_recs.release();
         pool->plan[k].d_counters.release();
     }
     delete pool;
@@ -690,6 +707,7 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.models = (const DevModel *)pool->d_models.ptr;
         prm.groups = (const Group *)kp.d_groups.ptr;
         prm.tiles = (const Tile *)kp.d_tiles.ptr;
+        prm.tile_recs = (const TileRec *)kp.d_tile_recs.ptr;
         prm.combines = (const Combine *)kp.d_combines.ptr;
         prm.cunits = (const CombineUnit *)kp.d_cunits.ptr;
         prm.n_tiles = (int)kp.tiles.size(); prm.n_combines = (int)kp.combines.size();
