@@ -166,14 +166,11 @@ __device__ inline void combine_unit(const DecodeParams &p, const Combine cu, int
 
 // ---------------------------------------------------------------------------------------
 // Warp-sized LSE combine unit (tensor-core kernels): ONE warp combines (128 >> zl) output
-// columns of one (group, head) described by a CombineUnit record; units are popped warp by
-// warp from a device counter, no CTA barrier.  The warp's lanes are (split lane z of
-// ZL = 2^zl) x (column quad cq of 32 / ZL): every lane fetches all its (<= 16) partial
-// vectors and (m, l) pairs in ONE batch of independent loads, so a unit costs two L2 round
-// trips (descriptor, data) whatever the split count.  Same arithmetic as combine_unit; all
-// sums run in a fixed order (k ascending per lane, then a fixed shuffle tree) => deterministic.
-// wsm: this warp's shared-memory scratch, >= n_splits floats.  n_splits <= kMaxSplits = 16 * 32
-// and n_splits <= 16 * ZL (the planner picks zl accordingly).
+// columns of one (group, head) described by a CombineUnit record; units are assigned statically
+// to the grid's warps, no CTA barrier.  The warp's lanes are (split lane z of ZL = 2^zl) x
+// (column quad cq of 32 / ZL).  Same arithmetic as combine_unit; all sums run in a fixed order
+// (s ascending per lane, then a fixed shuffle tree) => deterministic.
+// wsm: this warp's shared-memory scratch, >= n_splits floats (n_splits <= kMaxSplits).
 // ---------------------------------------------------------------------------------------
 __device__ __forceinline__ float ex2_ftz(float x)     // 2^x; ex2(-inf) = 0
 {
@@ -207,12 +204,12 @@ static __device__ __noinline__ void combine_warp_unit(const DecodeParams &p, con
 
     // pass 1: M = max_s m_s (lane-strided, then a fixed tree)
     float M = -INFINITY;
-#pragma unroll 4
+#pragma unroll 8
     for (int s = lane; s < ns; s += 32) M = fmaxf(M, __ldcg(mlp + s).x);
     for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
     // pass 2: weights w_s = 2^(m_s - M) to shared memory, L = sum_s w_s l_s
     float L = 0.f;
-#pragma unroll 4
+#pragma unroll 8
     for (int s = lane; s < ns; s += 32) {
         const float2 ml = __ldcg(mlp + s);
         const float w = ex2_ftz(ml.x - M);
