@@ -59,10 +59,11 @@ constexpr int MLA_HALF = 256;                       // value columns per work it
 constexpr int MLA_M = 128;                          // query heads = MMA M = TMEM lanes
 constexpr int MLA_TS = 32;                          // tokens per slice = MMA N of the score MMA
 constexpr int MLA_KB = MLA_DK / 64;                 // 9 column blocks of 64 (128 B, one swizzle row)
-constexpr int MLA_STAGES = 2;
+constexpr int MLA_STAGES = 4;
 constexpr int MLA_STAGE_BYTES = MLA_TS * MLA_DK * 2;        // 36864
 constexpr int MLA_BLK_BYTES = MLA_TS * 128;                 // one [32 x 64] swizzled tile: 4096
-constexpr int MLA_Q_BYTES = MLA_M * MLA_DK * 2;             // 147456: 9 blocks of [128 x 64]
+constexpr int MLA_KB_TMEM = 5;                      // query column blocks 0..4 live in TMEM (A operand, TS mode)
+constexpr int MLA_Q_BYTES = (MLA_KB - MLA_KB_TMEM) * MLA_M * 128;   // 65536: blocks 5..8 of [128 x 64] in shared memory
 constexpr int MLA_QBLK_BYTES = MLA_M * 128;                 // 16384
 constexpr int MLA_P_BYTES = MLA_M * MLA_TS * 2;             // 8192, one P buffer
 constexpr int MLA_THREADS = 192;
@@ -75,6 +76,7 @@ constexpr int MLA_SMEM_BYTES = MLA_SMEM_MISC + 1024;
 static_assert(MLA_SMEM_BYTES <= 232448, "MLA kernel exceeds the 227 KB shared-memory limit");
 constexpr uint32_t MLA_TMEM_COLS = 512;
 constexpr uint32_t MLA_TMEM_S0 = 256, MLA_TMEM_S1 = 288;       // two score buffers of MLA_TS columns
+constexpr uint32_t MLA_TMEM_Q = 320;                           // 160 columns: Q[:, 0:320) as bf16 pairs
 constexpr float MLA_LAZY_LOG2 = 8.0f;
 
 // What the producer hands to the other warps for one work item.
@@ -236,9 +238,13 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                         for (int kb = 0; kb < MLA_KB; ++kb) {
 #pragma unroll
                             for (int j = 0; j < 4; ++j) {        // K = 16 per MMA: 32 bytes inside the swizzled row
-                                const uint64_t ad = umma_smem_desc(q_base + kb * MLA_QBLK_BYTES + j * 32, 16, 1024, 2);
                                 const uint64_t bd = umma_smem_desc(c0 + kb * MLA_BLK_BYTES + j * 32, 16, 1024, 2);
-                                umma_bf16_ss(dcol, ad, bd, IDESC_S, (kb | j) != 0);
+                                if (kb < MLA_KB_TMEM) {          // A from tensor memory: 8 columns per K = 16
+                                    umma_bf16_ts(dcol, tmem + MLA_TMEM_Q + kb * 32 + j * 8, bd, IDESC_S, (kb | j) != 0);
+                                } else {
+                                    const uint64_t ad = umma_smem_desc(q_base + (kb - MLA_KB_TMEM) * MLA_QBLK_BYTES + j * 32, 16, 1024, 2);
+                                    umma_bf16_ss(dcol, ad, bd, IDESC_S, 1);
+                                }
                             }
                         }
                         umma_commit(smem_u32(&mi->s_full[b]));
@@ -289,16 +295,39 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             if (d.item < 0) break;
 
             if (d.load_q) {
-                // stage the query block [128 x 576] bf16 as 9 K-major [128 x 64] tiles with the 128-byte
-                // swizzle the MMA descriptor expects (16-B chunk index ^ (row & 7)); rows >= Hq are zero
-                const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + d.q_off);
-                for (int id = st; id < MLA_M * (MLA_DK / 8); id += 128) {
-                    const int r = id / (MLA_DK / 8), ch = id % (MLA_DK / 8);
-                    uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                    if (r < d.n_heads) v = __ldg(qg + id);
-                    const uint32_t a = q_base + (ch >> 3) * MLA_QBLK_BYTES + r * 128 + (((ch & 7) ^ (r & 7)) << 4);
-                    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+                // stage the query block [128 x 576] bf16.  Column blocks 0..4 go to tensor memory (this
+                // thread's head = its TMEM lane; two bf16 per 32-bit column, memory order), where the
+                // score MMAs read them as the A operand without shared-memory traffic; blocks 5..8 go
+                // to shared memory as K-major [128 x 64] tiles with the 128-byte swizzle the MMA
+                // descriptor expects (16-B chunk index ^ (row & 7)).  Rows >= Hq are zero.
+                {
+                    const uint4 *qr = reinterpret_cast<const uint4 *>(p.q + d.q_off + (int64_t)row * MLA_DK);
+                    const bool live = row < d.n_heads;
+                    for (int c = 0; c < MLA_KB_TMEM * 32; c += 16) {      // 16 columns = 32 bf16 = 4 x 16 B
+                        uint32_t w[16];
+#pragma unroll
+                        for (int v4 = 0; v4 < 4; ++v4) {
+                            uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                            if (live) v = __ldg(qr + c / 4 + v4);
+                            w[4 * v4] = v.x; w[4 * v4 + 1] = v.y; w[4 * v4 + 2] = v.z; w[4 * v4 + 3] = v.w;
+                        }
+                        tmem_st16(tl + MLA_TMEM_Q + c, w);
+                    }
+                    tmem_wait_st();
                 }
+                {
+                    constexpr int CPR = (MLA_KB - MLA_KB_TMEM) * 8;      // 16-B chunks per row in shared memory
+                    const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + d.q_off);
+#pragma unroll 4
+                    for (int id = st; id < MLA_M * CPR; id += 128) {
+                        const int r = id / CPR, ch = id % CPR;
+                        uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                        if (r < d.n_heads) v = __ldg(qg + r * (MLA_DK / 8) + MLA_KB_TMEM * 8 + ch);
+                        const uint32_t a = q_base + (ch >> 3) * MLA_QBLK_BYTES + r * 128 + (((ch & 7) ^ (r & 7)) << 4);
+                        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+                    }
+                }
+                tc_fence_before();
                 fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&mi->q_full));
