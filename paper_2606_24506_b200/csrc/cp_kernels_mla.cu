@@ -231,7 +231,7 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                     mbar_wait(smem_u32(&mi->s_empty[b]), ((g >> 1) & 1) ^ 1);
                     MLA_STAMP(2, lane == 0 && i == 50);
                     tc_fence_after();
-                    if (lane == 0) {
+                    if (elect_one()) {
                         const uint32_t c0 = st_base + slot * MLA_STAGE_BYTES;
                         const uint32_t dcol = tmem + (b ? MLA_TMEM_S1 : MLA_TMEM_S0);
 #pragma unroll
@@ -258,7 +258,7 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                     mbar_wait(smem_u32(&mi->p_full), g & 1);
                     MLA_STAMP(4, lane == 0 && i == 50);
                     tc_fence_after();
-                    if (lane == 0) {
+                    if (elect_one()) {
 #pragma unroll
                         for (int kk = 0; kk < MLA_TS / 16; ++kk) {    // K = 16 tokens per MMA
                             // P: no swizzle, core matrices of 8 rows x 16 B: 8-token chunks 2048 B apart, 8-row groups 128 B apart
