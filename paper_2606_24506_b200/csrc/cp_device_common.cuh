@@ -221,7 +221,7 @@ static __device__ __noinline__ void combine_warp_unit(const DecodeParams &p, con
     KV_STAMP(10, threadIdx.x == 0);
     // pass 3: O = sum_s w_s O_s over this lane's splits z, z + ZL, ... (in order), then the tree
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll 4
+#pragma unroll 8
     for (int s = z; s < ns; s += ZL) {
         const float4 v = ld_cg_f4(src + s * ss);
         const float w = wsm[s];

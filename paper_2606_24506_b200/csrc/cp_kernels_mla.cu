@@ -37,12 +37,12 @@
 namespace cp {
 
 #ifdef CP_KV_PROBE_TIMING        /* probe builds only */
-__device__ unsigned long long cp_mla_probe_ts[160 * 16];
+__device__ unsigned long long cp_mla_probe_ts[160 * 32];
 __device__ __forceinline__ void mla_stamp(int k)
 {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    cp_mla_probe_ts[blockIdx.x * 16 + k] = t;
+    cp_mla_probe_ts[blockIdx.x * 32 + k] = t;
 }
 #define MLA_STAMP(k, cond) do { if (cond) mla_stamp(k); } while (0)
 extern "C" int cp_mla_probe_read(unsigned long long *out_host)
@@ -117,6 +117,7 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     const uint32_t q_base = smem_u32(smem + MLA_SMEM_Q);
     const uint32_t st_base = smem_u32(smem + MLA_SMEM_STAGE);
     const uint32_t p_base = smem_u32(smem + MLA_SMEM_P);
+    MLA_STAMP(16, tid == 64);
 
     if (tid == 0) {
         for (int i = 0; i < MLA_STAGES; ++i) { mbar_init(smem_u32(&mi->full[i]), 1); mbar_init(smem_u32(&mi->empty[i]), 1); }
@@ -293,6 +294,7 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             if (lane == 0) mbar_arrive(smem_u32(&mi->tq_empty[qs]));
             ++qi;
             if (d.item < 0) break;
+            MLA_STAMP(17, tid == 64 && qi == 1);
 
             if (d.load_q) {
                 // stage the query block [128 x 576] bf16.  Column blocks 0..4 go to tensor memory (this
@@ -303,22 +305,30 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 {
                     const uint4 *qr = reinterpret_cast<const uint4 *>(p.q + d.q_off + (int64_t)row * MLA_DK);
                     const bool live = row < d.n_heads;
-                    for (int c = 0; c < MLA_KB_TMEM * 32; c += 16) {      // 16 columns = 32 bf16 = 4 x 16 B
-                        uint32_t w[16];
+                    for (int c0 = 0; c0 < MLA_KB_TMEM * 32; c0 += 80) {   // batches of 5 x 16 columns: 20 loads in flight
+                        uint4 v[20];
 #pragma unroll
-                        for (int v4 = 0; v4 < 4; ++v4) {
-                            uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                            if (live) v = __ldg(qr + c / 4 + v4);
-                            w[4 * v4] = v.x; w[4 * v4 + 1] = v.y; w[4 * v4 + 2] = v.z; w[4 * v4 + 3] = v.w;
+                        for (int i = 0; i < 20; ++i) {
+                            v[i] = make_uint4(0u, 0u, 0u, 0u);
+                            if (live) v[i] = __ldg(qr + c0 / 4 + i);
                         }
-                        tmem_st16(tl + MLA_TMEM_Q + c, w);
+#pragma unroll
+                        for (int b5 = 0; b5 < 5; ++b5) {                  // 16 columns = 32 bf16 = 4 x 16 B
+                            uint32_t w[16];
+#pragma unroll
+                            for (int v4 = 0; v4 < 4; ++v4) {
+                                w[4 * v4] = v[4 * b5 + v4].x; w[4 * v4 + 1] = v[4 * b5 + v4].y;
+                                w[4 * v4 + 2] = v[4 * b5 + v4].z; w[4 * v4 + 3] = v[4 * b5 + v4].w;
+                            }
+                            tmem_st16(tl + MLA_TMEM_Q + c0 + b5 * 16, w);
+                        }
                     }
                     tmem_wait_st();
                 }
                 {
                     constexpr int CPR = (MLA_KB - MLA_KB_TMEM) * 8;      // 16-B chunks per row in shared memory
                     const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + d.q_off);
-#pragma unroll 4
+#pragma unroll 8
                     for (int id = st; id < MLA_M * CPR; id += 128) {
                         const int r = id / CPR, ch = id % CPR;
                         uint4 v = make_uint4(0u, 0u, 0u, 0u);
@@ -333,6 +343,7 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 if (lane == 0) mbar_arrive(smem_u32(&mi->q_full));
             }
 
+            MLA_STAMP(18, tid == 64 && qi == 1);
             float m_run = -INFINITY, l_run = 0.f;
             const int n = d.n_slices;
             for (int i = 0; i < n; ++i) {
@@ -410,6 +421,8 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 if (lane == 0) mbar_arrive(smem_u32(&mi->p_full));
                 MLA_STAMP(13, tid == 64 && i == 50);
                 MLA_STAMP(14, tid == 64 && i == 51);
+                MLA_STAMP(19, tid == 64 && i == 0);
+                MLA_STAMP(20, tid == 64 && i == n - 1);
             }
             gs += (uint32_t)n;
 
@@ -448,17 +461,20 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                     __syncwarp();
                     if (lane == 0) red_release_add(p.group_counters + (size_t)d.group_idx * kCounterStride, 1);
                 }
+                MLA_STAMP(21, tid == 64);
             }
         }
         // ---- LSE combine (step a4): warp-sized units, statically assigned (see the MQA/GQA kernel)
         float *wsm = reinterpret_cast<float *>(smem + MLA_SMEM_P) + (warp - 2) * kMaxSplits;
         for (int u = blockIdx.x * 4 + (warp - 2); u < p.n_combine_units; u += gridDim.x * 4)
             combine_warp_unit(p, u, wsm, lane);
+        MLA_STAMP(22, tid == 64);
     }
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc(tmem, MLA_TMEM_COLS);
     scheduler_epilogue(p, &mi->flag);
+    MLA_STAMP(23, tid == 64);
 }
 
 // ----------------------------------------------------------------------------- host side

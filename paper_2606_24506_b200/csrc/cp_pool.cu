@@ -233,7 +233,10 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
                 if (ns > 1) {
                     for (int h = 0; h < g; ++h) kp.combines.push_back(Combine{gi, h});
                     // warp-sized units: split lanes ZL so that a lane holds <= 16 splits (8 for ZL = 1, 8)
-                    const int zl = ns <= 8 ? 0 : (ns <= 32 ? 3 : (ns <= 128 ? 4 : 5));   // <= 4..8 splits per lane
+                    // wide value rows (MLA, 512 columns): a unit costs a few L2 round trips whatever its
+                    // width, so keep units few and wide (zl = 0: one float4 column per lane, 128 columns)
+                    const int zl = (m.head_dim_v > 128 && ns <= 64) ? 0
+                                   : (ns <= 8 ? 0 : (ns <= 32 ? 3 : (ns <= 128 ? 4 : 5)));
                     const int cols = 128 >> zl;
                     const int mt = (g + 15) / 16;
                     int mtp = 1;
