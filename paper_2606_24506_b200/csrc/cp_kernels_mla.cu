@@ -62,8 +62,8 @@ constexpr int MLA_KB = MLA_DK / 64;                 // 9 column blocks of 64 (12
 constexpr int MLA_STAGES = 4;
 constexpr int MLA_STAGE_BYTES = MLA_TS * MLA_DK * 2;        // 36864
 constexpr int MLA_BLK_BYTES = MLA_TS * 128;                 // one [32 x 64] swizzled tile: 4096
-constexpr int MLA_KB_TMEM = 5;                      // query column blocks 0..4 live in TMEM (A operand, TS mode)
-constexpr int MLA_Q_BYTES = (MLA_KB - MLA_KB_TMEM) * MLA_M * 128;   // 65536: blocks 5..8 of [128 x 64] in shared memory
+constexpr int MLA_KB_TMEM = 6;                      // query column blocks 0..5 live in TMEM (A operand, TS mode)
+constexpr int MLA_Q_BYTES = (MLA_KB - MLA_KB_TMEM) * MLA_M * 128;   // 49152: blocks 6..8 of [128 x 64] in shared memory
 constexpr int MLA_QBLK_BYTES = MLA_M * 128;                 // 16384
 constexpr int MLA_P_BYTES = MLA_M * MLA_TS * 2;             // 8192, one P buffer
 constexpr int MLA_THREADS = 192;
@@ -76,7 +76,8 @@ constexpr int MLA_SMEM_BYTES = MLA_SMEM_MISC + 1024;
 static_assert(MLA_SMEM_BYTES <= 232448, "MLA kernel exceeds the 227 KB shared-memory limit");
 constexpr uint32_t MLA_TMEM_COLS = 512;
 constexpr uint32_t MLA_TMEM_S0 = 256, MLA_TMEM_S1 = 288;       // two score buffers of MLA_TS columns
-constexpr uint32_t MLA_TMEM_Q = 320;                           // 160 columns: Q[:, 0:320) as bf16 pairs
+constexpr uint32_t MLA_TMEM_Q = 320;                           // 192 columns: Q[:, 0:384) as bf16 pairs
+static_assert(MLA_TMEM_Q + MLA_KB_TMEM * 32 <= MLA_TMEM_COLS, "TMEM budget");
 constexpr float MLA_LAZY_LOG2 = 8.0f;
 
 // What the producer hands to the other warps for one work item.
@@ -297,30 +298,30 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             MLA_STAMP(17, tid == 64 && qi == 1);
 
             if (d.load_q) {
-                // stage the query block [128 x 576] bf16.  Column blocks 0..4 go to tensor memory (this
+                // stage the query block [128 x 576] bf16.  Column blocks 0..5 go to tensor memory (this
                 // thread's head = its TMEM lane; two bf16 per 32-bit column, memory order), where the
-                // score MMAs read them as the A operand without shared-memory traffic; blocks 5..8 go
+                // score MMAs read them as the A operand without shared-memory traffic; blocks 6..8 go
                 // to shared memory as K-major [128 x 64] tiles with the 128-byte swizzle the MMA
                 // descriptor expects (16-B chunk index ^ (row & 7)).  Rows >= Hq are zero.
                 {
                     const uint4 *qr = reinterpret_cast<const uint4 *>(p.q + d.q_off + (int64_t)row * MLA_DK);
                     const bool live = row < d.n_heads;
-                    for (int c0 = 0; c0 < MLA_KB_TMEM * 32; c0 += 80) {   // batches of 5 x 16 columns: 20 loads in flight
-                        uint4 v[20];
+                    for (int c0 = 0; c0 < MLA_KB_TMEM * 32; c0 += 64) {   // batches of 4 x 16 columns: 16 loads in flight
+                        uint4 v[16];
 #pragma unroll
-                        for (int i = 0; i < 20; ++i) {
+                        for (int i = 0; i < 16; ++i) {
                             v[i] = make_uint4(0u, 0u, 0u, 0u);
                             if (live) v[i] = __ldg(qr + c0 / 4 + i);
                         }
 #pragma unroll
-                        for (int b5 = 0; b5 < 5; ++b5) {                  // 16 columns = 32 bf16 = 4 x 16 B
+                        for (int b4 = 0; b4 < 4; ++b4) {                  // 16 columns = 32 bf16 = 4 x 16 B
                             uint32_t w[16];
 #pragma unroll
                             for (int v4 = 0; v4 < 4; ++v4) {
-                                w[4 * v4] = v[4 * b5 + v4].x; w[4 * v4 + 1] = v[4 * b5 + v4].y;
-                                w[4 * v4 + 2] = v[4 * b5 + v4].z; w[4 * v4 + 3] = v[4 * b5 + v4].w;
+                                w[4 * v4] = v[4 * b4 + v4].x; w[4 * v4 + 1] = v[4 * b4 + v4].y;
+                                w[4 * v4 + 2] = v[4 * b4 + v4].z; w[4 * v4 + 3] = v[4 * b4 + v4].w;
                             }
-                            tmem_st16(tl + MLA_TMEM_Q + c0 + b5 * 16, w);
+                            tmem_st16(tl + MLA_TMEM_Q + c0 + b4 * 16, w);
                         }
                     }
                     tmem_wait_st();
