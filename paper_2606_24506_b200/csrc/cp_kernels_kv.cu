@@ -336,7 +336,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                     const uint32_t slot = pc % NS;
                     const uint32_t par = ((pc / NS) & 1) ^ 1;
                     mbar_wait(smem_u32(empty_b + slot), par);
-                    if (lane == 0) {
+                    if (elect_one()) {
                         const uint32_t fb = smem_u32(full_b + slot);
 #ifdef CP_KV_PROBE_NO_LOAD      /* probe builds only: consumer capacity without memory traffic */
                         mbar_arrive(fb);

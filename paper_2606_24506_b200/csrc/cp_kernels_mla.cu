@@ -197,7 +197,7 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);
                     const uint32_t slot = gs % MLA_STAGES;
                     mbar_wait(smem_u32(&mi->empty[slot]), ((gs / MLA_STAGES) & 1) ^ 1);
-                    if (lane == 0) {
+                    if (elect_one()) {
                         const uint32_t fb = smem_u32(&mi->full[slot]);
                         mbar_arrive_expect_tx(fb, MLA_STAGE_BYTES);
                         const int row = my * rows_per_page + ((s0 + j) % spp) * MLA_TS;
