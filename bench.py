@@ -29,9 +29,9 @@ if ROOT not in sys.path:
 import numpy as np
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the decode kernel, from the committed
-# `ncu --set full` captures (profiles/r1_ncu_full_cfg{2,4}_kv_v3.txt, r1_ncu_full_cfg3_mla_v1.txt)
-NCU_TRAFFIC_BYTES = {2: 344.64e6 + 7.86e6, 3: 285.27e6 + 7.97e6, 4: 134.33e6 + 6.31e6}
-NCU_TENSOR_PIPE_PCT = {3: 13.4}       # sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active
+# `ncu --set full` captures (profiles/r1_ncu_full_cfg2_kv_v4.txt, r1_ncu_full_cfg4_kv_v3.txt, r1_ncu_full_cfg3_mla_v2.txt)
+NCU_TRAFFIC_BYTES = {2: 344.69e6 + 6.35e6, 3: 284.62e6 + 8.38e6, 4: 134.33e6 + 6.31e6}
+NCU_TENSOR_PIPE_PCT = {3: 33.2}       # sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active
 
 METRIC = "paged decode-attention KV GB/s"
 UNIT = "GB/s"
@@ -223,12 +223,12 @@ def main():
     sampler = ClockSampler(local_rank) if rank == 0 else None
 
     # ---------------- device-resident leg: K steps, inputs already in HBM
+    t_wall0 = time.time()               # clocks are sampled from the warm-up on (the timed region is a few ms)
     for _ in range(args.warmup):
         dw.decode()
     barrier()
     c0 = dw.pool.counters()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps)]
-    t_wall0 = time.time()
     start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     start.record()
     for i in range(args.steps):
