@@ -6,18 +6,19 @@
 // (241 flop per KV byte), so here -- and only here -- the 5th-generation tensor cores are used:
 //     S[128 x 32]   = Q[128 x 576] . C_slice^T      36 x tcgen05.mma M128 N32  K16 (A, B K-major)
 //     O[128 x 256] += P[128 x 32]  . C_slice[:, half]  2 x tcgen05.mma M128 N256 K16 (B MN-major)
-// per 32-token slice of a page (measured: an SS-mode MMA costs ~64 cycles of shared-memory operand
-// reads for the 4 KB A tile whatever N is, so the slice is as long as shared memory allows).  TMEM holds 512 fp32 columns per SM; O[128 x 512] alone would
-// fill it, so one work item is (tile, value half): it accumulates 256 of the 512 value columns
-// (TMEM columns 0..255) and keeps two S buffers (columns 256.., 288..).  The two halves of a
-// tile are adjacent work items, popped by different CTAs at about the same time, so the second
+// per 32-token slice of a page.  TMEM holds 512 fp32 columns per SM; O[128 x 512] alone would fill
+// it, so one work item is (tile, value half): 256 O columns (TMEM columns 0..255), two score
+// buffers (256.., 288..) and, in the remaining 192 columns, six of the nine 64-column blocks of Q
+// as the A operand of TS-mode MMAs (measured: an SS-mode MMA re-reads its 4 KB A tile from shared
+// memory, ~70 cycles whatever N is; A from tensor memory costs ~16 at N = 32).  The two halves of
+// a tile are adjacent work items, popped by different CTAs at about the same time, so the second
 // reader of a page hits L2 (DESIGN.md §6.3 states the cost: the QK^T part is computed twice).
 //
 // Warp roles (192 threads, 1 CTA/SM):
 //   warp 0      producer: pops work items, translates logical pages through the page table
-//               (step a2) and streams 32-token slices into a 2-stage ring with one 3-D TMA
+//               (step a2) and streams 32-token slices into a 4-stage ring with one 3-D TMA
 //               box each (9 swizzled [32 x 64] tiles), mbarrier complete_tx.
-//   warp 1      MMA issuer (one elected lane): S_{i+1} is issued before P_i V_i so the tensor
+//   warp 1      MMA issuer (one lane chosen by elect.sync): S_{i+1} is issued before P_i V_i so the tensor
 //               pipe computes the next scores while the softmax warps work on the current ones.
 //   warps 2..5  softmax: thread = one query head = one TMEM lane, so the row maximum and row
 //               sum need no shuffles; online softmax in fp32 (log2 units) with a lazy reference
