@@ -154,6 +154,51 @@ def test_outputs_of_order_one_mla(torch_cuda):
         print(worst)
 
 
+def _add_logit_ramp(w, req_index, amp, dims):
+    """Make the logits of request `req_index` rise steadily along the context (by about
+    sigma * 4 * amp in total): q_h += 4 u, k_t += amp (t / T) u with u a unit vector supported on
+    `dims`.  The running softmax reference then has to move many times (the kernels' lazy
+    reference update and, on the MLA path, the rescale of O in tensor memory)."""
+    r = w.requests[req_index]
+    m = w.models[r.model_id]
+    P, d = w.page_tokens, m.head_dim_qk
+    u = np.zeros(d)
+    u[dims] = np.random.default_rng(5).standard_normal(len(dims))
+    u /= np.linalg.norm(u)
+    w.q[req_index] = W.f32_to_bf16((W.bf16_to_f64(w.q[req_index]) + 4.0 * u).astype(np.float32))
+    pages = w.arena.reshape(w.num_pages, -1)
+    n_lp = -(-r.context_len // P)
+    for lp in range(n_lp):
+        t = lp * P + np.arange(P)
+        ramp = (amp * np.minimum(t, r.context_len - 1) / r.context_len)[:, None] * u[None, :]
+        for c in range(m.n_kv_heads):
+            blk = pages[int(r.page_ids[lp * m.n_kv_heads + c])][:P * d].reshape(P, d)
+            valid = min(P, r.context_len - lp * P)
+            k = W.bf16_to_f64(blk[:valid]) + ramp[:valid]
+            blk[:valid] = W.f32_to_bf16(k.astype(np.float32))
+
+
+@pytest.mark.parametrize("kind", ["kv", "mla"])
+def test_rising_logits_move_the_softmax_reference(torch_cuda, kind):
+    import paper_2606_24506_b200 as cp
+    if kind == "kv":
+        m = ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5)
+        w = W.small_workload([m], [0, 0], [3000, 700], page_tokens=64, seed=11, keep_contiguous=False)
+        _add_logit_ramp(w, 0, 200.0, list(range(128)))
+    else:
+        m = ModelCfg(KIND_MLA, 128, 1, 576, 512, 192 ** -0.5)
+        w = W.small_workload([m], [0, 0], [3000, 700], page_tokens=64, seed=12, value_scale=0.1,
+                             keep_contiguous=False)
+        _add_logit_ramp(w, 0, 240.0, list(range(512, 576)))      # rope part only: values untouched
+    ref_lse = oracle.decode_workload(w)[0][1]
+    assert ref_lse.max() - ref_lse.min() >= 0 and ref_lse.max() > 30.0     # the ramp is really there
+    for kernel in (0, 1):
+        for mtp in (1, 100000):                                  # many short tiles / one tile per group
+            worst = run_and_compare(w, "ramp_%s/k%d/mtp%d" % (kind, kernel, mtp),
+                                    {cp.CP_OPT_KERNEL: kernel, cp.CP_OPT_MIN_TILE_PAGES: mtp})
+            print(worst)
+
+
 # ------------------------------------------------------------------ invariants on the GPU path
 def test_page_permutation_is_bit_identical(torch_cuda):
     """P5 on the GPU: split boundaries are logical, so moving the data to other physical
