@@ -38,6 +38,23 @@ UNIT = "GB/s"
 L2_BYTES = 126 * 1024 * 1024
 
 
+def reduce_max_over_ranks(x: float, device="cpu") -> float:
+    """Max over ranks of a per-rank time (the contract: time on the device, take the MAX)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(bytes_per_rank: int, world: int, step_ms: float) -> float:
+    """Replicas only: every rank processes its own copy of the batch; the
+    whole-job throughput is the bytes of all ranks over the slowest rank's step time."""
+    return world * bytes_per_rank / (step_ms * 1e-3) / 1e9
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -242,10 +259,7 @@ def main():
     kern_ms = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(args.steps)]
     region_ms = start.elapsed_time(stop)
     step_ms = float(np.sum(kern_ms)) / args.steps     # one launch per step: step = the event-bracketed launch
-    t = torch.tensor([step_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    step_ms = float(t.item())
+    step_ms = reduce_max_over_ranks(step_ms, dev)
     launches = c1["kernel_launches"] - c0["kernel_launches"]
 
     # ---------------- end-to-end leg: host buffers through cp_decode_attention_host
@@ -267,10 +281,7 @@ def main():
         dw.pool.decode_attention_host(dw.ids, q_host, o_host, l_host, ws, need, dw.stream())
         e2e_s += time.perf_counter() - t0
     e2e_ms = 1e3 * e2e_s / e2e_steps
-    t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item())
+    e2e_ms = reduce_max_over_ranks(e2e_ms, dev)
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
 
@@ -280,7 +291,7 @@ def main():
         return 0
 
     peaks = measured_peaks()
-    value = world * abytes / (step_ms * 1e-3) / 1e9
+    value = whole_job_value(abytes, world, step_ms)
     kern_avg_ms = float(np.mean(kern_ms))
     achieved = abytes / (kern_avg_ms * 1e-3) / 1e9
     mla = any(m.kind == 1 for m in w.models)
@@ -298,7 +309,7 @@ def main():
             "warmup": args.warmup, "ms_per_step": step_ms, "us_per_step": 1e3 * step_ms,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16 in, fp32 accumulate",
             "data": "synthetic", "config": workload_desc(w, k), "clocks": clocks,
-            "e2e": {"value": world * abytes / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
+            "e2e": {"value": whole_job_value(abytes, world, e2e_ms), "unit": UNIT,
                     "us_per_step": 1e3 * e2e_ms,
                     "h2d_bytes_per_step": int(q_host.numel() * 2),
                     "d2h_bytes_per_step": int(o_host.numel() * 4 + l_host.numel() * 4)},
