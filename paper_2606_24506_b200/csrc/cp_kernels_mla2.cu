@@ -1,0 +1,448 @@
+// cp_kernels_mla2.cu -- MLA latent path on CTA PAIRS (cluster of 2 SMs, tcgen05 cta_group::2).
+//
+// Same computation as cp_kernels_mla.cu (hot-path steps a2, a3', a4-a6 for the 576/512 latent
+// shape), but one tile is processed by a pair of CTAs that share every MMA:
+//     S[128 x 32]   = Q[128 x 576] . C_slice^T     36 pair-MMAs M128 N32 K16
+//     O[128 x 512] += P[128 x 32] . C_slice[:, :512]  2 k-steps x 2 pair-MMAs M128 N256 K16
+// Each CTA holds 64 of the 128 heads (its rows of Q, S, P, O) and supplies half of every B
+// operand from its own shared memory: its 16 tokens of the slice for the score MMA, its 128 of
+// each 256 value columns for the value MMA.  With 64 rows per CTA the accumulator O[64 x 512]
+// takes 128 lanes x 256 TMEM columns (2 x 2 layout: columns 0..127 of an N = 256 MMA in lanes
+// 0..63, columns 128..255 in lanes 64..127), so all 512 value columns fit and QK^T is computed
+// once per tile (the single-CTA kernel computes it once per value half).
+//
+// Shared memory of one CTA per slice stage: [S area: its 16 tokens x 9 column blocks, K-major]
+// [PV area: for k-step kk in {0, 1} (tokens 16kk..16kk+15) and MMA j in {0, 1} its two 64-column
+// blocks 4j + 2r, 4j + 2r + 1 (r = CTA rank), MN-major].  Both areas sit at the same offsets in both
+// CTAs because one descriptor addresses both.
+//
+// Warp roles per CTA (192 threads): warp 0 TMA producer; warp 1 MMA issuer in the leader CTA
+// (rank 0), relay of the "slice landed" barrier in the peer; warps 2..5 softmax: thread = TMEM
+// lane = (head, token half), the two halves of a head exchange their row maximum through shared
+// memory.  Tiles are assigned statically to pairs (tile = pair, pair + #pairs, ...).
+//
+// Paper anchors: paged KV interface PAPER.md:L101,L122; MLA among the KV-head-limited families
+// PAPER.md:L21,L57; GPU-resident persistent control PAPER.md:L146.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdint>
+#include "cp_device_common.cuh"
+#include "cp_launch.h"
+#include "cp_ptx.cuh"
+
+namespace cp {
+
+constexpr int M2_DK = 576, M2_DV = 512;
+constexpr int M2_TS = 32;                           // tokens per slice (16 per CTA for the score MMA)
+constexpr int M2_KB = 9;                            // 64-column blocks of the latent row
+constexpr int M2_STAGES = 4;
+constexpr int M2_BLK = 16 * 128;                    // one [16 x 64] swizzled tile: 2048 bytes
+constexpr int M2_SAREA = M2_KB * M2_BLK;            // 18432
+constexpr int M2_PVAREA = 2 * 2 * 2 * M2_BLK;       // 16384: [kk][j][2 blocks]
+constexpr int M2_STAGE_BYTES = M2_SAREA + M2_PVAREA;        // 34816
+constexpr int M2_QBLK = 64 * 128;                   // one [64 x 64] K-major tile of this CTA's query rows
+constexpr int M2_Q_BYTES = M2_KB * M2_QBLK;         // 73728
+constexpr int M2_P_BYTES = 64 * M2_TS * 2;          // 4096
+constexpr int M2_THREADS = 192;
+constexpr int M2_SMEM_Q = 0;
+constexpr int M2_SMEM_STAGE = M2_Q_BYTES;
+constexpr int M2_SMEM_P = M2_SMEM_STAGE + M2_STAGES * M2_STAGE_BYTES;
+constexpr int M2_SMEM_MISC = M2_SMEM_P + M2_P_BYTES;
+constexpr int M2_SMEM_BYTES = M2_SMEM_MISC + 2048;
+static_assert(M2_SMEM_BYTES <= 232448, "MLA pair kernel exceeds the 227 KB shared-memory limit");
+constexpr uint32_t M2_TMEM_COLS = 512;
+constexpr uint32_t M2_TMEM_S0 = 256, M2_TMEM_S1 = 288;      // score buffers: 16 columns each (2 x 2 layout)
+constexpr float M2_LAZY_LOG2 = 8.0f;
+
+struct M2Misc {
+    uint64_t full[M2_STAGES];       // local TMA landed (this CTA's part of the slice)
+    uint64_t full_peer[M2_STAGES];  // leader only: the peer's part landed (arrived by the peer's relay warp)
+    uint64_t empty[M2_STAGES];      // pair-MMA commit (multicast): stage free
+    uint64_t s_full[2];             // pair-MMA commit (multicast): scores ready
+    uint64_t s_empty[2];            // leader only: 8 softmax warps of the pair have read the scores
+    uint64_t p_full;                // leader only: 8 softmax warps have written P
+    uint64_t p_done;                // pair-MMA commit (multicast): value MMAs of the slice complete
+    uint64_t q_full;                // leader only: 8 softmax warps have staged the query rows
+    float xmax[2][128];             // row maxima exchanged between the two token halves of a head (by slice parity)
+    float xsum[128];
+    uint32_t tmem_base;
+    int32_t flag;
+};
+static_assert(sizeof(M2Misc) <= 2048, "M2Misc must fit its reserved block");
+
+struct M2Item {                     // one tile, derived identically by every warp of the pair
+    int32_t valid;                  // false: no more work
+    int32_t group_idx, n_slices, valid_last, split, n_splits, n_heads, page_begin, req;
+    float scale_log2;
+    int64_t q_off, out_off, lse_off, part_off;
+};
+
+__device__ __forceinline__ M2Item m2_item(const DecodeParams &p, int tile_idx)
+{
+    M2Item it;
+    it.valid = tile_idx < p.n_tiles;
+    if (!it.valid) return it;
+    TileRec r;
+    const uint4 *src = reinterpret_cast<const uint4 *>(p.tile_recs + tile_idx);
+    uint4 *dst = reinterpret_cast<uint4 *>(&r);
+#pragma unroll
+    for (int i = 0; i < 5; ++i) dst[i] = __ldg(src + i);
+    const int ctx = __ldg(p.req_ctx + r.req);
+    const int P = (int)p.page_tokens;
+    const int t_begin = r.page_begin * P;
+    const int t_end = min((r.page_begin + r.n_pages) * P, ctx);
+    it.n_slices = (t_end - t_begin + M2_TS - 1) / M2_TS;
+    it.valid_last = t_end - t_begin - (it.n_slices - 1) * M2_TS;
+    it.group_idx = r.group; it.split = r.split; it.n_splits = r.n_splits; it.n_heads = r.n_q_heads;
+    it.page_begin = r.page_begin; it.req = r.req; it.scale_log2 = r.scale_log2;
+    it.q_off = r.q_off; it.out_off = r.out_off; it.lse_off = r.lse_off; it.part_off = r.part_off;
+    return it;
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(M2_THREADS, 1)
+cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap9,
+                      const __grid_constant__ CUtensorMap tmap2, int rows_per_page)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    M2Misc *mi = reinterpret_cast<M2Misc *>(smem + M2_SMEM_MISC);
+    const int tid = threadIdx.x;
+    const int warp = tid >> 5;
+    const int lane = tid & 31;
+    const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the pair MMAs)
+    const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+    const uint32_t q_base = smem_u32(smem + M2_SMEM_Q);
+    const uint32_t st_base = smem_u32(smem + M2_SMEM_STAGE);
+    const uint32_t p_base = smem_u32(smem + M2_SMEM_P);
+
+    if (tid == 0) {
+        for (int i = 0; i < M2_STAGES; ++i) {
+            mbar_init(smem_u32(&mi->full[i]), 1); mbar_init(smem_u32(&mi->full_peer[i]), 1);
+            mbar_init(smem_u32(&mi->empty[i]), 1);
+        }
+        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&mi->s_full[i]), 1); mbar_init(smem_u32(&mi->s_empty[i]), 8); }
+        mbar_init(smem_u32(&mi->p_full), 8); mbar_init(smem_u32(&mi->p_done), 1);
+        mbar_init(smem_u32(&mi->q_full), 8);
+        asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap9)) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap2)) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
+    }
+    if (warp == 1) tmem_alloc2(smem_u32(&mi->tmem_base), M2_TMEM_COLS);
+    tc_fence_before();
+    cluster_sync_all();                               // barriers of both CTAs initialised, TMEM allocated
+    tc_fence_after();
+    const uint32_t tmem = mi->tmem_base;
+    const int P = (int)p.page_tokens;
+    const int spp = P / M2_TS;
+    // leader's barriers as seen from this CTA (own address in the leader, mapped address in the peer)
+    const uint32_t L_s_empty0 = mapa_u32(smem_u32(&mi->s_empty[0]), 0), L_s_empty1 = mapa_u32(smem_u32(&mi->s_empty[1]), 0);
+    const uint32_t L_p_full = mapa_u32(smem_u32(&mi->p_full), 0), L_q_full = mapa_u32(smem_u32(&mi->q_full), 0);
+
+    if (warp == 0) {
+        // =========================================================== producer warp (each CTA loads its part)
+        uint64_t policy;
+        asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(policy));
+        uint32_t gs = 0;
+        for (int k = 0;; ++k) {
+            const M2Item it = m2_item(p, pair + k * n_pairs);
+            if (!it.valid) break;
+            const int32_t *pt = p.page_table + (int64_t)it.req * p.max_ppr;
+            for (int s0 = 0; s0 < it.n_slices; s0 += 32) {
+                int32_t pid = 0;
+                if (s0 + lane < it.n_slices) pid = __ldg(pt + it.page_begin + (s0 + lane) / spp);
+                const int ns = min(32, it.n_slices - s0);
+                for (int j = 0; j < ns; ++j) {
+                    const int32_t my = __shfl_sync(0xffffffffu, pid, j);
+                    const uint32_t slot = gs % M2_STAGES;
+                    mbar_wait(smem_u32(&mi->empty[slot]), ((gs / M2_STAGES) & 1) ^ 1);
+                    if (elect_one()) {
+                        const uint32_t fb = smem_u32(&mi->full[slot]);
+                        mbar_arrive_expect_tx(fb, M2_STAGE_BYTES);
+                        const int row0 = my * rows_per_page + ((s0 + j) % spp) * M2_TS;
+                        const uint32_t dst = st_base + slot * M2_STAGE_BYTES;
+                        // S area: this CTA's 16 tokens, all 9 column blocks
+                        tma_load_3d(dst, &tmap9, 0, row0 + 16 * (int)rank, 0, fb, policy);
+                        // PV area: tokens 16kk.., this CTA's column blocks 4j + 2r, 4j + 2r + 1
+#pragma unroll
+                        for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+                            for (int jj = 0; jj < 2; ++jj)
+                                tma_load_3d(dst + M2_SAREA + (kk * 2 + jj) * 2 * M2_BLK, &tmap2, 0, row0 + 16 * kk,
+                                            4 * jj + 2 * (int)rank, fb, policy);
+                    }
+                    ++gs;
+                }
+            }
+        }
+    } else if (warp == 1 && rank != 0) {
+        // =========================================================== peer: relay "my part of the slice landed"
+        uint32_t gs = 0;
+        for (int k = 0;; ++k) {
+            const M2Item it = m2_item(p, pair + k * n_pairs);
+            if (!it.valid) break;
+            for (int i = 0; i < it.n_slices; ++i, ++gs) {
+                const uint32_t slot = gs % M2_STAGES;
+                mbar_wait(smem_u32(&mi->full[slot]), (gs / M2_STAGES) & 1);
+                if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&mi->full_peer[slot]), 0));
+                __syncwarp();
+            }
+        }
+    } else if (warp == 1) {
+        // =========================================================== leader: pair-MMA issuer
+        constexpr uint32_t IDESC_S = umma_idesc_bf16(128, M2_TS, 0, 0);
+        constexpr uint32_t IDESC_PV = umma_idesc_bf16(128, 256, 0, 1);
+        uint32_t gs = 0, qn = 0;
+        int prev_group = -1;
+        for (int k = 0;; ++k) {
+            const M2Item it = m2_item(p, pair + k * n_pairs);
+            if (!it.valid) break;
+            if (it.group_idx != prev_group) { mbar_wait_cluster(smem_u32(&mi->q_full), qn & 1); ++qn; prev_group = it.group_idx; }
+            const int n = it.n_slices;
+            for (int i = 0; i <= n; ++i) {
+                if (i < n) {
+                    const uint32_t g = gs + (uint32_t)i, slot = g % M2_STAGES, b = g & 1;
+                    mbar_wait(smem_u32(&mi->full[slot]), (g / M2_STAGES) & 1);
+                    mbar_wait_cluster(smem_u32(&mi->full_peer[slot]), (g / M2_STAGES) & 1);
+                    mbar_wait_cluster(smem_u32(&mi->s_empty[b]), ((g >> 1) & 1) ^ 1);
+                    tc_fence_after();
+                    if (elect_one()) {
+                        const uint32_t c0 = st_base + slot * M2_STAGE_BYTES;
+                        const uint32_t dcol = tmem + (b ? M2_TMEM_S1 : M2_TMEM_S0);
+#pragma unroll
+                        for (int kb = 0; kb < M2_KB; ++kb)
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) {
+                                const uint64_t ad = umma_smem_desc(q_base + kb * M2_QBLK + j * 32, 16, 1024, 2);
+                                const uint64_t bd = umma_smem_desc(c0 + kb * M2_BLK + j * 32, 16, 1024, 2);
+                                umma2_bf16_ss(dcol, ad, bd, IDESC_S, (kb | j) != 0);
+                            }
+                        umma2_commit(smem_u32(&mi->s_full[b]));
+                    }
+                    __syncwarp();
+                }
+                if (i >= 1) {
+                    const uint32_t g = gs + (uint32_t)i - 1, slot = g % M2_STAGES;
+                    mbar_wait_cluster(smem_u32(&mi->p_full), g & 1);
+                    tc_fence_after();
+                    if (elect_one()) {
+                        const uint32_t pv = st_base + slot * M2_STAGE_BYTES + M2_SAREA;
+#pragma unroll
+                        for (int kk = 0; kk < 2; ++kk)
+#pragma unroll
+                            for (int jj = 0; jj < 2; ++jj) {
+                                // P: 8-token chunks of [64 rows x 16 B] 1024 B apart, 8-row groups 128 B apart
+                                const uint64_t ad = umma_smem_desc(p_base + kk * 2048, 1024, 128, 0);
+                                // V: two 64-column blocks 2048 B apart, 8-token groups 1024 B apart
+                                const uint64_t bd = umma_smem_desc(pv + (kk * 2 + jj) * 2 * M2_BLK, M2_BLK, 1024, 2);
+                                umma2_bf16_ss(tmem + jj * 128, ad, bd, IDESC_PV, (i > 1) || (kk > 0));
+                            }
+                        umma2_commit(smem_u32(&mi->empty[slot]));
+                        umma2_commit(smem_u32(&mi->p_done));
+                    }
+                    __syncwarp();
+                }
+            }
+            gs += (uint32_t)n;
+        }
+    } else {
+        // =========================================================== softmax warps
+        // thread = TMEM lane L: head (rank * 64 + L % 64), token half L / 64 of every slice
+        const int q4 = warp & 3;
+        const int L = q4 * 32 + lane;
+        const int hrow = L & 63;                          // row inside this CTA
+        const int head = (int)rank * 64 + hrow;
+        const int th = L >> 6;                            // token half: tokens 16 th .. 16 th + 15 of a slice
+        const uint32_t tl = tmem + ((uint32_t)(q4 * 32) << 16);
+        const int st = tid - 64;
+        uint32_t gs = 0;
+        int prev_group = -1;
+        for (int k = 0;; ++k) {
+            const M2Item it = m2_item(p, pair + k * n_pairs);
+            if (!it.valid) break;
+            if (it.group_idx != prev_group) {
+                // stage this CTA's 64 query rows as 9 K-major [64 x 64] tiles, 128-byte swizzle; rows >= Hq zero
+                prev_group = it.group_idx;
+                const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + it.q_off) + (int64_t)rank * 64 * (M2_DK / 8);
+#pragma unroll 8
+                for (int id = st; id < 64 * (M2_DK / 8); id += 128) {
+                    const int r = id / (M2_DK / 8), ch = id % (M2_DK / 8);
+                    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                    if ((int)rank * 64 + r < it.n_heads) v = __ldg(qg + id);
+                    const uint32_t a = q_base + (ch >> 3) * M2_QBLK + r * 128 + (((ch & 7) ^ (r & 7)) << 4);
+                    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+                }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(L_q_full);
+            }
+            float m_run = -INFINITY, l_run = 0.f;
+            const int n = it.n_slices;
+            for (int i = 0; i < n; ++i) {
+                const uint32_t g = gs + (uint32_t)i, b = g & 1, kq = g >> 1;
+                mbar_wait(smem_u32(&mi->s_full[b]), kq & 1);
+                tc_fence_after();
+                uint32_t sr[16];
+                tmem_ld16(tl + (b ? M2_TMEM_S1 : M2_TMEM_S0), sr);
+                tmem_wait_ld();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(b ? L_s_empty1 : L_s_empty0);
+                const int valid = ((i == n - 1) ? it.valid_last : M2_TS) - 16 * th;   // valid tokens of my half
+                float mx = -INFINITY;
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const float v = j < valid ? __uint_as_float(sr[j]) * it.scale_log2 : -INFINITY;
+                    sr[j] = __float_as_uint(v);
+                    mx = fmaxf(mx, v);
+                }
+                // the two token halves of a head agree on the row maximum through shared memory
+                mi->xmax[b][L] = mx;
+                asm volatile("bar.sync 2, 128;" ::: "memory");
+                mx = fmaxf(mx, mi->xmax[b][L ^ 64]);
+                const float m_new = (mx > m_run + M2_LAZY_LOG2) ? mx : m_run;
+                const bool need = (m_new != m_run) && i > 0;
+                const float a_resc = ex2_ftz(m_run - m_new);
+                if (m_new != m_run) { l_run *= a_resc; m_run = m_new; }
+                uint32_t pw[8];
+                float sum = 0.f;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const float p0 = ex2_ftz(__uint_as_float(sr[2 * j]) - m_run), p1 = ex2_ftz(__uint_as_float(sr[2 * j + 1]) - m_run);
+                    sum += p0 + p1;
+                    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pw[j]) : "f"(p1), "f"(p0));
+                }
+                l_run += sum;
+                mbar_wait(smem_u32(&mi->p_done), (g & 1) ^ 1);       // P buffer free, O quiescent
+                if (__any_sync(0xffffffffu, need)) {
+                    tc_fence_after();
+                    const float a = need ? a_resc : 1.f;
+                    for (int c = 0; c < 256; c += 16) {
+                        uint32_t o[16];
+                        tmem_ld16(tl + c, o);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * a);
+                        tmem_st16(tl + c, o);
+                    }
+                    tmem_wait_st();
+                }
+                // P[row][token] as 8-token chunks of [64 rows x 16 B]: chunk c at c * 1024 + row * 16
+                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p_base + (2 * th) * 1024 + hrow * 16), "r"(pw[0]), "r"(pw[1]), "r"(pw[2]), "r"(pw[3]) : "memory");
+                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p_base + (2 * th + 1) * 1024 + hrow * 16), "r"(pw[4]), "r"(pw[5]), "r"(pw[6]), "r"(pw[7]) : "memory");
+                if (i == n - 1 && it.valid_last < M2_TS) {
+                    // dead slots of the request's last slice may hold NaN: zero their value rows in the PV area
+                    // (warp q4 clears the two 64-column blocks of MMA j = q4 & 1 for k-step kk = q4 >> 1)
+                    const int kk = q4 >> 1, jj = q4 & 1;
+                    const int vrows = min(16, max(0, it.valid_last - 16 * kk));        // valid rows of this k-step
+                    const uint32_t blk = st_base + (g % M2_STAGES) * M2_STAGE_BYTES + M2_SAREA + (kk * 2 + jj) * 2 * M2_BLK;
+                    for (int e = lane; e < (16 - vrows) * 16; e += 32) {
+                        const int r = vrows + (e >> 4), ch = e & 15;
+                        asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(blk + (ch >> 3) * M2_BLK + r * 128 + (((ch & 7) ^ (r & 7)) << 4)), "r"(0u) : "memory");
+                    }
+                }
+                fence_proxy_async();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(L_p_full);
+            }
+            gs += (uint32_t)n;
+
+            // ---- end of tile: O rows from TMEM, publish
+            {
+                const uint32_t gl = gs - 1;
+                mbar_wait(smem_u32(&mi->p_done), gl & 1);
+                tc_fence_after();
+                mi->xsum[L] = l_run;
+                asm volatile("bar.sync 2, 128;" ::: "memory");
+                const float l_tot = th == 0 ? l_run + mi->xsum[L ^ 64] : mi->xsum[L ^ 64] + l_run;   // same order in both halves
+                const bool final_out = it.n_splits == 1;
+                const float inv = final_out ? 1.f / l_tot : 1.f;
+                float *rowp = final_out ? p.out + it.out_off + (int64_t)head * M2_DV
+                                        : p.workspace + it.part_off + part_o_off(head, it.split, it.n_splits, M2_DV);
+                for (int c = 0; c < 256; c += 16) {
+                    uint32_t o[16];
+                    tmem_ld16(tl + c, o);
+                    tmem_wait_ld();
+                    // TMEM column c of MMA jj = c / 128 holds value column 256 jj + 128 th + c % 128 of my head
+                    float *dst = rowp + 256 * (c >> 7) + 128 * th + (c & 127);
+                    if (head < it.n_heads) {
+#pragma unroll
+                        for (int j = 0; j < 16; j += 4)
+                            __stcg(reinterpret_cast<float4 *>(dst + j),
+                                   make_float4(__uint_as_float(o[j]) * inv, __uint_as_float(o[j + 1]) * inv,
+                                               __uint_as_float(o[j + 2]) * inv, __uint_as_float(o[j + 3]) * inv));
+                    }
+                }
+                tc_fence_before();
+                if (th == 0 && head < it.n_heads) {
+                    if (final_out)
+                        p.lse[it.lse_off + head] = (m_run + log2f(l_tot)) * 0.6931471805599453f;
+                    else
+                        __stcg(reinterpret_cast<float2 *>(p.workspace + it.part_off +
+                                                          part_ml_off(it.n_heads, head, it.split, it.n_splits, M2_DV)),
+                               make_float2(m_run, l_tot));
+                }
+                if (!final_out) {
+                    __syncwarp();
+                    if (lane == 0) red_release_add(p.group_counters + (size_t)it.group_idx * kCounterStride, 1);
+                }
+            }
+        }
+        // ---- LSE combine (step a4): warp-sized units, statically assigned
+        float *wsm = reinterpret_cast<float *>(smem + M2_SMEM_STAGE) + (warp - 2) * kMaxSplits;
+        for (int u = blockIdx.x * 4 + (warp - 2); u < p.n_combine_units; u += gridDim.x * 4)
+            combine_warp_unit(p, u, wsm, lane);
+    }
+    tc_fence_before();
+    cluster_sync_all();
+    if (warp == 1) tmem_dealloc2(tmem, M2_TMEM_COLS);
+    scheduler_epilogue(p, &mi->flag);
+}
+
+// ----------------------------------------------------------------------------- host side
+// 3-D views of the arena {64 columns, rows of 576 bf16, column blocks}: boxes of 16 tokens x 9 or 2 blocks.
+bool make_mla2_tensor_maps(void *out_map9, void *out_map2, const void *arena, uint64_t total_rows)
+{
+    typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                      const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                      CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                      CUtensorMapFloatOOBfill);
+    void *ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+        return false;
+    EncodeTiledFn fn = reinterpret_cast<EncodeTiledFn>(ptr);
+    cuuint64_t dims[3] = {64, total_rows, (cuuint64_t)M2_KB};
+    cuuint64_t strides[2] = {(cuuint64_t)M2_DK * 2, 128};
+    cuuint32_t estr[3] = {1, 1, 1};
+    for (int v = 0; v < 2; ++v) {
+        cuuint32_t box[3] = {64, 16, (cuuint32_t)(v == 0 ? M2_KB : 2)};
+        CUresult r = fn(reinterpret_cast<CUtensorMap *>(v == 0 ? out_map9 : out_map2), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3,
+                        const_cast<void *>(arena), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return false;
+    }
+    return true;
+}
+
+cudaError_t launch_decode_mla2(const DecodeParams &p, const void *tmap9, const void *tmap2, int rows_per_page,
+                               int n_ctas, cudaStream_t stream)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(cp_decode_mla2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             M2_SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    int pairs = p.n_tiles;
+    if (pairs < (p.n_combine_units + 7) / 8) pairs = (p.n_combine_units + 7) / 8;
+    if (pairs > n_ctas / 2) pairs = n_ctas / 2;
+    if (pairs < 1) pairs = 1;
+    cp_decode_mla2_kernel<<<2 * pairs, M2_THREADS, M2_SMEM_BYTES, stream>>>(
+        p, *reinterpret_cast<const CUtensorMap *>(tmap9), *reinterpret_cast<const CUtensorMap *>(tmap2), rows_per_page);
+    return cudaGetLastError();
+}
+
+}  // namespace cp

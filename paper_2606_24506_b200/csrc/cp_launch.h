@@ -27,4 +27,9 @@ bool make_mla_tensor_map(void *out_map, const void *arena, uint64_t total_rows);
 cudaError_t launch_decode_mla(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas,
                               cudaStream_t stream);
 
+// tcgen05 MLA path on CTA pairs (cp_kernels_mla2.cu)
+bool make_mla2_tensor_maps(void *out_map9, void *out_map2, const void *arena, uint64_t total_rows);
+cudaError_t launch_decode_mla2(const DecodeParams &p, const void *tmap9, const void *tmap2, int rows_per_page,
+                               int n_ctas, cudaStream_t stream);
+
 }  // namespace cp

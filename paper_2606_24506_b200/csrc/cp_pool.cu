@@ -102,6 +102,8 @@ struct cp_pool {
     bool kv_tmap_ok = false;
     alignas(64) unsigned char mla_tmap[128];  // CUtensorMap of the arena for the MLA kernel
     bool mla_tmap_ok = false;
+    alignas(64) unsigned char mla2_tmap9[128], mla2_tmap2[128];   // CTA-pair MLA kernel
+    bool mla2_tmap_ok = false;
 
     // counters
     uint64_t n_launches = 0, n_plan_builds = 0, n_h2d_bytes = 0;
@@ -163,7 +165,7 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         // that with waves = w every persistent CTA gets exactly w near-equal tiles (one tile more
         // on a few CTAs would cost a whole extra tile time at the end)
         // the tcgen05 MLA kernel runs every tile as two work items (value halves)
-        bool mla_fast = k == CP_KIND_MLA && pool->opt_kernel == 0 && mla_fast_supported(P, pool->page_bytes);
+        bool mla_fast = k == CP_KIND_MLA && pool->opt_kernel != 1 && mla_fast_supported(P, pool->page_bytes);
         if (mla_fast)
             for (int b = 0; b < n; ++b) {
                 const cp_model_cfg &m = pool->models[pool->reqs[ids[b]].model];
@@ -358,9 +360,12 @@ cp_status ensure_device(cp_pool *pool)
                            make_arena_tensor_map(pool->kv_tmap, pool->arena, rows, 128, 64, pool->P);
     }
     pool->mla_tmap_ok = false;
+    pool->mla2_tmap_ok = false;
     if (mla_fast_supported((int)pool->P, pool->page_bytes)) {
         const uint64_t rows = (uint64_t)pool->num_pages * (pool->page_bytes / 1152);
         pool->mla_tmap_ok = rows < (1ull << 32) && make_mla_tensor_map(pool->mla_tmap, pool->arena, rows);
+        pool->mla2_tmap_ok = rows < (1ull << 32) &&
+                             make_mla2_tensor_maps(pool->mla2_tmap9, pool->mla2_tmap2, pool->arena, rows);
     }
     pool->n_sm = sms;
     pool->dev_ready = true;
@@ -594,7 +599,7 @@ cp_status cp_pool_set_option(cp_pool *pool, int32_t key, int64_t value)
     if (!pool) return CP_ERR_INVALID_ARG;
     switch (key) {
     case CP_OPT_KERNEL:
-        if (value < 0 || value > 1) return CP_ERR_INVALID_ARG;
+        if (value < 0 || value > 2) return CP_ERR_INVALID_ARG;
         pool->opt_kernel = (int)value; break;
     case CP_OPT_NUM_CTAS:
         if (value < 0 || value > 65536) return CP_ERR_INVALID_ARG;
@@ -722,11 +727,15 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.group_counters = (int32_t *)kp.d_counters.ptr + 32;
         const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
         cudaError_t e;
-        if (k == CP_KIND_KV && pool->opt_kernel == 0 && kp.all_fast && pool->kv_tmap_ok) {
+        if (k == CP_KIND_KV && pool->opt_kernel != 1 && kp.all_fast && pool->kv_tmap_ok) {
             // warp-sized combine units, popped warp by warp after the tiles
             prm.n_combine_units = (int)kp.cunits.size();
             e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256),
                                  std::min(n_ctas, pool->n_sm), s);
+        } else if (k == CP_KIND_MLA && pool->opt_kernel == 2 && kp.all_fast && pool->mla2_tmap_ok) {
+            prm.n_combine_units = (int)kp.cunits.size();
+            e = launch_decode_mla2(prm, pool->mla2_tmap9, pool->mla2_tmap2, (int)(pool->page_bytes / 1152),
+                                   std::min(n_ctas, pool->n_sm), s);
         } else if (k == CP_KIND_MLA && pool->opt_kernel == 0 && kp.all_fast && pool->mla_tmap_ok) {
             prm.n_combine_units = (int)kp.cunits.size();
             e = launch_decode_mla(prm, pool->mla_tmap, (int)(pool->page_bytes / 1152),
