@@ -35,13 +35,14 @@ namespace cp {
 constexpr int M2_DK = 576, M2_DV = 512;
 constexpr int M2_TS = 32;                           // tokens per slice (16 per CTA for the score MMA)
 constexpr int M2_KB = 9;                            // 64-column blocks of the latent row
-constexpr int M2_STAGES = 4;
+constexpr int M2_STAGES = 6;
 constexpr int M2_BLK = 16 * 128;                    // one [16 x 64] swizzled tile: 2048 bytes
 constexpr int M2_SAREA = M2_KB * M2_BLK;            // 18432
 constexpr int M2_PVAREA = 2 * 2 * 2 * M2_BLK;       // 16384: [kk][j][2 blocks]
 constexpr int M2_STAGE_BYTES = M2_SAREA + M2_PVAREA;        // 34816
 constexpr int M2_QBLK = 64 * 128;                   // one [64 x 64] K-major tile of this CTA's query rows
-constexpr int M2_Q_BYTES = M2_KB * M2_QBLK;         // 73728
+constexpr int M2_KB_TMEM = 7;                       // query column blocks 0..6 live in TMEM (A operand, TS mode)
+constexpr int M2_Q_BYTES = (M2_KB - M2_KB_TMEM) * M2_QBLK;   // 16384: blocks 7, 8 in shared memory
 constexpr int M2_P_BYTES = 64 * M2_TS * 2;          // 4096
 constexpr int M2_THREADS = 192;
 constexpr int M2_SMEM_Q = 0;
@@ -51,7 +52,9 @@ constexpr int M2_SMEM_MISC = M2_SMEM_P + M2_P_BYTES;
 constexpr int M2_SMEM_BYTES = M2_SMEM_MISC + 2048;
 static_assert(M2_SMEM_BYTES <= 232448, "MLA pair kernel exceeds the 227 KB shared-memory limit");
 constexpr uint32_t M2_TMEM_COLS = 512;
-constexpr uint32_t M2_TMEM_S0 = 256, M2_TMEM_S1 = 288;      // score buffers: 16 columns each (2 x 2 layout)
+constexpr uint32_t M2_TMEM_S0 = 256, M2_TMEM_S1 = 272;      // score buffers: 16 columns each (2 x 2 layout)
+constexpr uint32_t M2_TMEM_Q = 288;                         // 224 columns: Q[:, 0:448) as bf16 pairs, rows duplicated in lanes 64..127
+static_assert(M2_TMEM_Q + M2_KB_TMEM * 32 <= M2_TMEM_COLS, "TMEM budget");
 constexpr float M2_LAZY_LOG2 = 8.0f;
 
 struct M2Misc {
@@ -212,9 +215,13 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                         for (int kb = 0; kb < M2_KB; ++kb)
 #pragma unroll
                             for (int j = 0; j < 4; ++j) {
-                                const uint64_t ad = umma_smem_desc(q_base + kb * M2_QBLK + j * 32, 16, 1024, 2);
                                 const uint64_t bd = umma_smem_desc(c0 + kb * M2_BLK + j * 32, 16, 1024, 2);
-                                umma2_bf16_ss(dcol, ad, bd, IDESC_S, (kb | j) != 0);
+                                if (kb < M2_KB_TMEM) {
+                                    umma2_bf16_ts(dcol, tmem + M2_TMEM_Q + kb * 32 + j * 8, bd, IDESC_S, (kb | j) != 0);
+                                } else {
+                                    const uint64_t ad = umma_smem_desc(q_base + (kb - M2_KB_TMEM) * M2_QBLK + j * 32, 16, 1024, 2);
+                                    umma2_bf16_ss(dcol, ad, bd, IDESC_S, 1);
+                                }
                             }
                         umma2_commit(smem_u32(&mi->s_full[b]));
                     }
@@ -260,17 +267,47 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             const M2Item it = m2_item(p, pair + k * n_pairs);
             if (!it.valid) break;
             if (it.group_idx != prev_group) {
-                // stage this CTA's 64 query rows as 9 K-major [64 x 64] tiles, 128-byte swizzle; rows >= Hq zero
+                // stage this CTA's 64 query rows.  Column blocks 0..6 go to tensor memory as the A operand of
+                // the TS-mode score MMAs: lane = row, two bf16 per 32-bit column, and for a pair MMA the rows
+                // are duplicated in lanes 64..127 -- exactly this thread layout (row = L % 64).  Blocks 7, 8 go
+                // to shared memory as K-major [64 x 64] tiles with the 128-byte swizzle.  Rows >= Hq are zero.
                 prev_group = it.group_idx;
-                const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + it.q_off) + (int64_t)rank * 64 * (M2_DK / 8);
-#pragma unroll 8
-                for (int id = st; id < 64 * (M2_DK / 8); id += 128) {
-                    const int r = id / (M2_DK / 8), ch = id % (M2_DK / 8);
-                    uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                    if ((int)rank * 64 + r < it.n_heads) v = __ldg(qg + id);
-                    const uint32_t a = q_base + (ch >> 3) * M2_QBLK + r * 128 + (((ch & 7) ^ (r & 7)) << 4);
-                    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+                {
+                    const uint4 *qr = reinterpret_cast<const uint4 *>(p.q + it.q_off + (int64_t)head * M2_DK);
+                    const bool live = head < it.n_heads;
+                    for (int c0 = 0; c0 < M2_KB_TMEM * 32; c0 += 32) {    // 32 columns = 64 bf16 = 8 x 16 B
+                        uint4 v[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            v[i] = make_uint4(0u, 0u, 0u, 0u);
+                            if (live) v[i] = __ldg(qr + c0 / 4 + i);
+                        }
+#pragma unroll
+                        for (int b2 = 0; b2 < 2; ++b2) {
+                            uint32_t w[16];
+#pragma unroll
+                            for (int v4 = 0; v4 < 4; ++v4) {
+                                w[4 * v4] = v[4 * b2 + v4].x; w[4 * v4 + 1] = v[4 * b2 + v4].y;
+                                w[4 * v4 + 2] = v[4 * b2 + v4].z; w[4 * v4 + 3] = v[4 * b2 + v4].w;
+                            }
+                            tmem_st16(tl + M2_TMEM_Q + c0 + b2 * 16, w);
+                        }
+                    }
+                    tmem_wait_st();
                 }
+                {
+                    constexpr int CPR = (M2_KB - M2_KB_TMEM) * 8;        // 16-B chunks per row in shared memory
+                    const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + it.q_off) + (int64_t)rank * 64 * (M2_DK / 8);
+#pragma unroll 8
+                    for (int id = st; id < 64 * CPR; id += 128) {
+                        const int r = id / CPR, ch = id % CPR;
+                        uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                        if ((int)rank * 64 + r < it.n_heads) v = __ldg(qg + r * (M2_DK / 8) + M2_KB_TMEM * 8 + ch);
+                        const uint32_t a = q_base + (ch >> 3) * M2_QBLK + r * 128 + (((ch & 7) ^ (r & 7)) << 4);
+                        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+                    }
+                }
+                tc_fence_before();
                 fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(L_q_full);
