@@ -32,6 +32,23 @@
 
 namespace cp {
 
+#ifdef CP_KV_PROBE_TIMING        /* probe builds only */
+__device__ unsigned long long cp_mla2_probe_ts[160 * 32];
+__device__ __forceinline__ void m2_stamp(int k)
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    cp_mla2_probe_ts[blockIdx.x * 32 + k] = t;
+}
+#define M2_STAMP(k, cond) do { if (cond) m2_stamp(k); } while (0)
+extern "C" int cp_mla2_probe_read(unsigned long long *out_host)
+{
+    return (int)cudaMemcpyFromSymbol(out_host, cp_mla2_probe_ts, sizeof(cp_mla2_probe_ts));
+}
+#else
+#define M2_STAMP(k, cond) do { } while (0)
+#endif
+
 constexpr int M2_DK = 576, M2_DV = 512;
 constexpr int M2_TS = 32;                           // tokens per slice (16 per CTA for the score MMA)
 constexpr int M2_KB = 9;                            // 64-column blocks of the latent row
@@ -116,6 +133,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     const uint32_t q_base = smem_u32(smem + M2_SMEM_Q);
     const uint32_t st_base = smem_u32(smem + M2_SMEM_STAGE);
     const uint32_t p_base = smem_u32(smem + M2_SMEM_P);
+    M2_STAMP(16, tid == 64);
 
     if (tid == 0) {
         for (int i = 0; i < M2_STAGES; ++i) {
@@ -204,9 +222,13 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             for (int i = 0; i <= n; ++i) {
                 if (i < n) {
                     const uint32_t g = gs + (uint32_t)i, slot = g % M2_STAGES, b = g & 1;
+                    M2_STAMP(0, lane == 0 && i == 50);
                     mbar_wait(smem_u32(&mi->full[slot]), (g / M2_STAGES) & 1);
+                    M2_STAMP(1, lane == 0 && i == 50);
                     mbar_wait_cluster(smem_u32(&mi->full_peer[slot]), (g / M2_STAGES) & 1);
+                    M2_STAMP(2, lane == 0 && i == 50);
                     mbar_wait_cluster(smem_u32(&mi->s_empty[b]), ((g >> 1) & 1) ^ 1);
+                    M2_STAMP(3, lane == 0 && i == 50);
                     tc_fence_after();
                     if (elect_one()) {
                         const uint32_t c0 = st_base + slot * M2_STAGE_BYTES;
@@ -226,10 +248,12 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                         umma2_commit(smem_u32(&mi->s_full[b]));
                     }
                     __syncwarp();
+                    M2_STAMP(4, lane == 0 && i == 50);
                 }
                 if (i >= 1) {
                     const uint32_t g = gs + (uint32_t)i - 1, slot = g % M2_STAGES;
                     mbar_wait_cluster(smem_u32(&mi->p_full), g & 1);
+                    M2_STAMP(5, lane == 0 && i == 50);
                     tc_fence_after();
                     if (elect_one()) {
                         const uint32_t pv = st_base + slot * M2_STAGE_BYTES + M2_SAREA;
@@ -247,6 +271,8 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                         umma2_commit(smem_u32(&mi->p_done));
                     }
                     __syncwarp();
+                    M2_STAMP(6, lane == 0 && i == 50);
+                    M2_STAMP(7, lane == 0 && i == 51);
                 }
             }
             gs += (uint32_t)n;
@@ -312,11 +338,14 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(L_q_full);
             }
+            M2_STAMP(18, tid == 64 && k == 0);
             float m_run = -INFINITY, l_run = 0.f;
             const int n = it.n_slices;
             for (int i = 0; i < n; ++i) {
                 const uint32_t g = gs + (uint32_t)i, b = g & 1, kq = g >> 1;
+                M2_STAMP(8, tid == 64 && i == 50);
                 mbar_wait(smem_u32(&mi->s_full[b]), kq & 1);
+                M2_STAMP(9, tid == 64 && i == 50);
                 tc_fence_after();
                 uint32_t sr[16];
                 tmem_ld16(tl + (b ? M2_TMEM_S1 : M2_TMEM_S0), sr);
@@ -336,6 +365,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 mi->xmax[b][L] = mx;
                 asm volatile("bar.sync 2, 128;" ::: "memory");
                 mx = fmaxf(mx, mi->xmax[b][L ^ 64]);
+                M2_STAMP(10, tid == 64 && i == 50);
                 const float m_new = (mx > m_run + M2_LAZY_LOG2) ? mx : m_run;
                 const bool need = (m_new != m_run) && i > 0;
                 const float a_resc = ex2_ftz(m_run - m_new);
@@ -349,7 +379,9 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pw[j]) : "f"(p1), "f"(p0));
                 }
                 l_run += sum;
+                M2_STAMP(11, tid == 64 && i == 50);
                 mbar_wait(smem_u32(&mi->p_done), (g & 1) ^ 1);       // P buffer free, O quiescent
+                M2_STAMP(12, tid == 64 && i == 50);
                 if (__any_sync(0xffffffffu, need)) {
                     tc_fence_after();
                     const float a = need ? a_resc : 1.f;
@@ -381,6 +413,10 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(L_p_full);
+                M2_STAMP(13, tid == 64 && i == 50);
+                M2_STAMP(14, tid == 64 && i == 51);
+                M2_STAMP(19, tid == 64 && i == 0);
+                M2_STAMP(20, tid == 64 && i == n - 1);
             }
             gs += (uint32_t)n;
 
@@ -423,12 +459,14 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                     __syncwarp();
                     if (lane == 0) red_release_add(p.group_counters + (size_t)it.group_idx * kCounterStride, 1);
                 }
+                M2_STAMP(21, tid == 64);
             }
         }
         // ---- LSE combine (step a4): warp-sized units, statically assigned
         float *wsm = reinterpret_cast<float *>(smem + M2_SMEM_STAGE) + (warp - 2) * kMaxSplits;
         for (int u = blockIdx.x * 4 + (warp - 2); u < p.n_combine_units; u += gridDim.x * 4)
             combine_warp_unit(p, u, wsm, lane);
+        M2_STAMP(22, tid == 64);
     }
     tc_fence_before();
     cluster_sync_all();
