@@ -85,8 +85,10 @@ typedef struct {
 
 /* Tunables (cp_pool_set_option). */
 enum {
-    CP_OPT_KERNEL = 0,       /* 0 = auto (tensor-core kernels where the shape allows),
-                                1 = force the generic SIMT kernel (any supported shape)      */
+    CP_OPT_KERNEL = 0,       /* 0 = auto (tensor-core kernels where the shape allows; MLA on CTA
+                                    pairs, tcgen05 cta_group::2),
+                                1 = force the generic SIMT kernel (any supported shape),
+                                2 = as 0, but MLA on the single-CTA tcgen05 kernel           */
     CP_OPT_NUM_CTAS = 1,     /* persistent grid size; 0 = number of SMs of the device       */
     CP_OPT_WAVES_X16 = 2,    /* target tiles per CTA, in 1/16 units (default 16 = 1.0)      */
     CP_OPT_MIN_TILE_PAGES = 3 /* lower bound on pages per tile (default 2)                   */

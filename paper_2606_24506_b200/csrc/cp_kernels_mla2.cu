@@ -462,9 +462,14 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 M2_STAMP(21, tid == 64);
             }
         }
-        // ---- LSE combine (step a4): warp-sized units, statically assigned
-        float *wsm = reinterpret_cast<float *>(smem + M2_SMEM_STAGE) + (warp - 2) * kMaxSplits;
-        for (int u = blockIdx.x * 4 + (warp - 2); u < p.n_combine_units; u += gridDim.x * 4)
+    }
+    // ---- LSE combine (step a4): warp-sized units, statically assigned to ALL six warps of every CTA.
+    // The barrier orders it after this CTA's last tile (every slice consumed, every MMA complete),
+    // so the slice stages can serve as the warps' scratch.
+    __syncthreads();
+    {
+        float *wsm = reinterpret_cast<float *>(smem + M2_SMEM_STAGE) + warp * kMaxSplits;
+        for (int u = blockIdx.x * 6 + warp; u < p.n_combine_units; u += gridDim.x * 6)
             combine_warp_unit(p, u, wsm, lane);
         M2_STAMP(22, tid == 64);
     }

@@ -732,11 +732,11 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
             prm.n_combine_units = (int)kp.cunits.size();
             e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256),
                                  std::min(n_ctas, pool->n_sm), s);
-        } else if (k == CP_KIND_MLA && pool->opt_kernel == 2 && kp.all_fast && pool->mla2_tmap_ok) {
+        } else if (k == CP_KIND_MLA && pool->opt_kernel == 0 && kp.all_fast && pool->mla2_tmap_ok) {
             prm.n_combine_units = (int)kp.cunits.size();
             e = launch_decode_mla2(prm, pool->mla2_tmap9, pool->mla2_tmap2, (int)(pool->page_bytes / 1152),
                                    std::min(n_ctas, pool->n_sm), s);
-        } else if (k == CP_KIND_MLA && pool->opt_kernel == 0 && kp.all_fast && pool->mla_tmap_ok) {
+        } else if (k == CP_KIND_MLA && pool->opt_kernel != 1 && kp.all_fast && pool->mla_tmap_ok) {
             prm.n_combine_units = (int)kp.cunits.size();
             e = launch_decode_mla(prm, pool->mla_tmap, (int)(pool->page_bytes / 1152),
                                   std::min(n_ctas, pool->n_sm), s);

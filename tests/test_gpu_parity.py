@@ -121,7 +121,7 @@ SMALL = [
 
 
 @pytest.mark.parametrize("case", range(len(SMALL)))
-@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("kernel", [0, 1, 2])
 def test_attention_small(torch_cuda, case, kernel):
     import paper_2606_24506_b200 as cp
     models, rm, rc, P, shift = SMALL[case]
@@ -149,7 +149,7 @@ def test_outputs_of_order_one_mla(torch_cuda):
     pid = int(r.page_ids[1234 // 64])
     row = w.arena.reshape(w.num_pages, -1)[pid].reshape(64, 576)
     row[1234 % 64] = W.f32_to_bf16((direction * 6.0 + 1.0).astype(np.float32))
-    for kernel in (0, 1):
+    for kernel in (0, 1, 2):
         worst = run_and_compare(w, "mla_O1/k%d" % kernel, {cp.CP_OPT_KERNEL: kernel})
         print(worst)
 
@@ -192,7 +192,7 @@ def test_rising_logits_move_the_softmax_reference(torch_cuda, kind):
         _add_logit_ramp(w, 0, 240.0, list(range(512, 576)))      # rope part only: values untouched
     ref_lse = oracle.decode_workload(w)[0][1]
     assert ref_lse.max() - ref_lse.min() >= 0 and ref_lse.max() > 30.0     # the ramp is really there
-    for kernel in (0, 1):
+    for kernel in (0, 1, 2):
         for mtp in (1, 100000):                                  # many short tiles / one tile per group
             worst = run_and_compare(w, "ramp_%s/k%d/mtp%d" % (kind, kernel, mtp),
                                     {cp.CP_OPT_KERNEL: kernel, cp.CP_OPT_MIN_TILE_PAGES: mtp})
@@ -348,3 +348,11 @@ def test_attention_full_config_generic_kernel(torch_cuda, k):
     w = W.config(k) if k == 2 else W.config3(ctx=(16384, 4096))
     worst = run_and_compare(w, "cfg%d-generic" % k, {cp.CP_OPT_KERNEL: 1})
     print("cfg%d generic: %s" % (k, worst))
+
+
+def test_attention_full_config_mla_single_cta_kernel(torch_cuda):
+    """cfg3 at full size on the single-CTA tcgen05 MLA kernel (CP_OPT_KERNEL = 2); the default
+    path (CTA pairs) is covered by test_attention_full_config."""
+    import paper_2606_24506_b200 as cp
+    worst = run_and_compare(W.config(3), "cfg3-single-cta", {cp.CP_OPT_KERNEL: 2})
+    print("cfg3 single-CTA kernel: %s" % worst)
