@@ -179,68 +179,103 @@ __device__ __forceinline__ float ex2_ftz(float x)     // 2^x; ex2(-inf) = 0
     return r;
 }
 
-// Deliberately compact (short loops unrolled by 4, 32-bit offsets): the code runs once per
+// Deliberately compact (short loops, 32-bit offsets): the code runs once per
 // launch per warp, so its cost is dominated by cold instruction-cache misses, not by issue slots.
-static __device__ __noinline__ void combine_warp_unit(const DecodeParams &p, const int u, float *wsm, const int lane)
+__device__ __forceinline__ CombineUnit load_combine_unit(const CombineUnit *units, int u)
 {
     CombineUnit cu;
-    {
-        const uint4 *src = reinterpret_cast<const uint4 *>(p.cunits + u);
-        uint4 *dst = reinterpret_cast<uint4 *>(&cu);
+    const uint4 *src = reinterpret_cast<const uint4 *>(units + u);
+    uint4 *dst = reinterpret_cast<uint4 *>(&cu);
 #pragma unroll
-        for (int i = 0; i < 4; ++i) dst[i] = __ldg(src + i);
-    }
-    KV_STAMP(8, threadIdx.x == 0);
-    const int ns = cu.n_splits;
-    const int zl = cu.zl_log2;
-    const int ZL = 1 << zl, CQ = 32 >> zl;
-    const int z = lane >> (5 - zl), cq = lane & (CQ - 1);
-    if (lane == 0) wait_group(p.group_counters, cu.group, cu.want);
-    __syncwarp();
-    KV_STAMP(9, threadIdx.x == 0);
-    const float2 *mlp = reinterpret_cast<const float2 *>(p.workspace + cu.ml_off);
-    const float *src = p.workspace + cu.part_off + cq * 4;
-    const int ss = cu.split_stride;
+    for (int i = 0; i < 4; ++i) dst[i] = __ldg(src + i);
+    return cu;
+}
 
-    // pass 1: M = max_s m_s (lane-strided, then a fixed tree)
-    float M = -INFINITY;
+// Runs the units first, first + stride, ... of one warp.  U3 = loads in flight per lane in the O
+// pass.  The record of the next unit is fetched while the current one is combined, and a group
+// already seen complete is not polled again (units are sorted by group).
+template <int U3>
+static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, const int stride, float *wsm, const int lane)
+{
+    if (u >= p.n_combine_units) return;
+    CombineUnit cu = load_combine_unit(p.cunits, u);
+    int done_group = -1;
+    for (;;) {
+        const int un = u + stride;
+        const bool has_next = un < p.n_combine_units;
+        CombineUnit nx;
+        if (has_next) nx = load_combine_unit(p.cunits, un);
+        KV_STAMP(8, threadIdx.x == 0);
+        const int ns = cu.n_splits;
+        const int zl = cu.zl_log2;
+        const int ZL = 1 << zl, CQ = 32 >> zl;
+        const int z = lane >> (5 - zl), cq = lane & (CQ - 1);
+        if (cu.group != done_group) {
+            if (lane == 0) wait_group(p.group_counters, cu.group, cu.want);
+            __syncwarp();
+            done_group = cu.group;
+        }
+        KV_STAMP(9, threadIdx.x == 0);
+        const float2 *mlp = reinterpret_cast<const float2 *>(p.workspace + cu.ml_off);
+        const float *src = p.workspace + cu.part_off + cq * 4;
+        const int ss = cu.split_stride;
+
+        float M = -INFINITY, L = 0.f;
+        if (ns <= 64) {
+            // (m, l) of splits lane and lane + 32 stay in registers: one round trip for both passes
+            float2 a = make_float2(-INFINITY, 0.f), b = make_float2(-INFINITY, 0.f);
+            if (lane < ns) a = __ldcg(mlp + lane);
+            if (lane + 32 < ns) b = __ldcg(mlp + lane + 32);
+            M = fmaxf(a.x, b.x);
+            for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+            const float wa = ex2_ftz(a.x - M), wb = ex2_ftz(b.x - M);     // 0 for absent splits (m = -inf)
+            if (lane < ns) wsm[lane] = wa;
+            if (lane + 32 < ns) wsm[lane + 32] = wb;
+            L = wa * a.y;
+            L += wb * b.y;
+        } else {
+            // pass 1: M = max_s m_s (lane-strided, then a fixed tree)
 #pragma unroll 8
-    for (int s = lane; s < ns; s += 32) M = fmaxf(M, __ldcg(mlp + s).x);
-    for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
-    // pass 2: weights w_s = 2^(m_s - M) to shared memory, L = sum_s w_s l_s
-    float L = 0.f;
+            for (int s = lane; s < ns; s += 32) M = fmaxf(M, __ldcg(mlp + s).x);
+            for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+            // pass 2: weights w_s = 2^(m_s - M) to shared memory, L = sum_s w_s l_s
 #pragma unroll 8
-    for (int s = lane; s < ns; s += 32) {
-        const float2 ml = __ldcg(mlp + s);
-        const float w = ex2_ftz(ml.x - M);
-        wsm[s] = w;
-        L += w * ml.y;
+            for (int s = lane; s < ns; s += 32) {
+                const float2 ml = __ldcg(mlp + s);
+                const float w = ex2_ftz(ml.x - M);
+                wsm[s] = w;
+                L += w * ml.y;
+            }
+        }
+        for (int o = 16; o > 0; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
+        __syncwarp();
+        KV_STAMP(10, threadIdx.x == 0);
+        // pass 3: O = sum_s w_s O_s over this lane's splits z, z + ZL, ... (in order), then the tree
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll U3
+        for (int s = z; s < ns; s += ZL) {
+            const float4 v = ld_cg_f4(src + s * ss);
+            const float w = wsm[s];
+            acc.x += w * v.x; acc.y += w * v.y; acc.z += w * v.z; acc.w += w * v.w;
+        }
+        for (int o = CQ; o < 32; o <<= 1) {               // warp-uniform trip count
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
+            acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+            acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
+            acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
+        }
+        if (z == 0) {
+            const float invL = 1.0f / L;
+            *reinterpret_cast<float4 *>(p.out + cu.out_off + cq * 4) =
+                make_float4(acc.x * invL, acc.y * invL, acc.z * invL, acc.w * invL);
+        }
+        if (cu.lse_off >= 0 && lane == 0) p.lse[cu.lse_off] = (M + log2f(L)) * 0.6931471805599453f;
+        __syncwarp();               // wsm is reused by this warp's next unit
+        KV_STAMP(11, threadIdx.x == 0);
+        if (!has_next) break;
+        cu = nx;
+        u = un;
     }
-    for (int o = 16; o > 0; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
-    __syncwarp();
-    KV_STAMP(10, threadIdx.x == 0);
-    // pass 3: O = sum_s w_s O_s over this lane's splits z, z + ZL, ... (in order), then the tree
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll 8
-    for (int s = z; s < ns; s += ZL) {
-        const float4 v = ld_cg_f4(src + s * ss);
-        const float w = wsm[s];
-        acc.x += w * v.x; acc.y += w * v.y; acc.z += w * v.z; acc.w += w * v.w;
-    }
-    for (int o = CQ; o < 32; o <<= 1) {               // warp-uniform trip count
-        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
-        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
-        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
-        acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
-    }
-    if (z == 0) {
-        const float invL = 1.0f / L;
-        *reinterpret_cast<float4 *>(p.out + cu.out_off + cq * 4) =
-            make_float4(acc.x * invL, acc.y * invL, acc.z * invL, acc.w * invL);
-    }
-    if (cu.lse_off >= 0 && lane == 0) p.lse[cu.lse_off] = (M + log2f(L)) * 0.6931471805599453f;
-    __syncwarp();               // wsm is reused by this warp's next unit
-    KV_STAMP(11, threadIdx.x == 0);
 }
 
 // Persistent-scheduler epilogue: the last CTA to finish resets the counters so that the

@@ -531,8 +531,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
         // the spin inside terminates.
         // Units are assigned statically (unit u -> consumer warp u mod #warps of the grid): popping
         // them from one counter would serialise thousands of same-address atomics at the L2.
-        for (int u = blockIdx.x * KV_CWARPS + warp; u < p.n_combine_units; u += gridDim.x * KV_CWARPS)
-            combine_warp_unit(p, u, merge + warp * KV_COMBINE_WARP_FLOATS, lane);
+        combine_units<8>(p, blockIdx.x * KV_CWARPS + warp, gridDim.x * KV_CWARPS, merge + warp * KV_COMBINE_WARP_FLOATS, lane);
 #endif
         KV_STAMP(6, tid == 0);
     }

@@ -468,8 +468,7 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
         }
         // ---- LSE combine (step a4): warp-sized units, statically assigned (see the MQA/GQA kernel)
         float *wsm = reinterpret_cast<float *>(smem + MLA_SMEM_P) + (warp - 2) * kMaxSplits;
-        for (int u = blockIdx.x * 4 + (warp - 2); u < p.n_combine_units; u += gridDim.x * 4)
-            combine_warp_unit(p, u, wsm, lane);
+        combine_units<16>(p, blockIdx.x * 4 + (warp - 2), gridDim.x * 4, wsm, lane);
         MLA_STAMP(22, tid == 64);
     }
     tc_fence_before();

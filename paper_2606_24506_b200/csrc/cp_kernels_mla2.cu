@@ -26,12 +26,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstdint>
-#include "cp_device_common.cuh"
-#include "cp_launch.h"
-#include "cp_ptx.cuh"
-
 namespace cp {
-
 #ifdef CP_KV_PROBE_TIMING        /* probe builds only */
 __device__ unsigned long long cp_mla2_probe_ts[160 * 32];
 __device__ __forceinline__ void m2_stamp(int k)
@@ -48,6 +43,16 @@ extern "C" int cp_mla2_probe_read(unsigned long long *out_host)
 #else
 #define M2_STAMP(k, cond) do { } while (0)
 #endif
+
+}  // namespace cp
+#ifdef CP_KV_PROBE_TIMING
+#define KV_STAMP(k, cond) M2_STAMP(16 + (k), cond)
+#endif
+#include "cp_device_common.cuh"
+#include "cp_launch.h"
+#include "cp_ptx.cuh"
+
+namespace cp {
 
 constexpr int M2_DK = 576, M2_DV = 512;
 constexpr int M2_TS = 32;                           // tokens per slice (16 per CTA for the score MMA)
@@ -469,8 +474,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     __syncthreads();
     {
         float *wsm = reinterpret_cast<float *>(smem + M2_SMEM_STAGE) + warp * kMaxSplits;
-        for (int u = blockIdx.x * 6 + warp; u < p.n_combine_units; u += gridDim.x * 6)
-            combine_warp_unit(p, u, wsm, lane);
+        combine_units<16>(p, blockIdx.x * 6 + warp, gridDim.x * 6, wsm, lane);
         M2_STAMP(22, tid == 64);
     }
     tc_fence_before();
