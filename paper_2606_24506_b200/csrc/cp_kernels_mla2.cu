@@ -57,14 +57,14 @@ namespace cp {
 constexpr int M2_DK = 576, M2_DV = 512;
 constexpr int M2_TS = 32;                           // tokens per slice (16 per CTA for the score MMA)
 constexpr int M2_KB = 9;                            // 64-column blocks of the latent row
-constexpr int M2_STAGES = 6;
+constexpr int M2_STAGES = 5;
 constexpr int M2_BLK = 16 * 128;                    // one [16 x 64] swizzled tile: 2048 bytes
 constexpr int M2_SAREA = M2_KB * M2_BLK;            // 18432
 constexpr int M2_PVAREA = 2 * 2 * 2 * M2_BLK;       // 16384: [kk][j][2 blocks]
 constexpr int M2_STAGE_BYTES = M2_SAREA + M2_PVAREA;        // 34816
 constexpr int M2_QBLK = 64 * 128;                   // one [64 x 64] K-major tile of this CTA's query rows
-constexpr int M2_KB_TMEM = 7;                       // query column blocks 0..6 live in TMEM (A operand, TS mode)
-constexpr int M2_Q_BYTES = (M2_KB - M2_KB_TMEM) * M2_QBLK;   // 16384: blocks 7, 8 in shared memory
+constexpr int M2_KB_TMEM = 6;                       // query column blocks 0..5 live in TMEM (A operand, TS mode)
+constexpr int M2_Q_BYTES = (M2_KB - M2_KB_TMEM) * M2_QBLK;   // 24576: blocks 6..8 in shared memory
 constexpr int M2_P_BYTES = 64 * M2_TS * 2;          // 4096
 constexpr int M2_THREADS = 192;
 constexpr int M2_SMEM_Q = 0;
@@ -74,8 +74,9 @@ constexpr int M2_SMEM_MISC = M2_SMEM_P + M2_P_BYTES;
 constexpr int M2_SMEM_BYTES = M2_SMEM_MISC + 2048;
 static_assert(M2_SMEM_BYTES <= 232448, "MLA pair kernel exceeds the 227 KB shared-memory limit");
 constexpr uint32_t M2_TMEM_COLS = 512;
-constexpr uint32_t M2_TMEM_S0 = 256, M2_TMEM_S1 = 272;      // score buffers: 16 columns each (2 x 2 layout)
-constexpr uint32_t M2_TMEM_Q = 288;                         // 224 columns: Q[:, 0:448) as bf16 pairs, rows duplicated in lanes 64..127
+constexpr int M2_SB = 3;                            // score buffers: the issuer runs two slices ahead of the value MMAs
+constexpr uint32_t M2_TMEM_S = 256;                         // score buffer b at 256 + 16 b: 16 columns each (2 x 2 layout)
+constexpr uint32_t M2_TMEM_Q = 304;                         // 192 columns: Q[:, 0:384) as bf16 pairs, rows duplicated in lanes 64..127
 static_assert(M2_TMEM_Q + M2_KB_TMEM * 32 <= M2_TMEM_COLS, "TMEM budget");
 constexpr float M2_LAZY_LOG2 = 8.0f;
 
@@ -83,8 +84,8 @@ struct M2Misc {
     uint64_t full[M2_STAGES];       // local TMA landed (this CTA's part of the slice)
     uint64_t full_peer[M2_STAGES];  // leader only: the peer's part landed (arrived by the peer's relay warp)
     uint64_t empty[M2_STAGES];      // pair-MMA commit (multicast): stage free
-    uint64_t s_full[2];             // pair-MMA commit (multicast): scores ready
-    uint64_t s_empty[2];            // leader only: 8 softmax warps of the pair have read the scores
+    uint64_t s_full[M2_SB];         // pair-MMA commit (multicast): scores ready
+    uint64_t s_empty[M2_SB];        // leader only: 8 softmax warps of the pair have read the scores
     uint64_t p_full;                // leader only: 8 softmax warps have written P
     uint64_t p_done;                // pair-MMA commit (multicast): value MMAs of the slice complete
     uint64_t q_full;                // leader only: 8 softmax warps have staged the query rows
@@ -145,7 +146,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             mbar_init(smem_u32(&mi->full[i]), 1); mbar_init(smem_u32(&mi->full_peer[i]), 1);
             mbar_init(smem_u32(&mi->empty[i]), 1);
         }
-        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&mi->s_full[i]), 1); mbar_init(smem_u32(&mi->s_empty[i]), 8); }
+        for (int i = 0; i < M2_SB; ++i) { mbar_init(smem_u32(&mi->s_full[i]), 1); mbar_init(smem_u32(&mi->s_empty[i]), 8); }
         mbar_init(smem_u32(&mi->p_full), 8); mbar_init(smem_u32(&mi->p_done), 1);
         mbar_init(smem_u32(&mi->q_full), 8);
         asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap9)) : "memory");
@@ -161,7 +162,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     const int P = (int)p.page_tokens;
     const int spp = P / M2_TS;
     // leader's barriers as seen from this CTA (own address in the leader, mapped address in the peer)
-    const uint32_t L_s_empty0 = mapa_u32(smem_u32(&mi->s_empty[0]), 0), L_s_empty1 = mapa_u32(smem_u32(&mi->s_empty[1]), 0);
+    const uint32_t L_s_empty = mapa_u32(smem_u32(&mi->s_empty[0]), 0);      // + 8 b for buffer b
     const uint32_t L_p_full = mapa_u32(smem_u32(&mi->p_full), 0), L_q_full = mapa_u32(smem_u32(&mi->q_full), 0);
 
     if (warp == 0) {
@@ -224,29 +225,31 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             if (!it.valid) break;
             if (it.group_idx != prev_group) { mbar_wait_cluster(smem_u32(&mi->q_full), qn & 1); ++qn; prev_group = it.group_idx; }
             const int n = it.n_slices;
-            for (int i = 0; i <= n; ++i) {
+            for (int i = 0; i <= n + 1; ++i) {
                 if (i < n) {
-                    const uint32_t g = gs + (uint32_t)i, slot = g % M2_STAGES, b = g & 1;
+                    const uint32_t g = gs + (uint32_t)i, slot = g % M2_STAGES, b = g % M2_SB;
                     M2_STAMP(0, lane == 0 && i == 50);
                     mbar_wait(smem_u32(&mi->full[slot]), (g / M2_STAGES) & 1);
                     M2_STAMP(1, lane == 0 && i == 50);
                     mbar_wait_cluster(smem_u32(&mi->full_peer[slot]), (g / M2_STAGES) & 1);
                     M2_STAMP(2, lane == 0 && i == 50);
-                    mbar_wait_cluster(smem_u32(&mi->s_empty[b]), ((g >> 1) & 1) ^ 1);
+                    mbar_wait_cluster(smem_u32(&mi->s_empty[b]), ((g / M2_SB) & 1) ^ 1);
                     M2_STAMP(3, lane == 0 && i == 50);
                     tc_fence_after();
                     if (elect_one()) {
                         const uint32_t c0 = st_base + slot * M2_STAGE_BYTES;
-                        const uint32_t dcol = tmem + (b ? M2_TMEM_S1 : M2_TMEM_S0);
+                        const uint32_t dcol = tmem + M2_TMEM_S + 16 * b;
+                        const uint64_t bd0 = umma_smem_desc(c0, 16, 1024, 2);
+                        const uint64_t ad0 = umma_smem_desc(q_base, 16, 1024, 2);
 #pragma unroll
                         for (int kb = 0; kb < M2_KB; ++kb)
 #pragma unroll
                             for (int j = 0; j < 4; ++j) {
-                                const uint64_t bd = umma_smem_desc(c0 + kb * M2_BLK + j * 32, 16, 1024, 2);
+                                const uint64_t bd = bd0 + (uint64_t)((kb * M2_BLK + j * 32) >> 4);      // start-address field
                                 if (kb < M2_KB_TMEM) {
                                     umma2_bf16_ts(dcol, tmem + M2_TMEM_Q + kb * 32 + j * 8, bd, IDESC_S, (kb | j) != 0);
                                 } else {
-                                    const uint64_t ad = umma_smem_desc(q_base + (kb - M2_KB_TMEM) * M2_QBLK + j * 32, 16, 1024, 2);
+                                    const uint64_t ad = ad0 + (uint64_t)(((kb - M2_KB_TMEM) * M2_QBLK + j * 32) >> 4);
                                     umma2_bf16_ss(dcol, ad, bd, IDESC_S, 1);
                                 }
                             }
@@ -255,22 +258,24 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                     __syncwarp();
                     M2_STAMP(4, lane == 0 && i == 50);
                 }
-                if (i >= 1) {
-                    const uint32_t g = gs + (uint32_t)i - 1, slot = g % M2_STAGES;
+                if (i >= 2) {
+                    const uint32_t g = gs + (uint32_t)i - 2, slot = g % M2_STAGES;
                     mbar_wait_cluster(smem_u32(&mi->p_full), g & 1);
                     M2_STAMP(5, lane == 0 && i == 50);
                     tc_fence_after();
                     if (elect_one()) {
                         const uint32_t pv = st_base + slot * M2_STAGE_BYTES + M2_SAREA;
+                        const uint64_t ad0 = umma_smem_desc(p_base, 1024, 128, 0);
+                        const uint64_t bd0 = umma_smem_desc(pv, M2_BLK, 1024, 2);
 #pragma unroll
                         for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
                             for (int jj = 0; jj < 2; ++jj) {
                                 // P: 8-token chunks of [64 rows x 16 B] 1024 B apart, 8-row groups 128 B apart
-                                const uint64_t ad = umma_smem_desc(p_base + kk * 2048, 1024, 128, 0);
+                                const uint64_t ad = ad0 + (uint64_t)((kk * 2048) >> 4);
                                 // V: two 64-column blocks 2048 B apart, 8-token groups 1024 B apart
-                                const uint64_t bd = umma_smem_desc(pv + (kk * 2 + jj) * 2 * M2_BLK, M2_BLK, 1024, 2);
-                                umma2_bf16_ss(tmem + jj * 128, ad, bd, IDESC_PV, (i > 1) || (kk > 0));
+                                const uint64_t bd = bd0 + (uint64_t)(((kk * 2 + jj) * 2 * M2_BLK) >> 4);
+                                umma2_bf16_ss(tmem + jj * 128, ad, bd, IDESC_PV, (i > 2) || (kk > 0));
                             }
                         umma2_commit(smem_u32(&mi->empty[slot]));
                         umma2_commit(smem_u32(&mi->p_done));
@@ -298,9 +303,9 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             const M2Item it = m2_item(p, pair + k * n_pairs);
             if (!it.valid) break;
             if (it.group_idx != prev_group) {
-                // stage this CTA's 64 query rows.  Column blocks 0..6 go to tensor memory as the A operand of
+                // stage this CTA's 64 query rows.  Column blocks 0..5 go to tensor memory as the A operand of
                 // the TS-mode score MMAs: lane = row, two bf16 per 32-bit column, and for a pair MMA the rows
-                // are duplicated in lanes 64..127 -- exactly this thread layout (row = L % 64).  Blocks 7, 8 go
+                // are duplicated in lanes 64..127 -- exactly this thread layout (row = L % 64).  Blocks 6..8 go
                 // to shared memory as K-major [64 x 64] tiles with the 128-byte swizzle.  Rows >= Hq are zero.
                 prev_group = it.group_idx;
                 {
@@ -347,17 +352,17 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             float m_run = -INFINITY, l_run = 0.f;
             const int n = it.n_slices;
             for (int i = 0; i < n; ++i) {
-                const uint32_t g = gs + (uint32_t)i, b = g & 1, kq = g >> 1;
+                const uint32_t g = gs + (uint32_t)i, b = g % M2_SB, kq = g / M2_SB, xb = g & 1;
                 M2_STAMP(8, tid == 64 && i == 50);
                 mbar_wait(smem_u32(&mi->s_full[b]), kq & 1);
                 M2_STAMP(9, tid == 64 && i == 50);
                 tc_fence_after();
                 uint32_t sr[16];
-                tmem_ld16(tl + (b ? M2_TMEM_S1 : M2_TMEM_S0), sr);
+                tmem_ld16(tl + M2_TMEM_S + 16 * b, sr);
                 tmem_wait_ld();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(b ? L_s_empty1 : L_s_empty0);
+                if (lane == 0) mbar_arrive_cluster(L_s_empty + 8 * b);
                 const int valid = ((i == n - 1) ? it.valid_last : M2_TS) - 16 * th;   // valid tokens of my half
                 float mx = -INFINITY;
 #pragma unroll
@@ -367,9 +372,9 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                     mx = fmaxf(mx, v);
                 }
                 // the two token halves of a head agree on the row maximum through shared memory
-                mi->xmax[b][L] = mx;
+                mi->xmax[xb][L] = mx;
                 asm volatile("bar.sync 2, 128;" ::: "memory");
-                mx = fmaxf(mx, mi->xmax[b][L ^ 64]);
+                mx = fmaxf(mx, mi->xmax[xb][L ^ 64]);
                 M2_STAMP(10, tid == 64 && i == 50);
                 const float m_new = (mx > m_run + M2_LAZY_LOG2) ? mx : m_run;
                 const bool need = (m_new != m_run) && i > 0;
