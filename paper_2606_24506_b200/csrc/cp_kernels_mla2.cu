@@ -65,12 +65,12 @@ constexpr int M2_STAGE_BYTES = M2_SAREA + M2_PVAREA;        // 34816
 constexpr int M2_QBLK = 64 * 128;                   // one [64 x 64] K-major tile of this CTA's query rows
 constexpr int M2_KB_TMEM = 6;                       // query column blocks 0..5 live in TMEM (A operand, TS mode)
 constexpr int M2_Q_BYTES = (M2_KB - M2_KB_TMEM) * M2_QBLK;   // 24576: blocks 6..8 in shared memory
-constexpr int M2_P_BYTES = 64 * M2_TS * 2;          // 4096
+constexpr int M2_P_BYTES = 64 * M2_TS * 2;          // 4096 per P buffer (two buffers)
 constexpr int M2_THREADS = 192;
 constexpr int M2_SMEM_Q = 0;
 constexpr int M2_SMEM_STAGE = M2_Q_BYTES;
 constexpr int M2_SMEM_P = M2_SMEM_STAGE + M2_STAGES * M2_STAGE_BYTES;
-constexpr int M2_SMEM_MISC = M2_SMEM_P + M2_P_BYTES;
+constexpr int M2_SMEM_MISC = M2_SMEM_P + 2 * M2_P_BYTES;
 constexpr int M2_SMEM_BYTES = M2_SMEM_MISC + 2048;
 static_assert(M2_SMEM_BYTES <= 232448, "MLA pair kernel exceeds the 227 KB shared-memory limit");
 constexpr uint32_t M2_TMEM_COLS = 512;
@@ -86,8 +86,8 @@ struct M2Misc {
     uint64_t empty[M2_STAGES];      // pair-MMA commit (multicast): stage free
     uint64_t s_full[M2_SB];         // pair-MMA commit (multicast): scores ready
     uint64_t s_empty[M2_SB];        // leader only: 8 softmax warps of the pair have read the scores
-    uint64_t p_full;                // leader only: 8 softmax warps have written P
-    uint64_t p_done;                // pair-MMA commit (multicast): value MMAs of the slice complete
+    uint64_t p_full[2];             // leader only: 8 softmax warps have written P buffer (slice & 1)
+    uint64_t p_done[2];             // pair-MMA commit (multicast): value MMAs of the slice complete
     uint64_t q_full;                // leader only: 8 softmax warps have staged the query rows
     float xmax[2][128];             // row maxima exchanged between the two token halves of a head (by slice parity)
     float xsum[128];
@@ -147,7 +147,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             mbar_init(smem_u32(&mi->empty[i]), 1);
         }
         for (int i = 0; i < M2_SB; ++i) { mbar_init(smem_u32(&mi->s_full[i]), 1); mbar_init(smem_u32(&mi->s_empty[i]), 8); }
-        mbar_init(smem_u32(&mi->p_full), 8); mbar_init(smem_u32(&mi->p_done), 1);
+        for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&mi->p_full[i]), 8); mbar_init(smem_u32(&mi->p_done[i]), 1); }
         mbar_init(smem_u32(&mi->q_full), 8);
         asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap9)) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap2)) : "memory");
@@ -163,7 +163,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     const int spp = P / M2_TS;
     // leader's barriers as seen from this CTA (own address in the leader, mapped address in the peer)
     const uint32_t L_s_empty = mapa_u32(smem_u32(&mi->s_empty[0]), 0);      // + 8 b for buffer b
-    const uint32_t L_p_full = mapa_u32(smem_u32(&mi->p_full), 0), L_q_full = mapa_u32(smem_u32(&mi->q_full), 0);
+    const uint32_t L_p_full = mapa_u32(smem_u32(&mi->p_full[0]), 0), L_q_full = mapa_u32(smem_u32(&mi->q_full), 0);
 
     if (warp == 0) {
         // =========================================================== producer warp (each CTA loads its part)
@@ -260,12 +260,12 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 }
                 if (i >= 2) {
                     const uint32_t g = gs + (uint32_t)i - 2, slot = g % M2_STAGES;
-                    mbar_wait_cluster(smem_u32(&mi->p_full), g & 1);
+                    mbar_wait_cluster(smem_u32(&mi->p_full[g & 1]), (g >> 1) & 1);
                     M2_STAMP(5, lane == 0 && i == 50);
                     tc_fence_after();
                     if (elect_one()) {
                         const uint32_t pv = st_base + slot * M2_STAGE_BYTES + M2_SAREA;
-                        const uint64_t ad0 = umma_smem_desc(p_base, 1024, 128, 0);
+                        const uint64_t ad0 = umma_smem_desc(p_base + (g & 1) * M2_P_BYTES, 1024, 128, 0);
                         const uint64_t bd0 = umma_smem_desc(pv, M2_BLK, 1024, 2);
 #pragma unroll
                         for (int kk = 0; kk < 2; ++kk)
@@ -278,7 +278,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                                 umma2_bf16_ss(tmem + jj * 128, ad, bd, IDESC_PV, (i > 2) || (kk > 0));
                             }
                         umma2_commit(smem_u32(&mi->empty[slot]));
-                        umma2_commit(smem_u32(&mi->p_done));
+                        umma2_commit(smem_u32(&mi->p_done[g & 1]));
                     }
                     __syncwarp();
                     M2_STAMP(6, lane == 0 && i == 50);
@@ -390,9 +390,11 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 }
                 l_run += sum;
                 M2_STAMP(11, tid == 64 && i == 50);
-                mbar_wait(smem_u32(&mi->p_done), (g & 1) ^ 1);       // P buffer free, O quiescent
+                mbar_wait(smem_u32(&mi->p_done[xb]), ((g >> 1) & 1) ^ 1);       // P buffer (slice & 1) free
                 M2_STAMP(12, tid == 64 && i == 50);
                 if (__any_sync(0xffffffffu, need)) {
+                    // O is rescaled in place: the value MMAs of the previous slice must be complete
+                    mbar_wait(smem_u32(&mi->p_done[(g - 1) & 1]), ((g - 1) >> 1) & 1);
                     tc_fence_after();
                     const float a = need ? a_resc : 1.f;
                     for (int c = 0; c < 256; c += 16) {
@@ -406,8 +408,8 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                     tmem_wait_st();
                 }
                 // P[row][token] as 8-token chunks of [64 rows x 16 B]: chunk c at c * 1024 + row * 16
-                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p_base + (2 * th) * 1024 + hrow * 16), "r"(pw[0]), "r"(pw[1]), "r"(pw[2]), "r"(pw[3]) : "memory");
-                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p_base + (2 * th + 1) * 1024 + hrow * 16), "r"(pw[4]), "r"(pw[5]), "r"(pw[6]), "r"(pw[7]) : "memory");
+                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p_base + xb * M2_P_BYTES + (2 * th) * 1024 + hrow * 16), "r"(pw[0]), "r"(pw[1]), "r"(pw[2]), "r"(pw[3]) : "memory");
+                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p_base + xb * M2_P_BYTES + (2 * th + 1) * 1024 + hrow * 16), "r"(pw[4]), "r"(pw[5]), "r"(pw[6]), "r"(pw[7]) : "memory");
                 if (i == n - 1 && it.valid_last < M2_TS) {
                     // dead slots of the request's last slice may hold NaN: zero their value rows in the PV area
                     // (warp q4 clears the two 64-column blocks of MMA j = q4 & 1 for k-step kk = q4 >> 1)
@@ -422,7 +424,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 fence_proxy_async();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(L_p_full);
+                if (lane == 0) mbar_arrive_cluster(L_p_full + 8 * xb);
                 M2_STAMP(13, tid == 64 && i == 50);
                 M2_STAMP(14, tid == 64 && i == 51);
                 M2_STAMP(19, tid == 64 && i == 0);
@@ -433,7 +435,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             // ---- end of tile: O rows from TMEM, publish
             {
                 const uint32_t gl = gs - 1;
-                mbar_wait(smem_u32(&mi->p_done), gl & 1);
+                mbar_wait(smem_u32(&mi->p_done[gl & 1]), (gl >> 1) & 1);
                 tc_fence_after();
                 mi->xsum[L] = l_run;
                 asm volatile("bar.sync 2, 128;" ::: "memory");
