@@ -78,6 +78,7 @@ constexpr int M2_SB = 3;                            // score buffers: the issuer
 constexpr uint32_t M2_TMEM_S = 256;                         // score buffer b at 256 + 16 b: 16 columns each (2 x 2 layout)
 constexpr uint32_t M2_TMEM_Q = 304;                         // 192 columns: Q[:, 0:384) as bf16 pairs, rows duplicated in lanes 64..127
 static_assert(M2_TMEM_Q + M2_KB_TMEM * 32 <= M2_TMEM_COLS, "TMEM budget");
+static_assert((M2_KB_TMEM * 32) % 96 == 0, "query staging batches");
 constexpr float M2_LAZY_LOG2 = 8.0f;
 
 struct M2Misc {
@@ -311,22 +312,22 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 {
                     const uint4 *qr = reinterpret_cast<const uint4 *>(p.q + it.q_off + (int64_t)head * M2_DK);
                     const bool live = head < it.n_heads;
-                    for (int c0 = 0; c0 < M2_KB_TMEM * 32; c0 += 32) {    // 32 columns = 64 bf16 = 8 x 16 B
-                        uint4 v[8];
+                    for (int c0 = 0; c0 < M2_KB_TMEM * 32; c0 += 96) {    // 96 columns = 192 bf16 = 24 x 16 B in flight
+                        uint4 v[24];
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) {
+                        for (int i = 0; i < 24; ++i) {
                             v[i] = make_uint4(0u, 0u, 0u, 0u);
                             if (live) v[i] = __ldg(qr + c0 / 4 + i);
                         }
 #pragma unroll
-                        for (int b2 = 0; b2 < 2; ++b2) {
+                        for (int b6 = 0; b6 < 6; ++b6) {
                             uint32_t w[16];
 #pragma unroll
                             for (int v4 = 0; v4 < 4; ++v4) {
-                                w[4 * v4] = v[4 * b2 + v4].x; w[4 * v4 + 1] = v[4 * b2 + v4].y;
-                                w[4 * v4 + 2] = v[4 * b2 + v4].z; w[4 * v4 + 3] = v[4 * b2 + v4].w;
+                                w[4 * v4] = v[4 * b6 + v4].x; w[4 * v4 + 1] = v[4 * b6 + v4].y;
+                                w[4 * v4 + 2] = v[4 * b6 + v4].z; w[4 * v4 + 3] = v[4 * b6 + v4].w;
                             }
-                            tmem_st16(tl + M2_TMEM_Q + c0 + b2 * 16, w);
+                            tmem_st16(tl + M2_TMEM_Q + c0 + b6 * 16, w);
                         }
                     }
                     tmem_wait_st();
@@ -334,7 +335,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 {
                     constexpr int CPR = (M2_KB - M2_KB_TMEM) * 8;        // 16-B chunks per row in shared memory
                     const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + it.q_off) + (int64_t)rank * 64 * (M2_DK / 8);
-#pragma unroll 8
+#pragma unroll 12
                     for (int id = st; id < 64 * CPR; id += 128) {
                         const int r = id / CPR, ch = id % CPR;
                         uint4 v = make_uint4(0u, 0u, 0u, 0u);
