@@ -443,20 +443,35 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 const float l_tot = th == 0 ? l_run + mi->xsum[L ^ 64] : mi->xsum[L ^ 64] + l_run;   // same order in both halves
                 const bool final_out = it.n_splits == 1;
                 const float inv = final_out ? 1.f / l_tot : 1.f;
-                float *rowp = final_out ? p.out + it.out_off + (int64_t)head * M2_DV
-                                        : p.workspace + it.part_off + part_o_off(head, it.split, it.n_splits, M2_DV);
+                // Rows leave through a per-warp transpose in shared memory (the query tiles are idle
+                // here): a thread owns a row in TMEM, but 32 lanes storing 16 B each into 32 different
+                // rows is the worst pattern for L2; after the transpose every store instruction writes
+                // 8 rows x 64 contiguous bytes.
+                const int head0 = (int)rank * 64 + (q4 & 1) * 32;            // first head of this warp's 32 rows
+                const int64_t rstride = final_out ? M2_DV : (int64_t)it.n_splits * M2_DV;
+                float *row0 = final_out ? p.out + it.out_off + (int64_t)head0 * M2_DV
+                                        : p.workspace + it.part_off + part_o_off(head0, it.split, it.n_splits, M2_DV);
+                const uint32_t scr = q_base + (uint32_t)(warp - 2) * 2560;   // [32 rows][16 floats + 4 pad]
                 for (int c = 0; c < 256; c += 16) {
                     uint32_t o[16];
                     tmem_ld16(tl + c, o);
                     tmem_wait_ld();
-                    // TMEM column c of MMA jj = c / 128 holds value column 256 jj + 128 th + c % 128 of my head
-                    float *dst = rowp + 256 * (c >> 7) + 128 * th + (c & 127);
-                    if (head < it.n_heads) {
+                    __syncwarp();                                            // previous chunk fully read back
 #pragma unroll
-                        for (int j = 0; j < 16; j += 4)
-                            __stcg(reinterpret_cast<float4 *>(dst + j),
-                                   make_float4(__uint_as_float(o[j]) * inv, __uint_as_float(o[j + 1]) * inv,
-                                               __uint_as_float(o[j + 2]) * inv, __uint_as_float(o[j + 3]) * inv));
+                    for (int j = 0; j < 16; j += 4)
+                        asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(scr + lane * 80 + j * 4),
+                                     "f"(__uint_as_float(o[j]) * inv), "f"(__uint_as_float(o[j + 1]) * inv),
+                                     "f"(__uint_as_float(o[j + 2]) * inv), "f"(__uint_as_float(o[j + 3]) * inv) : "memory");
+                    __syncwarp();
+                    // TMEM column c of MMA jj = c / 128 holds value column 256 jj + 128 th + c % 128
+                    const int col = 256 * (c >> 7) + 128 * th + (c & 127) + (lane & 3) * 4;
+#pragma unroll
+                    for (int r8 = 0; r8 < 4; ++r8) {
+                        const int r = r8 * 8 + (lane >> 2);
+                        float4 v;
+                        asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                                     : "r"(scr + r * 80 + (lane & 3) * 16) : "memory");
+                        if (head0 + r < it.n_heads) __stcg(reinterpret_cast<float4 *>(row0 + r * rstride + col), v);
                     }
                 }
                 tc_fence_before();
