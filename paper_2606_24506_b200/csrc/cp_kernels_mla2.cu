@@ -70,7 +70,8 @@ constexpr int M2_THREADS = 192;
 constexpr int M2_SMEM_Q = 0;
 constexpr int M2_SMEM_STAGE = M2_Q_BYTES;
 constexpr int M2_SMEM_P = M2_SMEM_STAGE + M2_STAGES * M2_STAGE_BYTES;
-constexpr int M2_SMEM_MISC = M2_SMEM_P + 2 * M2_P_BYTES;
+constexpr int M2_SMEM_XPOSE = M2_SMEM_P + 2 * M2_P_BYTES;   // epilogue transpose scratch: 4 warps x [32 rows][16 + 4 floats]
+constexpr int M2_SMEM_MISC = M2_SMEM_XPOSE + 4 * 2560;
 constexpr int M2_SMEM_BYTES = M2_SMEM_MISC + 2048;
 static_assert(M2_SMEM_BYTES <= 232448, "MLA pair kernel exceeds the 227 KB shared-memory limit");
 constexpr uint32_t M2_TMEM_COLS = 512;
@@ -443,15 +444,14 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 const float l_tot = th == 0 ? l_run + mi->xsum[L ^ 64] : mi->xsum[L ^ 64] + l_run;   // same order in both halves
                 const bool final_out = it.n_splits == 1;
                 const float inv = final_out ? 1.f / l_tot : 1.f;
-                // Rows leave through a per-warp transpose in shared memory (the query tiles are idle
-                // here): a thread owns a row in TMEM, but 32 lanes storing 16 B each into 32 different
+                // Rows leave through a per-warp transpose in shared memory: a thread owns a row in TMEM, but 32 lanes storing 16 B each into 32 different
                 // rows is the worst pattern for L2; after the transpose every store instruction writes
                 // 8 rows x 64 contiguous bytes.
                 const int head0 = (int)rank * 64 + (q4 & 1) * 32;            // first head of this warp's 32 rows
                 const int64_t rstride = final_out ? M2_DV : (int64_t)it.n_splits * M2_DV;
                 float *row0 = final_out ? p.out + it.out_off + (int64_t)head0 * M2_DV
                                         : p.workspace + it.part_off + part_o_off(head0, it.split, it.n_splits, M2_DV);
-                const uint32_t scr = q_base + (uint32_t)(warp - 2) * 2560;   // [32 rows][16 floats + 4 pad]
+                const uint32_t scr = smem_u32(smem + M2_SMEM_XPOSE) + (uint32_t)(warp - 2) * 2560;   // [32 rows][16 floats + 4 pad]
                 for (int c = 0; c < 256; c += 16) {
                     uint32_t o[16];
                     tmem_ld16(tl + c, o);

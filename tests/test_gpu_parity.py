@@ -199,6 +199,40 @@ def test_rising_logits_move_the_softmax_reference(torch_cuda, kind):
             print(worst)
 
 
+@pytest.mark.parametrize("n_ctas", [2, 4, 6])
+@pytest.mark.parametrize("kernel", [0, 2])
+def test_few_ctas_many_tiles_per_cta(torch_cuda, n_ctas, kernel):
+    """Persistent loops over many work items per CTA (or CTA pair): a grid of 2..6 CTAs on batches
+    that yield dozens of tiles, with group changes in between (query restaging, ring phases across
+    tiles, statically assigned combine units on a small grid)."""
+    import paper_2606_24506_b200 as cp
+    cases = [
+        ([ModelCfg(KIND_MLA, 128, 1, 576, 512, 192 ** -0.5), ModelCfg(KIND_MLA, 48, 1, 576, 512, 192 ** -0.5)],
+         [0, 1, 0], [1500, 700, 65], 64, 0.1),
+        ([ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5), ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5)],
+         [0, 1, 1], [1500, 3000, 65], 64, 1.0),
+    ]
+    for models, rm, rc, P, scale in cases:
+        w = W.small_workload(models, rm, rc, page_tokens=P, seed=55, value_scale=scale, keep_contiguous=False)
+        worst = run_and_compare(w, "few_ctas%d/k%d" % (n_ctas, kernel),
+                                {cp.CP_OPT_KERNEL: kernel, cp.CP_OPT_NUM_CTAS: n_ctas,
+                                 cp.CP_OPT_MIN_TILE_PAGES: 1, cp.CP_OPT_WAVES_X16: 16 * 12})
+        print(worst)
+
+
+@pytest.mark.parametrize("P", [32, 128])
+def test_mla_other_page_sizes(torch_cuda, P):
+    """MLA tensor-core kernels with 1 and 4 slices per page (P = 32, 128); P = 16 falls back to the
+    generic kernel (slices are 32 tokens) and must still be right."""
+    import paper_2606_24506_b200 as cp
+    m = ModelCfg(KIND_MLA, 128, 1, 576, 512, 192 ** -0.5)
+    for pt in (P, 16):
+        w = W.small_workload([m], [0, 0], [1111, 97], page_tokens=pt, seed=77, value_scale=0.1, keep_contiguous=False)
+        for kernel in (0, 2):
+            worst = run_and_compare(w, "mla_P%d/k%d" % (pt, kernel), {cp.CP_OPT_KERNEL: kernel, cp.CP_OPT_MIN_TILE_PAGES: 1})
+            print(worst)
+
+
 # ------------------------------------------------------------------ invariants on the GPU path
 def test_page_permutation_is_bit_identical(torch_cuda):
     """P5 on the GPU: split boundaries are logical, so moving the data to other physical
