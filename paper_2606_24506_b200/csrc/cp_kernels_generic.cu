@@ -15,36 +15,60 @@
 namespace cp {
 
 // ------------------------------------------------------------------------------ gather
-// grid.x covers (token, kv head) rows in chunks; each thread moves 16-byte vectors.
-__global__ void cp_gather_kernel(const uint8_t *__restrict__ arena, uint32_t page_tokens,
-                                 uint32_t page_bytes, const int32_t *__restrict__ page_ids,
-                                 int kind, int n_kv_heads, int d_k, int d_v, int context_len,
-                                 uint8_t *__restrict__ k_out, uint8_t *__restrict__ v_out)
+// Grid-stride over 16-byte vectors; every thread moves four vectors per iteration (four independent
+// translations + loads in flight before the first store), one page-table lookup per vector.
+template <class Idx>
+__device__ __forceinline__ void gather_addr(const uint8_t *arena, uint32_t page_tokens, uint32_t page_bytes,
+                                            const int32_t *page_ids, int kind, int n_kv_heads, int d_k, int d_v,
+                                            int kvec, int per_row, Idx i, uint8_t *k_out, uint8_t *v_out,
+                                            const uint4 *&src, uint4 *&dst)
+{
+    const Idx row = i / (Idx)per_row;           // row = t * Hkv + c
+    const int vec = (int)(i - row * (Idx)per_row);
+    const int t = (int)(row / (Idx)n_kv_heads);
+    const int c = (int)(row - (Idx)t * (Idx)n_kv_heads);
+    const int lp = t / (int)page_tokens;
+    const uint32_t slot = (uint32_t)(t - lp * (int)page_tokens);
+    const int32_t pid = __ldg(page_ids + (int64_t)lp * n_kv_heads + c);
+    const uint64_t base = (uint64_t)pid * page_bytes;
+    if (vec < kvec) {
+        src = reinterpret_cast<const uint4 *>(arena + base + (uint64_t)slot * d_k * 2 + vec * 16);
+        dst = reinterpret_cast<uint4 *>(k_out + (uint64_t)row * d_k * 2 + vec * 16);
+    } else {
+        const int vv = vec - kvec;
+        const uint64_t off = (kind == 1) ? (uint64_t)slot * d_k * 2
+                                         : (uint64_t)page_tokens * d_k * 2 + (uint64_t)slot * d_v * 2;
+        src = reinterpret_cast<const uint4 *>(arena + base + off + vv * 16);
+        dst = reinterpret_cast<uint4 *>(v_out + (uint64_t)row * d_v * 2 + vv * 16);
+    }
+}
+
+template <class Idx>      // uint32_t when the vector count fits (32-bit divisions), else uint64_t
+__global__ void __launch_bounds__(256)
+cp_gather_kernel(const uint8_t *__restrict__ arena, uint32_t page_tokens, uint32_t page_bytes,
+                 const int32_t *__restrict__ page_ids, int kind, int n_kv_heads, int d_k, int d_v,
+                 int context_len, uint8_t *__restrict__ k_out, uint8_t *__restrict__ v_out)
 {
     const int kvec = d_k / 8;                       // 16-B vectors per K row
     const int vvec = v_out ? d_v / 8 : 0;
     const int per_row = kvec + vvec;
-    const int64_t total = (int64_t)context_len * n_kv_heads * per_row;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total;
-         i += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t row = i / per_row;            // row = t * Hkv + c
-        const int vec = (int)(i % per_row);
-        const int t = (int)(row / n_kv_heads);
-        const int c = (int)(row % n_kv_heads);
-        const int lp = t / (int)page_tokens;
-        const uint32_t slot = (uint32_t)(t % (int)page_tokens);
-        const int32_t pid = __ldg(page_ids + (int64_t)lp * n_kv_heads + c);
-        const uint64_t base = (uint64_t)pid * page_bytes;
-        if (vec < kvec) {
-            const uint4 v = *reinterpret_cast<const uint4 *>(arena + base + (uint64_t)slot * d_k * 2 + vec * 16);
-            *reinterpret_cast<uint4 *>(k_out + row * d_k * 2 + vec * 16) = v;
-        } else {
-            const int vv = vec - kvec;
-            const uint64_t off = (kind == 1) ? (uint64_t)slot * d_k * 2
-                                             : (uint64_t)page_tokens * d_k * 2 + (uint64_t)slot * d_v * 2;
-            const uint4 v = *reinterpret_cast<const uint4 *>(arena + base + off + vv * 16);
-            *reinterpret_cast<uint4 *>(v_out + row * d_v * 2 + vv * 16) = v;
-        }
+    const Idx total = (Idx)context_len * (Idx)n_kv_heads * (Idx)per_row;
+    const Idx T = (Idx)gridDim.x * blockDim.x;
+    for (Idx i0 = (Idx)blockIdx.x * blockDim.x + threadIdx.x; i0 < total; i0 += 4 * T) {
+        const uint4 *src[4];
+        uint4 *dst[4];
+        uint4 val[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (i0 + u * T < total)
+                gather_addr<Idx>(arena, page_tokens, page_bytes, page_ids, kind, n_kv_heads, d_k, d_v, kvec, per_row,
+                            i0 + u * T, k_out, v_out, src[u], dst[u]);
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (i0 + u * T < total) val[u] = __ldcs(src[u]);          // streamed once
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (i0 + u * T < total) __stcs(dst[u], val[u]);
     }
 }
 
@@ -53,13 +77,18 @@ void launch_gather(const uint8_t *arena, uint32_t page_tokens, uint32_t page_byt
                    int context_len, void *k_out, void *v_out, int n_sm, cudaStream_t stream)
 {
     const int64_t total = (int64_t)context_len * n_kv_heads * (d_k / 8 + (v_out ? d_v / 8 : 0));
-    int64_t blocks = (total + 255) / 256;
-    const int64_t cap = (int64_t)n_sm * 8;
+    int64_t blocks = (total + 1023) / 1024;
+    const int64_t cap = (int64_t)n_sm * 16;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
-    cp_gather_kernel<<<(unsigned)blocks, 256, 0, stream>>>(
-        arena, page_tokens, page_bytes, page_ids_dev, kind, n_kv_heads, d_k, d_v, context_len,
-        (uint8_t *)k_out, (uint8_t *)v_out);
+    if (total + 4 * blocks * 256 < (int64_t)0xFFFFFFFFll)
+        cp_gather_kernel<uint32_t><<<(unsigned)blocks, 256, 0, stream>>>(
+            arena, page_tokens, page_bytes, page_ids_dev, kind, n_kv_heads, d_k, d_v, context_len,
+            (uint8_t *)k_out, (uint8_t *)v_out);
+    else
+        cp_gather_kernel<uint64_t><<<(unsigned)blocks, 256, 0, stream>>>(
+            arena, page_tokens, page_bytes, page_ids_dev, kind, n_kv_heads, d_k, d_v, context_len,
+            (uint8_t *)k_out, (uint8_t *)v_out);
 }
 
 // ---------------------------------------------------------------------- generic decode
