@@ -43,6 +43,10 @@ def lib():
         L.cpo_gather.argtypes = [u16p, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32,
                                  ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                  i32p, ctypes.c_int, ctypes.c_int, u16p, u16p]
+        L.cpo_append.restype = ctypes.c_int
+        L.cpo_append.argtypes = [u16p, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32,
+                                 ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                 i32p, ctypes.c_int, ctypes.c_int, u16p, u16p]
         L.cpo_attention.restype = ctypes.c_int
         L.cpo_attention.argtypes = [u16p, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32,
                                     ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
@@ -74,6 +78,24 @@ def gather(arena: np.ndarray, page_tokens: int, page_bytes: int, num_pages: int,
     if rc != 0:
         raise ValueError("cpo_gather failed: %d" % rc)
     return k, v
+
+
+def append(arena: np.ndarray, page_tokens: int, page_bytes: int, num_pages: int, kind: int,
+           n_kv_heads: int, d_k: int, d_v: int, page_ids: np.ndarray, pos: int,
+           k_new: np.ndarray, v_new: Optional[np.ndarray]):
+    """Write one new token's rows at position `pos` IN PLACE into `arena` (uint16, C-contiguous)."""
+    assert arena.dtype == np.uint16 and arena.flags["C_CONTIGUOUS"]
+    page_ids = np.ascontiguousarray(page_ids, dtype=np.int32)
+    k_new = np.ascontiguousarray(k_new, dtype=np.uint16)
+    vp = None
+    if v_new is not None:
+        v_new = np.ascontiguousarray(v_new, dtype=np.uint16)
+        vp = _p(v_new, ctypes.c_uint16)
+    rc = lib().cpo_append(_p(arena, ctypes.c_uint16), page_tokens, page_bytes, num_pages, kind,
+                          n_kv_heads, d_k, d_v, _p(page_ids, ctypes.c_int32), page_ids.size, pos,
+                          _p(k_new, ctypes.c_uint16), vp)
+    if rc != 0:
+        raise ValueError("cpo_append failed: %d" % rc)
 
 
 def attention(arena: np.ndarray, page_tokens: int, page_bytes: int, num_pages: int, kind: int,

@@ -117,6 +117,43 @@ int cpo_gather(const uint16_t *arena, uint32_t page_tokens, uint32_t page_bytes,
     return CPO_OK;
 }
 
+/*
+ * KV append (the step right before attention in every decode iteration:
+ * "physical KV pages [are mapped] on demand ... kept until their decode requests finish",
+ * PAPER.md:L122): write the rows of ONE new token at position `pos` (= the context length before
+ * the append) of a request: k_new [Hkv][d_k], v_new [Hkv][d_v] (MLA: k_new is the latent row
+ * [d_k], v_new is ignored).  The page list must already cover logical page pos / P.  Only the
+ * 16-bit patterns move; everything else in the arena stays untouched.
+ */
+int cpo_append(uint16_t *arena, uint32_t page_tokens, uint32_t page_bytes, uint32_t num_pages,
+               int kind, int n_kv_heads, int d_k, int d_v,
+               const int32_t *page_ids, int n_page_ids, int pos,
+               const uint16_t *k_new, const uint16_t *v_new)
+{
+    if (!arena || !page_ids || !k_new || page_tokens == 0 || pos < 0 || n_kv_heads < 1)
+        return CPO_ERR_ARG;
+    if (kind == CPO_KIND_MLA && n_kv_heads != 1)
+        return CPO_ERR_ARG;
+    if (kind != CPO_KIND_MLA && !v_new)
+        return CPO_ERR_ARG;
+    int lp = pos / (int)page_tokens;
+    uint32_t slot = (uint32_t)(pos % (int)page_tokens);
+    if (n_page_ids < (lp + 1) * n_kv_heads)
+        return CPO_ERR_ARG;
+    for (int c = 0; c < n_kv_heads; ++c) {
+        int32_t pid = page_ids[lp * n_kv_heads + c];
+        if (pid < 0 || (uint32_t)pid >= num_pages)
+            return CPO_ERR_ARG;
+        uint64_t ko = row_offset_u16(page_tokens, page_bytes, kind, d_k, d_v, pid, slot, 0);
+        memcpy(arena + ko, k_new + (uint64_t)c * d_k, (size_t)d_k * 2);
+        if (kind != CPO_KIND_MLA) {
+            uint64_t vo = row_offset_u16(page_tokens, page_bytes, kind, d_k, d_v, pid, slot, 1);
+            memcpy(arena + vo, v_new + (uint64_t)c * d_v, (size_t)d_v * 2);
+        }
+    }
+    return CPO_OK;
+}
+
 /* Attention of ONE query head over the token range [t0, t1) of one request, by the
  * definition: s_t = sigma * sum_i q_i k_{t,i} (i ascending); m = max_t s_t;
  * p_t = exp(s_t - m); l = sum_t p_t (t ascending); O_j = (sum_t p_t v_{t,j}) / l;

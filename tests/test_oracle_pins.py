@@ -349,6 +349,48 @@ def test_p12_gather_special_bit_patterns():
     assert gk.tobytes() == k.tobytes() and gv.tobytes() == v.tobytes()
 
 
+# ---------------------------------------------------------------- P13 append
+@pytest.mark.parametrize("kind", [KIND_KV, KIND_MLA])
+def test_p13_append_token_by_token(kind):
+    """Building a request with the oracle's append, one token at a time into an all-poison arena,
+    gives exactly the arena a direct scatter gives: the expected image is written here with the
+    address formula of DESIGN.md §4 (numpy indexing, not the oracle), compared byte for byte, so
+    every other byte must still be poison."""
+    P = 4
+    if kind == KIND_KV:
+        Hkv, dk, dv = 3, 16, 8
+        page_u16 = P * (dk + dv)
+    else:
+        Hkv, dk, dv = 1, 24, 16
+        page_u16 = P * dk
+    T, num_pages = 11, 20
+    rng = np.random.default_rng(77)
+    n_lp = -(-T // P)
+    page_ids = rng.permutation(num_pages)[:n_lp * Hkv].astype(np.int32)
+    k = rng.integers(0, 65536, size=(T, Hkv, dk)).astype(np.uint16)
+    v = rng.integers(0, 65536, size=(T, Hkv, dv)).astype(np.uint16)
+    arena = np.full(num_pages * page_u16, W.BF16_NAN, dtype=np.uint16)
+    expect = arena.copy().reshape(num_pages, page_u16)
+    for t in range(T):
+        oracle.append(arena, P, page_u16 * 2, num_pages, kind, Hkv, dk, dv, page_ids, t, k[t],
+                      None if kind == KIND_MLA else v[t])
+        for c in range(Hkv):
+            pg = expect[page_ids[(t // P) * Hkv + c]]
+            pg[(t % P) * dk:(t % P) * dk + dk] = k[t, c]
+            if kind == KIND_KV:
+                pg[P * dk + (t % P) * dv:P * dk + (t % P) * dv + dv] = v[t, c]
+        assert arena.tobytes() == expect.tobytes()
+    gk, gv = oracle.gather(arena, P, page_u16 * 2, num_pages, kind, Hkv, dk, dv, page_ids, T)
+    assert gk.tobytes() == k.tobytes()
+    if kind == KIND_KV:
+        assert gv.tobytes() == v.tobytes()
+    else:
+        assert gv.tobytes() == np.ascontiguousarray(k[:, :, :dv]).tobytes()
+    with pytest.raises(ValueError):          # page list does not cover the position
+        oracle.append(arena, P, page_u16 * 2, num_pages, kind, Hkv, dk, dv, page_ids, n_lp * P, k[0],
+                      None if kind == KIND_MLA else v[0])
+
+
 # ---------------------------------------------------------------- argument checks
 def test_oracle_rejects_bad_arguments():
     m = ModelCfg(KIND_KV, 4, 2, 16, 16, 0.25)
