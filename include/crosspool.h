@@ -169,6 +169,23 @@ cp_status cp_pool_gather_kv(cp_pool *pool, int32_t request_id,
                             void *k_out_dev, void *v_out_dev, void *stream);
 
 /*
+ * cp_pool_append_kv -- the step right before attention in every decode iteration (SURVEY.md §8(f)
+ * N1): write ONE new token per request into the pool at position context_len and raise
+ * context_len by one.  When the position opens a new logical page the library takes the n_kv_heads
+ * physical pages from its free list -- "map physical KV pages on demand" -- and
+ * rejects the whole batch with CP_ERR_NO_PAGES if the budget is exhausted (never preempts).
+ *   request_ids_host  batch order; ids must be distinct and mapped
+ *   k_new_dev  bf16, packed in batch order, per request [Hkv][d_k]  (MLA: the latent row [d_k])
+ *   v_new_dev  bf16, packed in batch order, per request [Hkv][d_v]  (MLA requests contribute nothing;
+ *              may be NULL when the batch has only MLA requests)
+ * All-or-nothing.  Only the 16-bit patterns move (bit-exact).  Runs on `stream`; the page table and
+ * context lengths seen by later compute calls on the same stream include the new token.
+ * Errors: INVALID_ARG (also: a page list that cannot grow), UNKNOWN_REQUEST, NO_PAGES, CUDA.
+ */
+cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                            const void *k_new_dev, const void *v_new_dev, void *stream);
+
+/*
  * cp_decode_workspace_bytes -- bytes of scratch cp_decode_attention needs for this batch
  * (split-KV partial results; 0 when no group is split).
  */

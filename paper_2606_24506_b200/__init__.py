@@ -80,6 +80,7 @@ def load_library():
         "cp_pool_stats": (i32, [vp, u32p, u32p]),
         "cp_pool_set_option": (i32, [vp, i32, ctypes.c_int64]),
         "cp_pool_gather_kv": (i32, [vp, i32, vp, vp, vp]),
+        "cp_pool_append_kv": (i32, [vp, i32p, i32, vp, vp, vp]),
         "cp_decode_workspace_bytes": (i32, [vp, i32p, i32, u64p]),
         "cp_decode_attention": (i32, [vp, i32p, i32, vp, vp, vp, vp, u64, vp]),
         "cp_decode_workspace_bytes_host": (i32, [vp, i32p, i32, u64p]),
@@ -98,6 +99,7 @@ def load_library():
 
 EXPORTED = ["cp_pool_create", "cp_pool_free", "cp_pool_map_pages", "cp_pool_unmap_request",
             "cp_pool_request_info", "cp_pool_stats", "cp_pool_set_option", "cp_pool_gather_kv",
+            "cp_pool_append_kv",
             "cp_decode_workspace_bytes", "cp_decode_attention", "cp_decode_workspace_bytes_host",
             "cp_decode_attention_host", "cp_decode_plan", "cp_pool_counters", "cp_status_string"]
 
@@ -209,6 +211,11 @@ class Pool:
     def gather_kv(self, request_id: int, k_out_dev, v_out_dev, stream: int = 0):
         _check(self._L.cp_pool_gather_kv(self._h, request_id, _ptr(k_out_dev), _ptr(v_out_dev), stream),
                "cp_pool_gather_kv")
+
+    def append_kv(self, request_ids, k_new_dev, v_new_dev, stream: int = 0):
+        ids = _ids(request_ids)
+        _check(self._L.cp_pool_append_kv(self._h, _i32p(ids), ids.size, _ptr(k_new_dev), _ptr(v_new_dev), stream),
+               "cp_pool_append_kv")
 
     def decode_workspace_bytes(self, request_ids) -> int:
         ids = _ids(request_ids)

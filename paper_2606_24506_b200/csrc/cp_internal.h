@@ -73,6 +73,12 @@ struct TileRec {
 };
 static_assert(sizeof(TileRec) == 80, "TileRec is loaded as five 16-byte vectors");
 
+// One request of a cp_pool_append_kv batch.
+struct AppendRec {
+    int32_t req, model, pos, pad;
+    int64_t k_off, v_off;          // element offsets of this request's rows in the packed k_new / v_new
+};
+
 // One unit of the LSE combine: one query head of a split group.
 struct Combine {
     int32_t group;

@@ -91,6 +91,43 @@ void launch_gather(const uint8_t *arena, uint32_t page_tokens, uint32_t page_byt
             (uint8_t *)k_out, (uint8_t *)v_out);
 }
 
+// ------------------------------------------------------------------------------ append
+// One block per request: translate (request, logical page of `pos`, kv head) through the page
+// table and copy the new token's K and V rows (16-byte vectors) into their slots.
+__global__ void cp_append_kernel(uint8_t *__restrict__ arena, uint32_t page_tokens, uint32_t page_bytes,
+                                 const int32_t *__restrict__ page_table, int max_ppr,
+                                 const DevModel *__restrict__ models, const AppendRec *__restrict__ recs,
+                                 const uint16_t *__restrict__ k_new, const uint16_t *__restrict__ v_new)
+{
+    const AppendRec r = recs[blockIdx.x];
+    const DevModel m = models[r.model];
+    const int lp = r.pos / (int)page_tokens;
+    const uint32_t slot = (uint32_t)(r.pos - lp * (int)page_tokens);
+    const int kvec = m.d_k / 8, vvec = m.kind == 1 ? 0 : m.d_v / 8;
+    const int per_head = kvec + vvec;
+    for (int i = threadIdx.x; i < m.n_kv_heads * per_head; i += blockDim.x) {
+        const int c = i / per_head, vec = i - c * per_head;
+        const int32_t pid = __ldg(page_table + (int64_t)r.req * max_ppr + (int64_t)lp * m.n_kv_heads + c);
+        const uint64_t base = (uint64_t)pid * page_bytes;
+        if (vec < kvec) {
+            const uint4 v = *reinterpret_cast<const uint4 *>(k_new + r.k_off + (int64_t)c * m.d_k + vec * 8);
+            *reinterpret_cast<uint4 *>(arena + base + (uint64_t)slot * m.d_k * 2 + vec * 16) = v;
+        } else {
+            const int vv = vec - kvec;
+            const uint4 v = *reinterpret_cast<const uint4 *>(v_new + r.v_off + (int64_t)c * m.d_v + vv * 8);
+            *reinterpret_cast<uint4 *>(arena + base + (uint64_t)page_tokens * m.d_k * 2 + (uint64_t)slot * m.d_v * 2 + vv * 16) = v;
+        }
+    }
+}
+
+void launch_append(uint8_t *arena, uint32_t page_tokens, uint32_t page_bytes, const int32_t *page_table,
+                   int max_ppr, const DevModel *models, const AppendRec *recs, int n_requests,
+                   const uint16_t *k_new, const uint16_t *v_new, cudaStream_t stream)
+{
+    cp_append_kernel<<<n_requests, 128, 0, stream>>>(arena, page_tokens, page_bytes, page_table, max_ppr, models,
+                                                    recs, k_new, v_new);
+}
+
 // ---------------------------------------------------------------------- generic decode
 constexpr int GEN_THREADS = 256;
 constexpr int GEN_HB = 16;      // query heads per pass

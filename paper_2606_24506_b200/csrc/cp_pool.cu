@@ -97,7 +97,7 @@ struct cp_pool {
     // device side (lazy)
     bool dev_ready = false;
     int n_sm = 148;
-    DevBuf d_page_table, d_ctx, d_models;
+    DevBuf d_page_table, d_ctx, d_models, d_append;
     alignas(64) unsigned char kv_tmap[128];   // CUtensorMap of the arena for the MQA/GQA kernel
     bool kv_tmap_ok = false;
     alignas(64) unsigned char mla_tmap[128];  // CUtensorMap of the arena for the MLA kernel
@@ -491,7 +491,7 @@ cp_status cp_pool_free(cp_pool *pool)
 {
     if (!pool) return CP_OK;
     if (pool->dev_ready) cudaDeviceSynchronize();
-    pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release();
+    pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release(); pool->d_append.release();
     for (int k = 0; k < 2; ++k) {
         pool->plan[k].d_groups.release(); pool->plan[k].d_tiles.release();
         pool->plan[k].d_combines.release(); pool->plan[k].d_cunits.release(); pool->plan[k].d_tile_recs.release();
@@ -680,6 +680,77 @@ cp_status cp_pool_gather_kv(cp_pool *pool, int32_t request_id, void *k_out_dev, 
                   (const int32_t *)pool->d_page_table.ptr + (size_t)request_id * pool->max_ppr,
                   m.kind, m.n_kv_heads, m.head_dim_qk, m.head_dim_v, r.ctx, k_out_dev, v_out_dev,
                   pool->n_sm, s);
+    pool->n_launches++;
+    if (cudaGetLastError() != cudaSuccess) return CP_ERR_CUDA;
+    return CP_OK;
+}
+
+cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                            const void *k_new_dev, const void *v_new_dev, void *stream)
+{
+    cp_status st = check_batch(pool, request_ids_host, n_requests);
+    if (st != CP_OK) return st;
+    if (!k_new_dev || ((uintptr_t)k_new_dev & 15u) || ((uintptr_t)v_new_dev & 15u)) return CP_ERR_INVALID_ARG;
+    // validate the whole batch first (all-or-nothing): capacity of the page lists, page budget
+    const int P = (int)pool->P;
+    uint32_t need_pages = 0;
+    bool any_v = false;
+    for (int b = 0; b < n_requests; ++b) {
+        const Request &r = pool->reqs[request_ids_host[b]];
+        const cp_model_cfg &m = pool->models[r.model];
+        if (m.kind != CP_KIND_MLA) any_v = true;
+        if (r.ctx == INT32_MAX) return CP_ERR_INVALID_ARG;
+        const size_t have_lp = r.pages.size() / m.n_kv_heads;
+        if ((size_t)(r.ctx / P) >= have_lp) {                 // position r.ctx opens a new logical page
+            if (r.pages.size() + m.n_kv_heads > (size_t)pool->max_ppr) return CP_ERR_INVALID_ARG;
+            need_pages += (uint32_t)m.n_kv_heads;
+        }
+    }
+    if (any_v && !v_new_dev) return CP_ERR_INVALID_ARG;
+    if (need_pages > pool->n_free) return CP_ERR_NO_PAGES;
+    st = ensure_device(pool);
+    if (st != CP_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (pool->d_append.ensure((size_t)n_requests * sizeof(AppendRec)) != cudaSuccess) {
+        cudaGetLastError();
+        return CP_ERR_CUDA;
+    }
+    // commit on the host: new pages from the free list, context lengths
+    std::vector<AppendRec> recs(n_requests);
+    int64_t ko = 0, vo = 0;
+    for (int b = 0; b < n_requests; ++b) {
+        const int rid = request_ids_host[b];
+        Request &r = pool->reqs[rid];
+        const cp_model_cfg &m = pool->models[r.model];
+        if ((size_t)(r.ctx / P) >= r.pages.size() / m.n_kv_heads) {
+            uint32_t cur = pool->alloc_cursor;
+            for (int i = 0; i < m.n_kv_heads;) {
+                if (pool->owner[cur] == -1) { pool->owner[cur] = rid; r.pages.push_back((int32_t)cur); ++i; }
+                cur = (cur + 1) % pool->num_pages;
+            }
+            pool->alloc_cursor = cur;
+            pool->n_free -= (uint32_t)m.n_kv_heads;
+        }
+        recs[b].req = rid; recs[b].model = r.model; recs[b].pos = r.ctx; recs[b].pad = 0;
+        recs[b].k_off = ko; recs[b].v_off = vo;
+        ko += (int64_t)m.n_kv_heads * m.head_dim_qk;
+        if (m.kind != CP_KIND_MLA) vo += (int64_t)m.n_kv_heads * m.head_dim_v;
+        const int old_planned = ceil_div(r.ctx, P);
+        r.ctx += 1;
+        pool->h_ctx[rid] = r.ctx;
+        pool->ctx_dirty_lo = std::min(pool->ctx_dirty_lo, rid);
+        pool->ctx_dirty_hi = std::max(pool->ctx_dirty_hi, rid);
+        if (ceil_div(r.ctx, P) != old_planned) pool->topo_version++;
+    }
+    st = flush_tables(pool, s);                            // new page ids (and context lengths) to the device
+    if (st != CP_OK) return st;
+    if (cudaMemcpyAsync(pool->d_append.ptr, recs.data(), recs.size() * sizeof(AppendRec), cudaMemcpyHostToDevice, s) !=
+        cudaSuccess)
+        return CP_ERR_CUDA;
+    pool->n_h2d_bytes += recs.size() * sizeof(AppendRec);
+    launch_append(pool->arena, pool->P, pool->page_bytes, (const int32_t *)pool->d_page_table.ptr, pool->max_ppr,
+                  (const DevModel *)pool->d_models.ptr, (const AppendRec *)pool->d_append.ptr, n_requests,
+                  (const uint16_t *)k_new_dev, (const uint16_t *)v_new_dev, s);
     pool->n_launches++;
     if (cudaGetLastError() != cudaSuccess) return CP_ERR_CUDA;
     return CP_OK;

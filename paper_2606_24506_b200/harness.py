@@ -14,13 +14,13 @@ from . import Pool
 class DeviceWorkload:
     """A `workloads.Workload` resident on the GPU behind a cp_pool."""
 
-    def __init__(self, w, device: str = "cuda:0", map_requests: bool = True):
+    def __init__(self, w, device: str = "cuda:0", map_requests: bool = True, page_list_slack: int = 0):
         self.w = w
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         # arena: one contiguous device buffer (torch allocations are >= 256-B aligned)
         self.arena = torch.from_numpy(w.arena.view(np.int16)).to(self.device)
-        max_ppr = max(r.page_ids.size for r in w.requests)
+        max_ppr = max(r.page_ids.size for r in w.requests) + page_list_slack    # room for appended pages
         self.pool = Pool(self.arena, self.arena.numel() * 2, w.page_tokens, w.page_bytes, w.num_pages,
                          w.models, max_requests=len(w.requests), max_pages_per_request=max_ppr)
         if map_requests:

@@ -203,3 +203,32 @@ def test_compute_calls_fail_loudly_without_a_device():
         p.gather_kv(0, FAKE_ARENA, FAKE_ARENA)
     assert e.value.status == cp.CP_ERR_CUDA
     p.close()
+
+
+def test_append_kv_host_validation_is_all_or_nothing():
+    """cp_pool_append_kv argument / budget errors are detected before anything changes (no GPU
+    needed: the device is only touched after validation)."""
+    models = [ModelCfg(KIND_KV, 8, 2, 128, 128, 0.1)]
+    p = make_pool(P=16, num_pages=6, models=models, max_requests=4, max_ppr=8)
+    p.map_pages(0, 0, None, 16, n_allocate=2)         # one full logical page (2 kv heads)
+    p.map_pages(1, 0, None, 5, n_allocate=2)          # room left in its page
+    p.map_pages(2, 0, None, 16, n_allocate=2)         # full page as well: pool is now exhausted
+    before = (p.stats(), [p.request_info(i)[:2] for i in range(3)])
+    k = np.zeros(3 * 2 * 128, dtype=np.uint16)
+    with pytest.raises(cp.CrossPoolError) as e:       # requests 0 and 2 each need 2 fresh pages: 0 free
+        p.append_kv([0, 1, 2], k, k)
+    assert e.value.status == cp.CP_ERR_NO_PAGES
+    with pytest.raises(cp.CrossPoolError) as e:
+        p.append_kv([1, 3], k, k)
+    assert e.value.status == cp.CP_ERR_UNKNOWN_REQUEST
+    with pytest.raises(cp.CrossPoolError) as e:
+        p.append_kv([1], None, k)
+    assert e.value.status == cp.CP_ERR_INVALID_ARG
+    with pytest.raises(cp.CrossPoolError) as e:       # KV-kind request without value rows
+        p.append_kv([1], k, None)
+    assert e.value.status == cp.CP_ERR_INVALID_ARG
+    with pytest.raises(cp.CrossPoolError) as e:
+        p.append_kv([1, 1], k, k)
+    assert e.value.status == cp.CP_ERR_INVALID_ARG
+    assert before == (p.stats(), [p.request_info(i)[:2] for i in range(3)])
+    p.close()

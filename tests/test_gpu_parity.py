@@ -334,6 +334,59 @@ def test_append_and_context_growth(torch_cuda):
     dw.close()
 
 
+@pytest.mark.parametrize("kind", ["kv", "mla"])
+def test_append_kv_matches_oracle_bit_for_bit(torch_cuda, kind):
+    """cp_pool_append_kv writes one token per request per call (pages taken from the
+    free list when a position opens a new logical page).  After every call the WHOLE device arena
+    equals the host arena the oracle's append produced with the same page ids (bit-exact, poison
+    included), and attention on the grown contexts tracks the oracle."""
+    import torch
+    if kind == "kv":
+        models = [ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5), ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5)]
+        rm, rc, P, scale = [0, 1, 1], [30, 64, 5], 16, 1.0
+    else:
+        models = [ModelCfg(KIND_MLA, 128, 1, 576, 512, 192 ** -0.5)]
+        rm, rc, P, scale = [0, 0], [63, 130], 32, 0.1
+    w = W.small_workload(models, rm, rc, page_tokens=P, seed=91, value_scale=scale, extra_pages=40,
+                         keep_contiguous=False)
+    dw = device_workload(w, page_list_slack=3 * max(m.n_kv_heads for m in models))
+    rng = np.random.default_rng(17)
+    host = w.arena.copy()
+    ctx = [r.context_len for r in w.requests]
+    for step in range(2 * P + 3):                       # crosses at least two page boundaries per request
+        ks, vs = [], []
+        for r in w.requests:
+            m = models[r.model_id]
+            ks.append(W.f32_to_bf16((scale * rng.standard_normal((m.n_kv_heads, m.head_dim_qk))).astype(np.float32)))
+            if m.kind == KIND_KV:
+                vs.append(W.f32_to_bf16((scale * rng.standard_normal((m.n_kv_heads, m.head_dim_v))).astype(np.float32)))
+        k_dev = torch.from_numpy(np.concatenate([x.reshape(-1) for x in ks]).view(np.int16)).to(dw.device)
+        v_dev = torch.from_numpy(np.concatenate([x.reshape(-1) for x in vs]).view(np.int16)).to(dw.device) if vs else None
+        dw.pool.append_kv(dw.ids, k_dev, v_dev, dw.stream())
+        vi = 0
+        for i, r in enumerate(w.requests):
+            m = models[r.model_id]
+            _, c, ids = dw.pool.request_info(r.request_id)
+            assert c == ctx[i] + 1
+            r.page_ids = ids                              # the library chose the new pages
+            v_new = None
+            if m.kind == KIND_KV:
+                v_new = vs[vi]; vi += 1
+            oracle.append(host, P, w.page_bytes, w.num_pages, m.kind, m.n_kv_heads, m.head_dim_qk, m.head_dim_v,
+                          ids, ctx[i], ks[i], v_new)
+            ctx[i] += 1
+            r.context_len = ctx[i]
+        if step % P in (0, 1) or step == 2 * P + 2:
+            torch.cuda.synchronize()
+            assert dw.arena.cpu().numpy().view(np.uint16).tobytes() == host.tobytes(), "arena differs at step %d" % step
+    w.arena = host
+    dw.decode()
+    got = dw.results()
+    dw.close()
+    worst = compare(w, got, oracle.decode_workload(w), "append_" + kind)
+    print(worst)
+
+
 def test_host_buffer_entry_point_matches_device_path(torch_cuda):
     torch = torch_cuda
     ms = [ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5), ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5)]
