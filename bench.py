@@ -214,7 +214,7 @@ def main():
 
     k = args.config
     w = W.config(k)
-    dw = DeviceWorkload(w, dev)
+    dw = DeviceWorkload(w, dev, page_list_slack=max(m.n_kv_heads for m in w.models))
     dw.pool.set_option(cp.CP_OPT_KERNEL, args.kernel)
     if args.waves_x16 > 0:
         dw.pool.set_option(cp.CP_OPT_WAVES_X16, args.waves_x16)
@@ -315,6 +315,26 @@ def main():
                   "note": "back-to-back launches (the gathered copy of a long request exceeds L2)"}
         del gk, gv
 
+    # ---------------- KV append step, last because it grows the contexts: one new token
+    # per request per call, launch-bound (a few KB per call); reported as us per call on the device
+    append = None
+    if rank == 0:
+        kn = sum(m.n_kv_heads * m.head_dim_qk for m in (w.models[r.model_id] for r in w.requests))
+        vn = sum(m.n_kv_heads * m.head_dim_v for m in (w.models[r.model_id] for r in w.requests) if m.kind == 0)
+        k_new = torch.zeros(kn, dtype=torch.int16, device=dev)
+        v_new = torch.zeros(max(vn, 8), dtype=torch.int16, device=dev)
+        reps = 8
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        dw.pool.append_kv(dw.ids, k_new, v_new, dw.stream())
+        torch.cuda._sleep(400000)          # keep the device busy while the host enqueues the calls
+        a0.record()
+        for _ in range(reps):
+            dw.pool.append_kv(dw.ids, k_new, v_new, dw.stream())
+        a1.record()
+        torch.cuda.synchronize()
+        append = {"us_per_call": 1e3 * a0.elapsed_time(a1) / reps, "requests": len(w.requests),
+                  "bytes_per_call": 2 * (kn + vn)}
+
     peaks = measured_peaks()
     if gather:
         gather["frac_of_measured_copy_peak"] = gather["traffic_gbs"] / peaks["hbm_gbs"]
@@ -340,7 +360,7 @@ def main():
                     "us_per_step": 1e3 * e2e_ms,
                     "h2d_bytes_per_step": int(q_host.numel() * 2),
                     "d2h_bytes_per_step": int(o_host.numel() * 4 + l_host.numel() * 4)},
-            "gpu_launches": int(launches), "roofline": roof, "gather": gather,
+            "gpu_launches": int(launches), "roofline": roof, "gather": gather, "append": append,
             "pct_of_hbm_peak": {"measured_copy": 100 * achieved / peaks["hbm_gbs"], "nominal_8TBs": 100 * achieved / 8000.0}}
 
     if not args.no_cpu_baseline:
