@@ -75,7 +75,7 @@ def workload_desc(w, k):
 
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed regions run."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
@@ -83,10 +83,12 @@ class ClockSampler:
         self.rows = []
         self.proc = None
         try:
-            self.proc = subprocess.Popen(
-                ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                 "--format=csv,noheader,nounits", "-lms", "20"],
-                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            import shutil
+            cmd = ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                   "--format=csv,noheader,nounits", "-lms", "5"]
+            if shutil.which("stdbuf"):
+                cmd = ["stdbuf", "-oL"] + cmd          # line-buffered: samples arrive while we run
+            self.proc = subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except Exception:
@@ -104,16 +106,24 @@ class ClockSampler:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
-        rows = [r for (t, r) in self.rows if t0 <= t <= t1] or [r for (_, r) in self.rows]
+        self.t.join(timeout=2)
+        # nvidia-smi's own timestamp decides whether a sample lies in the window (its stdout reaches
+        # us through a pipe in bursts, so the arrival time says little)
+        import datetime
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in rows:
+        parsed = []
+        for _, r in self.rows:
             f = [x.strip() for x in r.split(",")]
             try:
-                sm.append(float(f[0])); mx.append(float(f[1]))
+                ts = datetime.datetime.strptime(f[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                parsed.append((ts, float(f[1]), float(f[2]), f[4:8]))
             except Exception:
                 continue
-            for n, v in zip(names, f[3:7]):
+        inside = [x for x in parsed if t0 - 0.05 <= x[0] <= t1 + 0.05] or parsed
+        for _, a, b, fl in inside:
+            sm.append(a); mx.append(b)
+            for n, v in zip(names, fl):
                 if v.lower().startswith("active"):
                     reasons.add(n)
         return {"sm_mhz": float(np.median(sm)) if sm else None,
