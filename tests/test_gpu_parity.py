@@ -233,6 +233,26 @@ def test_mla_other_page_sizes(torch_cuda, P):
             print(worst)
 
 
+def test_kv_and_mla_models_share_one_pool(torch_cuda):
+    """GQA, MQA and MLA models colocated in ONE pool of fixed-size pages (page_bytes = the MLA page,
+    73 728 B; the K/V models use the first 32 KiB of theirs): one cp_decode_attention call = one
+    tensor-core launch per attention kind, pages of all models interleaved."""
+    import paper_2606_24506_b200 as cp
+    models = [ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5), ModelCfg(KIND_MLA, 128, 1, 576, 512, 192 ** -0.5),
+              ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5)]
+    w = W.small_workload(models, [0, 1, 2, 1], [700, 900, 1300, 65], page_tokens=64, seed=5, value_scale=0.3,
+                         keep_contiguous=False)
+    assert w.page_bytes == 64 * 576 * 2
+    dw = device_workload(w)
+    c0 = dw.pool.counters()["kernel_launches"]
+    dw.decode()
+    assert dw.pool.counters()["kernel_launches"] - c0 == 2          # one launch per kind, no per-request launches
+    dw.close()
+    for kernel in (0, 2):
+        worst = run_and_compare(w, "mixed_kinds/k%d" % kernel, {cp.CP_OPT_KERNEL: kernel, cp.CP_OPT_MIN_TILE_PAGES: 1})
+        print(worst)
+
+
 # ------------------------------------------------------------------ invariants on the GPU path
 def test_page_permutation_is_bit_identical(torch_cuda):
     """P5 on the GPU: split boundaries are logical, so moving the data to other physical
