@@ -221,18 +221,23 @@ static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, 
         const int ss = cu.split_stride;
 
         float M = -INFINITY, L = 0.f;
-        if (ns <= 64) {
-            // (m, l) of splits lane and lane + 32 stay in registers: one round trip for both passes
-            float2 a = make_float2(-INFINITY, 0.f), b = make_float2(-INFINITY, 0.f);
-            if (lane < ns) a = __ldcg(mlp + lane);
-            if (lane + 32 < ns) b = __ldcg(mlp + lane + 32);
-            M = fmaxf(a.x, b.x);
+        if (ns <= 256) {
+            // (m, l) of splits lane, lane + 32, ... stay in registers: one round trip for both passes
+            float2 ml[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                ml[k] = make_float2(-INFINITY, 0.f);
+                if (lane + 32 * k < ns) ml[k] = __ldcg(mlp + lane + 32 * k);
+            }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) M = fmaxf(M, ml[k].x);
             for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
-            const float wa = ex2_ftz(a.x - M), wb = ex2_ftz(b.x - M);     // 0 for absent splits (m = -inf)
-            if (lane < ns) wsm[lane] = wa;
-            if (lane + 32 < ns) wsm[lane + 32] = wb;
-            L = wa * a.y;
-            L += wb * b.y;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const float w = ex2_ftz(ml[k].x - M);          // 0 for absent splits (m = -inf)
+                if (lane + 32 * k < ns) wsm[lane + 32 * k] = w;
+                L += w * ml[k].y;
+            }
         } else {
             // pass 1: M = max_s m_s (lane-strided, then a fixed tree)
 #pragma unroll 8
