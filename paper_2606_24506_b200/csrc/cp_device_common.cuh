@@ -283,24 +283,15 @@ static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, 
     }
 }
 
-// Persistent-scheduler epilogue: the last CTA to finish resets the counters so that the
-// next launch (stream-ordered) starts from zero without a host memset.
-__device__ inline void scheduler_epilogue(const DecodeParams &p, int *s_flag)
+// The scheduler counters come in two sets used by alternate launches of a plan.  A launch works on
+// one set and, right at its start, one CTA clears the OTHER set -- dirty from the previous launch,
+// which has completed (stream order) -- for the next launch.  Nothing has to be reset at the end
+// of a kernel: no last-CTA election, no atomic round trip on the exit path.
+__device__ inline void scheduler_reset_other_set(const DecodeParams &p)
 {
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        *s_flag = (atomicAdd(p.work_counter + 1, 1) == (int)gridDim.x - 1);
-    }
-    __syncthreads();
-    if (*s_flag) {
-        for (int i = threadIdx.x; i < p.n_groups; i += blockDim.x) p.group_counters[(size_t)i * kCounterStride] = 0;
-        if (threadIdx.x == 0) {
-            p.work_counter[0] = 0;
-            p.work_counter[1] = 0;
-            p.work_counter[2] = 0;
-        }
-    }
+    if (blockIdx.x != gridDim.x - 1) return;
+    for (int i = threadIdx.x; i < p.n_groups; i += blockDim.x) p.reset_counters[32 + (size_t)i * kCounterStride] = 0;
+    if (threadIdx.x < 4) p.reset_counters[threadIdx.x] = 0;
 }
 
 }  // namespace cp

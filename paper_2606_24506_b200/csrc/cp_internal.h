@@ -123,9 +123,9 @@ struct DecodeParams {
     float *out;
     float *lse;
     float *workspace;              // split partials
-    int32_t *work_counter;         // [0] next work item (tile), [1] CTAs that finished,
-                                   // [2] next warp-sized combine unit, [3] pad
+    int32_t *work_counter;         // [0] next work item (tile); [1..3] spare
     int32_t *group_counters;       // [n_groups * kCounterStride] tile arrivals, counter g at g * kCounterStride
+    int32_t *reset_counters;       // the other counter set ([32] scheduler + group counters): cleared by this launch
 };
 
 }  // namespace cp

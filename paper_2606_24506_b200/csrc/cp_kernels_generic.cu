@@ -160,7 +160,6 @@ cp_decode_generic_kernel(const DecodeParams p, int max_dk, int max_dv, int any_k
 {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     __shared__ int s_work;
-    __shared__ int s_flag;
     const int tid = threadIdx.x;
     const int warp = tid >> 5;
     const int lane = tid & 31;
@@ -179,6 +178,7 @@ cp_decode_generic_kernel(const DecodeParams p, int max_dk, int max_dv, int any_k
         sm.l = reinterpret_cast<float *>(ptr);
     }
 
+    scheduler_reset_other_set(p);
     const int n_work = p.n_tiles + p.n_combines;
     for (;;) {
         if (tid == 0) s_work = atomicAdd(p.work_counter, 1);
@@ -347,7 +347,6 @@ cp_decode_generic_kernel(const DecodeParams p, int max_dk, int max_dv, int any_k
             if (tid == 0) red_release_add(p.group_counters + (size_t)tile.group * kCounterStride, 1);
         }
     }
-    scheduler_epilogue(p, &s_flag);
 }
 
 cudaError_t launch_decode_generic(const DecodeParams &p, int max_dk, int max_dv, bool any_kv_kind,

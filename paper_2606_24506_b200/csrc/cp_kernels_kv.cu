@@ -264,6 +264,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
     const int warp = tid >> 5;
     const int lane = tid & 31;
     KV_STAMP(0, tid == 0);
+    scheduler_reset_other_set(p);
 
     if (tid == 0) {
         // full[s]: one arrive.expect_tx by the producer + the TMA transaction bytes.
@@ -535,7 +536,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
 #endif
         KV_STAMP(6, tid == 0);
     }
-    scheduler_epilogue(p, s_flag);
     KV_STAMP(7, tid == 0);
 }
 

@@ -120,6 +120,7 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     const uint32_t st_base = smem_u32(smem + MLA_SMEM_STAGE);
     const uint32_t p_base = smem_u32(smem + MLA_SMEM_P);
     MLA_STAMP(16, tid == 64);
+    scheduler_reset_other_set(p);
 
     if (tid == 0) {
         for (int i = 0; i < MLA_STAGES; ++i) { mbar_init(smem_u32(&mi->full[i]), 1); mbar_init(smem_u32(&mi->empty[i]), 1); }
@@ -474,7 +475,6 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc(tmem, MLA_TMEM_COLS);
-    scheduler_epilogue(p, &mi->flag);
     MLA_STAMP(23, tid == 64);
 }
 

@@ -142,6 +142,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     const uint32_t st_base = smem_u32(smem + M2_SMEM_STAGE);
     const uint32_t p_base = smem_u32(smem + M2_SMEM_P);
     M2_STAMP(16, tid == 64);
+    scheduler_reset_other_set(p);
 
     if (tid == 0) {
         for (int i = 0; i < M2_STAGES; ++i) {
@@ -503,7 +504,6 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     tc_fence_before();
     cluster_sync_all();
     if (warp == 1) tmem_dealloc2(tmem, M2_TMEM_COLS);
-    scheduler_epilogue(p, &mi->flag);
 }
 
 // ----------------------------------------------------------------------------- host side

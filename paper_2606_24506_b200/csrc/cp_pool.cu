@@ -62,6 +62,7 @@ struct KindPlan {
     int max_group = 0;
     bool all_fast = false;           // every group of this kind runs on the tensor-core kernel
     bool uploaded = false;
+    int counter_set = 0;             // scheduler counter set the next launch uses (alternates)
     DevBuf d_groups, d_tiles, d_tile_recs, d_combines, d_cunits, d_counters;   // counters: [32] scheduler + [n_groups * kCounterStride]
 };
 
@@ -404,10 +405,9 @@ cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
 {
     if (kp.uploaded) return CP_OK;
     const size_t gb = kp.groups.size() * sizeof(Group), tb = kp.tiles.size() * sizeof(Tile);
-    const size_t cb = kp.combines.size() * sizeof(Combine), nb = (32 + kp.groups.size() * (size_t)kCounterStride) * 4;
+    const size_t cb = kp.combines.size() * sizeof(Combine), set_ints = 32 + kp.groups.size() * (size_t)kCounterStride, nb = 2 * set_ints * 4;
     const size_t ub = kp.cunits.size() * sizeof(CombineUnit);
     const size_t rb = kp.tile_recs.size() * sizeof(TileRec);
-    const bool counters_new = kp.d_counters.cap < nb;
     if (kp.d_groups.ensure(gb) != cudaSuccess || kp.d_tiles.ensure(tb) != cudaSuccess ||
         kp.d_combines.ensure(std::max(cb, (size_t)16)) != cudaSuccess ||
         kp.d_cunits.ensure(std::max(ub, (size_t)64)) != cudaSuccess ||
@@ -422,9 +422,10 @@ cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
         (rb && cudaMemcpyAsync(kp.d_tile_recs.ptr, kp.tile_recs.data(), rb, cudaMemcpyHostToDevice, stream) != cudaSuccess) ||
         (ub && cudaMemcpyAsync(kp.d_cunits.ptr, kp.cunits.data(), ub, cudaMemcpyHostToDevice, stream) != cudaSuccess))
         return CP_ERR_CUDA;
-    // counters are zero between launches (the kernels reset them); zero a fresh buffer
-    if (counters_new && cudaMemsetAsync(kp.d_counters.ptr, 0, kp.d_counters.cap, stream) != cudaSuccess)
+    // two counter sets for alternate launches (scheduler_reset_other_set); a new plan starts from zero
+    if (cudaMemsetAsync(kp.d_counters.ptr, 0, kp.d_counters.cap, stream) != cudaSuccess)
         return CP_ERR_CUDA;
+    kp.counter_set = 0;
     pool->n_h2d_bytes += gb + tb + cb + ub + rb;
     kp.uploaded = true;
     return CP_OK;
@@ -794,8 +795,11 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.n_groups = (int)kp.groups.size();
         prm.q = (const uint16_t *)q_dev; prm.out = out_dev; prm.lse = lse_dev;
         prm.workspace = (float *)workspace_dev;
-        prm.work_counter = (int32_t *)kp.d_counters.ptr;
-        prm.group_counters = (int32_t *)kp.d_counters.ptr + 32;
+        const size_t set_ints = 32 + kp.groups.size() * (size_t)kCounterStride;
+        prm.work_counter = (int32_t *)kp.d_counters.ptr + kp.counter_set * set_ints;
+        prm.group_counters = prm.work_counter + 32;
+        prm.reset_counters = (int32_t *)kp.d_counters.ptr + (1 - kp.counter_set) * set_ints;
+        kp.counter_set ^= 1;
         const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
         cudaError_t e;
         if (k == CP_KIND_KV && pool->opt_kernel != 1 && kp.all_fast && pool->kv_tmap_ok) {
