@@ -196,6 +196,7 @@ def main():
     ap.add_argument("--min-tile-pages", type=int, default=0, help="CP_OPT_MIN_TILE_PAGES (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (tuning sweeps only)")
+    ap.add_argument("--no-vmm", action="store_true", help="skip the CUDA-VMM arena leg (SURVEY 8(f) N2)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -325,6 +326,60 @@ def main():
                   "note": "back-to-back launches (the gathered copy of a long request exceeds L2)"}
         del gk, gv
 
+    # ---------------- CUDA-VMM-backed arena: the same step on an arena the library maps chunk
+    # by chunk, page ids by arithmetic (no table) and with the identity table read anyway; and what the
+    # slow path costs: mapping / unmapping the longest request's pages, against the software table's
+    vmm = None
+    if rank == 0 and not args.no_vmm:
+        dv = DeviceWorkload(w, dev, vmm=True)
+        dv.pool.set_option(cp.CP_OPT_KERNEL, args.kernel)
+        dv.ensure_workspace()
+        vmm = {"chunk_bytes": dv.pool.vmm_info()["chunk_bytes"], "chunks_mapped": dv.pool.vmm_info()["chunks_mapped"]}
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for table, name in ((0, "us_per_step_no_table"), (1, "us_per_step_identity_table")):
+            dv.pool.set_option(cp.CP_OPT_VMM_TABLE, table)
+            for _ in range(3):
+                dv.decode()
+            ts = []
+            for i in range(min(args.steps, 50)):
+                spacer(i)
+                e0.record()
+                dv.decode()
+                e1.record()
+                torch.cuda.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            vmm[name] = 1e3 * float(np.median(ts))
+        dv.close()
+        del dv
+        ri = max(range(len(w.requests)), key=lambda i: w.requests[i].page_ids.size)
+        rq = w.requests[ri]
+        n_pg = int(rq.page_ids.size)
+        vp = cp.Pool.create_vmm(n_pg * w.page_bytes + (4 << 20), w.page_tokens, w.page_bytes, w.models, 2, n_pg)
+
+        def wall_us(fn):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            fn()
+            return 1e6 * (time.perf_counter() - t0)
+
+        cold = wall_us(lambda: vp.map_pages(0, rq.model_id, None, rq.context_len, n_allocate=n_pg))
+        chunks = vp.vmm_info()["chunks_mapped"]
+        unmap = wall_us(lambda: vp.unmap_request(0))
+        warm = wall_us(lambda: vp.map_pages(0, rq.model_id, None, rq.context_len, n_allocate=n_pg))
+        vp.close()
+        sp = cp.Pool(dw.arena, dw.arena.numel() * 2, w.page_tokens, w.page_bytes, w.num_pages, w.models, 2, n_pg)
+        # (bookkeeping only: this pool never launches, the arena is not touched)
+        soft = wall_us(lambda: sp.map_pages(0, rq.model_id, None, rq.context_len, n_allocate=n_pg))
+        soft_unmap = wall_us(lambda: sp.unmap_request(0))
+        sp.close()
+        vmm["map_unmap_host_us"] = {
+            "pages": n_pg, "chunks": chunks,
+            "vmm_map_cold": cold, "vmm_map_parked_chunks": warm, "vmm_unmap": unmap,
+            "software_table_map": soft, "software_table_unmap": soft_unmap,
+            "note": "host wall clock of one cp_pool_map_pages / cp_pool_unmap_request call for the longest "
+                    "request; cold = cuMemCreate + cuMemMap + cuMemSetAccess per chunk, parked = cuMemMap + "
+                    "cuMemSetAccess; the software table's device upload is deferred to the next compute call"}
+
     # ---------------- KV append step, last because it grows the contexts: one new token
     # per request per call, launch-bound (a few KB per call); reported as us per call on the device
     append = None
@@ -370,7 +425,7 @@ def main():
                     "us_per_step": 1e3 * e2e_ms,
                     "h2d_bytes_per_step": int(q_host.numel() * 2),
                     "d2h_bytes_per_step": int(o_host.numel() * 4 + l_host.numel() * 4)},
-            "gpu_launches": int(launches), "roofline": roof, "gather": gather, "append": append,
+            "gpu_launches": int(launches), "roofline": roof, "gather": gather, "append": append, "vmm_arena": vmm,
             "pct_of_hbm_peak": {"measured_copy": 100 * achieved / peaks["hbm_gbs"], "nominal_8TBs": 100 * achieved / 8000.0}}
 
     if not args.no_cpu_baseline:

@@ -91,7 +91,10 @@ enum {
                                 2 = as 0, but MLA on the single-CTA tcgen05 kernel           */
     CP_OPT_NUM_CTAS = 1,     /* persistent grid size; 0 = number of SMs of the device       */
     CP_OPT_WAVES_X16 = 2,    /* target tiles per CTA, in 1/16 units (default 16 = 1.0)      */
-    CP_OPT_MIN_TILE_PAGES = 3 /* lower bound on pages per tile (default 2)                   */
+    CP_OPT_MIN_TILE_PAGES = 3, /* lower bound on pages per tile (default 2)                  */
+    CP_OPT_VMM_TABLE = 4     /* pool from cp_pool_create_vmm only: 1 = the decode kernels read the
+                                software page table anyway (it holds the same ids; for measuring
+                                what the table costs), 0 (default) = page ids by arithmetic   */
 };
 
 /*
@@ -116,6 +119,39 @@ cp_status cp_pool_create(void *arena_dev, uint64_t arena_bytes,
                          const cp_model_cfg *models, int32_t n_models,
                          int32_t max_requests, int32_t max_pages_per_request,
                          cp_pool **out);
+
+/*
+ * cp_pool_create_vmm -- the same pool on an arena the LIBRARY owns and backs with the CUDA
+ * virtual memory management API: "CUDA VMM APIs to reserve a virtual KV address range for each
+ * model and map physical KV pages on demand".  One virtual
+ * range is reserved and cut into max_requests slots; request id r owns slot r, a contiguous
+ * virtual KV space of slot_pages >= max_pages_per_request pages, so entry i of its page list is
+ * page r * slot_pages + i and the decode kernels need no table lookup (CP_OPT_VMM_TABLE).
+ * Physical memory is created in chunks of the device's allocation granularity (2 MiB) the first
+ * time a request grows into them, and parked for reuse when the request is unmapped; chunks in
+ * existence never exceed physical_budget_bytes / chunk size -- the pool page budget.
+ * Differences from a caller-owned arena:
+ *   - cp_pool_map_pages takes page_ids_host == NULL only (INVALID_ARG otherwise) and maps the
+ *     chunks under the new pages; NO_PAGES when the budget cannot back them (nothing changes);
+ *   - cp_pool_unmap_request synchronises the device, then unmaps the slot's chunks;
+ *   - cp_pool_stats reports free pages as what the chunks still available could hold;
+ *   - cp_pool_free unmaps and releases everything.
+ * Pages of different requests never share a chunk (a slot starts on a chunk boundary).
+ * Errors: INVALID_ARG, UNSUPPORTED (as cp_pool_create), CUDA (no device / driver call failed).
+ */
+cp_status cp_pool_create_vmm(uint64_t physical_budget_bytes,
+                             uint32_t page_tokens, uint32_t page_bytes,
+                             const cp_model_cfg *models, int32_t n_models,
+                             int32_t max_requests, int32_t max_pages_per_request,
+                             cp_pool **out);
+
+/* cp_pool_vmm_info -- geometry and occupancy of a VMM pool (INVALID_ARG for any other pool): base
+ * device address of the reserved range and its size, chunk size, pages per request slot, chunks
+ * mapped now, chunk budget.  Any out pointer may be NULL.  The bytes of request r's pages live at
+ * arena_dev + r * slot_pages * page_bytes; only its mapped prefix may be touched. */
+cp_status cp_pool_vmm_info(const cp_pool *pool, void **arena_dev, uint64_t *va_bytes,
+                           uint64_t *chunk_bytes, uint32_t *slot_pages,
+                           uint32_t *chunks_mapped, uint32_t *chunks_budget);
 
 /* cp_pool_free -- release the library's metadata (host and device).  Never touches the
  * arena.  NULL is accepted. */

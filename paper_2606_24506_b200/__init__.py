@@ -34,6 +34,7 @@ CP_OPT_KERNEL = 0
 CP_OPT_NUM_CTAS = 1
 CP_OPT_WAVES_X16 = 2
 CP_OPT_MIN_TILE_PAGES = 3
+CP_OPT_VMM_TABLE = 4
 
 
 class cp_model_cfg(ctypes.Structure):
@@ -73,6 +74,9 @@ def load_library():
     sig = {
         "cp_pool_create": (i32, [vp, u64, u32, u32, u32, ctypes.POINTER(cp_model_cfg), i32, i32, i32,
                                  ctypes.POINTER(vp)]),
+        "cp_pool_create_vmm": (i32, [u64, u32, u32, ctypes.POINTER(cp_model_cfg), i32, i32, i32,
+                                     ctypes.POINTER(vp)]),
+        "cp_pool_vmm_info": (i32, [vp, ctypes.POINTER(vp), u64p, u64p, u32p, u32p, u32p]),
         "cp_pool_free": (i32, [vp]),
         "cp_pool_map_pages": (i32, [vp, i32, i32, i32p, i32, i32]),
         "cp_pool_unmap_request": (i32, [vp, i32]),
@@ -97,7 +101,7 @@ def load_library():
     return L
 
 
-EXPORTED = ["cp_pool_create", "cp_pool_free", "cp_pool_map_pages", "cp_pool_unmap_request",
+EXPORTED = ["cp_pool_create", "cp_pool_create_vmm", "cp_pool_vmm_info", "cp_pool_free", "cp_pool_map_pages", "cp_pool_unmap_request",
             "cp_pool_request_info", "cp_pool_stats", "cp_pool_set_option", "cp_pool_gather_kv",
             "cp_pool_append_kv",
             "cp_decode_workspace_bytes", "cp_decode_attention", "cp_decode_workspace_bytes_host",
@@ -151,6 +155,36 @@ class Pool:
         self._h = h
         self._L = L
         self._keep = arena_dev        # keep the arena tensor alive
+
+    @staticmethod
+    def _models_array(models):
+        arr = (cp_model_cfg * len(models))()
+        for i, m in enumerate(models):
+            arr[i] = cp_model_cfg(int(m.kind), int(m.n_q_heads), int(m.n_kv_heads), int(m.head_dim_qk),
+                                  int(m.head_dim_v), float(m.softmax_scale))
+        return arr
+
+    @classmethod
+    def create_vmm(cls, physical_budget_bytes: int, page_tokens: int, page_bytes: int, models: Sequence,
+                   max_requests: int, max_pages_per_request: int) -> "Pool":
+        """cp_pool_create_vmm: the library owns the arena (CUDA virtual memory management)."""
+        L = load_library()
+        h = ctypes.c_void_p()
+        _check(L.cp_pool_create_vmm(physical_budget_bytes, page_tokens, page_bytes, cls._models_array(models),
+                                    len(models), max_requests, max_pages_per_request, ctypes.byref(h)),
+               "cp_pool_create_vmm")
+        self = cls.__new__(cls)
+        self._h, self._L, self._keep = h, L, None
+        return self
+
+    def vmm_info(self):
+        base = ctypes.c_void_p()
+        va, chunk = ctypes.c_uint64(), ctypes.c_uint64()
+        sp, cm, cb = ctypes.c_uint32(), ctypes.c_uint32(), ctypes.c_uint32()
+        _check(self._L.cp_pool_vmm_info(self._h, ctypes.byref(base), ctypes.byref(va), ctypes.byref(chunk),
+                                        ctypes.byref(sp), ctypes.byref(cm), ctypes.byref(cb)), "cp_pool_vmm_info")
+        return {"arena_dev": int(base.value or 0), "va_bytes": va.value, "chunk_bytes": chunk.value,
+                "slot_pages": sp.value, "chunks_mapped": cm.value, "chunks_budget": cb.value}
 
     def close(self):
         if getattr(self, "_h", None):

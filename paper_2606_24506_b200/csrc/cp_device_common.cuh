@@ -22,6 +22,14 @@ __device__ __forceinline__ int ld_acquire(const int32_t *p)
     return v;
 }
 
+// Physical page of entry `idx` of request `req`'s page list.  Software table (PAPER.md, reading R1)
+// or, on a CUDA-VMM arena, plain arithmetic on the request's contiguous virtual range.
+__device__ __forceinline__ int32_t page_of(const DecodeParams &p, int req, int64_t idx)
+{
+    if (p.slot_pages > 0) return req * p.slot_pages + (int32_t)idx;
+    return __ldg(p.page_table + (int64_t)req * p.max_ppr + idx);
+}
+
 // Wait until group counter `gi` has reached `want` (called by one lane).  Polls with exponential
 // back-off: hundreds of warps polling one L2 line every few dozen ns would saturate its slice
 // and delay the very arrivals they wait for.

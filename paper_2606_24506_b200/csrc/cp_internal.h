@@ -108,6 +108,8 @@ struct DecodeParams {
     uint32_t page_bytes;
     const int32_t *page_table;     // [max_requests][max_ppr]
     int32_t max_ppr;
+    int32_t slot_pages;            // > 0: contiguous virtual KV (CUDA VMM arena): page idx of request r is
+                                   // r * slot_pages + idx and the decode kernels read no page table
     const int32_t *req_ctx;        // [max_requests] current context length
     const DevModel *models;
     const Group *groups;

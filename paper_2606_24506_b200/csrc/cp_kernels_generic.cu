@@ -203,7 +203,6 @@ cp_decode_generic_kernel(const DecodeParams p, int max_dk, int max_dv, int any_k
         const int ctx = __ldg(p.req_ctx + g.req);
         const int t_begin = tile.page_begin * P;
         const int t_end = min(tile.page_end * P, ctx);
-        const int32_t *pt = p.page_table + (int64_t)g.req * p.max_ppr;
         const int ncol = (dv + GEN_THREADS - 1) / GEN_THREADS;      // 1 or 2 columns per thread
 
         for (int h0 = 0; h0 < m.group; h0 += GEN_HB) {
@@ -231,7 +230,7 @@ cp_decode_generic_kernel(const DecodeParams p, int max_dk, int max_dv, int any_k
                 for (int i = tid; i < nt * kvec; i += GEN_THREADS) {
                     const int r = i / kvec, vch = i % kvec;
                     const int t = t0 + r;
-                    const int32_t pid = __ldg(pt + (int64_t)(t / P) * m.n_kv_heads + g.kv_head);
+                    const int32_t pid = page_of(p, g.req, (int64_t)(t / P) * m.n_kv_heads + g.kv_head);
                     const uint4 val = *reinterpret_cast<const uint4 *>(
                         p.arena + row_byte_offset(p, m, pid, (uint32_t)(t % P), false) + vch * 16);
                     *reinterpret_cast<uint4 *>(sm.k + (size_t)r * krow + vch * 8) = val;
@@ -241,7 +240,7 @@ cp_decode_generic_kernel(const DecodeParams p, int max_dk, int max_dv, int any_k
                     for (int i = tid; i < nt * vvec; i += GEN_THREADS) {
                         const int r = i / vvec, vch = i % vvec;
                         const int t = t0 + r;
-                        const int32_t pid = __ldg(pt + (int64_t)(t / P) * m.n_kv_heads + g.kv_head);
+                        const int32_t pid = page_of(p, g.req, (int64_t)(t / P) * m.n_kv_heads + g.kv_head);
                         const uint4 val = *reinterpret_cast<const uint4 *>(
                             p.arena + row_byte_offset(p, m, pid, (uint32_t)(t % P), true) + vch * 16);
                         *reinterpret_cast<uint4 *>(sm.v + (size_t)r * vrow + vch * 8) = val;

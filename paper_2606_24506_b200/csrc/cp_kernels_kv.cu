@@ -324,13 +324,12 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             ++qi;
             if (item < 0) break;
 
-            const int32_t *pt = p.page_table + (int64_t)r.req * p.max_ppr + r.kv_head;
             const int npg = r.n_pages;
             const int hkv = r.n_kv_heads;
             for (int j0 = 0; j0 < npg; j0 += 32) {
                 // translate up to 32 logical pages at once (step a2: one page-table entry per lane)
                 int32_t pid = 0;
-                if (j0 + lane < npg) pid = __ldg(pt + (int64_t)(r.page_begin + j0 + lane) * hkv);
+                if (j0 + lane < npg) pid = page_of(p, r.req, (int64_t)(r.page_begin + j0 + lane) * hkv + r.kv_head);
                 const int nj = min(32, npg - j0);
                 for (int j = 0; j < nj; ++j) {
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);

@@ -189,11 +189,10 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             if (item < 0) break;
             resident_group = tile.group;
 
-            const int32_t *pt = p.page_table + (int64_t)g.req * p.max_ppr;
             for (int s0 = 0; s0 < n_slices; s0 += 32) {
                 // translate (step a2): one page-table entry per lane; slice s -> page s / spp
                 int32_t pid = 0;
-                if (s0 + lane < n_slices) pid = __ldg(pt + tile.page_begin + (s0 + lane) / spp);
+                if (s0 + lane < n_slices) pid = page_of(p, g.req, tile.page_begin + (s0 + lane) / spp);
                 const int ns = min(32, n_slices - s0);
                 for (int j = 0; j < ns; ++j) {
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);

@@ -176,10 +176,9 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
         for (int k = 0;; ++k) {
             const M2Item it = m2_item(p, pair + k * n_pairs);
             if (!it.valid) break;
-            const int32_t *pt = p.page_table + (int64_t)it.req * p.max_ppr;
             for (int s0 = 0; s0 < it.n_slices; s0 += 32) {
                 int32_t pid = 0;
-                if (s0 + lane < it.n_slices) pid = __ldg(pt + it.page_begin + (s0 + lane) / spp);
+                if (s0 + lane < it.n_slices) pid = page_of(p, it.req, it.page_begin + (s0 + lane) / spp);
                 const int ns = min(32, it.n_slices - s0);
                 for (int j = 0; j < ns; ++j) {
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);

@@ -13,6 +13,7 @@
 #include "../../include/crosspool.h"
 #include "cp_internal.h"
 #include "cp_launch.h"
+#include "cp_vmm.h"
 
 using namespace cp;
 
@@ -82,6 +83,12 @@ struct cp_pool {
     std::vector<int32_t> h_ctx;          // host mirror of the device ctx table
     int32_t ctx_dirty_lo = INT32_MAX, ctx_dirty_hi = -1;
     uint64_t topo_version = 1;           // bumps when any request's planned page count changes
+
+    // CUDA-VMM arena: the library owns the arena; request r's pages are the contiguous ids
+    // r * slot_pages .. and physical chunks are mapped as the request grows
+    VmmArena *vmm = nullptr;
+    uint32_t slot_pages = 0;
+    int opt_vmm_table = 0;               // 1: decode kernels read the (identity) page table anyway
 
     // options
     int opt_kernel = 0, opt_num_ctas = 0, opt_waves_x16 = 16, opt_min_tile_pages = 2;
@@ -488,10 +495,59 @@ cp_status cp_pool_create(void *arena_dev, uint64_t arena_bytes, uint32_t page_to
     return CP_OK;
 }
 
+cp_status cp_pool_create_vmm(uint64_t physical_budget_bytes, uint32_t page_tokens, uint32_t page_bytes,
+                             const cp_model_cfg *models, int32_t n_models, int32_t max_requests,
+                             int32_t max_pages_per_request, cp_pool **out)
+{
+    if (!out) return CP_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!models || n_models < 1 || max_requests < 1 || max_pages_per_request < 1 || physical_budget_bytes == 0)
+        return CP_ERR_INVALID_ARG;
+    if (page_tokens < 1 || page_tokens > 256 || page_bytes < 16 || page_bytes % 16) return CP_ERR_INVALID_ARG;
+    for (int i = 0; i < n_models; ++i)
+        if (!model_supported(models[i], page_tokens, page_bytes)) return CP_ERR_UNSUPPORTED;
+    VmmArena *vmm = nullptr;
+    const int rc = vmm_create(&vmm, (uint64_t)max_pages_per_request * page_bytes, max_requests, physical_budget_bytes,
+                              page_bytes);
+    if (rc != 0) return CP_ERR_CUDA;
+    const uint64_t slot_pages = vmm->slot_bytes / page_bytes;
+    const uint64_t num_pages = slot_pages * (uint64_t)max_requests;
+    if (num_pages > (uint64_t)INT32_MAX || vmm->budget_chunks == 0) {
+        vmm_destroy(vmm);
+        return CP_ERR_INVALID_ARG;
+    }
+    cp_pool *p = nullptr;
+    const cp_status st = cp_pool_create((void *)(uintptr_t)vmm->base, vmm->va_bytes, page_tokens, page_bytes,
+                                        (uint32_t)num_pages, models, n_models, max_requests,
+                                        max_pages_per_request, &p);
+    if (st != CP_OK) {
+        vmm_destroy(vmm);
+        return st;
+    }
+    p->vmm = vmm;
+    p->slot_pages = (uint32_t)slot_pages;
+    *out = p;
+    return CP_OK;
+}
+
+cp_status cp_pool_vmm_info(const cp_pool *pool, void **arena_dev, uint64_t *va_bytes, uint64_t *chunk_bytes,
+                           uint32_t *slot_pages, uint32_t *chunks_mapped, uint32_t *chunks_budget)
+{
+    if (!pool || !pool->vmm) return CP_ERR_INVALID_ARG;
+    if (arena_dev) *arena_dev = (void *)(uintptr_t)pool->vmm->base;
+    if (va_bytes) *va_bytes = pool->vmm->va_bytes;
+    if (chunk_bytes) *chunk_bytes = pool->vmm->chunk_bytes;
+    if (slot_pages) *slot_pages = pool->slot_pages;
+    if (chunks_mapped) *chunks_mapped = vmm_chunks_mapped(pool->vmm);
+    if (chunks_budget) *chunks_budget = pool->vmm->budget_chunks;
+    return CP_OK;
+}
+
 cp_status cp_pool_free(cp_pool *pool)
 {
     if (!pool) return CP_OK;
-    if (pool->dev_ready) cudaDeviceSynchronize();
+    if (pool->dev_ready || pool->vmm) cudaDeviceSynchronize();
+    if (pool->vmm) { vmm_destroy(pool->vmm); pool->vmm = nullptr; }
     pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release(); pool->d_append.release();
     for (int k = 0; k < 2; ++k) {
         pool->plan[k].d_groups.release(); pool->plan[k].d_tiles.release();
@@ -522,7 +578,16 @@ cp_status cp_pool_map_pages(cp_pool *pool, int32_t request_id, int32_t model_id,
     std::vector<int32_t> fresh;
     if (n_page_ids > 0) {
         fresh.resize(n_page_ids);
-        if (page_ids_host) {
+        if (pool->vmm) {
+            // contiguous virtual KV: the ids are the next entries of the request's slot; the physical
+            // chunks under them are mapped below, after every check has passed
+            if (page_ids_host) return CP_ERR_INVALID_ARG;
+            for (int i = 0; i < n_page_ids; ++i)
+                fresh[i] = (int32_t)((size_t)request_id * pool->slot_pages + have + i);
+            const int rc = vmm_back(pool->vmm, request_id, (uint64_t)total * pool->page_bytes);
+            if (rc == 3) return CP_ERR_NO_PAGES;
+            if (rc != 0) return CP_ERR_CUDA;
+        } else if (page_ids_host) {
             for (int i = 0; i < n_page_ids; ++i) {
                 const int32_t pid = page_ids_host[i];
                 if (pid < 0 || (uint32_t)pid >= pool->num_pages) return CP_ERR_PAGE_RANGE;
@@ -567,6 +632,11 @@ cp_status cp_pool_unmap_request(cp_pool *pool, int32_t request_id)
     if (!r.live) return CP_ERR_UNKNOWN_REQUEST;
     for (int32_t pid : r.pages) pool->owner[pid] = -1;
     pool->n_free += (uint32_t)r.pages.size();
+    if (pool->vmm) {
+        // kernels that may still read the slot must have finished before its memory is unmapped
+        cudaDeviceSynchronize();
+        if (vmm_release_slot(pool->vmm, request_id) != 0) { cudaGetLastError(); }
+    }
     r = Request();
     pool->topo_version++;
     return CP_OK;
@@ -590,6 +660,12 @@ cp_status cp_pool_request_info(const cp_pool *pool, int32_t request_id, int32_t 
 cp_status cp_pool_stats(const cp_pool *pool, uint32_t *free_pages, uint32_t *used_pages)
 {
     if (!pool) return CP_ERR_INVALID_ARG;
+    if (pool->vmm) {
+        // physical terms: pages that the chunks still available could hold / pages mapped to requests
+        if (free_pages) *free_pages = (uint32_t)((uint64_t)vmm_chunks_available(pool->vmm) * pool->vmm->chunk_bytes / pool->page_bytes);
+        if (used_pages) *used_pages = pool->num_pages - pool->n_free;
+        return CP_OK;
+    }
     if (free_pages) *free_pages = pool->n_free;
     if (used_pages) *used_pages = pool->num_pages - pool->n_free;
     return CP_OK;
@@ -611,6 +687,9 @@ cp_status cp_pool_set_option(cp_pool *pool, int32_t key, int64_t value)
     case CP_OPT_MIN_TILE_PAGES:
         if (value < 1 || value > (1 << 20)) return CP_ERR_INVALID_ARG;
         pool->opt_min_tile_pages = (int)value; break;
+    case CP_OPT_VMM_TABLE:
+        if (value < 0 || value > 1) return CP_ERR_INVALID_ARG;
+        pool->opt_vmm_table = (int)value; break;
     default: return CP_ERR_INVALID_ARG;
     }
     pool->plan_valid = false;
@@ -694,7 +773,7 @@ cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int3
     if (!k_new_dev || ((uintptr_t)k_new_dev & 15u) || ((uintptr_t)v_new_dev & 15u)) return CP_ERR_INVALID_ARG;
     // validate the whole batch first (all-or-nothing): capacity of the page lists, page budget
     const int P = (int)pool->P;
-    uint32_t need_pages = 0;
+    uint32_t need_pages = 0, need_chunks = 0;
     bool any_v = false;
     for (int b = 0; b < n_requests; ++b) {
         const Request &r = pool->reqs[request_ids_host[b]];
@@ -705,10 +784,13 @@ cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int3
         if ((size_t)(r.ctx / P) >= have_lp) {                 // position r.ctx opens a new logical page
             if (r.pages.size() + m.n_kv_heads > (size_t)pool->max_ppr) return CP_ERR_INVALID_ARG;
             need_pages += (uint32_t)m.n_kv_heads;
+            if (pool->vmm)
+                need_chunks += vmm_chunks_missing(pool->vmm, request_ids_host[b],
+                                                  (uint64_t)(r.pages.size() + m.n_kv_heads) * pool->page_bytes);
         }
     }
     if (any_v && !v_new_dev) return CP_ERR_INVALID_ARG;
-    if (need_pages > pool->n_free) return CP_ERR_NO_PAGES;
+    if (pool->vmm ? need_chunks > vmm_chunks_available(pool->vmm) : need_pages > pool->n_free) return CP_ERR_NO_PAGES;
     st = ensure_device(pool);
     if (st != CP_OK) return st;
     cudaStream_t s = (cudaStream_t)stream;
@@ -723,7 +805,15 @@ cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int3
         const int rid = request_ids_host[b];
         Request &r = pool->reqs[rid];
         const cp_model_cfg &m = pool->models[r.model];
-        if ((size_t)(r.ctx / P) >= r.pages.size() / m.n_kv_heads) {
+        if ((size_t)(r.ctx / P) >= r.pages.size() / m.n_kv_heads && pool->vmm) {
+            const uint64_t total = r.pages.size() + m.n_kv_heads;
+            if (vmm_back(pool->vmm, rid, total * pool->page_bytes) != 0) return CP_ERR_CUDA;   // budget checked above
+            for (int i = 0; i < m.n_kv_heads; ++i) {
+                const int32_t pid = (int32_t)((size_t)rid * pool->slot_pages + r.pages.size());
+                pool->owner[pid] = rid; r.pages.push_back(pid);
+            }
+            pool->n_free -= (uint32_t)m.n_kv_heads;
+        } else if ((size_t)(r.ctx / P) >= r.pages.size() / m.n_kv_heads) {
             uint32_t cur = pool->alloc_cursor;
             for (int i = 0; i < m.n_kv_heads;) {
                 if (pool->owner[cur] == -1) { pool->owner[cur] = rid; r.pages.push_back((int32_t)cur); ++i; }
@@ -783,6 +873,7 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         DecodeParams prm;
         prm.arena = pool->arena; prm.page_tokens = pool->P; prm.page_bytes = pool->page_bytes;
         prm.page_table = (const int32_t *)pool->d_page_table.ptr; prm.max_ppr = pool->max_ppr;
+        prm.slot_pages = (pool->vmm && !pool->opt_vmm_table) ? (int32_t)pool->slot_pages : 0;
         prm.req_ctx = (const int32_t *)pool->d_ctx.ptr;
         prm.models = (const DevModel *)pool->d_models.ptr;
         prm.groups = (const Group *)kp.d_groups.ptr;

@@ -11,21 +11,55 @@ import torch
 from . import Pool
 
 
+class _RawDeviceBytes:
+    """CUDA array interface over a raw device address (memory the library mapped, not torch)."""
+
+    def __init__(self, ptr: int, nbytes: int):
+        self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False),
+                                         "version": 3, "strides": None}
+
+
+def raw_device_tensor(ptr: int, nbytes: int, device) -> torch.Tensor:
+    """uint8 tensor view of `nbytes` at device address `ptr` (no copy, no ownership)."""
+    return torch.as_tensor(_RawDeviceBytes(ptr, nbytes), device=device)
+
+
 class DeviceWorkload:
     """A `workloads.Workload` resident on the GPU behind a cp_pool."""
 
-    def __init__(self, w, device: str = "cuda:0", map_requests: bool = True, page_list_slack: int = 0):
+    def __init__(self, w, device: str = "cuda:0", map_requests: bool = True, page_list_slack: int = 0,
+                 vmm: bool = False, vmm_budget_bytes: int = 0):
         self.w = w
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        # arena: one contiguous device buffer (torch allocations are >= 256-B aligned)
-        self.arena = torch.from_numpy(w.arena.view(np.int16)).to(self.device)
         max_ppr = max(r.page_ids.size for r in w.requests) + page_list_slack    # room for appended pages
-        self.pool = Pool(self.arena, self.arena.numel() * 2, w.page_tokens, w.page_bytes, w.num_pages,
-                         w.models, max_requests=len(w.requests), max_pages_per_request=max_ppr)
-        if map_requests:
-            for r in w.requests:
-                self.pool.map_pages(r.request_id, r.model_id, r.page_ids, r.context_len)
+        self.vmm = vmm
+        if vmm:
+            # the library owns the arena (cp_pool_create_vmm): every request gets its contiguous virtual
+            # slot, and the request's pages of the host image are copied there in page-list order
+            torch.zeros(1, device=self.device)                       # make sure the context exists
+            budget = vmm_budget_bytes or (w.num_pages * w.page_bytes + (len(w.requests) + 1) * (4 << 20))
+            self.arena = None
+            self.pool = Pool.create_vmm(budget, w.page_tokens, w.page_bytes, w.models,
+                                        max_requests=len(w.requests), max_pages_per_request=max_ppr)
+            if map_requests:
+                info = self.pool.vmm_info()
+                pages = w.arena.reshape(w.num_pages, w.page_bytes // 2)
+                for r in w.requests:
+                    self.pool.map_pages(r.request_id, r.model_id, None, r.context_len, n_allocate=r.page_ids.size)
+                    src = torch.from_numpy(np.ascontiguousarray(pages[r.page_ids]).view(np.int16)).to(self.device)
+                    dst = raw_device_tensor(info["arena_dev"] + r.request_id * info["slot_pages"] * w.page_bytes,
+                                            src.numel() * 2, self.device).view(torch.int16)
+                    dst.copy_(src.reshape(-1))
+                torch.cuda.synchronize(self.device)
+        else:
+            # arena: one contiguous device buffer (torch allocations are >= 256-B aligned)
+            self.arena = torch.from_numpy(w.arena.view(np.int16)).to(self.device)
+            self.pool = Pool(self.arena, self.arena.numel() * 2, w.page_tokens, w.page_bytes, w.num_pages,
+                             w.models, max_requests=len(w.requests), max_pages_per_request=max_ppr)
+            if map_requests:
+                for r in w.requests:
+                    self.pool.map_pages(r.request_id, r.model_id, r.page_ids, r.context_len)
         self.ids = np.array([r.request_id for r in w.requests], dtype=np.int32)
         self.q = torch.from_numpy(w.q_packed().view(np.int16)).to(self.device)
         rows = w.out_rows()

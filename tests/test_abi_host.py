@@ -232,3 +232,26 @@ def test_append_kv_host_validation_is_all_or_nothing():
     assert e.value.status == cp.CP_ERR_INVALID_ARG
     assert before == (p.stats(), [p.request_info(i)[:2] for i in range(3)])
     p.close()
+
+
+def test_vmm_pool_fails_loudly_without_a_device():
+    """cp_pool_create_vmm needs the driver (it reserves device virtual memory): argument errors are
+    reported first, then CP_ERR_CUDA on a host without a GPU -- never a host-memory stand-in."""
+    import torch
+    m = ModelCfg(KIND_KV, 8, 1, 128, 128, 0.1)
+    with pytest.raises(cp.CrossPoolError) as e:
+        cp.Pool.create_vmm(0, 16, 8192, [m], 4, 64)
+    assert e.value.status == cp.CP_ERR_INVALID_ARG
+    with pytest.raises(cp.CrossPoolError) as e:
+        cp.Pool.create_vmm(1 << 22, 16, 4096, [m], 4, 64)          # page too small for the model
+    assert e.value.status == cp.CP_ERR_UNSUPPORTED
+    if torch.cuda.is_available():
+        pytest.skip("CUDA present: the VMM arena itself is covered by tests/test_gpu_vmm.py")
+    with pytest.raises(cp.CrossPoolError) as e:
+        cp.Pool.create_vmm(1 << 22, 16, 8192, [m], 4, 64)
+    assert e.value.status == cp.CP_ERR_CUDA
+    p = make_pool()
+    with pytest.raises(cp.CrossPoolError) as e:
+        p.vmm_info()
+    assert e.value.status == cp.CP_ERR_INVALID_ARG
+    p.close()
