@@ -53,6 +53,15 @@ def lib():
                                     ctypes.c_int, ctypes.c_float,
                                     i32p, ctypes.c_int, ctypes.c_int,
                                     u16p, i32p, ctypes.c_int, ctypes.c_int, f64p, f64p]
+        i64p = ctypes.POINTER(ctypes.c_int64)
+        L.cpo_active_tokens.restype = ctypes.c_double
+        L.cpo_active_tokens.argtypes = [ctypes.c_double] * 4
+        L.cpo_pool_demand.restype = ctypes.c_int
+        L.cpo_pool_demand.argtypes = [ctypes.c_int, i64p, f64p, f64p, f64p, f64p, f64p, ctypes.c_int64, f64p, f64p]
+        L.cpo_quantile.restype = ctypes.c_int
+        L.cpo_quantile.argtypes = [f64p, ctypes.c_int64, ctypes.c_double, f64p, f64p]
+        L.cpo_page_budget.restype = ctypes.c_int64
+        L.cpo_page_budget.argtypes = [ctypes.c_double, ctypes.c_double]
         _lib = L
     return _lib
 
@@ -142,3 +151,41 @@ def decode_workload(w, heads_per_request: Optional[Sequence[Optional[Sequence[in
                              m.softmax_scale, r.page_ids, r.context_len, w.q[i],
                              heads=heads, n_splits=n_splits))
     return res
+
+
+# ---------------------------------------------------------------- KV-cache planner (Eq. (1)-(2))
+def active_tokens(u: float, o_p: float, o_d: float, t_res: float) -> float:
+    """Q_i(u) of Eq. (1)."""
+    return float(lib().cpo_active_tokens(float(u), float(o_p), float(o_d), float(t_res)))
+
+
+def pool_demand(offsets, kappa, arrival, o_p, o_d, t_res, t_obs) -> np.ndarray:
+    """K_pool(t) of Eq. (1)-(2) at every observation time (bytes, float64).  Model M owns trace
+    entries offsets[M] .. offsets[M+1]-1."""
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    arrs = [np.ascontiguousarray(a, dtype=np.float64) for a in (kappa, arrival, o_p, o_d, t_res, t_obs)]
+    kappa, arrival, o_p, o_d, t_res, t_obs = arrs
+    assert offsets.size == kappa.size + 1 and offsets[-1] == arrival.size == o_p.size == o_d.size == t_res.size
+    out = np.empty(t_obs.size, dtype=np.float64)
+    rc = lib().cpo_pool_demand(kappa.size, _p(offsets, ctypes.c_int64), _p(kappa, ctypes.c_double),
+                               _p(arrival, ctypes.c_double), _p(o_p, ctypes.c_double), _p(o_d, ctypes.c_double),
+                               _p(t_res, ctypes.c_double), t_obs.size, _p(t_obs, ctypes.c_double),
+                               _p(out, ctypes.c_double))
+    if rc != 0:
+        raise ValueError("cpo_pool_demand failed: %d" % rc)
+    return out
+
+
+def quantile(x, q: float) -> float:
+    """Empirical quantile x_(ceil(q n)) (no interpolation)."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    scratch = np.empty_like(x)
+    out = ctypes.c_double()
+    rc = lib().cpo_quantile(_p(x, ctypes.c_double), x.size, float(q), _p(scratch, ctypes.c_double), ctypes.byref(out))
+    if rc != 0:
+        raise ValueError("cpo_quantile failed: %d" % rc)
+    return float(out.value)
+
+
+def page_budget(k_bytes: float, page_bytes: float) -> int:
+    return int(lib().cpo_page_budget(float(k_bytes), float(page_bytes)))

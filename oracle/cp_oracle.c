@@ -297,3 +297,74 @@ int cpo_attention(const uint16_t *arena, uint32_t page_tokens, uint32_t page_byt
     }
     return failed ? CPO_ERR_MEM : CPO_OK;
 }
+
+/* ==========================================================================================
+ * KV-cache planner (Eq. (1)-(2)).  TEST INFRASTRUCTURE, as
+ * everything in this file.  Written out term by term in the paper's order and notation:
+ *
+ *   Q_i(u)     = (O_p,i + O_d,i * u / T_i) * 1{0 <= u < T_i}            active KV tokens at age u
+ *   K_M(t)     = sum_i kappa(M) * Q_i(t - A_i)                          Eq. (1)
+ *   K_pool(t)  = sum_M K_M(t)                                           Eq. (2)
+ *
+ * and the "P95/P99 trace-driven Monte Carlo quantile" (L112): K_pool evaluated at random
+ * observation times t_n over the trace (the draws are an INPUT), then the empirical quantile;
+ * "the planner rounds memory to pages and sets the shared KV-cache pool page budget".
+ * Readings: u / T_i is computed before the product with O_d,i; each term
+ * kappa * Q is rounded and added in trace order, models in index order; the empirical quantile
+ * is the order statistic x_(k), k = ceil(q * N) (1-based, no interpolation -- the conservative
+ * side); pages = ceil(K_q / page_bytes).
+ * Pins (tests/test_oracle_pins.py P14-P18): a request worked by hand and its interval ends; the
+ * exact time integral kappa * sum_i T_i (O_p,i + O_d,i / 2); linearity over models; the quantile
+ * against a sort on small vectors and its special cases; Little's law on a long Poisson trace.
+ * ========================================================================================== */
+
+/* Eq. (1), first line. */
+double cpo_active_tokens(double u, double o_p, double o_d, double t_res)
+{
+    if (!(u >= 0.0 && u < t_res)) return 0.0;
+    return o_p + o_d * (u / t_res);
+}
+
+/* Eq. (1)-(2) at n_t observation times.  Model M owns trace entries [offs[M], offs[M+1]). */
+int cpo_pool_demand(int n_models, const int64_t *offs, const double *kappa, const double *arrival,
+                    const double *o_p, const double *o_d, const double *t_res, int64_t n_t,
+                    const double *t_obs, double *k_pool)
+{
+    if (n_models < 0 || n_t < 0) return -1;
+    for (int64_t n = 0; n < n_t; ++n) {
+        double pool = 0.0;
+        for (int m = 0; m < n_models; ++m) {
+            double k_m = 0.0;
+            for (int64_t i = offs[m]; i < offs[m + 1]; ++i)
+                k_m += kappa[m] * cpo_active_tokens(t_obs[n] - arrival[i], o_p[i], o_d[i], t_res[i]);
+            pool += k_m;
+        }
+        k_pool[n] = pool;
+    }
+    return 0;
+}
+
+static int cmp_double(const void *a, const void *b)
+{
+    const double x = *(const double *)a, y = *(const double *)b;
+    return (x > y) - (x < y);
+}
+
+/* Empirical quantile: x_(k) with k = ceil(q * n), clamped to 1 .. n.  scratch: n doubles. */
+int cpo_quantile(const double *x, int64_t n, double q, double *scratch, double *out)
+{
+    if (n < 1 || !(q > 0.0 && q <= 1.0)) return -1;
+    for (int64_t i = 0; i < n; ++i) scratch[i] = x[i];
+    qsort(scratch, (size_t)n, sizeof(double), cmp_double);
+    int64_t k = (int64_t)ceil(q * (double)n);
+    if (k < 1) k = 1;
+    if (k > n) k = n;
+    *out = scratch[k - 1];
+    return 0;
+}
+
+/* "rounds memory to pages": pages that hold k_bytes. */
+int64_t cpo_page_budget(double k_bytes, double page_bytes)
+{
+    return (int64_t)ceil(k_bytes / page_bytes);
+}
