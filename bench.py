@@ -197,6 +197,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (tuning sweeps only)")
     ap.add_argument("--no-vmm", action="store_true", help="skip the CUDA-VMM arena leg (SURVEY 8(f) N2)")
+    ap.add_argument("--no-planner", action="store_true", help="skip the KV-cache planner leg (SURVEY 8(f) N3)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -380,6 +381,43 @@ def main():
                     "request; cold = cuMemCreate + cuMemMap + cuMemSetAccess per chunk, parked = cuMemMap + "
                     "cuMemSetAccess; the software table's device upload is deferred to the next compute call"}
 
+    # ---------------- KV-cache planner (Eq. (1)-(2)): pool demand at 100 000 observation
+    # times of a two-hour synthetic trace of 8 cold models, then P95 / P99 and the page budgets
+    planner = None
+    if rank == 0 and not args.no_planner:
+        from workloads.planner_traces import planner_trace
+        tr = planner_trace(1)
+        td = [torch.from_numpy(a).to(dev) for a in (tr.arrival, tr.o_p, tr.o_d, tr.t_res, tr.t_obs)]
+        kp = torch.empty(tr.t_obs.size, dtype=torch.float64, device=dev)
+        wsb = cp.planner_workspace_bytes()
+        pws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+        st = dw.stream()
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d_us, q_us = [], []
+        for i in range(6):
+            p0.record()
+            cp.planner_pool_demand(tr.offsets, tr.kappa, td[0], td[1], td[2], td[3], tr.t_obs.size, td[4], kp, pws, wsb, st)
+            p1.record()
+            torch.cuda.synchronize()
+            d_us.append(1e3 * p0.elapsed_time(p1))
+            t0 = time.perf_counter()
+            budgets = {q: cp.planner_quantile(kp, tr.t_obs.size, q, float(w.page_bytes), pws, wsb, st) for q in (0.95, 0.99)}
+            q_us.append(1e6 * (time.perf_counter() - t0) / 2)
+        planner = {"models": tr.n_models, "trace_requests": tr.n_requests, "observations": int(tr.t_obs.size),
+                   "demand_us": float(np.median(d_us[1:])), "quantile_us_host_wall": float(np.median(q_us[1:])),
+                   "observations_per_s": tr.t_obs.size / (float(np.median(d_us[1:])) * 1e-6),
+                   "p95_gib": budgets[0.95][0] / 2 ** 30, "p99_gib": budgets[0.99][0] / 2 ** 30,
+                   "p95_pages": budgets[0.95][1], "p99_pages": budgets[0.99][1], "page_bytes": int(w.page_bytes),
+                   "dtype": "f64"}
+        if not args.no_cpu_baseline:
+            import oracle
+            n_s = 2000
+            t0 = time.perf_counter()
+            oracle.pool_demand(tr.offsets, tr.kappa, tr.arrival, tr.o_p, tr.o_d, tr.t_res, tr.t_obs[:n_s])
+            planner["cpu_oracle_observations_per_s"] = n_s / (time.perf_counter() - t0)
+            planner["cpu_oracle_sample"] = "%d of the observation times, one core" % n_s
+        del td, kp, pws
+
     # ---------------- KV append step, last because it grows the contexts: one new token
     # per request per call, launch-bound (a few KB per call); reported as us per call on the device
     append = None
@@ -425,7 +463,7 @@ def main():
                     "us_per_step": 1e3 * e2e_ms,
                     "h2d_bytes_per_step": int(q_host.numel() * 2),
                     "d2h_bytes_per_step": int(o_host.numel() * 4 + l_host.numel() * 4)},
-            "gpu_launches": int(launches), "roofline": roof, "gather": gather, "append": append, "vmm_arena": vmm,
+            "gpu_launches": int(launches), "roofline": roof, "gather": gather, "append": append, "vmm_arena": vmm, "planner": planner,
             "pct_of_hbm_peak": {"measured_copy": 100 * achieved / peaks["hbm_gbs"], "nominal_8TBs": 100 * achieved / 8000.0}}
 
     if not args.no_cpu_baseline:

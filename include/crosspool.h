@@ -279,6 +279,51 @@ cp_status cp_decode_plan(cp_pool *pool, const int32_t *request_ids_host, int32_t
 cp_status cp_pool_counters(const cp_pool *pool, uint64_t *kernel_launches,
                            uint64_t *plan_builds, uint64_t *metadata_h2d_bytes);
 
+/*
+ * KV-cache planner: "The planner uses per-model prompt, output, and service-time
+ * samples, arrival rate, page size, per-token KV bytes kappa(M), and a target provisioning
+ * quantile.  It emits ... the total KV-cache pool page budget".  For request i of
+ * model M arriving at A_i with O_p,i prompt tokens, O_d,i output tokens and decode residence T_i,
+ *     Q_i(u) = (O_p,i + O_d,i u / T_i) 1{0 <= u < T_i},   K_M(t) = sum_i kappa(M) Q_i(t - A_i)   (1)
+ *     K_pool(t) = sum_M K_M(t)                                                                  (2)
+ * and the budget is the "P95/P99 trace-driven Monte Carlo quantile" of K_pool over random
+ * observation times, rounded up to pages (L112).  The observation times are drawn by the caller.
+ * All arithmetic is float64, each operation rounded separately in the order written above (terms in
+ * trace order, models in index order), so results equal a sequential evaluation bit for bit.
+ * The pool these numbers size is created with num_pages (cp_pool_create) or physical_budget_bytes
+ * (cp_pool_create_vmm) = the budget; the planner functions need no cp_pool.
+ *
+ * cp_planner_pool_demand -- K_pool at n_obs observation times (asynchronous on `stream`).
+ *   n_models             1 .. CP_PLANNER_MAX_MODELS
+ *   trace_offsets_host   [n_models + 1], offsets[0] = 0, non-decreasing: model M owns trace entries
+ *                        offsets[M] .. offsets[M+1]-1 of the four trace arrays
+ *   kappa_host           [n_models] per-token KV bytes, >= 0
+ *   arrival_dev          A_i (s), ASCENDING inside each model (precondition, not checked)
+ *   prompt_tokens_dev, output_tokens_dev, residence_dev   O_p,i, O_d,i, T_i (doubles; T_i <= 0
+ *                        makes the request contribute nothing)
+ *   t_obs_dev / k_pool_dev   [n_obs] in / out (bytes)
+ *   workspace_dev        >= cp_planner_workspace_bytes() bytes, 16-B aligned, caller-owned
+ * Errors: INVALID_ARG, WORKSPACE, CUDA.
+ *
+ * cp_planner_quantile -- the empirical quantile x_(k), k = ceil(q n) (1-based order statistic, no
+ * interpolation: at least a fraction q of the values is <= it) of n finite NON-NEGATIVE doubles in
+ * device memory, and pages = ceil(x_(k) / page_bytes).  Exact selection (radix select on the bit
+ * patterns); values_dev is not modified.  Synchronises `stream` and writes the two results to the
+ * host.  Either out pointer may be NULL.  Errors: INVALID_ARG (n < 1, q outside (0, 1]), WORKSPACE,
+ * CUDA.
+ */
+#define CP_PLANNER_MAX_MODELS 64
+uint64_t cp_planner_workspace_bytes(void);
+cp_status cp_planner_pool_demand(int32_t n_models, const int64_t *trace_offsets_host,
+                                 const double *kappa_host, const double *arrival_dev,
+                                 const double *prompt_tokens_dev, const double *output_tokens_dev,
+                                 const double *residence_dev, int64_t n_obs, const double *t_obs_dev,
+                                 double *k_pool_dev, void *workspace_dev, uint64_t workspace_bytes,
+                                 void *stream);
+cp_status cp_planner_quantile(const double *values_dev, int64_t n, double q, double page_bytes,
+                              void *workspace_dev, uint64_t workspace_bytes,
+                              double *quantile_out_host, uint64_t *pages_out_host, void *stream);
+
 /* cp_status_string -- static, never NULL. */
 const char *cp_status_string(cp_status status);
 

@@ -92,6 +92,11 @@ def load_library():
         "cp_decode_plan": (i32, [vp, i32p, i32, ctypes.POINTER(cp_tile_info), i32, i32p, i32p]),
         "cp_pool_counters": (i32, [vp, u64p, u64p, u64p]),
         "cp_status_string": (ctypes.c_char_p, [i32]),
+        "cp_planner_workspace_bytes": (u64, []),
+        "cp_planner_pool_demand": (i32, [i32, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_double),
+                                         vp, vp, vp, vp, ctypes.c_int64, vp, vp, vp, u64, vp]),
+        "cp_planner_quantile": (i32, [vp, ctypes.c_int64, ctypes.c_double, ctypes.c_double, vp, u64,
+                                      ctypes.POINTER(ctypes.c_double), u64p, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -105,7 +110,8 @@ EXPORTED = ["cp_pool_create", "cp_pool_create_vmm", "cp_pool_vmm_info", "cp_pool
             "cp_pool_request_info", "cp_pool_stats", "cp_pool_set_option", "cp_pool_gather_kv",
             "cp_pool_append_kv",
             "cp_decode_workspace_bytes", "cp_decode_attention", "cp_decode_workspace_bytes_host",
-            "cp_decode_attention_host", "cp_decode_plan", "cp_pool_counters", "cp_status_string"]
+            "cp_decode_attention_host", "cp_decode_plan", "cp_pool_counters", "cp_status_string",
+            "cp_planner_workspace_bytes", "cp_planner_pool_demand", "cp_planner_quantile"]
 
 
 def status_string(status: int) -> str:
@@ -278,3 +284,32 @@ class Pool:
         _check(self._L.cp_decode_attention_host(self._h, _i32p(ids), ids.size, _ptr(q_host), _ptr(out_host),
                                                 _ptr(lse_host), _ptr(workspace_dev), workspace_bytes, stream),
                "cp_decode_attention_host")
+
+
+# ---------------------------------------------------------------- KV-cache planner (Eq. (1)-(2))
+def planner_workspace_bytes() -> int:
+    return int(load_library().cp_planner_workspace_bytes())
+
+
+def planner_pool_demand(trace_offsets, kappa, arrival_dev, prompt_tokens_dev, output_tokens_dev, residence_dev,
+                        n_obs: int, t_obs_dev, k_pool_dev, workspace_dev, workspace_bytes: int, stream: int = 0):
+    """cp_planner_pool_demand: K_pool(t) at the caller's observation times (device float64 arrays)."""
+    offs = np.ascontiguousarray(trace_offsets, dtype=np.int64)
+    kap = np.ascontiguousarray(kappa, dtype=np.float64)
+    if offs.size != kap.size + 1:
+        raise ValueError("trace_offsets must have n_models + 1 entries")
+    _check(load_library().cp_planner_pool_demand(
+        kap.size, offs.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)),
+        kap.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), _ptr(arrival_dev), _ptr(prompt_tokens_dev),
+        _ptr(output_tokens_dev), _ptr(residence_dev), n_obs, _ptr(t_obs_dev), _ptr(k_pool_dev),
+        _ptr(workspace_dev), workspace_bytes, stream), "cp_planner_pool_demand")
+
+
+def planner_quantile(values_dev, n: int, q: float, page_bytes: float, workspace_dev, workspace_bytes: int,
+                     stream: int = 0):
+    """cp_planner_quantile -> (x_(ceil(q n)), pages)."""
+    val, pages = ctypes.c_double(), ctypes.c_uint64()
+    _check(load_library().cp_planner_quantile(_ptr(values_dev), n, q, page_bytes, _ptr(workspace_dev),
+                                              workspace_bytes, ctypes.byref(val), ctypes.byref(pages), stream),
+           "cp_planner_quantile")
+    return float(val.value), int(pages.value)

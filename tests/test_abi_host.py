@@ -255,3 +255,28 @@ def test_vmm_pool_fails_loudly_without_a_device():
         p.vmm_info()
     assert e.value.status == cp.CP_ERR_INVALID_ARG
     p.close()
+
+
+def test_planner_host_validation():
+    """cp_planner_* argument checks happen before any CUDA call."""
+    wsb = cp.planner_workspace_bytes()
+    assert wsb >= 4 * 65536 and wsb % 16 == 0
+    a = FAKE_ARENA
+    for offs, kap in (([0, 5, 3], [1.0, 1.0]),          # offsets decrease
+                      ([1, 5], [1.0]),                  # do not start at 0
+                      ([0, 5], [-1.0]),                 # negative kappa
+                      ([0, 5], [float("nan")])):
+        with pytest.raises(cp.CrossPoolError) as e:
+            cp.planner_pool_demand(offs, kap, a, a, a, a, 4, a, a, a, wsb)
+        assert e.value.status == cp.CP_ERR_INVALID_ARG
+    with pytest.raises(cp.CrossPoolError) as e:
+        cp.planner_pool_demand(list(range(0, 5 * 66, 5)), [1.0] * 65, a, a, a, a, 4, a, a, a, wsb)   # > 64 models
+    assert e.value.status == cp.CP_ERR_INVALID_ARG
+    with pytest.raises(cp.CrossPoolError) as e:
+        cp.planner_pool_demand([0, 5], [1.0], a, a, a, a, 4, a, a, a, wsb - 16)
+    assert e.value.status == cp.CP_ERR_WORKSPACE
+    cp.planner_pool_demand([0, 5], [1.0], a, a, a, a, 0, None, None, a, wsb)        # nothing to do: OK, no CUDA
+    for n, q in ((0, 0.5), (10, 0.0), (10, 1.5)):
+        with pytest.raises(cp.CrossPoolError) as e:
+            cp.planner_quantile(a, n, q, 4096.0, a, wsb)
+        assert e.value.status == cp.CP_ERR_INVALID_ARG
