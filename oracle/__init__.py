@@ -153,6 +153,48 @@ def decode_workload(w, heads_per_request: Optional[Sequence[Optional[Sequence[in
     return res
 
 
+# ---------------------------------------------------------------- layer-wise stages
+def _bf16_round(x: np.ndarray) -> np.ndarray:
+    """float32 -> bf16 bit patterns, round to nearest, ties to even (finite inputs)."""
+    u = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32).astype(np.uint64)
+    return ((u + 0x7FFF + ((u >> 16) & 1)) >> 16).astype(np.uint16)
+
+
+def _bf16_widen(b: np.ndarray) -> np.ndarray:
+    return (np.ascontiguousarray(b, dtype=np.uint16).astype(np.uint32) << np.uint32(16)).view(np.float32)
+
+
+def stage_query(q_in: np.ndarray, o_prev: np.ndarray, alpha: float) -> np.ndarray:
+    """Query of a dependent stage (reading M1): the attention output of the layer
+    before comes back through the (mocked) FFN as a residual, q = bf16(fp32(q_in) + alpha * O_prev),
+    one float32 product and one float32 sum, then round-to-nearest-even."""
+    prod = np.float32(alpha) * np.ascontiguousarray(o_prev, dtype=np.float32)
+    return _bf16_round(_bf16_widen(q_in) + prod)
+
+
+def decode_stages(w, stages: Sequence[Sequence[int]], deps: Sequence[int], q_in, alpha: float):
+    """Attention-only mock of the layer-wise pipeline: stage s is one attention step (one layer of one
+    in-flight batch) over the requests `stages[s]` (indices into w.requests) with queries q_in[s][j]
+    (bf16 bits [Hq, d_k]); if deps[s] >= 0 the query first takes the output of stage deps[s] (same
+    batch shape) through `stage_query`.  Stages are evaluated one after the other in list order.
+    Returns per stage a list of (O, LSE)."""
+    outs = []
+    for s, reqs in enumerate(stages):
+        res = []
+        for j, ri in enumerate(reqs):
+            r = w.requests[ri]
+            m = w.models[r.model_id]
+            q = np.ascontiguousarray(q_in[s][j], dtype=np.uint16)
+            if deps[s] >= 0:
+                assert deps[s] < s and m.head_dim_qk == m.head_dim_v
+                q = stage_query(q, outs[deps[s]][j][0], alpha)
+            res.append(attention(w.arena, w.page_tokens, w.page_bytes, w.num_pages, m.kind, m.n_q_heads,
+                                 m.n_kv_heads, m.head_dim_qk, m.head_dim_v, m.softmax_scale, r.page_ids,
+                                 r.context_len, q))
+        outs.append(res)
+    return outs
+
+
 # ---------------------------------------------------------------- KV-cache planner (PAPER.md Eq. (1)-(2))
 def active_tokens(u: float, o_p: float, o_d: float, t_res: float) -> float:
     """Q_i(u) of Eq. (1)."""

@@ -255,10 +255,9 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
     uint8_t *stage_base = smem;
     float *merge = reinterpret_cast<float *>(smem + (size_t)NS * STAGE_BYTES);
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + (size_t)NS * STAGE_BYTES + KV_MERGE_BYTES);
-    // bars: full[NS], empty[NS], tq_full[TQ], tq_empty[TQ]; then the tile queue, flag
+    // bars: full[NS], empty[NS], tq_full[TQ], tq_empty[TQ]; then the tile queue
     uint64_t *full_b = bars, *empty_b = bars + NS, *tqf_b = bars + 2 * NS, *tqe_b = bars + 2 * NS + KV_TQ;
     TileDesc *tq = reinterpret_cast<TileDesc *>(bars + 2 * NS + 2 * KV_TQ);
-    int *s_flag = reinterpret_cast<int *>(tq + KV_TQ);
 
     const int tid = threadIdx.x;
     const int warp = tid >> 5;

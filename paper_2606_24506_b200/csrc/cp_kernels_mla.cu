@@ -104,7 +104,6 @@ struct MlaMisc {
     uint64_t tq_full[MLA_TQ], tq_empty[MLA_TQ];         // work-item queue
     MlaDesc tq[MLA_TQ];
     uint32_t tmem_base;
-    int32_t flag;
 };
 static_assert(sizeof(MlaMisc) <= 1024, "MlaMisc must fit its reserved kilobyte");
 

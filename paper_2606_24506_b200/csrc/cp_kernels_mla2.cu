@@ -94,7 +94,6 @@ struct M2Misc {
     float xmax[2][128];             // row maxima exchanged between the two token halves of a head (by slice parity)
     float xsum[128];
     uint32_t tmem_base;
-    int32_t flag;
 };
 static_assert(sizeof(M2Misc) <= 2048, "M2Misc must fit its reserved block");
 

@@ -117,6 +117,8 @@ SMALL = [
     ([ModelCfg(KIND_MLA, 128, 1, 576, 512, 192 ** -0.5)], [0, 0], [2000, 129], 64, 0.0),
     ([ModelCfg(KIND_MLA, 16, 1, 576, 512, 192 ** -0.5)], [0], [777], 64, 0.0),
     ([ModelCfg(KIND_MLA, 8, 1, 64, 32, 0.3), ModelCfg(KIND_KV, 4, 2, 64, 64, 0.3)], [0, 1, 0], [100, 200, 7], 8, 0.0),
+    # MHA (Hq = Hkv, group size 1; the paper's Type I models, SURVEY 8(f) N4 names the variant)
+    ([ModelCfg(KIND_KV, 8, 8, 128, 128, 128 ** -0.5), ModelCfg(KIND_KV, 4, 4, 64, 64, 0.125)], [0, 1, 0], [1500, 300, 33], 16, 0.0),
 ]
 
 
