@@ -265,6 +265,40 @@ cp_status cp_decode_attention_host(cp_pool *pool, const int32_t *request_ids_hos
                                    void *stream);
 
 /*
+ * cp_decode_attention_stages -- several attention steps in ONE persistent launch: an
+ * attention-only mock of the layer-wise pipeline, "two in-flight batches, each with its own model
+ * id, layer cursor, and completion state" advanced "without requiring the two batches to have the
+ * same model or the same number of layers", with the control on the GPU:
+ * persistent CTAs that select the next ready work, wait "for computation ... completion, and update
+ * the batch state for the next layer" (L146) instead of one host launch per layer.
+ * A STAGE is one attention step = one layer of one batch, over stage_sizes_host[s] mapped requests
+ * (the KV of that layer; ids may repeat across stages, not inside one).  The caller lists the stages
+ * in the order the scheduler's state machine issues them (e.g. B1 L0, B2 L0, B1 L1, B2 L1, ...).
+ * stage_dep_host[s] = the stage whose output feeds stage s (the same batch one layer earlier), or
+ * -1.  The FFN between two layers lives in the other pool and is out of scope; it is mocked by a
+ * residual pass-through (reading M1): for a dependent stage the query rows are
+ *     q = bf16(fp32(q_in) + alpha * O_dep)        (float32 product, float32 sum, round-to-nearest-even)
+ * with q_in the rows given in q_dev.  A dependent stage must have the batch shape of its
+ * predecessor (same number of requests, same model per slot).  Tiles of a dependent stage stream
+ * their KV pages as soon as a CTA is free and wait only for their queries.
+ *   q_dev / out_dev / lse_dev   packed stage after stage, inside a stage as for cp_decode_attention
+ *   workspace_dev               >= cp_decode_stages_workspace_bytes(...) bytes, 16-B aligned
+ * Supported: MQA / GQA / MHA models with d_k = d_v = 128 on page sizes 16/32/64/128 (the tensor-core
+ * K/V kernel); anything else, or CP_OPT_KERNEL = 1: UNSUPPORTED.  Other errors: INVALID_ARG (bad
+ * sizes, dep >= s, shape mismatch with the predecessor, NaN alpha), UNKNOWN_REQUEST, WORKSPACE, CUDA.
+ */
+cp_status cp_decode_stages_workspace_bytes(cp_pool *pool, int32_t n_stages,
+                                           const int32_t *stage_sizes_host,
+                                           const int32_t *request_ids_host,
+                                           const int32_t *stage_dep_host, uint64_t *bytes_out);
+cp_status cp_decode_attention_stages(cp_pool *pool, int32_t n_stages,
+                                     const int32_t *stage_sizes_host,
+                                     const int32_t *request_ids_host,
+                                     const int32_t *stage_dep_host, float alpha,
+                                     const void *q_dev, float *out_dev, float *lse_dev,
+                                     void *workspace_dev, uint64_t workspace_bytes, void *stream);
+
+/*
  * cp_decode_plan -- introspection of the device work list the next cp_decode_attention on
  * this batch will consume (host only, no CUDA): writes up to cap tiles in the order the
  * persistent CTAs pop them.  n_tiles_out receives the total number of tiles,

@@ -89,6 +89,8 @@ def load_library():
         "cp_decode_attention": (i32, [vp, i32p, i32, vp, vp, vp, vp, u64, vp]),
         "cp_decode_workspace_bytes_host": (i32, [vp, i32p, i32, u64p]),
         "cp_decode_attention_host": (i32, [vp, i32p, i32, vp, vp, vp, vp, u64, vp]),
+        "cp_decode_stages_workspace_bytes": (i32, [vp, i32, i32p, i32p, i32p, u64p]),
+        "cp_decode_attention_stages": (i32, [vp, i32, i32p, i32p, i32p, ctypes.c_float, vp, vp, vp, vp, u64, vp]),
         "cp_decode_plan": (i32, [vp, i32p, i32, ctypes.POINTER(cp_tile_info), i32, i32p, i32p]),
         "cp_pool_counters": (i32, [vp, u64p, u64p, u64p]),
         "cp_status_string": (ctypes.c_char_p, [i32]),
@@ -110,7 +112,7 @@ EXPORTED = ["cp_pool_create", "cp_pool_create_vmm", "cp_pool_vmm_info", "cp_pool
             "cp_pool_request_info", "cp_pool_stats", "cp_pool_set_option", "cp_pool_gather_kv",
             "cp_pool_append_kv",
             "cp_decode_workspace_bytes", "cp_decode_attention", "cp_decode_workspace_bytes_host",
-            "cp_decode_attention_host", "cp_decode_plan", "cp_pool_counters", "cp_status_string",
+            "cp_decode_attention_host", "cp_decode_stages_workspace_bytes", "cp_decode_attention_stages", "cp_decode_plan", "cp_pool_counters", "cp_status_string",
             "cp_planner_workspace_bytes", "cp_planner_pool_demand", "cp_planner_quantile"]
 
 
@@ -235,6 +237,31 @@ class Pool:
         _check(self._L.cp_pool_counters(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)),
                "cp_pool_counters")
         return {"kernel_launches": a.value, "plan_builds": b.value, "metadata_h2d_bytes": c.value}
+
+    # --- several attention steps in one persistent launch (layer-wise stages)
+    @staticmethod
+    def _stage_args(stages, deps):
+        sizes = _ids([len(st) for st in stages])
+        ids = _ids(np.concatenate([np.asarray(st, dtype=np.int32) for st in stages]))
+        deps = _ids(deps)
+        if deps.size != sizes.size:
+            raise ValueError("one dependency entry per stage")
+        return sizes, ids, deps
+
+    def decode_stages_workspace_bytes(self, stages, deps) -> int:
+        sizes, ids, deps = self._stage_args(stages, deps)
+        out = ctypes.c_uint64()
+        _check(self._L.cp_decode_stages_workspace_bytes(self._h, sizes.size, _i32p(sizes), _i32p(ids), _i32p(deps),
+                                                        ctypes.byref(out)), "cp_decode_stages_workspace_bytes")
+        return int(out.value)
+
+    def decode_attention_stages(self, stages, deps, alpha: float, q_dev, out_dev, lse_dev, workspace_dev,
+                                workspace_bytes: int, stream: int = 0):
+        sizes, ids, deps = self._stage_args(stages, deps)
+        _check(self._L.cp_decode_attention_stages(self._h, sizes.size, _i32p(sizes), _i32p(ids), _i32p(deps),
+                                                  float(alpha), _ptr(q_dev), _ptr(out_dev), _ptr(lse_dev),
+                                                  _ptr(workspace_dev), workspace_bytes, stream),
+               "cp_decode_attention_stages")
 
     def decode_plan(self, request_ids):
         ids = _ids(request_ids)

@@ -202,15 +202,19 @@ __device__ __forceinline__ CombineUnit load_combine_unit(const CombineUnit *unit
 // Runs the units first, first + stride, ... of one warp.  U3 = loads in flight per lane in the O
 // pass.  The record of the next unit is fetched while the current one is combined, and a group
 // already seen complete is not polled again (units are sorted by group).
-template <int U3>
-static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, const int stride, float *wsm, const int lane)
+// STAGED (multi-stage launches): the units u < end of one stage; every finished unit is counted in
+// the stage's completion counter (release), which the dependent stage's tiles acquire.
+template <int U3, bool STAGED = false>
+static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, const int stride, float *wsm, const int lane,
+                                                  const int end = 0)
 {
-    if (u >= p.n_combine_units) return;
+    const int n_end = STAGED ? end : p.n_combine_units;
+    if (u >= n_end) return;
     CombineUnit cu = load_combine_unit(p.cunits, u);
     int done_group = -1;
     for (;;) {
         const int un = u + stride;
-        const bool has_next = un < p.n_combine_units;
+        const bool has_next = un < n_end;
         CombineUnit nx;
         if (has_next) nx = load_combine_unit(p.cunits, un);
         KV_STAMP(8, threadIdx.x == 0);
@@ -284,6 +288,10 @@ static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, 
         }
         if (cu.lse_off >= 0 && lane == 0) p.lse[cu.lse_off] = (M + log2f(L)) * 0.6931471805599453f;
         __syncwarp();               // wsm is reused by this warp's next unit
+        if (STAGED) {
+            // the unit's O / LSE stores happen-before this release (cumulative over the __syncwarp)
+            if (lane == 0) red_release_add(p.stage_done + (size_t)cu.pad[0] * kCounterStride, 1);
+        }
         KV_STAMP(11, threadIdx.x == 0);
         if (!has_next) break;
         cu = nx;

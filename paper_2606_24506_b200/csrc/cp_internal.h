@@ -101,6 +101,20 @@ struct CombineUnit {
 };
 static_assert(sizeof(CombineUnit) == 64, "CombineUnit is loaded as four 16-byte vectors");
 
+// One stage of a multi-stage launch (cp_decode_attention_stages): one attention step
+// = one layer of one in-flight batch.  A stage with dep >= 0 builds its queries from the output of
+// stage dep (same batch shape): q = bf16(q_in + alpha * O_dep), and may only do so once dep_target
+// completion signals of stage dep have been counted (its combine units and single-split tiles).
+struct StageRec {
+    int32_t dep;            // stage this one depends on, or -1
+    int32_t dep_target;     // value of stage_done[dep] that means "stage dep is complete"
+    int32_t cu_begin, cu_end;   // this stage's combine units
+    int64_t dep_out_delta;  // out offset of stage dep minus out offset of this stage (floats)
+    float alpha;
+    int32_t pad;
+};
+static_assert(sizeof(StageRec) == 32, "StageRec is loaded as two 16-byte vectors");
+
 // Kernel arguments common to all decode kernels (passed by value).
 struct DecodeParams {
     const uint8_t *arena;
@@ -127,7 +141,11 @@ struct DecodeParams {
     float *workspace;              // split partials
     int32_t *work_counter;         // [0] next work item (tile); [1..3] spare
     int32_t *group_counters;       // [n_groups * kCounterStride] tile arrivals, counter g at g * kCounterStride
-    int32_t *reset_counters;       // the other counter set ([32] scheduler + group counters): cleared by this launch
+    int32_t *reset_counters;
+    // multi-stage launches only (else nullptr / 0)
+    const StageRec *stages;
+    int32_t *stage_done;           // [n_stages] completion counters, kCounterStride apart
+    int32_t n_stages;       // the other counter set ([32] scheduler + group counters): cleared by this launch
 };
 
 }  // namespace cp

@@ -91,6 +91,8 @@ struct TileDesc {
     int32_t mt;              // 16-head M tiles (power of two)
     float scale_log2;
     int64_t q_off, out_off, lse_off, part_off;
+    int32_t stage;           // multi-stage launches: the stage of this tile
+    int32_t pad;
 };
 
 // ----------------------------------------------------------------------------- PTX helpers (see also cp_ptx.cuh)
@@ -240,7 +242,23 @@ __device__ __forceinline__ void kv_slice_unit(const uint32_t sb, const int tok0,
     }
 }
 
-template <int P>
+// Two query entries of a dependent stage: q = bf16(fp32(q_in) + alpha * O_prev), one rounded product
+// and one rounded sum in float32, then round-to-nearest-even (reading M1).
+__device__ __forceinline__ uint32_t stage_query2(uint32_t q_in, float2 o, float alpha)
+{
+    const float lo = __fadd_rn(__uint_as_float(q_in << 16), __fmul_rn(alpha, o.x));
+    const float hi = __fadd_rn(__uint_as_float(q_in & 0xFFFF0000u), __fmul_rn(alpha, o.y));
+    const uint32_t a = __float_as_uint(lo), b = __float_as_uint(hi);
+    const uint32_t ra = (a + 0x7FFFu + ((a >> 16) & 1u)) >> 16;
+    const uint32_t rb = (b + 0x7FFFu + ((b >> 16) & 1u)) >> 16;
+    return ra | (rb << 16);
+}
+
+// MULTI: the work list is the concatenation of several stages (cp_decode_attention_stages): a CTA
+// runs its combine units of every earlier stage before it starts a tile of a later one, and a tile
+// of a dependent stage waits for its predecessor's completion counter before it builds its queries
+// from that stage's output.  Waits only ever target earlier entries of the list, so they terminate.
+template <int P, bool MULTI>
 __global__ void __launch_bounds__(KV_THREADS, 1)
 cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap, int rows_per_page)
 {
@@ -306,7 +324,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             } else {
                 r.group = 0; r.req = 0; r.kv_head = 0; r.n_kv_heads = 1; r.page_begin = 0; r.n_pages = 0;
                 r.split = 0; r.n_splits = 1; r.gsize = 1; r.n_q_heads = 1; r.scale_log2 = 0.f;
-                r.q_off = r.out_off = r.lse_off = r.part_off = 0;
+                r.q_off = r.out_off = r.lse_off = r.part_off = 0; r.pad = 0;
             }
             // push the descriptor to the tile queue
             const uint32_t qs = qi % KV_TQ;
@@ -317,6 +335,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 d.npg = r.n_pages; d.split = r.split; d.n_splits = r.n_splits;
                 d.ctx = ctx; d.gsize = r.gsize; d.mt = mt; d.scale_log2 = r.scale_log2;
                 d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
+                d.stage = r.pad; d.pad = 0;
                 tq[qs] = d;
                 mbar_arrive(smem_u32(tqf_b + qs));     // release: consumers acquire via try_wait
             }
@@ -357,6 +376,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
         // =========================================================== consumer warps
         uint32_t pc = 0;          // pages consumed by this CTA so far (ring position of tile start)
         uint32_t qi = 0;
+        int cur_stage = 0;        // MULTI: stages whose combine units this CTA has run
         const int r0 = lane >> 2;             // fragment row (query head in the M tile), and r0 + 8
         const int cq = (lane & 3) * 2;        // fragment column pair
         // per-lane constants of the SWIZZLE_128B addressing (16-B chunk index ^ (row & 7), row & 7 = lane & 7)
@@ -371,6 +391,20 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(tqe_b + qs));
             ++qi;
+            if constexpr (MULTI) {
+                // combine units of every stage before this tile's (all of them once the list is exhausted)
+                const int upto = d.item < 0 ? p.n_stages : d.stage;
+                if (upto > cur_stage) {
+                    consumer_bar();                 // the merge slots of the previous tile are free
+                    for (int s = cur_stage; s < upto; ++s) {
+                        const int2 cur = __ldg(reinterpret_cast<const int2 *>(&p.stages[s].cu_begin));
+                        combine_units<8, true>(p, cur.x + blockIdx.x * KV_CWARPS + warp, gridDim.x * KV_CWARPS,
+                                               merge + warp * KV_COMBINE_WARP_FLOATS, lane, cur.y);
+                    }
+                    consumer_bar();                 // combine scratch is free before the next merge
+                    cur_stage = upto;
+                }
+            }
             if (d.item < 0) break;
             KV_STAMP(1, tid == 0 && qi == 1);
             const int mt = d.mt;
@@ -395,6 +429,32 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                     qf[ks][1] = h1 < gsize ? __ldg(reinterpret_cast<const uint32_t *>(q1 + k)) : 0u;
                     qf[ks][2] = h0 < gsize ? __ldg(reinterpret_cast<const uint32_t *>(q0 + k + 8)) : 0u;
                     qf[ks][3] = h1 < gsize ? __ldg(reinterpret_cast<const uint32_t *>(q1 + k + 8)) : 0u;
+                }
+                if constexpr (MULTI) {
+                    const int4 s0 = __ldg(reinterpret_cast<const int4 *>(p.stages + d.stage));
+                    if (s0.x >= 0) {
+                        // the predecessor's output is complete: all its combine units and single-split
+                        // tiles have signalled (acquire; the other lanes follow through the __syncwarp)
+                        if (lane == 0) wait_group(p.stage_done, s0.x, s0.y);
+                        __syncwarp();
+                        const int4 s1 = __ldg(reinterpret_cast<const int4 *>(p.stages + d.stage) + 1);
+                        const int64_t delta = (int64_t)(uint32_t)s1.x | ((int64_t)s1.y << 32);
+                        const float alpha = __int_as_float(s1.z);
+                        const float *o0 = p.out + d.out_off + delta + (int64_t)h0 * KV_D;
+                        const float *o1 = p.out + d.out_off + delta + (int64_t)h1 * KV_D;
+#pragma unroll
+                        for (int ks = 0; ks < 8; ++ks) {
+                            const int k = ks * 16 + cq;
+                            if (h0 < gsize) {
+                                qf[ks][0] = stage_query2(qf[ks][0], __ldcg(reinterpret_cast<const float2 *>(o0 + k)), alpha);
+                                qf[ks][2] = stage_query2(qf[ks][2], __ldcg(reinterpret_cast<const float2 *>(o0 + k + 8)), alpha);
+                            }
+                            if (h1 < gsize) {
+                                qf[ks][1] = stage_query2(qf[ks][1], __ldcg(reinterpret_cast<const float2 *>(o1 + k)), alpha);
+                                qf[ks][3] = stage_query2(qf[ks][3], __ldcg(reinterpret_cast<const float2 *>(o1 + k + 8)), alpha);
+                            }
+                        }
+                    }
                 }
             }
             float o[16][4];
@@ -503,6 +563,10 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                         if (h0 < gsize) p.lse[d.lse_off + h0] = (m_run[0] + log2f(l_run[0])) * 0.6931471805599453f;
                         if (h1 < gsize) p.lse[d.lse_off + h1] = (m_run[1] + log2f(l_run[1])) * 0.6931471805599453f;
                     }
+                    if constexpr (MULTI) {          // a single-split group is complete with this tile
+                        __syncwarp();
+                        if (lane == 0) red_release_add(p.stage_done + (size_t)d.stage * kCounterStride, 1);
+                    }
                 } else {
                     float *ws = p.workspace + d.part_off;
                     float *d0 = ws + part_o_off(h0, d.split, d.n_splits, KV_D) + cq;
@@ -530,7 +594,8 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
         // the spin inside terminates.
         // Units are assigned statically (unit u -> consumer warp u mod #warps of the grid): popping
         // them from one counter would serialise thousands of same-address atomics at the L2.
-        combine_units<8>(p, blockIdx.x * KV_CWARPS + warp, gridDim.x * KV_CWARPS, merge + warp * KV_COMBINE_WARP_FLOATS, lane);
+        if constexpr (!MULTI)
+            combine_units<8>(p, blockIdx.x * KV_CWARPS + warp, gridDim.x * KV_CWARPS, merge + warp * KV_COMBINE_WARP_FLOATS, lane);
 #endif
         KV_STAMP(6, tid == 0);
     }
@@ -582,19 +647,27 @@ extern "C" int cp_kv_probe_read(unsigned long long *out_host)
 
 bool kv_fast_supported(int P) { return P == 16 || P == 32 || P == 64 || P == 128; }
 
-template <int P>
-static cudaError_t launch_kv_t(const DecodeParams &p, const CUtensorMap &tmap, int rows_per_page, int grid,
-                               cudaStream_t stream)
+template <int P, bool MULTI>
+static cudaError_t launch_kv_tm(const DecodeParams &p, const CUtensorMap &tmap, int rows_per_page, int grid,
+                                cudaStream_t stream)
 {
     const int smem = kv_smem_bytes(P);
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(cp_decode_kv_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(cp_decode_kv_kernel<P, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    cp_decode_kv_kernel<P><<<grid, KV_THREADS, smem, stream>>>(p, tmap, rows_per_page);
+    cp_decode_kv_kernel<P, MULTI><<<grid, KV_THREADS, smem, stream>>>(p, tmap, rows_per_page);
     return cudaGetLastError();
+}
+
+template <int P>
+static cudaError_t launch_kv_t(const DecodeParams &p, const CUtensorMap &tmap, int rows_per_page, int grid,
+                               cudaStream_t stream)
+{
+    return p.n_stages > 0 ? launch_kv_tm<P, true>(p, tmap, rows_per_page, grid, stream)
+                          : launch_kv_tm<P, false>(p, tmap, rows_per_page, grid, stream);
 }
 
 cudaError_t launch_decode_kv(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas,

@@ -64,6 +64,7 @@ struct KindPlan {
     bool all_fast = false;           // every group of this kind runs on the tensor-core kernel
     bool uploaded = false;
     int counter_set = 0;             // scheduler counter set the next launch uses (alternates)
+    int extra_counters = 0;          // multi-stage plans: one completion counter per stage after the groups'
     DevBuf d_groups, d_tiles, d_tile_recs, d_combines, d_cunits, d_counters;   // counters: [32] scheduler + [n_groups * kCounterStride]
 };
 
@@ -112,6 +113,18 @@ struct cp_pool {
     bool mla_tmap_ok = false;
     alignas(64) unsigned char mla2_tmap9[128], mla2_tmap2[128];   // CTA-pair MLA kernel
     bool mla2_tmap_ok = false;
+
+    // multi-stage plan (cp_decode_attention_stages)
+    struct StagesPlan {
+        std::vector<int32_t> key;        // n_stages, sizes, ids, deps
+        uint64_t version = 0;
+        bool valid = false, uploaded = false;
+        KindPlan kp;
+        std::vector<StageRec> stages;
+        DevBuf d_stages;
+        uint64_t ws_floats = 0;
+        int64_t q_elems = 0, out_floats = 0, lse_floats = 0;
+    } splan;
 
     // counters
     uint64_t n_launches = 0, n_plan_builds = 0, n_h2d_bytes = 0;
@@ -412,7 +425,7 @@ cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
 {
     if (kp.uploaded) return CP_OK;
     const size_t gb = kp.groups.size() * sizeof(Group), tb = kp.tiles.size() * sizeof(Tile);
-    const size_t cb = kp.combines.size() * sizeof(Combine), set_ints = 32 + kp.groups.size() * (size_t)kCounterStride, nb = 2 * set_ints * 4;
+    const size_t cb = kp.combines.size() * sizeof(Combine), set_ints = 32 + (kp.groups.size() + kp.extra_counters) * (size_t)kCounterStride, nb = 2 * set_ints * 4;
     const size_t ub = kp.cunits.size() * sizeof(CombineUnit);
     const size_t rb = kp.tile_recs.size() * sizeof(TileRec);
     if (kp.d_groups.ensure(gb) != cudaSuccess || kp.d_tiles.ensure(tb) != cudaSuccess ||
@@ -554,6 +567,11 @@ cp_status cp_pool_free(cp_pool *pool)
         pool->plan[k].d_combines.release(); pool->plan[k].d_cunits.release(); pool->plan[k].d_tile_recs.release();
         pool->plan[k].d_counters.release();
     }
+    {
+        KindPlan &kp = pool->splan.kp;
+        kp.d_groups.release(); kp.d_tiles.release(); kp.d_combines.release(); kp.d_cunits.release();
+        kp.d_tile_recs.release(); kp.d_counters.release(); pool->splan.d_stages.release();
+    }
     delete pool;
     return CP_OK;
 }
@@ -693,6 +711,7 @@ cp_status cp_pool_set_option(cp_pool *pool, int32_t key, int64_t value)
     default: return CP_ERR_INVALID_ARG;
     }
     pool->plan_valid = false;
+    pool->splan.valid = false;
     return CP_OK;
 }
 
@@ -890,6 +909,7 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.work_counter = (int32_t *)kp.d_counters.ptr + kp.counter_set * set_ints;
         prm.group_counters = prm.work_counter + 32;
         prm.reset_counters = (int32_t *)kp.d_counters.ptr + (1 - kp.counter_set) * set_ints;
+        prm.stages = nullptr; prm.stage_done = nullptr; prm.n_stages = 0;
         kp.counter_set ^= 1;
         const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
         cudaError_t e;
@@ -912,6 +932,193 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         pool->n_launches++;
         if (e != cudaSuccess) return CP_ERR_CUDA;
     }
+    return CP_OK;
+}
+
+// ------------------------------------------------------------------ multi-stage launch
+namespace {
+
+cp_status build_stages_plan(cp_pool *pool, int32_t n_stages, const int32_t *sizes, const int32_t *ids,
+                            const int32_t *deps, float alpha)
+{
+    if (!pool || n_stages < 1 || n_stages > 4096 || !sizes || !ids || !deps) return CP_ERR_INVALID_ARG;
+    std::vector<int32_t> key;
+    key.push_back(n_stages);
+    int64_t total = 0;
+    for (int s = 0; s < n_stages; ++s) {
+        if (sizes[s] < 1) return CP_ERR_INVALID_ARG;
+        total += sizes[s];
+    }
+    key.insert(key.end(), sizes, sizes + n_stages);
+    key.insert(key.end(), ids, ids + total);
+    key.insert(key.end(), deps, deps + n_stages);
+    cp_pool::StagesPlan &sp = pool->splan;
+    if (sp.valid && sp.version == pool->topo_version && sp.key == key) {
+        if (alpha == alpha && alpha != sp.stages[0].alpha) {       // same work list, new residual weight
+            for (StageRec &sr : sp.stages) sr.alpha = alpha;
+            sp.uploaded = false;
+        }
+        return CP_OK;
+    }
+
+    if (pool->opt_kernel == 1 || !kv_fast_supported((int)pool->P)) return CP_ERR_UNSUPPORTED;
+    const int32_t *p_ids = ids;
+    for (int s = 0; s < n_stages; ++s) {
+        const cp_status st = check_batch(pool, p_ids, sizes[s]);
+        if (st != CP_OK) return st;
+        if (deps[s] >= s) return CP_ERR_INVALID_ARG;
+        if (deps[s] >= 0) {
+            // the dependent stage reads its predecessor's output row by row: same batch shape
+            if (sizes[deps[s]] != sizes[s]) return CP_ERR_INVALID_ARG;
+            const int32_t *d_ids = ids;
+            for (int t = 0; t < deps[s]; ++t) d_ids += sizes[t];
+            for (int b = 0; b < sizes[s]; ++b)
+                if (pool->reqs[p_ids[b]].model != pool->reqs[d_ids[b]].model) return CP_ERR_INVALID_ARG;
+        }
+        for (int b = 0; b < sizes[s]; ++b) {
+            const cp_model_cfg &m = pool->models[pool->reqs[p_ids[b]].model];
+            if (m.kind != CP_KIND_KV || m.head_dim_qk != 128 || m.head_dim_v != 128 || m.n_q_heads / m.n_kv_heads > 128)
+                return CP_ERR_UNSUPPORTED;
+        }
+        p_ids += sizes[s];
+    }
+
+    KindPlan &kp = sp.kp;
+    kp.groups.clear(); kp.tiles.clear(); kp.tile_recs.clear(); kp.combines.clear(); kp.cunits.clear();
+    kp.uploaded = false; kp.all_fast = true; kp.extra_counters = n_stages;
+    sp.stages.assign(n_stages, StageRec());
+    sp.uploaded = false;
+    std::vector<int64_t> out_base(n_stages);
+    std::vector<int32_t> target(n_stages);
+    int64_t qb = 0, ob = 0, lb = 0, wb = 0;
+    p_ids = ids;
+    for (int s = 0; s < n_stages; ++s) {
+        build_plan(pool, p_ids, sizes[s]);
+        const KindPlan &src = pool->plan[CP_KIND_KV];
+        const int gb = (int)kp.groups.size();
+        const int cb = (int)kp.cunits.size();
+        for (Group g : src.groups) {
+            g.q_off += qb; g.out_off += ob; g.lse_off += lb;
+            if (g.n_splits > 1) g.part_off += wb;
+            kp.groups.push_back(g);
+        }
+        int32_t direct = 0;
+        for (size_t i = 0; i < src.tiles.size(); ++i) {
+            Tile t = src.tiles[i];
+            t.group += gb;
+            kp.tiles.push_back(t);
+            TileRec r = src.tile_recs[i];
+            r.group += gb; r.q_off += qb; r.out_off += ob; r.lse_off += lb;
+            if (r.n_splits > 1) r.part_off += wb;
+            r.pad = s;
+            kp.tile_recs.push_back(r);
+            if (r.n_splits == 1) {              // its plane-0 warps (one per padded M tile) each signal once
+                int mt = (r.gsize + 15) / 16, mtp = 1;
+                while (mtp < mt) mtp <<= 1;
+                direct += mtp;
+            }
+        }
+        for (CombineUnit cu : src.cunits) {
+            cu.part_off += wb; cu.ml_off += wb; cu.out_off += ob;
+            if (cu.lse_off >= 0) cu.lse_off += lb;
+            cu.group += gb;
+            cu.pad[0] = s;
+            kp.cunits.push_back(cu);
+        }
+        StageRec &sr = sp.stages[s];
+        sr.dep = deps[s]; sr.dep_target = 0; sr.cu_begin = cb; sr.cu_end = (int)kp.cunits.size();
+        sr.dep_out_delta = 0; sr.alpha = alpha == alpha ? alpha : 0.f; sr.pad = 0;
+        target[s] = (sr.cu_end - sr.cu_begin) + direct;
+        out_base[s] = ob;
+        qb += pool->q_elems; ob += pool->out_floats; lb += pool->lse_floats; wb += (int64_t)pool->plan_ws_floats;
+        p_ids += sizes[s];
+    }
+    for (int s = 0; s < n_stages; ++s)
+        if (deps[s] >= 0) {
+            sp.stages[s].dep_target = target[deps[s]];
+            sp.stages[s].dep_out_delta = out_base[deps[s]] - out_base[s];
+        }
+    pool->plan_valid = false;                  // build_plan overwrote the single-step plan cache
+    sp.q_elems = qb; sp.out_floats = ob; sp.lse_floats = lb; sp.ws_floats = (uint64_t)wb;
+    sp.key.swap(key);
+    sp.version = pool->topo_version;
+    sp.valid = true;
+    return CP_OK;
+}
+
+}  // namespace
+
+cp_status cp_decode_stages_workspace_bytes(cp_pool *pool, int32_t n_stages, const int32_t *stage_sizes_host,
+                                           const int32_t *request_ids_host, const int32_t *stage_dep_host,
+                                           uint64_t *bytes_out)
+{
+    if (!bytes_out) return CP_ERR_INVALID_ARG;
+    const cp_status st = build_stages_plan(pool, n_stages, stage_sizes_host, request_ids_host, stage_dep_host,
+                                           std::nanf(""));          // NaN: leave the residual weight alone
+    if (st != CP_OK) return st;
+    *bytes_out = pool->splan.ws_floats * 4;
+    return CP_OK;
+}
+
+cp_status cp_decode_attention_stages(cp_pool *pool, int32_t n_stages, const int32_t *stage_sizes_host,
+                                     const int32_t *request_ids_host, const int32_t *stage_dep_host, float alpha,
+                                     const void *q_dev, float *out_dev, float *lse_dev, void *workspace_dev,
+                                     uint64_t workspace_bytes, void *stream)
+{
+    if (!pool || !q_dev || !out_dev || !lse_dev || !(alpha == alpha)) return CP_ERR_INVALID_ARG;
+    if (((uintptr_t)q_dev & 15u) || ((uintptr_t)out_dev & 15u) || ((uintptr_t)lse_dev & 3u)) return CP_ERR_INVALID_ARG;
+    cp_status st = build_stages_plan(pool, n_stages, stage_sizes_host, request_ids_host, stage_dep_host, alpha);
+    if (st != CP_OK) return st;
+    cp_pool::StagesPlan &sp = pool->splan;
+    if (sp.ws_floats * 4 > workspace_bytes) return CP_ERR_WORKSPACE;
+    if (sp.ws_floats && (!workspace_dev || ((uintptr_t)workspace_dev & 15u))) return CP_ERR_WORKSPACE;
+    st = ensure_device(pool);
+    if (st != CP_OK) return st;
+    if (!pool->kv_tmap_ok) return CP_ERR_UNSUPPORTED;
+    cudaStream_t s = (cudaStream_t)stream;
+    st = flush_tables(pool, s);
+    if (st != CP_OK) return st;
+    KindPlan &kp = sp.kp;
+    st = upload_plan(pool, kp, s);
+    if (st != CP_OK) return st;
+    if (!sp.uploaded) {
+        const size_t sb = sp.stages.size() * sizeof(StageRec);
+        if (sp.d_stages.ensure(sb) != cudaSuccess ||
+            cudaMemcpyAsync(sp.d_stages.ptr, sp.stages.data(), sb, cudaMemcpyHostToDevice, s) != cudaSuccess) {
+            cudaGetLastError();
+            return CP_ERR_CUDA;
+        }
+        pool->n_h2d_bytes += sb;
+        sp.uploaded = true;
+    }
+    DecodeParams prm;
+    prm.arena = pool->arena; prm.page_tokens = pool->P; prm.page_bytes = pool->page_bytes;
+    prm.page_table = (const int32_t *)pool->d_page_table.ptr; prm.max_ppr = pool->max_ppr;
+    prm.slot_pages = (pool->vmm && !pool->opt_vmm_table) ? (int32_t)pool->slot_pages : 0;
+    prm.req_ctx = (const int32_t *)pool->d_ctx.ptr;
+    prm.models = (const DevModel *)pool->d_models.ptr;
+    prm.groups = (const Group *)kp.d_groups.ptr;
+    prm.tiles = (const Tile *)kp.d_tiles.ptr;
+    prm.tile_recs = (const TileRec *)kp.d_tile_recs.ptr;
+    prm.combines = (const Combine *)kp.d_combines.ptr;
+    prm.cunits = (const CombineUnit *)kp.d_cunits.ptr;
+    prm.n_tiles = (int)kp.tiles.size(); prm.n_combines = 0;
+    prm.n_combine_units = (int)kp.cunits.size();
+    prm.n_groups = (int)kp.groups.size() + n_stages;           // counters the next launch's reset covers
+    prm.q = (const uint16_t *)q_dev; prm.out = out_dev; prm.lse = lse_dev;
+    prm.workspace = (float *)workspace_dev;
+    const size_t set_ints = 32 + (kp.groups.size() + (size_t)n_stages) * (size_t)kCounterStride;
+    prm.work_counter = (int32_t *)kp.d_counters.ptr + kp.counter_set * set_ints;
+    prm.group_counters = prm.work_counter + 32;
+    prm.reset_counters = (int32_t *)kp.d_counters.ptr + (1 - kp.counter_set) * set_ints;
+    prm.stages = (const StageRec *)sp.d_stages.ptr;
+    prm.stage_done = prm.group_counters + kp.groups.size() * (size_t)kCounterStride;
+    prm.n_stages = n_stages;
+    kp.counter_set ^= 1;
+    const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
+    const cudaError_t e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256), std::min(n_ctas, pool->n_sm), s);
+    pool->n_launches++;
+    if (e != cudaSuccess) return CP_ERR_CUDA;
     return CP_OK;
 }
 
