@@ -198,6 +198,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (tuning sweeps only)")
     ap.add_argument("--no-vmm", action="store_true", help="skip the CUDA-VMM arena leg (SURVEY 8(f) N2)")
     ap.add_argument("--no-planner", action="store_true", help="skip the KV-cache planner leg (SURVEY 8(f) N3)")
+    ap.add_argument("--no-stages", action="store_true", help="skip the multi-stage launch leg (SURVEY 8(f) N4)")
+    ap.add_argument("--stage-layers", type=int, default=4, help="layers per batch in the multi-stage leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -381,6 +383,125 @@ def main():
                     "request; cold = cuMemCreate + cuMemMap + cuMemSetAccess per chunk, parked = cuMemMap + "
                     "cuMemSetAccess; the software table's device upload is deferred to the next compute call"}
 
+    # ---------------- multi-stage persistent launch: L layers in ONE launch against L
+    # launches.  Every layer has its own copy of the workload's KV (distinct memory, L x the arena), so
+    # nothing is re-read from L2.  (a) one batch of all requests, L dependent layers; (b) one batch per
+    # model, two in flight, served in turn (the paper's layer-wise state machine), L layers each.
+    stages_leg = None
+    if rank == 0 and not args.no_stages and all(m.kind == 0 and m.head_dim_qk == 128 and m.head_dim_v == 128 for m in w.models):
+        L = args.stage_layers
+        nreq = len(w.requests)
+        arena_l = dw.arena.repeat(L)
+        max_ppr = max(r.page_ids.size for r in w.requests)
+        pool_l = cp.Pool(arena_l, arena_l.numel() * 2, w.page_tokens, w.page_bytes, w.num_pages * L, w.models,
+                         max_requests=nreq * L, max_pages_per_request=max_ppr)
+        for l in range(L):
+            for r in w.requests:
+                pool_l.map_pages(l * nreq + r.request_id, r.model_id, r.page_ids + l * w.num_pages, r.context_len)
+        sep_pools = {}
+
+        def sep_pool(batch_key, l, ids):
+            """Pool of one (batch, layer) for the separate launches: its plan stays cached."""
+            if (batch_key, l) not in sep_pools:
+                pl = cp.Pool(arena_l, arena_l.numel() * 2, w.page_tokens, w.page_bytes, w.num_pages * L, w.models,
+                             max_requests=nreq, max_pages_per_request=max_ppr)
+                for i in ids:
+                    r = w.requests[i]
+                    pl.map_pages(r.request_id, r.model_id, r.page_ids + l * w.num_pages, r.context_len)
+                sep_pools[(batch_key, l)] = pl
+            return sep_pools[(batch_key, l)]
+
+        req_ids = [r.request_id for r in w.requests]
+        by_model = [[r.request_id for r in w.requests if r.model_id == mi] for mi in range(len(w.models))]
+        by_model = [b for b in by_model if b]
+
+        def pipeline(layers, slots=2):
+            queue = list(range(len(layers)))
+            live = [queue.pop(0) for _ in range(min(slots, len(queue)))]
+            cur = {b: 0 for b in live}
+            order = []
+            while any(b is not None for b in live):
+                for i, b in enumerate(live):
+                    if b is None:
+                        continue
+                    order.append((b, cur[b]))
+                    cur[b] += 1
+                    if cur[b] == layers[b]:
+                        live[i] = queue.pop(0) if queue else None
+                        if live[i] is not None:
+                            cur[live[i]] = 0
+            return order
+
+        def rows_of(ids):
+            return sum(w.models[w.requests[i].model_id].n_q_heads for i in ids)     # request_id == index
+
+        def run_case(batches):
+            order = pipeline([L] * len(batches))
+            pos = {bl: s for s, bl in enumerate(order)}
+            stages = [[l * nreq + i for i in batches[b]] for b, l in order]
+            deps = [pos[(b, l - 1)] if l > 0 else -1 for b, l in order]
+            rows = sum(rows_of(batches[b]) for b, _ in order)
+            qs = torch.randn(rows * 128, device=dev).to(torch.bfloat16).view(torch.int16)
+            outs = torch.empty(rows * 128, dtype=torch.float32, device=dev)
+            lses = torch.empty(rows, dtype=torch.float32, device=dev)
+            wsb = max(pool_l.decode_stages_workspace_bytes(stages, deps), 256)
+            wss = torch.empty(wsb, dtype=torch.uint8, device=dev)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            one, sep = [], []
+            for i in range(3 + 15):
+                spacer(i)
+                e0.record()
+                pool_l.decode_attention_stages(stages, deps, 1.0, qs, outs, lses, wss, wsb, dw.stream())
+                e1.record()
+                torch.cuda.synchronize()
+                one.append(e0.elapsed_time(e1))
+            # the same stages as separate launches (plain steps, no dependency between them)
+            offs, ro = [], 0
+            for b, l in order:
+                offs.append(ro)
+                ro += rows_of(batches[b])
+            pools = [sep_pool((len(batches), b), l, batches[b]) for b, l in order]
+            wsb1 = max(max(pl.decode_workspace_bytes(batches[b]) for pl, (b, l) in zip(pools, order)), 256)
+            ws1 = torch.empty(wsb1, dtype=torch.uint8, device=dev)
+            for i in range(3 + 15):
+                spacer(i)
+                e0.record()
+                for s, (b, l) in enumerate(order):
+                    pools[s].decode_attention(batches[b], qs[offs[s] * 128:], outs[offs[s] * 128:], lses[offs[s]:],
+                                              ws1, wsb1, dw.stream())
+                e1.record()
+                torch.cuda.synchronize()
+                sep.append(e0.elapsed_time(e1))
+            # host-driven: the host sees every stage complete before it launches the next (PAPER.md Fig. 5a)
+            host = []
+            for i in range(2 + 8):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                for s, (b, l) in enumerate(order):
+                    pools[s].decode_attention(batches[b], qs[offs[s] * 128:], outs[offs[s] * 128:], lses[offs[s]:],
+                                              ws1, wsb1, dw.stream())
+                    torch.cuda.synchronize()
+                host.append(1e3 * (time.perf_counter() - t0))
+            t3 = float(np.median(host[2:]))
+            kv_bytes = sum(w.requests[i].context_len * w.models[w.requests[i].model_id].n_kv_heads * 512
+                           for b, _ in order for i in batches[b])
+            t1, t2 = float(np.median(one[3:])), float(np.median(sep[3:]))
+            return {"stages": len(order), "kv_bytes": int(kv_bytes), "one_launch_us": 1e3 * t1,
+                    "separate_launches_us": 1e3 * t2, "one_launch_us_per_stage": 1e3 * t1 / len(order),
+                    "separate_us_per_stage": 1e3 * t2 / len(order),
+                    "host_driven_us_per_stage_wall": 1e3 * t3 / len(order), "one_launch_gbs": kv_bytes / (t1 * 1e-3) / 1e9,
+                    "separate_gbs": kv_bytes / (t2 * 1e-3) / 1e9}
+
+        stages_leg = {"layers": L,
+                      "one_batch_of_all_requests": run_case([req_ids]),
+                      "one_batch_per_model_two_in_flight": run_case(by_model),
+                      "note": "separate launches: the same stages as back-to-back cp_decode_attention calls, each on a "
+                              "pool of its own so that its plan stays cached (no dependency between them)"}
+        pool_l.close()
+        for pl in sep_pools.values():
+            pl.close()
+        del arena_l
+
     # ---------------- KV-cache planner (SURVEY §8(f) N3; PAPER.md Eq. (1)-(2)): pool demand at 100 000 observation
     # times of a two-hour synthetic trace of 8 cold models, then P95 / P99 and the page budgets
     planner = None
@@ -463,7 +584,7 @@ def main():
                     "us_per_step": 1e3 * e2e_ms,
                     "h2d_bytes_per_step": int(q_host.numel() * 2),
                     "d2h_bytes_per_step": int(o_host.numel() * 4 + l_host.numel() * 4)},
-            "gpu_launches": int(launches), "roofline": roof, "gather": gather, "append": append, "vmm_arena": vmm, "planner": planner,
+            "gpu_launches": int(launches), "roofline": roof, "gather": gather, "append": append, "vmm_arena": vmm, "planner": planner, "stages": stages_leg,
             "pct_of_hbm_peak": {"measured_copy": 100 * achieved / peaks["hbm_gbs"], "nominal_8TBs": 100 * achieved / 8000.0}}
 
     if not args.no_cpu_baseline:
