@@ -153,6 +153,26 @@ def decode_workload(w, heads_per_request: Optional[Sequence[Optional[Sequence[in
     return res
 
 
+# ---------------------------------------------------------------- several query tokens per request (q_len > 1)
+def attention_qlen(arena, page_tokens: int, page_bytes: int, num_pages: int, kind: int, n_q_heads: int,
+                   n_kv_heads: int, d_k: int, d_v: int, softmax_scale: float, page_ids, context_len: int,
+                   q: np.ndarray):
+    """Causal attention of the LAST q_len tokens of a request (reading Q1): q is bf16 bits
+    [q_len, Hq, d_k]; query token j sits at position context_len - q_len + j (its own K/V is already in
+    the pool and counted by context_len) and attends to positions 0 .. context_len - q_len + j.  That
+    is, by definition, the single-token attention over the prefix that ends with token j.
+    -> (O float64 [q_len, Hq, d_v], LSE float64 [q_len, Hq])."""
+    q = np.ascontiguousarray(q, dtype=np.uint16)
+    q_len = q.shape[0]
+    assert 1 <= q_len <= context_len
+    out = np.empty((q_len, n_q_heads, d_v), dtype=np.float64)
+    lse = np.empty((q_len, n_q_heads), dtype=np.float64)
+    for j in range(q_len):
+        out[j], lse[j] = attention(arena, page_tokens, page_bytes, num_pages, kind, n_q_heads, n_kv_heads, d_k,
+                                   d_v, softmax_scale, page_ids, context_len - q_len + 1 + j, q[j])
+    return out, lse
+
+
 # ---------------------------------------------------------------- layer-wise stages (PAPER.md L126-L128, L144-L146)
 def _bf16_round(x: np.ndarray) -> np.ndarray:
     """float32 -> bf16 bit patterns, round to nearest, ties to even (finite inputs)."""
