@@ -265,6 +265,23 @@ cp_status cp_decode_attention_host(cp_pool *pool, const int32_t *request_ids_hos
                                    void *stream);
 
 /*
+ * cp_decode_attention_qlen -- the same step with q_len > 1 query tokens per request (the variant
+ * SURVEY 8(f) N4 names; e.g. the verification step of speculative decoding).  The query tokens are
+ * the LAST q_len tokens of each request: their K/V is already in the pool and counted by
+ * context_len (reading Q1).  Query token j (0-based) sits at position
+ * context_len - q_len + j and attends causally to positions 0 .. context_len - q_len + j.
+ *   q_dev    bf16, per request [q_len][Hq][d_k];  out_dev fp32 [q_len][Hq][d_v];  lse_dev [q_len][Hq]
+ *   q_len    1 .. 128 with (Hq / Hkv) * q_len <= 128; q_len = 1 is cp_decode_attention
+ * For q_len > 1: MQA / GQA / MHA models with d_k = d_v = 128 on page sizes 16/32/64/128 only
+ * (UNSUPPORTED otherwise, and with CP_OPT_KERNEL = 1); INVALID_ARG if a context is shorter than q_len.
+ */
+cp_status cp_decode_workspace_bytes_qlen(cp_pool *pool, const int32_t *request_ids_host,
+                                         int32_t n_requests, int32_t q_len, uint64_t *bytes_out);
+cp_status cp_decode_attention_qlen(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                                   int32_t q_len, const void *q_dev, float *out_dev, float *lse_dev,
+                                   void *workspace_dev, uint64_t workspace_bytes, void *stream);
+
+/*
  * cp_decode_attention_stages -- several attention steps in ONE persistent launch: an
  * attention-only mock of the layer-wise pipeline, "two in-flight batches, each with its own model
  * id, layer cursor, and completion state" advanced "without requiring the two batches to have the

@@ -89,6 +89,8 @@ def load_library():
         "cp_decode_attention": (i32, [vp, i32p, i32, vp, vp, vp, vp, u64, vp]),
         "cp_decode_workspace_bytes_host": (i32, [vp, i32p, i32, u64p]),
         "cp_decode_attention_host": (i32, [vp, i32p, i32, vp, vp, vp, vp, u64, vp]),
+        "cp_decode_workspace_bytes_qlen": (i32, [vp, i32p, i32, i32, u64p]),
+        "cp_decode_attention_qlen": (i32, [vp, i32p, i32, i32, vp, vp, vp, vp, u64, vp]),
         "cp_decode_stages_workspace_bytes": (i32, [vp, i32, i32p, i32p, i32p, u64p]),
         "cp_decode_attention_stages": (i32, [vp, i32, i32p, i32p, i32p, ctypes.c_float, vp, vp, vp, vp, u64, vp]),
         "cp_decode_plan": (i32, [vp, i32p, i32, ctypes.POINTER(cp_tile_info), i32, i32p, i32p]),
@@ -112,7 +114,8 @@ EXPORTED = ["cp_pool_create", "cp_pool_create_vmm", "cp_pool_vmm_info", "cp_pool
             "cp_pool_request_info", "cp_pool_stats", "cp_pool_set_option", "cp_pool_gather_kv",
             "cp_pool_append_kv",
             "cp_decode_workspace_bytes", "cp_decode_attention", "cp_decode_workspace_bytes_host",
-            "cp_decode_attention_host", "cp_decode_stages_workspace_bytes", "cp_decode_attention_stages", "cp_decode_plan", "cp_pool_counters", "cp_status_string",
+            "cp_decode_attention_host", "cp_decode_workspace_bytes_qlen", "cp_decode_attention_qlen",
+            "cp_decode_stages_workspace_bytes", "cp_decode_attention_stages", "cp_decode_plan", "cp_pool_counters", "cp_status_string",
             "cp_planner_workspace_bytes", "cp_planner_pool_demand", "cp_planner_quantile"]
 
 
@@ -237,6 +240,21 @@ class Pool:
         _check(self._L.cp_pool_counters(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)),
                "cp_pool_counters")
         return {"kernel_launches": a.value, "plan_builds": b.value, "metadata_h2d_bytes": c.value}
+
+    # --- several query tokens per request (causal over the context's last q_len tokens)
+    def decode_workspace_bytes_qlen(self, request_ids, q_len: int) -> int:
+        ids = _ids(request_ids)
+        out = ctypes.c_uint64()
+        _check(self._L.cp_decode_workspace_bytes_qlen(self._h, _i32p(ids), ids.size, q_len, ctypes.byref(out)),
+               "cp_decode_workspace_bytes_qlen")
+        return int(out.value)
+
+    def decode_attention_qlen(self, request_ids, q_len: int, q_dev, out_dev, lse_dev, workspace_dev,
+                              workspace_bytes: int, stream: int = 0):
+        ids = _ids(request_ids)
+        _check(self._L.cp_decode_attention_qlen(self._h, _i32p(ids), ids.size, q_len, _ptr(q_dev), _ptr(out_dev),
+                                                _ptr(lse_dev), _ptr(workspace_dev), workspace_bytes, stream),
+               "cp_decode_attention_qlen")
 
     # --- several attention steps in one persistent launch (layer-wise stages)
     @staticmethod

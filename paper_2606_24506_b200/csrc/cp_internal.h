@@ -143,6 +143,7 @@ struct DecodeParams {
     int32_t *group_counters;       // [n_groups * kCounterStride] tile arrivals, counter g at g * kCounterStride
     int32_t *reset_counters;
     // multi-stage launches only (else nullptr / 0)
+    int32_t q_len;                 // query tokens per request (1 except cp_decode_attention_qlen)
     const StageRec *stages;
     int32_t *stage_done;           // [n_stages] completion counters, kCounterStride apart
     int32_t n_stages;       // the other counter set ([32] scheduler + group counters): cleared by this launch

@@ -91,8 +91,8 @@ struct TileDesc {
     int32_t mt;              // 16-head M tiles (power of two)
     float scale_log2;
     int64_t q_off, out_off, lse_off, part_off;
-    int32_t stage;           // multi-stage launches: the stage of this tile
-    int32_t pad;
+    int32_t stage;           // multi-stage launches: the stage of this tile; q_len > 1: heads per kv head
+    int32_t hq;              // query heads of the model (row stride of a query token)
 };
 
 // ----------------------------------------------------------------------------- PTX helpers (see also cp_ptx.cuh)
@@ -139,15 +139,19 @@ struct ConsumerSync {
 // warp's 16-head M tile.  S (16 x 8NT) = Q K^T as NT independent accumulator chains (ILP for the
 // tensor pipe), one online-softmax update per unit (log2 units), O (16 x 128) += P V.
 // koff / vbase: per-lane swizzle constants (see the caller).
-template <int P, int NT>
+// QLEN (several query tokens per request): the two rows of a thread may belong to different query
+// tokens, each with its own causal limit (valid - back0 / valid - back1); a row can then have no
+// visible token in a slice, or none yet at all (m = -inf), which the single-token path never sees.
+template <int P, int NT, bool QLEN = false>
 __device__ __forceinline__ void kv_slice_unit(const uint32_t sb, const int tok0, const int valid,
                                               const uint32_t (&qf)[8][4], const float scale_log2,
                                               float (&o)[16][4], float (&m_run)[2], float (&l_run)[2],
                                               const int lane, const uint32_t (&koff)[2], const uint32_t vrow,
-                                              const uint32_t vbase)
+                                              const uint32_t vbase, const int back0 = 0, const int back1 = 0)
 {
     constexpr int SUB = P * 128;                    // one swizzled sub-tile: P rows x 128 B
     const int cq = (lane & 3) * 2;
+    const int valid0 = QLEN ? valid - back0 : valid, valid1 = QLEN ? valid - back1 : valid;
     // ---- S = Q K^T for 8*NT tokens
     float s[NT][4];
 #pragma unroll
@@ -180,10 +184,10 @@ __device__ __forceinline__ void kv_slice_unit(const uint32_t sb, const int tok0,
 #pragma unroll
     for (int nt = 0; nt < NT; ++nt) {
         const int t = tok0 + nt * 8 + cq;
-        s[nt][0] = (t < valid) ? s[nt][0] * scale_log2 : -INFINITY;
-        s[nt][1] = (t + 1 < valid) ? s[nt][1] * scale_log2 : -INFINITY;
-        s[nt][2] = (t < valid) ? s[nt][2] * scale_log2 : -INFINITY;
-        s[nt][3] = (t + 1 < valid) ? s[nt][3] * scale_log2 : -INFINITY;
+        s[nt][0] = (t < valid0) ? s[nt][0] * scale_log2 : -INFINITY;
+        s[nt][1] = (t + 1 < valid0) ? s[nt][1] * scale_log2 : -INFINITY;
+        s[nt][2] = (t < valid1) ? s[nt][2] * scale_log2 : -INFINITY;
+        s[nt][3] = (t + 1 < valid1) ? s[nt][3] * scale_log2 : -INFINITY;
         mx0 = fmaxf(mx0, fmaxf(s[nt][0], s[nt][1]));
         mx1 = fmaxf(mx1, fmaxf(s[nt][2], s[nt][3]));
     }
@@ -196,14 +200,21 @@ __device__ __forceinline__ void kv_slice_unit(const uint32_t sb, const int tok0,
     // overflow), so the O rescale below is rare instead of once per slice.  (m, l, O) stay
     // mutually consistent: any reference gives the same O / l and LSE = m + log2 l.
     // token tok0 is valid (the caller skips dead slices), so mn0 / mn1 are finite
-    const float mn0 = (mx0 > m_run[0] + KV_LAZY_LOG2) ? mx0 : m_run[0];
-    const float mn1 = (mx1 > m_run[1] + KV_LAZY_LOG2) ? mx1 : m_run[1];
-    if (__any_sync(0xffffffffu, (mn0 != m_run[0]) || (mn1 != m_run[1]))) {
+    float mn0 = (mx0 > m_run[0] + KV_LAZY_LOG2) ? mx0 : m_run[0];
+    float mn1 = (mx1 > m_run[1] + KV_LAZY_LOG2) ? mx1 : m_run[1];
+    // QLEN: a row that has seen no token yet keeps m = -inf; the exponents below then use 0 as the
+    // reference (2^(-inf - 0) = 0) instead of -inf - (-inf)
+    const float mk0 = mn0, mk1 = mn1;
+    if (QLEN) {
+        mn0 = (mn0 == -INFINITY) ? 0.f : mn0;
+        mn1 = (mn1 == -INFINITY) ? 0.f : mn1;
+    }
+    if (__any_sync(0xffffffffu, (mk0 != m_run[0]) || (mk1 != m_run[1]))) {
         const float a0 = ex2(m_run[0] - mn0), a1 = ex2(m_run[1] - mn1);
         l_run[0] *= a0; l_run[1] *= a1;
 #pragma unroll
         for (int i = 0; i < 16; ++i) { o[i][0] *= a0; o[i][1] *= a0; o[i][2] *= a1; o[i][3] *= a1; }
-        m_run[0] = mn0; m_run[1] = mn1;
+        m_run[0] = mk0; m_run[1] = mk1;
     }
     uint32_t pf[NT * 2];
     float sum0 = 0.f, sum1 = 0.f;
@@ -258,7 +269,10 @@ __device__ __forceinline__ uint32_t stage_query2(uint32_t q_in, float2 o, float 
 // runs its combine units of every earlier stage before it starts a tile of a later one, and a tile
 // of a dependent stage waits for its predecessor's completion counter before it builds its queries
 // from that stage's output.  Waits only ever target earlier entries of the list, so they terminate.
-template <int P, bool MULTI>
+// QLEN: q_len > 1 query tokens per request (cp_decode_attention_qlen).  Row r of a group is query token
+// r / g, head r % g of the kv head's g heads; its causal limit ends q_len - 1 - r / g tokens before the
+// context's end.
+template <int P, bool MULTI, bool QLEN>
 __global__ void __launch_bounds__(KV_THREADS, 1)
 cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap, int rows_per_page)
 {
@@ -335,7 +349,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 d.npg = r.n_pages; d.split = r.split; d.n_splits = r.n_splits;
                 d.ctx = ctx; d.gsize = r.gsize; d.mt = mt; d.scale_log2 = r.scale_log2;
                 d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
-                d.stage = r.pad; d.pad = 0;
+                d.stage = r.pad; d.hq = r.n_q_heads;
                 tq[qs] = d;
                 mbar_arrive(smem_u32(tqf_b + qs));     // release: consumers acquire via try_wait
             }
@@ -419,9 +433,19 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
 
             // ---- Q fragments (A operand, 16 heads x 128), rows beyond the group are zero
             uint32_t qf[8][4];
+            int64_t row0 = h0, row1 = h1;        // row offsets (in rows of 128) of my two rows in Q / O / LSE
+            int back0 = 0, back1 = 0;            // QLEN: tokens at the context's end my rows must not see
             {
-                const uint16_t *q0 = p.q + d.q_off + (int64_t)h0 * KV_D;
-                const uint16_t *q1 = p.q + d.q_off + (int64_t)h1 * KV_D;
+                if constexpr (QLEN) {
+                    const int g = d.stage;                       // heads per kv head
+                    const int j0q = h0 / g, j1q = h1 / g;
+                    row0 = (int64_t)j0q * d.hq + (h0 - j0q * g);
+                    row1 = (int64_t)j1q * d.hq + (h1 - j1q * g);
+                    back0 = h0 < gsize ? p.q_len - 1 - j0q : 0;
+                    back1 = h1 < gsize ? p.q_len - 1 - j1q : 0;
+                }
+                const uint16_t *q0 = p.q + d.q_off + row0 * KV_D;
+                const uint16_t *q1 = p.q + d.q_off + row1 * KV_D;
 #pragma unroll
                 for (int ks = 0; ks < 8; ++ks) {
                     const int k = ks * 16 + cq;
@@ -490,7 +514,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                         __syncwarp();
                     }
-                    kv_slice_unit<P, NT>(sb, tok0, valid, qf, scale_log2, o, m_run, l_run, lane, koff, vrow, vbase);
+                    kv_slice_unit<P, NT, QLEN>(sb, tok0, valid, qf, scale_log2, o, m_run, l_run, lane, koff, vrow, vbase, back0, back1);
                 }
 #endif
                 __syncwarp();
@@ -552,16 +576,16 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             if (plane == 0) {
                 if (d.n_splits == 1) {
                     const float i0 = 1.f / l_run[0], i1 = 1.f / l_run[1];
-                    float *d0 = p.out + d.out_off + (int64_t)h0 * KV_D + cq;
-                    float *d1 = p.out + d.out_off + (int64_t)h1 * KV_D + cq;
+                    float *d0 = p.out + d.out_off + row0 * KV_D + cq;
+                    float *d1 = p.out + d.out_off + row1 * KV_D + cq;
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
                         if (h0 < gsize) *reinterpret_cast<float2 *>(d0 + i * 8) = make_float2(o[i][0] * i0, o[i][1] * i0);
                         if (h1 < gsize) *reinterpret_cast<float2 *>(d1 + i * 8) = make_float2(o[i][2] * i1, o[i][3] * i1);
                     }
                     if ((lane & 3) == 0) {
-                        if (h0 < gsize) p.lse[d.lse_off + h0] = (m_run[0] + log2f(l_run[0])) * 0.6931471805599453f;
-                        if (h1 < gsize) p.lse[d.lse_off + h1] = (m_run[1] + log2f(l_run[1])) * 0.6931471805599453f;
+                        if (h0 < gsize) p.lse[d.lse_off + row0] = (m_run[0] + log2f(l_run[0])) * 0.6931471805599453f;
+                        if (h1 < gsize) p.lse[d.lse_off + row1] = (m_run[1] + log2f(l_run[1])) * 0.6931471805599453f;
                     }
                     if constexpr (MULTI) {          // a single-split group is complete with this tile
                         __syncwarp();
@@ -647,18 +671,18 @@ extern "C" int cp_kv_probe_read(unsigned long long *out_host)
 
 bool kv_fast_supported(int P) { return P == 16 || P == 32 || P == 64 || P == 128; }
 
-template <int P, bool MULTI>
+template <int P, bool MULTI, bool QLEN>
 static cudaError_t launch_kv_tm(const DecodeParams &p, const CUtensorMap &tmap, int rows_per_page, int grid,
                                 cudaStream_t stream)
 {
     const int smem = kv_smem_bytes(P);
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(cp_decode_kv_kernel<P, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(cp_decode_kv_kernel<P, MULTI, QLEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    cp_decode_kv_kernel<P, MULTI><<<grid, KV_THREADS, smem, stream>>>(p, tmap, rows_per_page);
+    cp_decode_kv_kernel<P, MULTI, QLEN><<<grid, KV_THREADS, smem, stream>>>(p, tmap, rows_per_page);
     return cudaGetLastError();
 }
 
@@ -666,8 +690,9 @@ template <int P>
 static cudaError_t launch_kv_t(const DecodeParams &p, const CUtensorMap &tmap, int rows_per_page, int grid,
                                cudaStream_t stream)
 {
-    return p.n_stages > 0 ? launch_kv_tm<P, true>(p, tmap, rows_per_page, grid, stream)
-                          : launch_kv_tm<P, false>(p, tmap, rows_per_page, grid, stream);
+    if (p.n_stages > 0) return launch_kv_tm<P, true, false>(p, tmap, rows_per_page, grid, stream);
+    if (p.q_len > 1) return launch_kv_tm<P, false, true>(p, tmap, rows_per_page, grid, stream);
+    return launch_kv_tm<P, false, false>(p, tmap, rows_per_page, grid, stream);
 }
 
 cudaError_t launch_decode_kv(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas,

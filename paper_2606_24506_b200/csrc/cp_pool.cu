@@ -94,6 +94,9 @@ struct cp_pool {
     // options
     int opt_kernel = 0, opt_num_ctas = 0, opt_waves_x16 = 16, opt_min_tile_pages = 2;
 
+    // query tokens per request of the call in progress (cp_decode_attention_qlen), and of the cached plan
+    int qlen = 1, plan_qlen = 1;
+
     // plan cache
     std::vector<int32_t> plan_batch;
     uint64_t plan_version = 0;
@@ -170,9 +173,9 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         const Request &r = pool->reqs[ids[b]];
         const cp_model_cfg &m = pool->models[r.model];
         pool->q_off[b] = qo; pool->out_off[b] = oo; pool->lse_off[b] = lo;
-        qo += (int64_t)m.n_q_heads * m.head_dim_qk;
-        oo += (int64_t)m.n_q_heads * m.head_dim_v;
-        lo += m.n_q_heads;
+        qo += (int64_t)pool->qlen * m.n_q_heads * m.head_dim_qk;
+        oo += (int64_t)pool->qlen * m.n_q_heads * m.head_dim_v;
+        lo += (int64_t)pool->qlen * m.n_q_heads;
         total_pages[m.kind] += (int64_t)ceil_div(r.ctx, P) * m.n_kv_heads;
     }
     pool->q_elems = qo; pool->out_floats = oo; pool->lse_floats = lo;
@@ -222,7 +225,8 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             const Request &r = pool->reqs[ids[b]];
             const cp_model_cfg &m = pool->models[r.model];
             if (m.kind != k) continue;
-            const int g = m.n_q_heads / m.n_kv_heads;
+            const int hpk = m.n_q_heads / m.n_kv_heads;       // query heads per kv head
+            const int g = hpk * pool->qlen;                   // rows of a group: (query token, head), token-major
             const int n_lp = ceil_div(r.ctx, P);
             int ns = (int)((n_lp + L - 1) / L);
             ns = std::min(ns, kMaxSplits);                // bounds the combine's shared memory
@@ -236,9 +240,9 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
                 Group gr;
                 gr.req = ids[b]; gr.model = r.model; gr.kv_head = c; gr.n_splits = ns;
                 gr.n_pages = n_lp; gr.batch_index = b;
-                gr.q_off = pool->q_off[b] + (int64_t)c * g * m.head_dim_qk;
-                gr.out_off = pool->out_off[b] + (int64_t)c * g * m.head_dim_v;
-                gr.lse_off = pool->lse_off[b] + (int64_t)c * g;
+                gr.q_off = pool->q_off[b] + (int64_t)c * hpk * m.head_dim_qk;
+                gr.out_off = pool->out_off[b] + (int64_t)c * hpk * m.head_dim_v;
+                gr.lse_off = pool->lse_off[b] + (int64_t)c * hpk;
                 gr.part_off = 0;
                 if (ns > 1) {
                     gr.part_off = (int64_t)ws;
@@ -270,8 +274,10 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
                             std::memset(&cu, 0, sizeof(cu));
                             cu.part_off = gr.part_off + part_o_off(h, 0, ns, m.head_dim_v) + c0;
                             cu.ml_off = gr.part_off + part_ml_off(g, h, 0, ns, m.head_dim_v);
-                            cu.out_off = gr.out_off + (int64_t)h * m.head_dim_v + c0;
-                            cu.lse_off = c0 == 0 ? gr.lse_off + h : -1;
+                            // row h = query token h / hpk, head h % hpk; a token's rows are Hq apart
+                            const int64_t row = (int64_t)(h / hpk) * m.n_q_heads + h % hpk;
+                            cu.out_off = gr.out_off + row * m.head_dim_v + c0;
+                            cu.lse_off = c0 == 0 ? gr.lse_off + row : -1;
                             cu.split_stride = m.head_dim_v;
                             cu.n_splits = ns;
                             cu.zl_log2 = zl;
@@ -296,7 +302,8 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             std::memset(&r, 0, sizeof(r));
             r.group = t.group; r.req = gr.req; r.kv_head = gr.kv_head; r.n_kv_heads = m.n_kv_heads;
             r.page_begin = t.page_begin; r.n_pages = t.page_end - t.page_begin; r.split = t.split;
-            r.n_splits = gr.n_splits; r.gsize = m.n_q_heads / m.n_kv_heads; r.n_q_heads = m.n_q_heads;
+            r.n_splits = gr.n_splits; r.gsize = m.n_q_heads / m.n_kv_heads * pool->qlen; r.n_q_heads = m.n_q_heads;
+            r.pad = pool->qlen > 1 ? m.n_q_heads / m.n_kv_heads : 0;
             r.scale_log2 = (float)((double)m.softmax_scale * 1.4426950408889634);
             r.q_off = gr.q_off; r.out_off = gr.out_off; r.lse_off = gr.lse_off; r.part_off = gr.part_off;
         }
@@ -312,6 +319,7 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
     pool->plan_ws_floats = ws;
     pool->plan_batch.assign(ids, ids + n);
     pool->plan_version = pool->topo_version;
+    pool->plan_qlen = pool->qlen;
     pool->plan_valid = true;
     pool->n_plan_builds++;
 }
@@ -333,7 +341,7 @@ cp_status check_batch(cp_pool *pool, const int32_t *ids, int n)
 
 void ensure_plan(cp_pool *pool, const int32_t *ids, int n)
 {
-    if (pool->plan_valid && pool->plan_version == pool->topo_version &&
+    if (pool->plan_valid && pool->plan_version == pool->topo_version && pool->plan_qlen == pool->qlen &&
         (int)pool->plan_batch.size() == n && std::equal(ids, ids + n, pool->plan_batch.begin()))
         return;
     build_plan(pool, ids, n);
@@ -909,7 +917,7 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.work_counter = (int32_t *)kp.d_counters.ptr + kp.counter_set * set_ints;
         prm.group_counters = prm.work_counter + 32;
         prm.reset_counters = (int32_t *)kp.d_counters.ptr + (1 - kp.counter_set) * set_ints;
-        prm.stages = nullptr; prm.stage_done = nullptr; prm.n_stages = 0;
+        prm.stages = nullptr; prm.stage_done = nullptr; prm.n_stages = 0; prm.q_len = pool->qlen;
         kp.counter_set ^= 1;
         const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
         cudaError_t e;
@@ -933,6 +941,60 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         if (e != cudaSuccess) return CP_ERR_CUDA;
     }
     return CP_OK;
+}
+
+// ------------------------------------------------------------------ q_len > 1 (SURVEY 8(f) N4 variant)
+namespace {
+
+cp_status check_qlen(cp_pool *pool, const int32_t *ids, int n, int q_len)
+{
+    cp_status st = check_batch(pool, ids, n);
+    if (st != CP_OK) return st;
+    if (q_len < 1 || q_len > 128) return CP_ERR_INVALID_ARG;
+    if (q_len == 1) return CP_OK;
+    if (pool->opt_kernel == 1 || !kv_fast_supported((int)pool->P)) return CP_ERR_UNSUPPORTED;
+    for (int b = 0; b < n; ++b) {
+        const Request &r = pool->reqs[ids[b]];
+        const cp_model_cfg &m = pool->models[r.model];
+        if (r.ctx < q_len) return CP_ERR_INVALID_ARG;           // the query tokens are the context's last q_len
+        if (m.kind != CP_KIND_KV || m.head_dim_qk != 128 || m.head_dim_v != 128 ||
+            m.n_q_heads / m.n_kv_heads * q_len > 128)
+            return CP_ERR_UNSUPPORTED;
+    }
+    return CP_OK;
+}
+
+}  // namespace
+
+cp_status cp_decode_workspace_bytes_qlen(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                                         int32_t q_len, uint64_t *bytes_out)
+{
+    if (!bytes_out) return CP_ERR_INVALID_ARG;
+    const cp_status st = check_qlen(pool, request_ids_host, n_requests, q_len);
+    if (st != CP_OK) return st;
+    pool->qlen = q_len;
+    ensure_plan(pool, request_ids_host, n_requests);
+    pool->qlen = 1;
+    *bytes_out = pool->plan_ws_floats * 4;
+    return CP_OK;
+}
+
+cp_status cp_decode_attention_qlen(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                                   int32_t q_len, const void *q_dev, float *out_dev, float *lse_dev,
+                                   void *workspace_dev, uint64_t workspace_bytes, void *stream)
+{
+    cp_status st = check_qlen(pool, request_ids_host, n_requests, q_len);
+    if (st != CP_OK) return st;
+    if (q_len > 1) {
+        st = ensure_device(pool);                               // the fast kernel needs its tensor map
+        if (st != CP_OK) return st;
+        if (!pool->kv_tmap_ok) return CP_ERR_UNSUPPORTED;
+    }
+    pool->qlen = q_len;
+    st = cp_decode_attention(pool, request_ids_host, n_requests, q_dev, out_dev, lse_dev, workspace_dev,
+                             workspace_bytes, stream);
+    pool->qlen = 1;
+    return st;
 }
 
 // ------------------------------------------------------------------ multi-stage launch
@@ -1113,7 +1175,7 @@ cp_status cp_decode_attention_stages(cp_pool *pool, int32_t n_stages, const int3
     prm.reset_counters = (int32_t *)kp.d_counters.ptr + (1 - kp.counter_set) * set_ints;
     prm.stages = (const StageRec *)sp.d_stages.ptr;
     prm.stage_done = prm.group_counters + kp.groups.size() * (size_t)kCounterStride;
-    prm.n_stages = n_stages;
+    prm.n_stages = n_stages; prm.q_len = 1;
     kp.counter_set ^= 1;
     const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
     const cudaError_t e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256), std::min(n_ctas, pool->n_sm), s);
