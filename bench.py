@@ -502,6 +502,30 @@ def main():
             pl.close()
         del arena_l
 
+    # ---------------- q_len > 1 (SURVEY §8(f) N4 variant): the same KV, four query tokens per request
+    qlen_leg = None
+    if rank == 0 and not args.no_stages and all(m.kind == 0 and m.head_dim_qk == 128 and m.head_dim_v == 128 and
+                                                m.n_q_heads // m.n_kv_heads * 4 <= 128 for m in w.models):
+        ql = 4
+        rows = w.out_rows() * ql
+        qq = torch.randn(rows * 128, device=dev).to(torch.bfloat16).view(torch.int16)
+        oq = torch.empty(rows * 128, dtype=torch.float32, device=dev)
+        lq = torch.empty(rows, dtype=torch.float32, device=dev)
+        wsb = max(dw.pool.decode_workspace_bytes_qlen(dw.ids, ql), 256)
+        wsq = torch.empty(wsb, dtype=torch.uint8, device=dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ts = []
+        for i in range(3 + 20):
+            spacer(i)
+            e0.record()
+            dw.pool.decode_attention_qlen(dw.ids, ql, qq, oq, lq, wsq, wsb, dw.stream())
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        t = float(np.median(ts[3:]))
+        qlen_leg = {"q_len": ql, "us_per_step": 1e3 * t, "kv_gbs": abytes / (t * 1e-3) / 1e9}
+        del qq, oq, lq, wsq
+
     # ---------------- KV-cache planner (Eq. (1)-(2)): pool demand at 100 000 observation
     # times of a two-hour synthetic trace of 8 cold models, then P95 / P99 and the page budgets
     planner = None
@@ -584,7 +608,7 @@ def main():
                     "us_per_step": 1e3 * e2e_ms,
                     "h2d_bytes_per_step": int(q_host.numel() * 2),
                     "d2h_bytes_per_step": int(o_host.numel() * 4 + l_host.numel() * 4)},
-            "gpu_launches": int(launches), "roofline": roof, "gather": gather, "append": append, "vmm_arena": vmm, "planner": planner, "stages": stages_leg,
+            "gpu_launches": int(launches), "roofline": roof, "gather": gather, "append": append, "vmm_arena": vmm, "planner": planner, "stages": stages_leg, "qlen": qlen_leg,
             "pct_of_hbm_peak": {"measured_copy": 100 * achieved / peaks["hbm_gbs"], "nominal_8TBs": 100 * achieved / 8000.0}}
 
     if not args.no_cpu_baseline:
