@@ -29,8 +29,8 @@ if ROOT not in sys.path:
 import numpy as np
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the decode kernel, from the committed
-# `ncu --set full` captures (profiles/r1_ncu_full_cfg2_kv_v5.txt, r1_ncu_full_cfg4_kv_v3.txt, r1_ncu_full_cfg3_mla_pair.txt)
-NCU_TRAFFIC_BYTES = {2: 344.70e6 + 6.07e6, 3: 285.04e6 + 9.61e6, 4: 134.33e6 + 6.31e6}
+# `ncu --set full` captures (profiles/r1_ncu_full_cfg2_kv_v6.txt, r1_ncu_full_cfg4_kv_v3.txt, r1_ncu_full_cfg3_mla_pair.txt)
+NCU_TRAFFIC_BYTES = {2: 344.66e6 + 6.97e6, 3: 285.04e6 + 9.61e6, 4: 134.33e6 + 6.31e6}
 NCU_TENSOR_PIPE_PCT = {3: 34.0}       # sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active
 
 METRIC = "paged decode-attention KV GB/s"
