@@ -316,6 +316,29 @@ cp_status cp_decode_attention_stages(cp_pool *pool, int32_t n_stages,
                                      void *workspace_dev, uint64_t workspace_bytes, void *stream);
 
 /*
+ * cp_decode_attention_stages_gated -- the same launch behind an ADMISSION DOORBELL: the persistent
+ * CTAs poll *published_dev (any device-accessible int32: device memory the host updates with a copy on
+ * another stream, or mapped pinned host memory) and hand out the tiles of stage s -- and request its
+ * KV pages -- only once *published_dev > s.  This is the GPU-side half of "persistent kernel[s]
+ * repeatedly poll per-model request queues on GPUs ... while the host remains responsible for
+ * coarse-grained admission": the host admits batches while the kernel runs and
+ * never launches per layer.  The caller must eventually publish n_stages.  A poll that lasts longer
+ * than timeout_ms stops gating (the launch then completes as the ungated one would) and raises a flag
+ * that cp_decode_stages_gate_status returns; the device is never left spinning.
+ * Extra errors: INVALID_ARG (NULL / misaligned doorbell, timeout_ms = 0).
+ * cp_decode_stages_gate_status synchronises `stream` and writes 1 if the last gated launch saw a
+ * poll time out, else 0.
+ */
+cp_status cp_decode_attention_stages_gated(cp_pool *pool, int32_t n_stages,
+                                           const int32_t *stage_sizes_host,
+                                           const int32_t *request_ids_host,
+                                           const int32_t *stage_dep_host, float alpha,
+                                           const void *q_dev, float *out_dev, float *lse_dev,
+                                           void *workspace_dev, uint64_t workspace_bytes, void *stream,
+                                           const int32_t *published_dev, uint32_t timeout_ms);
+cp_status cp_decode_stages_gate_status(cp_pool *pool, void *stream, int32_t *timed_out_host);
+
+/*
  * cp_decode_plan -- introspection of the device work list the next cp_decode_attention on
  * this batch will consume (host only, no CUDA): writes up to cap tiles in the order the
  * persistent CTAs pop them.  n_tiles_out receives the total number of tiles,

@@ -93,6 +93,9 @@ def load_library():
         "cp_decode_attention_qlen": (i32, [vp, i32p, i32, i32, vp, vp, vp, vp, u64, vp]),
         "cp_decode_stages_workspace_bytes": (i32, [vp, i32, i32p, i32p, i32p, u64p]),
         "cp_decode_attention_stages": (i32, [vp, i32, i32p, i32p, i32p, ctypes.c_float, vp, vp, vp, vp, u64, vp]),
+        "cp_decode_attention_stages_gated": (i32, [vp, i32, i32p, i32p, i32p, ctypes.c_float, vp, vp, vp, vp, u64, vp,
+                                                   vp, u32]),
+        "cp_decode_stages_gate_status": (i32, [vp, vp, i32p]),
         "cp_decode_plan": (i32, [vp, i32p, i32, ctypes.POINTER(cp_tile_info), i32, i32p, i32p]),
         "cp_pool_counters": (i32, [vp, u64p, u64p, u64p]),
         "cp_status_string": (ctypes.c_char_p, [i32]),
@@ -115,7 +118,8 @@ EXPORTED = ["cp_pool_create", "cp_pool_create_vmm", "cp_pool_vmm_info", "cp_pool
             "cp_pool_append_kv",
             "cp_decode_workspace_bytes", "cp_decode_attention", "cp_decode_workspace_bytes_host",
             "cp_decode_attention_host", "cp_decode_workspace_bytes_qlen", "cp_decode_attention_qlen",
-            "cp_decode_stages_workspace_bytes", "cp_decode_attention_stages", "cp_decode_plan", "cp_pool_counters", "cp_status_string",
+            "cp_decode_stages_workspace_bytes", "cp_decode_attention_stages", "cp_decode_attention_stages_gated",
+            "cp_decode_stages_gate_status", "cp_decode_plan", "cp_pool_counters", "cp_status_string",
             "cp_planner_workspace_bytes", "cp_planner_pool_demand", "cp_planner_quantile"]
 
 
@@ -280,6 +284,20 @@ class Pool:
                                                   float(alpha), _ptr(q_dev), _ptr(out_dev), _ptr(lse_dev),
                                                   _ptr(workspace_dev), workspace_bytes, stream),
                "cp_decode_attention_stages")
+
+    def decode_attention_stages_gated(self, stages, deps, alpha: float, q_dev, out_dev, lse_dev, workspace_dev,
+                                      workspace_bytes: int, stream: int, published_dev, timeout_ms: int):
+        sizes, ids, deps = self._stage_args(stages, deps)
+        _check(self._L.cp_decode_attention_stages_gated(self._h, sizes.size, _i32p(sizes), _i32p(ids), _i32p(deps),
+                                                        float(alpha), _ptr(q_dev), _ptr(out_dev), _ptr(lse_dev),
+                                                        _ptr(workspace_dev), workspace_bytes, stream,
+                                                        _ptr(published_dev), timeout_ms),
+               "cp_decode_attention_stages_gated")
+
+    def decode_stages_gate_status(self, stream: int = 0) -> int:
+        out = ctypes.c_int32()
+        _check(self._L.cp_decode_stages_gate_status(self._h, stream, ctypes.byref(out)), "cp_decode_stages_gate_status")
+        return int(out.value)
 
     def decode_plan(self, request_ids):
         ids = _ids(request_ids)

@@ -22,6 +22,20 @@ __device__ __forceinline__ int ld_acquire(const int32_t *p)
     return v;
 }
 
+__device__ __forceinline__ int ld_acquire_sys(const int32_t *p)
+{
+    int v;
+    asm volatile("ld.acquire.sys.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ unsigned long long global_timer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
 // Physical page of entry `idx` of request `req`'s page list.  Software table (PAPER.md, reading R1)
 // or, on a CUDA-VMM arena, plain arithmetic on the request's contiguous virtual range.
 __device__ __forceinline__ int32_t page_of(const DecodeParams &p, int req, int64_t idx)

@@ -145,6 +145,9 @@ struct DecodeParams {
     // multi-stage launches only (else nullptr / 0)
     int32_t q_len;                 // query tokens per request (1 except cp_decode_attention_qlen)
     const StageRec *stages;
+    const int32_t *published;      // admission doorbell (gated multi-stage launch) or nullptr: stages admitted so far
+    int32_t *gate_flag;            // set to 1 if a poll of the doorbell timed out
+    uint32_t gate_timeout_us;
     int32_t *stage_done;           // [n_stages] completion counters, kCounterStride apart
     int32_t n_stages;       // the other counter set ([32] scheduler + group counters): cleared by this launch
 };

@@ -340,6 +340,27 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 r.split = 0; r.n_splits = 1; r.gsize = 1; r.n_q_heads = 1; r.scale_log2 = 0.f;
                 r.q_off = r.out_off = r.lse_off = r.part_off = 0; r.pad = 0;
             }
+            if constexpr (MULTI) {
+                // Admission doorbell (cp_decode_attention_stages_gated): the host -- "coarse-grained admission"
+                // stays on the CPU, PAPER.md L146 -- raises *published as it admits batches; a tile is handed
+                // to the consumers, and its pages are requested, only once its stage is admitted.  A poll
+                // that outlasts the timeout stops gating and raises a flag instead of hanging the device.
+                if (p.published != nullptr && item >= 0) {
+                    if (lane == 0) {
+                        unsigned ns = 256;
+                        const unsigned long long t0 = global_timer_ns();
+                        while (ld_acquire_sys(p.published) <= r.pad) {
+                            __nanosleep(ns);
+                            if (ns < 4096) ns <<= 1;
+                            if (global_timer_ns() - t0 > (unsigned long long)p.gate_timeout_us * 1000ull) {
+                                atomicExch(p.gate_flag, 1);
+                                break;
+                            }
+                        }
+                    }
+                    __syncwarp();
+                }
+            }
             // push the descriptor to the tile queue
             const uint32_t qs = qi % KV_TQ;
             mbar_wait(smem_u32(tqe_b + qs), ((qi / KV_TQ) & 1) ^ 1);

@@ -124,7 +124,7 @@ struct cp_pool {
         bool valid = false, uploaded = false;
         KindPlan kp;
         std::vector<StageRec> stages;
-        DevBuf d_stages;
+        DevBuf d_stages, d_gate;
         uint64_t ws_floats = 0;
         int64_t q_elems = 0, out_floats = 0, lse_floats = 0;
     } splan;
@@ -578,7 +578,7 @@ cp_status cp_pool_free(cp_pool *pool)
     {
         KindPlan &kp = pool->splan.kp;
         kp.d_groups.release(); kp.d_tiles.release(); kp.d_combines.release(); kp.d_cunits.release();
-        kp.d_tile_recs.release(); kp.d_counters.release(); pool->splan.d_stages.release();
+        kp.d_tile_recs.release(); kp.d_counters.release(); pool->splan.d_stages.release(); pool->splan.d_gate.release();
     }
     delete pool;
     return CP_OK;
@@ -918,6 +918,7 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.group_counters = prm.work_counter + 32;
         prm.reset_counters = (int32_t *)kp.d_counters.ptr + (1 - kp.counter_set) * set_ints;
         prm.stages = nullptr; prm.stage_done = nullptr; prm.n_stages = 0; prm.q_len = pool->qlen;
+        prm.published = nullptr; prm.gate_flag = nullptr; prm.gate_timeout_us = 0;
         kp.counter_set ^= 1;
         const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
         cudaError_t e;
@@ -1122,10 +1123,11 @@ cp_status cp_decode_stages_workspace_bytes(cp_pool *pool, int32_t n_stages, cons
     return CP_OK;
 }
 
-cp_status cp_decode_attention_stages(cp_pool *pool, int32_t n_stages, const int32_t *stage_sizes_host,
-                                     const int32_t *request_ids_host, const int32_t *stage_dep_host, float alpha,
-                                     const void *q_dev, float *out_dev, float *lse_dev, void *workspace_dev,
-                                     uint64_t workspace_bytes, void *stream)
+static cp_status decode_stages_core(cp_pool *pool, int32_t n_stages, const int32_t *stage_sizes_host,
+                                    const int32_t *request_ids_host, const int32_t *stage_dep_host, float alpha,
+                                    const void *q_dev, float *out_dev, float *lse_dev, void *workspace_dev,
+                                    uint64_t workspace_bytes, void *stream, const int32_t *published_dev,
+                                    uint32_t timeout_ms)
 {
     if (!pool || !q_dev || !out_dev || !lse_dev || !(alpha == alpha)) return CP_ERR_INVALID_ARG;
     if (((uintptr_t)q_dev & 15u) || ((uintptr_t)out_dev & 15u) || ((uintptr_t)lse_dev & 3u)) return CP_ERR_INVALID_ARG;
@@ -1176,11 +1178,54 @@ cp_status cp_decode_attention_stages(cp_pool *pool, int32_t n_stages, const int3
     prm.stages = (const StageRec *)sp.d_stages.ptr;
     prm.stage_done = prm.group_counters + kp.groups.size() * (size_t)kCounterStride;
     prm.n_stages = n_stages; prm.q_len = 1;
+    prm.published = nullptr; prm.gate_flag = nullptr; prm.gate_timeout_us = 0;
+    if (published_dev) {
+        if (sp.d_gate.ensure(16) != cudaSuccess || cudaMemsetAsync(sp.d_gate.ptr, 0, 16, s) != cudaSuccess) {
+            cudaGetLastError();
+            return CP_ERR_CUDA;
+        }
+        prm.published = published_dev; prm.gate_flag = (int32_t *)sp.d_gate.ptr;
+        prm.gate_timeout_us = timeout_ms > 4000000u ? 4000000000u : timeout_ms * 1000u;
+    }
     kp.counter_set ^= 1;
     const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
     const cudaError_t e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256), std::min(n_ctas, pool->n_sm), s);
     pool->n_launches++;
     if (e != cudaSuccess) return CP_ERR_CUDA;
+    return CP_OK;
+}
+
+cp_status cp_decode_attention_stages(cp_pool *pool, int32_t n_stages, const int32_t *stage_sizes_host,
+                                     const int32_t *request_ids_host, const int32_t *stage_dep_host, float alpha,
+                                     const void *q_dev, float *out_dev, float *lse_dev, void *workspace_dev,
+                                     uint64_t workspace_bytes, void *stream)
+{
+    return decode_stages_core(pool, n_stages, stage_sizes_host, request_ids_host, stage_dep_host, alpha, q_dev, out_dev,
+                              lse_dev, workspace_dev, workspace_bytes, stream, nullptr, 0);
+}
+
+cp_status cp_decode_attention_stages_gated(cp_pool *pool, int32_t n_stages, const int32_t *stage_sizes_host,
+                                           const int32_t *request_ids_host, const int32_t *stage_dep_host,
+                                           float alpha, const void *q_dev, float *out_dev, float *lse_dev,
+                                           void *workspace_dev, uint64_t workspace_bytes, void *stream,
+                                           const int32_t *published_dev, uint32_t timeout_ms)
+{
+    if (!published_dev || ((uintptr_t)published_dev & 3u) || timeout_ms == 0) return CP_ERR_INVALID_ARG;
+    return decode_stages_core(pool, n_stages, stage_sizes_host, request_ids_host, stage_dep_host, alpha, q_dev, out_dev,
+                              lse_dev, workspace_dev, workspace_bytes, stream, published_dev, timeout_ms);
+}
+
+cp_status cp_decode_stages_gate_status(cp_pool *pool, void *stream, int32_t *timed_out_host)
+{
+    if (!pool || !timed_out_host) return CP_ERR_INVALID_ARG;
+    *timed_out_host = 0;
+    if (!pool->splan.d_gate.ptr) return CP_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (cudaMemcpyAsync(timed_out_host, pool->splan.d_gate.ptr, 4, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaStreamSynchronize(s) != cudaSuccess) {
+        cudaGetLastError();
+        return CP_ERR_CUDA;
+    }
     return CP_OK;
 }
 

@@ -192,3 +192,79 @@ def test_stages_argument_errors(torch_cuda):
         torch.cuda.synchronize()
     finally:
         dw.close()
+
+
+def test_gated_launch_follows_the_hosts_admissions(torch_cuda):
+    """The doorbell variant: the kernel is launched with two stages admitted, the host admits the rest
+    in two steps from another stream while the kernel is running.  The launch cannot finish before
+    the last admission, finishes right after it, and computes the same bits as the ungated launch."""
+    import time
+    import paper_2606_24506_b200 as cp
+    torch = torch_cuda
+    w, order, stages, deps, q_in = build_case(BATCHES, 32, seed=123)
+    dw = device_workload(w)
+    try:
+        dw.pool.set_option(cp.CP_OPT_MIN_TILE_PAGES, 1)
+        base = run_stages(torch, dw, w, stages, deps, q_in, 1.0, relaunch=False)
+        dev = dw.device
+        ids = [[w.requests[ri].request_id for ri in st] for st in stages]
+        q = torch.from_numpy(np.concatenate([x.reshape(-1) for st in q_in for x in st]).view(np.int16)).to(dev)
+        rows = sum(x.shape[0] for st in q_in for x in st)
+        out = torch.full((rows * 128,), float("nan"), dtype=torch.float32, device=dev)
+        lse = torch.full((rows,), float("nan"), dtype=torch.float32, device=dev)
+        wsb = max(dw.pool.decode_stages_workspace_bytes(ids, deps), 256)
+        ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+        published = torch.tensor([2], dtype=torch.int32, device=dev)
+        steps = [torch.tensor([v], dtype=torch.int32).pin_memory() for v in (5, len(stages))]
+        run, side = torch.cuda.Stream(), torch.cuda.Stream()
+        torch.cuda.synchronize()
+        done = torch.cuda.Event()
+        t0 = time.perf_counter()
+        dw.pool.decode_attention_stages_gated(ids, deps, 1.0, q, out, lse, ws, wsb, run.cuda_stream, published, 5000)
+        done.record(run)
+        with torch.cuda.stream(side):
+            time.sleep(0.02)
+            assert not done.query(), "the launch finished before all its stages were admitted"
+            published.copy_(steps[0], non_blocking=True)
+            side.synchronize()
+            time.sleep(0.02)
+            assert not done.query()
+            published.copy_(steps[1], non_blocking=True)
+            side.synchronize()
+        run.synchronize()
+        elapsed = time.perf_counter() - t0
+        assert 0.04 <= elapsed < 1.0, elapsed
+        assert dw.pool.decode_stages_gate_status(run.cuda_stream) == 0
+        o, l = out.cpu().numpy(), lse.cpu().numpy()
+        assert np.array_equal(o, np.concatenate([x[0].reshape(-1) for st in base for x in st]))
+        assert np.array_equal(l, np.concatenate([x[1] for st in base for x in st]))
+    finally:
+        dw.close()
+
+
+def test_gated_launch_times_out_instead_of_hanging(torch_cuda):
+    """A doorbell the host never rings: after timeout_ms the CTAs stop gating, the launch completes with
+    the right result and the status call reports the timeout."""
+    import paper_2606_24506_b200 as cp
+    torch = torch_cuda
+    w, order, stages, deps, q_in = build_case(BATCHES[:2], 16, seed=5)
+    dw = device_workload(w)
+    try:
+        base = run_stages(torch, dw, w, stages, deps, q_in, 0.5, relaunch=False)
+        dev = dw.device
+        ids = [[w.requests[ri].request_id for ri in st] for st in stages]
+        q = torch.from_numpy(np.concatenate([x.reshape(-1) for st in q_in for x in st]).view(np.int16)).to(dev)
+        rows = sum(x.shape[0] for st in q_in for x in st)
+        out = torch.full((rows * 128,), float("nan"), dtype=torch.float32, device=dev)
+        lse = torch.full((rows,), float("nan"), dtype=torch.float32, device=dev)
+        wsb = max(dw.pool.decode_stages_workspace_bytes(ids, deps), 256)
+        ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+        published = torch.tensor([1], dtype=torch.int32, device=dev)
+        dw.pool.decode_attention_stages_gated(ids, deps, 0.5, q, out, lse, ws, wsb, dw.stream(), published, 30)
+        assert dw.pool.decode_stages_gate_status(dw.stream()) == 1
+        assert np.array_equal(out.cpu().numpy(), np.concatenate([x[0].reshape(-1) for st in base for x in st]))
+        with pytest.raises(cp.CrossPoolError) as e:
+            dw.pool.decode_attention_stages_gated(ids, deps, 0.5, q, out, lse, ws, wsb, dw.stream(), published, 0)
+        assert e.value.status == cp.CP_ERR_INVALID_ARG
+    finally:
+        dw.close()
