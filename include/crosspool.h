@@ -376,7 +376,8 @@ cp_status cp_pool_counters(const cp_pool *pool, uint64_t *kernel_launches,
  *   prompt_tokens_dev, output_tokens_dev, residence_dev   O_p,i, O_d,i, T_i (doubles; T_i <= 0
  *                        makes the request contribute nothing)
  *   t_obs_dev / k_pool_dev   [n_obs] in / out (bytes)
- *   workspace_dev        >= cp_planner_workspace_bytes() bytes, 16-B aligned, caller-owned
+ *   workspace_dev        >= cp_planner_workspace_bytes(offsets[n_models]) bytes, 16-B aligned,
+ *                        caller-owned (cp_planner_quantile needs cp_planner_workspace_bytes(0))
  * Errors: INVALID_ARG, WORKSPACE, CUDA.
  *
  * cp_planner_quantile -- the empirical quantile x_(k), k = ceil(q n) (1-based order statistic, no
@@ -387,7 +388,7 @@ cp_status cp_pool_counters(const cp_pool *pool, uint64_t *kernel_launches,
  * CUDA.
  */
 #define CP_PLANNER_MAX_MODELS 64
-uint64_t cp_planner_workspace_bytes(void);
+uint64_t cp_planner_workspace_bytes(int64_t n_trace_entries);
 cp_status cp_planner_pool_demand(int32_t n_models, const int64_t *trace_offsets_host,
                                  const double *kappa_host, const double *arrival_dev,
                                  const double *prompt_tokens_dev, const double *output_tokens_dev,

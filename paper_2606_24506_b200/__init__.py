@@ -99,7 +99,7 @@ def load_library():
         "cp_decode_plan": (i32, [vp, i32p, i32, ctypes.POINTER(cp_tile_info), i32, i32p, i32p]),
         "cp_pool_counters": (i32, [vp, u64p, u64p, u64p]),
         "cp_status_string": (ctypes.c_char_p, [i32]),
-        "cp_planner_workspace_bytes": (u64, []),
+        "cp_planner_workspace_bytes": (u64, [ctypes.c_int64]),
         "cp_planner_pool_demand": (i32, [i32, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_double),
                                          vp, vp, vp, vp, ctypes.c_int64, vp, vp, vp, u64, vp]),
         "cp_planner_quantile": (i32, [vp, ctypes.c_int64, ctypes.c_double, ctypes.c_double, vp, u64,
@@ -350,8 +350,8 @@ class Pool:
 
 
 # ---------------------------------------------------------------- KV-cache planner (Eq. (1)-(2))
-def planner_workspace_bytes() -> int:
-    return int(load_library().cp_planner_workspace_bytes())
+def planner_workspace_bytes(n_trace_entries: int = 0) -> int:
+    return int(load_library().cp_planner_workspace_bytes(int(n_trace_entries)))
 
 
 def planner_pool_demand(trace_offsets, kappa, arrival_dev, prompt_tokens_dev, output_tokens_dev, residence_dev,

@@ -8,9 +8,11 @@
 // the page budget ("rounds memory to pages", L112).  Everything is float64 and every operation is a
 // separately rounded IEEE operation in the paper's order (intrinsics, no FMA contraction), one
 // thread per observation time summing its terms in trace order, so the demand vector equals a plain
-// sequential evaluation bit for bit.  What the kernel adds is only a window: arrivals are ascending
-// inside a model, and a request older than the model's longest residence time (or not yet arrived)
-// contributes an exact zero, so two binary searches bound the terms that can be non-zero.
+// sequential evaluation bit for bit.  What the kernel adds is only pruning of exact zeros: arrivals
+// are ascending inside a model, so two binary searches bound the requests that can be resident (not
+// yet arrived, or older than the model's longest residence time: zero), and inside that window a
+// block of 32 consecutive requests is skipped when even its youngest member is older than the block's
+// longest residence time (fl(t - A) is monotone in A, so the test is exact, not approximate).
 //
 // The quantile is an exact selection, not a sort: four passes of a 16-bit radix select over the bit
 // patterns (non-negative doubles order like their bit patterns), histogram by warp-aggregated
@@ -34,7 +36,8 @@ struct PlannerModels {
 };
 
 // workspace layout (bytes): [0, 512) selection state, [512, 512 + 8 * kMaxModels) longest residence
-// time per model (bit patterns), then the histogram
+// time per model (bit patterns), the histogram, then the longest residence time per block of 32
+// trace entries
 struct SelectState {
     unsigned long long prefix;      // digits fixed so far (high bits of the answer)
     unsigned long long k;           // 1-based rank still to find among the elements matching prefix
@@ -43,7 +46,25 @@ struct SelectState {
 };
 constexpr size_t kOffTmax = 512;
 constexpr size_t kOffHist = kOffTmax + 8 * (size_t)kMaxModels;
-constexpr size_t kWorkspaceBytes = kOffHist + 4 * (size_t)kBins;
+constexpr size_t kOffBlocks = kOffHist + 4 * (size_t)kBins;
+constexpr int kBlock = 32;
+
+size_t workspace_bytes_for(int64_t n_entries)
+{
+    return kOffBlocks + 8 * (size_t)((n_entries + kBlock - 1) / kBlock) + 16;
+}
+
+// longest residence time of every block of 32 consecutive trace entries (one warp per block)
+__global__ void planner_block_tmax_kernel(const double *__restrict__ t_res, int64_t n, double *__restrict__ blk_tmax)
+{
+    const int64_t b = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t i = b * kBlock + (threadIdx.x & 31);
+    if (b * kBlock >= n) return;
+    double t = i < n ? t_res[i] : 0.0;
+    if (!(t > 0.0)) t = 0.0;
+    for (int o = 16; o > 0; o >>= 1) t = fmax(t, __shfl_xor_sync(0xffffffffu, t, o));
+    if ((threadIdx.x & 31) == 0) blk_tmax[b] = t;
+}
 
 __global__ void planner_tmax_kernel(PlannerModels pm, const double *__restrict__ t_res, unsigned long long *tmax_bits)
 {
@@ -79,8 +100,8 @@ __device__ __forceinline__ int64_t upper_bound(const double *__restrict__ a, int
 __global__ void __launch_bounds__(128)
 planner_demand_kernel(PlannerModels pm, const double *__restrict__ arrival, const double *__restrict__ o_p,
                       const double *__restrict__ o_d, const double *__restrict__ t_res,
-                      const unsigned long long *__restrict__ tmax_bits, int64_t n_obs,
-                      const double *__restrict__ t_obs, double *__restrict__ k_pool)
+                      const unsigned long long *__restrict__ tmax_bits, const double *__restrict__ blk_tmax,
+                      int64_t n_obs, const double *__restrict__ t_obs, double *__restrict__ k_pool)
 {
     const int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= n_obs) return;
@@ -95,12 +116,19 @@ planner_demand_kernel(PlannerModels pm, const double *__restrict__ arrival, cons
         const int64_t hi = upper_bound(arrival, lo, pm.offs[m + 1], t);      // A_i > t: u < 0, zero
         const double kappa = pm.kappa[m];
         double k_m = 0.0;
-        for (int64_t i = lo; i < hi; ++i) {
-            const double u = __dsub_rn(t, __ldg(arrival + i));
-            const double T = __ldg(t_res + i);
-            if (u >= 0.0 && u < T) {
-                const double q = __dadd_rn(__ldg(o_p + i), __dmul_rn(__ldg(o_d + i), __ddiv_rn(u, T)));
-                k_m = __dadd_rn(k_m, __dmul_rn(kappa, q));
+        for (int64_t i = lo; i < hi;) {
+            const int64_t b = i / kBlock;
+            const int64_t end = min(hi, (b + 1) * kBlock);
+            // the youngest request of this part of the block has the smallest age; if even that age is not
+            // below the block's longest residence time, every term of the block is an exact zero
+            if (__dsub_rn(t, __ldg(arrival + end - 1)) >= __ldg(blk_tmax + b)) { i = end; continue; }
+            for (; i < end; ++i) {
+                const double u = __dsub_rn(t, __ldg(arrival + i));
+                const double T = __ldg(t_res + i);
+                if (u >= 0.0 && u < T) {
+                    const double q = __dadd_rn(__ldg(o_p + i), __dmul_rn(__ldg(o_d + i), __ddiv_rn(u, T)));
+                    k_m = __dadd_rn(k_m, __dmul_rn(kappa, q));
+                }
             }
         }
         pool = __dadd_rn(pool, k_m);
@@ -201,7 +229,10 @@ bool fill_models(PlannerModels &pm, int32_t n_models, const int64_t *offs, const
 
 extern "C" {
 
-uint64_t cp_planner_workspace_bytes(void) { return kWorkspaceBytes; }
+uint64_t cp_planner_workspace_bytes(int64_t n_trace_entries)
+{
+    return workspace_bytes_for(n_trace_entries < 0 ? 0 : n_trace_entries);
+}
 
 cp_status cp_planner_pool_demand(int32_t n_models, const int64_t *trace_offsets_host, const double *kappa_host,
                                  const double *arrival_dev, const double *prompt_tokens_dev,
@@ -215,19 +246,23 @@ cp_status cp_planner_pool_demand(int32_t n_models, const int64_t *trace_offsets_
     const int64_t n_req = pm.offs[n_models];
     if (n_req > 0 && (!arrival_dev || !prompt_tokens_dev || !output_tokens_dev || !residence_dev))
         return CP_ERR_INVALID_ARG;
-    if (!workspace_dev || workspace_bytes < kWorkspaceBytes || ((uintptr_t)workspace_dev & 15u)) return CP_ERR_WORKSPACE;
+    if (!workspace_dev || workspace_bytes < workspace_bytes_for(n_req) || ((uintptr_t)workspace_dev & 15u))
+        return CP_ERR_WORKSPACE;
     if (n_obs == 0) return CP_OK;
     cudaStream_t s = (cudaStream_t)stream;
     unsigned long long *tmax = (unsigned long long *)((uint8_t *)workspace_dev + kOffTmax);
+    double *blk_tmax = (double *)((uint8_t *)workspace_dev + kOffBlocks);
     if (cudaMemsetAsync(tmax, 0, 8 * (size_t)kMaxModels, s) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
     if (n_req > 0) {
         int64_t longest = 0;
         for (int m = 0; m < n_models; ++m) longest = longest > pm.offs[m + 1] - pm.offs[m] ? longest : pm.offs[m + 1] - pm.offs[m];
         const int bx = (int)((longest + 255) / 256 < 1024 ? (longest + 255) / 256 : 1024);
         planner_tmax_kernel<<<dim3(bx > 0 ? bx : 1, n_models), 256, 0, s>>>(pm, residence_dev, tmax);
+        const int64_t n_blk = (n_req + kBlock - 1) / kBlock;
+        planner_block_tmax_kernel<<<(unsigned)((n_blk * 32 + 255) / 256), 256, 0, s>>>(residence_dev, n_req, blk_tmax);
     }
     planner_demand_kernel<<<(unsigned)((n_obs + 127) / 128), 128, 0, s>>>(pm, arrival_dev, prompt_tokens_dev,
-                                                                          output_tokens_dev, residence_dev, tmax, n_obs,
+                                                                          output_tokens_dev, residence_dev, tmax, blk_tmax, n_obs,
                                                                           t_obs_dev, k_pool_dev);
     if (cudaGetLastError() != cudaSuccess) return CP_ERR_CUDA;
     return CP_OK;
@@ -238,7 +273,7 @@ cp_status cp_planner_quantile(const double *values_dev, int64_t n, double q, dou
                               void *stream)
 {
     if (!values_dev || n < 1 || !(q > 0.0 && q <= 1.0) || !(page_bytes > 0.0)) return CP_ERR_INVALID_ARG;
-    if (!workspace_dev || workspace_bytes < kWorkspaceBytes || ((uintptr_t)workspace_dev & 15u)) return CP_ERR_WORKSPACE;
+    if (!workspace_dev || workspace_bytes < workspace_bytes_for(0) || ((uintptr_t)workspace_dev & 15u)) return CP_ERR_WORKSPACE;
     int64_t k = (int64_t)std::ceil(q * (double)n);        // rank of the order statistic, 1-based
     if (k < 1) k = 1;
     if (k > n) k = n;

@@ -259,8 +259,9 @@ def test_vmm_pool_fails_loudly_without_a_device():
 
 def test_planner_host_validation():
     """cp_planner_* argument checks happen before any CUDA call."""
-    wsb = cp.planner_workspace_bytes()
-    assert wsb >= 4 * 65536 and wsb % 16 == 0
+    wsb = cp.planner_workspace_bytes(1000)
+    assert wsb >= 4 * 65536 + 8 * 32 and wsb % 8 == 0
+    assert cp.planner_workspace_bytes(0) < wsb < cp.planner_workspace_bytes(100000)
     a = FAKE_ARENA
     for offs, kap in (([0, 5, 3], [1.0, 1.0]),          # offsets decrease
                       ([1, 5], [1.0]),                  # do not start at 0
@@ -273,7 +274,7 @@ def test_planner_host_validation():
         cp.planner_pool_demand(list(range(0, 5 * 66, 5)), [1.0] * 65, a, a, a, a, 4, a, a, a, wsb)   # > 64 models
     assert e.value.status == cp.CP_ERR_INVALID_ARG
     with pytest.raises(cp.CrossPoolError) as e:
-        cp.planner_pool_demand([0, 5], [1.0], a, a, a, a, 4, a, a, a, wsb - 16)
+        cp.planner_pool_demand([0, 5], [1.0], a, a, a, a, 4, a, a, a, cp.planner_workspace_bytes(0))   # sized for no trace
     assert e.value.status == cp.CP_ERR_WORKSPACE
     cp.planner_pool_demand([0, 5], [1.0], a, a, a, a, 0, None, None, a, wsb)        # nothing to do: OK, no CUDA
     for n, q in ((0, 0.5), (10, 0.0), (10, 1.5)):

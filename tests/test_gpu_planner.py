@@ -23,7 +23,7 @@ def gpu_demand(torch, tr, t_obs=None):
     t_obs = tr.t_obs if t_obs is None else np.ascontiguousarray(t_obs, dtype=np.float64)
     d = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (tr.arrival, tr.o_p, tr.o_d, tr.t_res, t_obs)]
     out = torch.full((t_obs.size,), float("nan"), dtype=torch.float64, device=dev)
-    wsb = cp.planner_workspace_bytes()
+    wsb = cp.planner_workspace_bytes(tr.n_requests)
     ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
     cp.planner_pool_demand(tr.offsets, tr.kappa, d[0], d[1], d[2], d[3], t_obs.size, d[4], out, ws, wsb,
                            int(torch.cuda.current_stream().cuda_stream))
