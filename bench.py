@@ -343,7 +343,7 @@ def main():
     # by chunk, page ids by arithmetic (no table) and with the identity table read anyway; and what the
     # slow path costs: mapping / unmapping the longest request's pages, against the software table's
     vmm = None
-    if rank == 0 and not args.no_vmm:
+    if rank == 0 and world == 1 and not args.no_vmm:
         dv = DeviceWorkload(w, dev, vmm=True)
         dv.pool.set_option(cp.CP_OPT_KERNEL, args.kernel)
         dv.ensure_workspace()
@@ -398,7 +398,7 @@ def main():
     # nothing is re-read from L2.  (a) one batch of all requests, L dependent layers; (b) one batch per
     # model, two in flight, served in turn (the paper's layer-wise state machine), L layers each.
     stages_leg = None
-    if rank == 0 and not args.no_stages and all(m.kind == 0 and m.head_dim_qk == 128 and m.head_dim_v == 128 for m in w.models):
+    if rank == 0 and world == 1 and not args.no_stages and all(m.kind == 0 and m.head_dim_qk == 128 and m.head_dim_v == 128 for m in w.models):
         L = args.stage_layers
         nreq = len(w.requests)
         arena_l = dw.arena.repeat(L)
@@ -514,7 +514,7 @@ def main():
 
     # ---------------- q_len > 1 (SURVEY §8(f) N4 variant): the same KV, four query tokens per request
     qlen_leg = None
-    if rank == 0 and not args.no_stages and all(m.kind == 0 and m.head_dim_qk == 128 and m.head_dim_v == 128 and
+    if rank == 0 and world == 1 and not args.no_stages and all(m.kind == 0 and m.head_dim_qk == 128 and m.head_dim_v == 128 and
                                                 m.n_q_heads // m.n_kv_heads * 4 <= 128 for m in w.models):
         ql = 4
         rows = w.out_rows() * ql
@@ -539,7 +539,7 @@ def main():
     # ---------------- KV-cache planner (Eq. (1)-(2)): pool demand at 100 000 observation
     # times of a two-hour synthetic trace of 8 cold models, then P95 / P99 and the page budgets
     planner = None
-    if rank == 0 and not args.no_planner:
+    if rank == 0 and world == 1 and not args.no_planner:
         from workloads.planner_traces import planner_trace
         tr = planner_trace(1)
         td = [torch.from_numpy(a).to(dev) for a in (tr.arrival, tr.o_p, tr.o_d, tr.t_res, tr.t_obs)]
