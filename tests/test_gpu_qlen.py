@@ -16,12 +16,12 @@ MQA = ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5)
 MHA = ModelCfg(KIND_KV, 8, 8, 128, 128, 128 ** -0.5)
 
 
-def run_qlen(torch, w, q_len, options=None, seed=0):
+def run_qlen(torch, w, q_len, options=None, seed=0, vmm=False):
     import paper_2606_24506_b200 as cp
     rng = np.random.default_rng(1000 + seed)
     qs = [W.f32_to_bf16(rng.standard_normal((q_len, w.models[r.model_id].n_q_heads, 128)).astype(np.float32))
           for r in w.requests]
-    dw = device_workload(w)
+    dw = device_workload(w, vmm=vmm)
     try:
         for k, v in (options or {}).items():
             dw.pool.set_option(k, v)
@@ -123,3 +123,11 @@ def test_qlen_argument_errors(torch_cuda):
         assert e.value.status == cp.CP_ERR_UNSUPPORTED
     finally:
         dw.close()
+
+
+def test_qlen_on_a_vmm_arena(torch_cuda):
+    import paper_2606_24506_b200 as cp
+    models, rm, rc, P, q_len = CASES[4]
+    w = W.small_workload(models, rm, rc, page_tokens=P, seed=504, keep_contiguous=False)
+    worst = run_qlen(torch_cuda, w, q_len, {cp.CP_OPT_MIN_TILE_PAGES: 1}, seed=4, vmm=True)
+    print(worst)

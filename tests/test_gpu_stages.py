@@ -268,3 +268,21 @@ def test_gated_launch_times_out_instead_of_hanging(torch_cuda):
         assert e.value.status == cp.CP_ERR_INVALID_ARG
     finally:
         dw.close()
+
+
+def test_stages_on_a_vmm_arena(torch_cuda):
+    """The multi-stage launch on the CUDA-VMM-backed arena (page ids by arithmetic, no table): same bits
+    as on the caller-owned arena."""
+    import paper_2606_24506_b200 as cp
+    w, order, stages, deps, q_in = build_case(BATCHES, 64, seed=31)
+    res = []
+    for vmm in (False, True):
+        dw = device_workload(w, vmm=vmm)
+        try:
+            dw.pool.set_option(cp.CP_OPT_MIN_TILE_PAGES, 1)
+            res.append(run_stages(torch_cuda, dw, w, stages, deps, q_in, 1.0, relaunch=False))
+        finally:
+            dw.close()
+    for a, b in zip(res[0], res[1]):
+        for (o, l), (o2, l2) in zip(a, b):
+            assert np.array_equal(o, o2) and np.array_equal(l, l2)
