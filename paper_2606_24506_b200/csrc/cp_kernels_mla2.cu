@@ -66,7 +66,8 @@ constexpr int M2_QBLK = 64 * 128;                   // one [64 x 64] K-major til
 constexpr int M2_KB_TMEM = 6;                       // query column blocks 0..5 live in TMEM (A operand, TS mode)
 constexpr int M2_Q_BYTES = (M2_KB - M2_KB_TMEM) * M2_QBLK;   // 24576: blocks 6..8 in shared memory
 constexpr int M2_P_BYTES = 64 * M2_TS * 2;          // 4096 per P buffer (two buffers)
-constexpr int M2_THREADS = 192;
+constexpr int M2_WARPS = 8;                         // producer, MMA issuer, 4 softmax warps, 2 that only help with the combine
+constexpr int M2_THREADS = 32 * M2_WARPS;
 constexpr int M2_SMEM_Q = 0;
 constexpr int M2_SMEM_STAGE = M2_Q_BYTES;
 constexpr int M2_SMEM_P = M2_SMEM_STAGE + M2_STAGES * M2_STAGE_BYTES;
@@ -288,6 +289,8 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             }
             gs += (uint32_t)n;
         }
+    } else if (warp >= 6) {
+        // ======================================================= combine helpers: nothing to do until the combine
     } else {
         // =========================================================== softmax warps
         // thread = TMEM lane L: head (rank * 64 + L % 64), token half L / 64 of every slice
@@ -490,13 +493,13 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             }
         }
     }
-    // ---- LSE combine (step a4): warp-sized units, statically assigned to ALL six warps of every CTA.
+    // ---- LSE combine (step a4): warp-sized units, statically assigned to ALL warps of every CTA.
     // The barrier orders it after this CTA's last tile (every slice consumed, every MMA complete),
     // so the slice stages can serve as the warps' scratch.
     __syncthreads();
     {
         float *wsm = reinterpret_cast<float *>(smem + M2_SMEM_STAGE) + warp * kMaxSplits;
-        combine_units<16>(p, blockIdx.x * 6 + warp, gridDim.x * 6, wsm, lane);
+        combine_units<16>(p, blockIdx.x * M2_WARPS + warp, gridDim.x * M2_WARPS, wsm, lane);
         M2_STAMP(22, tid == 64);
     }
     tc_fence_before();
