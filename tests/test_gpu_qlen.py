@@ -131,3 +131,10 @@ def test_qlen_on_a_vmm_arena(torch_cuda):
     w = W.small_workload(models, rm, rc, page_tokens=P, seed=504, keep_contiguous=False)
     worst = run_qlen(torch_cuda, w, q_len, {cp.CP_OPT_MIN_TILE_PAGES: 1}, seed=4, vmm=True)
     print(worst)
+
+
+def test_qlen_full_size_cfg2(torch_cuda):
+    """Full size, default options (what bench.py's `qlen` leg times): BASELINE cfg2 with four query tokens
+    per request."""
+    worst = run_qlen(torch_cuda, W.config(2), 4, seed=77)
+    print("cfg2 q_len 4: %s" % worst)

@@ -286,3 +286,23 @@ def test_stages_on_a_vmm_arena(torch_cuda):
     for a, b in zip(res[0], res[1]):
         for (o, l), (o2, l2) in zip(a, b):
             assert np.array_equal(o, o2) and np.array_equal(l, l2)
+
+
+def test_stages_full_size_two_layers_of_cfg2(torch_cuda):
+    """Full size, default options (the configuration bench.py's `stages` leg times): the eight requests of
+    BASELINE cfg2 (four GQA models, 4 k - 32 k contexts) as two dependent layers, each layer with its own KV."""
+    _, rm, rc = W.config2_meta()
+    models = [ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5) for _ in range(4)]
+    n = len(rm)
+    w = W.small_workload(models, rm + rm, rc + rc, page_tokens=64, seed=2450602, keep_contiguous=False, extra_pages=64)
+    stages, deps = [list(range(n)), list(range(n, 2 * n))], [-1, 0]
+    rng = np.random.default_rng(11)
+    q_in = [[W.f32_to_bf16(rng.standard_normal((32, 128)).astype(np.float32)) for _ in st] for st in stages]
+    ref = oracle.decode_stages(w, stages, deps, q_in, alpha=1.0)
+    dw = device_workload(w)
+    try:
+        got = run_stages(torch_cuda, dw, w, stages, deps, q_in, 1.0)
+    finally:
+        dw.close()
+    for s in range(2):
+        print("layer %d: %s" % (s, compare_stage(got[s], ref[s], deps[s] >= 0, "cfg2 layer %d" % s)))
