@@ -92,9 +92,12 @@ enum {
     CP_OPT_NUM_CTAS = 1,     /* persistent grid size; 0 = number of SMs of the device       */
     CP_OPT_WAVES_X16 = 2,    /* target tiles per CTA, in 1/16 units (default 16 = 1.0)      */
     CP_OPT_MIN_TILE_PAGES = 3, /* lower bound on pages per tile (default 2)                  */
-    CP_OPT_VMM_TABLE = 4     /* pool from cp_pool_create_vmm only: 1 = the decode kernels read the
+    CP_OPT_VMM_TABLE = 4,    /* pool from cp_pool_create_vmm only: 1 = the decode kernels read the
                                 software page table anyway (it holds the same ids; for measuring
                                 what the table costs), 0 (default) = page ids by arithmetic   */
+    CP_OPT_HOST_ZERO_COPY = 5 /* cp_decode_attention_host: 1 (default) = pinned, device-mapped host
+                                buffers are accessed in place (O / LSE written once; Q only when
+                                its re-reads by the tiles stay under 1 MB), 0 = always staged  */
 };
 
 /*
@@ -253,7 +256,11 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
 /*
  * cp_decode_attention_host -- the same step with HOST query / result buffers: copies q
  * host->device, runs cp_decode_attention, copies O and LSE device->host and synchronises
- * `stream`.  The KV arena stays resident on the device (it is the cache).  The staging
+ * `stream`.  Host buffers that are pinned and device-mapped (cudaHostAlloc / cudaHostRegister) are
+ * accessed by the kernel in place instead (CP_OPT_HOST_ZERO_COPY): the same bytes cross the bus, without
+ * the separate copy operations before and after the kernel.  Otherwise O and LSE come back in one
+ * copy when lse_host directly follows out_host in memory, in two when not.
+ * The KV arena stays resident on the device (it is the cache).  The staging
  * copies of q / O / LSE live at the front of workspace_dev: it must hold
  * cp_decode_workspace_bytes_host(...) bytes.
  */

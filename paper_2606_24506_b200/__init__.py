@@ -35,6 +35,7 @@ CP_OPT_NUM_CTAS = 1
 CP_OPT_WAVES_X16 = 2
 CP_OPT_MIN_TILE_PAGES = 3
 CP_OPT_VMM_TABLE = 4
+CP_OPT_HOST_ZERO_COPY = 5
 
 
 class cp_model_cfg(ctypes.Structure):

@@ -90,6 +90,9 @@ struct cp_pool {
     VmmArena *vmm = nullptr;
     uint32_t slot_pages = 0;
     int opt_vmm_table = 0;               // 1: decode kernels read the (identity) page table anyway
+    int opt_host_zero_copy = 1;          // cp_decode_attention_host: access pinned host buffers in place
+    const void *zc_host[3] = {nullptr, nullptr, nullptr};   // last q / out / lse host pointers looked up ...
+    void *zc_dev[3] = {nullptr, nullptr, nullptr};           // ... and their device aliases (nullptr: not mapped)
 
     // options
     int opt_kernel = 0, opt_num_ctas = 0, opt_waves_x16 = 16, opt_min_tile_pages = 2;
@@ -716,6 +719,9 @@ cp_status cp_pool_set_option(cp_pool *pool, int32_t key, int64_t value)
     case CP_OPT_VMM_TABLE:
         if (value < 0 || value > 1) return CP_ERR_INVALID_ARG;
         pool->opt_vmm_table = (int)value; break;
+    case CP_OPT_HOST_ZERO_COPY:
+        if (value < 0 || value > 1) return CP_ERR_INVALID_ARG;
+        pool->opt_host_zero_copy = (int)value; break;
     default: return CP_ERR_INVALID_ARG;
     }
     pool->plan_valid = false;
@@ -1257,15 +1263,49 @@ cp_status cp_decode_attention_host(cp_pool *pool, const int32_t *request_ids_hos
     cudaStream_t s = (cudaStream_t)stream;
     uint8_t *w = (uint8_t *)workspace_dev;
     void *q_dev = w;                      w += align256((uint64_t)pool->q_elems * 2);
-    float *o_dev = (float *)w;            w += align256((uint64_t)pool->out_floats * 4);
-    float *l_dev = (float *)w;            w += align256((uint64_t)pool->lse_floats * 4);
+    // O and LSE staging back to back, so that one copy serves a caller whose two host buffers are adjacent
+    float *o_dev = (float *)w;
+    float *l_dev = o_dev + pool->out_floats;
+    w += align256((uint64_t)pool->out_floats * 4) + align256((uint64_t)pool->lse_floats * 4);
     const uint64_t rest = workspace_bytes - (uint64_t)(w - (uint8_t *)workspace_dev);
-    if (cudaMemcpyAsync(q_dev, q_host, (size_t)pool->q_elems * 2, cudaMemcpyHostToDevice, s) != cudaSuccess)
+    // Pinned (mapped) host buffers are accessed in place where that moves fewer bytes more directly:
+    // results are written exactly once, so O / LSE always qualify; Q is re-read by every tile of its
+    // group, so only when those re-reads stay small (K/V kernel, a few hundred KB per step).
+    void *zq = nullptr, *zo = nullptr, *zl = nullptr;
+    if (pool->opt_host_zero_copy) {
+        const void *hp[3] = {q_host, out_host, lse_host};
+        for (int i = 0; i < 3; ++i) {
+            if (pool->zc_host[i] != hp[i]) {
+                cudaPointerAttributes a;
+                pool->zc_host[i] = hp[i];
+                pool->zc_dev[i] = nullptr;
+                if (cudaPointerGetAttributes(&a, hp[i]) == cudaSuccess && a.type == cudaMemoryTypeHost && a.devicePointer &&
+                    ((uintptr_t)a.devicePointer & (i == 2 ? 3u : 15u)) == 0)
+                    pool->zc_dev[i] = a.devicePointer;
+                cudaGetLastError();
+            }
+        }
+        const KindPlan &kv = pool->plan[CP_KIND_KV];
+        uint64_t q_reread = 0;
+        for (const TileRec &r : kv.tile_recs) q_reread += (uint64_t)r.gsize * 256u;
+        if (pool->plan[CP_KIND_MLA].tiles.empty() && kv.all_fast && pool->opt_kernel != 1 && pool->kv_tmap_ok &&
+            q_reread <= (1u << 20))
+            zq = pool->zc_dev[0];
+        if (pool->zc_dev[1] && pool->zc_dev[2]) { zo = pool->zc_dev[1]; zl = pool->zc_dev[2]; }
+    }
+    if (!zq && cudaMemcpyAsync(q_dev, q_host, (size_t)pool->q_elems * 2, cudaMemcpyHostToDevice, s) != cudaSuccess)
         return CP_ERR_CUDA;
-    st = cp_decode_attention(pool, request_ids_host, n_requests, q_dev, o_dev, l_dev, w, rest, s);
+    st = cp_decode_attention(pool, request_ids_host, n_requests, zq ? zq : q_dev, zo ? (float *)zo : o_dev,
+                             zl ? (float *)zl : l_dev, w, rest, s);
     if (st != CP_OK) return st;
-    if (cudaMemcpyAsync(out_host, o_dev, (size_t)pool->out_floats * 4, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
-        cudaMemcpyAsync(lse_host, l_dev, (size_t)pool->lse_floats * 4, cudaMemcpyDeviceToHost, s) != cudaSuccess)
+    if (zo) {
+        // written in place by the kernel; visible to the host after the synchronisation below
+    } else if (lse_host == out_host + pool->out_floats) {
+        if (cudaMemcpyAsync(out_host, o_dev, (size_t)(pool->out_floats + pool->lse_floats) * 4, cudaMemcpyDeviceToHost, s) !=
+            cudaSuccess)
+            return CP_ERR_CUDA;
+    } else if (cudaMemcpyAsync(out_host, o_dev, (size_t)pool->out_floats * 4, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+               cudaMemcpyAsync(lse_host, l_dev, (size_t)pool->lse_floats * 4, cudaMemcpyDeviceToHost, s) != cudaSuccess)
         return CP_ERR_CUDA;
     if (cudaStreamSynchronize(s) != cudaSuccess) return CP_ERR_CUDA;
     return CP_OK;

@@ -425,6 +425,23 @@ def test_host_buffer_entry_point_matches_device_path(torch_cuda):
     o = np.concatenate([x[0].reshape(-1) for x in dev])
     l = np.concatenate([x[1].reshape(-1) for x in dev])
     assert np.array_equal(o_host.numpy(), o) and np.array_equal(l_host.numpy(), l)
+    # adjacent host buffers (LSE directly after O): the one-copy path gives the same bytes
+    ol = torch.full((dw.out.numel() + dw.lse.numel() + 8,), float("nan"), dtype=torch.float32).pin_memory()
+    dw.pool.decode_attention_host(dw.ids, q_host, ol[:dw.out.numel()], ol[dw.out.numel():], ws, need, dw.stream())
+    assert np.array_equal(ol[:dw.out.numel()].numpy(), o)
+    assert np.array_equal(ol[dw.out.numel():dw.out.numel() + dw.lse.numel()].numpy(), l)
+    assert np.isnan(ol[dw.out.numel() + dw.lse.numel():].numpy()).all()          # nothing written past the end
+    # the same with the in-place access of pinned buffers switched off, and with pageable host memory
+    import paper_2606_24506_b200 as cp
+    for zero_copy, pinned in ((0, True), (1, False), (1, True)):
+        dw.pool.set_option(cp.CP_OPT_HOST_ZERO_COPY, zero_copy)
+        oh = torch.full((dw.out.numel(),), float("nan"), dtype=torch.float32)
+        lh = torch.full((dw.lse.numel(),), float("nan"), dtype=torch.float32)
+        qh = torch.from_numpy(w.q_packed().view(np.int16).copy())
+        if pinned:
+            oh, lh, qh = oh.pin_memory(), lh.pin_memory(), qh.pin_memory()
+        dw.pool.decode_attention_host(dw.ids, qh, oh, lh, ws, need, dw.stream())
+        assert np.array_equal(oh.numpy(), o) and np.array_equal(lh.numpy(), l), (zero_copy, pinned)
     dw.close()
 
 
