@@ -85,19 +85,24 @@ typedef struct {
 
 /* Tunables (cp_pool_set_option). */
 enum {
-    CP_OPT_KERNEL = 0,       /* 0 = auto (tensor-core kernels where the shape allows; MLA on CTA
-                                    pairs, tcgen05 cta_group::2),
+    CP_OPT_KERNEL = 0,       /* 0 = auto (tensor-core kernels where the shape allows: MQA/GQA groups of up
+                                    to 32 rows on the tcgen05 tokens-on-M kernel, MLA on CTA pairs,
+                                    tcgen05 cta_group::2),
                                 1 = force the generic SIMT kernel (any supported shape),
-                                2 = as 0, but MLA on the single-CTA tcgen05 kernel           */
+                                2 = as 0, but MLA on the single-CTA tcgen05 kernel,
+                                3 = as 0, but MQA/GQA on the warp-MMA (mma.sync) kernel          */
     CP_OPT_NUM_CTAS = 1,     /* persistent grid size; 0 = number of SMs of the device       */
     CP_OPT_WAVES_X16 = 2,    /* target tiles per CTA, in 1/16 units (default 16 = 1.0)      */
     CP_OPT_MIN_TILE_PAGES = 3, /* lower bound on pages per tile (default 2)                  */
     CP_OPT_VMM_TABLE = 4,    /* pool from cp_pool_create_vmm only: 1 = the decode kernels read the
                                 software page table anyway (it holds the same ids; for measuring
                                 what the table costs), 0 (default) = page ids by arithmetic   */
-    CP_OPT_HOST_ZERO_COPY = 5 /* cp_decode_attention_host: 1 (default) = pinned, device-mapped host
+    CP_OPT_HOST_ZERO_COPY = 5, /* cp_decode_attention_host: 1 (default) = pinned, device-mapped host
                                 buffers are accessed in place (O / LSE written once; Q only when
                                 its re-reads by the tiles stay under 1 MB), 0 = always staged  */
+    CP_OPT_TIMELINE = 6      /* 1 = the next cp_decode_attention launches record per-CTA globaltimer
+                                stamps (cp_pool_read_timeline); 0 (default) = off.  Measurement aid of
+                                bench.py --probe timeline; kernels that do not stamp leave zeros.  */
 };
 
 /*
@@ -359,6 +364,15 @@ cp_status cp_decode_plan(cp_pool *pool, const int32_t *request_ids_host, int32_t
  * launched by the library, work-list (re)builds, host->device metadata bytes. */
 cp_status cp_pool_counters(const cp_pool *pool, uint64_t *kernel_launches,
                            uint64_t *plan_builds, uint64_t *metadata_h2d_bytes);
+
+/* cp_pool_read_timeline -- measurement aid (`bench.py --probe timeline`): with CP_OPT_TIMELINE = 1
+ * the persistent CTAs of the MQA/GQA tcgen05 kernel stamp %globaltimer (ns) at fixed points of their life:
+ *   slot 0 kernel entry, 1 first tile descriptor at the MMA warp, 2 first slice landed, 3 producer issued
+ *   its last page, 4 softmax of the last slice of a tile done, 5 tile published, 6 LSE combine begins,
+ *   7 combine done; slots 8..15 unused (0 = not stamped).
+ * Synchronises the device and copies the stamps of the last launch of the pool: stamps_out_host holds
+ * cap_ctas x 16 uint64; n_ctas_out receives the number of CTA rows available (the SM count). */
+cp_status cp_pool_read_timeline(cp_pool *pool, uint64_t *stamps_out_host, int32_t cap_ctas, int32_t *n_ctas_out);
 
 /*
  * KV-cache planner: "The planner uses per-model prompt, output, and service-time

@@ -36,6 +36,8 @@ CP_OPT_WAVES_X16 = 2
 CP_OPT_MIN_TILE_PAGES = 3
 CP_OPT_VMM_TABLE = 4
 CP_OPT_HOST_ZERO_COPY = 5
+CP_OPT_TIMELINE = 6
+TIMELINE_SLOTS = 16
 
 
 class cp_model_cfg(ctypes.Structure):
@@ -99,6 +101,7 @@ def load_library():
         "cp_decode_stages_gate_status": (i32, [vp, vp, i32p]),
         "cp_decode_plan": (i32, [vp, i32p, i32, ctypes.POINTER(cp_tile_info), i32, i32p, i32p]),
         "cp_pool_counters": (i32, [vp, u64p, u64p, u64p]),
+        "cp_pool_read_timeline": (i32, [vp, u64p, i32, i32p]),
         "cp_status_string": (ctypes.c_char_p, [i32]),
         "cp_planner_workspace_bytes": (u64, [ctypes.c_int64]),
         "cp_planner_pool_demand": (i32, [i32, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_double),
@@ -120,7 +123,7 @@ EXPORTED = ["cp_pool_create", "cp_pool_create_vmm", "cp_pool_vmm_info", "cp_pool
             "cp_decode_workspace_bytes", "cp_decode_attention", "cp_decode_workspace_bytes_host",
             "cp_decode_attention_host", "cp_decode_workspace_bytes_qlen", "cp_decode_attention_qlen",
             "cp_decode_stages_workspace_bytes", "cp_decode_attention_stages", "cp_decode_attention_stages_gated",
-            "cp_decode_stages_gate_status", "cp_decode_plan", "cp_pool_counters", "cp_status_string",
+            "cp_decode_stages_gate_status", "cp_decode_plan", "cp_pool_counters", "cp_pool_read_timeline", "cp_status_string",
             "cp_planner_workspace_bytes", "cp_planner_pool_demand", "cp_planner_quantile"]
 
 
@@ -245,6 +248,15 @@ class Pool:
         _check(self._L.cp_pool_counters(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)),
                "cp_pool_counters")
         return {"kernel_launches": a.value, "plan_builds": b.value, "metadata_h2d_bytes": c.value}
+
+    def read_timeline(self) -> np.ndarray:
+        """Per-CTA globaltimer stamps (ns) of the pool's last decode launch: uint64 [n_ctas][16]."""
+        n = ctypes.c_int32()
+        _check(self._L.cp_pool_read_timeline(self._h, None, 0, ctypes.byref(n)), "cp_pool_read_timeline")
+        out = np.zeros((max(n.value, 1), TIMELINE_SLOTS), dtype=np.uint64)
+        _check(self._L.cp_pool_read_timeline(self._h, out.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)), n.value,
+                                             ctypes.byref(n)), "cp_pool_read_timeline")
+        return out[:n.value]
 
     # --- several query tokens per request (causal over the context's last q_len tokens)
     def decode_workspace_bytes_qlen(self, request_ids, q_len: int) -> int:

@@ -24,7 +24,8 @@ __host__ __device__ inline int64_t part_group_floats(int g, int ns, int dv)
 constexpr int kMaxDk = 576;
 constexpr int kMaxDv = 512;
 constexpr int kMaxSplits = 512;
-constexpr int kCounterStride = 32;   // ints between group counters: one 128-byte line each (no false sharing under polling)      // KV splits per group (bounds the combine's shared memory)
+constexpr int kCounterStride = 32;   // ints between group counters: one 128-byte line each (no false sharing under polling)
+constexpr int kTimelineSlots = 16;   // globaltimer stamps per CTA (CP_OPT_TIMELINE)
 
 // Device copy of a model description (cp_model_cfg plus derived values).
 struct DevModel {
@@ -149,7 +150,8 @@ struct DecodeParams {
     int32_t *gate_flag;            // set to 1 if a poll of the doorbell timed out
     uint32_t gate_timeout_us;
     int32_t *stage_done;           // [n_stages] completion counters, kCounterStride apart
-    int32_t n_stages;       // the other counter set ([32] scheduler + group counters): cleared by this launch
+    int32_t n_stages;
+    unsigned long long *timeline;  // CP_OPT_TIMELINE: [grid][kTimelineSlots] globaltimer stamps, or nullptr
 };
 
 }  // namespace cp

@@ -25,6 +25,12 @@ bool make_arena_tensor_map(void *out_map, const void *arena, uint64_t total_rows
 cudaError_t launch_decode_kv(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas,
                              cudaStream_t stream);
 
+// tcgen05 MQA/GQA path, tokens on the MMA M dimension (cp_kernels_kvt.cu)
+bool kvt_supported(int page_tokens);
+int kvt_pad_rows(int max_group);      // N of the instantiation for groups of up to max_group rows, 0 = none
+cudaError_t launch_decode_kvt(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas, int max_group,
+                              cudaStream_t stream);
+
 // tcgen05 MLA path (cp_kernels_mla.cu)
 bool mla_fast_supported(int page_tokens, uint32_t page_bytes);
 bool make_mla_tensor_map(void *out_map, const void *arena, uint64_t total_rows);

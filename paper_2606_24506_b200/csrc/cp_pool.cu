@@ -62,6 +62,7 @@ struct KindPlan {
     int max_dk = 0, max_dv = 0;
     int max_group = 0;
     bool all_fast = false;           // every group of this kind runs on the tensor-core kernel
+    bool use_kvt = false;            // KV kind: the tcgen05 tokens-on-M kernel (else the mma.sync kernel)
     bool uploaded = false;
     int counter_set = 0;             // scheduler counter set the next launch uses (alternates)
     int extra_counters = 0;          // multi-stage plans: one completion counter per stage after the groups'
@@ -99,6 +100,10 @@ struct cp_pool {
 
     // query tokens per request of the call in progress (cp_decode_attention_qlen), and of the cached plan
     int qlen = 1, plan_qlen = 1;
+    bool plan_for_stages = false;        // build_plan is called for a multi-stage work list (mma.sync kernel)
+    int opt_timeline = 0;                // CP_OPT_TIMELINE: per-CTA globaltimer stamps of the next decode launches
+    int timeline_ctas = 0;               // grid size of the last launch that wrote stamps
+    int device = -1;                     // device of the arena (the compute calls require it to be current)
 
     // plan cache
     std::vector<int32_t> plan_batch;
@@ -112,7 +117,7 @@ struct cp_pool {
     // device side (lazy)
     bool dev_ready = false;
     int n_sm = 148;
-    DevBuf d_page_table, d_ctx, d_models, d_append;
+    DevBuf d_page_table, d_ctx, d_models, d_append, d_timeline;
     alignas(64) unsigned char kv_tmap[128];   // CUtensorMap of the arena for the MQA/GQA kernel
     bool kv_tmap_ok = false;
     alignas(64) unsigned char mla_tmap[128];  // CUtensorMap of the arena for the MLA kernel
@@ -201,6 +206,19 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             }
         const int64_t target_tiles =
             std::max<int64_t>(1, (int64_t)n_ctas * pool->opt_waves_x16 / 16 / (mla_fast ? 2 : 1));
+        // which K/V kernel will run this plan: it fixes how many arrivals a finished tile makes on its
+        // group's counter (tcgen05 tokens-on-M kernel: its 4 softmax warps; mma.sync kernel: one per M tile)
+        kp.all_fast = k == CP_KIND_KV ? true : mla_fast;
+        kp.max_group = 0;
+        for (int b = 0; b < n; ++b) {
+            const cp_model_cfg &m = pool->models[pool->reqs[ids[b]].model];
+            if (m.kind != k) continue;
+            const int g = m.n_q_heads / m.n_kv_heads * pool->qlen;
+            if (k == CP_KIND_KV && !(m.head_dim_qk == 128 && m.head_dim_v == 128 && g <= 128)) kp.all_fast = false;
+            kp.max_group = std::max(kp.max_group, g);
+        }
+        kp.use_kvt = k == CP_KIND_KV && kp.all_fast && (pool->opt_kernel == 0 || pool->opt_kernel == 2) &&
+                     pool->qlen == 1 && !pool->plan_for_stages && kvt_supported(P) && kvt_pad_rows(kp.max_group) > 0;
         auto tiles_for = [&](int64_t len) {
             int64_t t = 0;
             for (int b = 0; b < n; ++b) {
@@ -210,6 +228,7 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             }
             return t;
         };
+        // smallest tile length L (pages) for which the batch yields at most target_tiles tiles
         // (searched in [L_bal, 2 L_bal]; a batch of many short requests cannot meet the target at
         // all -- every group is at least one tile -- and then keeps the balanced length L_bal)
         const int64_t L_bal = std::max<int64_t>((total_pages[k] + target_tiles - 1) / target_tiles,
@@ -223,7 +242,38 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             }
             L = lo;
         }
-        kp.all_fast = k == CP_KIND_KV ? true : mla_fast;
+        // splits per request: ceil(pages / L), then the tiles still missing from the target go, one at a
+        // time, to the request whose tiles are longest (so that with waves = w every persistent CTA gets
+        // exactly w near-equal tiles whenever the groups allow it; one tile more on a few CTAs would cost
+        // a whole extra tile time at the end).  Depends on the context lengths only (deterministic).
+        std::vector<int> req_splits(n, 0);
+        {
+            int64_t have = 0;
+            for (int b = 0; b < n; ++b) {
+                const Request &r = pool->reqs[ids[b]];
+                const cp_model_cfg &m = pool->models[r.model];
+                if (m.kind != k) continue;
+                const int n_lp = ceil_div(r.ctx, P);
+                req_splits[b] = (int)std::min<int64_t>((n_lp + L - 1) / L, kMaxSplits);
+                have += (int64_t)req_splits[b] * m.n_kv_heads;
+            }
+            while (have < target_tiles) {
+                int best = -1;
+                double best_len = 0.0;
+                for (int b = 0; b < n; ++b) {
+                    const Request &r = pool->reqs[ids[b]];
+                    const cp_model_cfg &m = pool->models[r.model];
+                    if (m.kind != k || have + m.n_kv_heads > target_tiles) continue;
+                    const int n_lp = ceil_div(r.ctx, P);
+                    if (req_splits[b] + 1 > kMaxSplits || n_lp / (req_splits[b] + 1) < pool->opt_min_tile_pages) continue;
+                    const double len = (double)n_lp / req_splits[b];
+                    if (len > best_len) { best_len = len; best = b; }
+                }
+                if (best < 0) break;
+                req_splits[best] += 1;
+                have += pool->models[pool->reqs[ids[best]].model].n_kv_heads;
+            }
+        }
         for (int b = 0; b < n; ++b) {
             const Request &r = pool->reqs[ids[b]];
             const cp_model_cfg &m = pool->models[r.model];
@@ -231,14 +281,10 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             const int hpk = m.n_q_heads / m.n_kv_heads;       // query heads per kv head
             const int g = hpk * pool->qlen;                   // rows of a group: (query token, head), token-major
             const int n_lp = ceil_div(r.ctx, P);
-            int ns = (int)((n_lp + L - 1) / L);
-            ns = std::min(ns, kMaxSplits);                // bounds the combine's shared memory
-            if (k == CP_KIND_KV && !(m.head_dim_qk == 128 && m.head_dim_v == 128 && g <= 128))
-                kp.all_fast = false;
+            const int ns = req_splits[b];
             kp.max_splits = std::max(kp.max_splits, ns);
             kp.max_dk = std::max(kp.max_dk, m.head_dim_qk);
             kp.max_dv = std::max(kp.max_dv, m.head_dim_v);
-            kp.max_group = std::max(kp.max_group, g);
             for (int c = 0; c < m.n_kv_heads; ++c) {
                 Group gr;
                 gr.req = ids[b]; gr.model = r.model; gr.kv_head = c; gr.n_splits = ns;
@@ -284,7 +330,9 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
                             cu.split_stride = m.head_dim_v;
                             cu.n_splits = ns;
                             cu.zl_log2 = zl;
-                            cu.want = ns * (k == CP_KIND_KV ? mtp : 8);   // MLA: 4 softmax warps x 2 value halves
+                            // arrivals per finished tile: K/V tcgen05 kernel 4 (softmax warps), K/V mma.sync kernel one
+                            // per padded M tile, MLA 8 (4 softmax warps x 2 value halves / CTAs)
+                            cu.want = ns * (k == CP_KIND_KV ? (kp.use_kvt ? 4 : mtp) : 8);
                             cu.group = gi;
                             kp.cunits.push_back(cu);
                         }
@@ -353,17 +401,24 @@ void ensure_plan(cp_pool *pool, const int32_t *ids, int n)
 // ------------------------------------------------------------------------ device state
 cp_status ensure_device(cp_pool *pool)
 {
-    if (pool->dev_ready) return CP_OK;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
-    cudaPointerAttributes attr;
-    if (cudaPointerGetAttributes(&attr, pool->arena) != cudaSuccess ||
-        attr.type != cudaMemoryTypeDevice) {
-        cudaGetLastError();
-        return CP_ERR_INVALID_ARG;          // arena is not device memory
+    if (pool->dev_ready) return dev == pool->device ? CP_OK : CP_ERR_INVALID_ARG;   // the arena's device must be current
+    int adev = dev;
+    if (pool->vmm) {
+        // the base of a reserved range has no backing until slot 0 is mapped: take the device from the arena object
+        adev = pool->vmm->device;
+    } else {
+        cudaPointerAttributes attr;
+        if (cudaPointerGetAttributes(&attr, pool->arena) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+            cudaGetLastError();
+            return CP_ERR_INVALID_ARG;          // arena is not device memory
+        }
+        adev = attr.device;
     }
+    if (adev != dev) return CP_ERR_INVALID_ARG; // metadata, streams and launches all live on the arena's device
     int sms = 0;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, attr.device) != cudaSuccess)
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, adev) != cudaSuccess)
         return CP_ERR_CUDA;
     if (pool->d_page_table.ensure((size_t)pool->max_requests * pool->max_ppr * 4) != cudaSuccess ||
         pool->d_ctx.ensure((size_t)pool->max_requests * 4) != cudaSuccess ||
@@ -384,24 +439,28 @@ cp_status ensure_device(cp_pool *pool)
         return CP_ERR_CUDA;
     if (cudaMemset(pool->d_ctx.ptr, 0, (size_t)pool->max_requests * 4) != cudaSuccess)
         return CP_ERR_CUDA;
+    // TMA row coordinates are signed 32-bit: a tensor map is only used while every row index fits (a
+    // CUDA-VMM pool reserves virtual space only and can exceed that; it then runs on the generic kernel)
     pool->kv_tmap_ok = false;
     if (kv_fast_supported((int)pool->P) && pool->page_bytes % 256 == 0 &&
         pool->page_bytes >= pool->P * 512u) {
         const uint64_t rows = (uint64_t)pool->num_pages * (pool->page_bytes / 256);
-        pool->kv_tmap_ok = rows < (1ull << 32) &&
+        pool->kv_tmap_ok = rows < (1ull << 31) &&
                            make_arena_tensor_map(pool->kv_tmap, pool->arena, rows, 128, 64, pool->P);
     }
     pool->mla_tmap_ok = false;
     pool->mla2_tmap_ok = false;
     if (mla_fast_supported((int)pool->P, pool->page_bytes)) {
         const uint64_t rows = (uint64_t)pool->num_pages * (pool->page_bytes / 1152);
-        pool->mla_tmap_ok = rows < (1ull << 32) && make_mla_tensor_map(pool->mla_tmap, pool->arena, rows);
-        pool->mla2_tmap_ok = rows < (1ull << 32) &&
+        pool->mla_tmap_ok = rows < (1ull << 31) && make_mla_tensor_map(pool->mla_tmap, pool->arena, rows);
+        pool->mla2_tmap_ok = rows < (1ull << 31) &&
                              make_mla2_tensor_maps(pool->mla2_tmap9, pool->mla2_tmap2, pool->arena, rows);
     }
     pool->n_sm = sms;
+    pool->device = adev;
     pool->dev_ready = true;
     pool->plan_valid = false;               // the SM count feeds the planner
+    pool->splan.valid = false;
     // everything mapped so far is dirty
     for (auto &r : pool->reqs) r.uploaded = 0;
     pool->ctx_dirty_lo = 0; pool->ctx_dirty_hi = pool->max_requests - 1;
@@ -572,7 +631,7 @@ cp_status cp_pool_free(cp_pool *pool)
     if (!pool) return CP_OK;
     if (pool->dev_ready || pool->vmm) cudaDeviceSynchronize();
     if (pool->vmm) { vmm_destroy(pool->vmm); pool->vmm = nullptr; }
-    pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release(); pool->d_append.release();
+    pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release(); pool->d_append.release(); pool->d_timeline.release();
     for (int k = 0; k < 2; ++k) {
         pool->plan[k].d_groups.release(); pool->plan[k].d_tiles.release();
         pool->plan[k].d_combines.release(); pool->plan[k].d_cunits.release(); pool->plan[k].d_tile_recs.release();
@@ -705,7 +764,7 @@ cp_status cp_pool_set_option(cp_pool *pool, int32_t key, int64_t value)
     if (!pool) return CP_ERR_INVALID_ARG;
     switch (key) {
     case CP_OPT_KERNEL:
-        if (value < 0 || value > 2) return CP_ERR_INVALID_ARG;
+        if (value < 0 || value > 3) return CP_ERR_INVALID_ARG;
         pool->opt_kernel = (int)value; break;
     case CP_OPT_NUM_CTAS:
         if (value < 0 || value > 65536) return CP_ERR_INVALID_ARG;
@@ -722,6 +781,9 @@ cp_status cp_pool_set_option(cp_pool *pool, int32_t key, int64_t value)
     case CP_OPT_HOST_ZERO_COPY:
         if (value < 0 || value > 1) return CP_ERR_INVALID_ARG;
         pool->opt_host_zero_copy = (int)value; break;
+    case CP_OPT_TIMELINE:
+        if (value < 0 || value > 1) return CP_ERR_INVALID_ARG;
+        pool->opt_timeline = (int)value; return CP_OK;      // no effect on the plan
     default: return CP_ERR_INVALID_ARG;
     }
     pool->plan_valid = false;
@@ -736,6 +798,22 @@ cp_status cp_pool_counters(const cp_pool *pool, uint64_t *kernel_launches, uint6
     if (kernel_launches) *kernel_launches = pool->n_launches;
     if (plan_builds) *plan_builds = pool->n_plan_builds;
     if (metadata_h2d_bytes) *metadata_h2d_bytes = pool->n_h2d_bytes;
+    return CP_OK;
+}
+
+cp_status cp_pool_read_timeline(cp_pool *pool, uint64_t *stamps_out_host, int32_t cap_ctas, int32_t *n_ctas_out)
+{
+    if (!pool || cap_ctas < 0 || (cap_ctas > 0 && !stamps_out_host)) return CP_ERR_INVALID_ARG;
+    if (n_ctas_out) *n_ctas_out = 0;
+    if (!pool->d_timeline.ptr) return CP_OK;
+    if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+    const int n = std::min<int>(cap_ctas, pool->n_sm);
+    if (n > 0 && cudaMemcpy(stamps_out_host, pool->d_timeline.ptr, (size_t)n * kTimelineSlots * sizeof(uint64_t),
+                            cudaMemcpyDeviceToHost) != cudaSuccess) {
+        cudaGetLastError();
+        return CP_ERR_CUDA;
+    }
+    if (n_ctas_out) *n_ctas_out = pool->n_sm;
     return CP_OK;
 }
 
@@ -925,10 +1003,25 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.reset_counters = (int32_t *)kp.d_counters.ptr + (1 - kp.counter_set) * set_ints;
         prm.stages = nullptr; prm.stage_done = nullptr; prm.n_stages = 0; prm.q_len = pool->qlen;
         prm.published = nullptr; prm.gate_flag = nullptr; prm.gate_timeout_us = 0;
+        prm.timeline = nullptr;
+        if (pool->opt_timeline) {
+            const size_t tb = (size_t)pool->n_sm * kTimelineSlots * sizeof(unsigned long long);
+            if (pool->d_timeline.ensure(tb) != cudaSuccess || cudaMemsetAsync(pool->d_timeline.ptr, 0, tb, s) != cudaSuccess) {
+                cudaGetLastError();
+                return CP_ERR_CUDA;
+            }
+            prm.timeline = (unsigned long long *)pool->d_timeline.ptr;
+        }
         kp.counter_set ^= 1;
         const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
         cudaError_t e;
-        if (k == CP_KIND_KV && pool->opt_kernel != 1 && kp.all_fast && pool->kv_tmap_ok) {
+        if (k == CP_KIND_KV && kp.use_kvt && pool->kv_tmap_ok) {
+            prm.n_combine_units = (int)kp.cunits.size();
+            e = launch_decode_kvt(prm, pool->kv_tmap, (int)(pool->page_bytes / 256), std::min(n_ctas, pool->n_sm),
+                                  kp.max_group, s);
+        } else if (k == CP_KIND_KV && kp.use_kvt) {
+            return CP_ERR_UNSUPPORTED;      // planned for the tcgen05 kernel but no tensor map (cannot happen: same conditions)
+        } else if (k == CP_KIND_KV && pool->opt_kernel != 1 && kp.all_fast && pool->kv_tmap_ok) {
             // warp-sized combine units, popped warp by warp after the tiles
             prm.n_combine_units = (int)kp.cunits.size();
             e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256),
@@ -1062,7 +1155,9 @@ cp_status build_stages_plan(cp_pool *pool, int32_t n_stages, const int32_t *size
     int64_t qb = 0, ob = 0, lb = 0, wb = 0;
     p_ids = ids;
     for (int s = 0; s < n_stages; ++s) {
+        pool->plan_for_stages = true;
         build_plan(pool, p_ids, sizes[s]);
+        pool->plan_for_stages = false;
         const KindPlan &src = pool->plan[CP_KIND_KV];
         const int gb = (int)kp.groups.size();
         const int cb = (int)kp.cunits.size();
@@ -1185,6 +1280,7 @@ static cp_status decode_stages_core(cp_pool *pool, int32_t n_stages, const int32
     prm.stage_done = prm.group_counters + kp.groups.size() * (size_t)kCounterStride;
     prm.n_stages = n_stages; prm.q_len = 1;
     prm.published = nullptr; prm.gate_flag = nullptr; prm.gate_timeout_us = 0;
+    prm.timeline = nullptr;
     if (published_dev) {
         if (sp.d_gate.ensure(16) != cudaSuccess || cudaMemsetAsync(sp.d_gate.ptr, 0, 16, s) != cudaSuccess) {
             cudaGetLastError();
