@@ -100,6 +100,10 @@ enum {
     CP_OPT_HOST_ZERO_COPY = 5, /* cp_decode_attention_host: 1 (default) = pinned, device-mapped host
                                 buffers are accessed in place (O / LSE written once; Q only when
                                 its re-reads by the tiles stay under 1 MB), 0 = always staged  */
+    CP_OPT_STATIC_PCT = 7,   /* tcgen05 MQA/GQA kernel: per cent of every group's 128-token slices that go into the
+                                static, equally long per-CTA pieces (default 100); the rest forms short
+                                tiles the CTAs pop dynamically when their static lists are done      */
+    CP_OPT_TAIL_TILE_SLICES = 8, /* ... and the length of those tiles in slices (default 2)            */
     CP_OPT_TIMELINE = 6      /* 1 = the next cp_decode_attention launches record per-CTA globaltimer
                                 stamps (cp_pool_read_timeline); 0 (default) = off.  Measurement aid of
                                 bench.py --probe timeline; kernels that do not stamp leave zeros.  */
@@ -373,6 +377,17 @@ cp_status cp_pool_counters(const cp_pool *pool, uint64_t *kernel_launches,
  * Synchronises the device and copies the stamps of the last launch of the pool: stamps_out_host holds
  * cap_ctas x 16 uint64; n_ctas_out receives the number of CTA rows available (the SM count). */
 cp_status cp_pool_read_timeline(cp_pool *pool, uint64_t *stamps_out_host, int32_t cap_ctas, int32_t *n_ctas_out);
+
+/* Measurement aids without any part in the hot path (cp_probe.cu; `bench.py --probe ...`).
+ * cp_probe_globaltimer: a one-thread kernel on `stream` that stores %globaltimer (ns) to *stamp_dev (8-byte
+ *   aligned device memory); bracketing a decode launch with two of them relates the per-CTA stamps of
+ *   cp_pool_read_timeline to the stream's own order (launch gap before the first CTA, drain after the last).
+ * cp_probe_read_stream: reads `bytes` of device memory once with 16-byte loads from n_ctas CTAs of 512
+ *   threads (nothing is written; *sink_dev, 4 bytes of device memory, only keeps the loads alive): the
+ *   read-only HBM ceiling next to the copy bandwidth of MEASURED_PEAKS.json.
+ * Both return INVALID_ARG for null / misaligned pointers, CUDA when the launch fails. */
+cp_status cp_probe_globaltimer(uint64_t *stamp_dev, void *stream);
+cp_status cp_probe_read_stream(const void *src_dev, uint64_t bytes, int32_t n_ctas, uint32_t *sink_dev, void *stream);
 
 /*
  * KV-cache planner: "The planner uses per-model prompt, output, and service-time

@@ -37,6 +37,8 @@ CP_OPT_MIN_TILE_PAGES = 3
 CP_OPT_VMM_TABLE = 4
 CP_OPT_HOST_ZERO_COPY = 5
 CP_OPT_TIMELINE = 6
+CP_OPT_STATIC_PCT = 7
+CP_OPT_TAIL_TILE_SLICES = 8
 TIMELINE_SLOTS = 16
 
 
@@ -103,6 +105,8 @@ def load_library():
         "cp_pool_counters": (i32, [vp, u64p, u64p, u64p]),
         "cp_pool_read_timeline": (i32, [vp, u64p, i32, i32p]),
         "cp_status_string": (ctypes.c_char_p, [i32]),
+        "cp_probe_globaltimer": (i32, [vp, vp]),
+        "cp_probe_read_stream": (i32, [vp, u64, i32, vp, vp]),
         "cp_planner_workspace_bytes": (u64, [ctypes.c_int64]),
         "cp_planner_pool_demand": (i32, [i32, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_double),
                                          vp, vp, vp, vp, ctypes.c_int64, vp, vp, vp, u64, vp]),
@@ -124,6 +128,7 @@ EXPORTED = ["cp_pool_create", "cp_pool_create_vmm", "cp_pool_vmm_info", "cp_pool
             "cp_decode_attention_host", "cp_decode_workspace_bytes_qlen", "cp_decode_attention_qlen",
             "cp_decode_stages_workspace_bytes", "cp_decode_attention_stages", "cp_decode_attention_stages_gated",
             "cp_decode_stages_gate_status", "cp_decode_plan", "cp_pool_counters", "cp_pool_read_timeline", "cp_status_string",
+            "cp_probe_globaltimer", "cp_probe_read_stream",
             "cp_planner_workspace_bytes", "cp_planner_pool_demand", "cp_planner_quantile"]
 
 
@@ -363,6 +368,16 @@ class Pool:
 
 
 # ---------------------------------------------------------------- KV-cache planner (Eq. (1)-(2))
+def probe_globaltimer(stamp_dev, stream: int = 0):
+    """One-thread kernel on `stream` that stores %globaltimer (ns) to the 8-byte device location stamp_dev."""
+    _check(load_library().cp_probe_globaltimer(_ptr(stamp_dev), stream), "cp_probe_globaltimer")
+
+
+def probe_read_stream(src_dev, nbytes: int, n_ctas: int, sink_dev, stream: int = 0):
+    """Read nbytes of device memory once (16-byte loads, nothing written): the read-only HBM ceiling."""
+    _check(load_library().cp_probe_read_stream(_ptr(src_dev), nbytes, n_ctas, _ptr(sink_dev), stream), "cp_probe_read_stream")
+
+
 def planner_workspace_bytes(n_trace_entries: int = 0) -> int:
     return int(load_library().cp_planner_workspace_bytes(int(n_trace_entries)))
 

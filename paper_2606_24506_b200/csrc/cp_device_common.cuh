@@ -32,7 +32,7 @@ __device__ __forceinline__ int ld_acquire_sys(const int32_t *p)
 __device__ __forceinline__ unsigned long long global_timer_ns()
 {
     unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t) :: "memory");
     return t;
 }
 

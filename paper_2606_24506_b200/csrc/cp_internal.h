@@ -133,6 +133,8 @@ struct DecodeParams {
     const Combine *combines;
     const CombineUnit *cunits;     // [n_combine_units] (tensor-core kernels)
     int32_t n_tiles;
+    int32_t n_static_slots;        // tcgen05 K/V kernel: records [0, n_static_slots) are the CTAs' static lists (slot j of CTA b
+                                   // at j * gridDim.x + b, TileRec::pad bit 0 = another slot follows), the rest is popped
     int32_t n_combines;            // work items after the tiles (CTA-sized combine items)
     int32_t n_combine_units;       // tensor-core kernels: warp-sized combine units; else = n_combines
     int32_t n_groups;

@@ -4,36 +4,40 @@
 //
 // A (request, kv head) group has g = Hq / Hkv query rows -- 8 to 32 here -- far fewer than the 128
 // rows a tcgen05 tile wants, so the roles are swapped: a slice of 128 cached tokens is the M
-// dimension and the group's rows (padded to N = 16 / 32 / ...) are the N dimension,
+// dimension and the group's rows (padded to N = 16 / 32) are the N dimension,
 //     S^T[128 tok x N] = K_slice[128 tok x 128 d] . Q^T          8 x tcgen05.mma M128 N K16
 //                        (A = the K blocks exactly as TMA lands them, K-major SWIZZLE_128B;
 //                         B = the query rows, K-major SWIZZLE_128B)
 //     O^T[128 d x N]  += V_slice^T[128 d x 128 tok] . P^T         8 x tcgen05.mma M128 N K16
 //                        (A = the V blocks as landed, read MN-major; B = P^T written by the softmax
 //                         threads as bf16, MN-major without swizzle),
-// both accumulators in tensor memory (2 score buffers + O = 3 N columns).  A softmax thread owns one
-// TMEM lane = one token of the slice and N scores, one per query row.  It needs the row (= query
-// head) maximum only as a REFERENCE for the exponent, not exactly: every thread keeps the same
-// per-head reference m_ref[h] and computes p = 2^(s - m_ref[h]) with no cross-thread reduction;
-// the reference moves (and O / l are rescaled) only when some score exceeds it by more than 2^8,
-// which the 128 threads agree on with one barrier.red.or per slice (for the data at hand: once,
-// on the first slice of a tile).  The row sums l[h] are per-thread partial sums that are reduced
-// once per tile in a fixed shuffle tree, so results are deterministic.
+// accumulators in tensor memory: two score buffers and TWO O^T buffers (4 N columns), so that the
+// tile that follows starts its MMAs while the finished tile's O^T is still being written out.
+// A softmax thread owns one TMEM lane = one token of the slice and N scores, one per query row.  It
+// needs the row (= query head) maximum only as a REFERENCE for the exponent, not exactly: every
+// thread keeps the same per-head reference m_ref[h] and computes p = 2^(s - m_ref[h]) with no
+// cross-thread reduction; the reference moves (and O / l are rescaled) only when some score exceeds
+// it by more than 2^8, which the 128 threads agree on with one barrier.red.or per slice (for the
+// data at hand: once, on the first slice of a tile).  The row sums l[h] are per-thread partial sums
+// reduced once per tile in a fixed shuffle tree, so results are deterministic.
 //
 // Why tcgen05 here although north_star keeps it "only on the MLA path": measured in round 1, eight
 // mma.sync consumer warps sustain 3.4 TB/s-equivalent at g = 32 (cfg4) and their end-of-tile merge
 // through shared memory costs ~3 us; with the tokens on M one elected thread issues 16 MMAs per 128
-// tokens (~950 cycles against a 2800-cycle HBM budget per slice and SM), for ANY g <= N, and the
-// tile result sits in ONE accumulator.
+// tokens for ANY g <= N, and the tile result sits in ONE accumulator.
 //
-// Warp roles (256 threads, 1 CTA / SM):
-//   warp 0      producer: pops tiles, translates logical pages through the page table (step a2) and
-//               streams them with TMA into a ring of 64 KB slice stages [K d0-63 | K d64-127 |
-//               V d0-63 | V d64-127], each a [128 tok x 128 B] SWIZZLE_128B block that the pages of
-//               the slice fill top to bottom.
-//   warp 1      MMA issuer (one lane by elect.sync); stages the tile's query rows into shared memory.
-//   warps 2..5  softmax (thread = token of the slice), epilogue (thread = value column d).
-//   warps 6..7  only help with the LSE combine units after the last tile.
+// Warp roles (320 threads, 1 CTA / SM):
+//   warp 0      producer: walks this CTA's static tiles, then pops the dynamic ones (step a5); translates
+//               logical pages through the page table (step a2) and streams them with TMA into a ring of
+//               64 KB slice stages [K d0-63 | K d64-127 | V d0-63 | V d64-127], each a [128 tok x 128 B]
+//               SWIZZLE_128B block that the pages of the slice fill top to bottom; stages the tile's
+//               query rows in shared memory (the next tile's record is fetched while the current streams).
+//   warp 1      MMA issuer (one lane by elect.sync); the slices of consecutive tiles form one software
+//               pipeline: S of slice j is issued before P.V of slice j - 1, across tile boundaries.
+//   warps 2..5  softmax (thread = token of the slice).
+//   warps 6..9  epilogue (thread = value column d): O^T from TMEM -> normalised output or split partial,
+//               (m, l), release of the group's arrival counter (step a6).
+//   all warps   LSE combine units after the CTA's last tile (step a4).
 //
 // Paper anchors: paged KV interface PAPER.md:L101,L122; KV-head-limited attention under low
 // concurrency PAPER.md:L21,L57; GPU-resident persistent control PAPER.md:L146.
@@ -51,18 +55,19 @@ constexpr int KT_SLICE = 128;                        // tokens per slice = MMA M
 constexpr int KT_SUBB = KT_SLICE * 128;              // one swizzled block: 128 rows x 128 B
 constexpr int KT_STAGE_BYTES = 4 * KT_SUBB;          // 65536
 constexpr int KT_TQ = 4;                             // tile-queue depth
-constexpr int KT_WARPS = 8;
+constexpr int KT_WARPS = 10;
 constexpr int KT_THREADS = 32 * KT_WARPS;
 constexpr int KT_MISC_BYTES = 3072;
 constexpr int KT_SMEM_LIMIT = 232448;                // 227 KB opt-in maximum per CTA
 constexpr float KT_LAZY_LOG2 = 8.0f;                 // the reference moves when a score exceeds it by 2^8
+constexpr int KT_NMAX = 32;
 
 __host__ __device__ constexpr int kt_q_bytes(int N) { return 2 * N * 128; }          // one query buffer: 2 blocks [N x 128 B]
 __host__ __device__ constexpr int kt_p_bytes(int N) { return (N / 8) * 2048; }       // one P^T buffer
 __host__ __device__ constexpr int kt_fixed_bytes(int N) { return 2 * kt_q_bytes(N) + 2 * kt_p_bytes(N) + KT_MISC_BYTES; }
 __host__ __device__ constexpr int kt_num_stages(int N) { return (KT_SMEM_LIMIT - kt_fixed_bytes(N)) / KT_STAGE_BYTES; }
 __host__ __device__ constexpr int kt_smem_bytes(int N) { return kt_num_stages(N) * KT_STAGE_BYTES + kt_fixed_bytes(N); }
-__host__ __device__ constexpr uint32_t kt_tmem_cols(int N) { return 3 * N <= 32 ? 32u : 3 * N <= 64 ? 64u : 3 * N <= 128 ? 128u : 3 * N <= 256 ? 256u : 512u; }
+__host__ __device__ constexpr uint32_t kt_tmem_cols(int N) { return 4 * N <= 32 ? 32u : 4 * N <= 64 ? 64u : 4 * N <= 128 ? 128u : 4 * N <= 256 ? 256u : 512u; }
 
 struct KtDesc {                  // what the producer hands to the other warps for one tile
     int32_t item;                // work index; < 0: no more work
@@ -72,6 +77,8 @@ struct KtDesc {                  // what the producer hands to the other warps f
     int32_t split, n_splits;
     int32_t gsize;               // query rows of the group
     float scale_log2;
+    int32_t zl;                  // log2 of the split lanes of the group's combine units: fixes the partial layout
+    int32_t pad;
     int64_t q_off, out_off, lse_off, part_off;
 };
 
@@ -80,11 +87,16 @@ struct KtMisc {
     uint64_t s_full[2], s_empty[2];              // score buffers in TMEM: MMA -> softmax -> MMA
     uint64_t p_full[2], p_done[2];               // P^T buffers: softmax -> MMA, MMA (commit) -> softmax
     uint64_t q_free[2];                          // query buffers: score MMAs of the tile that used it are complete
+    uint64_t o_done[2];                          // O^T buffer: every value MMA of the tile is complete (MMA commit)
+    uint64_t e_full[2];                          // tile's row sums / references are in red[] / mref[] (4 softmax warps)
+    uint64_t o_free[2];                          // epilogue has read O^T, red[], mref[] of the tile (4 epilogue warps)
     uint64_t tq_full[KT_TQ], tq_empty[KT_TQ];
     KtDesc tq[KT_TQ];
     uint32_t tmem_base;
     uint32_t pad[3];
-    float red[4 * 128];                          // cross-warp reductions: [column][warp]
+    float redmax[4 * KT_NMAX];                   // slice maxima when the reference moves: [row][warp]
+    float red[2][4 * KT_NMAX];                   // per-tile row sums: [O buffer][row][warp]
+    float mref[2][KT_NMAX];                      // per-tile exponent reference (log2 units): [O buffer][row]
 };
 static_assert(sizeof(KtMisc) <= KT_MISC_BYTES, "KtMisc must fit its reserved block");
 
@@ -96,6 +108,7 @@ __device__ __forceinline__ bool bar_red_or_softmax(bool pred)       // barrier 2
     return r != 0;
 }
 __device__ __forceinline__ void bar_sync_softmax() { asm volatile("bar.sync 2, 128;" ::: "memory"); }
+__device__ __forceinline__ void bar_sync_combine() { asm volatile("bar.sync 3, 320;" ::: "memory"); }
 
 __device__ __forceinline__ void kt_stamp(const DecodeParams &p, int k)
 {
@@ -130,6 +143,151 @@ __device__ __forceinline__ float col_reduce(float (&v)[CN], const int lane, Op o
     return v[0];
 }
 
+__device__ __forceinline__ TileRec load_tile_rec(const TileRec *recs, int item)
+{
+    TileRec r;
+    const uint4 *src = reinterpret_cast<const uint4 *>(recs + item);
+    uint4 *dst = reinterpret_cast<uint4 *>(&r);
+#pragma unroll
+    for (int i = 0; i < 5; ++i) dst[i] = __ldg(src + i);
+    return r;
+}
+
+// ---------------------------------------------------------------------------------------
+// LSE combine, kvt flavour (step a4).  Same arithmetic and the same fixed summation order as
+// combine_units() of cp_device_common.cuh, restructured for latency -- it is the tail of the
+// kernel: (1) ONE warp per CTA polls the arrival counters of the round's units (lane i for
+// unit i; a few hundred pollers on one L2 line delay the very arrivals they wait for) and the
+// CTA's warps pass a named barrier; (2) a lane loads the (m, l) pairs AND the O rows of its own
+// splits z, z + ZL, ... in ONE round trip and needs no shared memory: weights are computed
+// per lane, maxima and sums go through shuffles over the split-lane bits.
+// ---------------------------------------------------------------------------------------
+template <int KMAX>
+__device__ __forceinline__ void combine_one_unit(const DecodeParams &p, const CombineUnit &cu, const int lane, const int sb = 13)
+{
+    const int ns = cu.n_splits;
+    const int zl = cu.zl_log2;
+    const int ZL = 1 << zl, CQ = 32 >> zl;
+    const int z = lane >> (5 - zl), cq = lane & (CQ - 1);
+    const float2 *mlp = reinterpret_cast<const float2 *>(p.workspace + cu.ml_off);
+    const float *src = p.workspace + cu.part_off + cq * 4;
+    const int ss = cu.split_stride;
+    float2 ml[KMAX];
+    float4 v[KMAX];
+#pragma unroll
+    for (int k = 0; k < KMAX; ++k) {
+        const int s = z + k * ZL;
+        ml[k] = make_float2(-INFINITY, 0.f);
+        v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (s < ns) {
+            ml[k] = __ldcg(mlp + s);
+            v[k] = ld_cg_f4(src + (size_t)s * ss);
+        }
+    }
+    float M = -INFINITY;
+#pragma unroll
+    for (int k = 0; k < KMAX; ++k) M = fmaxf(M, ml[k].x);
+    for (int o = CQ; o < 32; o <<= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+    if (threadIdx.x == 0) kt_stamp(p, sb);
+    float L = 0.f;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < KMAX; ++k) {
+        const float w = ex2_ftz(ml[k].x - M);          // 0 for absent splits (m = -inf)
+        L += w * ml[k].y;
+        acc.x += w * v[k].x; acc.y += w * v[k].y; acc.z += w * v[k].z; acc.w += w * v[k].w;
+    }
+    for (int o = CQ; o < 32; o <<= 1) {                // warp-uniform trip count
+        L += __shfl_xor_sync(0xffffffffu, L, o);
+        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
+        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
+        acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
+    }
+    if (threadIdx.x == 0) kt_stamp(p, sb + 1);
+    if (z == 0) {
+        const float invL = 1.0f / L;
+        *reinterpret_cast<float4 *>(p.out + cu.out_off + cq * 4) =
+            make_float4(acc.x * invL, acc.y * invL, acc.z * invL, acc.w * invL);
+    }
+    if (cu.lse_off >= 0 && lane == 0) p.lse[cu.lse_off] = (M + log2f(L)) * 0.6931471805599453f;
+}
+
+// More than KMAX splits per lane: two passes (maximum, then weights and sums), same order.
+__device__ __noinline__ void combine_one_unit_long(const DecodeParams &p, const CombineUnit &cu, const int lane)
+{
+    const int ns = cu.n_splits;
+    const int zl = cu.zl_log2;
+    const int ZL = 1 << zl, CQ = 32 >> zl;
+    const int z = lane >> (5 - zl), cq = lane & (CQ - 1);
+    const float2 *mlp = reinterpret_cast<const float2 *>(p.workspace + cu.ml_off);
+    const float *src = p.workspace + cu.part_off + cq * 4;
+    const int ss = cu.split_stride;
+    float M = -INFINITY;
+    for (int s = z; s < ns; s += ZL) M = fmaxf(M, __ldcg(mlp + s).x);
+    for (int o = CQ; o < 32; o <<= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+    float L = 0.f;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 4
+    for (int s = z; s < ns; s += ZL) {
+        const float2 ml = __ldcg(mlp + s);
+        const float4 v = ld_cg_f4(src + (size_t)s * ss);
+        const float w = ex2_ftz(ml.x - M);
+        L += w * ml.y;
+        acc.x += w * v.x; acc.y += w * v.y; acc.z += w * v.z; acc.w += w * v.w;
+    }
+    for (int o = CQ; o < 32; o <<= 1) {
+        L += __shfl_xor_sync(0xffffffffu, L, o);
+        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
+        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
+        acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
+    }
+    if (z == 0) {
+        const float invL = 1.0f / L;
+        *reinterpret_cast<float4 *>(p.out + cu.out_off + cq * 4) =
+            make_float4(acc.x * invL, acc.y * invL, acc.z * invL, acc.w * invL);
+    }
+    if (cu.lse_off >= 0 && lane == 0) p.lse[cu.lse_off] = (M + log2f(L)) * 0.6931471805599453f;
+}
+
+// Called by ALL threads of the CTA (named barrier 3).  Round r of CTA b holds the KT_WARPS consecutive
+// units (r * gridDim.x + b) * KT_WARPS + warp; units are sorted by group, so a round polls one or two
+// counters.  A unit only waits for tiles that are already running on some SM (every CTA reaches this
+// point only after the tile lists are exhausted), so the polling terminates.
+__device__ __forceinline__ void kt_combine(const DecodeParams &p, const int warp, const int lane)
+{
+    const int n = p.n_combine_units;
+    for (int base = blockIdx.x * KT_WARPS; base < n; base += gridDim.x * KT_WARPS) {
+        const int u = base + warp;
+        CombineUnit cu;
+        if (u < n) cu = load_combine_unit(p.cunits, u);
+        if (warp == 0) {
+            const int32_t *ctr = nullptr;
+            int want = 0;
+            if (lane < KT_WARPS && base + lane < n) {
+                const int4 a = __ldg(reinterpret_cast<const int4 *>(&p.cunits[base + lane].split_stride));   // stride, n_splits, zl, want
+                const int grp = __ldg(&p.cunits[base + lane].group);
+                want = a.w;
+                ctr = p.group_counters + (size_t)grp * kCounterStride;
+            }
+            for (;;) {
+                const bool ok = ctr == nullptr || ld_acquire(ctr) >= want;
+                if (__all_sync(0xffffffffu, ok)) break;
+                __nanosleep(100);
+            }
+            if (lane == 0) kt_stamp(p, 12);
+        }
+        bar_sync_combine();
+        if (threadIdx.x == 0) kt_stamp(p, 1);
+        if (u < n) {
+            const int per_lane = (cu.n_splits + (1 << cu.zl_log2) - 1) >> cu.zl_log2;
+            if (per_lane <= 8) combine_one_unit<8>(p, cu, lane);
+            else combine_one_unit_long(p, cu, lane);
+        }
+    }
+}
+
 template <int N>
 __global__ void __launch_bounds__(KT_THREADS, 1)
 cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap, int rows_per_page)
@@ -138,7 +296,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     constexpr int CN = N >= 32 ? 32 : 16;            // column block of the reductions
     constexpr int NB = N / CN;
     static_assert(NS >= 2 && NS <= 4, "slice ring depth");
-    static_assert(N % 16 == 0 && N >= 16 && N <= 128, "N = padded query rows of a group");
+    static_assert(N % 16 == 0 && N >= 16 && N <= KT_NMAX, "N = padded query rows of a group");
 
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t st_base = smem_u32(smem);
@@ -149,28 +307,45 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     const int tid = threadIdx.x;
     const int warp = tid >> 5;
     const int lane = tid & 31;
-    if (tid == 0) kt_stamp(p, 0);
+    const int P = (int)p.page_tokens;
+    const int pps = KT_SLICE / P;                    // pages per slice
+
+    // the producer's first tile record is requested before anything else: its latency (the L2 is cold
+    // at the start of a step) runs under the barrier / tensor-memory set-up
+    TileRec r_next;
+    bool has_next = false;
+    if (warp == 0) {
+        has_next = (int)blockIdx.x < p.n_static_slots;
+        if (has_next) r_next = load_tile_rec(p.tile_recs, blockIdx.x);
+    }
+    if (tid == 0) {
+        kt_stamp(p, 0);
+        if (p.timeline) {
+            uint32_t smid;
+            asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+            p.timeline[(size_t)blockIdx.x * kTimelineSlots + 8] = smid;
+        }
+    }
     scheduler_reset_other_set(p);
 
-    if (tid == 0) {
+    if (tid == 32) {
         for (int i = 0; i < NS; ++i) { mbar_init(smem_u32(&mi->full[i]), 1); mbar_init(smem_u32(&mi->empty[i]), 1); }
         for (int i = 0; i < 2; ++i) {
             mbar_init(smem_u32(&mi->s_full[i]), 1); mbar_init(smem_u32(&mi->s_empty[i]), 4);
             mbar_init(smem_u32(&mi->p_full[i]), 4); mbar_init(smem_u32(&mi->p_done[i]), 1);
             mbar_init(smem_u32(&mi->q_free[i]), 1);
+            mbar_init(smem_u32(&mi->o_done[i]), 1); mbar_init(smem_u32(&mi->e_full[i]), 4); mbar_init(smem_u32(&mi->o_free[i]), 4);
         }
-        for (int i = 0; i < KT_TQ; ++i) { mbar_init(smem_u32(&mi->tq_full[i]), 1); mbar_init(smem_u32(&mi->tq_empty[i]), 5); }
+        for (int i = 0; i < KT_TQ; ++i) { mbar_init(smem_u32(&mi->tq_full[i]), 1); mbar_init(smem_u32(&mi->tq_empty[i]), 9); }
         asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap)) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_proxy_async();
     }
-    if (warp == 1) tmem_alloc(smem_u32(&mi->tmem_base), kt_tmem_cols(N));
+    if (warp == 2) tmem_alloc(smem_u32(&mi->tmem_base), kt_tmem_cols(N));
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = mi->tmem_base;
-    const int P = (int)p.page_tokens;
-    const int pps = KT_SLICE / P;                    // pages per slice
 
     if (warp == 0) {
         // =========================================================== producer warp
@@ -178,51 +353,84 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
         asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
         uint32_t gs = 0;          // slices issued by this CTA (ring position)
         uint32_t qi = 0;          // work items pushed
+        int item_next = has_next ? (int)blockIdx.x : -3;     // -3: no static slot at all, start with the dynamic list
+        bool in_static = true;
+        int n_done = 0;
         for (;;) {
-            // the first tile of a CTA is static (its block index): no atomic round trip at start-up
-            int work = 0;
-            if (qi == 0) work = blockIdx.x;
-            else {
-                if (lane == 0) work = atomicAdd(p.work_counter, 1) + (int)gridDim.x;
-                work = __shfl_sync(0xffffffffu, work, 0);
+            // ---- the tile to run now (fetched during the previous tile) ...
+            int item = item_next;
+            TileRec r = r_next;
+            if (item >= 0 && r.n_pages == 0) item = -2;          // empty static slot of this CTA: skip, go dynamic
+            // ---- ... and the one after it: the next static slot of this CTA, else a pop from the dynamic list.
+            // The pop's result is not looked at before this tile's first pages are requested (resolve_next).
+            int nx_raw = -1;
+            bool nx_pending = false;
+            if (item != -1) {
+                if (in_static && item >= 0 && (r.pad & 1)) nx_raw = item + (int)gridDim.x;
+                else {
+                    in_static = false;
+                    if (lane == 0) nx_raw = atomicAdd(p.work_counter, 1) + p.n_static_slots;
+                    nx_pending = true;
+                }
             }
-            const int item = work < p.n_tiles ? work : -1;
-            TileRec r;
-            int n_slices = 0, valid_last = KT_SLICE, npg = 0;
-            if (item >= 0) {
-                const uint4 *src = reinterpret_cast<const uint4 *>(p.tile_recs + item);
-                uint4 *dst = reinterpret_cast<uint4 *>(&r);
+            auto resolve_next = [&]() {
+                int nx = nx_raw;
+                if (nx_pending) {
+                    nx = __shfl_sync(0xffffffffu, nx_raw, 0);
+                    if (nx >= p.n_tiles) nx = -1;
+                    nx_pending = false;
+                }
+                item_next = nx;
+                if (nx >= 0) r_next = load_tile_rec(p.tile_recs, nx);
+            };
+            if (item <= -2) { resolve_next(); continue; }
+            if (item == -1) {
+                // ---- no more work: the end marker goes through the same queue
+                const uint32_t qs = qi % KT_TQ;
+                mbar_wait(smem_u32(&mi->tq_empty[qs]), ((qi / KT_TQ) & 1) ^ 1);
+                if (lane == 0) {
+                    KtDesc d;
+                    d.item = -1; d.group_idx = 0; d.n_slices = 0; d.valid_last = KT_SLICE; d.split = 0; d.n_splits = 1;
+                    d.gsize = 1; d.scale_log2 = 0.f; d.q_off = d.out_off = d.lse_off = d.part_off = 0;
+                    mi->tq[qs] = d;
+                    mbar_arrive(smem_u32(&mi->tq_full[qs]));
+                }
+                break;
+            }
+            // ---- one round trip: the first 32 page ids (needed first: the tile's first pages are requested as
+            // soon as they are known), the context length (decides only how many tokens of the tile's LAST
+            // slice are valid: every planned page holds a valid token, contexts never shrink under a plan)
+            // and the query rows.  Volatile asm: issued here, in this order, not sunk to their first use.
+            int32_t pid0 = 0;
+            int ctx;
+            uint4 qv[N / 2];
+            if (lane < r.n_pages) {
+                if (p.slot_pages > 0) pid0 = r.req * p.slot_pages + (r.page_begin + lane) * r.n_kv_heads + r.kv_head;
+                else
+                    asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(pid0)
+                                 : "l"(p.page_table + (int64_t)r.req * p.max_ppr + (int64_t)(r.page_begin + lane) * r.n_kv_heads + r.kv_head));
+            }
+            asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(ctx) : "l"(p.req_ctx + r.req));
+            {
+                const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + r.q_off);
 #pragma unroll
-                for (int i = 0; i < 5; ++i) dst[i] = __ldg(src + i);
-                const int ctx = __ldg(p.req_ctx + r.req);
-                const int t_begin = r.page_begin * P;
-                const int t_end = min((r.page_begin + r.n_pages) * P, ctx);
-                n_slices = (t_end - t_begin + KT_SLICE - 1) / KT_SLICE;
-                valid_last = t_end - t_begin - (n_slices - 1) * KT_SLICE;
-                npg = (t_end - t_begin + P - 1) / P;         // pages of the tile that hold at least one valid token
-            } else {
-                r.group = 0; r.req = 0; r.kv_head = 0; r.n_kv_heads = 1; r.page_begin = 0; r.n_pages = 0;
-                r.split = 0; r.n_splits = 1; r.gsize = 1; r.n_q_heads = 1; r.scale_log2 = 0.f;
-                r.q_off = r.out_off = r.lse_off = r.part_off = 0; r.pad = 0;
+                for (int k = 0; k < N / 2; ++k) {
+                    const int id = lane + 32 * k;
+                    qv[k] = make_uint4(0u, 0u, 0u, 0u);
+                    if ((id >> 4) < r.gsize)
+                        asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(qv[k].x), "=r"(qv[k].y), "=r"(qv[k].z), "=r"(qv[k].w) : "l"(qg + id));
+                }
             }
-            const uint32_t qs = qi % KT_TQ;
-            mbar_wait(smem_u32(&mi->tq_empty[qs]), ((qi / KT_TQ) & 1) ^ 1);
-            if (lane == 0) {
-                KtDesc d;
-                d.item = item; d.group_idx = r.group; d.n_slices = n_slices; d.valid_last = valid_last;
-                d.split = r.split; d.n_splits = r.n_splits; d.gsize = r.gsize; d.scale_log2 = r.scale_log2;
-                d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
-                mi->tq[qs] = d;
-                mbar_arrive(smem_u32(&mi->tq_full[qs]));     // release: the consumers acquire via try_wait
-            }
-            ++qi;
-            if (item < 0) break;
-
+            const int npg = r.n_pages;
             const int hkv = r.n_kv_heads;
+            ++n_done;
             for (int j0 = 0; j0 < npg; j0 += 32) {
                 // translate up to 32 logical pages at once (step a2: one page-table entry per lane)
-                int32_t pid = 0;
-                if (j0 + lane < npg) pid = page_of(p, r.req, (int64_t)(r.page_begin + j0 + lane) * hkv + r.kv_head);
+                int32_t pid = pid0;
+                if (j0 > 0) {
+                    pid = 0;
+                    if (j0 + lane < npg) pid = page_of(p, r.req, (int64_t)(r.page_begin + j0 + lane) * hkv + r.kv_head);
+                }
                 const int nj = min(32, npg - j0);
                 for (int j = 0; j < nj; ++j) {
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);
@@ -239,16 +447,140 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                         tma_load_2d(dst + KT_SUBB, &tmap, 64, row, fb, policy);         // K, d 64..127
                         tma_load_2d(dst + 2 * KT_SUBB, &tmap, 0, row + P, fb, policy);  // V, d 0..63
                         tma_load_2d(dst + 3 * KT_SUBB, &tmap, 64, row + P, fb, policy); // V, d 64..127
+                        if (gs == 0 && pg == 0) kt_stamp(p, 9);
                     }
                     if (pg == pps - 1 || jj == npg - 1) ++gs;
+                    if (jj == min(npg, pps) - 1) {
+                        // ---- the first slice is on its way: now hand the tile to the other warps.  Query rows ->
+                        // buffer (qi & 1): two K-major [N x 64] blocks, 128-byte swizzle (16-B chunk index ^
+                        // (row & 7)); rows beyond the group are zero.  The buffer is free once the score MMAs
+                        // of tile qi - 2 are complete.
+                        const int t_begin = r.page_begin * P;
+                        const int t_end = min((r.page_begin + r.n_pages) * P, ctx);
+                        const int n_slices = (t_end - t_begin + KT_SLICE - 1) / KT_SLICE;
+                        const int valid_last = t_end - t_begin - (n_slices - 1) * KT_SLICE;
+                        const uint32_t qs = qi % KT_TQ;
+                        mbar_wait(smem_u32(&mi->tq_empty[qs]), ((qi / KT_TQ) & 1) ^ 1);
+                        if (qi >= 2) mbar_wait(smem_u32(&mi->q_free[qi & 1]), ((qi >> 1) - 1) & 1);
+                        const uint32_t qb = q_base + (qi & 1) * kt_q_bytes(N);
+#pragma unroll
+                        for (int k = 0; k < N / 2; ++k) {
+                            const int id = lane + 32 * k;
+                            const int row = id >> 4, ch = id & 15;
+                            const uint32_t a = qb + (ch >> 3) * (N * 128) + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
+                            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(qv[k].x), "r"(qv[k].y), "r"(qv[k].z), "r"(qv[k].w) : "memory");
+                        }
+                        fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0) {
+                            KtDesc d;
+                            d.item = item; d.group_idx = r.group; d.n_slices = n_slices; d.valid_last = valid_last;
+                            d.split = r.split; d.n_splits = r.n_splits; d.gsize = r.gsize; d.scale_log2 = r.scale_log2;
+                            d.zl = (r.pad >> 8) & 0xff;
+                            d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
+                            mi->tq[qs] = d;
+                            mbar_arrive(smem_u32(&mi->tq_full[qs]));     // release: the consumers acquire via try_wait
+                        }
+                        ++qi;
+                        resolve_next();
+                    }
                 }
             }
         }
-        if (lane == 0) kt_stamp(p, 3);
+        if (lane == 0) {
+            kt_stamp(p, 3);
+            if (p.timeline) p.timeline[(size_t)blockIdx.x * kTimelineSlots + 11] = (unsigned long long)n_done;
+        }
     } else if (warp == 1) {
         // =========================================================== MMA issuer warp
         constexpr uint32_t IDESC_S = umma_idesc_bf16(KT_SLICE, N, 0, 0);      // K (K-major) x Q^T (K-major)
         constexpr uint32_t IDESC_PV = umma_idesc_bf16(KT_SLICE, N, 1, 1);     // V^T (MN-major) x P^T (MN-major)
+        uint32_t gs = 0, qi = 0, tc = 0;
+        // the value MMAs of the slice issued last, not yet issued themselves (software pipeline across tiles)
+        bool pend = false;
+        uint32_t pe_g = 0, pe_tc = 0;
+        int pe_ksteps = 0;
+        bool pe_first = false, pe_last = false;
+        auto issue_pv = [&]() {
+            // ---- O^T += V^T P^T of slice pe_g, 16 tokens per MMA; a tile's last slice stops after its last valid 16
+            const uint32_t slot = pe_g % NS, b = pe_g & 1, ob = pe_tc & 1;
+            mbar_wait(smem_u32(&mi->p_full[b]), (pe_g >> 1) & 1);
+            if (pe_first && pe_tc >= 2) mbar_wait(smem_u32(&mi->o_free[ob]), ((pe_tc >> 1) - 1) & 1);   // epilogue of tile tc - 2
+            tc_fence_after();
+            if (elect_one()) {
+                const uint32_t v0 = st_base + slot * KT_STAGE_BYTES + 2 * KT_SUBB;
+                const uint32_t pb = p_base + b * kt_p_bytes(N);
+                for (int k = 0; k < pe_ksteps; ++k) {
+                    // V: 64-column blocks KT_SUBB apart (LBO), 8-token groups 1024 B apart (SBO)
+                    const uint64_t ad = umma_smem_desc(v0 + k * 2048, KT_SUBB, 1024, 2);
+                    // P^T: 8-token groups 128 B apart (LBO), 8-row groups 2048 B apart (SBO)
+                    const uint64_t bd = umma_smem_desc(pb + k * 256, 128, 2048, 0);
+                    umma_bf16_ss(tmem + (2 + ob) * N, ad, bd, IDESC_PV, (!pe_first) || (k > 0));
+                }
+                umma_commit(smem_u32(&mi->empty[slot]));      // slice consumed: the stage is free
+                umma_commit(smem_u32(&mi->p_done[b]));        // P^T buffer free, O updated
+                if (pe_last) umma_commit(smem_u32(&mi->o_done[ob]));
+            }
+            __syncwarp();
+            pend = false;
+        };
+        for (;;) {
+            const uint32_t qs = qi % KT_TQ;
+            // never sit on finished work while waiting for the next tile
+            if (pend && !mbar_try_wait(smem_u32(&mi->tq_full[qs]), (qi / KT_TQ) & 1)) issue_pv();
+            mbar_wait(smem_u32(&mi->tq_full[qs]), (qi / KT_TQ) & 1);
+            const KtDesc d = mi->tq[qs];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&mi->tq_empty[qs]));
+            ++qi;
+            if (d.item < 0) break;
+            const uint32_t qb = q_base + (tc & 1) * kt_q_bytes(N);
+            const int n = d.n_slices;
+            if (n == 0) {
+                // empty (warm-up) tile: nothing to multiply, the hand-overs still happen
+                if (pend) issue_pv();
+                if (elect_one()) {
+                    umma_commit(smem_u32(&mi->q_free[tc & 1]));
+                    umma_commit(smem_u32(&mi->o_done[tc & 1]));
+                }
+                __syncwarp();
+            }
+            for (int i = 0; i < n; ++i) {
+                // ---- S_i^T = K_i Q^T into score buffer (g & 1)
+                const uint32_t g = gs + (uint32_t)i, slot = g % NS, b = g & 1;
+                mbar_wait(smem_u32(&mi->full[slot]), (g / NS) & 1);
+                if (lane == 0 && g == 0) kt_stamp(p, 2);
+                if (lane == 0 && i == n - 1) kt_stamp(p, 10);
+                mbar_wait(smem_u32(&mi->s_empty[b]), ((g >> 1) & 1) ^ 1);
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint32_t k0 = st_base + slot * KT_STAGE_BYTES;
+#pragma unroll
+                    for (int sb = 0; sb < 2; ++sb)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {           // K = 16 per MMA: 32 bytes inside the swizzled row
+                            const uint64_t ad = umma_smem_desc(k0 + sb * KT_SUBB + j * 32, 16, 1024, 2);
+                            const uint64_t bd = umma_smem_desc(qb + sb * (N * 128) + j * 32, 16, 1024, 2);
+                            umma_bf16_ss(tmem + b * N, ad, bd, IDESC_S, (sb | j) != 0);
+                        }
+                    umma_commit(smem_u32(&mi->s_full[b]));
+                    if (i == n - 1) umma_commit(smem_u32(&mi->q_free[tc & 1]));
+                }
+                __syncwarp();
+                if (pend) issue_pv();
+                pend = true;
+                pe_g = g; pe_tc = tc; pe_first = i == 0; pe_last = i == n - 1;
+                pe_ksteps = (i == n - 1) ? (d.valid_last + 15) >> 4 : KT_SLICE / 16;
+            }
+            gs += (uint32_t)n;
+            ++tc;
+        }
+        if (pend) issue_pv();
+    } else if (warp < 6) {
+        // =========================================================== softmax warps (thread = token of the slice)
+        const int q4 = warp & 3;                          // TMEM lane quadrant this warp may access
+        const int st = q4 * 32 + lane;                    // token of the slice
+        const uint32_t tl = tmem + ((uint32_t)(q4 * 32) << 16);
         uint32_t gs = 0, qi = 0, tc = 0;
         for (;;) {
             const uint32_t qs = qi % KT_TQ;
@@ -258,88 +590,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             if (lane == 0) mbar_arrive(smem_u32(&mi->tq_empty[qs]));
             ++qi;
             if (d.item < 0) break;
-            if (lane == 0 && tc == 0) kt_stamp(p, 1);
-            // ---- the tile's query rows -> buffer (tc & 1): two K-major [N x 64] blocks, 128-byte swizzle
-            // (16-B chunk index ^ (row & 7)); rows beyond the group are zero.  The buffer is free once
-            // the score MMAs of tile tc - 2 are complete.
-            const uint32_t qb = q_base + (tc & 1) * kt_q_bytes(N);
-            if (tc >= 2) mbar_wait(smem_u32(&mi->q_free[tc & 1]), ((tc >> 1) - 1) & 1);
-            {
-                const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + d.q_off);
-#pragma unroll 4
-                for (int id = lane; id < N * 16; id += 32) {
-                    const int r = id >> 4, ch = id & 15;
-                    uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                    if (r < d.gsize) v = __ldg(qg + id);
-                    const uint32_t a = qb + (ch >> 3) * (N * 128) + r * 128 + (((ch & 7) ^ (r & 7)) << 4);
-                    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-                }
-                fence_proxy_async();
-                __syncwarp();
-            }
-            const int n = d.n_slices;
-            for (int i = 0; i <= n; ++i) {
-                if (i < n) {
-                    // ---- S_i^T = K_i Q^T into score buffer (g & 1)
-                    const uint32_t g = gs + (uint32_t)i, slot = g % NS, b = g & 1;
-                    mbar_wait(smem_u32(&mi->full[slot]), (g / NS) & 1);
-                    if (lane == 0 && g == 0) kt_stamp(p, 2);
-                    mbar_wait(smem_u32(&mi->s_empty[b]), ((g >> 1) & 1) ^ 1);
-                    tc_fence_after();
-                    if (elect_one()) {
-                        const uint32_t k0 = st_base + slot * KT_STAGE_BYTES;
-#pragma unroll
-                        for (int sb = 0; sb < 2; ++sb)
-#pragma unroll
-                            for (int j = 0; j < 4; ++j) {           // K = 16 per MMA: 32 bytes inside the swizzled row
-                                const uint64_t ad = umma_smem_desc(k0 + sb * KT_SUBB + j * 32, 16, 1024, 2);
-                                const uint64_t bd = umma_smem_desc(qb + sb * (N * 128) + j * 32, 16, 1024, 2);
-                                umma_bf16_ss(tmem + b * N, ad, bd, IDESC_S, (sb | j) != 0);
-                            }
-                        umma_commit(smem_u32(&mi->s_full[b]));
-                        if (i == n - 1) umma_commit(smem_u32(&mi->q_free[tc & 1]));
-                    }
-                    __syncwarp();
-                }
-                if (i >= 1) {
-                    // ---- O^T += V_{i-1}^T P_{i-1}^T, 16 tokens per MMA; the last slice stops after its last valid 16
-                    const uint32_t g = gs + (uint32_t)i - 1, slot = g % NS, b = g & 1;
-                    mbar_wait(smem_u32(&mi->p_full[b]), (g >> 1) & 1);
-                    tc_fence_after();
-                    const int ksteps = (i == n) ? (d.valid_last + 15) >> 4 : KT_SLICE / 16;
-                    if (elect_one()) {
-                        const uint32_t v0 = st_base + slot * KT_STAGE_BYTES + 2 * KT_SUBB;
-                        const uint32_t pb = p_base + b * kt_p_bytes(N);
-                        for (int k = 0; k < ksteps; ++k) {
-                            // V: 64-column blocks KT_SUBB apart (LBO), 8-token groups 1024 B apart (SBO)
-                            const uint64_t ad = umma_smem_desc(v0 + k * 2048, KT_SUBB, 1024, 2);
-                            // P^T: 8-token groups 128 B apart (LBO), 8-row groups 2048 B apart (SBO)
-                            const uint64_t bd = umma_smem_desc(pb + k * 256, 128, 2048, 0);
-                            umma_bf16_ss(tmem + 2 * N, ad, bd, IDESC_PV, (i > 1) || (k > 0));
-                        }
-                        umma_commit(smem_u32(&mi->empty[slot]));      // slice consumed: the stage is free
-                        umma_commit(smem_u32(&mi->p_done[b]));        // P^T buffer free, O updated
-                    }
-                    __syncwarp();
-                }
-            }
-            gs += (uint32_t)n;
-            ++tc;
-        }
-    } else if (warp < 6) {
-        // =========================================================== softmax warps (thread = token of the slice)
-        const int q4 = warp & 3;                          // TMEM lane quadrant this warp may access
-        const int st = q4 * 32 + lane;                    // token of the slice / value column of the epilogue
-        const uint32_t tl = tmem + ((uint32_t)(q4 * 32) << 16);
-        uint32_t gs = 0, qi = 0;
-        for (;;) {
-            const uint32_t qs = qi % KT_TQ;
-            mbar_wait(smem_u32(&mi->tq_full[qs]), (qi / KT_TQ) & 1);
-            const KtDesc d = mi->tq[qs];
-            __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(&mi->tq_empty[qs]));
-            ++qi;
-            if (d.item < 0) break;
+            const uint32_t ob = tc & 1;
 
             float m_ref[N], l_part[N];
 #pragma unroll
@@ -376,12 +627,12 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
 #pragma unroll
                         for (int h = 0; h < CN; ++h) v[h] = tv ? x[cb * CN + h] : -INFINITY;
                         const float cm = col_reduce<CN>(v, lane, OpMax());
-                        if (lane < CN) mi->red[(cb * CN + lane) * 4 + q4] = cm;
+                        if (lane < CN) mi->redmax[(cb * CN + lane) * 4 + q4] = cm;
                     }
                     bar_sync_softmax();
 #pragma unroll
                     for (int h = 0; h < N; ++h) {
-                        const float4 r4 = *reinterpret_cast<const float4 *>(&mi->red[h * 4]);
+                        const float4 r4 = *reinterpret_cast<const float4 *>(&mi->redmax[h * 4]);
                         mn[h] = fmaxf(m_ref[h], fmaxf(fmaxf(r4.x, r4.y), fmaxf(r4.z, r4.w)));
                     }
                     if (i > 0) {
@@ -392,12 +643,12 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
 #pragma unroll
                         for (int c = 0; c < N; c += 16) {
                             uint32_t o[16];
-                            tmem_ld16(tl + 2 * N + c, o);
+                            tmem_ld16(tl + (2 + ob) * N + c, o);
                             tmem_wait_ld();
 #pragma unroll
                             for (int j = 0; j < 16; ++j)
                                 o[j] = __float_as_uint(__uint_as_float(o[j]) * ex2_ftz(m_ref[c + j] - mn[c + j]));
-                            tmem_st16(tl + 2 * N + c, o);
+                            tmem_st16(tl + (2 + ob) * N + c, o);
                         }
                         tmem_wait_st();
                         tc_fence_before();
@@ -407,7 +658,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                         l_part[h] *= ex2_ftz(m_ref[h] - mn[h]);       // 2^(-inf) = 0 on the first slice (l_part is 0 there)
                         m_ref[h] = mn[h];
                     }
-                    bar_sync_softmax();        // red[] may be rewritten (end of tile) only after every thread has read it
+                    bar_sync_softmax();        // redmax[] may be rewritten only after every thread has read it
                 }
                 uint32_t pw[N / 2];
 #pragma unroll
@@ -444,81 +695,110 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             gs += (uint32_t)n;
             if (tid == 64) kt_stamp(p, 4);
 
-            // ---- end of tile: row sums (fixed tree), then O^T from TMEM (thread = value column st)
+            // ---- end of tile: row sums (fixed tree) and references into this O buffer's hand-over area,
+            // which the epilogue of tile tc - 2 must have read
+            if (tc >= 2) mbar_wait(smem_u32(&mi->o_free[ob]), ((tc >> 1) - 1) & 1);
 #pragma unroll
             for (int cb = 0; cb < NB; ++cb) {
                 float v[CN];
 #pragma unroll
                 for (int h = 0; h < CN; ++h) v[h] = l_part[cb * CN + h];
                 const float s = col_reduce<CN>(v, lane, OpAdd());
-                if (lane < CN) mi->red[(cb * CN + lane) * 4 + q4] = s;
+                if (lane < CN) mi->red[ob][(cb * CN + lane) * 4 + q4] = s;
             }
-            bar_sync_softmax();
-            {
-                const uint32_t gl = gs - 1;
-                mbar_wait(smem_u32(&mi->p_done[gl & 1]), (gl >> 1) & 1);      // all value MMAs of the tile are complete
-                tc_fence_after();
-            }
-            const bool final_out = d.n_splits == 1;
-            float *dst = final_out ? p.out + d.out_off + st
-                                   : p.workspace + d.part_off + part_o_off(0, d.split, d.n_splits, KT_D) + st;
-            const int64_t hstride = final_out ? KT_D : (int64_t)d.n_splits * KT_D;
-#pragma unroll
-            for (int c = 0; c < N; c += 16) {
-                uint32_t o[16];
-                tmem_ld16(tl + 2 * N + c, o);
-                tmem_wait_ld();
-#pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const int h = c + j;
-                    if (h < d.gsize) {
-                        if (final_out) {
-                            const float4 r4 = *reinterpret_cast<const float4 *>(&mi->red[h * 4]);
-                            dst[h * hstride] = __uint_as_float(o[j]) / ((r4.x + r4.y) + (r4.z + r4.w));
-                        } else {
-                            __stcg(dst + h * hstride, __uint_as_float(o[j]));
-                        }
-                    }
-                }
-            }
-            tc_fence_before();
-            // (m, l) of row st, written by the thread whose index is the row
-            if (st < d.gsize) {
+            if (q4 == 0) {
                 float mr = 0.f;
 #pragma unroll
-                for (int h = 0; h < N; ++h) mr = (h == st) ? m_ref[h] : mr;
-                const float4 r4 = *reinterpret_cast<const float4 *>(&mi->red[st * 4]);
-                const float L = (r4.x + r4.y) + (r4.z + r4.w);
-                if (final_out)
-                    p.lse[d.lse_off + st] = (mr + log2f(L)) * 0.6931471805599453f;
-                else
-                    __stcg(reinterpret_cast<float2 *>(p.workspace + d.part_off + part_ml_off(d.gsize, st, d.split, d.n_splits, KT_D)),
-                           make_float2(mr, L));
+                for (int h = 0; h < N; ++h) mr = (h == lane) ? m_ref[h] : mr;
+                if (lane < N) mi->mref[ob][lane] = mr;
             }
-            if (!final_out) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&mi->e_full[ob]));           // release; the epilogue warps acquire
+            ++tc;
+        }
+    } else {
+        // =========================================================== epilogue warps (thread = value column d)
+        const int q4 = warp & 3;
+        const int dcol = q4 * 32 + lane;
+        const uint32_t tl = tmem + ((uint32_t)(q4 * 32) << 16);
+        uint32_t qi = 0, tc = 0;
+        for (;;) {
+            const uint32_t qs = qi % KT_TQ;
+            mbar_wait(smem_u32(&mi->tq_full[qs]), (qi / KT_TQ) & 1);
+            const KtDesc d = mi->tq[qs];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&mi->tq_empty[qs]));
+            ++qi;
+            if (d.item < 0) break;
+            const uint32_t ob = tc & 1, ph = (tc >> 1) & 1;
+            mbar_wait(smem_u32(&mi->e_full[ob]), ph);        // row sums and references are there
+            mbar_wait(smem_u32(&mi->o_done[ob]), ph);        // every value MMA of the tile is complete
+            tc_fence_after();
+            uint32_t o[N];
+#pragma unroll
+            for (int c = 0; c < N; c += 16)
+                tmem_ld16(tl + (2 + ob) * N + c, *reinterpret_cast<uint32_t (*)[16]>(&o[c]));
+            const bool final_out = d.n_splits == 1;
+            // row sum of head h: the four softmax warps' parts in a fixed order
+            float Lh = 1.f, mr = 0.f;
+            if (dcol < d.gsize) {
+                const float4 r4 = *reinterpret_cast<const float4 *>(&mi->red[ob][dcol * 4]);
+                Lh = (r4.x + r4.y) + (r4.z + r4.w);
+                mr = mi->mref[ob][dcol];
+            }
+            float inv[N];
+            if (final_out) {
+#pragma unroll
+                for (int h = 0; h < N; ++h) {
+                    const float4 r4 = *reinterpret_cast<const float4 *>(&mi->red[ob][h * 4]);
+                    inv[h] = 1.0f / ((r4.x + r4.y) + (r4.z + r4.w));
+                }
+            }
+            tmem_wait_ld();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&mi->o_free[ob]));           // O^T buffer and hand-over area are free
+            if (final_out) {
+                float *dst = p.out + d.out_off + dcol;
+#pragma unroll
+                for (int h = 0; h < N; ++h)
+                    if (h < d.gsize) dst[h * KT_D] = __uint_as_float(o[h]) * inv[h];
+                if (dcol < d.gsize) p.lse[d.lse_off + dcol] = (mr + log2f(Lh)) * 0.6931471805599453f;
+            } else {
+                // O partial of head h, split s, column c: [h][c / (4 CQ)][s][(c / 4) % CQ][c % 4] with
+                // CQ = 32 >> zl column quads per combine unit, so that the 32 lanes of a combine unit -- 2^zl
+                // split lanes x CQ quads -- read 512 contiguous bytes
+                const int cq_log2 = 5 - d.zl, quad = dcol >> 2;
+                float *dst = p.workspace + d.part_off +
+                             ((((int64_t)(quad >> cq_log2) * d.n_splits + d.split) << cq_log2) + (quad & ((1 << cq_log2) - 1))) * 4 + (dcol & 3);
+                const int64_t hstride = (int64_t)d.n_splits * KT_D;
+#pragma unroll
+                for (int h = 0; h < N; ++h)
+                    if (h < d.gsize) __stcg(dst + h * hstride, __uint_as_float(o[h]));
+                // (m, l) of row dcol, written by the thread whose index is the row
+                if (dcol < d.gsize)
+                    __stcg(reinterpret_cast<float2 *>(p.workspace + d.part_off + part_ml_off(d.gsize, dcol, d.split, d.n_splits, KT_D)),
+                           make_float2(mr, Lh));
                 // the warp's partial stores happen-before lane 0's gpu-scope release (cumulative over the
-                // __syncwarp), which the combine units acquire: no membar needed
+                // __syncwarp), which the combine acquires: no membar needed
                 __syncwarp();
-                if (lane == 0) red_release_add(p.group_counters + (size_t)d.group_idx * kCounterStride, 1);
+                if (lane == 0 && d.gsize > 0) red_release_add(p.group_counters + (size_t)d.group_idx * kCounterStride, 1);
             }
-            bar_sync_softmax();            // red[] is rewritten by the next tile's first slice
-            if (tid == 64) kt_stamp(p, 5);
+            if (tid == 192) kt_stamp(p, 5);
+            ++tc;
         }
     }
-    // ---- LSE combine (step a4): warp-sized units, statically assigned to ALL warps of every CTA.  The
-    // barrier orders it after this CTA's last tile (every slice consumed, every MMA complete), so the
-    // slice stages can serve as the warps' scratch.  A unit only waits for tiles that are already
-    // running on some SM, so the spin inside terminates.
+    // ---- LSE combine (step a4): warp-sized units, statically assigned to ALL warps of every CTA
     __syncthreads();
     if (tid == 0) kt_stamp(p, 6);
-    {
-        float *wsm = reinterpret_cast<float *>(smem) + warp * kMaxSplits;
-        combine_units<8>(p, blockIdx.x * KT_WARPS + warp, gridDim.x * KT_WARPS, wsm, lane);
-    }
+    kt_combine(p, warp, lane);
     tc_fence_before();
     __syncthreads();
     if (tid == 0) kt_stamp(p, 7);
-    if (warp == 1) tmem_dealloc(tmem, kt_tmem_cols(N));
+    if (warp == 2) {
+        tmem_dealloc(tmem, kt_tmem_cols(N));
+        if (lane == 0) kt_stamp(p, 15);
+    }
 }
 
 // ----------------------------------------------------------------------------- host side
@@ -546,13 +826,12 @@ static cudaError_t launch_kvt_n(const DecodeParams &p, const CUtensorMap &tmap, 
     return cudaGetLastError();
 }
 
-cudaError_t launch_decode_kvt(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas, int max_group,
+// grid: the number of CTAs the plan's static tile lists were laid out for (slot j of CTA b is record
+// j * grid + b); CTAs beyond the tiles still help with the combine units.
+cudaError_t launch_decode_kvt(const DecodeParams &p, const void *tmap, int rows_per_page, int grid, int max_group,
                               cudaStream_t stream)
 {
     const CUtensorMap &tm = *reinterpret_cast<const CUtensorMap *>(tmap);
-    int grid = p.n_tiles > (p.n_combine_units + KT_WARPS - 1) / KT_WARPS
-                   ? p.n_tiles : (p.n_combine_units + KT_WARPS - 1) / KT_WARPS;
-    if (grid > n_ctas) grid = n_ctas;
     if (grid < 1) grid = 1;
     switch (kvt_pad_rows(max_group)) {
     case 16: return launch_kvt_n<16>(p, tm, rows_per_page, grid, stream);

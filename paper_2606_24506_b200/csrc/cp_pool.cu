@@ -63,6 +63,8 @@ struct KindPlan {
     int max_group = 0;
     bool all_fast = false;           // every group of this kind runs on the tensor-core kernel
     bool use_kvt = false;            // KV kind: the tcgen05 tokens-on-M kernel (else the mma.sync kernel)
+    int grid = 0;                    // tcgen05 K/V kernel: CTAs the static tile lists were laid out for
+    int n_static_slots = 0;          // ... and the length of the static section of tile_recs (rounds * grid)
     bool uploaded = false;
     int counter_set = 0;             // scheduler counter set the next launch uses (alternates)
     int extra_counters = 0;          // multi-stage plans: one completion counter per stage after the groups'
@@ -97,6 +99,8 @@ struct cp_pool {
 
     // options
     int opt_kernel = 0, opt_num_ctas = 0, opt_waves_x16 = 16, opt_min_tile_pages = 2;
+    int opt_static_pct = 100;            // tcgen05 K/V kernel: share of every group's slices in the static (equal) pieces
+    int opt_tail_slices = 2;             // ... and the length of the dynamically popped tiles that hold the rest
 
     // query tokens per request of the call in progress (cp_decode_attention_qlen), and of the cached plan
     int qlen = 1, plan_qlen = 1;
@@ -162,6 +166,207 @@ bool model_supported(const cp_model_cfg &m, uint32_t P, uint32_t page_bytes)
     return need <= page_bytes;
 }
 
+
+// ----------------------------------------------------------------------------- planner, tcgen05 K/V kernel
+// Step a1 for the tokens-on-M kernel.  The unit of work is a 128-token slice.  Every (request, kv
+// head) group gives its first static_pct % slices to the STATIC part: the groups' static slices,
+// laid end to end, are cut into n_ctas * waves pieces of equal length (the boundaries ignore the
+// groups, as in a stream-K decomposition of a GEMM), piece j goes to CTA j mod n_ctas, and a
+// piece that spans several groups becomes several tiles that its CTA runs one after the other
+// (the kernel overlaps a tile's epilogue with the next tile's stream, so a tile boundary costs
+// no bandwidth).  Equal pieces take away the 10 % spread that "near-equal splits of every
+// group" leave between the CTAs' byte counts (cfg2: 64..78 pages per tile).  What remains of a
+// group forms short TAIL tiles of tail_slices slices that the CTAs pop from one counter when
+// their static lists are done: the SMs' streaming rates differ by a few per cent, and the tail
+// lets the fast ones take more.  Every tile is a fixed token range with its own split slot, so
+// results do not depend on which CTA runs it (deterministic).
+void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint64_t &ws)
+{
+    const int P = (int)pool->P;
+    const int pps = 128 / P;                                   // pages per slice
+    const int n_ctas = std::max(1, std::min(pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm, pool->n_sm));
+    struct GInfo { int b, c, n_lp, n_sl, s_static; };
+    std::vector<GInfo> gi;
+    for (int b = 0; b < n; ++b) {
+        const Request &r = pool->reqs[ids[b]];
+        const cp_model_cfg &m = pool->models[r.model];
+        if (m.kind != CP_KIND_KV) continue;
+        const int n_lp = ceil_div(r.ctx, P), n_sl = ceil_div(n_lp, pps);
+        int st = (int)((int64_t)n_sl * pool->opt_static_pct / 100);
+        if (n_sl - st < 1 || pool->opt_static_pct >= 100) st = n_sl;
+        for (int c = 0; c < m.n_kv_heads; ++c) gi.push_back(GInfo{b, c, n_lp, n_sl, st});
+        kp.max_dk = std::max(kp.max_dk, m.head_dim_qk);
+        kp.max_dv = std::max(kp.max_dv, m.head_dim_v);
+    }
+    const int ng = (int)gi.size();
+    int64_t S = 0;
+    for (const GInfo &g : gi) S += g.s_static;
+    const int min_sl = std::max(1, ceil_div(pool->opt_min_tile_pages, pps));
+    int64_t want_pieces = std::max<int64_t>(1, (int64_t)n_ctas * pool->opt_waves_x16 / 16);
+
+    struct T { int g, sl0, sl1, piece; };                      // tile: slices [sl0, sl1) of group g; piece < 0: tail tile
+    std::vector<T> tl;
+    std::vector<int> n_static_of(ng), n_tail_of(ng), tail_len(ng);
+    for (;;) {
+        tl.clear();
+        std::fill(n_static_of.begin(), n_static_of.end(), 0);
+        const int64_t n_pieces = std::max<int64_t>(1, std::min<int64_t>(want_pieces, S));
+        // cut positions in static-slice coordinates, snapped to a group boundary when they would leave
+        // a fragment shorter than the minimum tile
+        std::vector<int64_t> cut(n_pieces + 1);
+        {
+            std::vector<int64_t> gstart(ng + 1, 0);
+            for (int g = 0; g < ng; ++g) gstart[g + 1] = gstart[g] + gi[g].s_static;
+            int g = 0;
+            for (int64_t j = 0; j <= n_pieces; ++j) {
+                int64_t c = S * j / n_pieces;
+                while (g < ng && gstart[g + 1] <= c && g + 1 < ng) ++g;
+                if (j > 0 && j < n_pieces) {
+                    if (c - gstart[g] < min_sl) c = gstart[g];
+                    else if (gstart[g + 1] - c < min_sl) c = gstart[g + 1];
+                }
+                cut[j] = j > 0 ? std::max(c, cut[j - 1]) : 0;
+            }
+            cut[n_pieces] = S;
+        }
+        {
+            int g = 0;
+            int64_t gs0 = 0;                                   // static coordinate of group g's first slice
+            for (int64_t j = 0; j < n_pieces; ++j) {
+                int64_t a = cut[j];
+                const int64_t e = cut[j + 1];
+                while (a < e) {
+                    while (g < ng && gs0 + gi[g].s_static <= a) { gs0 += gi[g].s_static; ++g; }
+                    const int64_t ge = gs0 + gi[g].s_static;
+                    const int64_t stop = std::min(e, ge);
+                    tl.push_back(T{g, (int)(a - gs0), (int)(stop - gs0), (int)j});
+                    n_static_of[g]++;
+                    a = stop;
+                }
+            }
+        }
+        bool ok = true;
+        for (int g = 0; g < ng; ++g) {
+            const int rest = gi[g].n_sl - gi[g].s_static;
+            int tlen = std::max(pool->opt_tail_slices, 1);
+            const int room = kMaxSplits - n_static_of[g];
+            if (rest > 0 && room < 1) ok = false;
+            else if (rest > 0) tlen = std::max(tlen, ceil_div(rest, room));
+            tail_len[g] = tlen;
+            n_tail_of[g] = rest > 0 ? ceil_div(rest, tlen) : 0;
+            if (n_static_of[g] > kMaxSplits) ok = false;
+        }
+        if (ok || want_pieces == 1) break;
+        want_pieces = std::max<int64_t>(1, want_pieces / 2);
+    }
+    const int n_static_tiles = (int)tl.size();
+    for (int g = 0; g < ng; ++g)
+        for (int t = 0; t < n_tail_of[g]; ++t) {
+            const int a = gi[g].s_static + t * tail_len[g];
+            tl.push_back(T{g, a, std::min(a + tail_len[g], gi[g].n_sl), -1});
+        }
+
+    // groups, split slots (in token order: static tiles, then tail tiles), combine units
+    std::vector<int> split_base(ng, 0);
+    for (int g = 0; g < ng; ++g) {
+        const GInfo &G = gi[g];
+        const Request &r = pool->reqs[ids[G.b]];
+        const cp_model_cfg &m = pool->models[r.model];
+        const int hpk = m.n_q_heads / m.n_kv_heads;
+        const int ns = n_static_of[g] + n_tail_of[g];
+        kp.max_splits = std::max(kp.max_splits, ns);
+        Group gr;
+        gr.req = ids[G.b]; gr.model = r.model; gr.kv_head = G.c; gr.n_splits = ns;
+        gr.n_pages = G.n_lp; gr.batch_index = G.b;
+        gr.q_off = pool->q_off[G.b] + (int64_t)G.c * hpk * m.head_dim_qk;
+        gr.out_off = pool->out_off[G.b] + (int64_t)G.c * hpk * m.head_dim_v;
+        gr.lse_off = pool->lse_off[G.b] + (int64_t)G.c * hpk;
+        gr.part_off = 0;
+        if (ns > 1) {
+            gr.part_off = (int64_t)ws;
+            ws += (uint64_t)part_group_floats(hpk, ns, m.head_dim_v);
+            const int zl = ns <= 8 ? 0 : (ns <= 32 ? 3 : (ns <= 128 ? 4 : 5));
+            const int cols = 128 >> zl;
+            for (int h = 0; h < hpk; ++h) {
+                kp.combines.push_back(Combine{g, h});
+                for (int c0 = 0; c0 < m.head_dim_v; c0 += cols) {
+                    CombineUnit cu;
+                    std::memset(&cu, 0, sizeof(cu));
+                    // partial layout of this kernel: [h][c0 / cols][s][cols] (the unit's 512-byte reads are contiguous)
+                    cu.part_off = gr.part_off + (int64_t)h * ns * m.head_dim_v + (int64_t)(c0 / cols) * ns * cols;
+                    cu.ml_off = gr.part_off + part_ml_off(hpk, h, 0, ns, m.head_dim_v);
+                    cu.out_off = gr.out_off + (int64_t)h * m.head_dim_v + c0;
+                    cu.lse_off = c0 == 0 ? gr.lse_off + h : -1;
+                    cu.split_stride = cols;
+                    cu.n_splits = ns;
+                    cu.zl_log2 = zl;
+                    cu.want = ns * 4;                       // one arrival per epilogue warp and tile
+                    cu.group = g;
+                    kp.cunits.push_back(cu);
+                }
+            }
+        }
+        kp.groups.push_back(gr);
+    }
+    auto zl_of = [](int ns) { return ns <= 8 ? 0 : (ns <= 32 ? 3 : (ns <= 128 ? 4 : 5)); };
+    auto make_rec = [&](const T &t, int split) {
+        const GInfo &G = gi[t.g];
+        const Group &gr = kp.groups[t.g];
+        const cp_model_cfg &m = pool->models[gr.model];
+        TileRec r;
+        std::memset(&r, 0, sizeof(r));
+        r.group = t.g; r.req = gr.req; r.kv_head = gr.kv_head; r.n_kv_heads = m.n_kv_heads;
+        r.page_begin = t.sl0 * pps; r.n_pages = std::min(t.sl1 * pps, G.n_lp) - r.page_begin;
+        r.split = split; r.n_splits = gr.n_splits;
+        r.gsize = m.n_q_heads / m.n_kv_heads; r.n_q_heads = m.n_q_heads;
+        r.scale_log2 = (float)((double)m.softmax_scale * 1.4426950408889634);
+        r.q_off = gr.q_off; r.out_off = gr.out_off; r.lse_off = gr.lse_off; r.part_off = gr.part_off;
+        r.pad = zl_of(gr.n_splits) << 8;               // bits 8..15: partial layout; bit 0 (set below): another static slot follows
+        return r;
+    };
+    // split index of a tile = its rank inside the group by position (tl is in that order per group)
+    std::vector<int> split_of(tl.size());
+    for (size_t i = 0; i < tl.size(); ++i) split_of[i] = split_base[tl[i].g]++;
+
+    // device order: the CTAs' static lists interleaved (slot j of CTA b at j * grid + b), then the tail tiles, longest first
+    const int64_t n_pieces_used = n_static_tiles ? tl[n_static_tiles - 1].piece + 1 : 0;
+    int grid = (int)std::min<int64_t>(n_ctas, std::max<int64_t>(std::max<int64_t>(n_pieces_used, 1),
+                                                                 ((int64_t)kp.cunits.size() + 9) / 10));
+    if (tl.size() > (size_t)n_static_tiles) grid = n_ctas;          // dynamic tiles: every CTA may take some
+    std::vector<std::vector<int>> lists(grid);
+    for (int i = 0; i < n_static_tiles; ++i) lists[tl[i].piece % grid].push_back(i);
+    size_t rounds = 0;
+    for (const auto &l : lists) rounds = std::max(rounds, l.size());
+    if (n_static_tiles == 0) rounds = 0;
+    kp.tile_recs.assign(rounds * (size_t)grid, TileRec());
+    for (auto &r : kp.tile_recs) std::memset(&r, 0, sizeof(r));
+    std::vector<int> order;                                     // real tiles in device order (reporting)
+    for (size_t j = 0; j < rounds; ++j)
+        for (int b = 0; b < grid; ++b)
+            if (j < lists[b].size()) {
+                const int i = lists[b][j];
+                TileRec r = make_rec(tl[i], split_of[i]);
+                r.pad |= j + 1 < lists[b].size() ? 1 : 0;
+                kp.tile_recs[j * grid + b] = r;
+                order.push_back(i);
+            }
+    std::vector<int> tails;
+    for (size_t i = n_static_tiles; i < tl.size(); ++i) tails.push_back((int)i);
+    std::stable_sort(tails.begin(), tails.end(), [&](int a, int b) {
+        return (tl[a].sl1 - tl[a].sl0) > (tl[b].sl1 - tl[b].sl0);
+    });
+    for (int i : tails) {
+        kp.tile_recs.push_back(make_rec(tl[i], split_of[i]));
+        order.push_back(i);
+    }
+    for (int i : order) {
+        const TileRec r = make_rec(tl[i], split_of[i]);
+        kp.tiles.push_back(Tile{r.group, r.split, r.page_begin, r.page_begin + r.n_pages});
+    }
+    kp.grid = grid;
+    kp.n_static_slots = (int)(rounds * (size_t)grid);
+}
+
 // ----------------------------------------------------------------------------- planner
 // Step a1: cut every (request, kv head) group into page-aligned KV splits of near-equal
 // length so that the whole batch yields about n_ctas * waves tiles; tiles are ordered
@@ -219,6 +424,12 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         }
         kp.use_kvt = k == CP_KIND_KV && kp.all_fast && (pool->opt_kernel == 0 || pool->opt_kernel == 2) &&
                      pool->qlen == 1 && !pool->plan_for_stages && kvt_supported(P) && kvt_pad_rows(kp.max_group) > 0;
+        if (kp.use_kvt) {
+            kp.tile_recs.clear();
+            build_plan_kvt(pool, ids, n, kp, ws);
+            continue;
+        }
+        kp.grid = 0; kp.n_static_slots = 0;
         auto tiles_for = [&](int64_t len) {
             int64_t t = 0;
             for (int b = 0; b < n; ++b) {
@@ -781,6 +992,12 @@ cp_status cp_pool_set_option(cp_pool *pool, int32_t key, int64_t value)
     case CP_OPT_HOST_ZERO_COPY:
         if (value < 0 || value > 1) return CP_ERR_INVALID_ARG;
         pool->opt_host_zero_copy = (int)value; break;
+    case CP_OPT_STATIC_PCT:
+        if (value < 0 || value > 100) return CP_ERR_INVALID_ARG;
+        pool->opt_static_pct = (int)value; break;
+    case CP_OPT_TAIL_TILE_SLICES:
+        if (value < 1 || value > 4096) return CP_ERR_INVALID_ARG;
+        pool->opt_tail_slices = (int)value; break;
     case CP_OPT_TIMELINE:
         if (value < 0 || value > 1) return CP_ERR_INVALID_ARG;
         pool->opt_timeline = (int)value; return CP_OK;      // no effect on the plan
@@ -993,6 +1210,7 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.combines = (const Combine *)kp.d_combines.ptr;
         prm.cunits = (const CombineUnit *)kp.d_cunits.ptr;
         prm.n_tiles = (int)kp.tiles.size(); prm.n_combines = (int)kp.combines.size();
+        prm.n_static_slots = 0;
         prm.n_combine_units = prm.n_combines;
         prm.n_groups = (int)kp.groups.size();
         prm.q = (const uint16_t *)q_dev; prm.out = out_dev; prm.lse = lse_dev;
@@ -1017,8 +1235,9 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         cudaError_t e;
         if (k == CP_KIND_KV && kp.use_kvt && pool->kv_tmap_ok) {
             prm.n_combine_units = (int)kp.cunits.size();
-            e = launch_decode_kvt(prm, pool->kv_tmap, (int)(pool->page_bytes / 256), std::min(n_ctas, pool->n_sm),
-                                  kp.max_group, s);
+            prm.n_tiles = (int)kp.tile_recs.size();          // static slots (some empty) + dynamic tiles
+            prm.n_static_slots = kp.n_static_slots;
+            e = launch_decode_kvt(prm, pool->kv_tmap, (int)(pool->page_bytes / 256), kp.grid, kp.max_group, s);
         } else if (k == CP_KIND_KV && kp.use_kvt) {
             return CP_ERR_UNSUPPORTED;      // planned for the tcgen05 kernel but no tensor map (cannot happen: same conditions)
         } else if (k == CP_KIND_KV && pool->opt_kernel != 1 && kp.all_fast && pool->kv_tmap_ok) {
@@ -1268,6 +1487,7 @@ static cp_status decode_stages_core(cp_pool *pool, int32_t n_stages, const int32
     prm.combines = (const Combine *)kp.d_combines.ptr;
     prm.cunits = (const CombineUnit *)kp.d_cunits.ptr;
     prm.n_tiles = (int)kp.tiles.size(); prm.n_combines = 0;
+    prm.n_static_slots = 0;
     prm.n_combine_units = (int)kp.cunits.size();
     prm.n_groups = (int)kp.groups.size() + n_stages;           // counters the next launch's reset covers
     prm.q = (const uint16_t *)q_dev; prm.out = out_dev; prm.lse = lse_dev;

@@ -50,6 +50,10 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map
                  ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(policy)
                  : "memory");
 }
+__device__ __forceinline__ void prefetch_l2(const void *p)     // also fills the address translation of p's page
+{
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p) : "memory");
+}
 __device__ __forceinline__ void fence_proxy_async()      // generic-proxy smem writes -> async proxy (TMA, tcgen05)
 {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");

@@ -106,8 +106,8 @@ def test_map_unmap_ownership_and_budget():
     p.close()
 
 
-def _coverage(tiles, n_groups_expected, pages_of):
-    """every (batch, kv head) group's logical pages covered exactly once, splits contiguous"""
+def _coverage(tiles, n_groups_expected, pages_of, near_equal=True):
+    """every (batch, kv head) group's logical pages covered exactly once, splits contiguous and numbered in token order"""
     by_group = {}
     for (b, c, s, ns, p0, p1) in tiles:
         assert p1 > p0
@@ -122,14 +122,14 @@ def _coverage(tiles, n_groups_expected, pages_of):
             pos = p1
         assert pos == pages_of[b]
         lens = [x[3] - x[2] for x in lst]
-        assert max(lens) - min(lens) <= 1            # near-equal splits
+        if near_equal:
+            assert max(lens) - min(lens) <= 1            # near-equal splits
 
 
-def test_tile_plan_covers_every_page_once_and_balances():
+def _plan_pool():
     models = [ModelCfg(KIND_KV, 64, 8, 128, 128, 0.1), ModelCfg(KIND_KV, 16, 1, 128, 128, 0.1)]
     P = 32
     p = make_pool(P=P, num_pages=40000, models=models, max_requests=16, max_ppr=4096)
-    rng = np.random.default_rng(0)
     ctxs = [129, 4000, 65, 16000, 31, 2048, 9000]
     mids = [0, 1, 0, 1, 1, 0, 0]
     pages_of = {}
@@ -137,7 +137,14 @@ def test_tile_plan_covers_every_page_once_and_balances():
         n = -(-c // P) * models[m].n_kv_heads
         p.map_pages(i, m, None, c, n_allocate=n)
         pages_of[i] = -(-c // P)
-    ids = list(range(len(ctxs)))
+    return p, models, mids, pages_of
+
+
+def test_tile_plan_covers_every_page_once_and_balances():
+    """The near-equal-splits planner of the warp-MMA K/V kernel (CP_OPT_KERNEL = 3), the MLA and the generic kernels."""
+    p, models, mids, pages_of = _plan_pool()
+    p.set_option(cp.CP_OPT_KERNEL, 3)
+    ids = list(range(len(mids)))
     tiles, n_groups = p.decode_plan(ids)
     assert n_groups == sum(models[m].n_kv_heads for m in mids)
     _coverage(tiles, n_groups, pages_of)
@@ -175,13 +182,68 @@ def test_tile_plan_covers_every_page_once_and_balances():
     p.close()
 
 
+def test_tile_plan_of_the_tcgen05_kv_kernel_equal_pieces_and_tail():
+    """Default planner of the MQA/GQA path: the groups' 128-token slices laid end to end and cut
+    into n_ctas equal pieces whatever the group boundaries; with CP_OPT_STATIC_PCT < 100 the rest of every group
+    forms short tiles for the dynamic list.  Tiles come in device order: static slot j of CTA b at j * n_ctas + b
+    (empty slots are not reported), then the dynamic tiles, longest first."""
+    p, models, mids, pages_of = _plan_pool()
+    ids = list(range(len(mids)))
+    P, pps = 32, 4
+    tiles, n_groups = p.decode_plan(ids)
+    assert n_groups == sum(models[m].n_kv_heads for m in mids)
+    _coverage(tiles, n_groups, pages_of, near_equal=False)
+    slices = lambda t: -(-(t[5] - t[4]) // pps)
+    total = sum(-(-pages_of[i] // pps) * models[m].n_kv_heads for i, m in enumerate(mids))
+    # every tile but a group's last is a whole number of slices, and starts on a slice boundary of its group
+    for t in tiles:
+        assert t[4] % pps == 0
+        if t[2] != t[3] - 1:
+            assert (t[5] - t[4]) % pps == 0
+    # 148 pieces of floor/ceil(total / 148) slices: a piece is a run of consecutive tiles in token order, so the
+    # tiles, re-sorted by position, can be cut into 148 runs whose lengths differ by at most the snapping slack
+    assert sum(slices(t) for t in tiles) == total
+    assert len(tiles) >= 148 and len(tiles) <= 148 + n_groups
+    assert max(slices(t) for t in tiles) <= -(-total // 148) + 1
+    # a quarter of every group left to the dynamic list, in tiles of at most 2 slices
+    p.set_option(cp.CP_OPT_STATIC_PCT, 75)
+    p.set_option(cp.CP_OPT_TAIL_TILE_SLICES, 2)
+    tiles_t, _ = p.decode_plan(ids)
+    _coverage(tiles_t, n_groups, pages_of, near_equal=False)
+    n_tail = 0
+    for i, m in enumerate(mids):
+        n_sl = -(-pages_of[i] // pps)
+        rest = n_sl - n_sl * 75 // 100
+        n_tail += models[m].n_kv_heads * (-(-rest // 2) if rest >= 1 else 0)
+    tail = tiles_t[len(tiles_t) - n_tail:]
+    assert all(slices(t) <= 2 for t in tail)
+    assert [slices(t) for t in tail] == sorted((slices(t) for t in tail), reverse=True)
+    # a tail tile is the END of its group: every static tile of the group lies before it
+    first_tail = {}
+    for t in tail:
+        first_tail[(t[0], t[1])] = min(first_tail.get((t[0], t[1]), 1 << 30), t[4])
+    for t in tiles_t[:len(tiles_t) - n_tail]:
+        assert t[5] <= first_tail.get((t[0], t[1]), 1 << 30)
+    # few CTAs: the pieces follow the option, every CTA's share is equal to within one slice
+    p.set_option(cp.CP_OPT_STATIC_PCT, 100)
+    p.set_option(cp.CP_OPT_NUM_CTAS, 4)
+    tiles4, _ = p.decode_plan(ids)
+    _coverage(tiles4, n_groups, pages_of, near_equal=False)
+    assert len(tiles4) <= 4 + n_groups
+    p.set_option(cp.CP_OPT_MIN_TILE_PAGES, 64)        # cuts closer than 16 slices to a group boundary snap to it
+    tiles5, _ = p.decode_plan(ids)
+    _coverage(tiles5, n_groups, pages_of, near_equal=False)
+    assert all(slices(t) >= 16 for t in tiles5 if t[3] > 1)        # no sliver next to a group boundary
+    p.close()
+
+
 def test_workspace_bytes_formula():
     m = ModelCfg(KIND_KV, 32, 1, 128, 128, 0.1)
     p = make_pool(P=64, num_pages=5000, models=[m], max_requests=2, max_ppr=4096)
     p.map_pages(0, 0, None, 4096 * 64, n_allocate=4096)
     tiles, ng = p.decode_plan([0])
     ns = tiles[0][3]
-    assert ng == 1 and ns == len(tiles) and 74 <= ns <= 148     # one wave on 148 CTAs
+    assert ng == 1 and ns == len(tiles) and ns == 148           # one equal piece per CTA (2048 slices / 148)
     # per group: O[g][ns][d_v] + (m, l)[g][ns] floats (head-major partial layout, DESIGN.md §4)
     assert p.decode_workspace_bytes([0]) == ns * 32 * (128 + 2) * 4
     p.map_pages(1, 0, None, 64, n_allocate=1)       # single-tile request adds no workspace
