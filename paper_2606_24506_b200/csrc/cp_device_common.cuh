@@ -22,6 +22,13 @@ __device__ __forceinline__ int ld_acquire(const int32_t *p)
     return v;
 }
 
+__device__ __forceinline__ int ld_relaxed(const int32_t *p)
+{
+    int v;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
 __device__ __forceinline__ int ld_acquire_sys(const int32_t *p)
 {
     int v;

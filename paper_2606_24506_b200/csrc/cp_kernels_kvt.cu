@@ -55,7 +55,8 @@ constexpr int KT_SLICE = 128;                        // tokens per slice = MMA M
 constexpr int KT_SUBB = KT_SLICE * 128;              // one swizzled block: 128 rows x 128 B
 constexpr int KT_STAGE_BYTES = 4 * KT_SUBB;          // 65536
 constexpr int KT_TQ = 4;                             // tile-queue depth
-constexpr int KT_WARPS = 10;
+constexpr int KT_WARPS = 11;
+constexpr int KT_MQ = 3;                             // tile records the scheduler warp may run ahead of the producer
 constexpr int KT_THREADS = 32 * KT_WARPS;
 constexpr int KT_MISC_BYTES = 3072;
 constexpr int KT_SMEM_LIMIT = 232448;                // 227 KB opt-in maximum per CTA
@@ -82,6 +83,14 @@ struct KtDesc {                  // what the producer hands to the other warps f
     int64_t q_off, out_off, lse_off, part_off;
 };
 
+struct KtMeta {                  // what the scheduler warp hands to the producer for one tile
+    TileRec r;
+    int32_t ctx;
+    int32_t item;                // < 0: no more work
+    int32_t pid[32];             // the tile's first 32 physical pages
+};
+static_assert(sizeof(KtMeta) == 216, "KtMeta layout");
+
 struct KtMisc {
     uint64_t full[4], empty[4];                  // slice ring: TMA -> MMA, MMA (commit) -> TMA
     uint64_t s_full[2], s_empty[2];              // score buffers in TMEM: MMA -> softmax -> MMA
@@ -90,10 +99,13 @@ struct KtMisc {
     uint64_t o_done[2];                          // O^T buffer: every value MMA of the tile is complete (MMA commit)
     uint64_t e_full[2];                          // tile's row sums / references are in red[] / mref[] (4 softmax warps)
     uint64_t o_free[2];                          // epilogue has read O^T, red[], mref[] of the tile (4 epilogue warps)
-    uint64_t tq_full[KT_TQ], tq_empty[KT_TQ];
+    uint64_t q_full[2];                          // query buffers: the tile's rows have landed (cp.async of the scheduler warp)
+    uint64_t tq_full[KT_TQ], tq_empty[KT_TQ];    // tile descriptors: scheduler -> MMA, softmax, epilogue warps
+    uint64_t meta_full[KT_MQ], meta_empty[KT_MQ];   // tile records: scheduler -> producer
     KtDesc tq[KT_TQ];
+    KtMeta meta[KT_MQ];
     uint32_t tmem_base;
-    uint32_t pad[3];
+    uint32_t pad[1];
     float redmax[4 * KT_NMAX];                   // slice maxima when the reference moves: [row][warp]
     float red[2][4 * KT_NMAX];                   // per-tile row sums: [O buffer][row][warp]
     float mref[2][KT_NMAX];                      // per-tile exponent reference (log2 units): [O buffer][row]
@@ -108,7 +120,7 @@ __device__ __forceinline__ bool bar_red_or_softmax(bool pred)       // barrier 2
     return r != 0;
 }
 __device__ __forceinline__ void bar_sync_softmax() { asm volatile("bar.sync 2, 128;" ::: "memory"); }
-__device__ __forceinline__ void bar_sync_combine() { asm volatile("bar.sync 3, 320;" ::: "memory"); }
+__device__ __forceinline__ void bar_sync_combine() { asm volatile("bar.sync 3, 352;" ::: "memory"); }
 
 __device__ __forceinline__ void kt_stamp(const DecodeParams &p, int k)
 {
@@ -163,7 +175,7 @@ __device__ __forceinline__ TileRec load_tile_rec(const TileRec *recs, int item)
 // per lane, maxima and sums go through shuffles over the split-lane bits.
 // ---------------------------------------------------------------------------------------
 template <int KMAX>
-__device__ __forceinline__ void combine_one_unit(const DecodeParams &p, const CombineUnit &cu, const int lane, const int sb = 13)
+__device__ __forceinline__ void combine_one_unit(const DecodeParams &p, const CombineUnit &cu, const int lane)
 {
     const int ns = cu.n_splits;
     const int zl = cu.zl_log2;
@@ -180,15 +192,17 @@ __device__ __forceinline__ void combine_one_unit(const DecodeParams &p, const Co
         ml[k] = make_float2(-INFINITY, 0.f);
         v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
         if (s < ns) {
-            ml[k] = __ldcg(mlp + s);
-            v[k] = ld_cg_f4(src + (size_t)s * ss);
+            // plain (weak) loads: strong gpu-scope loads complete one after the other (measured: 16 of them
+            // take 1.5-2.4 us, 16 weak ones one L2 latency); the acquire fence of kt_combine orders them
+            ml[k] = mlp[s];
+            v[k] = *reinterpret_cast<const float4 *>(src + (size_t)s * ss);
         }
     }
     float M = -INFINITY;
 #pragma unroll
     for (int k = 0; k < KMAX; ++k) M = fmaxf(M, ml[k].x);
     for (int o = CQ; o < 32; o <<= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
-    if (threadIdx.x == 0) kt_stamp(p, sb);
+    if (threadIdx.x == 0) kt_stamp(p, 13);
     float L = 0.f;
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
@@ -204,7 +218,6 @@ __device__ __forceinline__ void combine_one_unit(const DecodeParams &p, const Co
         acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
         acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
     }
-    if (threadIdx.x == 0) kt_stamp(p, sb + 1);
     if (z == 0) {
         const float invL = 1.0f / L;
         *reinterpret_cast<float4 *>(p.out + cu.out_off + cq * 4) =
@@ -224,14 +237,14 @@ __device__ __noinline__ void combine_one_unit_long(const DecodeParams &p, const 
     const float *src = p.workspace + cu.part_off + cq * 4;
     const int ss = cu.split_stride;
     float M = -INFINITY;
-    for (int s = z; s < ns; s += ZL) M = fmaxf(M, __ldcg(mlp + s).x);
+    for (int s = z; s < ns; s += ZL) M = fmaxf(M, mlp[s].x);
     for (int o = CQ; o < 32; o <<= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
     float L = 0.f;
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 4
     for (int s = z; s < ns; s += ZL) {
-        const float2 ml = __ldcg(mlp + s);
-        const float4 v = ld_cg_f4(src + (size_t)s * ss);
+        const float2 ml = mlp[s];
+        const float4 v = *reinterpret_cast<const float4 *>(src + (size_t)s * ss);
         const float w = ex2_ftz(ml.x - M);
         L += w * ml.y;
         acc.x += w * v.x; acc.y += w * v.y; acc.z += w * v.z; acc.w += w * v.w;
@@ -271,15 +284,18 @@ __device__ __forceinline__ void kt_combine(const DecodeParams &p, const int warp
                 want = a.w;
                 ctr = p.group_counters + (size_t)grp * kCounterStride;
             }
+            // Relaxed gpu-scope polling, then ONE acquire fence (an acquire load would invalidate the L1 on every
+            // iteration): the writers' release (stores, fence, red) and this fence order the partials before
+            // the plain loads that follow the CTA barrier below.
             for (;;) {
-                const bool ok = ctr == nullptr || ld_acquire(ctr) >= want;
+                const bool ok = ctr == nullptr || ld_relaxed(ctr) >= want;
                 if (__all_sync(0xffffffffu, ok)) break;
                 __nanosleep(100);
             }
+            __threadfence();
             if (lane == 0) kt_stamp(p, 12);
         }
         bar_sync_combine();
-        if (threadIdx.x == 0) kt_stamp(p, 1);
         if (u < n) {
             const int per_lane = (cu.n_splits + (1 << cu.zl_log2) - 1) >> cu.zl_log2;
             if (per_lane <= 8) combine_one_unit<8>(p, cu, lane);
@@ -310,11 +326,11 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     const int P = (int)p.page_tokens;
     const int pps = KT_SLICE / P;                    // pages per slice
 
-    // the producer's first tile record is requested before anything else: its latency (the L2 is cold
+    // the scheduler's first tile record is requested before anything else: its latency (the L2 is cold
     // at the start of a step) runs under the barrier / tensor-memory set-up
     TileRec r_next;
     bool has_next = false;
-    if (warp == 0) {
+    if (warp == KT_WARPS - 1) {
         has_next = (int)blockIdx.x < p.n_static_slots;
         if (has_next) r_next = load_tile_rec(p.tile_recs, blockIdx.x);
     }
@@ -333,10 +349,11 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
         for (int i = 0; i < 2; ++i) {
             mbar_init(smem_u32(&mi->s_full[i]), 1); mbar_init(smem_u32(&mi->s_empty[i]), 4);
             mbar_init(smem_u32(&mi->p_full[i]), 4); mbar_init(smem_u32(&mi->p_done[i]), 1);
-            mbar_init(smem_u32(&mi->q_free[i]), 1);
+            mbar_init(smem_u32(&mi->q_free[i]), 1); mbar_init(smem_u32(&mi->q_full[i]), 32);
             mbar_init(smem_u32(&mi->o_done[i]), 1); mbar_init(smem_u32(&mi->e_full[i]), 4); mbar_init(smem_u32(&mi->o_free[i]), 4);
         }
         for (int i = 0; i < KT_TQ; ++i) { mbar_init(smem_u32(&mi->tq_full[i]), 1); mbar_init(smem_u32(&mi->tq_empty[i]), 9); }
+        for (int i = 0; i < KT_MQ; ++i) { mbar_init(smem_u32(&mi->meta_full[i]), 1); mbar_init(smem_u32(&mi->meta_empty[i]), 1); }
         asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap)) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_proxy_async();
@@ -348,89 +365,27 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     const uint32_t tmem = mi->tmem_base;
 
     if (warp == 0) {
-        // =========================================================== producer warp
+        // =========================================================== producer warp: pure TMA issue
         uint64_t policy;
         asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
         uint32_t gs = 0;          // slices issued by this CTA (ring position)
-        uint32_t qi = 0;          // work items pushed
-        int item_next = has_next ? (int)blockIdx.x : -3;     // -3: no static slot at all, start with the dynamic list
-        bool in_static = true;
-        int n_done = 0;
+        uint32_t ti = 0;          // tiles taken from the scheduler
         for (;;) {
-            // ---- the tile to run now (fetched during the previous tile) ...
-            int item = item_next;
-            TileRec r = r_next;
-            if (item >= 0 && r.n_pages == 0) item = -2;          // empty static slot of this CTA: skip, go dynamic
-            // ---- ... and the one after it: the next static slot of this CTA, else a pop from the dynamic list.
-            // The pop's result is not looked at before this tile's first pages are requested (resolve_next).
-            int nx_raw = -1;
-            bool nx_pending = false;
-            if (item != -1) {
-                if (in_static && item >= 0 && (r.pad & 1)) nx_raw = item + (int)gridDim.x;
-                else {
-                    in_static = false;
-                    if (lane == 0) nx_raw = atomicAdd(p.work_counter, 1) + p.n_static_slots;
-                    nx_pending = true;
-                }
-            }
-            auto resolve_next = [&]() {
-                int nx = nx_raw;
-                if (nx_pending) {
-                    nx = __shfl_sync(0xffffffffu, nx_raw, 0);
-                    if (nx >= p.n_tiles) nx = -1;
-                    nx_pending = false;
-                }
-                item_next = nx;
-                if (nx >= 0) r_next = load_tile_rec(p.tile_recs, nx);
-            };
-            if (item <= -2) { resolve_next(); continue; }
-            if (item == -1) {
-                // ---- no more work: the end marker goes through the same queue
-                const uint32_t qs = qi % KT_TQ;
-                mbar_wait(smem_u32(&mi->tq_empty[qs]), ((qi / KT_TQ) & 1) ^ 1);
-                if (lane == 0) {
-                    KtDesc d;
-                    d.item = -1; d.group_idx = 0; d.n_slices = 0; d.valid_last = KT_SLICE; d.split = 0; d.n_splits = 1;
-                    d.gsize = 1; d.scale_log2 = 0.f; d.q_off = d.out_off = d.lse_off = d.part_off = 0;
-                    mi->tq[qs] = d;
-                    mbar_arrive(smem_u32(&mi->tq_full[qs]));
-                }
-                break;
-            }
-            // ---- one round trip: the first 32 page ids (needed first: the tile's first pages are requested as
-            // soon as they are known), the context length (decides only how many tokens of the tile's LAST
-            // slice are valid: every planned page holds a valid token, contexts never shrink under a plan)
-            // and the query rows.  Volatile asm: issued here, in this order, not sunk to their first use.
-            int32_t pid0 = 0;
-            int ctx;
-            uint4 qv[N / 2];
-            if (lane < r.n_pages) {
-                if (p.slot_pages > 0) pid0 = r.req * p.slot_pages + (r.page_begin + lane) * r.n_kv_heads + r.kv_head;
-                else
-                    asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(pid0)
-                                 : "l"(p.page_table + (int64_t)r.req * p.max_ppr + (int64_t)(r.page_begin + lane) * r.n_kv_heads + r.kv_head));
-            }
-            asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(ctx) : "l"(p.req_ctx + r.req));
-            {
-                const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + r.q_off);
-#pragma unroll
-                for (int k = 0; k < N / 2; ++k) {
-                    const int id = lane + 32 * k;
-                    qv[k] = make_uint4(0u, 0u, 0u, 0u);
-                    if ((id >> 4) < r.gsize)
-                        asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(qv[k].x), "=r"(qv[k].y), "=r"(qv[k].z), "=r"(qv[k].w) : "l"(qg + id));
-                }
-            }
-            const int npg = r.n_pages;
-            const int hkv = r.n_kv_heads;
-            ++n_done;
+            const uint32_t ms = ti % KT_MQ;
+            mbar_wait(smem_u32(&mi->meta_full[ms]), (ti / KT_MQ) & 1);
+            const KtMeta *mt = &mi->meta[ms];
+            const int item = mt->item;
+            if (item < 0) break;
+            const int req = mt->r.req, hkv = mt->r.n_kv_heads, kvh = mt->r.kv_head, pb = mt->r.page_begin, npg = mt->r.n_pages;
+            int32_t pid = mt->pid[lane];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&mi->meta_empty[ms]));
+            ++ti;
             for (int j0 = 0; j0 < npg; j0 += 32) {
-                // translate up to 32 logical pages at once (step a2: one page-table entry per lane)
-                int32_t pid = pid0;
-                if (j0 > 0) {
-                    pid = 0;
-                    if (j0 + lane < npg) pid = page_of(p, r.req, (int64_t)(r.page_begin + j0 + lane) * hkv + r.kv_head);
-                }
+                // translation of the batch after this one (step a2: one page-table entry per lane) is requested
+                // now and looked at when this batch's pages have been issued
+                int32_t pid_nx = 0;
+                if (j0 + 32 + lane < npg) pid_nx = page_of(p, req, (int64_t)(pb + j0 + 32 + lane) * hkv + kvh);
                 const int nj = min(32, npg - j0);
                 for (int j = 0; j < nj; ++j) {
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);
@@ -450,46 +405,120 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                         if (gs == 0 && pg == 0) kt_stamp(p, 9);
                     }
                     if (pg == pps - 1 || jj == npg - 1) ++gs;
-                    if (jj == min(npg, pps) - 1) {
-                        // ---- the first slice is on its way: now hand the tile to the other warps.  Query rows ->
-                        // buffer (qi & 1): two K-major [N x 64] blocks, 128-byte swizzle (16-B chunk index ^
-                        // (row & 7)); rows beyond the group are zero.  The buffer is free once the score MMAs
-                        // of tile qi - 2 are complete.
-                        const int t_begin = r.page_begin * P;
-                        const int t_end = min((r.page_begin + r.n_pages) * P, ctx);
-                        const int n_slices = (t_end - t_begin + KT_SLICE - 1) / KT_SLICE;
-                        const int valid_last = t_end - t_begin - (n_slices - 1) * KT_SLICE;
-                        const uint32_t qs = qi % KT_TQ;
-                        mbar_wait(smem_u32(&mi->tq_empty[qs]), ((qi / KT_TQ) & 1) ^ 1);
-                        if (qi >= 2) mbar_wait(smem_u32(&mi->q_free[qi & 1]), ((qi >> 1) - 1) & 1);
-                        const uint32_t qb = q_base + (qi & 1) * kt_q_bytes(N);
-#pragma unroll
-                        for (int k = 0; k < N / 2; ++k) {
-                            const int id = lane + 32 * k;
-                            const int row = id >> 4, ch = id & 15;
-                            const uint32_t a = qb + (ch >> 3) * (N * 128) + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
-                            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(qv[k].x), "r"(qv[k].y), "r"(qv[k].z), "r"(qv[k].w) : "memory");
-                        }
-                        fence_proxy_async();
-                        __syncwarp();
-                        if (lane == 0) {
-                            KtDesc d;
-                            d.item = item; d.group_idx = r.group; d.n_slices = n_slices; d.valid_last = valid_last;
-                            d.split = r.split; d.n_splits = r.n_splits; d.gsize = r.gsize; d.scale_log2 = r.scale_log2;
-                            d.zl = (r.pad >> 8) & 0xff;
-                            d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
-                            mi->tq[qs] = d;
-                            mbar_arrive(smem_u32(&mi->tq_full[qs]));     // release: the consumers acquire via try_wait
-                        }
-                        ++qi;
-                        resolve_next();
-                    }
                 }
+                pid = pid_nx;
             }
         }
         if (lane == 0) {
             kt_stamp(p, 3);
-            if (p.timeline) p.timeline[(size_t)blockIdx.x * kTimelineSlots + 11] = (unsigned long long)n_done;
+            if (p.timeline) p.timeline[(size_t)blockIdx.x * kTimelineSlots + 11] = (unsigned long long)ti;
+        }
+    } else if (warp == KT_WARPS - 1) {
+        // =========================================================== scheduler warp (step a5): the control plane.
+        // Walks this CTA's static tile list, then pops the dynamic one; for every tile it fetches the record,
+        // the context length and the first 32 page ids, stages the query rows in shared memory (cp.async) and
+        // hands the tile to the producer (meta ring) and to the MMA / softmax / epilogue warps (tile queue),
+        // up to KT_MQ tiles ahead of the producer -- a dependent global load takes microseconds while 148 SMs
+        // stream at full rate, and none of them is on the producer's path.
+        int item = has_next ? (int)blockIdx.x : -3;          // -3: no static slot at all, start with the dynamic list
+        TileRec r = r_next;
+        bool in_static = true;
+        uint32_t ti = 0;
+        for (;;) {
+            if (item >= 0 && r.n_pages == 0) item = -2;      // empty static slot of this CTA: skip, go dynamic
+            // ---- the tile after this one: the next static slot of this CTA, else a pop from the dynamic list
+            // (the pop's result is looked at only after this tile's own loads have been issued)
+            int nx_raw = -1;
+            bool nx_pending = false;
+            if (item != -1) {
+                if (in_static && item >= 0 && (r.pad & 1)) nx_raw = item + (int)gridDim.x;
+                else {
+                    in_static = false;
+                    if (lane == 0) nx_raw = atomicAdd(p.work_counter, 1) + p.n_static_slots;
+                    nx_pending = true;
+                }
+            }
+            int item_next = -1;
+            auto resolve_next = [&]() {
+                int nx = nx_raw;
+                if (nx_pending) {
+                    nx = __shfl_sync(0xffffffffu, nx_raw, 0);
+                    if (nx >= p.n_tiles) nx = -1;
+                }
+                item_next = nx;
+                if (nx >= 0) r_next = load_tile_rec(p.tile_recs, nx);
+            };
+            if (item <= -2) { resolve_next(); item = item_next; r = r_next; continue; }
+            const uint32_t ms = ti % KT_MQ, qs = ti % KT_TQ;
+            if (item == -1) {
+                // ---- no more work: the end marker goes through both queues
+                mbar_wait(smem_u32(&mi->meta_empty[ms]), ((ti / KT_MQ) & 1) ^ 1);
+                mbar_wait(smem_u32(&mi->tq_empty[qs]), ((ti / KT_TQ) & 1) ^ 1);
+                if (lane == 0) {
+                    mi->meta[ms].item = -1;
+                    mi->tq[qs].item = -1;
+                    mbar_arrive(smem_u32(&mi->meta_full[ms]));
+                    mbar_arrive(smem_u32(&mi->tq_full[qs]));
+                }
+                break;
+            }
+            // ---- one round trip: the first 32 page ids and the context length (which decides only how many
+            // tokens of the tile's LAST slice are valid: every planned page holds a valid token, contexts never
+            // shrink under a plan).  Volatile asm: issued here, not sunk to their first use.
+            int32_t pid0 = 0;
+            int ctx;
+            if (lane < r.n_pages) {
+                if (p.slot_pages > 0) pid0 = r.req * p.slot_pages + (r.page_begin + lane) * r.n_kv_heads + r.kv_head;
+                else
+                    asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(pid0)
+                                 : "l"(p.page_table + (int64_t)r.req * p.max_ppr + (int64_t)(r.page_begin + lane) * r.n_kv_heads + r.kv_head));
+            }
+            asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(ctx) : "l"(p.req_ctx + r.req));
+            // ---- the tile's query rows -> buffer (ti & 1), asynchronously: two K-major [N x 64] blocks, 128-byte
+            // swizzle (16-B chunk index ^ (row & 7)); rows beyond the group are zero-filled.  The buffer is free
+            // once the score MMAs of tile ti - 2 are complete; q_full counts the 32 lanes' copies.
+            if (ti >= 2) mbar_wait(smem_u32(&mi->q_free[ti & 1]), ((ti >> 1) - 1) & 1);
+            {
+                const uint4 *qg = reinterpret_cast<const uint4 *>(p.q + r.q_off);
+                const uint32_t qb = q_base + (ti & 1) * kt_q_bytes(N);
+#pragma unroll
+                for (int k = 0; k < N / 2; ++k) {
+                    const int id = lane + 32 * k;
+                    const int row = id >> 4, ch = id & 15;
+                    const uint32_t a = qb + (ch >> 3) * (N * 128) + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
+                    const uint32_t nbytes = row < r.gsize ? 16u : 0u;
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a), "l"(qg + (row < r.gsize ? id : 0)), "r"(nbytes) : "memory");
+                }
+                asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(&mi->q_full[ti & 1])) : "memory");
+            }
+            resolve_next();
+            mbar_wait(smem_u32(&mi->meta_empty[ms]), ((ti / KT_MQ) & 1) ^ 1);
+            mbar_wait(smem_u32(&mi->tq_empty[qs]), ((ti / KT_TQ) & 1) ^ 1);
+            {
+                KtMeta *mt = &mi->meta[ms];
+                if (lane < 10) reinterpret_cast<uint2 *>(&mt->r)[lane] = reinterpret_cast<const uint2 *>(&r)[lane];   // KtMeta is 8-byte aligned
+                mt->pid[lane] = pid0;
+                if (lane == 0) {
+                    mt->ctx = ctx; mt->item = item;
+                    const int t_begin = r.page_begin * P;
+                    const int t_end = min((r.page_begin + r.n_pages) * P, ctx);
+                    const int n_slices = (t_end - t_begin + KT_SLICE - 1) / KT_SLICE;
+                    KtDesc d;
+                    d.item = item; d.group_idx = r.group; d.n_slices = n_slices;
+                    d.valid_last = t_end - t_begin - (n_slices - 1) * KT_SLICE;
+                    d.split = r.split; d.n_splits = r.n_splits; d.gsize = r.gsize; d.scale_log2 = r.scale_log2;
+                    d.zl = (r.pad >> 8) & 0xff; d.pad = 0;
+                    d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
+                    mi->tq[qs] = d;
+                }
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive(smem_u32(&mi->meta_full[ms]));   // release: the producer acquires via try_wait
+                    mbar_arrive(smem_u32(&mi->tq_full[qs]));
+                }
+            }
+            ++ti;
+            item = item_next; r = r_next;
         }
     } else if (warp == 1) {
         // =========================================================== MMA issuer warp
@@ -536,15 +565,9 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             if (d.item < 0) break;
             const uint32_t qb = q_base + (tc & 1) * kt_q_bytes(N);
             const int n = d.n_slices;
-            if (n == 0) {
-                // empty (warm-up) tile: nothing to multiply, the hand-overs still happen
-                if (pend) issue_pv();
-                if (elect_one()) {
-                    umma_commit(smem_u32(&mi->q_free[tc & 1]));
-                    umma_commit(smem_u32(&mi->o_done[tc & 1]));
-                }
-                __syncwarp();
-            }
+            // the tile's query rows (cp.async of the scheduler warp, generic proxy) must be visible to the tensor core
+            mbar_wait(smem_u32(&mi->q_full[tc & 1]), (tc >> 1) & 1);
+            fence_proxy_async();
             for (int i = 0; i < n; ++i) {
                 // ---- S_i^T = K_i Q^T into score buffer (g & 1)
                 const uint32_t g = gs + (uint32_t)i, slot = g % NS, b = g & 1;
@@ -716,7 +739,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             if (lane == 0) mbar_arrive(smem_u32(&mi->e_full[ob]));           // release; the epilogue warps acquire
             ++tc;
         }
-    } else {
+    } else if (warp < 10) {
         // =========================================================== epilogue warps (thread = value column d)
         const int q4 = warp & 3;
         const int dcol = q4 * 32 + lane;
@@ -774,15 +797,15 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 const int64_t hstride = (int64_t)d.n_splits * KT_D;
 #pragma unroll
                 for (int h = 0; h < N; ++h)
-                    if (h < d.gsize) __stcg(dst + h * hstride, __uint_as_float(o[h]));
+                    if (h < d.gsize) dst[h * hstride] = __uint_as_float(o[h]);
                 // (m, l) of row dcol, written by the thread whose index is the row
                 if (dcol < d.gsize)
-                    __stcg(reinterpret_cast<float2 *>(p.workspace + d.part_off + part_ml_off(d.gsize, dcol, d.split, d.n_splits, KT_D)),
-                           make_float2(mr, Lh));
+                    *reinterpret_cast<float2 *>(p.workspace + d.part_off + part_ml_off(d.gsize, dcol, d.split, d.n_splits, KT_D)) =
+                        make_float2(mr, Lh);
                 // the warp's partial stores happen-before lane 0's gpu-scope release (cumulative over the
                 // __syncwarp), which the combine acquires: no membar needed
                 __syncwarp();
-                if (lane == 0 && d.gsize > 0) red_release_add(p.group_counters + (size_t)d.group_idx * kCounterStride, 1);
+                if (lane == 0) red_release_add(p.group_counters + (size_t)d.group_idx * kCounterStride, 1);
             }
             if (tid == 192) kt_stamp(p, 5);
             ++tc;
@@ -795,10 +818,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     tc_fence_before();
     __syncthreads();
     if (tid == 0) kt_stamp(p, 7);
-    if (warp == 2) {
-        tmem_dealloc(tmem, kt_tmem_cols(N));
-        if (lane == 0) kt_stamp(p, 15);
-    }
+    if (warp == 2) tmem_dealloc(tmem, kt_tmem_cols(N));
 }
 
 // ----------------------------------------------------------------------------- host side

@@ -57,10 +57,14 @@ def run_and_compare(w, label="", options=None, heads=None):
             dw.pool.set_option(k, v)
         dw.out.fill_(float("nan"))
         dw.lse.fill_(float("nan"))
+        dw.ensure_workspace()
+        dw.ws.fill_(0xFF)            # split partials start as NaN: a combine that reads one too early shows
         dw.decode()
         got = dw.results()
-        # a second launch on the same pool must give the same bits (counters reset, determinism)
+        # a second launch on the same pool must give the same bits (counters reset, determinism); the
+        # workspace is poisoned again, so partials left by the first launch cannot stand in for late ones
         dw.out.fill_(float("nan"))
+        dw.ws.fill_(0xFF)
         dw.decode()
         got2 = dw.results()
         for (o, l), (o2, l2) in zip(got, got2):
@@ -123,7 +127,7 @@ SMALL = [
 
 
 @pytest.mark.parametrize("case", range(len(SMALL)))
-@pytest.mark.parametrize("kernel", [0, 1, 2])
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
 def test_attention_small(torch_cuda, case, kernel):
     import paper_2606_24506_b200 as cp
     models, rm, rc, P, shift = SMALL[case]
@@ -194,7 +198,7 @@ def test_rising_logits_move_the_softmax_reference(torch_cuda, kind):
         _add_logit_ramp(w, 0, 240.0, list(range(512, 576)))      # rope part only: values untouched
     ref_lse = oracle.decode_workload(w)[0][1]
     assert ref_lse.max() - ref_lse.min() >= 0 and ref_lse.max() > 30.0     # the ramp is really there
-    for kernel in (0, 1, 2):
+    for kernel in (0, 1, 2, 3):
         for mtp in (1, 100000):                                  # many short tiles / one tile per group
             worst = run_and_compare(w, "ramp_%s/k%d/mtp%d" % (kind, kernel, mtp),
                                     {cp.CP_OPT_KERNEL: kernel, cp.CP_OPT_MIN_TILE_PAGES: mtp})
@@ -202,7 +206,7 @@ def test_rising_logits_move_the_softmax_reference(torch_cuda, kind):
 
 
 @pytest.mark.parametrize("n_ctas", [2, 4, 6])
-@pytest.mark.parametrize("kernel", [0, 2])
+@pytest.mark.parametrize("kernel", [0, 2, 3])
 def test_few_ctas_many_tiles_per_cta(torch_cuda, n_ctas, kernel):
     """Persistent loops over many work items per CTA (or CTA pair): a grid of 2..6 CTAs on batches
     that yield dozens of tiles, with group changes in between (query restaging, ring phases across
@@ -474,6 +478,27 @@ def test_attention_full_config_generic_kernel(torch_cuda, k):
     w = W.config(k) if k == 2 else W.config3(ctx=(16384, 4096))
     worst = run_and_compare(w, "cfg%d-generic" % k, {cp.CP_OPT_KERNEL: 1})
     print("cfg%d generic: %s" % (k, worst))
+
+
+@pytest.mark.parametrize("k", [2, 4, 5])
+def test_attention_full_config_warp_mma_kernel(torch_cuda, k):
+    """The warp-MMA (mma.sync) K/V kernel of round 1 on full-size inputs (CP_OPT_KERNEL = 3): kept as the kernel of
+    the multi-stage and q_len > 1 launches and as a second tensor-core cross-check of the tcgen05 kernel."""
+    import paper_2606_24506_b200 as cp
+    worst = run_and_compare(W.config(k), "cfg%d-warp-mma" % k, {cp.CP_OPT_KERNEL: 3})
+    print("cfg%d warp-MMA kernel: %s" % (k, worst))
+
+
+@pytest.mark.parametrize("k", [2, 4, 5])
+@pytest.mark.parametrize("pct,tail,waves", [(85, 2, 16), (60, 1, 16), (0, 3, 16), (100, 2, 40)])
+def test_attention_full_config_dynamic_tail(torch_cuda, k, pct, tail, waves):
+    """Full-size inputs with part of every group left to the dynamically popped tail tiles (CP_OPT_STATIC_PCT,
+    CP_OPT_TAIL_TILE_SLICES) and with several static rounds per CTA: results within the same bars, and -- since
+    every tile is a fixed token range with its own split slot -- identical bits on a relaunch whatever CTA ran it."""
+    import paper_2606_24506_b200 as cp
+    worst = run_and_compare(W.config(k), "cfg%d-tail%d/%d/%d" % (k, pct, tail, waves),
+                            {cp.CP_OPT_STATIC_PCT: pct, cp.CP_OPT_TAIL_TILE_SLICES: tail, cp.CP_OPT_WAVES_X16: waves})
+    print("cfg%d pct %d tail %d waves %d: %s" % (k, pct, tail, waves, worst))
 
 
 def test_attention_full_config_mla_single_cta_kernel(torch_cuda):

@@ -41,7 +41,9 @@ def draw_case(seed):
     rc = [max(1, c) for c in rc]
     if rng.random() < 0.5:
         rc[0] = int(rng.choice([1, P - 1, P, P + 1, 2 * P]))          # page-boundary contexts
-    opts = {cp.CP_OPT_KERNEL: int(rng.choice([0, 0, 1, 2])),
+    opts = {cp.CP_OPT_KERNEL: int(rng.choice([0, 0, 1, 2, 3])),
+            cp.CP_OPT_STATIC_PCT: int(rng.choice([100, 100, 80, 50, 0])),
+            cp.CP_OPT_TAIL_TILE_SLICES: int(rng.choice([1, 2, 5])),
             cp.CP_OPT_MIN_TILE_PAGES: int(rng.choice([1, 2, 4])),
             cp.CP_OPT_NUM_CTAS: int(rng.choice([0, 0, 3, 17, 100])),
             cp.CP_OPT_WAVES_X16: int(rng.choice([16, 8, 40]))}

@@ -150,6 +150,9 @@ def test_stages_alpha_zero_equal_single_steps_bit_for_bit(torch_cuda):
     dw = device_workload(w)
     try:
         dw.pool.set_option(cp.CP_OPT_MIN_TILE_PAGES, 1)
+        # the multi-stage launch runs on the warp-MMA K/V kernel: compare with the single step on the same kernel
+        # (the default single step is the tcgen05 kernel, whose tiling and summation order differ)
+        dw.pool.set_option(cp.CP_OPT_KERNEL, 3)
         got = run_stages(torch, dw, w, stages, deps, q_in, 0.0)
         for s, st in enumerate(stages):
             ids = np.array([w.requests[ri].request_id for ri in st], dtype=np.int32)
