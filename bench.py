@@ -4,13 +4,15 @@
 A "step" is one pass of the whole hot path (translation + split-KV partial attention + LSE
 combine, all inside one persistent launch) over one synthetic batch: one
 cp_decode_attention call.  Default workload: BASELINE.json configs[1], the shared pool of
-4 cold GQA models (344 MB of KV per step).  Before every timed step the L2 is flushed with a read-only
-pass over 512 MB (no dirty lines left behind); the back-to-back number beside it has no flush.
+4 cold GQA models (344 MB of KV per step = 2.7 x the 126 MB L2): K steps back to back inside one
+CUDA-event pair; the same steps with a read-only L2 flush before each are reported beside it, and the
+other four BASELINE configs go through the same protocol in the `per_config` block (class StepTimer).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+                    [--probe timeline|stream|launch]
 
-Prints ONE JSON line (see DESIGN.md §7 for every field).  N > 1 = independent replicas
-(the path does not shard: BASELINE north_star fixes one GPU, DESIGN.md §8).
+Prints ONE JSON line (see DESIGN.md 7 for every field).  N > 1 = independent replicas
+(the path does not shard: BASELINE north_star fixes one GPU, DESIGN.md 8).
 """
 from __future__ import annotations
 
@@ -69,8 +71,9 @@ def workload_desc(w, k):
     return {"workload": "cfg%d:%s" % (k, w.name), "requests": len(w.requests),
             "tokens": w.total_tokens(), "page_tokens": w.page_tokens,
             "kv_bytes_per_step": w.algorithmic_bytes(), "flops_per_step": w.flops(),
-            "l2": "L2 flushed before every timed step (read-only pass over 512 MB, outside the per-step events); "
-                  "the back-to-back number has no flush"}
+            "l2": ("inputs %.0f MB > 2 x L2 (126 MB): K steps back to back, no flush; the flushed number is reported beside it"
+                   % (w.algorithmic_bytes() / 1e6)) if w.algorithmic_bytes() > 2 * L2_BYTES else
+                  "L2 flushed before every timed step (read-only pass over 512 MB, outside the step's event pair)"}
 
 
 class ClockSampler:
@@ -184,6 +187,155 @@ def run_reference(args, w, k):
     print(json.dumps(line))
 
 
+class StepTimer:
+    """Timing protocol of one workload.  All numbers come from CUDA events on the launching stream.
+
+    region      K steps back to back inside ONE event pair: the contract's number.  Legitimate as an HBM
+                measurement only when a step's inputs exceed the L2 (126 MB) several times over, so that nothing
+                of step i is left when step i + 1 asks for it (cfg2, cfg3, cfg5).
+    flushed     every step bracketed by its own event pair, a read-only pass over 512 MB (clean lines only: a
+                write would leave dirty lines the timed kernel has to evict) and a short device-side spin
+                before it; p10 / p50 / p90, p50 is "the" flushed number.  The number for inputs near or below
+                the L2 size (cfg1, cfg4); reported for every config.  An event pair around an EMPTY kernel
+                already reads ~6 us on this box and a kernel boundary inside a region ~2 us (both measured
+                beside it: empty_kernel_events_us, empty_kernel_region_us), so a flushed number carries ~4 us that a
+                region number does not; flushed_calibrated_us subtracts that difference and is reported
+                only as a reading aid.
+    device      %globaltimer stamps written by the kernel itself (CP_OPT_TIMELINE): first CTA entry to last
+                CTA exit of flushed steps; where the launch and event overheads are not.
+    """
+
+    def __init__(self, torch, cp, dev, stream):
+        self.torch, self.cp, self.dev, self.stream = torch, cp, dev, stream
+        self.flush_buf = torch.zeros(512 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)
+        self.flush_sink = torch.zeros((), dtype=torch.float32, device=dev)
+        self.stamp = torch.zeros(2, dtype=torch.int64, device=dev)
+        self.event_overhead_us = 0.0      # empty_kernel_events_us - empty_kernel_region_us, set by the caller
+
+    def l2_flush(self):
+        self.torch.sum(self.flush_buf, dim=(0,), out=self.flush_sink)
+
+    def _region(self, steps, fn):
+        torch = self.torch
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        torch.cuda._sleep(4000000)          # ~2 ms: the host enqueues the whole region behind a device-side spin
+        e0.record()
+        for i in range(steps):
+            fn(i)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps  # ms per step
+
+    def region(self, steps, step_fn):
+        return self._region(steps, lambda i: step_fn())
+
+    def per_step(self, steps, step_fn):
+        torch = self.torch
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * steps)]
+        torch.cuda.synchronize()
+        for i in range(steps):
+            self.l2_flush()
+            torch.cuda._sleep(100000)       # ~50 us: keeps the host a step ahead
+            ev[2 * i].record()
+            step_fn()
+            ev[2 * i + 1].record()
+        torch.cuda.synchronize()
+        return [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(steps)]
+
+    def empty_kernel_events_us(self, reps=20):
+        """What an event pair around a one-thread kernel reads: the floor of every per-step number."""
+        return 1e3 * float(np.median(self.per_step(reps, lambda: self.cp.probe_globaltimer(self.stamp, self.stream))))
+
+    def empty_kernel_region_us(self, reps=50):
+        """Back-to-back one-thread kernels inside one event pair: what a kernel boundary costs."""
+        return 1e3 * self.region(reps, lambda: self.cp.probe_globaltimer(self.stamp, self.stream))
+
+
+TL = {"entry": 0, "first_tma": 9, "first_slice_landed": 2, "last_page_issued": 3, "last_slice_landed": 10,
+      "softmax_done": 4, "published": 5, "poll_ok": 12, "partials_loaded": 13, "combine_done": 7}
+
+
+def device_timeline(timer, dw, cp, reps=5):
+    """Per-CTA %globaltimer stamps of flushed steps of the tcgen05 K/V kernel (cp_pool_read_timeline): kernel
+    duration on the device and where it goes, as [min, median, max] over the CTAs, us after the first CTA's entry."""
+    torch = timer.torch
+    dw.pool.set_option(cp.CP_OPT_TIMELINE, 1)
+    dur, phases = [], {k: [] for k in TL}
+    try:
+        for _ in range(reps):
+            timer.l2_flush()
+            torch.cuda._sleep(100000)
+            dw.decode()
+            torch.cuda.synchronize()
+            t = dw.pool.read_timeline().astype(np.int64)
+            t = t[t[:, 0] > 0]
+            if t.size == 0 or t[:, 7].max() == 0:
+                return None                 # a kernel that does not stamp
+            t0 = t[:, 0].min()
+            dur.append((t[:, 7].max() - t0) / 1e3)
+            for name, slot in TL.items():
+                col = t[:, slot][t[:, slot] > 0]
+                if col.size:
+                    phases[name].append([(col.min() - t0) / 1e3, (float(np.median(col)) - t0) / 1e3, (col.max() - t0) / 1e3])
+    finally:
+        dw.pool.set_option(cp.CP_OPT_TIMELINE, 0)
+    return {"kernel_us": float(np.median(dur)), "reps": reps,
+            "phases_us_min_med_max_over_ctas": {k: [round(float(x), 2) for x in np.median(np.array(v), axis=0)] for k, v in phases.items() if v},
+            "note": "first CTA entry to last CTA's combine done; stamps taken right after a barrier show the arrival"}
+
+
+def parity_sample(w, got, budget_s=1.5):
+    """Achieved error of this run's outputs against the CPU oracle on a bounded sample of (request, head) pairs."""
+    import oracle
+    heads, frac = oracle_sample_plan(w, budget_s)
+    ref = oracle.decode_workload(w, heads_per_request=heads)
+    worst = {"max_abs": 0.0, "rel_fro": 0.0, "lse_abs": 0.0}
+    for (o, l), (ro, rl), hs in zip(got, ref, heads):
+        o, l = o[hs].astype(np.float64), l[hs].astype(np.float64)
+        worst["max_abs"] = max(worst["max_abs"], float(np.abs(o - ro).max()))
+        worst["rel_fro"] = max(worst["rel_fro"], float(np.linalg.norm(o - ro) / np.linalg.norm(ro)))
+        worst["lse_abs"] = max(worst["lse_abs"], float(np.abs(l - rl).max()))
+    worst["sample"] = "%.1f%% of the (head, token) pairs, every request" % (100 * frac)
+    return worst
+
+
+def measure_config(timer, cp, k, w, dw, steps, peaks, with_parity=True):
+    """One workload through the whole protocol; returns the per_config entry."""
+    abytes = w.algorithmic_bytes()
+    dw.ensure_workspace()
+    for _ in range(5):
+        dw.decode()
+    region_ms = min(timer.region(steps, dw.decode) for _ in range(2))
+    ps = timer.per_step(max(steps // 2, 20), dw.decode)
+    flushed_ms = float(np.median(ps))
+    big = abytes > 2 * L2_BYTES
+    used_ms = region_ms if big else flushed_ms
+    achieved = abytes / (used_ms * 1e-3) / 1e9
+    entry = {"workload": "cfg%d:%s" % (k, w.name), "kv_bytes_per_step": abytes,
+             "region_us": 1e3 * region_ms, "flushed_us": 1e3 * flushed_ms,
+             "flushed_us_p10_p50_p90": [1e3 * float(x) for x in np.percentile(ps, [10, 50, 90])],
+             "flushed_calibrated_us": 1e3 * flushed_ms - timer.event_overhead_us,
+             "roofline_uses": "region (inputs %.0f MB > 2 x L2)" % (abytes / 1e6) if big else "flushed (inputs %.0f MB fit or nearly fit the 126 MB L2)" % (abytes / 1e6),
+             "kernel_us": 1e3 * used_ms, "gbs": achieved, "frac_of_measured_peak": achieved / peaks["hbm_gbs"],
+             "frac_of_nominal_8000": achieved / 8000.0, "flushed_gbs": abytes / (flushed_ms * 1e-3) / 1e9,
+             "traffic": NCU_TRAFFIC_BYTES.get(k)}
+    tl = device_timeline(timer, dw, cp)
+    if tl:
+        entry["device"] = tl
+        entry["device_gbs"] = abytes / (tl["kernel_us"] * 1e-6) / 1e9
+    if any(m.kind == 1 for m in w.models):
+        tf = w.flops() / (used_ms * 1e-3) / 1e12
+        entry["tensor"] = {"achieved_tflops": tf, "peak_burst": peaks["bf16_tflops"], "frac_burst": tf / peaks["bf16_tflops"],
+                           "frac_sustained": tf / peaks["bf16_tflops_sustained"], "tensor_pipe_pct_ncu": NCU_TENSOR_PIPE_PCT.get(k)}
+    if with_parity:
+        dw.out.fill_(float("nan"))
+        dw.lse.fill_(float("nan"))
+        dw.decode()
+        entry["parity_vs_oracle"] = parity_sample(w, dw.results())
+    return entry
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -200,6 +352,9 @@ def main():
     ap.add_argument("--no-planner", action="store_true", help="skip the KV-cache planner leg (SURVEY 8(f) N3)")
     ap.add_argument("--no-stages", action="store_true", help="skip the multi-stage launch leg (SURVEY 8(f) N4)")
     ap.add_argument("--stage-layers", type=int, default=4, help="layers per batch in the multi-stage leg")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (the other four BASELINE configs)")
+    ap.add_argument("--probe", default="", choices=["", "timeline", "stream", "launch"],
+                    help="measurement aids: per-CTA timeline of the K/V kernel, read-only HBM ceiling, launch / event floor")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -236,19 +391,13 @@ def main():
         dw.pool.set_option(cp.CP_OPT_MIN_TILE_PAGES, args.min_tile_pages)
     dw.ensure_workspace()
     abytes = w.algorithmic_bytes()
-    # Before every
-    # timed step a short device-side spin (no memory traffic) keeps the GPU busy while the host
-    # enqueues the step, so the per-step events never include host launch latency.
-    flush = torch.zeros(int(os.environ.get('CP_FLUSH_MB', '512')) * 1024 * 1024 // 4, dtype=torch.float32, device=dev)
-    flush_sink = torch.zeros((), dtype=torch.float32, device=dev)
-
-    def l2_flush():
-        # a READ-ONLY pass over 512 MB (4 x the 126 MB L2) evicts the previous step's KV without leaving
-        # dirty lines behind, which a write (fill_) would: the timed kernel would have to wait for their
-        # write-back ("L2 flushed between calls")
-        torch.sum(flush, dim=(0,), out=flush_sink)
+    peaks = measured_peaks()
+    timer = StepTimer(torch, cp, dev, dw.stream())
+    l2_flush = timer.l2_flush
 
     def spacer(i):
+        """Before a per-step-timed call of the side legs: L2 flush (read-only), then a short device-side spin
+        that keeps the host a step ahead, so that host launch latency never lands inside a measurement."""
         l2_flush()
         torch.cuda._sleep(100000)       # ~50 us at 1.9 GHz
 
@@ -259,38 +408,59 @@ def main():
 
     sampler = ClockSampler(local_rank) if rank == 0 else None
 
-    # ---------------- device-resident leg: K steps, inputs already in HBM
+    # ---------------- probes (measurement aids; one JSON line each, then exit)
+    if args.probe:
+        if args.probe == "timeline":
+            out = {"probe": "timeline", "config": workload_desc(w, k), "device": device_timeline(timer, dw, cp, reps=8)}
+        elif args.probe == "stream":
+            buf = torch.zeros(1 << 30, dtype=torch.uint8, device=dev)
+            sink = torch.zeros(1, dtype=torch.int32, device=dev)
+            res = {}
+            for n_ctas in (148, 296, 592, 1184, 2368):
+                ms = min(timer.region(10, lambda: cp.probe_read_stream(buf, buf.numel(), n_ctas, sink, dw.stream())) for _ in range(3))
+                res[str(n_ctas)] = buf.numel() / (ms * 1e-3) / 1e9
+            out = {"probe": "stream", "what": "read-only pass over 1 GiB, 16-byte loads, CTAs of 512 threads (cp_probe_read_stream)",
+                   "gbs_by_ctas": res, "copy_peak_gbs": peaks["hbm_gbs"]}
+        else:
+            out = {"probe": "launch", "empty_kernel_event_pair_us": timer.empty_kernel_events_us(),
+                   "back_to_back_empty_kernels_us": 1e3 * timer.region(50, lambda: cp.probe_globaltimer(timer.stamp, dw.stream()))}
+        print(json.dumps(out))
+        dw.close()
+        return 0
+
+    # ---------------- device-resident leg: K steps, inputs already in HBM, back to back inside one event pair
     t_wall0 = time.time()               # clocks are sampled from the warm-up on (the timed region is a few ms)
     for _ in range(args.warmup):
         dw.decode()
     barrier()
     c0 = dw.pool.counters()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps)]
-    start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    start.record()
+    e_start, e_stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda._sleep(4000000)          # the host enqueues the K steps behind a ~2 ms device-side spin
+    e_start.record()
     for i in range(args.steps):
-        spacer(i)
-        ev[2 * i].record()
         dw.decode()
-        ev[2 * i + 1].record()
-    stop.record()
+    e_stop.record()
     barrier()
     c1 = dw.pool.counters()
-    kern_ms = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(args.steps)]
-    region_ms = start.elapsed_time(stop)
-    step_ms = float(np.sum(kern_ms)) / args.steps     # one launch per step: step = the event-bracketed launch
-    step_ms = reduce_max_over_ranks(step_ms, dev)
+    region_ms = e_start.elapsed_time(e_stop) / args.steps
     launches = c1["kernel_launches"] - c0["kernel_launches"]
-
-    # second number, labelled as such: the same K steps back to back (no spacer, no L2 flush)
-    bb0, bb1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda._sleep(400000)                      # the host enqueues behind a device-side spin
-    bb0.record()
-    for i in range(args.steps):
+    big = abytes > 2 * L2_BYTES
+    # the same steps, each after a read-only L2 flush and bracketed by its own event pair (see StepTimer)
+    per_step = timer.per_step(max(args.steps // 2, 20), dw.decode)
+    flushed_ms = float(np.median(per_step))
+    empty_us = timer.empty_kernel_events_us()
+    empty_region_us = timer.empty_kernel_region_us()
+    timer.event_overhead_us = max(empty_us - empty_region_us, 0.0)
+    kern_ms = region_ms if big else flushed_ms         # the kernel's launch duration the roofline uses
+    step_ms = reduce_max_over_ranks(kern_ms, dev)
+    back_to_back_us = 1e3 * region_ms
+    device_tl = device_timeline(timer, dw, cp) if rank == 0 else None
+    headline_parity = None
+    if rank == 0 and world == 1 and not args.no_per_config:
+        dw.out.fill_(float("nan"))
+        dw.lse.fill_(float("nan"))
         dw.decode()
-    bb1.record()
-    torch.cuda.synchronize()
-    back_to_back_us = 1e3 * bb0.elapsed_time(bb1) / args.steps
+        headline_parity = parity_sample(w, dw.results())
 
     # ---------------- end-to-end leg: host buffers through cp_decode_attention_host
     need = dw.pool.decode_workspace_bytes_host(dw.ids)
@@ -304,7 +474,8 @@ def main():
     barrier()
     e2e_s = 0.0
     for i in range(e2e_steps):
-        l2_flush()
+        if not big:
+            l2_flush()
         torch.cuda.synchronize()
         t0 = time.perf_counter()       # the call copies q H2D, runs the step, copies O/LSE D2H and syncs
         dw.pool.decode_attention_host(dw.ids, q_host, o_host, l_host, ws, need, dw.stream())
@@ -598,23 +769,42 @@ def main():
         append = {"us_per_call": 1e3 * a0.elapsed_time(a1) / reps, "requests": len(w.requests),
                   "bytes_per_call": 2 * (kn + vn)}
 
-    peaks = measured_peaks()
     if gather:
         gather["frac_of_measured_copy_peak"] = gather["traffic_gbs"] / peaks["hbm_gbs"]
     value = whole_job_value(abytes, world, step_ms)
-    kern_avg_ms = float(np.mean(kern_ms))
-    achieved = abytes / (kern_avg_ms * 1e-3) / 1e9
+    achieved = abytes / (kern_ms * 1e-3) / 1e9
     mla = any(m.kind == 1 for m in w.models)
     roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
             "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get(k), "peak_source": peaks["source"],
-            "kernel_us": 1e3 * kern_avg_ms, "kernel_us_p10_p50_p90":
-                [float(x) * 1e3 for x in np.percentile(kern_ms, [10, 50, 90])],
-            "frac_of_nominal_8000": achieved / 8000.0}
+            "kernel_us": 1e3 * kern_ms,
+            "kernel_us_is": ("K steps back to back inside one event pair (inputs %.0f MB > 2 x L2, no flush)" % (abytes / 1e6)) if big
+                            else "median of K steps, each after a read-only L2 flush and inside its own event pair",
+            "region_us": 1e3 * region_ms, "flushed_us": 1e3 * flushed_ms, "flushed_gbs": abytes / (flushed_ms * 1e-3) / 1e9,
+            "flushed_us_p10_p50_p90": [float(x) * 1e3 for x in np.percentile(per_step, [10, 50, 90])],
+            "flushed_calibrated_us": 1e3 * flushed_ms - timer.event_overhead_us,
+            "empty_kernel_events_us": empty_us, "empty_kernel_region_us": empty_region_us,
+            "device": device_tl, "device_gbs": (abytes / (device_tl["kernel_us"] * 1e-6) / 1e9) if device_tl else None,
+            "frac_of_nominal_8000": achieved / 8000.0, "parity_vs_oracle": headline_parity}
     if mla:
-        tf = w.flops() / (kern_avg_ms * 1e-3) / 1e12
+        tf = w.flops() / (kern_ms * 1e-3) / 1e12
         roof["tensor"] = {"achieved_tflops": tf, "peak_burst": peaks["bf16_tflops"],
                           "frac_burst": tf / peaks["bf16_tflops"],
                           "tensor_pipe_pct_ncu": NCU_TENSOR_PIPE_PCT.get(k)}
+
+    # ---------------- the other BASELINE configs through the same protocol (north_star: "all five configs")
+    per_config = None
+    if rank == 0 and world == 1 and not args.no_per_config and k == 2:
+        per_config = {}
+        for kk in (1, 3, 4, 5):
+            wk = W.config(kk)
+            dk = DeviceWorkload(wk, dev)
+            dk.pool.set_option(cp.CP_OPT_KERNEL, args.kernel)
+            try:
+                per_config["cfg%d" % kk] = measure_config(timer, cp, kk, wk, dk, max(args.steps // 2, 30), peaks)
+            finally:
+                dk.close()
+            del dk, wk
+
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": step_ms, "us_per_step": 1e3 * step_ms,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16 in, fp32 accumulate",
@@ -623,7 +813,9 @@ def main():
                     "us_per_step": 1e3 * e2e_ms,
                     "h2d_bytes_per_step": int(q_host.numel() * 2),
                     "d2h_bytes_per_step": int(o_host.numel() * 4 + l_host.numel() * 4)},
-            "gpu_launches": int(launches), "back_to_back_no_flush_us_per_step": back_to_back_us, "roofline": roof, "gather": gather, "append": append, "vmm_arena": vmm, "planner": planner, "stages": stages_leg, "qlen": qlen_leg,
+            "gpu_launches": int(launches), "back_to_back_no_flush_us_per_step": back_to_back_us, "roofline": roof,
+            "per_config": per_config, "gather": gather, "append": append, "vmm_arena": vmm, "planner": planner,
+            "stages": stages_leg, "qlen": qlen_leg,
             "pct_of_hbm_peak": {"measured_copy": 100 * achieved / peaks["hbm_gbs"], "nominal_8TBs": 100 * achieved / 8000.0}}
 
     if not args.no_cpu_baseline:
