@@ -383,7 +383,7 @@ def main():
 
     k = args.config
     w = W.config(k)
-    dw = DeviceWorkload(w, dev, page_list_slack=max(m.n_kv_heads for m in w.models))
+    dw = DeviceWorkload(w, dev, page_list_slack=6 * max(m.n_kv_heads for m in w.models))
     dw.pool.set_option(cp.CP_OPT_KERNEL, args.kernel)
     if args.waves_x16 > 0:
         dw.pool.set_option(cp.CP_OPT_WAVES_X16, args.waves_x16)
@@ -768,6 +768,47 @@ def main():
         torch.cuda.synchronize()
         append = {"us_per_call": 1e3 * a0.elapsed_time(a1) / reps, "requests": len(w.requests),
                   "bytes_per_call": 2 * (kn + vn)}
+        # a decode LOOP as a serving engine runs it (one new token per request per iteration, page boundaries
+        # included, so the tile plan is rebuilt and re-uploaded whenever a request opens a page):
+        #   fused   cp_decode_step: append + attention, one launch per iteration on the tcgen05 K/V kernel
+        #   two     cp_pool_append_kv then cp_decode_attention
+        # device time of the whole loop inside one event pair (the host enqueues behind a device-side spin; if
+        # the host cannot keep up -- plan rebuilds -- that shows here, as it would in a server) and host wall
+        # clock per iteration without the spin.
+        n_loop = max(2 * w.page_tokens, 64)
+        need = max(dw.pool.decode_step_workspace_bytes(dw.ids), dw.ws_bytes, 256)
+        wsl = torch.empty(need + (1 << 20), dtype=torch.uint8, device=dev)
+
+        def loop(fused, steps, spin):
+            c0 = dw.pool.counters()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            if spin:
+                torch.cuda._sleep(spin)
+            t0 = time.perf_counter()
+            e0.record()
+            for _ in range(steps):
+                if fused:
+                    dw.pool.decode_step(dw.ids, k_new, v_new, dw.q, dw.out, dw.lse, wsl, wsl.numel(), dw.stream())
+                else:
+                    dw.pool.append_kv(dw.ids, k_new, v_new, dw.stream())
+                    dw.pool.decode_attention(dw.ids, dw.q, dw.out, dw.lse, wsl, wsl.numel(), dw.stream())
+            e1.record()
+            t_enq = time.perf_counter() - t0
+            torch.cuda.synchronize()
+            c1 = dw.pool.counters()
+            return {"device_us_per_iteration": 1e3 * e0.elapsed_time(e1) / steps,
+                    "host_enqueue_us_per_iteration": 1e6 * t_enq / steps,
+                    "launches_per_iteration": (c1["kernel_launches"] - c0["kernel_launches"]) / steps,
+                    "plan_builds": c1["plan_builds"] - c0["plan_builds"]}
+        loop(True, 4, 0)
+        append["decode_loop"] = {"iterations": n_loop,
+                                 "fused_cp_decode_step": loop(True, n_loop, 20000000),
+                                 "append_then_attention": loop(False, n_loop, 20000000),
+                                 "plain_step_cached_plan_us": back_to_back_us,
+                                 "note": "every request crosses a page boundary at least once in the loop; device time is "
+                                         "what the stream saw for the whole loop behind a ~10 ms spin (host already ahead)"}
+        del wsl
 
     if gather:
         gather["frac_of_measured_copy_peak"] = gather["traffic_gbs"] / peaks["hbm_gbs"]

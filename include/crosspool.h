@@ -263,6 +263,28 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
                               void *workspace_dev, uint64_t workspace_bytes, void *stream);
 
 /*
+ * cp_decode_step -- one decode ITERATION in one call: append the new token of every request
+ * (cp_pool_append_kv's semantics: position context_len, page growth from the free list, all-or-nothing)
+ * and attend over the grown contexts (cp_decode_attention's semantics and layouts).  "map physical KV
+ * pages on demand" and attend over them.  For MQA / GQA models on the
+ * tcgen05 kernel the append costs no launch: the persistent CTA whose tile holds a group's last page writes
+ * the new K and V rows through the page table before it requests that page, so the iteration is ONE kernel
+ * (cp_pool_counters counts one launch); requests of other kinds / kernels get cp_pool_append_kv's kernel in
+ * front of theirs.  The device arena after the call is bit-identical to append-then-attend.
+ *   k_new_dev, v_new_dev  as cp_pool_append_kv;  q_dev, out_dev, lse_dev, workspace_dev  as cp_decode_attention
+ *   (the queries are those of the NEW token: they see context_len + 1 tokens)
+ * cp_decode_step_workspace_bytes: scratch the call needs, i.e. for the contexts grown by one token (host
+ * arithmetic on a plan of the grown contexts; the pool is not changed).
+ * Errors: those of both calls.  WORKSPACE is detected after the host bookkeeping of the append and takes it
+ * back (context lengths, free list), so the pool is unchanged on every error but CUDA.
+ */
+cp_status cp_decode_step_workspace_bytes(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                                         uint64_t *bytes_out);
+cp_status cp_decode_step(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                         const void *k_new_dev, const void *v_new_dev, const void *q_dev, float *out_dev,
+                         float *lse_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream);
+
+/*
  * cp_decode_attention_host -- the same step with HOST query / result buffers: copies q
  * host->device, runs cp_decode_attention, copies O and LSE device->host and synchronises
  * `stream`.  Host buffers that are pinned and device-mapped (cudaHostAlloc / cudaHostRegister) are

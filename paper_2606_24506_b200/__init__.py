@@ -105,6 +105,8 @@ def load_library():
         "cp_pool_counters": (i32, [vp, u64p, u64p, u64p]),
         "cp_pool_read_timeline": (i32, [vp, u64p, i32, i32p]),
         "cp_status_string": (ctypes.c_char_p, [i32]),
+        "cp_decode_step_workspace_bytes": (i32, [vp, i32p, i32, u64p]),
+        "cp_decode_step": (i32, [vp, i32p, i32, vp, vp, vp, vp, vp, vp, u64, vp]),
         "cp_probe_globaltimer": (i32, [vp, vp]),
         "cp_probe_read_stream": (i32, [vp, u64, i32, vp, vp]),
         "cp_planner_workspace_bytes": (u64, [ctypes.c_int64]),
@@ -128,7 +130,7 @@ EXPORTED = ["cp_pool_create", "cp_pool_create_vmm", "cp_pool_vmm_info", "cp_pool
             "cp_decode_attention_host", "cp_decode_workspace_bytes_qlen", "cp_decode_attention_qlen",
             "cp_decode_stages_workspace_bytes", "cp_decode_attention_stages", "cp_decode_attention_stages_gated",
             "cp_decode_stages_gate_status", "cp_decode_plan", "cp_pool_counters", "cp_pool_read_timeline", "cp_status_string",
-            "cp_probe_globaltimer", "cp_probe_read_stream",
+            "cp_probe_globaltimer", "cp_probe_read_stream", "cp_decode_step_workspace_bytes", "cp_decode_step",
             "cp_planner_workspace_bytes", "cp_planner_pool_demand", "cp_planner_quantile"]
 
 
@@ -337,6 +339,21 @@ class Pool:
         ids = _ids(request_ids)
         _check(self._L.cp_pool_append_kv(self._h, _i32p(ids), ids.size, _ptr(k_new_dev), _ptr(v_new_dev), stream),
                "cp_pool_append_kv")
+
+    def decode_step_workspace_bytes(self, request_ids) -> int:
+        ids = _ids(request_ids)
+        out = ctypes.c_uint64()
+        _check(self._L.cp_decode_step_workspace_bytes(self._h, _i32p(ids), ids.size, ctypes.byref(out)),
+               "cp_decode_step_workspace_bytes")
+        return int(out.value)
+
+    def decode_step(self, request_ids, k_new_dev, v_new_dev, q_dev, out_dev, lse_dev, workspace_dev,
+                    workspace_bytes: int, stream: int = 0):
+        """Append one token per request and attend over the grown contexts (one call, one launch where fused)."""
+        ids = _ids(request_ids)
+        _check(self._L.cp_decode_step(self._h, _i32p(ids), ids.size, _ptr(k_new_dev), _ptr(v_new_dev), _ptr(q_dev),
+                                      _ptr(out_dev), _ptr(lse_dev), _ptr(workspace_dev), workspace_bytes, stream),
+               "cp_decode_step")
 
     def decode_workspace_bytes(self, request_ids) -> int:
         ids = _ids(request_ids)

@@ -69,10 +69,13 @@ struct TileRec {
     int32_t page_begin, n_pages, split, n_splits;
     int32_t gsize, n_q_heads;
     float scale_log2;
-    int32_t pad;
+    int32_t pad;                   // bit 0: another static slot of this CTA follows (tcgen05 K/V kernel); bit 1: the tile
+                                   // holds its group's LAST planned page (where a fused append writes); bits 8..15: zl
+                                   // of the group's partial layout; other kernels: see their planner
     int64_t q_off, out_off, lse_off, part_off;
+    int64_t app_k_off, app_v_off;  // element offsets of this group's new K / V row in the packed k_new / v_new of cp_decode_step
 };
-static_assert(sizeof(TileRec) == 80, "TileRec is loaded as five 16-byte vectors");
+static_assert(sizeof(TileRec) == 96, "TileRec is loaded as 16-byte vectors (five for the fields the older kernels use, six in all)");
 
 // One request of a cp_pool_append_kv batch.
 struct AppendRec {
@@ -154,6 +157,8 @@ struct DecodeParams {
     int32_t *stage_done;           // [n_stages] completion counters, kCounterStride apart
     int32_t n_stages;
     unsigned long long *timeline;  // CP_OPT_TIMELINE: [grid][kTimelineSlots] globaltimer stamps, or nullptr
+    const uint16_t *app_k, *app_v; // cp_decode_step: packed new K / V rows the launch writes at position
+                                   // context_len - 1 of every request before the page that holds it is read, or nullptr
 };
 
 }  // namespace cp

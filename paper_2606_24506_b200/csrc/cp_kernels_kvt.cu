@@ -84,12 +84,12 @@ struct KtDesc {                  // what the producer hands to the other warps f
 };
 
 struct KtMeta {                  // what the scheduler warp hands to the producer for one tile
-    TileRec r;
-    int32_t ctx;
     int32_t item;                // < 0: no more work
+    int32_t req, kv_head, n_kv_heads, page_begin, n_pages;
+    int32_t pad[2];
     int32_t pid[32];             // the tile's first 32 physical pages
 };
-static_assert(sizeof(KtMeta) == 216, "KtMeta layout");
+static_assert(sizeof(KtMeta) == 160, "KtMeta layout");
 
 struct KtMisc {
     uint64_t full[4], empty[4];                  // slice ring: TMA -> MMA, MMA (commit) -> TMA
@@ -106,7 +106,7 @@ struct KtMisc {
     KtMeta meta[KT_MQ];
     uint32_t tmem_base;
     uint32_t pad[1];
-    float redmax[4 * KT_NMAX];                   // slice maxima when the reference moves: [row][warp]
+    alignas(16) float redmax[4 * KT_NMAX];       // slice maxima when the reference moves: [row][warp]
     float red[2][4 * KT_NMAX];                   // per-tile row sums: [O buffer][row][warp]
     float mref[2][KT_NMAX];                      // per-tile exponent reference (log2 units): [O buffer][row]
 };
@@ -161,7 +161,7 @@ __device__ __forceinline__ TileRec load_tile_rec(const TileRec *recs, int item)
     const uint4 *src = reinterpret_cast<const uint4 *>(recs + item);
     uint4 *dst = reinterpret_cast<uint4 *>(&r);
 #pragma unroll
-    for (int i = 0; i < 5; ++i) dst[i] = __ldg(src + i);
+    for (int i = 0; i < 6; ++i) dst[i] = __ldg(src + i);
     return r;
 }
 
@@ -376,7 +376,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             const KtMeta *mt = &mi->meta[ms];
             const int item = mt->item;
             if (item < 0) break;
-            const int req = mt->r.req, hkv = mt->r.n_kv_heads, kvh = mt->r.kv_head, pb = mt->r.page_begin, npg = mt->r.n_pages;
+            const int req = mt->req, hkv = mt->n_kv_heads, kvh = mt->kv_head, pb = mt->page_begin, npg = mt->n_pages;
             int32_t pid = mt->pid[lane];
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(&mi->meta_empty[ms]));
@@ -474,6 +474,19 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                                  : "l"(p.page_table + (int64_t)r.req * p.max_ppr + (int64_t)(r.page_begin + lane) * r.n_kv_heads + r.kv_head));
             }
             asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(ctx) : "l"(p.req_ctx + r.req));
+            // ---- fused append (cp_decode_step): the tile that holds its group's last page writes the
+            // new token's K and V rows (position ctx - 1) before the producer is told about the tile, i.e. before
+            // the page is requested.  Source row and the page's id travel in the same round trip.
+            const bool app = p.app_k != nullptr && (r.pad & 2);
+            uint4 app_row = make_uint4(0u, 0u, 0u, 0u);
+            int32_t app_pid = 0;
+            if (app) {
+                const uint16_t *src = lane < 16 ? p.app_k + r.app_k_off + lane * 8 : p.app_v + r.app_v_off + (lane - 16) * 8;
+                asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(app_row.x), "=r"(app_row.y), "=r"(app_row.z), "=r"(app_row.w) : "l"(src));
+                const int64_t idx = (int64_t)(r.page_begin + r.n_pages - 1) * r.n_kv_heads + r.kv_head;
+                if (p.slot_pages > 0) app_pid = r.req * p.slot_pages + (int32_t)idx;
+                else asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(app_pid) : "l"(p.page_table + (int64_t)r.req * p.max_ppr + idx));
+            }
             // ---- the tile's query rows -> buffer (ti & 1), asynchronously: two K-major [N x 64] blocks, 128-byte
             // swizzle (16-B chunk index ^ (row & 7)); rows beyond the group are zero-filled.  The buffer is free
             // once the score MMAs of tile ti - 2 are complete; q_full counts the 32 lanes' copies.
@@ -492,14 +505,24 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(&mi->q_full[ti & 1])) : "memory");
             }
             resolve_next();
+            if (app) {
+                const int slot = (ctx - 1) % P;
+                uint8_t *dst = const_cast<uint8_t *>(p.arena) + (size_t)app_pid * p.page_bytes + (size_t)slot * (KT_D * 2) +
+                               (lane < 16 ? (size_t)lane * 16 : (size_t)P * (KT_D * 2) + (size_t)(lane - 16) * 16);
+                *reinterpret_cast<uint4 *>(dst) = app_row;
+                // the row is read by TMA (async proxy) that another thread issues after the hand-over below
+                __threadfence();
+                fence_proxy_async_all();
+                __syncwarp();
+            }
             mbar_wait(smem_u32(&mi->meta_empty[ms]), ((ti / KT_MQ) & 1) ^ 1);
             mbar_wait(smem_u32(&mi->tq_empty[qs]), ((ti / KT_TQ) & 1) ^ 1);
             {
                 KtMeta *mt = &mi->meta[ms];
-                if (lane < 10) reinterpret_cast<uint2 *>(&mt->r)[lane] = reinterpret_cast<const uint2 *>(&r)[lane];   // KtMeta is 8-byte aligned
                 mt->pid[lane] = pid0;
                 if (lane == 0) {
-                    mt->ctx = ctx; mt->item = item;
+                    mt->item = item; mt->req = r.req; mt->kv_head = r.kv_head; mt->n_kv_heads = r.n_kv_heads;
+                    mt->page_begin = r.page_begin; mt->n_pages = r.n_pages;
                     const int t_begin = r.page_begin * P;
                     const int t_end = min((r.page_begin + r.n_pages) * P, ctx);
                     const int n_slices = (t_end - t_begin + KT_SLICE - 1) / KT_SLICE;

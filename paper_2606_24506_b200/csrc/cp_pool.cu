@@ -105,6 +105,7 @@ struct cp_pool {
     // query tokens per request of the call in progress (cp_decode_attention_qlen), and of the cached plan
     int qlen = 1, plan_qlen = 1;
     bool plan_for_stages = false;        // build_plan is called for a multi-stage work list (mma.sync kernel)
+    const uint16_t *step_k = nullptr, *step_v = nullptr;   // cp_decode_step in progress: new rows the decode launch itself writes
     int opt_timeline = 0;                // CP_OPT_TIMELINE: per-CTA globaltimer stamps of the next decode launches
     int timeline_ctas = 0;               // grid size of the last launch that wrote stamps
     int device = -1;                     // device of the arena (the compute calls require it to be current)
@@ -116,6 +117,7 @@ struct cp_pool {
     KindPlan plan[2];
     uint64_t plan_ws_floats = 0;
     std::vector<int64_t> q_off, out_off, lse_off;   // per batch slot (packed offsets)
+    std::vector<int64_t> app_k_off, app_v_off;      // per batch slot: element offsets into the packed k_new / v_new of an append
     int64_t q_elems = 0, out_floats = 0, lse_floats = 0;
 
     // device side (lazy)
@@ -322,6 +324,9 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
         r.scale_log2 = (float)((double)m.softmax_scale * 1.4426950408889634);
         r.q_off = gr.q_off; r.out_off = gr.out_off; r.lse_off = gr.lse_off; r.part_off = gr.part_off;
         r.pad = zl_of(gr.n_splits) << 8;               // bits 8..15: partial layout; bit 0 (set below): another static slot follows
+        if (r.page_begin + r.n_pages == G.n_lp) r.pad |= 2;      // the group's last planned page is in this tile
+        r.app_k_off = pool->app_k_off[G.b] + (int64_t)gr.kv_head * m.head_dim_qk;
+        r.app_v_off = pool->app_v_off[G.b] + (int64_t)gr.kv_head * m.head_dim_v;
         return r;
     };
     // split index of a tile = its rank inside the group by position (tl is in that order per group)
@@ -380,7 +385,8 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         kp.max_splits = 1; kp.max_dk = kp.max_dv = kp.max_group = 0; kp.uploaded = false;
     }
     pool->q_off.assign(n, 0); pool->out_off.assign(n, 0); pool->lse_off.assign(n, 0);
-    int64_t qo = 0, oo = 0, lo = 0;
+    pool->app_k_off.assign(n, 0); pool->app_v_off.assign(n, 0);
+    int64_t qo = 0, oo = 0, lo = 0, ako = 0, avo = 0;
     int64_t total_pages[2] = {0, 0};
     for (int b = 0; b < n; ++b) {
         const Request &r = pool->reqs[ids[b]];
@@ -389,6 +395,9 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         qo += (int64_t)pool->qlen * m.n_q_heads * m.head_dim_qk;
         oo += (int64_t)pool->qlen * m.n_q_heads * m.head_dim_v;
         lo += (int64_t)pool->qlen * m.n_q_heads;
+        pool->app_k_off[b] = ako; pool->app_v_off[b] = avo;
+        ako += (int64_t)m.n_kv_heads * m.head_dim_qk;
+        if (m.kind != CP_KIND_MLA) avo += (int64_t)m.n_kv_heads * m.head_dim_v;
         total_pages[m.kind] += (int64_t)ceil_div(r.ctx, P) * m.n_kv_heads;
     }
     pool->q_elems = qo; pool->out_floats = oo; pool->lse_floats = lo;
@@ -568,6 +577,8 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             r.pad = pool->qlen > 1 ? m.n_q_heads / m.n_kv_heads : 0;
             r.scale_log2 = (float)((double)m.softmax_scale * 1.4426950408889634);
             r.q_off = gr.q_off; r.out_off = gr.out_off; r.lse_off = gr.lse_off; r.part_off = gr.part_off;
+            r.app_k_off = pool->app_k_off[gr.batch_index] + (int64_t)gr.kv_head * m.head_dim_qk;
+            r.app_v_off = pool->app_v_off[gr.batch_index] + (int64_t)gr.kv_head * m.head_dim_v;
         }
         std::vector<int> last_pos(kp.groups.size(), 0);
         for (size_t i = 0; i < kp.tiles.size(); ++i) last_pos[kp.tiles[i].group] = (int)i;
@@ -1093,18 +1104,20 @@ cp_status cp_pool_gather_kv(cp_pool *pool, int32_t request_id, void *k_out_dev, 
     return CP_OK;
 }
 
-cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
-                            const void *k_new_dev, const void *v_new_dev, void *stream)
+namespace {
+
+// Host half of an append (cp_pool_append_kv, cp_decode_step): validate the whole batch first (all-or-nothing:
+// capacity of the page lists, page budget), then commit -- new pages from the free list where a position opens
+// a logical page, context lengths + 1 -- and describe the device half in recs.  grew[b] = pages added to
+// request b (what append_rollback takes back).
+cp_status append_host(cp_pool *pool, const int32_t *ids, int n, bool need_v_ptr, const void *v_new_dev,
+                      std::vector<AppendRec> &recs, std::vector<int> &grew)
 {
-    cp_status st = check_batch(pool, request_ids_host, n_requests);
-    if (st != CP_OK) return st;
-    if (!k_new_dev || ((uintptr_t)k_new_dev & 15u) || ((uintptr_t)v_new_dev & 15u)) return CP_ERR_INVALID_ARG;
-    // validate the whole batch first (all-or-nothing): capacity of the page lists, page budget
     const int P = (int)pool->P;
     uint32_t need_pages = 0, need_chunks = 0;
     bool any_v = false;
-    for (int b = 0; b < n_requests; ++b) {
-        const Request &r = pool->reqs[request_ids_host[b]];
+    for (int b = 0; b < n; ++b) {
+        const Request &r = pool->reqs[ids[b]];
         const cp_model_cfg &m = pool->models[r.model];
         if (m.kind != CP_KIND_MLA) any_v = true;
         if (r.ctx == INT32_MAX) return CP_ERR_INVALID_ARG;
@@ -1113,24 +1126,18 @@ cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int3
             if (r.pages.size() + m.n_kv_heads > (size_t)pool->max_ppr) return CP_ERR_INVALID_ARG;
             need_pages += (uint32_t)m.n_kv_heads;
             if (pool->vmm)
-                need_chunks += vmm_chunks_missing(pool->vmm, request_ids_host[b],
-                                                  (uint64_t)(r.pages.size() + m.n_kv_heads) * pool->page_bytes);
+                need_chunks += vmm_chunks_missing(pool->vmm, ids[b], (uint64_t)(r.pages.size() + m.n_kv_heads) * pool->page_bytes);
         }
     }
-    if (any_v && !v_new_dev) return CP_ERR_INVALID_ARG;
+    if (need_v_ptr && any_v && !v_new_dev) return CP_ERR_INVALID_ARG;
     if (pool->vmm ? need_chunks > vmm_chunks_available(pool->vmm) : need_pages > pool->n_free) return CP_ERR_NO_PAGES;
-    st = ensure_device(pool);
+    const cp_status st = ensure_device(pool);
     if (st != CP_OK) return st;
-    cudaStream_t s = (cudaStream_t)stream;
-    if (pool->d_append.ensure((size_t)n_requests * sizeof(AppendRec)) != cudaSuccess) {
-        cudaGetLastError();
-        return CP_ERR_CUDA;
-    }
-    // commit on the host: new pages from the free list, context lengths
-    std::vector<AppendRec> recs(n_requests);
+    recs.resize(n);
+    grew.assign(n, 0);
     int64_t ko = 0, vo = 0;
-    for (int b = 0; b < n_requests; ++b) {
-        const int rid = request_ids_host[b];
+    for (int b = 0; b < n; ++b) {
+        const int rid = ids[b];
         Request &r = pool->reqs[rid];
         const cp_model_cfg &m = pool->models[r.model];
         if ((size_t)(r.ctx / P) >= r.pages.size() / m.n_kv_heads && pool->vmm) {
@@ -1141,6 +1148,7 @@ cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int3
                 pool->owner[pid] = rid; r.pages.push_back(pid);
             }
             pool->n_free -= (uint32_t)m.n_kv_heads;
+            grew[b] = m.n_kv_heads;
         } else if ((size_t)(r.ctx / P) >= r.pages.size() / m.n_kv_heads) {
             uint32_t cur = pool->alloc_cursor;
             for (int i = 0; i < m.n_kv_heads;) {
@@ -1149,6 +1157,7 @@ cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int3
             }
             pool->alloc_cursor = cur;
             pool->n_free -= (uint32_t)m.n_kv_heads;
+            grew[b] = m.n_kv_heads;
         }
         recs[b].req = rid; recs[b].model = r.model; recs[b].pos = r.ctx; recs[b].pad = 0;
         recs[b].k_off = ko; recs[b].v_off = vo;
@@ -1161,18 +1170,63 @@ cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int3
         pool->ctx_dirty_hi = std::max(pool->ctx_dirty_hi, rid);
         if (ceil_div(r.ctx, P) != old_planned) pool->topo_version++;
     }
-    st = flush_tables(pool, s);                            // new page ids (and context lengths) to the device
-    if (st != CP_OK) return st;
-    if (cudaMemcpyAsync(pool->d_append.ptr, recs.data(), recs.size() * sizeof(AppendRec), cudaMemcpyHostToDevice, s) !=
-        cudaSuccess)
+    return CP_OK;
+}
+
+// Take back what append_host committed (a cp_decode_step that finds its workspace too small): the token is not
+// appended, the pages it opened return to the free list (a CUDA-VMM chunk mapped for them stays mapped, parked
+// under the request's slot).  Nothing has been sent to the device yet.
+void append_rollback(cp_pool *pool, const int32_t *ids, int n, const std::vector<int> &grew)
+{
+    for (int b = 0; b < n; ++b) {
+        const int rid = ids[b];
+        Request &r = pool->reqs[rid];
+        for (int i = 0; i < grew[b]; ++i) {
+            pool->owner[r.pages.back()] = -1;
+            r.pages.pop_back();
+        }
+        pool->n_free += (uint32_t)grew[b];
+        r.uploaded = std::min(r.uploaded, r.pages.size());
+        r.ctx -= 1;
+        pool->h_ctx[rid] = r.ctx;
+        pool->ctx_dirty_lo = std::min(pool->ctx_dirty_lo, rid);
+        pool->ctx_dirty_hi = std::max(pool->ctx_dirty_hi, rid);
+    }
+    pool->topo_version++;
+}
+
+cp_status launch_append_recs(cp_pool *pool, const std::vector<AppendRec> &recs, const void *k_new_dev, const void *v_new_dev,
+                             cudaStream_t s)
+{
+    if (recs.empty()) return CP_OK;
+    if (pool->d_append.ensure(recs.size() * sizeof(AppendRec)) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+    if (cudaMemcpyAsync(pool->d_append.ptr, recs.data(), recs.size() * sizeof(AppendRec), cudaMemcpyHostToDevice, s) != cudaSuccess)
         return CP_ERR_CUDA;
     pool->n_h2d_bytes += recs.size() * sizeof(AppendRec);
     launch_append(pool->arena, pool->P, pool->page_bytes, (const int32_t *)pool->d_page_table.ptr, pool->max_ppr,
-                  (const DevModel *)pool->d_models.ptr, (const AppendRec *)pool->d_append.ptr, n_requests,
+                  (const DevModel *)pool->d_models.ptr, (const AppendRec *)pool->d_append.ptr, (int)recs.size(),
                   (const uint16_t *)k_new_dev, (const uint16_t *)v_new_dev, s);
     pool->n_launches++;
     if (cudaGetLastError() != cudaSuccess) return CP_ERR_CUDA;
     return CP_OK;
+}
+
+}  // namespace
+
+cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                            const void *k_new_dev, const void *v_new_dev, void *stream)
+{
+    cp_status st = check_batch(pool, request_ids_host, n_requests);
+    if (st != CP_OK) return st;
+    if (!k_new_dev || ((uintptr_t)k_new_dev & 15u) || ((uintptr_t)v_new_dev & 15u)) return CP_ERR_INVALID_ARG;
+    std::vector<AppendRec> recs;
+    std::vector<int> grew;
+    st = append_host(pool, request_ids_host, n_requests, true, v_new_dev, recs, grew);
+    if (st != CP_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    st = flush_tables(pool, s);                            // new page ids (and context lengths) to the device
+    if (st != CP_OK) return st;
+    return launch_append_recs(pool, recs, k_new_dev, v_new_dev, s);
 }
 
 cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
@@ -1222,6 +1276,7 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.stages = nullptr; prm.stage_done = nullptr; prm.n_stages = 0; prm.q_len = pool->qlen;
         prm.published = nullptr; prm.gate_flag = nullptr; prm.gate_timeout_us = 0;
         prm.timeline = nullptr;
+        prm.app_k = pool->step_k; prm.app_v = pool->step_v;
         if (pool->opt_timeline) {
             const size_t tb = (size_t)pool->n_sm * kTimelineSlots * sizeof(unsigned long long);
             if (pool->d_timeline.ensure(tb) != cudaSuccess || cudaMemsetAsync(pool->d_timeline.ptr, 0, tb, s) != cudaSuccess) {
@@ -1259,6 +1314,63 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         pool->n_launches++;
         if (e != cudaSuccess) return CP_ERR_CUDA;
     }
+    return CP_OK;
+}
+
+// ------------------------------------------------------------------ append + attend in one call
+cp_status cp_decode_step(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
+                         const void *k_new_dev, const void *v_new_dev, const void *q_dev, float *out_dev,
+                         float *lse_dev, void *workspace_dev, uint64_t workspace_bytes, void *stream)
+{
+    cp_status st = check_batch(pool, request_ids_host, n_requests);
+    if (st != CP_OK) return st;
+    if (!k_new_dev || ((uintptr_t)k_new_dev & 15u) || ((uintptr_t)v_new_dev & 15u)) return CP_ERR_INVALID_ARG;
+    if (!q_dev || !out_dev || !lse_dev) return CP_ERR_INVALID_ARG;
+    if (((uintptr_t)q_dev & 15u) || ((uintptr_t)out_dev & 15u) || ((uintptr_t)lse_dev & 3u)) return CP_ERR_INVALID_ARG;
+    std::vector<AppendRec> recs;
+    std::vector<int> grew;
+    st = append_host(pool, request_ids_host, n_requests, true, v_new_dev, recs, grew);
+    if (st != CP_OK) return st;
+    // the plan of the grown contexts decides the workspace; too small: the append is taken back, nothing changed
+    ensure_plan(pool, request_ids_host, n_requests);
+    if (pool->plan_ws_floats * 4 > workspace_bytes ||
+        (pool->plan_ws_floats && (!workspace_dev || ((uintptr_t)workspace_dev & 15u)))) {
+        append_rollback(pool, request_ids_host, n_requests, grew);
+        return CP_ERR_WORKSPACE;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    // Requests whose attention kernel writes the new row itself (the tcgen05 K/V kernel: the tile that holds a
+    // group's last page stores the row before it requests the page) need no launch of their own; the others
+    // (MLA, generic shapes, CP_OPT_KERNEL = 1 / 3) get the append kernel first.
+    const bool fused_kv = pool->plan[CP_KIND_KV].use_kvt && pool->kv_tmap_ok;
+    std::vector<AppendRec> sep;
+    for (int b = 0; b < n_requests; ++b)
+        if (!(fused_kv && pool->models[recs[b].model].kind == CP_KIND_KV)) sep.push_back(recs[b]);
+    st = flush_tables(pool, s);
+    if (st != CP_OK) return st;
+    st = launch_append_recs(pool, sep, k_new_dev, v_new_dev, s);
+    if (st != CP_OK) return st;
+    pool->step_k = fused_kv ? (const uint16_t *)k_new_dev : nullptr;
+    pool->step_v = fused_kv ? (const uint16_t *)v_new_dev : nullptr;
+    st = cp_decode_attention(pool, request_ids_host, n_requests, q_dev, out_dev, lse_dev, workspace_dev, workspace_bytes, stream);
+    pool->step_k = pool->step_v = nullptr;
+    return st;
+}
+
+cp_status cp_decode_step_workspace_bytes(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests, uint64_t *bytes_out)
+{
+    if (!bytes_out) return CP_ERR_INVALID_ARG;
+    cp_status st = check_batch(pool, request_ids_host, n_requests);
+    if (st != CP_OK) return st;
+    // plan of the contexts as they will be after the append (host arithmetic only; the cached plan is dropped)
+    for (int b = 0; b < n_requests; ++b) {
+        if (pool->reqs[request_ids_host[b]].ctx == INT32_MAX) return CP_ERR_INVALID_ARG;
+        pool->reqs[request_ids_host[b]].ctx += 1;
+    }
+    build_plan(pool, request_ids_host, n_requests);
+    *bytes_out = pool->plan_ws_floats * 4;
+    for (int b = 0; b < n_requests; ++b) pool->reqs[request_ids_host[b]].ctx -= 1;
+    pool->plan_valid = false;
     return CP_OK;
 }
 
@@ -1501,6 +1613,7 @@ static cp_status decode_stages_core(cp_pool *pool, int32_t n_stages, const int32
     prm.n_stages = n_stages; prm.q_len = 1;
     prm.published = nullptr; prm.gate_flag = nullptr; prm.gate_timeout_us = 0;
     prm.timeline = nullptr;
+    prm.app_k = nullptr; prm.app_v = nullptr;
     if (published_dev) {
         if (sp.d_gate.ensure(16) != cudaSuccess || cudaMemsetAsync(sp.d_gate.ptr, 0, 16, s) != cudaSuccess) {
             cudaGetLastError();

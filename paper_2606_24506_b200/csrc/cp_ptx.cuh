@@ -54,6 +54,10 @@ __device__ __forceinline__ void prefetch_l2(const void *p)     // also fills the
 {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p) : "memory");
 }
+__device__ __forceinline__ void fence_proxy_async_all()  // generic-proxy writes to ANY state space (here: global) -> async proxy
+{
+    asm volatile("fence.proxy.async;" ::: "memory");
+}
 __device__ __forceinline__ void fence_proxy_async()      // generic-proxy smem writes -> async proxy (TMA, tcgen05)
 {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");

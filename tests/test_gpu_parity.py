@@ -413,6 +413,97 @@ def test_append_kv_matches_oracle_bit_for_bit(torch_cuda, kind):
     print(worst)
 
 
+@pytest.mark.parametrize("kind", ["kv", "kv_vmm", "mla", "mixed", "kv_warp_mma"])
+def test_decode_step_appends_and_attends_in_one_call(torch_cuda, kind):
+    """SURVEY 8(f) N1, second half: cp_decode_step = append + attend.  For MQA / GQA models on the tcgen05 kernel
+    the iteration is ONE launch (the tile that holds a group's last page writes the new rows before requesting
+    the page); other kinds / kernels get the append kernel in front.  After every step the whole device arena is
+    bit-identical to the oracle's append, and the attention over the T + 1 tokens is within the bars."""
+    import torch
+    import paper_2606_24506_b200 as cp
+    vmm = kind == "kv_vmm"
+    if kind in ("kv", "kv_vmm", "kv_warp_mma"):
+        models = [ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5), ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5)]
+        rm, rc, P, scale = [0, 1, 1], [2500, 64, 5], 16, 1.0
+    elif kind == "mla":
+        models = [ModelCfg(KIND_MLA, 128, 1, 576, 512, 192 ** -0.5)]
+        rm, rc, P, scale = [0, 0], [63, 700], 32, 0.1
+    else:
+        models = [ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5), ModelCfg(KIND_MLA, 128, 1, 576, 512, 192 ** -0.5)]
+        rm, rc, P, scale = [0, 1, 0], [700, 130, 31], 32, 0.3
+    w = W.small_workload(models, rm, rc, page_tokens=P, seed=93, value_scale=scale, extra_pages=60, keep_contiguous=False)
+    dw = device_workload(w, page_list_slack=3 * max(m.n_kv_heads for m in models), vmm=vmm,
+                         **({"vmm_budget_bytes": (w.num_pages + 64) * w.page_bytes + (16 << 20)} if vmm else {}))
+    dw.pool.set_option(cp.CP_OPT_MIN_TILE_PAGES, 1)
+    if kind == "kv_warp_mma":
+        dw.pool.set_option(cp.CP_OPT_KERNEL, 3)
+    rng = np.random.default_rng(19)
+    host = w.arena.copy()
+    ctx = [r.context_len for r in w.requests]
+    host_free = sorted(set(range(w.num_pages)) - set(int(x) for r in w.requests for x in r.page_ids))
+    n_steps = 2 * P + 3
+    for step in range(n_steps):                       # crosses at least two page boundaries per request
+        ks, vs, qs = [], [], []
+        for r in w.requests:
+            m = models[r.model_id]
+            ks.append(W.f32_to_bf16((scale * rng.standard_normal((m.n_kv_heads, m.head_dim_qk))).astype(np.float32)))
+            if m.kind == KIND_KV:
+                vs.append(W.f32_to_bf16((scale * rng.standard_normal((m.n_kv_heads, m.head_dim_v))).astype(np.float32)))
+            qs.append(W.f32_to_bf16((scale * rng.standard_normal((m.n_q_heads, m.head_dim_qk))).astype(np.float32)))
+        k_dev = torch.from_numpy(np.concatenate([x.reshape(-1) for x in ks]).view(np.int16)).to(dw.device)
+        v_dev = torch.from_numpy(np.concatenate([x.reshape(-1) for x in vs]).view(np.int16)).to(dw.device) if vs else None
+        q_dev = torch.from_numpy(np.concatenate([x.reshape(-1) for x in qs]).view(np.int16)).to(dw.device)
+        need = max(dw.pool.decode_step_workspace_bytes(dw.ids), 256)
+        ws = torch.full((need,), 0xFF, dtype=torch.uint8, device=dw.device)
+        dw.out.fill_(float("nan"))
+        dw.lse.fill_(float("nan"))
+        c0 = dw.pool.counters()["kernel_launches"]
+        dw.pool.decode_step(dw.ids, k_dev, v_dev, q_dev, dw.out, dw.lse, ws, need, dw.stream())
+        launches = dw.pool.counters()["kernel_launches"] - c0
+        if kind in ("kv", "kv_vmm"):
+            assert launches == 1, "the fused iteration must be one launch, got %d" % launches
+        elif kind == "mixed":
+            assert launches == 3          # append kernel for the MLA requests, then one decode launch per kind
+        vi = 0
+        for i, r in enumerate(w.requests):
+            m = models[r.model_id]
+            _, c, ids = dw.pool.request_info(r.request_id)
+            assert c == ctx[i] + 1
+            v_new = None
+            if m.kind == KIND_KV:
+                v_new = vs[vi]; vi += 1
+            if vmm:
+                # the library's arena is its own contiguous virtual range: the oracle keeps the host image and takes
+                # pages of its own choice when a position opens one (where a page lies does not enter the results)
+                if ctx[i] % P == 0 and ctx[i] // P * m.n_kv_heads >= r.page_ids.size:
+                    r.page_ids = np.concatenate([r.page_ids, np.array([host_free.pop() for _ in range(m.n_kv_heads)], dtype=np.int32)])
+            else:
+                r.page_ids = ids
+            oracle.append(host, P, w.page_bytes, w.num_pages, m.kind, m.n_kv_heads, m.head_dim_qk, m.head_dim_v,
+                          r.page_ids, ctx[i], ks[i], v_new)
+            ctx[i] += 1
+            r.context_len = ctx[i]
+            w.q[i] = qs[i]
+        if step % P in (0, 1, 2) or step == n_steps - 1:
+            torch.cuda.synchronize()
+            if not vmm:
+                assert dw.arena.cpu().numpy().view(np.uint16).tobytes() == host.tobytes(), "arena differs at step %d" % step
+            w.arena = host
+            got = dw.results()
+            worst = compare(w, got, oracle.decode_workload(w), "decode_step_%s_%d" % (kind, step))
+    print(worst)
+    # too small a workspace: the append is taken back, nothing changed
+    before = [dw.pool.request_info(r.request_id) for r in w.requests]
+    free_before = dw.pool.stats()
+    if dw.pool.decode_step_workspace_bytes(dw.ids) > 0:
+        with pytest.raises(cp.CrossPoolError) as e:
+            dw.pool.decode_step(dw.ids, k_dev, v_dev, q_dev, dw.out, dw.lse, ws, 16, dw.stream())
+        assert e.value.status == cp.CP_ERR_WORKSPACE
+        after = [dw.pool.request_info(r.request_id) for r in w.requests]
+        assert all(a[1] == b[1] and list(a[2]) == list(b[2]) for a, b in zip(after, before)) and dw.pool.stats() == free_before
+    dw.close()
+
+
 def test_host_buffer_entry_point_matches_device_path(torch_cuda):
     torch = torch_cuda
     ms = [ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5), ModelCfg(KIND_KV, 16, 1, 128, 128, 128 ** -0.5)]
