@@ -641,6 +641,26 @@ def main():
                 e1.record()
                 torch.cuda.synchronize()
                 one.append(e0.elapsed_time(e1))
+            # the same stages through the request queue (cp_queue_*): nothing is known to the kernel at launch, the
+            # planner warp on the GPU cuts every stage into tiles as it reads it from the ring.  All stages are
+            # pushed before the launch here, so this times the device-side planning, not the host's push rate.
+            qtimes = []
+            ids_l = [[int(x) for x in st] for st in stages]
+            wsq = torch.empty(max(4 * wsb, 64 << 20), dtype=torch.uint8, device=dev)
+            for i in range(3 + 10):
+                qu = cp.Queue(pool_l, max_stages=len(stages) + 1)
+                for st_ids, dp in zip(ids_l, deps):
+                    qu.push(st_ids, dp, 1.0)
+                qu.close_queue()
+                spacer(i)
+                e0.record()
+                qu.launch(qs, outs, lses, wsq, wsq.numel(), 2000, dw.stream())
+                e1.record()
+                torch.cuda.synchronize()
+                qtimes.append(e0.elapsed_time(e1))
+                qst = qu.status(dw.stream())
+                qu.free()
+            del wsq
             # the same stages as separate launches (plain steps, no dependency between them)
             offs, ro = [], 0
             for b, l in order:
@@ -672,7 +692,9 @@ def main():
             kv_bytes = sum(w.requests[i].context_len * w.models[w.requests[i].model_id].n_kv_heads * 512
                            for b, _ in order for i in batches[b])
             t1, t2 = float(np.median(one[3:])), float(np.median(sep[3:]))
+            tq = float(np.median(qtimes[3:]))
             return {"stages": len(order), "kv_bytes": int(kv_bytes), "one_launch_us": 1e3 * t1,
+                    "queue_launch_us": 1e3 * tq, "queue_us_per_stage": 1e3 * tq / len(order), "queue_device_error": qst["error"],
                     "separate_launches_us": 1e3 * t2, "one_launch_us_per_stage": 1e3 * t1 / len(order),
                     "separate_us_per_stage": 1e3 * t2 / len(order),
                     "host_driven_us_per_stage_wall": 1e3 * t3 / len(order), "one_launch_gbs": kv_bytes / (t1 * 1e-3) / 1e9,

@@ -400,6 +400,41 @@ cp_status cp_pool_counters(const cp_pool *pool, uint64_t *kernel_launches,
  * cap_ctas x 16 uint64; n_ctas_out receives the number of CTA rows available (the SM count). */
 cp_status cp_pool_read_timeline(cp_pool *pool, uint64_t *stamps_out_host, int32_t cap_ctas, int32_t *n_ctas_out);
 
+/*
+ * Request queue of a persistent launch: "persistent kernels repeatedly poll per-model request
+ * queues on GPUs, select the next ready batch ... and update the batch state for the next layer", while "the host
+ * remains responsible for coarse-grained admission" (state machine L126-L128).  Unlike
+ * cp_decode_attention_stages, whose stage list is built by the host before the launch, the kernel started by
+ * cp_queue_launch knows NOTHING of the work to come: the host pushes stage descriptors -- a batch of request ids
+ * and the stage that feeds it -- into a ring in mapped host memory WHILE THE KERNEL RUNS, a planner warp on the
+ * GPU cuts every batch into tiles as it arrives (the arithmetic of the host planner, from the device-resident
+ * context lengths and model shapes) and the persistent CTAs consume them; a batch that exits early simply stops
+ * being pushed; cp_queue_close ends the launch.  Stage semantics are those of cp_decode_attention_stages
+ * (reading M1: q = bf16(q_in + alpha * O_dep)); stage s's rows follow stage s - 1's in q / out / lse.
+ *   cp_queue_create   max_stages = capacity of the ring (no wrap: a queue serves one launch).  MQA / GQA / MHA
+ *                     models with 128-wide heads only (the warp-MMA K/V kernel): UNSUPPORTED otherwise.
+ *   cp_queue_launch   starts the persistent kernel on `stream` and returns; workspace_dev holds the split
+ *                     partials of ALL stages (handed out cumulatively; a stage that does not fit ends the
+ *                     launch with error 2).  timeout_ms: a planner that sees no push for that long closes the
+ *                     launch itself (error 1) instead of spinning forever.  The requests' pages and context
+ *                     lengths must not change while the launch runs.
+ *   cp_queue_push     host only, any time before cp_queue_close (before or after the launch): at most 12 distinct
+ *                     mapped requests; dep_stage = index of an earlier stage of the same batch shape, or -1.
+ *                     *stage_index_out receives the stage's index.  Errors: INVALID_ARG, UNKNOWN_REQUEST, UNSUPPORTED.
+ *   cp_queue_close    no further pushes; the kernel drains and exits.
+ *   cp_queue_status   synchronises `stream`; stages / tiles the device planned and the device's error word
+ *                     (0 none, 1 timed out, 2 a capacity was exceeded, 3 malformed entry).
+ */
+typedef struct cp_queue cp_queue;
+cp_status cp_queue_create(cp_pool *pool, int32_t max_stages, cp_queue **out);
+cp_status cp_queue_launch(cp_queue *q, const void *q_dev, float *out_dev, float *lse_dev, void *workspace_dev,
+                          uint64_t workspace_bytes, uint32_t timeout_ms, void *stream);
+cp_status cp_queue_push(cp_queue *q, const int32_t *request_ids_host, int32_t n_requests, int32_t dep_stage,
+                        float alpha, int32_t *stage_index_out);
+cp_status cp_queue_close(cp_queue *q);
+cp_status cp_queue_status(cp_queue *q, void *stream, int32_t *stages_planned, int32_t *tiles_planned, int32_t *error);
+cp_status cp_queue_free(cp_queue *q);
+
 /* Measurement aids without any part in the hot path (cp_probe.cu; `bench.py --probe ...`).
  * cp_probe_globaltimer: a one-thread kernel on `stream` that stores %globaltimer (ns) to *stamp_dev (8-byte
  *   aligned device memory); bracketing a decode launch with two of them relates the per-CTA stamps of

@@ -107,6 +107,12 @@ def load_library():
         "cp_status_string": (ctypes.c_char_p, [i32]),
         "cp_decode_step_workspace_bytes": (i32, [vp, i32p, i32, u64p]),
         "cp_decode_step": (i32, [vp, i32p, i32, vp, vp, vp, vp, vp, vp, u64, vp]),
+        "cp_queue_create": (i32, [vp, i32, ctypes.POINTER(vp)]),
+        "cp_queue_launch": (i32, [vp, vp, vp, vp, vp, u64, ctypes.c_uint32, vp]),
+        "cp_queue_push": (i32, [vp, i32p, i32, i32, ctypes.c_float, i32p]),
+        "cp_queue_close": (i32, [vp]),
+        "cp_queue_status": (i32, [vp, vp, i32p, i32p, i32p]),
+        "cp_queue_free": (i32, [vp]),
         "cp_probe_globaltimer": (i32, [vp, vp]),
         "cp_probe_read_stream": (i32, [vp, u64, i32, vp, vp]),
         "cp_planner_workspace_bytes": (u64, [ctypes.c_int64]),
@@ -130,7 +136,8 @@ EXPORTED = ["cp_pool_create", "cp_pool_create_vmm", "cp_pool_vmm_info", "cp_pool
             "cp_decode_attention_host", "cp_decode_workspace_bytes_qlen", "cp_decode_attention_qlen",
             "cp_decode_stages_workspace_bytes", "cp_decode_attention_stages", "cp_decode_attention_stages_gated",
             "cp_decode_stages_gate_status", "cp_decode_plan", "cp_pool_counters", "cp_pool_read_timeline", "cp_status_string",
-            "cp_probe_globaltimer", "cp_probe_read_stream", "cp_decode_step_workspace_bytes", "cp_decode_step",
+            "cp_probe_globaltimer", "cp_probe_read_stream", "cp_queue_create", "cp_queue_launch", "cp_queue_push",
+            "cp_queue_close", "cp_queue_status", "cp_queue_free", "cp_decode_step_workspace_bytes", "cp_decode_step",
             "cp_planner_workspace_bytes", "cp_planner_pool_demand", "cp_planner_quantile"]
 
 
@@ -385,6 +392,40 @@ class Pool:
 
 
 # ---------------------------------------------------------------- KV-cache planner (Eq. (1)-(2))
+class Queue:
+    """Request queue of one persistent launch (cp_queue_*): stages are pushed while the kernel runs."""
+
+    def __init__(self, pool: "Pool", max_stages: int):
+        self._L = load_library()
+        h = ctypes.c_void_p()
+        _check(self._L.cp_queue_create(pool._h, max_stages, ctypes.byref(h)), "cp_queue_create")
+        self._h = h
+        self.pool = pool
+
+    def launch(self, q_dev, out_dev, lse_dev, workspace_dev, workspace_bytes: int, timeout_ms: int = 2000, stream: int = 0):
+        _check(self._L.cp_queue_launch(self._h, _ptr(q_dev), _ptr(out_dev), _ptr(lse_dev), _ptr(workspace_dev),
+                                       workspace_bytes, timeout_ms, stream), "cp_queue_launch")
+
+    def push(self, request_ids, dep_stage: int = -1, alpha: float = 0.0) -> int:
+        ids = _ids(request_ids)
+        out = ctypes.c_int32()
+        _check(self._L.cp_queue_push(self._h, _i32p(ids), ids.size, dep_stage, alpha, ctypes.byref(out)), "cp_queue_push")
+        return int(out.value)
+
+    def close_queue(self):
+        _check(self._L.cp_queue_close(self._h), "cp_queue_close")
+
+    def status(self, stream: int = 0):
+        a, b, c = ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32()
+        _check(self._L.cp_queue_status(self._h, stream, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)), "cp_queue_status")
+        return {"stages_planned": a.value, "tiles_planned": b.value, "error": c.value}
+
+    def free(self):
+        if self._h:
+            self._L.cp_queue_free(self._h)
+            self._h = None
+
+
 def probe_globaltimer(stamp_dev, stream: int = 0):
     """One-thread kernel on `stream` that stores %globaltimer (ns) to the 8-byte device location stamp_dev."""
     _check(load_library().cp_probe_globaltimer(_ptr(stamp_dev), stream), "cp_probe_globaltimer")

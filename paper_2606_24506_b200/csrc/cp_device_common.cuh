@@ -210,13 +210,16 @@ __device__ __forceinline__ float ex2_ftz(float x)     // 2^x; ex2(-inf) = 0
 
 // Deliberately compact (short loops, 32-bit offsets): the code runs once per
 // launch per warp, so its cost is dominated by cold instruction-cache misses, not by issue slots.
+// CG: the records were written during this launch (request queue: the planner warp of CTA 0): read them from
+// the L2 (ld.cg), not through the non-coherent path, whose lines may predate the write.
+template <bool CG = false>
 __device__ __forceinline__ CombineUnit load_combine_unit(const CombineUnit *units, int u)
 {
     CombineUnit cu;
     const uint4 *src = reinterpret_cast<const uint4 *>(units + u);
     uint4 *dst = reinterpret_cast<uint4 *>(&cu);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) dst[i] = __ldg(src + i);
+    for (int i = 0; i < 4; ++i) dst[i] = CG ? __ldcg(src + i) : __ldg(src + i);
     return cu;
 }
 
@@ -225,19 +228,19 @@ __device__ __forceinline__ CombineUnit load_combine_unit(const CombineUnit *unit
 // already seen complete is not polled again (units are sorted by group).
 // STAGED (multi-stage launches): the units u < end of one stage; every finished unit is counted in
 // the stage's completion counter (release), which the dependent stage's tiles acquire.
-template <int U3, bool STAGED = false>
+template <int U3, bool STAGED = false, bool CG = false>
 static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, const int stride, float *wsm, const int lane,
                                                   const int end = 0)
 {
     const int n_end = STAGED ? end : p.n_combine_units;
     if (u >= n_end) return;
-    CombineUnit cu = load_combine_unit(p.cunits, u);
+    CombineUnit cu = load_combine_unit<CG>(p.cunits, u);
     int done_group = -1;
     for (;;) {
         const int un = u + stride;
         const bool has_next = un < n_end;
         CombineUnit nx;
-        if (has_next) nx = load_combine_unit(p.cunits, un);
+        if (has_next) nx = load_combine_unit<CG>(p.cunits, un);
         KV_STAMP(8, threadIdx.x == 0);
         const int ns = cu.n_splits;
         const int zl = cu.zl_log2;

@@ -119,6 +119,85 @@ struct StageRec {
 };
 static_assert(sizeof(StageRec) == 32, "StageRec is loaded as two 16-byte vectors");
 
+// Splits per request of one tile plan (hot-path step a1) -- the arithmetic shared by the host planner
+// (build_plan) and the device-side planner of the request queue (cp_queue_*), so that a stage
+// planned on the GPU is cut exactly like the same batch planned on the host.  n_lp[b] = logical pages of
+// request b, hkv[b] = its kv heads (groups).  Smallest tile length L (pages) for which the batch yields at most
+// target_tiles tiles (searched in [L_bal, 2 L_bal]; a batch of many short requests cannot meet the target at
+// all -- every group is at least one tile -- and keeps the balanced length L_bal); then the tiles still missing
+// from the target go, one at a time, to the request whose tiles are longest.  Depends on the page counts only.
+__host__ __device__ inline void plan_request_splits(int n, const int *n_lp, const int *hkv, int64_t target_tiles,
+                                                    int min_tile_pages, int max_splits, int *splits)
+{
+    // (32-bit divisions and an integer comparison of the tile lengths: the device-side planner runs this on one
+    // thread of a GPU whose 64-bit integer and floating-point division are slow)
+    int64_t total = 0;
+    for (int b = 0; b < n; ++b) total += (int64_t)n_lp[b] * hkv[b];
+    if (total == 0) return;
+    auto tiles_for = [&](int len) {
+        int64_t t = 0;
+        for (int b = 0; b < n; ++b) t += (int64_t)hkv[b] * ((n_lp[b] + len - 1) / len);
+        return t;
+    };
+    int64_t L_bal64 = (total + target_tiles - 1) / target_tiles;
+    if (L_bal64 < min_tile_pages) L_bal64 = min_tile_pages;
+    if (L_bal64 > (1 << 29)) L_bal64 = 1 << 29;
+    const int L_bal = (int)L_bal64;
+    int L = L_bal;
+    if (tiles_for(2 * L_bal) <= target_tiles) {
+        int lo = L_bal, hi = 2 * L_bal;
+        while (lo < hi) {
+            const int mid = lo + (hi - lo) / 2;
+            if (tiles_for(mid) <= target_tiles) hi = mid; else lo = mid + 1;
+        }
+        L = lo;
+    }
+    int64_t have = 0;
+    for (int b = 0; b < n; ++b) {
+        if (hkv[b] == 0) { splits[b] = 0; continue; }
+        int sp = (n_lp[b] + L - 1) / L;
+        if (sp > max_splits) sp = max_splits;
+        splits[b] = sp;
+        have += (int64_t)sp * hkv[b];
+    }
+    while (have < target_tiles) {
+        // the request whose tiles are longest, n_lp / splits compared exactly as a fraction (first one wins a tie)
+        int best = -1;
+        for (int b = 0; b < n; ++b) {
+            if (hkv[b] == 0 || have + hkv[b] > target_tiles) continue;
+            if (splits[b] + 1 > max_splits || n_lp[b] / (splits[b] + 1) < min_tile_pages) continue;
+            if (best < 0 || (int64_t)n_lp[b] * splits[best] > (int64_t)n_lp[best] * splits[b]) best = b;
+        }
+        if (best < 0) break;
+        splits[best] += 1;
+        have += hkv[best];
+    }
+}
+
+// Request queue of a persistent launch (cp_queue_*; "persistent kernels repeatedly
+// poll per-model request queues on GPUs, select the next ready batch ...").  One entry = one stage = one
+// attention step of one batch.  Written by the HOST into mapped pinned memory after the kernel has started;
+// the planner warp of CTA 0 polls `tail`, cuts the batch into tiles on arrival and publishes them in QueueState.
+constexpr int kQueueMaxReq = 12;
+struct QueueEntry {
+    int32_t n_req;
+    int32_t dep;            // stage whose output feeds this one's queries (same batch shape), or -1
+    float alpha;
+    int32_t close;          // 1: no further entries; the kernel drains and exits
+    int32_t ids[kQueueMaxReq];
+};
+static_assert(sizeof(QueueEntry) == 64, "QueueEntry is one 64-byte record");
+struct QueueState {         // device memory; planner (CTA 0) -> every CTA
+    int32_t planned_tiles;  // tile records [0, planned_tiles) are complete
+    int32_t planned_stages;
+    int32_t closed;         // 1: planned_tiles / planned_stages are final
+    int32_t error;          // 1 queue poll timed out, 2 a capacity (tiles / units / groups / workspace) was exceeded,
+                            // 3 an entry was malformed (request not mapped, unsupported shape, dep)
+    int32_t n_units, n_groups;
+    int32_t pad[2];
+    int64_t q_rows, ws_floats;        // running totals: query / output rows and workspace floats handed out
+};
+
 // Kernel arguments common to all decode kernels (passed by value).
 struct DecodeParams {
     const uint8_t *arena;
@@ -157,6 +236,16 @@ struct DecodeParams {
     int32_t *stage_done;           // [n_stages] completion counters, kCounterStride apart
     int32_t n_stages;
     unsigned long long *timeline;  // CP_OPT_TIMELINE: [grid][kTimelineSlots] globaltimer stamps, or nullptr
+    // request queue (cp_queue_launch) only, else nullptr / 0
+    const QueueEntry *queue;       // [q_max_stages] host-written entries (mapped pinned memory)
+    const int32_t *queue_tail;     // entries pushed so far (mapped pinned memory)
+    QueueState *qstate;
+    const int32_t *req_model;      // [max_requests] model of every mapped request, -1 if none
+    int64_t *q_out_base;           // [q_max_stages] first output row of every planned stage
+    int32_t *q_target;             // [q_max_stages] completion signals that mean "stage complete"
+    int32_t q_max_stages, q_max_tiles, q_max_units, q_max_groups;
+    int32_t q_target_tiles, q_min_tile_pages;
+    int64_t q_ws_floats_cap;
     const uint16_t *app_k, *app_v; // cp_decode_step: packed new K / V rows the launch writes at position
                                    // context_len - 1 of every request before the page that holds it is read, or nullptr
 };

@@ -265,6 +265,187 @@ __device__ __forceinline__ uint32_t stage_query2(uint32_t q_in, float2 o, float 
     return ra | (rb << 16);
 }
 
+// ---------------------------------------------------------------------------------------
+// Device-side tile planner of the request queue (cp_queue_*; the persistent
+// kernel "repeatedly poll[s] per-model request queues on GPUs, select[s] the next ready batch ... and update[s]
+// the batch state for the next layer").  Run by ONE warp (the planner warp of CTA 0) while the other warps of
+// the grid stream KV: it waits for the host to push entry s into the mapped ring, cuts the batch into tiles with
+// the same arithmetic as the host planner (plan_request_splits: a stage planned here is cut exactly like the
+// same batch planned by cp_decode_attention), writes the stage's tile records, combine units and StageRec into
+// the launch's work list and publishes them with a release; the producers of all CTAs acquire
+// QueueState::planned_tiles before they take a tile.  Everything a stage needs is derived from device-resident
+// tables (context lengths, request -> model, model shapes): the host sends request ids and a dependency only.
+// ---------------------------------------------------------------------------------------
+__device__ __noinline__ void queue_planner(const DecodeParams &p, const int lane)
+{
+    TileRec *recs = const_cast<TileRec *>(p.tile_recs);
+    CombineUnit *units = const_cast<CombineUnit *>(p.cunits);
+    StageRec *stages = const_cast<StageRec *>(p.stages);
+    QueueState *qs = p.qstate;
+    const int P = (int)p.page_tokens;
+    int n_tiles = 0, n_units = 0, n_groups = 0, n_stages = 0, err = 0;
+    int64_t rows = 0, ws = 0;
+    for (int s = 0; s < p.q_max_stages && !err; ++s) {
+        // ---- wait for entry s (system-scope acquire: the host wrote the entry, then the tail)
+        int have = 0;
+        if (lane == 0) {
+            unsigned ns = 128;
+            const unsigned long long t0 = global_timer_ns();
+            while ((have = ld_acquire_sys(p.queue_tail)) <= s) {
+                __nanosleep(ns);
+                if (ns < 2048) ns <<= 1;
+                if (global_timer_ns() - t0 > (unsigned long long)p.gate_timeout_us * 1000ull) { have = -1; break; }
+            }
+        }
+        have = __shfl_sync(0xffffffffu, have, 0);
+        if (have < 0) { err = 1; break; }
+        int word = 0;
+        if (lane < 16) asm volatile("ld.relaxed.sys.global.s32 %0, [%1];" : "=r"(word) : "l"(reinterpret_cast<const int32_t *>(p.queue + s) + lane) : "memory");
+        const int n_req = __shfl_sync(0xffffffffu, word, 0);
+        const int dep = __shfl_sync(0xffffffffu, word, 1);
+        const float alpha = __int_as_float(__shfl_sync(0xffffffffu, word, 2));
+        const int close = __shfl_sync(0xffffffffu, word, 3);
+        if (close) break;
+        if (n_req < 1 || n_req > kQueueMaxReq || dep >= s) { err = 3; break; }
+        // ---- per request: model shape, pages (lane b = request b), then the splits (lane 0, sequential: <= 12 requests)
+        const int my_req = __shfl_sync(0xffffffffu, word, 4 + (lane < n_req ? lane : 0));
+        int my_lp = 0, my_hkv = 0, my_hpk = 0, my_hq = 0, bad = 0;
+        float my_scale = 0.f;
+        if (lane < n_req) {
+            const int mid = my_req >= 0 ? __ldg(p.req_model + my_req) : -1;
+            if (mid < 0) bad = 1;
+            else {
+                const DevModel m = p.models[mid];
+                if (m.kind != 0 || m.d_k != KV_D || m.d_v != KV_D || m.group > 128) bad = 1;
+                my_hkv = m.n_kv_heads; my_hpk = m.group; my_hq = m.n_q_heads; my_scale = m.scale_log2;
+                my_lp = (__ldg(p.req_ctx + my_req) + P - 1) / P;
+                if (my_lp < 1) bad = 1;
+            }
+        }
+        if (__any_sync(0xffffffffu, bad)) { err = 3; break; }
+        int my_splits = 0;
+        {
+            int v_lp[kQueueMaxReq], v_hkv[kQueueMaxReq], v_sp[kQueueMaxReq];
+#pragma unroll
+            for (int b = 0; b < kQueueMaxReq; ++b) {
+                v_lp[b] = __shfl_sync(0xffffffffu, my_lp, b);
+                v_hkv[b] = b < n_req ? __shfl_sync(0xffffffffu, my_hkv, b) : 0;
+                if (b >= n_req) v_lp[b] = 0;
+                v_sp[b] = 0;
+            }
+            if (lane == 0) plan_request_splits(n_req, v_lp, v_hkv, p.q_target_tiles, p.q_min_tile_pages, kMaxSplits, v_sp);
+#pragma unroll
+            for (int b = 0; b < kQueueMaxReq; ++b) {
+                const int sp = __shfl_sync(0xffffffffu, v_sp[b], 0);
+                if (lane == b) my_splits = sp;
+            }
+        }
+        // ---- capacities
+        int st_tiles = my_splits * my_hkv, st_groups = my_hkv, st_rows = my_hq;
+        for (int o = 16; o > 0; o >>= 1) {
+            st_tiles += __shfl_xor_sync(0xffffffffu, st_tiles, o);
+            st_groups += __shfl_xor_sync(0xffffffffu, st_groups, o);
+            st_rows += __shfl_xor_sync(0xffffffffu, st_rows, o);
+        }
+        if (n_tiles + st_tiles > p.q_max_tiles || n_groups + st_groups > p.q_max_groups) { err = 2; break; }
+        // ---- emit, request by request, kv head by kv head (all lanes walk together; parameters by shuffle)
+        const int cu_begin = n_units;
+        int direct = 0;                  // completion signals of single-split tiles (one per padded M tile)
+        int64_t row_b = 0;
+        for (int b = 0; b < n_req && !err; ++b) {
+            const int req = __shfl_sync(0xffffffffu, my_req, b), n_lp = __shfl_sync(0xffffffffu, my_lp, b);
+            const int hkv = __shfl_sync(0xffffffffu, my_hkv, b), hpk = __shfl_sync(0xffffffffu, my_hpk, b);
+            const int hq = __shfl_sync(0xffffffffu, my_hq, b), nsp = __shfl_sync(0xffffffffu, my_splits, b);
+            const float scale = __shfl_sync(0xffffffffu, my_scale, b);
+            int mtp = 1;
+            while (mtp < (hpk + 15) / 16) mtp <<= 1;
+            for (int c = 0; c < hkv && !err; ++c) {
+                const int gi = n_groups++;
+                const int64_t row0 = rows + row_b + (int64_t)c * hpk;
+                int64_t part_off = 0;
+                if (nsp > 1) {
+                    part_off = ws;
+                    ws += part_group_floats(hpk, nsp, KV_D);
+                    if (ws > p.q_ws_floats_cap) { err = 2; break; }
+                }
+                // tiles: near-equal page-aligned splits, lane t writes tile t (six 16-byte stores)
+                const int base = n_lp / nsp, rem = n_lp % nsp;
+                for (int t0 = 0; t0 < nsp; t0 += 32) {
+                    const int t = t0 + lane;
+                    if (t < nsp) {
+                        TileRec r;
+                        r.group = gi; r.req = req; r.kv_head = c; r.n_kv_heads = hkv;
+                        r.page_begin = t * base + min(t, rem); r.n_pages = base + (t < rem ? 1 : 0);
+                        r.split = t; r.n_splits = nsp; r.gsize = hpk; r.n_q_heads = hq; r.scale_log2 = scale; r.pad = s;
+                        r.q_off = row0 * KV_D; r.out_off = row0 * KV_D; r.lse_off = row0; r.part_off = part_off;
+                        r.app_k_off = 0; r.app_v_off = 0;
+                        uint4 *dst = reinterpret_cast<uint4 *>(recs + n_tiles + t);
+                        const uint4 *src = reinterpret_cast<const uint4 *>(&r);
+#pragma unroll
+                        for (int i = 0; i < 6; ++i) __stcg(dst + i, src[i]);
+                    }
+                }
+                n_tiles += nsp;
+                if (nsp == 1) direct += mtp;
+                else {
+                    // combine units: one per (head, column block), as the host planner lays them out
+                    const int zl = nsp <= 8 ? 0 : (nsp <= 32 ? 3 : (nsp <= 128 ? 4 : 5));
+                    const int cols = 128 >> zl, nb = KV_D / cols, nu = hpk * nb;
+                    if (n_units + nu > p.q_max_units) { err = 2; break; }
+                    for (int u0 = 0; u0 < nu; u0 += 32) {
+                        const int u = u0 + lane;
+                        if (u < nu) {
+                            const int h = u / nb, c0 = (u % nb) * cols;
+                            CombineUnit cu;
+                            cu.part_off = part_off + part_o_off(h, 0, nsp, KV_D) + c0;
+                            cu.ml_off = part_off + part_ml_off(hpk, h, 0, nsp, KV_D);
+                            cu.out_off = (row0 + h) * KV_D + c0;
+                            cu.lse_off = c0 == 0 ? row0 + h : -1;
+                            cu.split_stride = KV_D; cu.n_splits = nsp; cu.zl_log2 = zl; cu.want = nsp * mtp;
+                            cu.group = gi; cu.pad[0] = s; cu.pad[1] = 0; cu.pad[2] = 0;
+                            uint4 *dst = reinterpret_cast<uint4 *>(units + n_units + u);
+                            const uint4 *src = reinterpret_cast<const uint4 *>(&cu);
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) __stcg(dst + i, src[i]);
+                        }
+                    }
+                    n_units += nu;
+                }
+            }
+            row_b += hq;
+        }
+        if (err) break;
+        if (lane == 0) {
+            StageRec sr;
+            sr.dep = dep; sr.dep_target = dep >= 0 ? __ldcg(p.q_target + dep) : 0;
+            sr.cu_begin = cu_begin; sr.cu_end = n_units;
+            sr.dep_out_delta = dep >= 0 ? (__ldcg(p.q_out_base + dep) - rows) * KV_D : 0;
+            sr.alpha = alpha; sr.pad = 0;
+            uint4 *dst = reinterpret_cast<uint4 *>(stages + s);
+            const uint4 *src = reinterpret_cast<const uint4 *>(&sr);
+            __stcg(dst, src[0]);
+            __stcg(dst + 1, src[1]);
+            __stcg(p.q_target + s, (n_units - cu_begin) + direct);
+            __stcg(p.q_out_base + s, rows);
+        }
+        rows += st_rows;
+        n_stages = s + 1;
+        // ---- publish: the stage's records happen-before the counters (cumulative release over the warp barrier)
+        __syncwarp();
+        if (lane == 0) {
+            __threadfence();
+            asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(&qs->planned_stages), "r"(n_stages) : "memory");
+            asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(&qs->planned_tiles), "r"(n_tiles) : "memory");
+        }
+    }
+    if (lane == 0) {
+        qs->error = err; qs->n_units = n_units; qs->n_groups = n_groups; qs->q_rows = rows; qs->ws_floats = ws;
+        __threadfence();
+        asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(&qs->planned_stages), "r"(n_stages) : "memory");
+        asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(&qs->closed), "r"(1) : "memory");
+    }
+}
+
 // MULTI: the work list is the concatenation of several stages (cp_decode_attention_stages): a CTA
 // runs its combine units of every earlier stage before it starts a tile of a later one, and a tile
 // of a dependent stage waits for its predecessor's completion counter before it builds its queries
@@ -272,8 +453,8 @@ __device__ __forceinline__ uint32_t stage_query2(uint32_t q_in, float2 o, float 
 // QLEN: q_len > 1 query tokens per request (cp_decode_attention_qlen).  Row r of a group is query token
 // r / g, head r % g of the kv head's g heads; its causal limit ends q_len - 1 - r / g tokens before the
 // context's end.
-template <int P, bool MULTI, bool QLEN>
-__global__ void __launch_bounds__(KV_THREADS, 1)
+template <int P, int MULTI, bool QLEN>      // MULTI: 0 one step, 1 host-built stage list, 2 request queue (stages planned on the device)
+__global__ void __launch_bounds__(KV_THREADS + 32, 1)
 cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap, int rows_per_page)
 {
     constexpr int STAGE_BYTES = P * 4 * KV_D;
@@ -325,14 +506,35 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 if (lane == 0) work = atomicAdd(p.work_counter, 1) + (int)gridDim.x;
                 work = __shfl_sync(0xffffffffu, work, 0);
             }
-            const int item = work < p.n_tiles ? work : -1;      // tiles only; combine units are static
+            int item = work < p.n_tiles ? work : -1;      // tiles only; combine units are static
+            int final_stages = p.n_stages;
+            if constexpr (MULTI == 2) {
+                // request queue: tile `work` exists once the planner (CTA 0) has published more than `work` tiles;
+                // after the close marker the counts are final
+                int pt = 0, cl = 0;
+                if (lane == 0) {
+                    unsigned ns = 64;
+                    for (;;) {
+                        pt = ld_acquire(&p.qstate->planned_tiles);
+                        if (pt > work) break;
+                        cl = ld_acquire(&p.qstate->closed);
+                        if (cl) { pt = ld_acquire(&p.qstate->planned_tiles); break; }
+                        __nanosleep(ns);
+                        if (ns < 1024) ns <<= 1;
+                    }
+                    final_stages = cl ? ld_acquire(&p.qstate->planned_stages) : 0;
+                }
+                pt = __shfl_sync(0xffffffffu, pt, 0);
+                final_stages = __shfl_sync(0xffffffffu, final_stages, 0);
+                item = work < pt ? work : -1;
+            }
             TileRec r;
             int ctx = 0, mt = 1;
             if (item >= 0) {
                 const uint4 *src = reinterpret_cast<const uint4 *>(p.tile_recs + item);
                 uint4 *dst = reinterpret_cast<uint4 *>(&r);
 #pragma unroll
-                for (int i = 0; i < 5; ++i) dst[i] = __ldg(src + i);
+                for (int i = 0; i < 5; ++i) dst[i] = MULTI == 2 ? __ldcg(src + i) : __ldg(src + i);
                 ctx = __ldg(p.req_ctx + r.req);
                 mt = kv_mtiles(r.gsize);
             } else {
@@ -370,7 +572,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 d.npg = r.n_pages; d.split = r.split; d.n_splits = r.n_splits;
                 d.ctx = ctx; d.gsize = r.gsize; d.mt = mt; d.scale_log2 = r.scale_log2;
                 d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
-                d.stage = r.pad; d.hq = r.n_q_heads;
+                d.stage = item >= 0 ? r.pad : final_stages; d.hq = r.n_q_heads;
                 tq[qs] = d;
                 mbar_arrive(smem_u32(tqf_b + qs));     // release: consumers acquire via try_wait
             }
@@ -407,6 +609,11 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 }
             }
         }
+    } else if (warp == KV_CWARPS + 1) {
+        // =========================================================== planner warp (request queue; CTA 0 only)
+        if constexpr (MULTI == 2) {
+            if (blockIdx.x == 0) queue_planner(p, lane);
+        }
     } else {
         // =========================================================== consumer warps
         uint32_t pc = 0;          // pages consumed by this CTA so far (ring position of tile start)
@@ -428,13 +635,14 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
             ++qi;
             if constexpr (MULTI) {
                 // combine units of every stage before this tile's (all of them once the list is exhausted)
-                const int upto = d.item < 0 ? p.n_stages : d.stage;
+                const int upto = d.stage;           // the end marker carries the number of stages
                 if (upto > cur_stage) {
                     consumer_bar();                 // the merge slots of the previous tile are free
                     for (int s = cur_stage; s < upto; ++s) {
-                        const int2 cur = __ldg(reinterpret_cast<const int2 *>(&p.stages[s].cu_begin));
-                        combine_units<8, true>(p, cur.x + blockIdx.x * KV_CWARPS + warp, gridDim.x * KV_CWARPS,
-                                               merge + warp * KV_COMBINE_WARP_FLOATS, lane, cur.y);
+                        const int2 cur = MULTI == 2 ? __ldcg(reinterpret_cast<const int2 *>(&p.stages[s].cu_begin))
+                                                    : __ldg(reinterpret_cast<const int2 *>(&p.stages[s].cu_begin));
+                        combine_units<8, true, MULTI == 2>(p, cur.x + blockIdx.x * KV_CWARPS + warp, gridDim.x * KV_CWARPS,
+                                                           merge + warp * KV_COMBINE_WARP_FLOATS, lane, cur.y);
                     }
                     consumer_bar();                 // combine scratch is free before the next merge
                     cur_stage = upto;
@@ -476,13 +684,15 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                     qf[ks][3] = h1 < gsize ? __ldg(reinterpret_cast<const uint32_t *>(q1 + k + 8)) : 0u;
                 }
                 if constexpr (MULTI) {
-                    const int4 s0 = __ldg(reinterpret_cast<const int4 *>(p.stages + d.stage));
+                    const int4 s0 = MULTI == 2 ? __ldcg(reinterpret_cast<const int4 *>(p.stages + d.stage))
+                                               : __ldg(reinterpret_cast<const int4 *>(p.stages + d.stage));
                     if (s0.x >= 0) {
                         // the predecessor's output is complete: all its combine units and single-split
                         // tiles have signalled (acquire; the other lanes follow through the __syncwarp)
                         if (lane == 0) wait_group(p.stage_done, s0.x, s0.y);
                         __syncwarp();
-                        const int4 s1 = __ldg(reinterpret_cast<const int4 *>(p.stages + d.stage) + 1);
+                        const int4 s1 = MULTI == 2 ? __ldcg(reinterpret_cast<const int4 *>(p.stages + d.stage) + 1)
+                                                   : __ldg(reinterpret_cast<const int4 *>(p.stages + d.stage) + 1);
                         const int64_t delta = (int64_t)(uint32_t)s1.x | ((int64_t)s1.y << 32);
                         const float alpha = __int_as_float(s1.z);
                         const float *o0 = p.out + d.out_off + delta + (int64_t)h0 * KV_D;
@@ -692,18 +902,22 @@ extern "C" int cp_kv_probe_read(unsigned long long *out_host)
 
 bool kv_fast_supported(int P) { return P == 16 || P == 32 || P == 64 || P == 128; }
 
-template <int P, bool MULTI, bool QLEN>
+template <int P, int MULTI, bool QLEN>
 static cudaError_t launch_kv_tm(const DecodeParams &p, const CUtensorMap &tmap, int rows_per_page, int grid,
                                 cudaStream_t stream)
 {
     const int smem = kv_smem_bytes(P);
-    static bool configured = false;
-    if (!configured) {
+    static bool configured[64] = {};              // per device: the attribute belongs to the device's copy of the function
+    int dev = 0;
+    cudaError_t e0 = cudaGetDevice(&dev);
+    if (e0 != cudaSuccess) return e0;
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
         cudaError_t e = cudaFuncSetAttribute(cp_decode_kv_kernel<P, MULTI, QLEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (dev >= 0 && dev < 64) configured[dev] = true;
     }
-    cp_decode_kv_kernel<P, MULTI, QLEN><<<grid, KV_THREADS, smem, stream>>>(p, tmap, rows_per_page);
+    // the request queue adds the planner warp (only CTA 0's does anything)
+    cp_decode_kv_kernel<P, MULTI, QLEN><<<grid, MULTI == 2 ? KV_THREADS + 32 : KV_THREADS, smem, stream>>>(p, tmap, rows_per_page);
     return cudaGetLastError();
 }
 
@@ -711,9 +925,10 @@ template <int P>
 static cudaError_t launch_kv_t(const DecodeParams &p, const CUtensorMap &tmap, int rows_per_page, int grid,
                                cudaStream_t stream)
 {
-    if (p.n_stages > 0) return launch_kv_tm<P, true, false>(p, tmap, rows_per_page, grid, stream);
-    if (p.q_len > 1) return launch_kv_tm<P, false, true>(p, tmap, rows_per_page, grid, stream);
-    return launch_kv_tm<P, false, false>(p, tmap, rows_per_page, grid, stream);
+    if (p.queue != nullptr) return launch_kv_tm<P, 2, false>(p, tmap, rows_per_page, grid, stream);
+    if (p.n_stages > 0) return launch_kv_tm<P, 1, false>(p, tmap, rows_per_page, grid, stream);
+    if (p.q_len > 1) return launch_kv_tm<P, 0, true>(p, tmap, rows_per_page, grid, stream);
+    return launch_kv_tm<P, 0, false>(p, tmap, rows_per_page, grid, stream);
 }
 
 cudaError_t launch_decode_kv(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas,
@@ -723,6 +938,7 @@ cudaError_t launch_decode_kv(const DecodeParams &p, const void *tmap, int rows_p
     int grid = p.n_tiles > (p.n_combine_units + KV_CWARPS - 1) / KV_CWARPS
                    ? p.n_tiles : (p.n_combine_units + KV_CWARPS - 1) / KV_CWARPS;
     if (grid > n_ctas) grid = n_ctas;
+    if (p.queue != nullptr) grid = n_ctas;          // the work is not known yet
     if (grid < 1) grid = 1;
     switch (p.page_tokens) {
     case 16: return launch_kv_t<16>(p, tm, rows_per_page, grid, stream);

@@ -439,60 +439,18 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             continue;
         }
         kp.grid = 0; kp.n_static_slots = 0;
-        auto tiles_for = [&](int64_t len) {
-            int64_t t = 0;
-            for (int b = 0; b < n; ++b) {
-                const Request &r = pool->reqs[ids[b]];
-                const cp_model_cfg &m = pool->models[r.model];
-                if (m.kind == k) t += (int64_t)m.n_kv_heads * ((ceil_div(r.ctx, P) + len - 1) / len);
-            }
-            return t;
-        };
-        // smallest tile length L (pages) for which the batch yields at most target_tiles tiles
-        // (searched in [L_bal, 2 L_bal]; a batch of many short requests cannot meet the target at
-        // all -- every group is at least one tile -- and then keeps the balanced length L_bal)
-        const int64_t L_bal = std::max<int64_t>((total_pages[k] + target_tiles - 1) / target_tiles,
-                                                pool->opt_min_tile_pages);
-        int64_t L = L_bal;
-        if (tiles_for(2 * L_bal) <= target_tiles) {
-            int64_t lo = L_bal, hi = 2 * L_bal;
-            while (lo < hi) {
-                const int64_t mid = (lo + hi) / 2;
-                if (tiles_for(mid) <= target_tiles) hi = mid; else lo = mid + 1;
-            }
-            L = lo;
-        }
-        // splits per request: ceil(pages / L), then the tiles still missing from the target go, one at a
-        // time, to the request whose tiles are longest (so that with waves = w every persistent CTA gets
-        // exactly w near-equal tiles whenever the groups allow it; one tile more on a few CTAs would cost
-        // a whole extra tile time at the end).  Depends on the context lengths only (deterministic).
+        // splits per request (shared with the device-side planner of the request queue: plan_request_splits)
         std::vector<int> req_splits(n, 0);
         {
-            int64_t have = 0;
+            std::vector<int> v_lp(n, 0), v_hkv(n, 0);
             for (int b = 0; b < n; ++b) {
                 const Request &r = pool->reqs[ids[b]];
                 const cp_model_cfg &m = pool->models[r.model];
                 if (m.kind != k) continue;
-                const int n_lp = ceil_div(r.ctx, P);
-                req_splits[b] = (int)std::min<int64_t>((n_lp + L - 1) / L, kMaxSplits);
-                have += (int64_t)req_splits[b] * m.n_kv_heads;
+                v_lp[b] = ceil_div(r.ctx, P);
+                v_hkv[b] = m.n_kv_heads;
             }
-            while (have < target_tiles) {
-                int best = -1;
-                double best_len = 0.0;
-                for (int b = 0; b < n; ++b) {
-                    const Request &r = pool->reqs[ids[b]];
-                    const cp_model_cfg &m = pool->models[r.model];
-                    if (m.kind != k || have + m.n_kv_heads > target_tiles) continue;
-                    const int n_lp = ceil_div(r.ctx, P);
-                    if (req_splits[b] + 1 > kMaxSplits || n_lp / (req_splits[b] + 1) < pool->opt_min_tile_pages) continue;
-                    const double len = (double)n_lp / req_splits[b];
-                    if (len > best_len) { best_len = len; best = b; }
-                }
-                if (best < 0) break;
-                req_splits[best] += 1;
-                have += pool->models[pool->reqs[ids[best]].model].n_kv_heads;
-            }
+            plan_request_splits(n, v_lp.data(), v_hkv.data(), target_tiles, pool->opt_min_tile_pages, kMaxSplits, req_splits.data());
         }
         for (int b = 0; b < n; ++b) {
             const Request &r = pool->reqs[ids[b]];
@@ -1253,6 +1211,7 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         st = upload_plan(pool, kp, s);
         if (st != CP_OK) return st;
         DecodeParams prm;
+        std::memset(&prm, 0, sizeof(prm));            // every field a launch does not use is null / 0
         prm.arena = pool->arena; prm.page_tokens = pool->P; prm.page_bytes = pool->page_bytes;
         prm.page_table = (const int32_t *)pool->d_page_table.ptr; prm.max_ppr = pool->max_ppr;
         prm.slot_pages = (pool->vmm && !pool->opt_vmm_table) ? (int32_t)pool->slot_pages : 0;
@@ -1588,6 +1547,7 @@ static cp_status decode_stages_core(cp_pool *pool, int32_t n_stages, const int32
         sp.uploaded = true;
     }
     DecodeParams prm;
+    std::memset(&prm, 0, sizeof(prm));
     prm.arena = pool->arena; prm.page_tokens = pool->P; prm.page_bytes = pool->page_bytes;
     prm.page_table = (const int32_t *)pool->d_page_table.ptr; prm.max_ppr = pool->max_ppr;
     prm.slot_pages = (pool->vmm && !pool->opt_vmm_table) ? (int32_t)pool->slot_pages : 0;
@@ -1737,6 +1697,191 @@ cp_status cp_decode_attention_host(cp_pool *pool, const int32_t *request_ids_hos
                cudaMemcpyAsync(lse_host, l_dev, (size_t)pool->lse_floats * 4, cudaMemcpyDeviceToHost, s) != cudaSuccess)
         return CP_ERR_CUDA;
     if (cudaStreamSynchronize(s) != cudaSuccess) return CP_ERR_CUDA;
+    return CP_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------ request queue of a persistent launch
+struct cp_queue {
+    cp_pool *pool = nullptr;
+    int max_stages = 0, max_tiles = 0, max_units = 0, max_groups = 0;
+    QueueEntry *h_ring = nullptr;        // mapped pinned memory: [max_stages + 1] entries ...
+    int32_t *h_tail = nullptr;           // ... and the tail counter (its own 64-byte line behind them)
+    void *d_ring = nullptr, *d_tail = nullptr;
+    DevBuf d_recs, d_units, d_stages, d_state, d_counters, d_out_base, d_target, d_req_model;
+    int pushed = 0;
+    bool closed = false, launched = false;
+    std::vector<std::vector<int32_t>> stage_models;     // per pushed stage: model of every request (shape check of dependents)
+    int64_t rows_pushed = 0;
+};
+
+extern "C" {
+
+cp_status cp_queue_create(cp_pool *pool, int32_t max_stages, cp_queue **out)
+{
+    if (!out) return CP_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!pool || max_stages < 1 || max_stages > 65536) return CP_ERR_INVALID_ARG;
+    cp_status st = ensure_device(pool);
+    if (st != CP_OK) return st;
+    if (!pool->kv_tmap_ok) return CP_ERR_UNSUPPORTED;
+    cp_queue *q = new (std::nothrow) cp_queue();
+    if (!q) return CP_ERR_INVALID_ARG;
+    q->pool = pool;
+    q->max_stages = max_stages;
+    q->max_tiles = max_stages * 256;
+    q->max_units = max_stages * 2048;
+    q->max_groups = max_stages * 96;
+    const size_t ring_bytes = (size_t)(max_stages + 1) * sizeof(QueueEntry) + 64;
+    void *h = nullptr;
+    if (cudaHostAlloc(&h, ring_bytes, cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); delete q; return CP_ERR_CUDA; }
+    std::memset(h, 0, ring_bytes);
+    q->h_ring = (QueueEntry *)h;
+    q->h_tail = (int32_t *)((uint8_t *)h + (size_t)(max_stages + 1) * sizeof(QueueEntry));
+    void *d = nullptr;
+    if (cudaHostGetDevicePointer(&d, h, 0) != cudaSuccess) { cudaGetLastError(); cudaFreeHost(h); delete q; return CP_ERR_CUDA; }
+    q->d_ring = d;
+    q->d_tail = (uint8_t *)d + (size_t)(max_stages + 1) * sizeof(QueueEntry);
+    const size_t counters = 64 + ((size_t)q->max_groups + (size_t)max_stages) * kCounterStride;
+    if (q->d_recs.ensure((size_t)q->max_tiles * sizeof(TileRec)) != cudaSuccess ||
+        q->d_units.ensure((size_t)q->max_units * sizeof(CombineUnit)) != cudaSuccess ||
+        q->d_stages.ensure((size_t)max_stages * sizeof(StageRec)) != cudaSuccess ||
+        q->d_state.ensure(256) != cudaSuccess || q->d_counters.ensure(counters * 4) != cudaSuccess ||
+        q->d_out_base.ensure((size_t)max_stages * 8) != cudaSuccess || q->d_target.ensure((size_t)max_stages * 4) != cudaSuccess ||
+        q->d_req_model.ensure((size_t)pool->max_requests * 4) != cudaSuccess) {
+        cudaGetLastError();
+        cp_queue_free(q);
+        return CP_ERR_CUDA;
+    }
+    *out = q;
+    return CP_OK;
+}
+
+cp_status cp_queue_free(cp_queue *q)
+{
+    if (!q) return CP_OK;
+    cudaDeviceSynchronize();
+    q->d_recs.release(); q->d_units.release(); q->d_stages.release(); q->d_state.release(); q->d_counters.release();
+    q->d_out_base.release(); q->d_target.release(); q->d_req_model.release();
+    if (q->h_ring) cudaFreeHost(q->h_ring);
+    delete q;
+    return CP_OK;
+}
+
+cp_status cp_queue_push(cp_queue *q, const int32_t *request_ids_host, int32_t n_requests, int32_t dep_stage, float alpha,
+                        int32_t *stage_index_out)
+{
+    if (!q || q->closed || q->pushed >= q->max_stages || !(alpha == alpha)) return CP_ERR_INVALID_ARG;
+    cp_pool *pool = q->pool;
+    cp_status st = check_batch(pool, request_ids_host, n_requests);
+    if (st != CP_OK) return st;
+    if (n_requests > kQueueMaxReq || dep_stage >= q->pushed || dep_stage < -1) return CP_ERR_INVALID_ARG;
+    std::vector<int32_t> models(n_requests);
+    int64_t rows = 0;
+    for (int b = 0; b < n_requests; ++b) {
+        const Request &r = pool->reqs[request_ids_host[b]];
+        const cp_model_cfg &m = pool->models[r.model];
+        if (m.kind != CP_KIND_KV || m.head_dim_qk != 128 || m.head_dim_v != 128 || m.n_q_heads / m.n_kv_heads > 128)
+            return CP_ERR_UNSUPPORTED;
+        models[b] = r.model;
+        rows += m.n_q_heads;
+    }
+    if (dep_stage >= 0 && q->stage_models[dep_stage] != models) return CP_ERR_INVALID_ARG;   // same batch shape as its predecessor
+    QueueEntry e;
+    std::memset(&e, 0, sizeof(e));
+    e.n_req = n_requests; e.dep = dep_stage; e.alpha = alpha; e.close = 0;
+    for (int b = 0; b < n_requests; ++b) e.ids[b] = request_ids_host[b];
+    // entry first, then the tail (release): the planner warp acquires the tail at system scope
+    std::memcpy((void *)&q->h_ring[q->pushed], &e, sizeof(e));
+    __atomic_store_n(q->h_tail, q->pushed + 1, __ATOMIC_RELEASE);
+    if (stage_index_out) *stage_index_out = q->pushed;
+    q->stage_models.push_back(std::move(models));
+    q->rows_pushed += rows;
+    q->pushed++;
+    return CP_OK;
+}
+
+cp_status cp_queue_close(cp_queue *q)
+{
+    if (!q) return CP_ERR_INVALID_ARG;
+    if (q->closed) return CP_OK;
+    QueueEntry e;
+    std::memset(&e, 0, sizeof(e));
+    e.close = 1;
+    std::memcpy((void *)&q->h_ring[q->pushed], &e, sizeof(e));
+    __atomic_store_n(q->h_tail, q->pushed + 1, __ATOMIC_RELEASE);
+    q->closed = true;
+    return CP_OK;
+}
+
+cp_status cp_queue_launch(cp_queue *q, const void *q_dev, float *out_dev, float *lse_dev, void *workspace_dev,
+                          uint64_t workspace_bytes, uint32_t timeout_ms, void *stream)
+{
+    if (!q || q->launched || !q_dev || !out_dev || !lse_dev || timeout_ms == 0) return CP_ERR_INVALID_ARG;
+    if (((uintptr_t)q_dev & 15u) || ((uintptr_t)out_dev & 15u) || ((uintptr_t)lse_dev & 3u) || ((uintptr_t)workspace_dev & 15u))
+        return CP_ERR_INVALID_ARG;
+    cp_pool *pool = q->pool;
+    cp_status st = ensure_device(pool);
+    if (st != CP_OK) return st;
+    if (!pool->kv_tmap_ok) return CP_ERR_UNSUPPORTED;
+    cudaStream_t s = (cudaStream_t)stream;
+    st = flush_tables(pool, s);
+    if (st != CP_OK) return st;
+    std::vector<int32_t> rm(pool->max_requests, -1);
+    for (int i = 0; i < pool->max_requests; ++i)
+        if (pool->reqs[i].live) rm[i] = pool->reqs[i].model;
+    if (cudaMemcpyAsync(q->d_req_model.ptr, rm.data(), rm.size() * 4, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+        cudaMemsetAsync(q->d_state.ptr, 0, 256, s) != cudaSuccess ||
+        cudaMemsetAsync(q->d_counters.ptr, 0, q->d_counters.cap, s) != cudaSuccess)
+        return CP_ERR_CUDA;
+    DecodeParams prm;
+    std::memset(&prm, 0, sizeof(prm));
+    prm.arena = pool->arena; prm.page_tokens = pool->P; prm.page_bytes = pool->page_bytes;
+    prm.page_table = (const int32_t *)pool->d_page_table.ptr; prm.max_ppr = pool->max_ppr;
+    prm.slot_pages = (pool->vmm && !pool->opt_vmm_table) ? (int32_t)pool->slot_pages : 0;
+    prm.req_ctx = (const int32_t *)pool->d_ctx.ptr;
+    prm.models = (const DevModel *)pool->d_models.ptr;
+    prm.tile_recs = (const TileRec *)q->d_recs.ptr;
+    prm.cunits = (const CombineUnit *)q->d_units.ptr;
+    prm.stages = (const StageRec *)q->d_stages.ptr;
+    prm.n_tiles = 0; prm.n_stages = 0; prm.q_len = 1;
+    prm.q = (const uint16_t *)q_dev; prm.out = out_dev; prm.lse = lse_dev; prm.workspace = (float *)workspace_dev;
+    int32_t *ctr = (int32_t *)q->d_counters.ptr;
+    prm.work_counter = ctr;                       // [0] next tile; [32..63] the other set's scheduler words (unused here)
+    prm.reset_counters = ctr + 32; prm.n_groups = 0;
+    prm.group_counters = ctr + 64;
+    prm.stage_done = ctr + 64 + (size_t)q->max_groups * kCounterStride;
+    prm.gate_timeout_us = timeout_ms > 4000000u ? 4000000000u : timeout_ms * 1000u;
+    prm.queue = (const QueueEntry *)q->d_ring; prm.queue_tail = (const int32_t *)q->d_tail;
+    prm.qstate = (QueueState *)q->d_state.ptr;
+    prm.req_model = (const int32_t *)q->d_req_model.ptr;
+    prm.q_out_base = (int64_t *)q->d_out_base.ptr; prm.q_target = (int32_t *)q->d_target.ptr;
+    prm.q_max_stages = q->max_stages; prm.q_max_tiles = q->max_tiles; prm.q_max_units = q->max_units; prm.q_max_groups = q->max_groups;
+    const int n_ctas = std::min(pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm, pool->n_sm);
+    prm.q_target_tiles = std::max(1, n_ctas * pool->opt_waves_x16 / 16);
+    prm.q_min_tile_pages = pool->opt_min_tile_pages;
+    prm.q_ws_floats_cap = (int64_t)(workspace_bytes / 4);
+    const cudaError_t e = launch_decode_kv(prm, pool->kv_tmap, (int)(pool->page_bytes / 256), n_ctas, s);
+    pool->n_launches++;
+    if (e != cudaSuccess) return CP_ERR_CUDA;
+    q->launched = true;
+    return CP_OK;
+}
+
+cp_status cp_queue_status(cp_queue *q, void *stream, int32_t *stages_planned, int32_t *tiles_planned, int32_t *error)
+{
+    if (!q) return CP_ERR_INVALID_ARG;
+    QueueState st;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (cudaMemcpyAsync(&st, q->d_state.ptr, sizeof(st), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaStreamSynchronize(s) != cudaSuccess) {
+        cudaGetLastError();
+        return CP_ERR_CUDA;
+    }
+    if (stages_planned) *stages_planned = st.planned_stages;
+    if (tiles_planned) *tiles_planned = st.planned_tiles;
+    if (error) *error = st.error;
     return CP_OK;
 }
 
