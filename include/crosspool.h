@@ -257,6 +257,13 @@ cp_status cp_decode_workspace_bytes(cp_pool *pool, const int32_t *request_ids_ho
  *   lse_dev  fp32, packed in batch order, per request [Hq] (natural log, scale inside)
  *   workspace_dev / workspace_bytes  >= cp_decode_workspace_bytes(...), 16-B aligned
  * Errors: INVALID_ARG, UNKNOWN_REQUEST, WORKSPACE, CUDA.
+ * Streams: the compute calls of one pool (gather, append, decode*, stages, queue launch) reuse device-side
+ * scheduler state from call to call -- the uploaded work list, two alternating sets of scheduler counters, the
+ * page and context tables.  Calls on ONE stream are ordered by the stream.  A call on another stream than the
+ * pool's previous call first waits (cudaStreamWaitEvent) for everything the previous stream was given, so two
+ * streams may drive one pool in turn; calls are NOT thread-safe, and a launch must not be captured into a CUDA
+ * graph and replayed (the host alternates the counter sets and re-uploads plans between launches).  A batch
+ * with models of both attention kinds launches its second kernel on an internal stream and joins it back.
  */
 cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, int32_t n_requests,
                               const void *q_dev, float *out_dev, float *lse_dev,

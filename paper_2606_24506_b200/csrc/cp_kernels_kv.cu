@@ -548,7 +548,8 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 // to the consumers, and its pages are requested, only once its stage is admitted.  A poll
                 // that outlasts the timeout stops gating and raises a flag instead of hanging the device.
                 if (p.published != nullptr && item >= 0) {
-                    if (lane == 0) {
+                    // (once a poll has timed out the launch stops gating: later tiles do not wait again)
+                    if (lane == 0 && ld_relaxed(p.gate_flag) == 0) {
                         unsigned ns = 256;
                         const unsigned long long t0 = global_timer_ns();
                         while (ld_acquire_sys(p.published) <= r.pad) {

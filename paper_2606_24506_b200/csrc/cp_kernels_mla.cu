@@ -509,12 +509,14 @@ bool make_mla_tensor_map(void *out_map, const void *arena, uint64_t total_rows)
 cudaError_t launch_decode_mla(const DecodeParams &p, const void *tmap, int rows_per_page, int n_ctas,
                               cudaStream_t stream)
 {
-    static bool configured = false;
-    if (!configured) {
+    static bool configured[64] = {};              // per device: the attribute belongs to the device's copy of the function
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
         cudaError_t e = cudaFuncSetAttribute(cp_decode_mla_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              MLA_SMEM_BYTES);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (dev >= 0 && dev < 64) configured[dev] = true;
     }
     int grid = 2 * p.n_tiles;
     if (grid < (p.n_combine_units + 3) / 4) grid = (p.n_combine_units + 3) / 4;

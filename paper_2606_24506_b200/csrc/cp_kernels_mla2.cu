@@ -537,12 +537,14 @@ bool make_mla2_tensor_maps(void *out_map9, void *out_map2, const void *arena, ui
 cudaError_t launch_decode_mla2(const DecodeParams &p, const void *tmap9, const void *tmap2, int rows_per_page,
                                int n_ctas, cudaStream_t stream)
 {
-    static bool configured = false;
-    if (!configured) {
+    static bool configured[64] = {};              // per device: the attribute belongs to the device's copy of the function
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
         cudaError_t e = cudaFuncSetAttribute(cp_decode_mla2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              M2_SMEM_BYTES);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (dev >= 0 && dev < 64) configured[dev] = true;
     }
     int pairs = p.n_tiles;
     if (pairs < (p.n_combine_units + 7) / 8) pairs = (p.n_combine_units + 7) / 8;

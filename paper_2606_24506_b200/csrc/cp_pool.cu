@@ -143,6 +143,15 @@ struct cp_pool {
         int64_t q_elems = 0, out_floats = 0, lse_floats = 0;
     } splan;
 
+    // stream the last compute call ran on: the scheduler state of a plan (work list, counter sets, page table, context
+    // table) is reused from call to call, so a call on ANOTHER stream first waits for everything the previous stream
+    // was given (adopt_stream); side stream + events for the second attention kind of a mixed batch
+    cudaStream_t last_stream = nullptr;
+    bool last_stream_valid = false;
+    cudaEvent_t ev_switch = nullptr, ev_fork = nullptr, ev_join = nullptr;
+    cudaStream_t side_stream = nullptr;
+    int kind_ctas[2] = {0, 0};           // CTAs each attention kind of the cached plan was planned for
+
     // counters
     uint64_t n_launches = 0, n_plan_builds = 0, n_h2d_bytes = 0;
 };
@@ -186,7 +195,7 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
 {
     const int P = (int)pool->P;
     const int pps = 128 / P;                                   // pages per slice
-    const int n_ctas = std::max(1, std::min(pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm, pool->n_sm));
+    const int n_ctas = std::max(1, std::min(pool->kind_ctas[CP_KIND_KV], pool->n_sm));
     struct GInfo { int b, c, n_lp, n_sl, s_static; };
     std::vector<GInfo> gi;
     for (int b = 0; b < n; ++b) {
@@ -402,7 +411,12 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
     }
     pool->q_elems = qo; pool->out_floats = oo; pool->lse_floats = lo;
 
-    const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
+    // (A batch with models of both attention kinds runs two persistent kernels, each planned for ALL CTAs: either
+    // needs every SM to reach its own rate -- measured: splitting the SMs between them in proportion to their bytes
+    // makes the step longer than running them one after the other -- but launched on two streams the second
+    // kernel's CTAs move in as the first one's leave, which hides the first's tail and the second's start-up.)
+    const int n_all = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
+    pool->kind_ctas[0] = pool->kind_ctas[1] = n_all;
     uint64_t ws = 0;
     for (int k = 0; k < 2; ++k) {
         KindPlan &kp = pool->plan[k];
@@ -418,6 +432,7 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
                 if (m.kind == CP_KIND_MLA && !(m.head_dim_qk == 576 && m.head_dim_v == 512 && m.n_q_heads <= 128))
                     mla_fast = false;
             }
+        const int n_ctas = pool->kind_ctas[k];
         const int64_t target_tiles =
             std::max<int64_t>(1, (int64_t)n_ctas * pool->opt_waves_x16 / 16 / (mla_fast ? 2 : 1));
         // which K/V kernel will run this plan: it fixes how many arrivals a finished tile makes on its
@@ -647,6 +662,27 @@ cp_status ensure_device(cp_pool *pool)
     return CP_OK;
 }
 
+// Calls of one pool are stream-ordered by the caller in the common case (one stream).  A call on another stream than
+// the previous one is made to wait for all work the previous stream holds -- the earlier launch may still be reading
+// the work list, counters and tables this call is about to rewrite.  Costs nothing while the stream stays the same.
+cp_status adopt_stream(cp_pool *pool, cudaStream_t s)
+{
+    if (pool->last_stream_valid && pool->last_stream != s) {
+        if (!pool->ev_switch && cudaEventCreateWithFlags(&pool->ev_switch, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            return CP_ERR_CUDA;
+        }
+        if (cudaEventRecord(pool->ev_switch, pool->last_stream) != cudaSuccess ||
+            cudaStreamWaitEvent(s, pool->ev_switch, 0) != cudaSuccess) {
+            cudaGetLastError();
+            return CP_ERR_CUDA;
+        }
+    }
+    pool->last_stream = s;
+    pool->last_stream_valid = true;
+    return CP_OK;
+}
+
 // Upload page-table rows and context lengths that changed since the last device call.
 cp_status flush_tables(cp_pool *pool, cudaStream_t stream)
 {
@@ -811,6 +847,10 @@ cp_status cp_pool_free(cp_pool *pool)
     if (!pool) return CP_OK;
     if (pool->dev_ready || pool->vmm) cudaDeviceSynchronize();
     if (pool->vmm) { vmm_destroy(pool->vmm); pool->vmm = nullptr; }
+    if (pool->ev_switch) cudaEventDestroy(pool->ev_switch);
+    if (pool->ev_fork) cudaEventDestroy(pool->ev_fork);
+    if (pool->ev_join) cudaEventDestroy(pool->ev_join);
+    if (pool->side_stream) cudaStreamDestroy(pool->side_stream);
     pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release(); pool->d_append.release(); pool->d_timeline.release();
     for (int k = 0; k < 2; ++k) {
         pool->plan[k].d_groups.release(); pool->plan[k].d_tiles.release();
@@ -1050,6 +1090,8 @@ cp_status cp_pool_gather_kv(cp_pool *pool, int32_t request_id, void *k_out_dev, 
     cp_status st = ensure_device(pool);
     if (st != CP_OK) return st;
     cudaStream_t s = (cudaStream_t)stream;
+    st = adopt_stream(pool, s);
+    if (st != CP_OK) return st;
     st = flush_tables(pool, s);
     if (st != CP_OK) return st;
     const cp_model_cfg &m = pool->models[r.model];
@@ -1182,6 +1224,8 @@ cp_status cp_pool_append_kv(cp_pool *pool, const int32_t *request_ids_host, int3
     st = append_host(pool, request_ids_host, n_requests, true, v_new_dev, recs, grew);
     if (st != CP_OK) return st;
     cudaStream_t s = (cudaStream_t)stream;
+    st = adopt_stream(pool, s);
+    if (st != CP_OK) return st;
     st = flush_tables(pool, s);                            // new page ids (and context lengths) to the device
     if (st != CP_OK) return st;
     return launch_append_recs(pool, recs, k_new_dev, v_new_dev, s);
@@ -1202,14 +1246,41 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
     if (pool->plan_ws_floats * 4 > workspace_bytes) return CP_ERR_WORKSPACE;
     if (pool->plan_ws_floats && (!workspace_dev || ((uintptr_t)workspace_dev & 15u))) return CP_ERR_WORKSPACE;
     cudaStream_t s = (cudaStream_t)stream;
+    st = adopt_stream(pool, s);
+    if (st != CP_OK) return st;
     st = flush_tables(pool, s);
     if (st != CP_OK) return st;
 
+    // A batch with both attention kinds: everything either launch reads is uploaded on the caller's stream first;
+    // then the second kind's kernel runs beside the first on a stream of the pool's own (fork here, join below).
+    const bool both_kinds = !pool->plan[0].tiles.empty() && !pool->plan[1].tiles.empty();
+    cudaStream_t s_main = s;
+    for (int k = 0; k < 2; ++k) {
+        if (pool->plan[k].tiles.empty()) continue;
+        st = upload_plan(pool, pool->plan[k], s_main);
+        if (st != CP_OK) return st;
+    }
+    if (pool->opt_timeline) {
+        const size_t tb = (size_t)pool->n_sm * kTimelineSlots * sizeof(unsigned long long);
+        if (pool->d_timeline.ensure(tb) != cudaSuccess || cudaMemsetAsync(pool->d_timeline.ptr, 0, tb, s_main) != cudaSuccess) {
+            cudaGetLastError();
+            return CP_ERR_CUDA;
+        }
+    }
+    if (both_kinds) {
+        if ((!pool->side_stream && cudaStreamCreateWithFlags(&pool->side_stream, cudaStreamNonBlocking) != cudaSuccess) ||
+            (!pool->ev_fork && cudaEventCreateWithFlags(&pool->ev_fork, cudaEventDisableTiming) != cudaSuccess) ||
+            (!pool->ev_join && cudaEventCreateWithFlags(&pool->ev_join, cudaEventDisableTiming) != cudaSuccess) ||
+            cudaEventRecord(pool->ev_fork, s_main) != cudaSuccess ||
+            cudaStreamWaitEvent(pool->side_stream, pool->ev_fork, 0) != cudaSuccess) {
+            cudaGetLastError();
+            return CP_ERR_CUDA;
+        }
+    }
     for (int k = 0; k < 2; ++k) {
         KindPlan &kp = pool->plan[k];
         if (kp.tiles.empty()) continue;
-        st = upload_plan(pool, kp, s);
-        if (st != CP_OK) return st;
+        s = (both_kinds && k == 1) ? pool->side_stream : s_main;
         DecodeParams prm;
         std::memset(&prm, 0, sizeof(prm));            // every field a launch does not use is null / 0
         prm.arena = pool->arena; prm.page_tokens = pool->P; prm.page_bytes = pool->page_bytes;
@@ -1236,16 +1307,9 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.published = nullptr; prm.gate_flag = nullptr; prm.gate_timeout_us = 0;
         prm.timeline = nullptr;
         prm.app_k = pool->step_k; prm.app_v = pool->step_v;
-        if (pool->opt_timeline) {
-            const size_t tb = (size_t)pool->n_sm * kTimelineSlots * sizeof(unsigned long long);
-            if (pool->d_timeline.ensure(tb) != cudaSuccess || cudaMemsetAsync(pool->d_timeline.ptr, 0, tb, s) != cudaSuccess) {
-                cudaGetLastError();
-                return CP_ERR_CUDA;
-            }
-            prm.timeline = (unsigned long long *)pool->d_timeline.ptr;
-        }
+        if (pool->opt_timeline && !(both_kinds && k == 1)) prm.timeline = (unsigned long long *)pool->d_timeline.ptr;
         kp.counter_set ^= 1;
-        const int n_ctas = pool->opt_num_ctas > 0 ? pool->opt_num_ctas : pool->n_sm;
+        const int n_ctas = pool->kind_ctas[k];
         cudaError_t e;
         if (k == CP_KIND_KV && kp.use_kvt && pool->kv_tmap_ok) {
             prm.n_combine_units = (int)kp.cunits.size();
@@ -1272,6 +1336,11 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
                                       std::min(n_ctas, pool->n_sm), s);
         pool->n_launches++;
         if (e != cudaSuccess) return CP_ERR_CUDA;
+    }
+    if (both_kinds &&
+        (cudaEventRecord(pool->ev_join, pool->side_stream) != cudaSuccess || cudaStreamWaitEvent(s_main, pool->ev_join, 0) != cudaSuccess)) {
+        cudaGetLastError();
+        return CP_ERR_CUDA;
     }
     return CP_OK;
 }
@@ -1305,6 +1374,8 @@ cp_status cp_decode_step(cp_pool *pool, const int32_t *request_ids_host, int32_t
     std::vector<AppendRec> sep;
     for (int b = 0; b < n_requests; ++b)
         if (!(fused_kv && pool->models[recs[b].model].kind == CP_KIND_KV)) sep.push_back(recs[b]);
+    st = adopt_stream(pool, s);
+    if (st != CP_OK) return st;
     st = flush_tables(pool, s);
     if (st != CP_OK) return st;
     st = launch_append_recs(pool, sep, k_new_dev, v_new_dev, s);
@@ -1531,6 +1602,8 @@ static cp_status decode_stages_core(cp_pool *pool, int32_t n_stages, const int32
     if (st != CP_OK) return st;
     if (!pool->kv_tmap_ok) return CP_ERR_UNSUPPORTED;
     cudaStream_t s = (cudaStream_t)stream;
+    st = adopt_stream(pool, s);
+    if (st != CP_OK) return st;
     st = flush_tables(pool, s);
     if (st != CP_OK) return st;
     KindPlan &kp = sp.kp;
@@ -1826,6 +1899,8 @@ cp_status cp_queue_launch(cp_queue *q, const void *q_dev, float *out_dev, float 
     if (st != CP_OK) return st;
     if (!pool->kv_tmap_ok) return CP_ERR_UNSUPPORTED;
     cudaStream_t s = (cudaStream_t)stream;
+    st = adopt_stream(pool, s);
+    if (st != CP_OK) return st;
     st = flush_tables(pool, s);
     if (st != CP_OK) return st;
     std::vector<int32_t> rm(pool->max_requests, -1);

@@ -169,6 +169,42 @@ def test_stages_alpha_zero_equal_single_steps_bit_for_bit(torch_cuda):
         dw.close()
 
 
+def teacher_forced_reference(w, stages, deps, q_in, alpha, got):
+    """Oracle stage s fed the GPU's OWN output of stage deps[s]: both sides then quantise the same previous
+    output, the bf16 rounding of the query cannot differ, and the dependent stage is held to the plain bars
+    (LSE 1e-3) -- a real 5e-3 LSE error in a dependent stage cannot hide behind the free-running 1e-2."""
+    ref = []
+    for s, reqs in enumerate(stages):
+        res = []
+        for j, ri in enumerate(reqs):
+            r = w.requests[ri]
+            m = w.models[r.model_id]
+            q = np.ascontiguousarray(q_in[s][j], dtype=np.uint16)
+            if deps[s] >= 0:
+                q = oracle.stage_query(q, got[deps[s]][j][0], alpha)
+            res.append(oracle.attention(w.arena, w.page_tokens, w.page_bytes, w.num_pages, m.kind, m.n_q_heads,
+                                        m.n_kv_heads, m.head_dim_qk, m.head_dim_v, m.softmax_scale, r.page_ids,
+                                        r.context_len, q))
+        ref.append(res)
+    return ref
+
+
+@pytest.mark.parametrize("P", [16, 64])
+def test_dependent_stages_teacher_forced_at_the_plain_lse_bar(torch_cuda, P):
+    import paper_2606_24506_b200 as cp
+    w, order, stages, deps, q_in = build_case(BATCHES, P, seed=410 + P)
+    dw = device_workload(w)
+    try:
+        dw.pool.set_option(cp.CP_OPT_MIN_TILE_PAGES, 1)
+        got = run_stages(torch_cuda, dw, w, stages, deps, q_in, 1.0)
+    finally:
+        dw.close()
+    ref = teacher_forced_reference(w, stages, deps, q_in, 1.0, got)
+    for s, (b, layer) in enumerate(order):
+        worst = compare_stage(got[s], ref[s], False, "teacher-forced stage %d (batch %d layer %d)" % (s, b, layer))
+    print("P=%d teacher-forced, last stage: %s" % (P, worst))
+
+
 def test_stages_argument_errors(torch_cuda):
     import paper_2606_24506_b200 as cp
     torch = torch_cuda

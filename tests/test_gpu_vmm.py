@@ -72,6 +72,42 @@ def test_vmm_gather_bit_exact(torch_cuda):
         dw.close()
 
 
+def test_vmm_first_compute_call_with_slot_zero_unmapped(torch_cuda):
+    """The base of the reserved range has no backing until request slot 0 is mapped: the first compute call of a
+    pool whose only request sits in the LAST slot must still find the arena's device (taken from the arena
+    object, not from the pointer) and give the right attention."""
+    import torch
+    import paper_2606_24506_b200 as cp
+    from paper_2606_24506_b200.harness import raw_device_tensor
+    m = ModelCfg(KIND_KV, 32, 4, 128, 128, 128 ** -0.5)
+    w = W.small_workload([m], [0], [3000], page_tokens=64, seed=9, keep_contiguous=False)
+    r = w.requests[0]
+    n_req = 5
+    torch.zeros(1, device="cuda:0")
+    pool = cp.Pool.create_vmm(w.num_pages * w.page_bytes + (8 << 20), 64, w.page_bytes, w.models, n_req, r.page_ids.size)
+    try:
+        rid = n_req - 1
+        pool.map_pages(rid, 0, None, r.context_len, n_allocate=r.page_ids.size)
+        info = pool.vmm_info()
+        pages = w.arena.reshape(w.num_pages, w.page_bytes // 2)
+        src = torch.from_numpy(np.ascontiguousarray(pages[r.page_ids]).view(np.int16)).to("cuda:0")
+        dst = raw_device_tensor(info["arena_dev"] + rid * info["slot_pages"] * w.page_bytes, src.numel() * 2, torch.device("cuda:0")).view(torch.int16)
+        dst.copy_(src.reshape(-1))
+        q = torch.from_numpy(w.q_packed().view(np.int16)).to("cuda:0")
+        out = torch.full((32 * 128,), float("nan"), dtype=torch.float32, device="cuda:0")
+        lse = torch.full((32,), float("nan"), dtype=torch.float32, device="cuda:0")
+        need = max(pool.decode_workspace_bytes([rid]), 256)
+        ws = torch.full((need,), 0xFF, dtype=torch.uint8, device="cuda:0")
+        pool.decode_attention([rid], q, out, lse, ws, need, int(torch.cuda.current_stream().cuda_stream))
+        torch.cuda.synchronize()
+        (ro, rl), = oracle.decode_workload(w)
+        o = out.cpu().numpy().reshape(32, 128)
+        assert np.abs(o - ro).max() <= 1e-2 and np.linalg.norm(o - ro) / np.linalg.norm(ro) <= 1e-2
+        assert np.abs(lse.cpu().numpy() - rl).max() <= 1e-3
+    finally:
+        pool.close()
+
+
 def test_vmm_append_crosses_a_chunk_boundary(torch_cuda):
     """A request that grows token by token maps its next physical chunk when a new page falls past
     the backed prefix of its slot; K/V written on both sides of the boundary read back bit-exact and
