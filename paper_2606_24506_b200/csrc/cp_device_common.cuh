@@ -6,10 +6,6 @@
 #include <cstdint>
 #include "cp_internal.h"
 
-#ifndef KV_STAMP
-#define KV_STAMP(k, cond) do { } while (0)
-#endif
-
 namespace cp {
 
 __device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
@@ -241,7 +237,6 @@ static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, 
         const bool has_next = un < n_end;
         CombineUnit nx;
         if (has_next) nx = load_combine_unit<CG>(p.cunits, un);
-        KV_STAMP(8, threadIdx.x == 0);
         const int ns = cu.n_splits;
         const int zl = cu.zl_log2;
         const int ZL = 1 << zl, CQ = 32 >> zl;
@@ -251,7 +246,6 @@ static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, 
             __syncwarp();
             done_group = cu.group;
         }
-        KV_STAMP(9, threadIdx.x == 0);
         const float2 *mlp = reinterpret_cast<const float2 *>(p.workspace + cu.ml_off);
         const float *src = p.workspace + cu.part_off + cq * 4;
         const int ss = cu.split_stride;
@@ -290,7 +284,6 @@ static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, 
         }
         for (int o = 16; o > 0; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
         __syncwarp();
-        KV_STAMP(10, threadIdx.x == 0);
         // pass 3: O = sum_s w_s O_s over this lane's splits z, z + ZL, ... (in order), then the tree
         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll U3
@@ -316,7 +309,6 @@ static __device__ __noinline__ void combine_units(const DecodeParams &p, int u, 
             // the unit's O / LSE stores happen-before this release (cumulative over the __syncwarp)
             if (lane == 0) red_release_add(p.stage_done + (size_t)cu.pad[0] * kCounterStride, 1);
         }
-        KV_STAMP(11, threadIdx.x == 0);
         if (!has_next) break;
         cu = nx;
         u = un;

@@ -23,21 +23,6 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstdint>
-namespace cp {
-#ifdef CP_KV_PROBE_TIMING        /* probe builds only: per-CTA globaltimer stamps */
-__device__ unsigned long long cp_kv_probe_ts[160 * 16];
-__device__ __forceinline__ void probe_stamp(int k)
-{
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    cp_kv_probe_ts[blockIdx.x * 16 + k] = t;
-}
-#define KV_STAMP(k, cond) do { if (cond) probe_stamp(k); } while (0)
-#else
-#define KV_STAMP(k, cond) do { } while (0)
-#endif
-
-}  // namespace cp
 #include "cp_device_common.cuh"
 #include "cp_ptx.cuh"
 #include "cp_launch.h"
@@ -475,7 +460,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
     const int tid = threadIdx.x;
     const int warp = tid >> 5;
     const int lane = tid & 31;
-    KV_STAMP(0, tid == 0);
     scheduler_reset_other_set(p);
 
     if (tid == 0) {
@@ -594,9 +578,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                     mbar_wait(smem_u32(empty_b + slot), par);
                     if (elect_one()) {
                         const uint32_t fb = smem_u32(full_b + slot);
-#ifdef CP_KV_PROBE_NO_LOAD      /* probe builds only: consumer capacity without memory traffic */
-                        mbar_arrive(fb);
-#else
                         mbar_arrive_expect_tx(fb, STAGE_BYTES);
                         const uint32_t dst = smem_u32(stage_base + (size_t)slot * STAGE_BYTES);
                         const int row = my * rows_per_page;
@@ -604,7 +585,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                         tma_load_2d(dst + SUB, &tmap, 64, row, fb, policy);        // K, d 64..127
                         tma_load_2d(dst + 2 * SUB, &tmap, 0, row + P, fb, policy); // V, d 0..63
                         tma_load_2d(dst + 3 * SUB, &tmap, 64, row + P, fb, policy);// V, d 64..127
-#endif
                     }
                     ++pc;
                 }
@@ -650,7 +630,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 }
             }
             if (d.item < 0) break;
-            KV_STAMP(1, tid == 0 && qi == 1);
             const int mt = d.mt;
             const int NL = KV_CWARPS / mt;            // slice lanes per M tile
             const int mtile = warp % mt;
@@ -726,10 +705,8 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 const uint32_t pidx = pc + (uint32_t)j;
                 const uint32_t slot = pidx % NS;
                 mbar_wait(smem_u32(full_b + slot), (pidx / NS) & 1);
-                KV_STAMP(2, tid == 0 && qi == 1 && j == 0);
                 const uint32_t sb = smem_u32(stage_base + (size_t)slot * STAGE_BYTES);
                 const int valid = ctx - (d.page_begin + j) * P;     // >= 1; < P only on the request's last page
-#ifndef CP_KV_PROBE_NO_COMPUTE
 #pragma unroll
                 for (int s = 0; s < SPP; ++s) {
                     if (((j * SPP + s) & (NL - 1)) != plane) continue;
@@ -748,12 +725,10 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                     }
                     kv_slice_unit<P, NT, QLEN>(sb, tok0, valid, qf, scale_log2, o, m_run, l_run, lane, koff, vrow, vbase, back0, back1);
                 }
-#endif
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(empty_b + slot));
             }
             pc += (uint32_t)npg;
-            KV_STAMP(3, tid == 0);
 
             // ---- quad-reduce the row sums, then merge the slice lanes (fixed tree)
             l_run[0] += __shfl_xor_sync(0xffffffffu, l_run[0], 1);
@@ -803,7 +778,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 consumer_bar();
             }
 
-            KV_STAMP(4, tid == 0);
             // ---- publish (slice lane 0 of every M tile)
             if (plane == 0) {
                 if (d.n_splits == 1) {
@@ -843,8 +817,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 }
             }
         }
-        KV_STAMP(5, tid == 0);
-#ifndef CP_KV_PROBE_NO_COMBINE
         // ---- LSE combine (step a4): no tile is left to pop; every consumer warp runs its
         // warp-sized units.  A unit only waits for tiles that are already running on some SM, so
         // the spin inside terminates.
@@ -852,10 +824,7 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
         // them from one counter would serialise thousands of same-address atomics at the L2.
         if constexpr (!MULTI)
             combine_units<8>(p, blockIdx.x * KV_CWARPS + warp, gridDim.x * KV_CWARPS, merge + warp * KV_COMBINE_WARP_FLOATS, lane);
-#endif
-        KV_STAMP(6, tid == 0);
     }
-    KV_STAMP(7, tid == 0);
 }
 
 // ----------------------------------------------------------------------------- host side
@@ -894,12 +863,6 @@ bool make_arena_tensor_map(void *out_map, const void *arena, uint64_t total_rows
     return r == CUDA_SUCCESS;
 }
 
-#ifdef CP_KV_PROBE_TIMING
-extern "C" int cp_kv_probe_read(unsigned long long *out_host)
-{
-    return (int)cudaMemcpyFromSymbol(out_host, cp_kv_probe_ts, sizeof(cp_kv_probe_ts));
-}
-#endif
 
 bool kv_fast_supported(int P) { return P == 16 || P == 32 || P == 64 || P == 128; }
 

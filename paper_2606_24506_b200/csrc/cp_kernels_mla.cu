@@ -37,23 +37,6 @@
 
 namespace cp {
 
-#ifdef CP_KV_PROBE_TIMING        /* probe builds only */
-__device__ unsigned long long cp_mla_probe_ts[160 * 32];
-__device__ __forceinline__ void mla_stamp(int k)
-{
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    cp_mla_probe_ts[blockIdx.x * 32 + k] = t;
-}
-#define MLA_STAMP(k, cond) do { if (cond) mla_stamp(k); } while (0)
-extern "C" int cp_mla_probe_read(unsigned long long *out_host)
-{
-    return (int)cudaMemcpyFromSymbol(out_host, cp_mla_probe_ts, sizeof(cp_mla_probe_ts));
-}
-#else
-#define MLA_STAMP(k, cond) do { } while (0)
-#endif
-
 constexpr int MLA_DK = 576;                         // latent row width (512 latent + 64 rope)
 constexpr int MLA_DV = 512;                         // value = first 512 entries of the row
 constexpr int MLA_HALF = 256;                       // value columns per work item
@@ -118,7 +101,6 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     const uint32_t q_base = smem_u32(smem + MLA_SMEM_Q);
     const uint32_t st_base = smem_u32(smem + MLA_SMEM_STAGE);
     const uint32_t p_base = smem_u32(smem + MLA_SMEM_P);
-    MLA_STAMP(16, tid == 64);
     scheduler_reset_other_set(p);
 
     if (tid == 0) {
@@ -227,11 +209,8 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 if (i < n) {
                     // ---- S_i = Q C_i^T into score buffer (g & 1)
                     const uint32_t g = gs + (uint32_t)i, slot = g % MLA_STAGES, b = g & 1;
-                    MLA_STAMP(0, lane == 0 && i == 50);
                     mbar_wait(smem_u32(&mi->full[slot]), (g / MLA_STAGES) & 1);
-                    MLA_STAMP(1, lane == 0 && i == 50);
                     mbar_wait(smem_u32(&mi->s_empty[b]), ((g >> 1) & 1) ^ 1);
-                    MLA_STAMP(2, lane == 0 && i == 50);
                     tc_fence_after();
                     if (elect_one()) {
                         const uint32_t c0 = st_base + slot * MLA_STAGE_BYTES;
@@ -252,13 +231,11 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                         umma_commit(smem_u32(&mi->s_full[b]));
                     }
                     __syncwarp();
-                    MLA_STAMP(3, lane == 0 && i == 50);
                 }
                 if (i >= 1) {
                     // ---- O += P_{i-1} V_{i-1} (value half of the work item)
                     const uint32_t g = gs + (uint32_t)i - 1, slot = g % MLA_STAGES;
                     mbar_wait(smem_u32(&mi->p_full), g & 1);
-                    MLA_STAMP(4, lane == 0 && i == 50);
                     tc_fence_after();
                     if (elect_one()) {
 #pragma unroll
@@ -274,8 +251,6 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                         umma_commit(smem_u32(&mi->p_done));           // P buffer free, O updated
                     }
                     __syncwarp();
-                    MLA_STAMP(5, lane == 0 && i == 50);
-                    MLA_STAMP(6, lane == 0 && i == 51);
                 }
             }
             gs += (uint32_t)n;
@@ -295,7 +270,6 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             if (lane == 0) mbar_arrive(smem_u32(&mi->tq_empty[qs]));
             ++qi;
             if (d.item < 0) break;
-            MLA_STAMP(17, tid == 64 && qi == 1);
 
             if (d.load_q) {
                 // stage the query block [128 x 576] bf16.  Column blocks 0..5 go to tensor memory (this
@@ -344,14 +318,11 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 if (lane == 0) mbar_arrive(smem_u32(&mi->q_full));
             }
 
-            MLA_STAMP(18, tid == 64 && qi == 1);
             float m_run = -INFINITY, l_run = 0.f;
             const int n = d.n_slices;
             for (int i = 0; i < n; ++i) {
                 const uint32_t g = gs + (uint32_t)i, b = g & 1, k = g >> 1;
-                MLA_STAMP(8, tid == 64 && i == 50);
                 mbar_wait(smem_u32(&mi->s_full[b]), k & 1);
-                MLA_STAMP(9, tid == 64 && i == 50);
                 tc_fence_after();
                 uint32_t sr[MLA_TS];
 #pragma unroll
@@ -361,7 +332,6 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&mi->s_empty[b]));       // score buffer free
-                MLA_STAMP(10, tid == 64 && i == 50);
                 const int valid = (i == n - 1) ? d.valid_last : MLA_TS;
                 float mx = -INFINITY;
 #pragma unroll
@@ -385,9 +355,7 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 }
                 l_run += sum;
                 // the P buffer (and O, if it must be rescaled) is free once P_{i-1} V_{i-1} has completed
-                MLA_STAMP(11, tid == 64 && i == 50);
                 mbar_wait(smem_u32(&mi->p_done), (g & 1) ^ 1);
-                MLA_STAMP(12, tid == 64 && i == 50);
                 if (__any_sync(0xffffffffu, need)) {
                     // rescale this warp's O rows in TMEM
                     tc_fence_after();
@@ -420,10 +388,6 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&mi->p_full));
-                MLA_STAMP(13, tid == 64 && i == 50);
-                MLA_STAMP(14, tid == 64 && i == 51);
-                MLA_STAMP(19, tid == 64 && i == 0);
-                MLA_STAMP(20, tid == 64 && i == n - 1);
             }
             gs += (uint32_t)n;
 
@@ -462,18 +426,15 @@ cp_decode_mla_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                     __syncwarp();
                     if (lane == 0) red_release_add(p.group_counters + (size_t)d.group_idx * kCounterStride, 1);
                 }
-                MLA_STAMP(21, tid == 64);
             }
         }
         // ---- LSE combine (step a4): warp-sized units, statically assigned (see the MQA/GQA kernel)
         float *wsm = reinterpret_cast<float *>(smem + MLA_SMEM_P) + (warp - 2) * kMaxSplits;
         combine_units<16>(p, blockIdx.x * 4 + (warp - 2), gridDim.x * 4, wsm, lane);
-        MLA_STAMP(22, tid == 64);
     }
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc(tmem, MLA_TMEM_COLS);
-    MLA_STAMP(23, tid == 64);
 }
 
 // ----------------------------------------------------------------------------- host side

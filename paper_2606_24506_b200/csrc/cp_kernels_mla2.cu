@@ -26,28 +26,6 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstdint>
-namespace cp {
-#ifdef CP_KV_PROBE_TIMING        /* probe builds only */
-__device__ unsigned long long cp_mla2_probe_ts[160 * 32];
-__device__ __forceinline__ void m2_stamp(int k)
-{
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    cp_mla2_probe_ts[blockIdx.x * 32 + k] = t;
-}
-#define M2_STAMP(k, cond) do { if (cond) m2_stamp(k); } while (0)
-extern "C" int cp_mla2_probe_read(unsigned long long *out_host)
-{
-    return (int)cudaMemcpyFromSymbol(out_host, cp_mla2_probe_ts, sizeof(cp_mla2_probe_ts));
-}
-#else
-#define M2_STAMP(k, cond) do { } while (0)
-#endif
-
-}  // namespace cp
-#ifdef CP_KV_PROBE_TIMING
-#define KV_STAMP(k, cond) M2_STAMP(16 + (k), cond)
-#endif
 #include "cp_device_common.cuh"
 #include "cp_launch.h"
 #include "cp_ptx.cuh"
@@ -141,7 +119,6 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     const uint32_t q_base = smem_u32(smem + M2_SMEM_Q);
     const uint32_t st_base = smem_u32(smem + M2_SMEM_STAGE);
     const uint32_t p_base = smem_u32(smem + M2_SMEM_P);
-    M2_STAMP(16, tid == 64);
     scheduler_reset_other_set(p);
 
     if (tid == 0) {
@@ -230,13 +207,9 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             for (int i = 0; i <= n + 1; ++i) {
                 if (i < n) {
                     const uint32_t g = gs + (uint32_t)i, slot = g % M2_STAGES, b = g % M2_SB;
-                    M2_STAMP(0, lane == 0 && i == 50);
                     mbar_wait(smem_u32(&mi->full[slot]), (g / M2_STAGES) & 1);
-                    M2_STAMP(1, lane == 0 && i == 50);
                     mbar_wait_cluster(smem_u32(&mi->full_peer[slot]), (g / M2_STAGES) & 1);
-                    M2_STAMP(2, lane == 0 && i == 50);
                     mbar_wait_cluster(smem_u32(&mi->s_empty[b]), ((g / M2_SB) & 1) ^ 1);
-                    M2_STAMP(3, lane == 0 && i == 50);
                     tc_fence_after();
                     if (elect_one()) {
                         const uint32_t c0 = st_base + slot * M2_STAGE_BYTES;
@@ -258,12 +231,10 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                         umma2_commit(smem_u32(&mi->s_full[b]));
                     }
                     __syncwarp();
-                    M2_STAMP(4, lane == 0 && i == 50);
                 }
                 if (i >= 2) {
                     const uint32_t g = gs + (uint32_t)i - 2, slot = g % M2_STAGES;
                     mbar_wait_cluster(smem_u32(&mi->p_full[g & 1]), (g >> 1) & 1);
-                    M2_STAMP(5, lane == 0 && i == 50);
                     tc_fence_after();
                     if (elect_one()) {
                         const uint32_t pv = st_base + slot * M2_STAGE_BYTES + M2_SAREA;
@@ -283,8 +254,6 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                         umma2_commit(smem_u32(&mi->p_done[g & 1]));
                     }
                     __syncwarp();
-                    M2_STAMP(6, lane == 0 && i == 50);
-                    M2_STAMP(7, lane == 0 && i == 51);
                 }
             }
             gs += (uint32_t)n;
@@ -352,14 +321,11 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(L_q_full);
             }
-            M2_STAMP(18, tid == 64 && k == 0);
             float m_run = -INFINITY, l_run = 0.f;
             const int n = it.n_slices;
             for (int i = 0; i < n; ++i) {
                 const uint32_t g = gs + (uint32_t)i, b = g % M2_SB, kq = g / M2_SB, xb = g & 1;
-                M2_STAMP(8, tid == 64 && i == 50);
                 mbar_wait(smem_u32(&mi->s_full[b]), kq & 1);
-                M2_STAMP(9, tid == 64 && i == 50);
                 tc_fence_after();
                 uint32_t sr[16];
                 tmem_ld16(tl + M2_TMEM_S + 16 * b, sr);
@@ -379,7 +345,6 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 mi->xmax[xb][L] = mx;
                 asm volatile("bar.sync 2, 128;" ::: "memory");
                 mx = fmaxf(mx, mi->xmax[xb][L ^ 64]);
-                M2_STAMP(10, tid == 64 && i == 50);
                 const float m_new = (mx > m_run + M2_LAZY_LOG2) ? mx : m_run;
                 const bool need = (m_new != m_run) && i > 0;
                 const float a_resc = ex2_ftz(m_run - m_new);
@@ -393,9 +358,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pw[j]) : "f"(p1), "f"(p0));
                 }
                 l_run += sum;
-                M2_STAMP(11, tid == 64 && i == 50);
                 mbar_wait(smem_u32(&mi->p_done[xb]), ((g >> 1) & 1) ^ 1);       // P buffer (slice & 1) free
-                M2_STAMP(12, tid == 64 && i == 50);
                 if (__any_sync(0xffffffffu, need)) {
                     // O is rescaled in place: the value MMAs of the previous slice must be complete
                     mbar_wait(smem_u32(&mi->p_done[(g - 1) & 1]), ((g - 1) >> 1) & 1);
@@ -429,10 +392,6 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(L_p_full + 8 * xb);
-                M2_STAMP(13, tid == 64 && i == 50);
-                M2_STAMP(14, tid == 64 && i == 51);
-                M2_STAMP(19, tid == 64 && i == 0);
-                M2_STAMP(20, tid == 64 && i == n - 1);
             }
             gs += (uint32_t)n;
 
@@ -489,7 +448,6 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                     __syncwarp();
                     if (lane == 0) red_release_add(p.group_counters + (size_t)it.group_idx * kCounterStride, 1);
                 }
-                M2_STAMP(21, tid == 64);
             }
         }
     }
@@ -500,7 +458,6 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     {
         float *wsm = reinterpret_cast<float *>(smem + M2_SMEM_STAGE) + warp * kMaxSplits;
         combine_units<16>(p, blockIdx.x * M2_WARPS + warp, gridDim.x * M2_WARPS, wsm, lane);
-        M2_STAMP(22, tid == 64);
     }
     tc_fence_before();
     cluster_sync_all();
