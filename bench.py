@@ -30,10 +30,10 @@ if ROOT not in sys.path:
 
 import numpy as np
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the decode kernel, from the committed
-# `ncu --set full` captures (profiles/r1_ncu_full_cfg2_kv_v6.txt, r1_ncu_full_cfg4_kv_v3.txt, r1_ncu_full_cfg3_mla_pair.txt)
-NCU_TRAFFIC_BYTES = {2: 344.66e6 + 6.97e6, 3: 285.04e6 + 9.61e6, 4: 134.33e6 + 6.31e6}
-NCU_TENSOR_PIPE_PCT = {3: 34.0}       # sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the decode kernel, from the committed `ncu --set full`
+# captures profiles/r2_ncu_full_cfg{2,3,4,5}.txt (cfg1, 0.66 MB, has no capture: its launch is latency, not traffic)
+NCU_TRAFFIC_BYTES = {2: 344.68e6 + 11.19e6, 3: 285.38e6 + 15.34e6, 4: 134.41e6 + 7.81e6, 5: 806.38e6 + 7.25e6}
+NCU_TENSOR_PIPE_PCT = {3: 36.8}       # sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active
 
 METRIC = "paged decode-attention KV GB/s"
 UNIT = "GB/s"
@@ -383,7 +383,9 @@ def main():
 
     k = args.config
     w = W.config(k)
-    dw = DeviceWorkload(w, dev, page_list_slack=6 * max(m.n_kv_heads for m in w.models))
+    # room in the page lists for the tokens the append / decode-loop legs add (16 + 2 loops of max(2 P, 64) tokens)
+    loop_tokens = 16 + 2 * max(2 * w.page_tokens, 64) + 8
+    dw = DeviceWorkload(w, dev, page_list_slack=(-(-loop_tokens // w.page_tokens) + 2) * max(m.n_kv_heads for m in w.models))
     dw.pool.set_option(cp.CP_OPT_KERNEL, args.kernel)
     if args.waves_x16 > 0:
         dw.pool.set_option(cp.CP_OPT_WAVES_X16, args.waves_x16)
@@ -644,10 +646,11 @@ def main():
             # the same stages through the request queue (cp_queue_*): nothing is known to the kernel at launch, the
             # planner warp on the GPU cuts every stage into tiles as it reads it from the ring.  All stages are
             # pushed before the launch here, so this times the device-side planning, not the host's push rate.
-            qtimes = []
+            qtimes, qst = [], {"error": None}
             ids_l = [[int(x) for x in st] for st in stages]
+            use_queue = max(len(st) for st in stages) <= 12          # a queue entry holds at most 12 requests
             wsq = torch.empty(max(4 * wsb, 64 << 20), dtype=torch.uint8, device=dev)
-            for i in range(3 + 10):
+            for i in range(3 + 10 if use_queue else 0):
                 qu = cp.Queue(pool_l, max_stages=len(stages) + 1)
                 for st_ids, dp in zip(ids_l, deps):
                     qu.push(st_ids, dp, 1.0)
@@ -692,9 +695,10 @@ def main():
             kv_bytes = sum(w.requests[i].context_len * w.models[w.requests[i].model_id].n_kv_heads * 512
                            for b, _ in order for i in batches[b])
             t1, t2 = float(np.median(one[3:])), float(np.median(sep[3:]))
-            tq = float(np.median(qtimes[3:]))
+            tq = float(np.median(qtimes[3:])) if use_queue else None
             return {"stages": len(order), "kv_bytes": int(kv_bytes), "one_launch_us": 1e3 * t1,
-                    "queue_launch_us": 1e3 * tq, "queue_us_per_stage": 1e3 * tq / len(order), "queue_device_error": qst["error"],
+                    "queue_launch_us": 1e3 * tq if use_queue else None,
+                    "queue_us_per_stage": 1e3 * tq / len(order) if use_queue else None, "queue_device_error": qst["error"],
                     "separate_launches_us": 1e3 * t2, "one_launch_us_per_stage": 1e3 * t1 / len(order),
                     "separate_us_per_stage": 1e3 * t2 / len(order),
                     "host_driven_us_per_stage_wall": 1e3 * t3 / len(order), "one_launch_gbs": kv_bytes / (t1 * 1e-3) / 1e9,
