@@ -3,7 +3,10 @@
 TEST INFRASTRUCTURE ONLY: importable from tests/, `__graft_entry__.smoke()` and
 `bench.py`'s cpu_baseline / `--impl reference` legs.  Nothing under
 `paper_2606_24506_b200/` may import it, and it imports nothing from there.
-This file only marshals arguments; all arithmetic is in the C file.
+The attention, gather, append and planner arithmetic is in the C file; this file marshals arguments and holds
+the three pieces written in numpy / Python loops (each pinned like the C parts): `stage_query` / `_bf16_round`
+(bf16 rounding of a dependent stage's query, pin P20), the stage loop of `decode_stages` (P19, P21, P22) and the
+per-query-token loop of `attention_qlen` (P23-P25).
 """
 from __future__ import annotations
 
