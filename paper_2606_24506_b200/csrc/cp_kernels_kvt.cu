@@ -26,17 +26,19 @@
 // through shared memory costs ~3 us; with the tokens on M one elected thread issues 16 MMAs per 128
 // tokens for ANY g <= N, and the tile result sits in ONE accumulator.
 //
-// Warp roles (320 threads, 1 CTA / SM):
-//   warp 0      producer: walks this CTA's static tiles, then pops the dynamic ones (step a5); translates
-//               logical pages through the page table (step a2) and streams them with TMA into a ring of
-//               64 KB slice stages [K d0-63 | K d64-127 | V d0-63 | V d64-127], each a [128 tok x 128 B]
-//               SWIZZLE_128B block that the pages of the slice fill top to bottom; stages the tile's
-//               query rows in shared memory (the next tile's record is fetched while the current streams).
+// Warp roles (352 threads, 1 CTA / SM):
+//   warp 0      producer: pure TMA issue.  Takes tiles from the scheduler warp, translates the logical pages beyond
+//               the first 32 through the page table (step a2) and streams the pages into a ring of 64 KB slice
+//               stages [K d0-63 | K d64-127 | V d0-63 | V d64-127], each a [128 tok x 128 B] SWIZZLE_128B block
+//               that the pages of the slice fill top to bottom.
 //   warp 1      MMA issuer (one lane by elect.sync); the slices of consecutive tiles form one software
 //               pipeline: S of slice j is issued before P.V of slice j - 1, across tile boundaries.
 //   warps 2..5  softmax (thread = token of the slice).
 //   warps 6..9  epilogue (thread = value column d): O^T from TMEM -> normalised output or split partial,
 //               (m, l), release of the group's arrival counter (step a6).
+//   warp 10     scheduler, the control plane (step a5): walks this CTA's static tile list, then pops the dynamic
+//               one; fetches records, context lengths, first page ids; stages the query rows (cp.async); writes
+//               the new K / V rows of a fused append (cp_decode_step); announces tiles up to three ahead.
 //   all warps   LSE combine units after the CTA's last tile (step a4).
 //
 // Paper anchors: paged KV interface PAPER.md:L101,L122; KV-head-limited attention under low
