@@ -74,8 +74,10 @@ struct TileRec {
                                    // of the group's partial layout; other kernels: see their planner
     int64_t q_off, out_off, lse_off, part_off;
     int64_t app_k_off, app_v_off;  // element offsets of this group's new K / V row in the packed k_new / v_new of cp_decode_step
+    int32_t first_pid[8];          // tcgen05 K/V kernel: physical ids of the tile's first pages (one 128-token slice: 128 / P <= 8),
+                                   // so that the first TMA loads need no page-table round trip (ids of mapped pages never change)
 };
-static_assert(sizeof(TileRec) == 96, "TileRec is loaded as 16-byte vectors (five for the fields the older kernels use, six in all)");
+static_assert(sizeof(TileRec) == 128, "TileRec is loaded as 16-byte vectors (five for the fields the older kernels use, eight in all)");
 
 // One request of a cp_pool_append_kv batch.
 struct AppendRec {
@@ -246,6 +248,10 @@ struct DecodeParams {
     int32_t q_max_stages, q_max_tiles, q_max_units, q_max_groups;
     int32_t q_target_tiles, q_min_tile_pages;
     int64_t q_ws_floats_cap;
+    int32_t *req_ctx_next;         // cp_decode_step on the tcgen05 K/V kernel: the OTHER context table, which the launch fills
+                                   // (all max_requests entries copied, the batch's requests + ctx_add), or nullptr
+    int32_t ctx_add;               // added to every context length the launch reads (1 during such a step, else 0)
+    int32_t max_requests;
     const uint16_t *app_k, *app_v; // cp_decode_step: packed new K / V rows the launch writes at position
                                    // context_len - 1 of every request before the page that holds it is read, or nullptr
 };

@@ -364,10 +364,12 @@ __device__ __noinline__ void queue_planner(const DecodeParams &p, const int lane
                         r.split = t; r.n_splits = nsp; r.gsize = hpk; r.n_q_heads = hq; r.scale_log2 = scale; r.pad = s;
                         r.q_off = row0 * KV_D; r.out_off = row0 * KV_D; r.lse_off = row0; r.part_off = part_off;
                         r.app_k_off = 0; r.app_v_off = 0;
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) r.first_pid[i] = 0;
                         uint4 *dst = reinterpret_cast<uint4 *>(recs + n_tiles + t);
                         const uint4 *src = reinterpret_cast<const uint4 *>(&r);
 #pragma unroll
-                        for (int i = 0; i < 6; ++i) __stcg(dst + i, src[i]);
+                        for (int i = 0; i < 8; ++i) __stcg(dst + i, src[i]);
                     }
                 }
                 n_tiles += nsp;

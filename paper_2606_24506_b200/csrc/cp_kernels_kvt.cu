@@ -89,9 +89,9 @@ struct KtMeta {                  // what the scheduler warp hands to the produce
     int32_t item;                // < 0: no more work
     int32_t req, kv_head, n_kv_heads, page_begin, n_pages;
     int32_t pad[2];
-    int32_t pid[32];             // the tile's first 32 physical pages
+    int32_t pid[8];              // the physical pages of the tile's first slice (from the tile record)
 };
-static_assert(sizeof(KtMeta) == 160, "KtMeta layout");
+static_assert(sizeof(KtMeta) == 64, "KtMeta layout");
 
 struct KtMisc {
     uint64_t full[4], empty[4];                  // slice ring: TMA -> MMA, MMA (commit) -> TMA
@@ -163,7 +163,7 @@ __device__ __forceinline__ TileRec load_tile_rec(const TileRec *recs, int item)
     const uint4 *src = reinterpret_cast<const uint4 *>(recs + item);
     uint4 *dst = reinterpret_cast<uint4 *>(&r);
 #pragma unroll
-    for (int i = 0; i < 6; ++i) dst[i] = __ldg(src + i);
+    for (int i = 0; i < 8; ++i) dst[i] = __ldg(src + i);
     return r;
 }
 
@@ -345,6 +345,11 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
         }
     }
     scheduler_reset_other_set(p);
+    // Fused decode step: the same CTA fills the context table of the launches that follow -- every entry copied here,
+    // the batch's requests set to + ctx_add after the barrier below (no launch reads the table it writes).
+    const bool fill_ctx = p.req_ctx_next != nullptr && blockIdx.x == gridDim.x - 1;
+    if (fill_ctx)
+        for (int i = tid; i < p.max_requests; i += KT_THREADS) p.req_ctx_next[i] = __ldg(p.req_ctx + i);
 
     if (tid == 32) {
         for (int i = 0; i < NS; ++i) { mbar_init(smem_u32(&mi->full[i]), 1); mbar_init(smem_u32(&mi->empty[i]), 1); }
@@ -365,6 +370,12 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = mi->tmem_base;
+    if (tid == 0) kt_stamp(p, 14);
+    if (fill_ctx && warp == 9)                      // an epilogue warp: idle until the first tile ends
+        for (int g = lane; g < p.n_groups; g += 32) {
+            const Group gr = p.groups[g];
+            if (gr.kv_head == 0) p.req_ctx_next[gr.req] = __ldg(p.req_ctx + gr.req) + p.ctx_add;
+        }
 
     if (warp == 0) {
         // =========================================================== producer warp: pure TMA issue
@@ -378,17 +389,19 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             const KtMeta *mt = &mi->meta[ms];
             const int item = mt->item;
             if (item < 0) break;
+            if (lane == 0 && ti == 0) kt_stamp(p, 1);
             const int req = mt->req, hkv = mt->n_kv_heads, kvh = mt->kv_head, pb = mt->page_begin, npg = mt->n_pages;
-            int32_t pid = mt->pid[lane];
+            const int nf = min(pps, npg);                    // pages of the first slice: ids came with the tile record
+            int32_t pid = lane < 8 ? mt->pid[lane] : 0;
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(&mi->meta_empty[ms]));
             ++ti;
-            for (int j0 = 0; j0 < npg; j0 += 32) {
-                // translation of the batch after this one (step a2: one page-table entry per lane) is requested
-                // now and looked at when this batch's pages have been issued
-                int32_t pid_nx = 0;
-                if (j0 + 32 + lane < npg) pid_nx = page_of(p, req, (int64_t)(pb + j0 + 32 + lane) * hkv + kvh);
-                const int nj = min(32, npg - j0);
+            // translation of the pages behind them (step a2: one page-table entry per lane, 32 at a time) is
+            // requested now -- it travels while the first slice is issued -- and one batch ahead from then on
+            int32_t pid_nx = 0;
+            if (nf + lane < npg) pid_nx = page_of(p, req, (int64_t)(pb + nf + lane) * hkv + kvh);
+            for (int j0 = 0; j0 < npg;) {
+                const int nj = j0 == 0 ? nf : min(32, npg - j0);
                 for (int j = 0; j < nj; ++j) {
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);
                     const int jj = j0 + j;
@@ -408,7 +421,10 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                     }
                     if (pg == pps - 1 || jj == npg - 1) ++gs;
                 }
+                j0 += nj;
                 pid = pid_nx;
+                pid_nx = 0;
+                if (j0 + 32 + lane < npg) pid_nx = page_of(p, req, (int64_t)(pb + j0 + 32 + lane) * hkv + kvh);
             }
         }
         if (lane == 0) {
@@ -464,22 +480,32 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 }
                 break;
             }
-            // ---- one round trip: the first 32 page ids and the context length (which decides only how many
-            // tokens of the tile's LAST slice are valid: every planned page holds a valid token, contexts never
-            // shrink under a plan).  Volatile asm: issued here, not sunk to their first use.
-            int32_t pid0 = 0;
+            // ---- the producer gets the tile as soon as its record is here: the ids of the first slice's pages came
+            // with the record, it translates the rest itself.  (Not for the tile a fused append writes into: its
+            // last page must not be requested before the new row is stored, see below.)
+            const bool app = p.app_k != nullptr && (r.pad & 2);
+            auto hand_to_producer = [&]() {
+                mbar_wait(smem_u32(&mi->meta_empty[ms]), ((ti / KT_MQ) & 1) ^ 1);
+                KtMeta *mt = &mi->meta[ms];
+                if (lane < 8) mt->pid[lane] = r.first_pid[lane];
+                if (lane == 0) {
+                    mt->item = item; mt->req = r.req; mt->kv_head = r.kv_head; mt->n_kv_heads = r.n_kv_heads;
+                    mt->page_begin = r.page_begin; mt->n_pages = r.n_pages;
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&mi->meta_full[ms]));   // release: the producer acquires via try_wait
+            };
+            if (lane == 0 && ti == 0) kt_stamp(p, 15);
+            if (!app) hand_to_producer();
+            // ---- one round trip: the context length (it decides only how many tokens of the tile's LAST slice are
+            // valid: every planned page holds a valid token, contexts never shrink under a plan), the query rows
+            // and, for a fused append, the new row and its page.  Volatile asm: issued here, not sunk to first use.
             int ctx;
-            if (lane < r.n_pages) {
-                if (p.slot_pages > 0) pid0 = r.req * p.slot_pages + (r.page_begin + lane) * r.n_kv_heads + r.kv_head;
-                else
-                    asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(pid0)
-                                 : "l"(p.page_table + (int64_t)r.req * p.max_ppr + (int64_t)(r.page_begin + lane) * r.n_kv_heads + r.kv_head));
-            }
             asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(ctx) : "l"(p.req_ctx + r.req));
+            ctx += p.ctx_add;                    // a fused step reads the table of the step before (see req_ctx_next)
             // ---- fused append (cp_decode_step): the tile that holds its group's last page writes the
             // new token's K and V rows (position ctx - 1) before the producer is told about the tile, i.e. before
             // the page is requested.  Source row and the page's id travel in the same round trip.
-            const bool app = p.app_k != nullptr && (r.pad & 2);
             uint4 app_row = make_uint4(0u, 0u, 0u, 0u);
             int32_t app_pid = 0;
             if (app) {
@@ -516,32 +542,23 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 __threadfence();
                 fence_proxy_async_all();
                 __syncwarp();
+                hand_to_producer();
             }
-            mbar_wait(smem_u32(&mi->meta_empty[ms]), ((ti / KT_MQ) & 1) ^ 1);
             mbar_wait(smem_u32(&mi->tq_empty[qs]), ((ti / KT_TQ) & 1) ^ 1);
-            {
-                KtMeta *mt = &mi->meta[ms];
-                mt->pid[lane] = pid0;
-                if (lane == 0) {
-                    mt->item = item; mt->req = r.req; mt->kv_head = r.kv_head; mt->n_kv_heads = r.n_kv_heads;
-                    mt->page_begin = r.page_begin; mt->n_pages = r.n_pages;
-                    const int t_begin = r.page_begin * P;
-                    const int t_end = min((r.page_begin + r.n_pages) * P, ctx);
-                    const int n_slices = (t_end - t_begin + KT_SLICE - 1) / KT_SLICE;
-                    KtDesc d;
-                    d.item = item; d.group_idx = r.group; d.n_slices = n_slices;
-                    d.valid_last = t_end - t_begin - (n_slices - 1) * KT_SLICE;
-                    d.split = r.split; d.n_splits = r.n_splits; d.gsize = r.gsize; d.scale_log2 = r.scale_log2;
-                    d.zl = (r.pad >> 8) & 0xff; d.pad = 0;
-                    d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
-                    mi->tq[qs] = d;
-                }
-                __syncwarp();
-                if (lane == 0) {
-                    mbar_arrive(smem_u32(&mi->meta_full[ms]));   // release: the producer acquires via try_wait
-                    mbar_arrive(smem_u32(&mi->tq_full[qs]));
-                }
+            if (lane == 0) {
+                const int t_begin = r.page_begin * P;
+                const int t_end = min((r.page_begin + r.n_pages) * P, ctx);
+                const int n_slices = (t_end - t_begin + KT_SLICE - 1) / KT_SLICE;
+                KtDesc d;
+                d.item = item; d.group_idx = r.group; d.n_slices = n_slices;
+                d.valid_last = t_end - t_begin - (n_slices - 1) * KT_SLICE;
+                d.split = r.split; d.n_splits = r.n_splits; d.gsize = r.gsize; d.scale_log2 = r.scale_log2;
+                d.zl = (r.pad >> 8) & 0xff; d.pad = 0;
+                d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
+                mi->tq[qs] = d;
+                mbar_arrive(smem_u32(&mi->tq_full[qs]));     // release: the consumers acquire via try_wait
             }
+            __syncwarp();
             ++ti;
             item = item_next; r = r_next;
         }

@@ -68,7 +68,14 @@ struct KindPlan {
     bool uploaded = false;
     int counter_set = 0;             // scheduler counter set the next launch uses (alternates)
     int extra_counters = 0;          // multi-stage plans: one completion counter per stage after the groups'
-    DevBuf d_groups, d_tiles, d_tile_recs, d_combines, d_cunits, d_counters;   // counters: [32] scheduler + [n_groups * kCounterStride]
+    // device copy: ONE buffer (one host -> device copy per new plan) holding groups | tiles | tile_recs | combines | cunits,
+    // the p_* pointers into it, and the counters: [32] scheduler + [n_groups * kCounterStride], twice
+    DevBuf d_pack, d_counters;
+    // pinned staging, a ring of four: a pageable source would make cudaMemcpyAsync wait for the stream (the copy is
+    // staged chunk by chunk behind the work already queued), i.e. synchronise host and device on every new plan
+    struct PinBuf { void *ptr = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; bool used = false; } pin[4];
+    unsigned pin_next = 0;
+    void *p_groups = nullptr, *p_tiles = nullptr, *p_tile_recs = nullptr, *p_combines = nullptr, *p_cunits = nullptr;
 };
 
 }  // namespace
@@ -106,6 +113,7 @@ struct cp_pool {
     int qlen = 1, plan_qlen = 1;
     bool plan_for_stages = false;        // build_plan is called for a multi-stage work list (mma.sync kernel)
     const uint16_t *step_k = nullptr, *step_v = nullptr;   // cp_decode_step in progress: new rows the decode launch itself writes
+    bool step_ctx_on_device = false;     // ... and the launch advances the device context table itself
     int opt_timeline = 0;                // CP_OPT_TIMELINE: per-CTA globaltimer stamps of the next decode launches
     int timeline_ctas = 0;               // grid size of the last launch that wrote stamps
     int device = -1;                     // device of the arena (the compute calls require it to be current)
@@ -123,7 +131,9 @@ struct cp_pool {
     // device side (lazy)
     bool dev_ready = false;
     int n_sm = 148;
-    DevBuf d_page_table, d_ctx, d_models, d_append, d_timeline;
+    DevBuf d_page_table, d_ctx, d_models, d_append, d_timeline;   // d_ctx: TWO context tables of max_requests ints
+    int ctx_cur = 0;                     // the table launches read; a fused decode step lets its kernel write the other
+                                         // one (every entry copied, the batch's + 1) and flips this: no upload per step
     alignas(64) unsigned char kv_tmap[128];   // CUtensorMap of the arena for the MQA/GQA kernel
     bool kv_tmap_ok = false;
     alignas(64) unsigned char mla_tmap[128];  // CUtensorMap of the arena for the MLA kernel
@@ -191,6 +201,8 @@ bool model_supported(const cp_model_cfg &m, uint32_t P, uint32_t page_bytes)
 // their static lists are done: the SMs' streaming rates differ by a few per cent, and the tail
 // lets the fast ones take more.  Every tile is a fixed token range with its own split slot, so
 // results do not depend on which CTA runs it (deterministic).
+constexpr int KT_COMBINE_WARPS = 11;     // warps per CTA of the tcgen05 K/V kernel (all of them run combine units)
+
 void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint64_t &ws)
 {
     const int P = (int)pool->P;
@@ -279,6 +291,7 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
 
     // groups, split slots (in token order: static tiles, then tail tiles), combine units
     std::vector<int> split_base(ng, 0);
+    kp.groups.reserve(ng);
     for (int g = 0; g < ng; ++g) {
         const GInfo &G = gi[g];
         const Request &r = pool->reqs[ids[G.b]];
@@ -336,6 +349,11 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
         if (r.page_begin + r.n_pages == G.n_lp) r.pad |= 2;      // the group's last planned page is in this tile
         r.app_k_off = pool->app_k_off[G.b] + (int64_t)gr.kv_head * m.head_dim_qk;
         r.app_v_off = pool->app_v_off[G.b] + (int64_t)gr.kv_head * m.head_dim_v;
+        {
+            const Request &rq = pool->reqs[gr.req];
+            for (int i = 0; i < 8 && i < r.n_pages && i < pps; ++i)
+                r.first_pid[i] = rq.pages[(size_t)(r.page_begin + i) * m.n_kv_heads + gr.kv_head];
+        }
         return r;
     };
     // split index of a tile = its rank inside the group by position (tl is in that order per group)
@@ -345,38 +363,32 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
     // device order: the CTAs' static lists interleaved (slot j of CTA b at j * grid + b), then the tail tiles, longest first
     const int64_t n_pieces_used = n_static_tiles ? tl[n_static_tiles - 1].piece + 1 : 0;
     int grid = (int)std::min<int64_t>(n_ctas, std::max<int64_t>(std::max<int64_t>(n_pieces_used, 1),
-                                                                 ((int64_t)kp.cunits.size() + 9) / 10));
+                                                                 ((int64_t)kp.cunits.size() + KT_COMBINE_WARPS - 1) / KT_COMBINE_WARPS));
     if (tl.size() > (size_t)n_static_tiles) grid = n_ctas;          // dynamic tiles: every CTA may take some
-    std::vector<std::vector<int>> lists(grid);
-    for (int i = 0; i < n_static_tiles; ++i) lists[tl[i].piece % grid].push_back(i);
+    // (tl holds the static tiles in piece order, so CTA b's list is b's tiles in tl order: two counting passes)
+    std::vector<int> cnt(grid, 0), slot_of(n_static_tiles);
+    for (int i = 0; i < n_static_tiles; ++i) slot_of[i] = cnt[tl[i].piece % grid]++;
     size_t rounds = 0;
-    for (const auto &l : lists) rounds = std::max(rounds, l.size());
-    if (n_static_tiles == 0) rounds = 0;
-    kp.tile_recs.assign(rounds * (size_t)grid, TileRec());
-    for (auto &r : kp.tile_recs) std::memset(&r, 0, sizeof(r));
-    std::vector<int> order;                                     // real tiles in device order (reporting)
-    for (size_t j = 0; j < rounds; ++j)
-        for (int b = 0; b < grid; ++b)
-            if (j < lists[b].size()) {
-                const int i = lists[b][j];
-                TileRec r = make_rec(tl[i], split_of[i]);
-                r.pad |= j + 1 < lists[b].size() ? 1 : 0;
-                kp.tile_recs[j * grid + b] = r;
-                order.push_back(i);
-            }
+    for (int b = 0; b < grid; ++b) rounds = std::max(rounds, (size_t)cnt[b]);
+    kp.tile_recs.resize(rounds * (size_t)grid + (tl.size() - n_static_tiles));
+    std::memset(kp.tile_recs.data(), 0, kp.tile_recs.size() * sizeof(TileRec));
+    for (int i = 0; i < n_static_tiles; ++i) {
+        const int b = tl[i].piece % grid, j = slot_of[i];
+        TileRec &r = kp.tile_recs[(size_t)j * grid + b];
+        r = make_rec(tl[i], split_of[i]);
+        r.pad |= j + 1 < cnt[b] ? 1 : 0;
+    }
     std::vector<int> tails;
     for (size_t i = n_static_tiles; i < tl.size(); ++i) tails.push_back((int)i);
     std::stable_sort(tails.begin(), tails.end(), [&](int a, int b) {
         return (tl[a].sl1 - tl[a].sl0) > (tl[b].sl1 - tl[b].sl0);
     });
-    for (int i : tails) {
-        kp.tile_recs.push_back(make_rec(tl[i], split_of[i]));
-        order.push_back(i);
-    }
-    for (int i : order) {
-        const TileRec r = make_rec(tl[i], split_of[i]);
-        kp.tiles.push_back(Tile{r.group, r.split, r.page_begin, r.page_begin + r.n_pages});
-    }
+    for (size_t t = 0; t < tails.size(); ++t)
+        kp.tile_recs[rounds * (size_t)grid + t] = make_rec(tl[tails[t]], split_of[tails[t]]);
+    // the real tiles in device order (reporting: cp_decode_plan)
+    kp.tiles.reserve(tl.size());
+    for (const TileRec &r : kp.tile_recs)
+        if (r.n_pages > 0) kp.tiles.push_back(Tile{r.group, r.split, r.page_begin, r.page_begin + r.n_pages});
     kp.grid = grid;
     kp.n_static_slots = (int)(rounds * (size_t)grid);
 }
@@ -616,7 +628,7 @@ cp_status ensure_device(cp_pool *pool)
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, adev) != cudaSuccess)
         return CP_ERR_CUDA;
     if (pool->d_page_table.ensure((size_t)pool->max_requests * pool->max_ppr * 4) != cudaSuccess ||
-        pool->d_ctx.ensure((size_t)pool->max_requests * 4) != cudaSuccess ||
+        pool->d_ctx.ensure((size_t)pool->max_requests * 4 * 2) != cudaSuccess ||
         pool->d_models.ensure(pool->models.size() * sizeof(DevModel)) != cudaSuccess) {
         cudaGetLastError();
         return CP_ERR_CUDA;
@@ -632,7 +644,8 @@ cp_status ensure_device(cp_pool *pool)
     if (cudaMemcpy(pool->d_models.ptr, dm.data(), dm.size() * sizeof(DevModel),
                    cudaMemcpyHostToDevice) != cudaSuccess)
         return CP_ERR_CUDA;
-    if (cudaMemset(pool->d_ctx.ptr, 0, (size_t)pool->max_requests * 4) != cudaSuccess)
+    pool->ctx_cur = 0;
+    if (cudaMemset(pool->d_ctx.ptr, 0, (size_t)pool->max_requests * 4 * 2) != cudaSuccess)
         return CP_ERR_CUDA;
     // TMA row coordinates are signed 32-bit: a tensor map is only used while every row index fits (a
     // CUDA-VMM pool reserves virtual space only and can exceed that; it then runs on the generic kernel)
@@ -698,7 +711,7 @@ cp_status flush_tables(cp_pool *pool, cudaStream_t stream)
     }
     if (pool->ctx_dirty_hi >= pool->ctx_dirty_lo) {
         const int lo = pool->ctx_dirty_lo, hi = pool->ctx_dirty_hi;
-        if (cudaMemcpyAsync((int32_t *)pool->d_ctx.ptr + lo, pool->h_ctx.data() + lo, (size_t)(hi - lo + 1) * 4,
+        if (cudaMemcpyAsync((int32_t *)pool->d_ctx.ptr + (size_t)pool->ctx_cur * pool->max_requests + lo, pool->h_ctx.data() + lo, (size_t)(hi - lo + 1) * 4,
                             cudaMemcpyHostToDevice, stream) != cudaSuccess)
             return CP_ERR_CUDA;
         pool->n_h2d_bytes += (size_t)(hi - lo + 1) * 4;
@@ -710,29 +723,41 @@ cp_status flush_tables(cp_pool *pool, cudaStream_t stream)
 cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
 {
     if (kp.uploaded) return CP_OK;
-    const size_t gb = kp.groups.size() * sizeof(Group), tb = kp.tiles.size() * sizeof(Tile);
-    const size_t cb = kp.combines.size() * sizeof(Combine), set_ints = 32 + (kp.groups.size() + kp.extra_counters) * (size_t)kCounterStride, nb = 2 * set_ints * 4;
-    const size_t ub = kp.cunits.size() * sizeof(CombineUnit);
-    const size_t rb = kp.tile_recs.size() * sizeof(TileRec);
-    if (kp.d_groups.ensure(gb) != cudaSuccess || kp.d_tiles.ensure(tb) != cudaSuccess ||
-        kp.d_combines.ensure(std::max(cb, (size_t)16)) != cudaSuccess ||
-        kp.d_cunits.ensure(std::max(ub, (size_t)64)) != cudaSuccess ||
-        kp.d_tile_recs.ensure(std::max(rb, (size_t)80)) != cudaSuccess ||
-        kp.d_counters.ensure(nb) != cudaSuccess) {
+    const size_t set_ints = 32 + (kp.groups.size() + kp.extra_counters) * (size_t)kCounterStride, nb = 2 * set_ints * 4;
+    const void *src[5] = {kp.groups.data(), kp.tiles.data(), kp.tile_recs.data(), kp.combines.data(), kp.cunits.data()};
+    const size_t bytes[5] = {kp.groups.size() * sizeof(Group), kp.tiles.size() * sizeof(Tile), kp.tile_recs.size() * sizeof(TileRec),
+                             kp.combines.size() * sizeof(Combine), kp.cunits.size() * sizeof(CombineUnit)};
+    size_t off[5], total = 0;
+    for (int i = 0; i < 5; ++i) { off[i] = total; total += (bytes[i] + 255) & ~(size_t)255; }
+    total = std::max(total, (size_t)256);
+    if (kp.d_pack.ensure(total) != cudaSuccess || kp.d_counters.ensure(nb) != cudaSuccess) {
         cudaGetLastError();
         return CP_ERR_CUDA;
     }
-    if (cudaMemcpyAsync(kp.d_groups.ptr, kp.groups.data(), gb, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
-        cudaMemcpyAsync(kp.d_tiles.ptr, kp.tiles.data(), tb, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
-        (cb && cudaMemcpyAsync(kp.d_combines.ptr, kp.combines.data(), cb, cudaMemcpyHostToDevice, stream) != cudaSuccess) ||
-        (rb && cudaMemcpyAsync(kp.d_tile_recs.ptr, kp.tile_recs.data(), rb, cudaMemcpyHostToDevice, stream) != cudaSuccess) ||
-        (ub && cudaMemcpyAsync(kp.d_cunits.ptr, kp.cunits.data(), ub, cudaMemcpyHostToDevice, stream) != cudaSuccess))
+    KindPlan::PinBuf &pb = kp.pin[kp.pin_next++ % 4];
+    if (pb.used && cudaEventSynchronize(pb.ev) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }   // its last copy (4 plans ago) is done
+    if (pb.cap < total) {
+        if (pb.ptr) cudaFreeHost(pb.ptr);
+        pb.ptr = nullptr; pb.cap = 0;
+        const size_t want = (total * 3 / 2 + 4095) & ~(size_t)4095;
+        if (cudaHostAlloc(&pb.ptr, want, cudaHostAllocDefault) != cudaSuccess) { cudaGetLastError(); pb.ptr = nullptr; return CP_ERR_CUDA; }
+        pb.cap = want;
+    }
+    if (!pb.ev && cudaEventCreateWithFlags(&pb.ev, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+    for (int i = 0; i < 5; ++i)
+        if (bytes[i]) std::memcpy((uint8_t *)pb.ptr + off[i], src[i], bytes[i]);
+    if (cudaMemcpyAsync(kp.d_pack.ptr, pb.ptr, total, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
+        cudaEventRecord(pb.ev, stream) != cudaSuccess)
         return CP_ERR_CUDA;
+    pb.used = true;
+    uint8_t *base = (uint8_t *)kp.d_pack.ptr;
+    kp.p_groups = base + off[0]; kp.p_tiles = base + off[1]; kp.p_tile_recs = base + off[2];
+    kp.p_combines = base + off[3]; kp.p_cunits = base + off[4];
     // two counter sets for alternate launches (scheduler_reset_other_set); a new plan starts from zero
     if (cudaMemsetAsync(kp.d_counters.ptr, 0, kp.d_counters.cap, stream) != cudaSuccess)
         return CP_ERR_CUDA;
     kp.counter_set = 0;
-    pool->n_h2d_bytes += gb + tb + cb + ub + rb;
+    pool->n_h2d_bytes += total;
     kp.uploaded = true;
     return CP_OK;
 }
@@ -853,14 +878,13 @@ cp_status cp_pool_free(cp_pool *pool)
     if (pool->side_stream) cudaStreamDestroy(pool->side_stream);
     pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release(); pool->d_append.release(); pool->d_timeline.release();
     for (int k = 0; k < 2; ++k) {
-        pool->plan[k].d_groups.release(); pool->plan[k].d_tiles.release();
-        pool->plan[k].d_combines.release(); pool->plan[k].d_cunits.release(); pool->plan[k].d_tile_recs.release();
-        pool->plan[k].d_counters.release();
+        pool->plan[k].d_pack.release(); pool->plan[k].d_counters.release();
+        for (auto &pb : pool->plan[k].pin) { if (pb.ptr) cudaFreeHost(pb.ptr); if (pb.ev) cudaEventDestroy(pb.ev); }
     }
     {
         KindPlan &kp = pool->splan.kp;
-        kp.d_groups.release(); kp.d_tiles.release(); kp.d_combines.release(); kp.d_cunits.release();
-        kp.d_tile_recs.release(); kp.d_counters.release(); pool->splan.d_stages.release(); pool->splan.d_gate.release();
+        kp.d_pack.release(); kp.d_counters.release(); pool->splan.d_stages.release(); pool->splan.d_gate.release();
+        for (auto &pb : kp.pin) { if (pb.ptr) cudaFreeHost(pb.ptr); if (pb.ev) cudaEventDestroy(pb.ev); }
     }
     delete pool;
     return CP_OK;
@@ -1286,13 +1310,13 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.arena = pool->arena; prm.page_tokens = pool->P; prm.page_bytes = pool->page_bytes;
         prm.page_table = (const int32_t *)pool->d_page_table.ptr; prm.max_ppr = pool->max_ppr;
         prm.slot_pages = (pool->vmm && !pool->opt_vmm_table) ? (int32_t)pool->slot_pages : 0;
-        prm.req_ctx = (const int32_t *)pool->d_ctx.ptr;
+        prm.req_ctx = (const int32_t *)pool->d_ctx.ptr + (size_t)pool->ctx_cur * pool->max_requests;
         prm.models = (const DevModel *)pool->d_models.ptr;
-        prm.groups = (const Group *)kp.d_groups.ptr;
-        prm.tiles = (const Tile *)kp.d_tiles.ptr;
-        prm.tile_recs = (const TileRec *)kp.d_tile_recs.ptr;
-        prm.combines = (const Combine *)kp.d_combines.ptr;
-        prm.cunits = (const CombineUnit *)kp.d_cunits.ptr;
+        prm.groups = (const Group *)kp.p_groups;
+        prm.tiles = (const Tile *)kp.p_tiles;
+        prm.tile_recs = (const TileRec *)kp.p_tile_recs;
+        prm.combines = (const Combine *)kp.p_combines;
+        prm.cunits = (const CombineUnit *)kp.p_cunits;
         prm.n_tiles = (int)kp.tiles.size(); prm.n_combines = (int)kp.combines.size();
         prm.n_static_slots = 0;
         prm.n_combine_units = prm.n_combines;
@@ -1307,6 +1331,13 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.published = nullptr; prm.gate_flag = nullptr; prm.gate_timeout_us = 0;
         prm.timeline = nullptr;
         prm.app_k = pool->step_k; prm.app_v = pool->step_v;
+        if (pool->step_ctx_on_device) {
+            // fused decode step whose kernel advances the context table itself: it reads table ctx_cur (+ 1 for the
+            // batch's requests) and writes the other one for the launches that follow
+            prm.ctx_add = 1;
+            prm.req_ctx_next = (int32_t *)pool->d_ctx.ptr + (size_t)(1 - pool->ctx_cur) * pool->max_requests;
+            prm.max_requests = pool->max_requests;
+        }
         if (pool->opt_timeline && !(both_kinds && k == 1)) prm.timeline = (unsigned long long *)pool->d_timeline.ptr;
         kp.counter_set ^= 1;
         const int n_ctas = pool->kind_ctas[k];
@@ -1357,6 +1388,13 @@ cp_status cp_decode_step(cp_pool *pool, const int32_t *request_ids_host, int32_t
     if (((uintptr_t)q_dev & 15u) || ((uintptr_t)out_dev & 15u) || ((uintptr_t)lse_dev & 3u)) return CP_ERR_INVALID_ARG;
     std::vector<AppendRec> recs;
     std::vector<int> grew;
+    cudaStream_t s = (cudaStream_t)stream;
+    st = ensure_device(pool);
+    if (st != CP_OK) return st;
+    st = adopt_stream(pool, s);
+    if (st != CP_OK) return st;
+    st = flush_tables(pool, s);                 // whatever earlier calls left pending: the device tables are current now
+    if (st != CP_OK) return st;
     st = append_host(pool, request_ids_host, n_requests, true, v_new_dev, recs, grew);
     if (st != CP_OK) return st;
     // the plan of the grown contexts decides the workspace; too small: the append is taken back, nothing changed
@@ -1366,7 +1404,6 @@ cp_status cp_decode_step(cp_pool *pool, const int32_t *request_ids_host, int32_t
         append_rollback(pool, request_ids_host, n_requests, grew);
         return CP_ERR_WORKSPACE;
     }
-    cudaStream_t s = (cudaStream_t)stream;
     // Requests whose attention kernel writes the new row itself (the tcgen05 K/V kernel: the tile that holds a
     // group's last page stores the row before it requests the page) need no launch of their own; the others
     // (MLA, generic shapes, CP_OPT_KERNEL = 1 / 3) get the append kernel first.
@@ -1374,16 +1411,29 @@ cp_status cp_decode_step(cp_pool *pool, const int32_t *request_ids_host, int32_t
     std::vector<AppendRec> sep;
     for (int b = 0; b < n_requests; ++b)
         if (!(fused_kv && pool->models[recs[b].model].kind == CP_KIND_KV)) sep.push_back(recs[b]);
-    st = adopt_stream(pool, s);
-    if (st != CP_OK) return st;
+    // Every request fused: the kernel also advances the context table (reads the current one + 1, writes the other
+    // one for later launches), so a decode iteration uploads nothing but the ids of newly opened pages.
+    const bool ctx_on_device = fused_kv && sep.empty() && pool->plan[CP_KIND_MLA].tiles.empty();
+    if (ctx_on_device) { pool->ctx_dirty_lo = INT32_MAX; pool->ctx_dirty_hi = -1; }     // the only dirty entries are this step's
     st = flush_tables(pool, s);
     if (st != CP_OK) return st;
     st = launch_append_recs(pool, sep, k_new_dev, v_new_dev, s);
     if (st != CP_OK) return st;
     pool->step_k = fused_kv ? (const uint16_t *)k_new_dev : nullptr;
     pool->step_v = fused_kv ? (const uint16_t *)v_new_dev : nullptr;
+    pool->step_ctx_on_device = ctx_on_device;
     st = cp_decode_attention(pool, request_ids_host, n_requests, q_dev, out_dev, lse_dev, workspace_dev, workspace_bytes, stream);
     pool->step_k = pool->step_v = nullptr;
+    pool->step_ctx_on_device = false;
+    if (ctx_on_device) {
+        if (st == CP_OK) pool->ctx_cur ^= 1;
+        else {                                   // the launch did not happen: the host values must be uploaded after all
+            for (int b = 0; b < n_requests; ++b) {
+                pool->ctx_dirty_lo = std::min(pool->ctx_dirty_lo, request_ids_host[b]);
+                pool->ctx_dirty_hi = std::max(pool->ctx_dirty_hi, request_ids_host[b]);
+            }
+        }
+    }
     return st;
 }
 
@@ -1624,13 +1674,13 @@ static cp_status decode_stages_core(cp_pool *pool, int32_t n_stages, const int32
     prm.arena = pool->arena; prm.page_tokens = pool->P; prm.page_bytes = pool->page_bytes;
     prm.page_table = (const int32_t *)pool->d_page_table.ptr; prm.max_ppr = pool->max_ppr;
     prm.slot_pages = (pool->vmm && !pool->opt_vmm_table) ? (int32_t)pool->slot_pages : 0;
-    prm.req_ctx = (const int32_t *)pool->d_ctx.ptr;
+    prm.req_ctx = (const int32_t *)pool->d_ctx.ptr + (size_t)pool->ctx_cur * pool->max_requests;
     prm.models = (const DevModel *)pool->d_models.ptr;
-    prm.groups = (const Group *)kp.d_groups.ptr;
-    prm.tiles = (const Tile *)kp.d_tiles.ptr;
-    prm.tile_recs = (const TileRec *)kp.d_tile_recs.ptr;
-    prm.combines = (const Combine *)kp.d_combines.ptr;
-    prm.cunits = (const CombineUnit *)kp.d_cunits.ptr;
+    prm.groups = (const Group *)kp.p_groups;
+    prm.tiles = (const Tile *)kp.p_tiles;
+    prm.tile_recs = (const TileRec *)kp.p_tile_recs;
+    prm.combines = (const Combine *)kp.p_combines;
+    prm.cunits = (const CombineUnit *)kp.p_cunits;
     prm.n_tiles = (int)kp.tiles.size(); prm.n_combines = 0;
     prm.n_static_slots = 0;
     prm.n_combine_units = (int)kp.cunits.size();
@@ -1915,7 +1965,7 @@ cp_status cp_queue_launch(cp_queue *q, const void *q_dev, float *out_dev, float 
     prm.arena = pool->arena; prm.page_tokens = pool->P; prm.page_bytes = pool->page_bytes;
     prm.page_table = (const int32_t *)pool->d_page_table.ptr; prm.max_ppr = pool->max_ppr;
     prm.slot_pages = (pool->vmm && !pool->opt_vmm_table) ? (int32_t)pool->slot_pages : 0;
-    prm.req_ctx = (const int32_t *)pool->d_ctx.ptr;
+    prm.req_ctx = (const int32_t *)pool->d_ctx.ptr + (size_t)pool->ctx_cur * pool->max_requests;
     prm.models = (const DevModel *)pool->d_models.ptr;
     prm.tile_recs = (const TileRec *)q->d_recs.ptr;
     prm.cunits = (const CombineUnit *)q->d_units.ptr;
