@@ -462,7 +462,8 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
     const int tid = threadIdx.x;
     const int warp = tid >> 5;
     const int lane = tid & 31;
-    scheduler_reset_other_set(p);
+    // programmatic dependent launch: see cp_kernels_kvt.cu (set-up overlaps the previous kernel's tail)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     if (tid == 0) {
         // full[s]: one arrive.expect_tx by the producer + the TMA transaction bytes.
@@ -476,6 +477,8 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
+    asm volatile("griddepcontrol.wait;" ::: "memory");    // from here on: data the previous kernel may have written
+    scheduler_reset_other_set(p);
 
 
     if (warp == KV_CWARPS) {
@@ -883,8 +886,13 @@ static cudaError_t launch_kv_tm(const DecodeParams &p, const CUtensorMap &tmap, 
         if (dev >= 0 && dev < 64) configured[dev] = true;
     }
     // the request queue adds the planner warp (only CTA 0's does anything)
-    cp_decode_kv_kernel<P, MULTI, QLEN><<<grid, MULTI == 2 ? KV_THREADS + 32 : KV_THREADS, smem, stream>>>(p, tmap, rows_per_page);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(MULTI == 2 ? KV_THREADS + 32 : KV_THREADS); cfg.dynamicSmemBytes = (size_t)smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, cp_decode_kv_kernel<P, MULTI, QLEN>, p, tmap, rows_per_page);
 }
 
 template <int P>

@@ -328,6 +328,9 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     const int P = (int)p.page_tokens;
     const int pps = KT_SLICE / P;                    // pages per slice
 
+    // the next kernel of the stream, if it was launched as a programmatic dependent, may take the SMs this grid's
+    // CTAs leave as they leave them (it waits for this grid's completion before it reads anything of ours)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // the scheduler's first tile record is requested before anything else: its latency (the L2 is cold
     // at the start of a step) runs under the barrier / tensor-memory set-up
     TileRec r_next;
@@ -344,13 +347,6 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             p.timeline[(size_t)blockIdx.x * kTimelineSlots + 8] = smid;
         }
     }
-    scheduler_reset_other_set(p);
-    // Fused decode step: the same CTA fills the context table of the launches that follow -- every entry copied here,
-    // the batch's requests set to + ctx_add after the barrier below (no launch reads the table it writes).
-    const bool fill_ctx = p.req_ctx_next != nullptr && blockIdx.x == gridDim.x - 1;
-    if (fill_ctx)
-        for (int i = tid; i < p.max_requests; i += KT_THREADS) p.req_ctx_next[i] = __ldg(p.req_ctx + i);
-
     if (tid == 32) {
         for (int i = 0; i < NS; ++i) { mbar_init(smem_u32(&mi->full[i]), 1); mbar_init(smem_u32(&mi->empty[i]), 1); }
         for (int i = 0; i < 2; ++i) {
@@ -370,12 +366,24 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = mi->tmem_base;
+    // Programmatic dependent launch: everything above (and the scheduler's first record, part of a plan uploaded
+    // before the previous kernel even started) ran while the previous kernel of the stream was still finishing, on
+    // the SMs its CTAs had already left.  From here on this launch touches what that kernel may have written
+    // (queries, the arena of a fused append, counters, partials), so it waits for its completion.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (tid == 0) kt_stamp(p, 14);
-    if (fill_ctx && warp == 9)                      // an epilogue warp: idle until the first tile ends
-        for (int g = lane; g < p.n_groups; g += 32) {
-            const Group gr = p.groups[g];
-            if (gr.kv_head == 0) p.req_ctx_next[gr.req] = __ldg(p.req_ctx + gr.req) + p.ctx_add;
-        }
+    scheduler_reset_other_set(p);
+    // Fused decode step: the last CTA fills the context table of the launches that follow -- every entry copied, then
+    // the batch's requests set to + ctx_add (no launch reads the table it writes).
+    if (p.req_ctx_next != nullptr && blockIdx.x == gridDim.x - 1) {
+        for (int i = tid; i < p.max_requests; i += KT_THREADS) p.req_ctx_next[i] = __ldg(p.req_ctx + i);
+        __syncthreads();
+        if (warp == 9)                              // an epilogue warp: idle until the first tile ends
+            for (int g = lane; g < p.n_groups; g += 32) {
+                const Group gr = p.groups[g];
+                if (gr.kv_head == 0) p.req_ctx_next[gr.req] = __ldg(p.req_ctx + gr.req) + p.ctx_add;
+            }
+    }
 
     if (warp == 0) {
         // =========================================================== producer warp: pure TMA issue
@@ -884,8 +892,14 @@ static cudaError_t launch_kvt_n(const DecodeParams &p, const CUtensorMap &tmap, 
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) configured[dev] = true;
     }
-    cp_decode_kvt_kernel<N><<<grid, KT_THREADS, kt_smem_bytes(N), stream>>>(p, tmap, rows_per_page);
-    return cudaGetLastError();
+    // launched as a programmatic dependent of the stream's previous kernel (see griddepcontrol.wait in the kernel)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(KT_THREADS); cfg.dynamicSmemBytes = (size_t)kt_smem_bytes(N); cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, cp_decode_kvt_kernel<N>, p, tmap, rows_per_page);
 }
 
 // grid: the number of CTAs the plan's static tile lists were laid out for (slot j of CTA b is record

@@ -119,7 +119,8 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     const uint32_t q_base = smem_u32(smem + M2_SMEM_Q);
     const uint32_t st_base = smem_u32(smem + M2_SMEM_STAGE);
     const uint32_t p_base = smem_u32(smem + M2_SMEM_P);
-    scheduler_reset_other_set(p);
+    // programmatic dependent launch: see cp_kernels_kvt.cu (set-up overlaps the previous kernel's tail)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     if (tid == 0) {
         for (int i = 0; i < M2_STAGES; ++i) {
@@ -138,6 +139,8 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     tc_fence_before();
     cluster_sync_all();                               // barriers of both CTAs initialised, TMEM allocated
     tc_fence_after();
+    asm volatile("griddepcontrol.wait;" ::: "memory");    // from here on: data the previous kernel may have written
+    scheduler_reset_other_set(p);
     const uint32_t tmem = mi->tmem_base;
     const int P = (int)p.page_tokens;
     const int spp = P / M2_TS;
@@ -507,9 +510,14 @@ cudaError_t launch_decode_mla2(const DecodeParams &p, const void *tmap9, const v
     if (pairs < (p.n_combine_units + 7) / 8) pairs = (p.n_combine_units + 7) / 8;
     if (pairs > n_ctas / 2) pairs = n_ctas / 2;
     if (pairs < 1) pairs = 1;
-    cp_decode_mla2_kernel<<<2 * pairs, M2_THREADS, M2_SMEM_BYTES, stream>>>(
-        p, *reinterpret_cast<const CUtensorMap *>(tmap9), *reinterpret_cast<const CUtensorMap *>(tmap2), rows_per_page);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(2 * pairs)); cfg.blockDim = dim3(M2_THREADS); cfg.dynamicSmemBytes = M2_SMEM_BYTES; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, cp_decode_mla2_kernel, p, *reinterpret_cast<const CUtensorMap *>(tmap9),
+                              *reinterpret_cast<const CUtensorMap *>(tmap2), rows_per_page);
 }
 
 }  // namespace cp
