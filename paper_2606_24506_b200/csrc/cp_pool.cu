@@ -70,7 +70,14 @@ struct KindPlan {
     int extra_counters = 0;          // multi-stage plans: one completion counter per stage after the groups'
     // device copy: ONE buffer (one host -> device copy per new plan) holding groups | tiles | tile_recs | combines | cunits,
     // the p_* pointers into it, and the counters: [32] scheduler + [n_groups * kCounterStride], twice
-    DevBuf d_pack, d_counters;
+    // Both exist twice: a new plan is copied into the pair the running launch does not use, on the pool's copy stream, so
+    // the upload overlaps the previous kernel instead of standing between two kernels of the stream.
+    DevBuf d_pack2[2], d_counters2[2];
+    int buf = 0;                          // the pair the current plan lives in
+    cudaEvent_t ev_users[2] = {nullptr, nullptr};   // [b]: every launch that read pair b so far (recorded when the plan moves away from b)
+    cudaEvent_t ev_copied = nullptr;                // the copy stream has finished the current plan's upload
+    void *p_counters = nullptr;
+    bool users_recorded[2] = {false, false};
     // pinned staging, a ring of four: a pageable source would make cudaMemcpyAsync wait for the stream (the copy is
     // staged chunk by chunk behind the work already queued), i.e. synchronise host and device on every new plan
     struct PinBuf { void *ptr = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; bool used = false; } pin[4];
@@ -159,7 +166,7 @@ struct cp_pool {
     cudaStream_t last_stream = nullptr;
     bool last_stream_valid = false;
     cudaEvent_t ev_switch = nullptr, ev_fork = nullptr, ev_join = nullptr;
-    cudaStream_t side_stream = nullptr;
+    cudaStream_t side_stream = nullptr, copy_stream = nullptr;
     int kind_ctas[2] = {0, 0};           // CTAs each attention kind of the cached plan was planned for
 
     // counters
@@ -730,10 +737,15 @@ cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
     size_t off[5], total = 0;
     for (int i = 0; i < 5; ++i) { off[i] = total; total += (bytes[i] + 255) & ~(size_t)255; }
     total = std::max(total, (size_t)256);
-    if (kp.d_pack.ensure(total) != cudaSuccess || kp.d_counters.ensure(nb) != cudaSuccess) {
+    const int t = 1 - kp.buf;                 // target pair: not the one the stream's queued launches read
+    if (kp.d_pack2[t].ensure(total) != cudaSuccess || kp.d_counters2[t].ensure(nb) != cudaSuccess) {
         cudaGetLastError();
         return CP_ERR_CUDA;
     }
+    if (!pool->copy_stream && cudaStreamCreateWithFlags(&pool->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+    for (int i = 0; i < 2; ++i)
+        if (!kp.ev_users[i] && cudaEventCreateWithFlags(&kp.ev_users[i], cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+    if (!kp.ev_copied && cudaEventCreateWithFlags(&kp.ev_copied, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
     KindPlan::PinBuf &pb = kp.pin[kp.pin_next++ % 4];
     if (pb.used && cudaEventSynchronize(pb.ev) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }   // its last copy (4 plans ago) is done
     if (pb.cap < total) {
@@ -746,16 +758,25 @@ cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
     if (!pb.ev && cudaEventCreateWithFlags(&pb.ev, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
     for (int i = 0; i < 5; ++i)
         if (bytes[i]) std::memcpy((uint8_t *)pb.ptr + off[i], src[i], bytes[i]);
-    if (cudaMemcpyAsync(kp.d_pack.ptr, pb.ptr, total, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
-        cudaEventRecord(pb.ev, stream) != cudaSuccess)
+    // copy stream: wait for the launches that read pair t (all enqueued before the plan moved to the other pair: ev_users[t]
+    // was recorded then), copy, clear the counters (two sets for alternate launches; a new plan starts from zero)
+    cudaStream_t cs = pool->copy_stream;
+    if ((kp.users_recorded[t] && cudaStreamWaitEvent(cs, kp.ev_users[t], 0) != cudaSuccess) ||
+        cudaMemcpyAsync(kp.d_pack2[t].ptr, pb.ptr, total, cudaMemcpyHostToDevice, cs) != cudaSuccess ||
+        cudaEventRecord(pb.ev, cs) != cudaSuccess ||
+        cudaMemsetAsync(kp.d_counters2[t].ptr, 0, kp.d_counters2[t].cap, cs) != cudaSuccess ||
+        cudaEventRecord(kp.ev_copied, cs) != cudaSuccess)
         return CP_ERR_CUDA;
     pb.used = true;
-    uint8_t *base = (uint8_t *)kp.d_pack.ptr;
+    // caller's stream: everything enqueued so far may read the old pair; the launches that follow wait for the copy
+    if (cudaEventRecord(kp.ev_users[kp.buf], stream) != cudaSuccess || cudaStreamWaitEvent(stream, kp.ev_copied, 0) != cudaSuccess)
+        return CP_ERR_CUDA;
+    kp.users_recorded[kp.buf] = true;
+    kp.buf = t;
+    uint8_t *base = (uint8_t *)kp.d_pack2[t].ptr;
     kp.p_groups = base + off[0]; kp.p_tiles = base + off[1]; kp.p_tile_recs = base + off[2];
     kp.p_combines = base + off[3]; kp.p_cunits = base + off[4];
-    // two counter sets for alternate launches (scheduler_reset_other_set); a new plan starts from zero
-    if (cudaMemsetAsync(kp.d_counters.ptr, 0, kp.d_counters.cap, stream) != cudaSuccess)
-        return CP_ERR_CUDA;
+    kp.p_counters = kp.d_counters2[t].ptr;
     kp.counter_set = 0;
     pool->n_h2d_bytes += total;
     kp.uploaded = true;
@@ -876,14 +897,20 @@ cp_status cp_pool_free(cp_pool *pool)
     if (pool->ev_fork) cudaEventDestroy(pool->ev_fork);
     if (pool->ev_join) cudaEventDestroy(pool->ev_join);
     if (pool->side_stream) cudaStreamDestroy(pool->side_stream);
+    if (pool->copy_stream) cudaStreamDestroy(pool->copy_stream);
     pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release(); pool->d_append.release(); pool->d_timeline.release();
     for (int k = 0; k < 2; ++k) {
-        pool->plan[k].d_pack.release(); pool->plan[k].d_counters.release();
+        pool->plan[k].d_pack2[0].release(); pool->plan[k].d_pack2[1].release(); pool->plan[k].d_counters2[0].release(); pool->plan[k].d_counters2[1].release();
+        for (auto &e : pool->plan[k].ev_users) if (e) cudaEventDestroy(e);
+        if (pool->plan[k].ev_copied) cudaEventDestroy(pool->plan[k].ev_copied);
         for (auto &pb : pool->plan[k].pin) { if (pb.ptr) cudaFreeHost(pb.ptr); if (pb.ev) cudaEventDestroy(pb.ev); }
     }
     {
         KindPlan &kp = pool->splan.kp;
-        kp.d_pack.release(); kp.d_counters.release(); pool->splan.d_stages.release(); pool->splan.d_gate.release();
+        kp.d_pack2[0].release(); kp.d_pack2[1].release(); kp.d_counters2[0].release(); kp.d_counters2[1].release();
+        for (auto &e : kp.ev_users) if (e) cudaEventDestroy(e);
+        if (kp.ev_copied) cudaEventDestroy(kp.ev_copied);
+        pool->splan.d_stages.release(); pool->splan.d_gate.release();
         for (auto &pb : kp.pin) { if (pb.ptr) cudaFreeHost(pb.ptr); if (pb.ev) cudaEventDestroy(pb.ev); }
     }
     delete pool;
@@ -1324,9 +1351,9 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         prm.q = (const uint16_t *)q_dev; prm.out = out_dev; prm.lse = lse_dev;
         prm.workspace = (float *)workspace_dev;
         const size_t set_ints = 32 + kp.groups.size() * (size_t)kCounterStride;
-        prm.work_counter = (int32_t *)kp.d_counters.ptr + kp.counter_set * set_ints;
+        prm.work_counter = (int32_t *)kp.p_counters + kp.counter_set * set_ints;
         prm.group_counters = prm.work_counter + 32;
-        prm.reset_counters = (int32_t *)kp.d_counters.ptr + (1 - kp.counter_set) * set_ints;
+        prm.reset_counters = (int32_t *)kp.p_counters + (1 - kp.counter_set) * set_ints;
         prm.stages = nullptr; prm.stage_done = nullptr; prm.n_stages = 0; prm.q_len = pool->qlen;
         prm.published = nullptr; prm.gate_flag = nullptr; prm.gate_timeout_us = 0;
         prm.timeline = nullptr;
@@ -1688,9 +1715,9 @@ static cp_status decode_stages_core(cp_pool *pool, int32_t n_stages, const int32
     prm.q = (const uint16_t *)q_dev; prm.out = out_dev; prm.lse = lse_dev;
     prm.workspace = (float *)workspace_dev;
     const size_t set_ints = 32 + (kp.groups.size() + (size_t)n_stages) * (size_t)kCounterStride;
-    prm.work_counter = (int32_t *)kp.d_counters.ptr + kp.counter_set * set_ints;
+    prm.work_counter = (int32_t *)kp.p_counters + kp.counter_set * set_ints;
     prm.group_counters = prm.work_counter + 32;
-    prm.reset_counters = (int32_t *)kp.d_counters.ptr + (1 - kp.counter_set) * set_ints;
+    prm.reset_counters = (int32_t *)kp.p_counters + (1 - kp.counter_set) * set_ints;
     prm.stages = (const StageRec *)sp.d_stages.ptr;
     prm.stage_done = prm.group_counters + kp.groups.size() * (size_t)kCounterStride;
     prm.n_stages = n_stages; prm.q_len = 1;
