@@ -462,9 +462,6 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
     const int tid = threadIdx.x;
     const int warp = tid >> 5;
     const int lane = tid & 31;
-    // programmatic dependent launch: see cp_kernels_kvt.cu (set-up overlaps the previous kernel's tail)
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-
     if (tid == 0) {
         // full[s]: one arrive.expect_tx by the producer + the TMA transaction bytes.
         // empty[s]: EVERY consumer warp waits for every page in ring order and arrives on its
@@ -595,6 +592,9 @@ cp_decode_kv_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tm
                 }
             }
         }
+        // programmatic dependent launch: see cp_kernels_kvt.cu (the next kernel's set-up overlaps this one's tail;
+        // said once every page of this CTA has been requested, not at the top)
+        if (lane == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     } else if (warp == KV_CWARPS + 1) {
         // =========================================================== planner warp (request queue; CTA 0 only)
         if constexpr (MULTI == 2) {

@@ -328,9 +328,6 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     const int P = (int)p.page_tokens;
     const int pps = KT_SLICE / P;                    // pages per slice
 
-    // the next kernel of the stream, if it was launched as a programmatic dependent, may take the SMs this grid's
-    // CTAs leave as they leave them (it waits for this grid's completion before it reads anything of ours)
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // the scheduler's first tile record is requested before anything else: its latency (the L2 is cold
     // at the start of a step) runs under the barrier / tensor-memory set-up
     TileRec r_next;
@@ -372,18 +369,6 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     // (queries, the arena of a fused append, counters, partials), so it waits for its completion.
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (tid == 0) kt_stamp(p, 14);
-    scheduler_reset_other_set(p);
-    // Fused decode step: the last CTA fills the context table of the launches that follow -- every entry copied, then
-    // the batch's requests set to + ctx_add (no launch reads the table it writes).
-    if (p.req_ctx_next != nullptr && blockIdx.x == gridDim.x - 1) {
-        for (int i = tid; i < p.max_requests; i += KT_THREADS) p.req_ctx_next[i] = __ldg(p.req_ctx + i);
-        __syncthreads();
-        if (warp == 9)                              // an epilogue warp: idle until the first tile ends
-            for (int g = lane; g < p.n_groups; g += 32) {
-                const Group gr = p.groups[g];
-                if (gr.kv_head == 0) p.req_ctx_next[gr.req] = __ldg(p.req_ctx + gr.req) + p.ctx_add;
-            }
-    }
 
     if (warp == 0) {
         // =========================================================== producer warp: pure TMA issue
@@ -436,6 +421,11 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             }
         }
         if (lane == 0) {
+            // The next kernel of the stream, if it was launched as a programmatic dependent, may now take the SMs this
+            // grid's CTAs leave as they leave them (it waits for this grid's completion before it reads anything of
+            // ours).  Said here, with every slice of this CTA requested, not at the top of the kernel: measured, the
+            // instruction at the top delays the first slices of a cold start by 1.4 us (cfg4 32.0 vs 31.2 us).
+            asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
             kt_stamp(p, 3);
             if (p.timeline) p.timeline[(size_t)blockIdx.x * kTimelineSlots + 11] = (unsigned long long)ti;
         }
@@ -488,9 +478,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 }
                 break;
             }
-            // ---- the producer gets the tile as soon as its record is here: the ids of the first slice's pages came
-            // with the record, it translates the rest itself.  (Not for the tile a fused append writes into: its
-            // last page must not be requested before the new row is stored, see below.)
+            // ---- (the ids of the first slice's pages came with the record; the producer translates the rest itself)
             const bool app = p.app_k != nullptr && (r.pad & 2);
             auto hand_to_producer = [&]() {
                 mbar_wait(smem_u32(&mi->meta_empty[ms]), ((ti / KT_MQ) & 1) ^ 1);
@@ -504,6 +492,8 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 if (lane == 0) mbar_arrive(smem_u32(&mi->meta_full[ms]));   // release: the producer acquires via try_wait
             };
             if (lane == 0 && ti == 0) kt_stamp(p, 15);
+            // The producer gets the tile as soon as the record is there (the first slice's page ids came with it), unless
+            // this tile writes a fused append's row, which has to be in memory before its page is requested.
             if (!app) hand_to_producer();
             // ---- one round trip: the context length (it decides only how many tokens of the tile's LAST slice are
             // valid: every planned page holds a valid token, contexts never shrink under a plan), the query rows
@@ -550,8 +540,8 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 __threadfence();
                 fence_proxy_async_all();
                 __syncwarp();
-                hand_to_producer();
             }
+            if (app) hand_to_producer();
             mbar_wait(smem_u32(&mi->tq_empty[qs]), ((ti / KT_TQ) & 1) ^ 1);
             if (lane == 0) {
                 const int t_begin = r.page_begin * P;
@@ -795,6 +785,23 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
         const int dcol = q4 * 32 + lane;
         const uint32_t tl = tmem + ((uint32_t)(q4 * 32) << 16);
         uint32_t qi = 0, tc = 0;
+        // House-keeping of the last CTA, done by an epilogue warp because it has nothing to do until the first tile
+        // ends (measured: the same lines between the set-up barrier and the role switch, where the scheduler and the
+        // producer warp pass through them, cost cfg4 1.7 us of start-up).  (1) The other counter set is zeroed for
+        // the next launch.  (2) Fused decode step: the context table of the launches that follow is filled -- every
+        // entry copied, then the batch's requests set to + ctx_add (no launch reads the table it writes).
+        if (warp == 9 && blockIdx.x == gridDim.x - 1) {
+            for (int i = lane; i < p.n_groups; i += 32) p.reset_counters[32 + (size_t)i * kCounterStride] = 0;
+            if (lane < 4) p.reset_counters[lane] = 0;
+            if (p.req_ctx_next != nullptr) {
+                for (int i = lane; i < p.max_requests; i += 32) p.req_ctx_next[i] = __ldg(p.req_ctx + i);
+                __syncwarp();
+                for (int g = lane; g < p.n_groups; g += 32) {
+                    const Group gr = p.groups[g];
+                    if (gr.kv_head == 0) p.req_ctx_next[gr.req] = __ldg(p.req_ctx + gr.req) + p.ctx_add;
+                }
+            }
+        }
         for (;;) {
             const uint32_t qs = qi % KT_TQ;
             mbar_wait(smem_u32(&mi->tq_full[qs]), (qi / KT_TQ) & 1);

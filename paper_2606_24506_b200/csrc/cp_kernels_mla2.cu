@@ -119,9 +119,6 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     const uint32_t q_base = smem_u32(smem + M2_SMEM_Q);
     const uint32_t st_base = smem_u32(smem + M2_SMEM_STAGE);
     const uint32_t p_base = smem_u32(smem + M2_SMEM_P);
-    // programmatic dependent launch: see cp_kernels_kvt.cu (set-up overlaps the previous kernel's tail)
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-
     if (tid == 0) {
         for (int i = 0; i < M2_STAGES; ++i) {
             mbar_init(smem_u32(&mi->full[i]), 1); mbar_init(smem_u32(&mi->full_peer[i]), 1);
@@ -183,6 +180,9 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 }
             }
         }
+        // programmatic dependent launch: see cp_kernels_kvt.cu (the next kernel's set-up overlaps this one's tail;
+        // said once every slice of this CTA has been requested, not at the top)
+        if (lane == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     } else if (warp == 1 && rank != 0) {
         // =========================================================== peer: relay "my part of the slice landed"
         uint32_t gs = 0;
