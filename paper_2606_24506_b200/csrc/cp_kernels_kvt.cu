@@ -81,6 +81,10 @@ struct KtDesc {                  // what the producer hands to the other warps f
     int32_t gsize;               // query rows of the group
     float scale_log2;
     int32_t zl;                  // log2 of the split lanes of the group's combine units: fixes the partial layout
+    int32_t q_len;               // query tokens per request (cp_decode_attention_qlen); row = (query token, head of the group)
+    int32_t hpk;                 // query heads per K/V head = gsize / q_len
+    int32_t n_q_heads;           // row (t, h) of the group is row t * n_q_heads + h of its request's Q / O / LSE
+    int32_t rem0;                // context length - first token of the tile (q_len > 1: causal limit of the rows)
     int32_t pad;
     int64_t q_off, out_off, lse_off, part_off;
 };
@@ -127,6 +131,15 @@ __device__ __forceinline__ void bar_sync_combine() { asm volatile("bar.sync 3, 3
 __device__ __forceinline__ void kt_stamp(const DecodeParams &p, int k)
 {
     if (p.timeline) p.timeline[(size_t)blockIdx.x * kTimelineSlots + k] = global_timer_ns();
+}
+
+// Factor that moves an accumulator from exponent reference m_old to m_new >= m_old (log2 units).  A row that has seen
+// no token yet has m_old = -inf and an accumulator of 0: the factor is 0; if it still sees none (q_len > 1: the whole
+// slice is behind the row's causal limit) m_new is -inf too and the factor must not be 2^(NaN).
+template <bool QL>
+__device__ __forceinline__ float kt_rescale(float m_old, float m_new)
+{
+    return QL && m_new == -INFINITY ? 0.f : ex2_ftz(m_old - m_new);
 }
 
 struct OpAdd { __device__ __forceinline__ float operator()(float a, float b) const { return a + b; } };
@@ -306,7 +319,9 @@ __device__ __forceinline__ void kt_combine(const DecodeParams &p, const int warp
     }
 }
 
-template <int N>
+// QL: the instantiation for q_len > 1 (cp_decode_attention_qlen); the q_len = 1 instantiations carry none of its
+// code -- a cold step fetches its instructions from HBM, and every line on the way to the first MMA counts.
+template <int N, bool QL>
 __global__ void __launch_bounds__(KT_THREADS, 1)
 cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap, int rows_per_page)
 {
@@ -412,7 +427,16 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                         tma_load_2d(dst + 3 * KT_SUBB, &tmap, 64, row + P, fb, policy); // V, d 64..127
                         if (gs == 0 && pg == 0) kt_stamp(p, 9);
                     }
-                    if (pg == pps - 1 || jj == npg - 1) ++gs;
+                    if (pg == pps - 1 || jj == npg - 1) {
+                        ++gs;
+                        // Cold start: after its very first slice the producer waits until the scheduler has announced
+                        // the tile, i.e. until the context length (and, requested with it, the query rows) has come
+                        // back.  Measured: otherwise 148 SMs put a whole ring (28 MB) in front of those two small loads
+                        // whenever they lose the race by a few hundred ns, the MMA warp starts 5-8 us late and the
+                        // step takes 37 instead of 31 us (cfg4).  (tq slot 0 is in its first phase for as long as the
+                        // producer is on its first tile: the scheduler runs at most KT_MQ < KT_TQ tiles ahead.)
+                        if (gs == 1) mbar_wait(smem_u32(&mi->tq_full[0]), 0);
+                    }
                 }
                 j0 += nj;
                 pid = pid_nx;
@@ -480,6 +504,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             }
             // ---- (the ids of the first slice's pages came with the record; the producer translates the rest itself)
             const bool app = p.app_k != nullptr && (r.pad & 2);
+            const int hpk = QL ? r.gsize / p.q_len : r.gsize;    // query heads per K/V head
             auto hand_to_producer = [&]() {
                 mbar_wait(smem_u32(&mi->meta_empty[ms]), ((ti / KT_MQ) & 1) ^ 1);
                 KtMeta *mt = &mi->meta[ms];
@@ -526,7 +551,10 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                     const int row = id >> 4, ch = id & 15;
                     const uint32_t a = qb + (ch >> 3) * (N * 128) + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
                     const uint32_t nbytes = row < r.gsize ? 16u : 0u;
-                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a), "l"(qg + (row < r.gsize ? id : 0)), "r"(nbytes) : "memory");
+                    // q_len > 1: row (t, h) of the group (token-major) is row t * Hq + h of the request's queries
+                    int src = row < r.gsize ? id : 0;
+                    if (QL && row < r.gsize) src = ((row / hpk) * r.n_q_heads + row % hpk) * 16 + ch;
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(a), "l"(qg + src), "r"(nbytes) : "memory");
                 }
                 asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(&mi->q_full[ti & 1])) : "memory");
             }
@@ -552,6 +580,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 d.valid_last = t_end - t_begin - (n_slices - 1) * KT_SLICE;
                 d.split = r.split; d.n_splits = r.n_splits; d.gsize = r.gsize; d.scale_log2 = r.scale_log2;
                 d.zl = (r.pad >> 8) & 0xff; d.pad = 0;
+                d.q_len = p.q_len; d.hpk = hpk; d.n_q_heads = r.n_q_heads; d.rem0 = ctx - t_begin;
                 d.q_off = r.q_off; d.out_off = r.out_off; d.lse_off = r.lse_off; d.part_off = r.part_off;
                 mi->tq[qs] = d;
                 mbar_arrive(smem_u32(&mi->tq_full[qs]));     // release: the consumers acquire via try_wait
@@ -675,11 +704,22 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 const bool tv = st < nvalid;
                 float x[N];
                 float ex = -INFINITY;
+                // q_len > 1 (causal among the query tokens): row (t, h) sees positions < ctx - (q_len - 1 - t), i.e. this
+                // thread's token, rem = ctx - position, is seen by the rows t >= q_len - rem: rows hmin .. N - 1.  Only the
+                // slices that reach into the context's last q_len - 1 tokens take this path (CTA-uniform).
+                const int rem_slice = d.rem0 - i * KT_SLICE;          // context length - first token of the slice
+                const bool cmask = QL && rem_slice < KT_SLICE + d.q_len - 1;
+                int hmin = 0;
+                if (cmask) hmin = max(0, d.q_len - (rem_slice - st)) * d.hpk;
 #pragma unroll
-                for (int h = 0; h < N; ++h) {
-                    x[h] = __uint_as_float(xr[h]) * d.scale_log2;
-                    ex = fmaxf(ex, x[h] - m_ref[h]);
+                for (int h = 0; h < N; ++h) x[h] = __uint_as_float(xr[h]) * d.scale_log2;
+                if (cmask) {
+#pragma unroll
+                    for (int h = 0; h < N; ++h)
+                        if (h < hmin) x[h] = -INFINITY;
                 }
+#pragma unroll
+                for (int h = 0; h < N; ++h) ex = fmaxf(ex, x[h] - m_ref[h]);     // (-inf) - (-inf) = NaN never wins the maximum
                 // NaN scores (NaN inputs) never trigger: they flow into P and O as in the definition
                 if (bar_red_or_softmax(tv && ex > KT_LAZY_LOG2)) {
                     // ---- the reference moves: column maxima of the slice, rescale O and the partial sums
@@ -710,7 +750,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                             tmem_wait_ld();
 #pragma unroll
                             for (int j = 0; j < 16; ++j)
-                                o[j] = __float_as_uint(__uint_as_float(o[j]) * ex2_ftz(m_ref[c + j] - mn[c + j]));
+                                o[j] = __float_as_uint(__uint_as_float(o[j]) * kt_rescale<QL>(m_ref[c + j], mn[c + j]));
                             tmem_st16(tl + (2 + ob) * N + c, o);
                         }
                         tmem_wait_st();
@@ -718,19 +758,32 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                     }
 #pragma unroll
                     for (int h = 0; h < N; ++h) {
-                        l_part[h] *= ex2_ftz(m_ref[h] - mn[h]);       // 2^(-inf) = 0 on the first slice (l_part is 0 there)
+                        l_part[h] *= kt_rescale<QL>(m_ref[h], mn[h]);     // 2^(-inf) = 0 on the first slice (l_part is 0 there)
                         m_ref[h] = mn[h];
                     }
                     bar_sync_softmax();        // redmax[] may be rewritten only after every thread has read it
                 }
                 uint32_t pw[N / 2];
+                if (!cmask) {
 #pragma unroll
-                for (int h = 0; h < N; h += 2) {
-                    const float p0 = tv ? ex2_ftz(x[h] - m_ref[h]) : 0.f;
-                    const float p1 = tv ? ex2_ftz(x[h + 1] - m_ref[h + 1]) : 0.f;
-                    l_part[h] += p0;
-                    l_part[h + 1] += p1;
-                    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pw[h >> 1]) : "f"(p1), "f"(p0));
+                    for (int h = 0; h < N; h += 2) {
+                        const float p0 = tv ? ex2_ftz(x[h] - m_ref[h]) : 0.f;
+                        const float p1 = tv ? ex2_ftz(x[h + 1] - m_ref[h + 1]) : 0.f;
+                        l_part[h] += p0;
+                        l_part[h + 1] += p1;
+                        asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pw[h >> 1]) : "f"(p1), "f"(p0));
+                    }
+                } else {
+                    // a masked score (-inf) under a reference that is still -inf (a row that sees no token of the tile
+                    // so far) would give 2^(NaN): such entries are 0 by the row test, not by the exponential
+#pragma unroll
+                    for (int h = 0; h < N; h += 2) {
+                        const float p0 = tv && h >= hmin ? ex2_ftz(x[h] - m_ref[h]) : 0.f;
+                        const float p1 = tv && h + 1 >= hmin ? ex2_ftz(x[h + 1] - m_ref[h + 1]) : 0.f;
+                        l_part[h] += p0;
+                        l_part[h + 1] += p1;
+                        asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(pw[h >> 1]) : "f"(p1), "f"(p0));
+                    }
                 }
                 // the P^T buffer is free once the value MMAs of slice g - 2 are complete
                 mbar_wait(smem_u32(&mi->p_done[b]), ((g >> 1) & 1) ^ 1);
@@ -840,10 +893,22 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             if (lane == 0) mbar_arrive(smem_u32(&mi->o_free[ob]));           // O^T buffer and hand-over area are free
             if (final_out) {
                 float *dst = p.out + d.out_off + dcol;
+                if (!QL) {
 #pragma unroll
-                for (int h = 0; h < N; ++h)
-                    if (h < d.gsize) dst[h * KT_D] = __uint_as_float(o[h]) * inv[h];
-                if (dcol < d.gsize) p.lse[d.lse_off + dcol] = (mr + log2f(Lh)) * 0.6931471805599453f;
+                    for (int h = 0; h < N; ++h)
+                        if (h < d.gsize) dst[h * KT_D] = __uint_as_float(o[h]) * inv[h];
+                    if (dcol < d.gsize) p.lse[d.lse_off + dcol] = (mr + log2f(Lh)) * 0.6931471805599453f;
+                } else {
+                    // row (t, hh) of the group is row t * Hq + hh of the request's output
+                    int t = 0, hh = 0;
+#pragma unroll
+                    for (int h = 0; h < N; ++h) {
+                        if (h < d.gsize) dst[(size_t)(t * d.n_q_heads + hh) * KT_D] = __uint_as_float(o[h]) * inv[h];
+                        if (++hh == d.hpk) { hh = 0; ++t; }
+                    }
+                    if (dcol < d.gsize)
+                        p.lse[d.lse_off + (dcol / d.hpk) * d.n_q_heads + dcol % d.hpk] = (mr + log2f(Lh)) * 0.6931471805599453f;
+                }
             } else {
                 // O partial of head h, split s, column c: [h][c / (4 CQ)][s][(c / 4) % CQ][c % 4] with
                 // CQ = 32 >> zl column quads per combine unit, so that the 32 lanes of a combine unit -- 2^zl
@@ -886,7 +951,7 @@ int kvt_pad_rows(int g)          // N of the instantiation that serves groups of
     return g <= 16 ? 16 : g <= 32 ? 32 : 0;
 }
 
-template <int N>
+template <int N, bool QL>
 static cudaError_t launch_kvt_n(const DecodeParams &p, const CUtensorMap &tmap, int rows_per_page, int grid,
                                 cudaStream_t stream)
 {
@@ -895,7 +960,7 @@ static cudaError_t launch_kvt_n(const DecodeParams &p, const CUtensorMap &tmap, 
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64 || !configured[dev]) {
-        e = cudaFuncSetAttribute(cp_decode_kvt_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, kt_smem_bytes(N));
+        e = cudaFuncSetAttribute(cp_decode_kvt_kernel<N, QL>, cudaFuncAttributeMaxDynamicSharedMemorySize, kt_smem_bytes(N));
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) configured[dev] = true;
     }
@@ -906,7 +971,7 @@ static cudaError_t launch_kvt_n(const DecodeParams &p, const CUtensorMap &tmap, 
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, cp_decode_kvt_kernel<N>, p, tmap, rows_per_page);
+    return cudaLaunchKernelEx(&cfg, cp_decode_kvt_kernel<N, QL>, p, tmap, rows_per_page);
 }
 
 // grid: the number of CTAs the plan's static tile lists were laid out for (slot j of CTA b is record
@@ -917,8 +982,10 @@ cudaError_t launch_decode_kvt(const DecodeParams &p, const void *tmap, int rows_
     const CUtensorMap &tm = *reinterpret_cast<const CUtensorMap *>(tmap);
     if (grid < 1) grid = 1;
     switch (kvt_pad_rows(max_group)) {
-    case 16: return launch_kvt_n<16>(p, tm, rows_per_page, grid, stream);
-    case 32: return launch_kvt_n<32>(p, tm, rows_per_page, grid, stream);
+    case 16: return p.q_len > 1 ? launch_kvt_n<16, true>(p, tm, rows_per_page, grid, stream)
+                                : launch_kvt_n<16, false>(p, tm, rows_per_page, grid, stream);
+    case 32: return p.q_len > 1 ? launch_kvt_n<32, true>(p, tm, rows_per_page, grid, stream)
+                                : launch_kvt_n<32, false>(p, tm, rows_per_page, grid, stream);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -304,6 +304,7 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
         const Request &r = pool->reqs[ids[G.b]];
         const cp_model_cfg &m = pool->models[r.model];
         const int hpk = m.n_q_heads / m.n_kv_heads;
+        const int rows = hpk * pool->qlen;             // rows of the group: (query token, head), token-major
         const int ns = n_static_of[g] + n_tail_of[g];
         kp.max_splits = std::max(kp.max_splits, ns);
         Group gr;
@@ -315,19 +316,21 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
         gr.part_off = 0;
         if (ns > 1) {
             gr.part_off = (int64_t)ws;
-            ws += (uint64_t)part_group_floats(hpk, ns, m.head_dim_v);
+            ws += (uint64_t)part_group_floats(rows, ns, m.head_dim_v);
             const int zl = ns <= 8 ? 0 : (ns <= 32 ? 3 : (ns <= 128 ? 4 : 5));
             const int cols = 128 >> zl;
-            for (int h = 0; h < hpk; ++h) {
+            for (int h = 0; h < rows; ++h) {
                 kp.combines.push_back(Combine{g, h});
+                // row (t, hh) of the group is row t * Hq + hh of the request's output (q_len = 1: row h)
+                const int64_t orow = (int64_t)(h / hpk) * m.n_q_heads + h % hpk;
                 for (int c0 = 0; c0 < m.head_dim_v; c0 += cols) {
                     CombineUnit cu;
                     std::memset(&cu, 0, sizeof(cu));
                     // partial layout of this kernel: [h][c0 / cols][s][cols] (the unit's 512-byte reads are contiguous)
                     cu.part_off = gr.part_off + (int64_t)h * ns * m.head_dim_v + (int64_t)(c0 / cols) * ns * cols;
-                    cu.ml_off = gr.part_off + part_ml_off(hpk, h, 0, ns, m.head_dim_v);
-                    cu.out_off = gr.out_off + (int64_t)h * m.head_dim_v + c0;
-                    cu.lse_off = c0 == 0 ? gr.lse_off + h : -1;
+                    cu.ml_off = gr.part_off + part_ml_off(rows, h, 0, ns, m.head_dim_v);
+                    cu.out_off = gr.out_off + orow * m.head_dim_v + c0;
+                    cu.lse_off = c0 == 0 ? gr.lse_off + orow : -1;
                     cu.split_stride = cols;
                     cu.n_splits = ns;
                     cu.zl_log2 = zl;
@@ -349,7 +352,7 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
         r.group = t.g; r.req = gr.req; r.kv_head = gr.kv_head; r.n_kv_heads = m.n_kv_heads;
         r.page_begin = t.sl0 * pps; r.n_pages = std::min(t.sl1 * pps, G.n_lp) - r.page_begin;
         r.split = split; r.n_splits = gr.n_splits;
-        r.gsize = m.n_q_heads / m.n_kv_heads; r.n_q_heads = m.n_q_heads;
+        r.gsize = m.n_q_heads / m.n_kv_heads * pool->qlen; r.n_q_heads = m.n_q_heads;
         r.scale_log2 = (float)((double)m.softmax_scale * 1.4426950408889634);
         r.q_off = gr.q_off; r.out_off = gr.out_off; r.lse_off = gr.lse_off; r.part_off = gr.part_off;
         r.pad = zl_of(gr.n_splits) << 8;               // bits 8..15: partial layout; bit 0 (set below): another static slot follows
@@ -466,7 +469,7 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             kp.max_group = std::max(kp.max_group, g);
         }
         kp.use_kvt = k == CP_KIND_KV && kp.all_fast && (pool->opt_kernel == 0 || pool->opt_kernel == 2) &&
-                     pool->qlen == 1 && !pool->plan_for_stages && kvt_supported(P) && kvt_pad_rows(kp.max_group) > 0;
+                     !pool->plan_for_stages && kvt_supported(P) && kvt_pad_rows(kp.max_group) > 0;
         if (kp.use_kvt) {
             kp.tile_recs.clear();
             build_plan_kvt(pool, ids, n, kp, ws);

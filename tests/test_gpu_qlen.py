@@ -31,11 +31,12 @@ def run_qlen(torch, w, q_len, options=None, seed=0, vmm=False):
         out = torch.full((rows * 128,), float("nan"), dtype=torch.float32, device=dev)
         lse = torch.full((rows,), float("nan"), dtype=torch.float32, device=dev)
         wsb = max(dw.pool.decode_workspace_bytes_qlen(dw.ids, q_len), 256)
-        ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+        ws = torch.full((wsb,), 0xFF, dtype=torch.uint8, device=dev)     # NaN patterns: nothing may be read unwritten
         dw.pool.decode_attention_qlen(dw.ids, q_len, q, out, lse, ws, wsb, dw.stream())
         torch.cuda.synchronize()
         o, l = out.cpu().numpy(), lse.cpu().numpy()
         out.fill_(float("nan"))
+        ws.fill_(0xFF)
         dw.pool.decode_attention_qlen(dw.ids, q_len, q, out, lse, ws, wsb, dw.stream())
         torch.cuda.synchronize()
         assert np.array_equal(o, out.cpu().numpy()) and np.array_equal(l, lse.cpu().numpy()), "relaunch differs"
@@ -61,20 +62,41 @@ CASES = [
     ([MQA], [0], [3000], 128, 8),                        # 128 rows, one long request, many splits
     ([MHA, GQA, MQA], [0, 1, 2, 0], [410, 90, 1234, 5], 32, 5),
     ([GQA], [0], [2050], 32, 2),
+    # groups of at most 32 rows: the tcgen05 K/V kernel (query rows on the MMA N dimension, causal limit per row)
+    ([MHA], [0, 0, 0], [131, 258, 1000], 16, 7),         # last slice shorter than q_len - 1: the mask spans two slices
+    ([GQA], [0], [128 * 20 + 2], 32, 4),                 # a last tile of two tokens that the first two query tokens do not see
+    ([MHA, GQA], [0, 1, 0], [5000, 4099, 32], 64, 4),    # 4-row and 32-row groups in one launch
+    ([MHA], [0, 0], [32, 777], 16, 32),                  # 32 rows of one head; a context of query tokens only
+    ([GQA], [0, 0], [3, 12345], 128, 3),
 ]
 
 
 @pytest.mark.parametrize("case", range(len(CASES)))
 @pytest.mark.parametrize("n_ctas", [0, 3])
-def test_qlen_matches_oracle(torch_cuda, case, n_ctas):
+@pytest.mark.parametrize("kernel", [0, 3])
+def test_qlen_matches_oracle(torch_cuda, case, n_ctas, kernel):
+    """kernel 0: the default choice (tcgen05 K/V kernel for groups of <= 32 rows, else the warp-MMA kernel);
+    kernel 3: the warp-MMA kernel for every case."""
     import paper_2606_24506_b200 as cp
     models, rm, rc, P, q_len = CASES[case]
     w = W.small_workload(models, rm, rc, page_tokens=P, seed=500 + case, keep_contiguous=False)
-    opts = {cp.CP_OPT_MIN_TILE_PAGES: 1}
+    opts = {cp.CP_OPT_MIN_TILE_PAGES: 1, cp.CP_OPT_KERNEL: kernel}
     if n_ctas:
         opts[cp.CP_OPT_NUM_CTAS] = n_ctas
     worst = run_qlen(torch_cuda, w, q_len, opts, seed=case)
-    print("case %d ctas %d: %s" % (case, n_ctas, worst))
+    print("case %d ctas %d kernel %d: %s" % (case, n_ctas, kernel, worst))
+
+
+@pytest.mark.parametrize("case", [6, 7, 8, 10])
+def test_qlen_with_dynamic_tail_tiles(torch_cuda, case):
+    """Short tail tiles popped from the work counter: the last one may hold nothing but tokens that the first
+    query tokens do not see (a split with m = -inf, l = 0 for those rows)."""
+    import paper_2606_24506_b200 as cp
+    models, rm, rc, P, q_len = CASES[case]
+    w = W.small_workload(models, rm, rc, page_tokens=P, seed=500 + case, keep_contiguous=False)
+    opts = {cp.CP_OPT_MIN_TILE_PAGES: 1, cp.CP_OPT_STATIC_PCT: 50, cp.CP_OPT_TAIL_TILE_SLICES: 1}
+    worst = run_qlen(torch_cuda, w, q_len, opts, seed=case)
+    print("case %d tail tiles: %s" % (case, worst))
 
 
 def test_qlen_one_is_the_single_token_step(torch_cuda):
@@ -133,8 +155,9 @@ def test_qlen_on_a_vmm_arena(torch_cuda):
     print(worst)
 
 
-def test_qlen_full_size_cfg2(torch_cuda):
-    """Full size, default options (what bench.py's `qlen` leg times): BASELINE cfg2 with four query tokens
-    per request."""
-    worst = run_qlen(torch_cuda, W.config(2), 4, seed=77)
-    print("cfg2 q_len 4: %s" % worst)
+@pytest.mark.parametrize("cfg", [2, 4])
+def test_qlen_full_size(torch_cuda, cfg):
+    """Full size, default options (what bench.py's `qlen` leg times): BASELINE cfg2 / cfg4 with four query
+    tokens per request."""
+    worst = run_qlen(torch_cuda, W.config(cfg), 4, seed=77)
+    print("cfg%d q_len 4: %s" % (cfg, worst))
