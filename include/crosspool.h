@@ -89,7 +89,8 @@ enum {
                                     to 32 rows on the tcgen05 tokens-on-M kernel, MLA on CTA pairs,
                                     tcgen05 cta_group::2),
                                 1 = force the generic SIMT kernel (any supported shape),
-                                2 = as 0, but MLA on the single-CTA tcgen05 kernel,
+                                2 = as 0, but MLA on the single-CTA tcgen05 kernel, and q_len > 1 on the
+                                    tcgen05 K/V kernel for groups of up to 32 rows (0: up to 16 rows),
                                 3 = as 0, but MQA/GQA on the warp-MMA (mma.sync) kernel          */
     CP_OPT_NUM_CTAS = 1,     /* persistent grid size; 0 = number of SMs of the device       */
     CP_OPT_WAVES_X16 = 2,    /* target tiles per CTA, in 1/16 units (default 16 = 1.0)      */
@@ -319,6 +320,9 @@ cp_status cp_decode_attention_host(cp_pool *pool, const int32_t *request_ids_hos
  *   q_len    1 .. 128 with (Hq / Hkv) * q_len <= 128; q_len = 1 is cp_decode_attention
  * For q_len > 1: MQA / GQA / MHA models with d_k = d_v = 128 on page sizes 16/32/64/128 only
  * (UNSUPPORTED otherwise, and with CP_OPT_KERNEL = 1); INVALID_ARG if a context is shorter than q_len.
+ * Kernel: a batch whose groups have at most 16 rows ((Hq / Hkv) * q_len; 32 with CP_OPT_KERNEL = 2) runs
+ * on the tcgen05 K/V kernel (the rows sit on the MMA N dimension, the causal limit is applied per row in
+ * the slices that reach the context's last q_len - 1 tokens), any other on the warp-MMA kernel.
  */
 cp_status cp_decode_workspace_bytes_qlen(cp_pool *pool, const int32_t *request_ids_host,
                                          int32_t n_requests, int32_t q_len, uint64_t *bytes_out);

@@ -35,11 +35,13 @@ namespace cp {
 constexpr int M2_DK = 576, M2_DV = 512;
 constexpr int M2_TS = 32;                           // tokens per slice (16 per CTA for the score MMA)
 constexpr int M2_KB = 9;                            // 64-column blocks of the latent row
-constexpr int M2_STAGES = 5;
+constexpr int M2_STAGES = 6;                        // value ring: slices (32 tokens) in flight for the value MMAs
+constexpr int M2_SR = 2;                            // score ring: slice PAIRS (64 tokens) in flight for the score MMAs
 constexpr int M2_BLK = 16 * 128;                    // one [16 x 64] swizzled tile: 2048 bytes
-constexpr int M2_SAREA = M2_KB * M2_BLK;            // 18432
+constexpr int M2_SAREA = M2_KB * M2_BLK;            // 18432: this CTA's 16 tokens of one slice, 9 column blocks
+constexpr int M2_SPAIR = 2 * M2_SAREA;              // 36864: score region of a slice pair, [column block][slice of the pair][16 tokens]
 constexpr int M2_PVAREA = 2 * 2 * 2 * M2_BLK;       // 16384: [kk][j][2 blocks]
-constexpr int M2_STAGE_BYTES = M2_SAREA + M2_PVAREA;        // 34816
+constexpr int M2_STAGE_BYTES = M2_PVAREA;           // one stage of the value ring
 constexpr int M2_QBLK = 64 * 128;                   // one [64 x 64] K-major tile of this CTA's query rows
 constexpr int M2_KB_TMEM = 6;                       // query column blocks 0..5 live in TMEM (A operand, TS mode)
 constexpr int M2_Q_BYTES = (M2_KB - M2_KB_TMEM) * M2_QBLK;   // 24576: blocks 6..8 in shared memory
@@ -47,26 +49,30 @@ constexpr int M2_P_BYTES = 64 * M2_TS * 2;          // 4096 per P buffer (two bu
 constexpr int M2_WARPS = 8;                         // producer, MMA issuer, 4 softmax warps, 2 that only help with the combine
 constexpr int M2_THREADS = 32 * M2_WARPS;
 constexpr int M2_SMEM_Q = 0;
-constexpr int M2_SMEM_STAGE = M2_Q_BYTES;
-constexpr int M2_SMEM_P = M2_SMEM_STAGE + M2_STAGES * M2_STAGE_BYTES;
+constexpr int M2_SMEM_STAGE = M2_Q_BYTES;                    // value ring
+constexpr int M2_SMEM_SRING = M2_SMEM_STAGE + M2_STAGES * M2_STAGE_BYTES;
+constexpr int M2_SMEM_P = M2_SMEM_SRING + M2_SR * M2_SPAIR;
 constexpr int M2_SMEM_XPOSE = M2_SMEM_P + 2 * M2_P_BYTES;   // epilogue transpose scratch: 4 warps x [32 rows][16 + 4 floats]
 constexpr int M2_SMEM_MISC = M2_SMEM_XPOSE + 4 * 2560;
 constexpr int M2_SMEM_BYTES = M2_SMEM_MISC + 2048;
 static_assert(M2_SMEM_BYTES <= 232448, "MLA pair kernel exceeds the 227 KB shared-memory limit");
 constexpr uint32_t M2_TMEM_COLS = 512;
-constexpr int M2_SB = 3;                            // score buffers: the issuer runs two slices ahead of the value MMAs
-constexpr uint32_t M2_TMEM_S = 256;                         // score buffer b at 256 + 16 b: 16 columns each (2 x 2 layout)
-constexpr uint32_t M2_TMEM_Q = 304;                         // 192 columns: Q[:, 0:384) as bf16 pairs, rows duplicated in lanes 64..127
+constexpr int M2_SB = 2;                            // score buffers, one slice PAIR each: the score issuer runs one pair ahead
+constexpr uint32_t M2_TMEM_S = 256;                         // score buffer b at 256 + 32 b: 2 slices x 16 columns (2 x 2 layout)
+constexpr uint32_t M2_TMEM_Q = 320;                         // 192 columns: Q[:, 0:384) as bf16 pairs, rows duplicated in lanes 64..127
 static_assert(M2_TMEM_Q + M2_KB_TMEM * 32 <= M2_TMEM_COLS, "TMEM budget");
 static_assert((M2_KB_TMEM * 32) % 96 == 0, "query staging batches");
 constexpr float M2_LAZY_LOG2 = 8.0f;
 
 struct M2Misc {
-    uint64_t full[M2_STAGES];       // local TMA landed (this CTA's part of the slice)
+    uint64_t full[M2_STAGES];       // value ring: local TMA landed (this CTA's part of the slice)
     uint64_t full_peer[M2_STAGES];  // leader only: the peer's part landed (arrived by the peer's relay warp)
-    uint64_t empty[M2_STAGES];      // pair-MMA commit (multicast): stage free
-    uint64_t s_full[M2_SB];         // pair-MMA commit (multicast): scores ready
-    uint64_t s_empty[M2_SB];        // leader only: 8 softmax warps of the pair have read the scores
+    uint64_t empty[M2_STAGES];      // pair-MMA commit (multicast): value stage free
+    uint64_t sl_full[M2_SR];        // score ring: local TMA landed (this CTA's 16 tokens of each slice of the pair)
+    uint64_t sl_full_peer[M2_SR];   // leader only: the peer's part landed
+    uint64_t sl_empty[M2_SR];       // pair-MMA commit (multicast): score region free
+    uint64_t s_full[M2_SB];         // pair-MMA commit (multicast): scores of a slice pair ready
+    uint64_t s_empty[M2_SB];        // leader only: 8 softmax warps of the pair have read the scores of both slices
     uint64_t p_full[2];             // leader only: 8 softmax warps have written P buffer (slice & 1)
     uint64_t p_done[2];             // pair-MMA commit (multicast): value MMAs of the slice complete
     uint64_t q_full;                // leader only: 8 softmax warps have staged the query rows
@@ -118,11 +124,16 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
     const uint32_t q_base = smem_u32(smem + M2_SMEM_Q);
     const uint32_t st_base = smem_u32(smem + M2_SMEM_STAGE);
+    const uint32_t sr_base = smem_u32(smem + M2_SMEM_SRING);
     const uint32_t p_base = smem_u32(smem + M2_SMEM_P);
     if (tid == 0) {
         for (int i = 0; i < M2_STAGES; ++i) {
             mbar_init(smem_u32(&mi->full[i]), 1); mbar_init(smem_u32(&mi->full_peer[i]), 1);
             mbar_init(smem_u32(&mi->empty[i]), 1);
+        }
+        for (int i = 0; i < M2_SR; ++i) {
+            mbar_init(smem_u32(&mi->sl_full[i]), 1); mbar_init(smem_u32(&mi->sl_full_peer[i]), 1);
+            mbar_init(smem_u32(&mi->sl_empty[i]), 1);
         }
         for (int i = 0; i < M2_SB; ++i) { mbar_init(smem_u32(&mi->s_full[i]), 1); mbar_init(smem_u32(&mi->s_empty[i]), 8); }
         for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&mi->p_full[i]), 8); mbar_init(smem_u32(&mi->p_done[i]), 1); }
@@ -149,7 +160,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
         // =========================================================== producer warp (each CTA loads its part)
         uint64_t policy;
         asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(policy));
-        uint32_t gs = 0;
+        uint32_t gs = 0, gp = 0;                          // slices / slice pairs issued so far (ring positions)
         for (int k = 0;; ++k) {
             const M2Item it = m2_item(p, pair + k * n_pairs);
             if (!it.valid) break;
@@ -159,105 +170,140 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 const int ns = min(32, it.n_slices - s0);
                 for (int j = 0; j < ns; ++j) {
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);
+                    const int i = s0 + j;                                  // slice of the tile; pair i / 2, half i & 1
                     const uint32_t slot = gs % M2_STAGES;
+                    const uint32_t gq = gp + (uint32_t)(i >> 1), reg = gq % M2_SR;
+                    if ((i & 1) == 0) mbar_wait(smem_u32(&mi->sl_empty[reg]), ((gq / M2_SR) & 1) ^ 1);
                     mbar_wait(smem_u32(&mi->empty[slot]), ((gs / M2_STAGES) & 1) ^ 1);
                     if (elect_one()) {
+                        const int row0 = my * rows_per_page + (i % spp) * M2_TS;
+                        // score region of the pair: this CTA's 16 tokens of the slice, one load per column block
+                        // (block kb of half h at kb * 4096 + h * 2048: the four 8-token groups of a block are 1024 B
+                        // apart, which is what lets one N = 64 MMA take both slices)
+                        const uint32_t sb = smem_u32(&mi->sl_full[reg]);
+                        if ((i & 1) == 0) mbar_arrive_expect_tx(sb, (i + 1 < it.n_slices ? 2u : 1u) * M2_SAREA);
+                        const uint32_t sdst = sr_base + reg * M2_SPAIR + (uint32_t)(i & 1) * M2_BLK;
+#pragma unroll
+                        for (int kb = 0; kb < M2_KB; ++kb)
+                            tma_load_3d(sdst + kb * 2 * M2_BLK, &tmap9, 0, row0 + 16 * (int)rank, kb, sb, policy);
+                        // value stage: tokens 16kk.., this CTA's column blocks 4j + 2r, 4j + 2r + 1
                         const uint32_t fb = smem_u32(&mi->full[slot]);
                         mbar_arrive_expect_tx(fb, M2_STAGE_BYTES);
-                        const int row0 = my * rows_per_page + ((s0 + j) % spp) * M2_TS;
                         const uint32_t dst = st_base + slot * M2_STAGE_BYTES;
-                        // S area: this CTA's 16 tokens, all 9 column blocks
-                        tma_load_3d(dst, &tmap9, 0, row0 + 16 * (int)rank, 0, fb, policy);
-                        // PV area: tokens 16kk.., this CTA's column blocks 4j + 2r, 4j + 2r + 1
 #pragma unroll
                         for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
                             for (int jj = 0; jj < 2; ++jj)
-                                tma_load_3d(dst + M2_SAREA + (kk * 2 + jj) * 2 * M2_BLK, &tmap2, 0, row0 + 16 * kk,
+                                tma_load_3d(dst + (kk * 2 + jj) * 2 * M2_BLK, &tmap2, 0, row0 + 16 * kk,
                                             4 * jj + 2 * (int)rank, fb, policy);
                     }
                     ++gs;
                 }
             }
+            gp += (uint32_t)(it.n_slices + 1) >> 1;
         }
         // programmatic dependent launch: see cp_kernels_kvt.cu (the next kernel's set-up overlaps this one's tail;
         // said once every slice of this CTA has been requested, not at the top)
         if (lane == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     } else if (warp == 1 && rank != 0) {
         // =========================================================== peer: relay "my part of the slice landed"
-        uint32_t gs = 0;
+        uint32_t gs = 0, gp = 0;
         for (int k = 0;; ++k) {
             const M2Item it = m2_item(p, pair + k * n_pairs);
             if (!it.valid) break;
             for (int i = 0; i < it.n_slices; ++i, ++gs) {
+                if ((i & 1) == 0) {
+                    const uint32_t gq = gp + (uint32_t)(i >> 1), reg = gq % M2_SR;
+                    mbar_wait(smem_u32(&mi->sl_full[reg]), (gq / M2_SR) & 1);
+                    if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&mi->sl_full_peer[reg]), 0));
+                    __syncwarp();
+                }
                 const uint32_t slot = gs % M2_STAGES;
                 mbar_wait(smem_u32(&mi->full[slot]), (gs / M2_STAGES) & 1);
                 if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&mi->full_peer[slot]), 0));
                 __syncwarp();
             }
+            gp += (uint32_t)(it.n_slices + 1) >> 1;
         }
     } else if (warp == 1) {
-        // =========================================================== leader: pair-MMA issuer
-        constexpr uint32_t IDESC_S = umma_idesc_bf16(128, M2_TS, 0, 0);
-        constexpr uint32_t IDESC_PV = umma_idesc_bf16(128, 256, 0, 1);
-        uint32_t gs = 0, qn = 0;
+        // =========================================================== leader: issuer of the score MMAs
+        // One N = 64 MMA per k-step computes the scores of a PAIR of slices (measured: a score MMA costs ~19 cycles
+        // whether N is 32 or 64 -- it is bound by the A operand, not by the arithmetic -- so pairing halves the 36
+        // instructions per slice that used to pace the whole kernel).  Each CTA supplies 32 B rows: its 16 tokens of
+        // slice 0, then of slice 1; D columns 0..15 (per lane half) are slice 0, 16..31 slice 1.  A tile's last
+        // pair may hold one slice: the other half of the region is stale, its score columns are never read.
+        constexpr uint32_t IDESC_S = umma_idesc_bf16(128, 2 * M2_TS, 0, 0);
+        uint32_t gp = 0, qn = 0;
         int prev_group = -1;
         for (int k = 0;; ++k) {
             const M2Item it = m2_item(p, pair + k * n_pairs);
             if (!it.valid) break;
             if (it.group_idx != prev_group) { mbar_wait_cluster(smem_u32(&mi->q_full), qn & 1); ++qn; prev_group = it.group_idx; }
+            const int np = (it.n_slices + 1) >> 1;
+            for (int i = 0; i < np; ++i) {
+                const uint32_t gq = gp + (uint32_t)i, reg = gq % M2_SR, b = gq % M2_SB;
+                mbar_wait(smem_u32(&mi->sl_full[reg]), (gq / M2_SR) & 1);
+                mbar_wait_cluster(smem_u32(&mi->sl_full_peer[reg]), (gq / M2_SR) & 1);
+                mbar_wait_cluster(smem_u32(&mi->s_empty[b]), ((gq / M2_SB) & 1) ^ 1);
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint32_t c0 = sr_base + reg * M2_SPAIR;
+                    const uint32_t dcol = tmem + M2_TMEM_S + 32 * b;
+                    const uint64_t bd0 = umma_smem_desc(c0, 16, 1024, 2);
+                    const uint64_t ad0 = umma_smem_desc(q_base, 16, 1024, 2);
+#pragma unroll
+                    for (int kb = 0; kb < M2_KB; ++kb)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const uint64_t bd = bd0 + (uint64_t)((kb * 2 * M2_BLK + j * 32) >> 4);      // start-address field
+                            if (kb < M2_KB_TMEM) {
+                                umma2_bf16_ts(dcol, tmem + M2_TMEM_Q + kb * 32 + j * 8, bd, IDESC_S, (kb | j) != 0);
+                            } else {
+                                const uint64_t ad = ad0 + (uint64_t)(((kb - M2_KB_TMEM) * M2_QBLK + j * 32) >> 4);
+                                umma2_bf16_ss(dcol, ad, bd, IDESC_S, 1);
+                            }
+                        }
+                    umma2_commit(smem_u32(&mi->s_full[b]));
+                    umma2_commit(smem_u32(&mi->sl_empty[reg]));
+                }
+                __syncwarp();
+            }
+            gp += (uint32_t)np;
+        }
+    } else if (warp == 6 && rank == 0) {
+        // =========================================================== leader: issuer of the value MMAs
+        // (a warp of its own: neither issuer waits for what only the other one needs, and a commit covers the MMAs of
+        // the thread that makes it)
+        constexpr uint32_t IDESC_PV = umma_idesc_bf16(128, 256, 0, 1);
+        uint32_t gs = 0;
+        for (int k = 0;; ++k) {
+            const M2Item it = m2_item(p, pair + k * n_pairs);
+            if (!it.valid) break;
             const int n = it.n_slices;
-            for (int i = 0; i <= n + 1; ++i) {
-                if (i < n) {
-                    const uint32_t g = gs + (uint32_t)i, slot = g % M2_STAGES, b = g % M2_SB;
-                    mbar_wait(smem_u32(&mi->full[slot]), (g / M2_STAGES) & 1);
-                    mbar_wait_cluster(smem_u32(&mi->full_peer[slot]), (g / M2_STAGES) & 1);
-                    mbar_wait_cluster(smem_u32(&mi->s_empty[b]), ((g / M2_SB) & 1) ^ 1);
-                    tc_fence_after();
-                    if (elect_one()) {
-                        const uint32_t c0 = st_base + slot * M2_STAGE_BYTES;
-                        const uint32_t dcol = tmem + M2_TMEM_S + 16 * b;
-                        const uint64_t bd0 = umma_smem_desc(c0, 16, 1024, 2);
-                        const uint64_t ad0 = umma_smem_desc(q_base, 16, 1024, 2);
+            for (int i = 0; i < n; ++i) {
+                const uint32_t g = gs + (uint32_t)i, slot = g % M2_STAGES;
+                mbar_wait(smem_u32(&mi->full[slot]), (g / M2_STAGES) & 1);
+                mbar_wait_cluster(smem_u32(&mi->full_peer[slot]), (g / M2_STAGES) & 1);
+                mbar_wait_cluster(smem_u32(&mi->p_full[g & 1]), (g >> 1) & 1);
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint32_t pv = st_base + slot * M2_STAGE_BYTES;
+                    const uint64_t ad0 = umma_smem_desc(p_base + (g & 1) * M2_P_BYTES, 1024, 128, 0);
+                    const uint64_t bd0 = umma_smem_desc(pv, M2_BLK, 1024, 2);
 #pragma unroll
-                        for (int kb = 0; kb < M2_KB; ++kb)
+                    for (int kk = 0; kk < 2; ++kk)
 #pragma unroll
-                            for (int j = 0; j < 4; ++j) {
-                                const uint64_t bd = bd0 + (uint64_t)((kb * M2_BLK + j * 32) >> 4);      // start-address field
-                                if (kb < M2_KB_TMEM) {
-                                    umma2_bf16_ts(dcol, tmem + M2_TMEM_Q + kb * 32 + j * 8, bd, IDESC_S, (kb | j) != 0);
-                                } else {
-                                    const uint64_t ad = ad0 + (uint64_t)(((kb - M2_KB_TMEM) * M2_QBLK + j * 32) >> 4);
-                                    umma2_bf16_ss(dcol, ad, bd, IDESC_S, 1);
-                                }
-                            }
-                        umma2_commit(smem_u32(&mi->s_full[b]));
-                    }
-                    __syncwarp();
+                        for (int jj = 0; jj < 2; ++jj) {
+                            // P: 8-token chunks of [64 rows x 16 B] 1024 B apart, 8-row groups 128 B apart
+                            const uint64_t ad = ad0 + (uint64_t)((kk * 2048) >> 4);
+                            // V: two 64-column blocks 2048 B apart, 8-token groups 1024 B apart
+                            const uint64_t bd = bd0 + (uint64_t)(((kk * 2 + jj) * 2 * M2_BLK) >> 4);
+                            umma2_bf16_ss(tmem + jj * 128, ad, bd, IDESC_PV, (i > 0) || (kk > 0));
+                        }
+                    umma2_commit(smem_u32(&mi->empty[slot]));
+                    umma2_commit(smem_u32(&mi->p_done[g & 1]));
                 }
-                if (i >= 2) {
-                    const uint32_t g = gs + (uint32_t)i - 2, slot = g % M2_STAGES;
-                    mbar_wait_cluster(smem_u32(&mi->p_full[g & 1]), (g >> 1) & 1);
-                    tc_fence_after();
-                    if (elect_one()) {
-                        const uint32_t pv = st_base + slot * M2_STAGE_BYTES + M2_SAREA;
-                        const uint64_t ad0 = umma_smem_desc(p_base + (g & 1) * M2_P_BYTES, 1024, 128, 0);
-                        const uint64_t bd0 = umma_smem_desc(pv, M2_BLK, 1024, 2);
-#pragma unroll
-                        for (int kk = 0; kk < 2; ++kk)
-#pragma unroll
-                            for (int jj = 0; jj < 2; ++jj) {
-                                // P: 8-token chunks of [64 rows x 16 B] 1024 B apart, 8-row groups 128 B apart
-                                const uint64_t ad = ad0 + (uint64_t)((kk * 2048) >> 4);
-                                // V: two 64-column blocks 2048 B apart, 8-token groups 1024 B apart
-                                const uint64_t bd = bd0 + (uint64_t)(((kk * 2 + jj) * 2 * M2_BLK) >> 4);
-                                umma2_bf16_ss(tmem + jj * 128, ad, bd, IDESC_PV, (i > 2) || (kk > 0));
-                            }
-                        umma2_commit(smem_u32(&mi->empty[slot]));
-                        umma2_commit(smem_u32(&mi->p_done[g & 1]));
-                    }
-                    __syncwarp();
-                }
+                __syncwarp();
             }
             gs += (uint32_t)n;
         }
@@ -273,7 +319,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
         const int th = L >> 6;                            // token half: tokens 16 th .. 16 th + 15 of a slice
         const uint32_t tl = tmem + ((uint32_t)(q4 * 32) << 16);
         const int st = tid - 64;
-        uint32_t gs = 0;
+        uint32_t gs = 0, gp = 0;
         int prev_group = -1;
         for (int k = 0;; ++k) {
             const M2Item it = m2_item(p, pair + k * n_pairs);
@@ -327,15 +373,16 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             float m_run = -INFINITY, l_run = 0.f;
             const int n = it.n_slices;
             for (int i = 0; i < n; ++i) {
-                const uint32_t g = gs + (uint32_t)i, b = g % M2_SB, kq = g / M2_SB, xb = g & 1;
-                mbar_wait(smem_u32(&mi->s_full[b]), kq & 1);
+                const uint32_t g = gs + (uint32_t)i, xb = g & 1;
+                const uint32_t gq = gp + (uint32_t)(i >> 1), b = gq % M2_SB;       // the slice's pair and its score buffer
+                if ((i & 1) == 0) mbar_wait(smem_u32(&mi->s_full[b]), (gq / M2_SB) & 1);
                 tc_fence_after();
                 uint32_t sr[16];
-                tmem_ld16(tl + M2_TMEM_S + 16 * b, sr);
+                tmem_ld16(tl + M2_TMEM_S + 32 * b + 16 * (i & 1), sr);
                 tmem_wait_ld();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(L_s_empty + 8 * b);
+                if (lane == 0 && ((i & 1) || i == n - 1)) mbar_arrive_cluster(L_s_empty + 8 * b);   // both slices read
                 const int valid = ((i == n - 1) ? it.valid_last : M2_TS) - 16 * th;   // valid tokens of my half
                 float mx = -INFINITY;
 #pragma unroll
@@ -385,7 +432,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                     // (warp q4 clears the two 64-column blocks of MMA j = q4 & 1 for k-step kk = q4 >> 1)
                     const int kk = q4 >> 1, jj = q4 & 1;
                     const int vrows = min(16, max(0, it.valid_last - 16 * kk));        // valid rows of this k-step
-                    const uint32_t blk = st_base + (g % M2_STAGES) * M2_STAGE_BYTES + M2_SAREA + (kk * 2 + jj) * 2 * M2_BLK;
+                    const uint32_t blk = st_base + (g % M2_STAGES) * M2_STAGE_BYTES + (kk * 2 + jj) * 2 * M2_BLK;
                     for (int e = lane; e < (16 - vrows) * 16; e += 32) {
                         const int r = vrows + (e >> 4), ch = e & 15;
                         asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(blk + (ch >> 3) * M2_BLK + r * 128 + (((ch & 7) ^ (r & 7)) << 4)), "r"(0u) : "memory");
@@ -397,6 +444,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 if (lane == 0) mbar_arrive_cluster(L_p_full + 8 * xb);
             }
             gs += (uint32_t)n;
+            gp += (uint32_t)(n + 1) >> 1;
 
             // ---- end of tile: O rows from TMEM, publish
             {
@@ -468,7 +516,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
 }
 
 // ----------------------------------------------------------------------------- host side
-// 3-D views of the arena {64 columns, rows of 576 bf16, column blocks}: boxes of 16 tokens x 9 or 2 blocks.
+// 3-D views of the arena {64 columns, rows of 576 bf16, column blocks}: boxes of 16 tokens x 1 or 2 blocks.
 bool make_mla2_tensor_maps(void *out_map9, void *out_map2, const void *arena, uint64_t total_rows)
 {
     typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -485,7 +533,7 @@ bool make_mla2_tensor_maps(void *out_map9, void *out_map2, const void *arena, ui
     cuuint64_t strides[2] = {(cuuint64_t)M2_DK * 2, 128};
     cuuint32_t estr[3] = {1, 1, 1};
     for (int v = 0; v < 2; ++v) {
-        cuuint32_t box[3] = {64, 16, (cuuint32_t)(v == 0 ? M2_KB : 2)};
+        cuuint32_t box[3] = {64, 16, (cuuint32_t)(v == 0 ? 1 : 2)};
         CUresult r = fn(reinterpret_cast<CUtensorMap *>(v == 0 ? out_map9 : out_map2), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3,
                         const_cast<void *>(arena), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);

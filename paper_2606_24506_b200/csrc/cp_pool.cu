@@ -470,6 +470,11 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
         }
         kp.use_kvt = k == CP_KIND_KV && kp.all_fast && (pool->opt_kernel == 0 || pool->opt_kernel == 2) &&
                      !pool->plan_for_stages && kvt_supported(P) && kvt_pad_rows(kp.max_group) > 0;
+        // q_len > 1: the 32-row instantiation (three ring stages, twice the softmax work per byte) beats the warp-MMA
+        // kernel only back to back on long contexts (cfg2, q_len 4: 62.0 vs 64.3 us; after a flush 75.8 vs 71.7; cfg5,
+        // q_len 2: 135 vs 126 us), so by default only groups of up to 16 rows go to the tcgen05 kernel; CP_OPT_KERNEL = 2
+        // asks for it up to 32 rows
+        if (kp.use_kvt && pool->qlen > 1 && pool->opt_kernel == 0 && kp.max_group > 16) kp.use_kvt = false;
         if (kp.use_kvt) {
             kp.tile_recs.clear();
             build_plan_kvt(pool, ids, n, kp, ws);

@@ -73,10 +73,10 @@ CASES = [
 
 @pytest.mark.parametrize("case", range(len(CASES)))
 @pytest.mark.parametrize("n_ctas", [0, 3])
-@pytest.mark.parametrize("kernel", [0, 3])
+@pytest.mark.parametrize("kernel", [0, 2, 3])
 def test_qlen_matches_oracle(torch_cuda, case, n_ctas, kernel):
-    """kernel 0: the default choice (tcgen05 K/V kernel for groups of <= 32 rows, else the warp-MMA kernel);
-    kernel 3: the warp-MMA kernel for every case."""
+    """kernel 0: the default choice (tcgen05 K/V kernel for groups of <= 16 rows, else the warp-MMA kernel);
+    kernel 2: the tcgen05 kernel up to 32 rows; kernel 3: the warp-MMA kernel for every case."""
     import paper_2606_24506_b200 as cp
     models, rm, rc, P, q_len = CASES[case]
     w = W.small_workload(models, rm, rc, page_tokens=P, seed=500 + case, keep_contiguous=False)
@@ -94,7 +94,7 @@ def test_qlen_with_dynamic_tail_tiles(torch_cuda, case):
     import paper_2606_24506_b200 as cp
     models, rm, rc, P, q_len = CASES[case]
     w = W.small_workload(models, rm, rc, page_tokens=P, seed=500 + case, keep_contiguous=False)
-    opts = {cp.CP_OPT_MIN_TILE_PAGES: 1, cp.CP_OPT_STATIC_PCT: 50, cp.CP_OPT_TAIL_TILE_SLICES: 1}
+    opts = {cp.CP_OPT_MIN_TILE_PAGES: 1, cp.CP_OPT_STATIC_PCT: 50, cp.CP_OPT_TAIL_TILE_SLICES: 1, cp.CP_OPT_KERNEL: 2}
     worst = run_qlen(torch_cuda, w, q_len, opts, seed=case)
     print("case %d tail tiles: %s" % (case, worst))
 
