@@ -35,8 +35,9 @@ namespace cp {
 constexpr int M2_DK = 576, M2_DV = 512;
 constexpr int M2_TS = 32;                           // tokens per slice (16 per CTA for the score MMA)
 constexpr int M2_KB = 9;                            // 64-column blocks of the latent row
-constexpr int M2_STAGES = 6;                        // value ring: slices (32 tokens) in flight for the value MMAs
-constexpr int M2_SR = 2;                            // score ring: slice PAIRS (64 tokens) in flight for the score MMAs
+constexpr int M2_STAGES = 4;                        // value ring: slices (32 tokens) in flight for the value MMAs
+constexpr int M2_PF = 8;                            // L2 prefetch distance of the producer, slices
+constexpr int M2_SR = 3;                            // score ring: slice PAIRS (64 tokens) in flight for the score MMAs
 constexpr int M2_BLK = 16 * 128;                    // one [16 x 64] swizzled tile: 2048 bytes
 constexpr int M2_SAREA = M2_KB * M2_BLK;            // 18432: this CTA's 16 tokens of one slice, 9 column blocks
 constexpr int M2_SPAIR = 2 * M2_SAREA;              // 36864: score region of a slice pair, [column block][slice of the pair][16 tokens]
@@ -157,24 +158,40 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     const uint32_t L_p_full = mapa_u32(smem_u32(&mi->p_full[0]), 0), L_q_full = mapa_u32(smem_u32(&mi->q_full), 0);
 
     if (warp == 0) {
-        // =========================================================== producer warp (each CTA loads its part)
+        // =========================================================== producer warp of the score ring (each CTA loads
+        // its 16 tokens of every slice; the value ring has a producer of its own, warp 7: the two rings are filled at
+        // their own pace -- a value stage is needed a softmax later than the score region of the same slice)
         uint64_t policy;
         asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(policy));
-        uint32_t gs = 0, gp = 0;                          // slices / slice pairs issued so far (ring positions)
+        uint32_t gp = 0;                                  // slice pairs issued so far (ring position)
         for (int k = 0;; ++k) {
             const M2Item it = m2_item(p, pair + k * n_pairs);
             if (!it.valid) break;
+            int32_t pid_nx = 0;                               // page ids one batch of 32 slices ahead
+            if (lane < it.n_slices) pid_nx = page_of(p, it.req, it.page_begin + lane / spp);
             for (int s0 = 0; s0 < it.n_slices; s0 += 32) {
-                int32_t pid = 0;
-                if (s0 + lane < it.n_slices) pid = page_of(p, it.req, it.page_begin + (s0 + lane) / spp);
+                const int32_t pid = pid_nx;
+                pid_nx = 0;
+                if (s0 + 32 + lane < it.n_slices) pid_nx = page_of(p, it.req, it.page_begin + (s0 + 32 + lane) / spp);
                 const int ns = min(32, it.n_slices - s0);
                 for (int j = 0; j < ns; ++j) {
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);
                     const int i = s0 + j;                                  // slice of the tile; pair i / 2, half i & 1
-                    const uint32_t slot = gs % M2_STAGES;
+                    // The rings hold ~5 slices per CTA (every slice is staged twice: K-major for the scores, MN-major
+                    // for the values) and an HBM round trip under load is ~2 us, which bounds a slice at ~0.48 us
+                    // whatever the MMAs do.  So each CTA asks for its half of the slice M2_PF slices ahead to be
+                    // brought into L2 (the rows are contiguous: one bulk prefetch), and the TMA loads below find
+                    // their data at L2 latency.
+                    {
+                        const int t = j + M2_PF;
+                        const int32_t pg = __shfl_sync(0xffffffffu, t < 32 ? pid : pid_nx, t & 31);
+                        if (i + M2_PF < it.n_slices && lane == 0) {
+                            const int rowp = pg * rows_per_page + ((i + M2_PF) % spp) * M2_TS + 16 * (int)rank;
+                            bulk_prefetch_l2(p.arena + (size_t)rowp * (M2_DK * 2), 16 * M2_DK * 2);
+                        }
+                    }
                     const uint32_t gq = gp + (uint32_t)(i >> 1), reg = gq % M2_SR;
                     if ((i & 1) == 0) mbar_wait(smem_u32(&mi->sl_empty[reg]), ((gq / M2_SR) & 1) ^ 1);
-                    mbar_wait(smem_u32(&mi->empty[slot]), ((gs / M2_STAGES) & 1) ^ 1);
                     if (elect_one()) {
                         const int row0 = my * rows_per_page + (i % spp) * M2_TS;
                         // score region of the pair: this CTA's 16 tokens of the slice, one load per column block
@@ -186,7 +203,62 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
 #pragma unroll
                         for (int kb = 0; kb < M2_KB; ++kb)
                             tma_load_3d(sdst + kb * 2 * M2_BLK, &tmap9, 0, row0 + 16 * (int)rank, kb, sb, policy);
-                        // value stage: tokens 16kk.., this CTA's column blocks 4j + 2r, 4j + 2r + 1
+                    }
+                }
+            }
+            gp += (uint32_t)(it.n_slices + 1) >> 1;
+        }
+        // programmatic dependent launch: see cp_kernels_kvt.cu (the next kernel's set-up overlaps this one's tail;
+        // said once every slice of this CTA has been requested, not at the top)
+        if (lane == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    } else if (warp == 1 && rank != 0) {
+        // =========================================================== peer: relay "my part of the slice landed"
+        uint32_t gp = 0;
+        for (int k = 0;; ++k) {
+            const M2Item it = m2_item(p, pair + k * n_pairs);
+            if (!it.valid) break;
+            const int np = (it.n_slices + 1) >> 1;
+            for (int i = 0; i < np; ++i) {
+                const uint32_t gq = gp + (uint32_t)i, reg = gq % M2_SR;
+                mbar_wait(smem_u32(&mi->sl_full[reg]), (gq / M2_SR) & 1);
+                if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&mi->sl_full_peer[reg]), 0));
+                __syncwarp();
+            }
+            gp += (uint32_t)np;
+        }
+    } else if (warp == 6 && rank != 0) {
+        // =========================================================== peer: relay "my part of the value stage landed"
+        uint32_t gs = 0;
+        for (int k = 0;; ++k) {
+            const M2Item it = m2_item(p, pair + k * n_pairs);
+            if (!it.valid) break;
+            for (int i = 0; i < it.n_slices; ++i, ++gs) {
+                const uint32_t slot = gs % M2_STAGES;
+                mbar_wait(smem_u32(&mi->full[slot]), (gs / M2_STAGES) & 1);
+                if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&mi->full_peer[slot]), 0));
+                __syncwarp();
+            }
+        }
+    } else if (warp == 7) {
+        // =========================================================== producer warp of the value ring
+        uint64_t policy;
+        asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(policy));
+        uint32_t gs = 0;
+        for (int k = 0;; ++k) {
+            const M2Item it = m2_item(p, pair + k * n_pairs);
+            if (!it.valid) break;
+            for (int s0 = 0; s0 < it.n_slices; s0 += 32) {
+                int32_t pid = 0;
+                if (s0 + lane < it.n_slices) pid = page_of(p, it.req, it.page_begin + (s0 + lane) / spp);
+                const int ns = min(32, it.n_slices - s0);
+                for (int j = 0; j < ns; ++j, ++gs) {
+                    const int32_t my = __shfl_sync(0xffffffffu, pid, j);
+                    const int i = s0 + j;
+                    const uint32_t slot = gs % M2_STAGES;
+                    mbar_wait(smem_u32(&mi->empty[slot]), ((gs / M2_STAGES) & 1) ^ 1);
+                    if (elect_one()) {
+                        const int row0 = my * rows_per_page + (i % spp) * M2_TS;
+                        // tokens 16kk.., this CTA's column blocks 4j + 2r, 4j + 2r + 1
                         const uint32_t fb = smem_u32(&mi->full[slot]);
                         mbar_arrive_expect_tx(fb, M2_STAGE_BYTES);
                         const uint32_t dst = st_base + slot * M2_STAGE_BYTES;
@@ -197,33 +269,8 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                                 tma_load_3d(dst + (kk * 2 + jj) * 2 * M2_BLK, &tmap2, 0, row0 + 16 * kk,
                                             4 * jj + 2 * (int)rank, fb, policy);
                     }
-                    ++gs;
                 }
             }
-            gp += (uint32_t)(it.n_slices + 1) >> 1;
-        }
-        // programmatic dependent launch: see cp_kernels_kvt.cu (the next kernel's set-up overlaps this one's tail;
-        // said once every slice of this CTA has been requested, not at the top)
-        if (lane == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    } else if (warp == 1 && rank != 0) {
-        // =========================================================== peer: relay "my part of the slice landed"
-        uint32_t gs = 0, gp = 0;
-        for (int k = 0;; ++k) {
-            const M2Item it = m2_item(p, pair + k * n_pairs);
-            if (!it.valid) break;
-            for (int i = 0; i < it.n_slices; ++i, ++gs) {
-                if ((i & 1) == 0) {
-                    const uint32_t gq = gp + (uint32_t)(i >> 1), reg = gq % M2_SR;
-                    mbar_wait(smem_u32(&mi->sl_full[reg]), (gq / M2_SR) & 1);
-                    if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&mi->sl_full_peer[reg]), 0));
-                    __syncwarp();
-                }
-                const uint32_t slot = gs % M2_STAGES;
-                mbar_wait(smem_u32(&mi->full[slot]), (gs / M2_STAGES) & 1);
-                if (lane == 0) mbar_arrive_cluster(mapa_u32(smem_u32(&mi->full_peer[slot]), 0));
-                __syncwarp();
-            }
-            gp += (uint32_t)(it.n_slices + 1) >> 1;
         }
     } else if (warp == 1) {
         // =========================================================== leader: issuer of the score MMAs
@@ -307,8 +354,6 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
             }
             gs += (uint32_t)n;
         }
-    } else if (warp >= 6) {
-        // ======================================================= combine helpers: nothing to do until the combine
     } else {
         // =========================================================== softmax warps
         // thread = TMEM lane L: head (rank * 64 + L % 64), token half L / 64 of every slice

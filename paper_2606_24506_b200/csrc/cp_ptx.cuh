@@ -50,6 +50,12 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map
                  ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(policy)
                  : "memory");
 }
+// bulk prefetch of [p, p + bytes) into L2 (bytes a multiple of 16, p 16-byte aligned): no shared memory, no barrier
+__device__ __forceinline__ void bulk_prefetch_l2(const void *p, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 __device__ __forceinline__ void prefetch_l2(const void *p)     // also fills the address translation of p's page
 {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p) : "memory");
