@@ -36,7 +36,7 @@ constexpr int M2_DK = 576, M2_DV = 512;
 constexpr int M2_TS = 32;                           // tokens per slice (16 per CTA for the score MMA)
 constexpr int M2_KB = 9;                            // 64-column blocks of the latent row
 constexpr int M2_STAGES = 4;                        // value ring: slices (32 tokens) in flight for the value MMAs
-constexpr int M2_PF = 8;                            // L2 prefetch distance of the producer, slices
+constexpr int M2_PF = 4;                            // L2 prefetch distance of the score producer, slice pairs
 constexpr int M2_SR = 3;                            // score ring: slice PAIRS (64 tokens) in flight for the score MMAs
 constexpr int M2_BLK = 16 * 128;                    // one [16 x 64] swizzled tile: 2048 bytes
 constexpr int M2_SAREA = M2_KB * M2_BLK;            // 18432: this CTA's 16 tokens of one slice, 9 column blocks
@@ -164,49 +164,50 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
         uint64_t policy;
         asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(policy));
         uint32_t gp = 0;                                  // slice pairs issued so far (ring position)
+        const int ppp = P / (2 * M2_TS);                  // slice pairs per page (pages hold 64 k tokens: a pair never straddles)
         for (int k = 0;; ++k) {
             const M2Item it = m2_item(p, pair + k * n_pairs);
             if (!it.valid) break;
-            int32_t pid_nx = 0;                               // page ids one batch of 32 slices ahead
-            if (lane < it.n_slices) pid_nx = page_of(p, it.req, it.page_begin + lane / spp);
-            for (int s0 = 0; s0 < it.n_slices; s0 += 32) {
+            const int np = (it.n_slices + 1) >> 1;
+            int32_t pid_nx = 0;                               // page ids one batch of 32 pairs ahead
+            if (lane < np) pid_nx = page_of(p, it.req, it.page_begin + lane / ppp);
+            for (int q0 = 0; q0 < np; q0 += 32) {
                 const int32_t pid = pid_nx;
                 pid_nx = 0;
-                if (s0 + 32 + lane < it.n_slices) pid_nx = page_of(p, it.req, it.page_begin + (s0 + 32 + lane) / spp);
-                const int ns = min(32, it.n_slices - s0);
-                for (int j = 0; j < ns; ++j) {
+                if (q0 + 32 + lane < np) pid_nx = page_of(p, it.req, it.page_begin + (q0 + 32 + lane) / ppp);
+                const int nq = min(32, np - q0);
+                for (int j = 0; j < nq; ++j) {
                     const int32_t my = __shfl_sync(0xffffffffu, pid, j);
-                    const int i = s0 + j;                                  // slice of the tile; pair i / 2, half i & 1
+                    const int i = q0 + j;                                  // pair of the tile
                     // The rings hold ~5 slices per CTA (every slice is staged twice: K-major for the scores, MN-major
                     // for the values) and an HBM round trip under load is ~2 us, which bounds a slice at ~0.48 us
-                    // whatever the MMAs do.  So each CTA asks for its half of the slice M2_PF slices ahead to be
-                    // brought into L2 (the rows are contiguous: one bulk prefetch), and the TMA loads below find
-                    // their data at L2 latency.
+                    // whatever the MMAs do.  So each CTA asks for its half of the tokens M2_PF pairs ahead to be
+                    // brought into L2 (the rows are contiguous: one bulk prefetch per slice), and the TMA loads of both
+                    // rings find their data at L2 latency.
                     {
                         const int t = j + M2_PF;
                         const int32_t pg = __shfl_sync(0xffffffffu, t < 32 ? pid : pid_nx, t & 31);
-                        if (i + M2_PF < it.n_slices && lane == 0) {
-                            const int rowp = pg * rows_per_page + ((i + M2_PF) % spp) * M2_TS + 16 * (int)rank;
+                        if (i + M2_PF < np && lane < 2) {
+                            const int rowp = pg * rows_per_page + ((i + M2_PF) % ppp) * 2 * M2_TS + lane * M2_TS + 16 * (int)rank;
                             bulk_prefetch_l2(p.arena + (size_t)rowp * (M2_DK * 2), 16 * M2_DK * 2);
                         }
                     }
-                    const uint32_t gq = gp + (uint32_t)(i >> 1), reg = gq % M2_SR;
-                    if ((i & 1) == 0) mbar_wait(smem_u32(&mi->sl_empty[reg]), ((gq / M2_SR) & 1) ^ 1);
+                    const uint32_t gq = gp + (uint32_t)i, reg = gq % M2_SR;
+                    mbar_wait(smem_u32(&mi->sl_empty[reg]), ((gq / M2_SR) & 1) ^ 1);
                     if (elect_one()) {
-                        const int row0 = my * rows_per_page + (i % spp) * M2_TS;
-                        // score region of the pair: this CTA's 16 tokens of the slice, one load per column block
-                        // (block kb of half h at kb * 4096 + h * 2048: the four 8-token groups of a block are 1024 B
-                        // apart, which is what lets one N = 64 MMA take both slices)
+                        // score region of the pair: this CTA's 16 tokens of each of the two slices, all 9 column blocks,
+                        // with ONE 4-D box {64 columns, 16 tokens, 2 slices, 9 blocks}: block kb of slice h lands at
+                        // kb * 4096 + h * 2048, i.e. the four 8-token groups of a block are 1024 B apart, which is what
+                        // lets one N = 64 MMA take both slices.  (A tile's last pair may hold one slice: the second half
+                        // of the page is loaded anyway and never looked at.)
+                        const int row0 = my * rows_per_page + (i % ppp) * 2 * M2_TS;
                         const uint32_t sb = smem_u32(&mi->sl_full[reg]);
-                        if ((i & 1) == 0) mbar_arrive_expect_tx(sb, (i + 1 < it.n_slices ? 2u : 1u) * M2_SAREA);
-                        const uint32_t sdst = sr_base + reg * M2_SPAIR + (uint32_t)(i & 1) * M2_BLK;
-#pragma unroll
-                        for (int kb = 0; kb < M2_KB; ++kb)
-                            tma_load_3d(sdst + kb * 2 * M2_BLK, &tmap9, 0, row0 + 16 * (int)rank, kb, sb, policy);
+                        mbar_arrive_expect_tx(sb, M2_SPAIR);
+                        tma_load_4d(sr_base + reg * M2_SPAIR, &tmap9, 0, row0 + 16 * (int)rank, 0, 0, sb, policy);
                     }
                 }
             }
-            gp += (uint32_t)(it.n_slices + 1) >> 1;
+            gp += (uint32_t)np;
         }
         // programmatic dependent launch: see cp_kernels_kvt.cu (the next kernel's set-up overlaps this one's tail;
         // said once every slice of this CTA has been requested, not at the top)
@@ -561,7 +562,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
 }
 
 // ----------------------------------------------------------------------------- host side
-// 3-D views of the arena {64 columns, rows of 576 bf16, column blocks}: boxes of 16 tokens x 1 or 2 blocks.
+// Views of the arena as 64-column blocks of rows of 576 bf16.
 bool make_mla2_tensor_maps(void *out_map9, void *out_map2, const void *arena, uint64_t total_rows)
 {
     typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -574,12 +575,25 @@ bool make_mla2_tensor_maps(void *out_map9, void *out_map2, const void *arena, ui
         qres != cudaDriverEntryPointSuccess)
         return false;
     EncodeTiledFn fn = reinterpret_cast<EncodeTiledFn>(ptr);
-    cuuint64_t dims[3] = {64, total_rows, (cuuint64_t)M2_KB};
-    cuuint64_t strides[2] = {(cuuint64_t)M2_DK * 2, 128};
-    cuuint32_t estr[3] = {1, 1, 1};
-    for (int v = 0; v < 2; ++v) {
-        cuuint32_t box[3] = {64, 16, (cuuint32_t)(v == 0 ? 1 : 2)};
-        CUresult r = fn(reinterpret_cast<CUtensorMap *>(v == 0 ? out_map9 : out_map2), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3,
+    {
+        // value operand: {64 columns, rows of 576 bf16, column blocks}, boxes of 16 tokens x 2 blocks
+        cuuint64_t dims[3] = {64, total_rows, (cuuint64_t)M2_KB};
+        cuuint64_t strides[2] = {(cuuint64_t)M2_DK * 2, 128};
+        cuuint32_t estr[3] = {1, 1, 1};
+        cuuint32_t box[3] = {64, 16, 2};
+        CUresult r = fn(reinterpret_cast<CUtensorMap *>(out_map2), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3,
+                        const_cast<void *>(arena), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return false;
+    }
+    {
+        // score operand: {64 columns, rows, slice of a pair (32 rows further), column blocks}, one box of
+        // 16 tokens x 2 slices x 9 blocks per slice pair and CTA
+        cuuint64_t dims[4] = {64, total_rows, 2, (cuuint64_t)M2_KB};
+        cuuint64_t strides[3] = {(cuuint64_t)M2_DK * 2, (cuuint64_t)M2_TS * M2_DK * 2, 128};
+        cuuint32_t estr[4] = {1, 1, 1, 1};
+        cuuint32_t box[4] = {64, 16, 2, (cuuint32_t)M2_KB};
+        CUresult r = fn(reinterpret_cast<CUtensorMap *>(out_map9), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4,
                         const_cast<void *>(arena), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return false;

@@ -676,7 +676,8 @@ cp_status ensure_device(cp_pool *pool)
     if (mla_fast_supported((int)pool->P, pool->page_bytes)) {
         const uint64_t rows = (uint64_t)pool->num_pages * (pool->page_bytes / 1152);
         pool->mla_tmap_ok = rows < (1ull << 31) && make_mla_tensor_map(pool->mla_tmap, pool->arena, rows);
-        pool->mla2_tmap_ok = rows < (1ull << 31) &&
+        // (the pair kernel loads the score operand of a slice PAIR, 64 tokens, with one box: pages of 64 k tokens)
+        pool->mla2_tmap_ok = rows < (1ull << 31) && pool->P % 64 == 0 &&
                              make_mla2_tensor_maps(pool->mla2_tmap9, pool->mla2_tmap2, pool->arena, rows);
     }
     pool->n_sm = sms;
