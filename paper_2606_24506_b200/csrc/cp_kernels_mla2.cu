@@ -112,6 +112,70 @@ __device__ __forceinline__ M2Item m2_item(const DecodeParams &p, int tile_idx)
     return it;
 }
 
+// LSE combine of this kernel (step a4).  The plan's units are 128 value columns of one (group, head) each (zl = 0: a
+// lane owns a float4 column and walks the splits in order), four per head; a warp takes TWO neighbouring units at once
+// -- they share the head's (m, l) pairs and weights -- so that the 4 x 128 heads x 2 pairs of cfg3 are one round over
+// the grid's warps instead of two (measured: a round is ~5 us of dependent L2 round trips at the very end of the
+// kernel).  Same arithmetic and summation order as combine_units().
+static __device__ __noinline__ void m2_combine(const DecodeParams &p, int w, const int stride, float *wsm, const int lane)
+{
+    const int n = p.n_combine_units >> 1;
+    int done_group = -1;
+    for (; w < n; w += stride) {
+        const CombineUnit cu = load_combine_unit<false>(p.cunits, 2 * w);
+        const int ns = cu.n_splits;
+        if (cu.group != done_group) {
+            if (lane == 0) wait_group(p.group_counters, cu.group, cu.want);
+            __syncwarp();
+            done_group = cu.group;
+        }
+        const float2 *mlp = reinterpret_cast<const float2 *>(p.workspace + cu.ml_off);
+        const float *src = p.workspace + cu.part_off + lane * 4;
+        const int ss = cu.split_stride;
+        // the first value rows travel with the (m, l) pairs
+        float4 va[4], vb[4];
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            va[s] = vb[s] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (s < ns) { va[s] = ld_cg_f4(src + s * ss); vb[s] = ld_cg_f4(src + s * ss + 128); }
+        }
+        float M = -INFINITY, L = 0.f;
+#pragma unroll 8
+        for (int s = lane; s < ns; s += 32) M = fmaxf(M, __ldcg(mlp + s).x);
+        for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+#pragma unroll 8
+        for (int s = lane; s < ns; s += 32) {
+            const float2 ml = __ldcg(mlp + s);
+            const float wgt = ex2_ftz(ml.x - M);
+            wsm[s] = wgt;
+            L += wgt * ml.y;
+        }
+        for (int o = 16; o > 0; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
+        __syncwarp();
+        float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+#pragma unroll
+        for (int s = 0; s < 4; ++s)
+            if (s < ns) {
+                const float wgt = wsm[s];
+                a.x += wgt * va[s].x; a.y += wgt * va[s].y; a.z += wgt * va[s].z; a.w += wgt * va[s].w;
+                b.x += wgt * vb[s].x; b.y += wgt * vb[s].y; b.z += wgt * vb[s].z; b.w += wgt * vb[s].w;
+            }
+#pragma unroll 16
+        for (int s = 4; s < ns; ++s) {
+            const float4 x = ld_cg_f4(src + s * ss), y = ld_cg_f4(src + s * ss + 128);
+            const float wgt = wsm[s];
+            a.x += wgt * x.x; a.y += wgt * x.y; a.z += wgt * x.z; a.w += wgt * x.w;
+            b.x += wgt * y.x; b.y += wgt * y.y; b.z += wgt * y.z; b.w += wgt * y.w;
+        }
+        const float invL = 1.0f / L;
+        float *dst = p.out + cu.out_off + lane * 4;
+        *reinterpret_cast<float4 *>(dst) = make_float4(a.x * invL, a.y * invL, a.z * invL, a.w * invL);
+        *reinterpret_cast<float4 *>(dst + 128) = make_float4(b.x * invL, b.y * invL, b.z * invL, b.w * invL);
+        if (cu.lse_off >= 0 && lane == 0) p.lse[cu.lse_off] = (M + log2f(L)) * 0.6931471805599453f;
+        __syncwarp();                                          // wsm is rewritten by the next unit pair
+    }
+}
+
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(M2_THREADS, 1)
 cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap tmap9,
                       const __grid_constant__ CUtensorMap tmap2, int rows_per_page)
@@ -554,7 +618,7 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
     __syncthreads();
     {
         float *wsm = reinterpret_cast<float *>(smem + M2_SMEM_STAGE) + warp * kMaxSplits;
-        combine_units<16>(p, blockIdx.x * M2_WARPS + warp, gridDim.x * M2_WARPS, wsm, lane);
+        m2_combine(p, blockIdx.x * M2_WARPS + warp, gridDim.x * M2_WARPS, wsm, lane);
     }
     tc_fence_before();
     cluster_sync_all();

@@ -531,8 +531,8 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
                     // warp-sized units: split lanes ZL so that a lane holds <= 16 splits (8 for ZL = 1, 8)
                     // wide value rows (MLA, 512 columns): a unit costs a few L2 round trips whatever its
                     // width, so keep units few and wide (zl = 0: one float4 column per lane, 128 columns)
-                    const int zl = (m.head_dim_v > 128 && ns <= 64) ? 0
-                                   : (ns <= 8 ? 0 : (ns <= 32 ? 3 : (ns <= 128 ? 4 : 5)));
+                    // (the MLA pair kernel's own combine relies on zl = 0 for 512-column rows)
+                    const int zl = m.head_dim_v > 128 ? 0 : (ns <= 8 ? 0 : (ns <= 32 ? 3 : (ns <= 128 ? 4 : 5)));
                     const int cols = 128 >> zl;
                     const int mt = (g + 15) / 16;
                     int mtp = 1;
