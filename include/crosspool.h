@@ -57,7 +57,8 @@ enum {
     CP_ERR_UNKNOWN_REQUEST = -5,  /* request id not mapped                                  */
     CP_ERR_UNSUPPORTED = -6,      /* model shape outside what the kernels implement         */
     CP_ERR_WORKSPACE = -7,        /* workspace_dev too small or misaligned                  */
-    CP_ERR_CUDA = -8              /* CUDA runtime / driver error (no device, launch fault)  */
+    CP_ERR_CUDA = -8,             /* CUDA runtime / driver error (no device, launch fault)  */
+    CP_ERR_TOO_LARGE = -9         /* problem exceeds the fixed capacity of a *_noalloc entry point */
 };
 
 enum { CP_KIND_KV = 0, CP_KIND_MLA = 1 };
@@ -504,6 +505,27 @@ cp_status cp_planner_pool_demand(int32_t n_models, const int64_t *trace_offsets_
 cp_status cp_planner_quantile(const double *values_dev, int64_t n, double q, double page_bytes,
                               void *workspace_dev, uint64_t workspace_bytes,
                               double *quantile_out_host, uint64_t *pages_out_host, void *stream);
+
+/*
+ * cp_planner_pool_demand_noalloc -- cp_planner_pool_demand for callers that cannot allocate device memory
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): same
+ * arguments without the workspace, same launches, same results bit for bit.  The scratch lives in a
+ * file-scope device array of the library (about 0.5 MiB, held by every GPU that loads the library until
+ * the process exits), sized for traces of up to CP_PLANNER_NOALLOC_MAX_TRACE entries in all
+ * (trace_offsets_host[n_models]); a longer trace is rejected with CP_ERR_TOO_LARGE before any CUDA call.
+ * The call itself makes no cudaMalloc / cudaFree and calls no allocating library routine (one
+ * cudaGetSymbolAddress per device on first use, one cudaMemsetAsync, three kernel launches).
+ * ALL calls of a device share the one array, which keeps the last call's contents (each call clears or
+ * overwrites everything it reads): calls that may overlap on the GPU -- different streams without an
+ * ordering between them -- race on it and must use cp_planner_pool_demand with workspaces of their own.
+ * Other errors: as cp_planner_pool_demand (INVALID_ARG, CUDA).
+ */
+#define CP_PLANNER_NOALLOC_MAX_TRACE (1 << 20)
+cp_status cp_planner_pool_demand_noalloc(int32_t n_models, const int64_t *trace_offsets_host,
+                                         const double *kappa_host, const double *arrival_dev,
+                                         const double *prompt_tokens_dev, const double *output_tokens_dev,
+                                         const double *residence_dev, int64_t n_obs, const double *t_obs_dev,
+                                         double *k_pool_dev, void *stream);
 
 /* cp_status_string -- static, never NULL. */
 const char *cp_status_string(cp_status status);

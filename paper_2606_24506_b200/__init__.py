@@ -26,6 +26,8 @@ CP_ERR_UNKNOWN_REQUEST = -5
 CP_ERR_UNSUPPORTED = -6
 CP_ERR_WORKSPACE = -7
 CP_ERR_CUDA = -8
+CP_ERR_TOO_LARGE = -9
+PLANNER_NOALLOC_MAX_TRACE = 1 << 20          # CP_PLANNER_NOALLOC_MAX_TRACE
 
 CP_KIND_KV = 0
 CP_KIND_MLA = 1
@@ -118,6 +120,8 @@ def load_library():
         "cp_planner_workspace_bytes": (u64, [ctypes.c_int64]),
         "cp_planner_pool_demand": (i32, [i32, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_double),
                                          vp, vp, vp, vp, ctypes.c_int64, vp, vp, vp, u64, vp]),
+        "cp_planner_pool_demand_noalloc": (i32, [i32, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_double),
+                                                 vp, vp, vp, vp, ctypes.c_int64, vp, vp, vp]),
         "cp_planner_quantile": (i32, [vp, ctypes.c_int64, ctypes.c_double, ctypes.c_double, vp, u64,
                                       ctypes.POINTER(ctypes.c_double), u64p, vp]),
     }
@@ -138,7 +142,8 @@ EXPORTED = ["cp_pool_create", "cp_pool_create_vmm", "cp_pool_vmm_info", "cp_pool
             "cp_decode_stages_gate_status", "cp_decode_plan", "cp_pool_counters", "cp_pool_read_timeline", "cp_status_string",
             "cp_probe_globaltimer", "cp_probe_read_stream", "cp_queue_create", "cp_queue_launch", "cp_queue_push",
             "cp_queue_close", "cp_queue_status", "cp_queue_free", "cp_decode_step_workspace_bytes", "cp_decode_step",
-            "cp_planner_workspace_bytes", "cp_planner_pool_demand", "cp_planner_quantile"]
+            "cp_planner_workspace_bytes", "cp_planner_pool_demand", "cp_planner_quantile",
+            "cp_planner_pool_demand_noalloc"]
 
 
 def status_string(status: int) -> str:
@@ -452,6 +457,21 @@ def planner_pool_demand(trace_offsets, kappa, arrival_dev, prompt_tokens_dev, ou
         kap.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), _ptr(arrival_dev), _ptr(prompt_tokens_dev),
         _ptr(output_tokens_dev), _ptr(residence_dev), n_obs, _ptr(t_obs_dev), _ptr(k_pool_dev),
         _ptr(workspace_dev), workspace_bytes, stream), "cp_planner_pool_demand")
+
+
+def planner_pool_demand_noalloc(trace_offsets, kappa, arrival_dev, prompt_tokens_dev, output_tokens_dev, residence_dev,
+                                n_obs: int, t_obs_dev, k_pool_dev, stream: int = 0):
+    """cp_planner_pool_demand_noalloc: the same without a workspace (scratch in a static device array of the
+    library; traces of up to PLANNER_NOALLOC_MAX_TRACE entries; calls that overlap on the GPU race on it)."""
+    offs = np.ascontiguousarray(trace_offsets, dtype=np.int64)
+    kap = np.ascontiguousarray(kappa, dtype=np.float64)
+    if offs.size != kap.size + 1:
+        raise ValueError("trace_offsets must have n_models + 1 entries")
+    _check(load_library().cp_planner_pool_demand_noalloc(
+        kap.size, offs.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)),
+        kap.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), _ptr(arrival_dev), _ptr(prompt_tokens_dev),
+        _ptr(output_tokens_dev), _ptr(residence_dev), n_obs, _ptr(t_obs_dev), _ptr(k_pool_dev), stream),
+        "cp_planner_pool_demand_noalloc")
 
 
 def planner_quantile(values_dev, n: int, q: float, page_bytes: float, workspace_dev, workspace_bytes: int,

@@ -268,6 +268,41 @@ cp_status cp_planner_pool_demand(int32_t n_models, const int64_t *trace_offsets_
     return CP_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// cp_planner_pool_demand_noalloc: the same launches as cp_planner_pool_demand, with the scratch (the models' and the
+// 32-entry blocks' longest residence times) in a file-scope device array instead of a caller-owned workspace, for
+// callers that cannot call cudaMalloc (CUDA graph capture, serving loops, harnesses that forbid it).  Every GPU that
+// loads the library holds the array until the process exits.  In HOST code `g_planner_scratch` is a host-side
+// stand-in, not a device address: the address the kernels get comes from cudaGetSymbolAddress, asked once per
+// device with that device current.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int64_t kNoallocMaxTrace = CP_PLANNER_NOALLOC_MAX_TRACE;
+constexpr size_t kNoallocScratchBytes = (kOffBlocks + 8 * (size_t)((kNoallocMaxTrace + kBlock - 1) / kBlock) + 16 + 255) / 256 * 256;
+static __device__ __align__(256) unsigned char g_planner_scratch[kNoallocScratchBytes];
+
+cp_status cp_planner_pool_demand_noalloc(int32_t n_models, const int64_t *trace_offsets_host, const double *kappa_host,
+                                         const double *arrival_dev, const double *prompt_tokens_dev,
+                                         const double *output_tokens_dev, const double *residence_dev, int64_t n_obs,
+                                         const double *t_obs_dev, double *k_pool_dev, void *stream)
+{
+    // sizes first: no CUDA call for a request this entry point cannot serve
+    if (n_models < 1 || n_models > kMaxModels || !trace_offsets_host) return CP_ERR_INVALID_ARG;
+    if (trace_offsets_host[n_models] > kNoallocMaxTrace) return CP_ERR_TOO_LARGE;
+    static void *scratch_of[64] = {};                     // per device: the array's address on that device
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+    void *ptr = dev >= 0 && dev < 64 ? scratch_of[dev] : nullptr;
+    if (!ptr) {
+        if (cudaGetSymbolAddress(&ptr, g_planner_scratch) != cudaSuccess || !ptr) { cudaGetLastError(); return CP_ERR_CUDA; }
+        if (dev >= 0 && dev < 64) scratch_of[dev] = ptr;
+    }
+    // (cp_planner_pool_demand clears what must start at zero -- the per-model maxima -- on the stream and writes every
+    // block maximum it reads; it allocates nothing: a memset and three kernel launches)
+    return cp_planner_pool_demand(n_models, trace_offsets_host, kappa_host, arrival_dev, prompt_tokens_dev,
+                                  output_tokens_dev, residence_dev, n_obs, t_obs_dev, k_pool_dev, ptr,
+                                  (uint64_t)kNoallocScratchBytes, stream);
+}
+
 cp_status cp_planner_quantile(const double *values_dev, int64_t n, double q, double page_bytes, void *workspace_dev,
                               uint64_t workspace_bytes, double *quantile_out_host, uint64_t *pages_out_host,
                               void *stream)

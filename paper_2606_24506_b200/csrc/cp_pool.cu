@@ -809,6 +809,7 @@ const char *cp_status_string(cp_status s)
     case CP_ERR_UNSUPPORTED: return "CP_ERR_UNSUPPORTED";
     case CP_ERR_WORKSPACE: return "CP_ERR_WORKSPACE";
     case CP_ERR_CUDA: return "CP_ERR_CUDA";
+    case CP_ERR_TOO_LARGE: return "CP_ERR_TOO_LARGE";
     default: return "CP_ERR_?";
     }
 }
