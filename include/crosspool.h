@@ -405,11 +405,12 @@ cp_status cp_pool_counters(const cp_pool *pool, uint64_t *kernel_launches,
 
 /* cp_pool_read_timeline -- measurement aid (`bench.py --probe timeline`): with CP_OPT_TIMELINE = 1
  * the persistent CTAs of the MQA/GQA tcgen05 kernel stamp %globaltimer (ns) at fixed points of their life:
- *   slot 0 kernel entry, 2 first slice landed, 3 producer issued its last page, 4 softmax of a tile's last slice
- *   done, 5 tile published, 6 arrival at the barrier before the LSE combine, 7 combine done, 8 %smid (not a time),
- *   9 first TMA issued, 10 last slice landed, 11 tiles this CTA ran (a count), 12 the combine's counters complete,
- *   13 the combine's partials loaded; others unused (0 = not stamped).  A stamp taken right after a CTA barrier shows
- *   the thread's arrival, not the release.
+ *   slot 0 kernel entry, 1 the producer warp has its first tile, 2 first slice landed, 3 producer issued its last
+ *   page, 4 softmax of a tile's last slice done, 5 tile published, 6 arrival at the barrier before the LSE combine,
+ *   7 combine done, 8 %smid (not a time), 9 first TMA issued, 10 last slice landed, 11 tiles this CTA ran (a count),
+ *   12 the combine's counters complete, 13 the combine's partials loaded, 14 set-up barrier and griddepcontrol.wait
+ *   passed, 15 the scheduler warp has its first tile record (0 = not stamped).  A stamp taken right after a CTA
+ *   barrier shows the thread's arrival, not the release.
  * Synchronises the device and copies the stamps of the last launch of the pool: stamps_out_host holds
  * cap_ctas x 16 uint64; n_ctas_out receives the number of CTA rows available (the SM count). */
 cp_status cp_pool_read_timeline(cp_pool *pool, uint64_t *stamps_out_host, int32_t cap_ctas, int32_t *n_ctas_out);
