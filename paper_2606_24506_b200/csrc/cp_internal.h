@@ -73,7 +73,9 @@ struct TileRec {
                                    // holds its group's LAST planned page (where a fused append writes); bits 8..15: zl
                                    // of the group's partial layout; other kernels: see their planner
     int64_t q_off, out_off, lse_off, part_off;
-    int64_t app_k_off, app_v_off;  // element offsets of this group's new K / V row in the packed k_new / v_new of cp_decode_step
+    int32_t app_k_off, app_v_off;  // element offsets of this group's new K / V row in the packed k_new / v_new of cp_decode_step
+    int32_t next;                  // tcgen05 K/V kernel: index of the next record of this CTA's static list (valid with pad bit 0)
+    int32_t pad2;
     int32_t first_pid[8];          // tcgen05 K/V kernel: physical ids of the tile's first pages (one 128-token slice: 128 / P <= 8),
                                    // so that the first TMA loads need no page-table round trip (ids of mapped pages never change)
 };
@@ -218,7 +220,7 @@ struct DecodeParams {
     const CombineUnit *cunits;     // [n_combine_units] (tensor-core kernels)
     int32_t n_tiles;
     int32_t n_static_slots;        // tcgen05 K/V kernel: records [0, n_static_slots) are the CTAs' static lists (slot j of CTA b
-                                   // at j * gridDim.x + b, TileRec::pad bit 0 = another slot follows), the rest is popped
+                                   // at index b < gridDim.x, TileRec::pad bit 0 = another one follows at TileRec::next), the rest is popped
     int32_t n_combines;            // work items after the tiles (CTA-sized combine items)
     int32_t n_combine_units;       // tensor-core kernels: warp-sized combine units; else = n_combines
     int32_t n_groups;

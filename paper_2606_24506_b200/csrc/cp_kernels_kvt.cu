@@ -471,7 +471,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             int nx_raw = -1;
             bool nx_pending = false;
             if (item != -1) {
-                if (in_static && item >= 0 && (r.pad & 1)) nx_raw = item + (int)gridDim.x;
+                if (in_static && item >= 0 && (r.pad & 1)) nx_raw = r.next;
                 else {
                     in_static = false;
                     if (lane == 0) nx_raw = atomicAdd(p.work_counter, 1) + p.n_static_slots;
@@ -975,7 +975,7 @@ static cudaError_t launch_kvt_n(const DecodeParams &p, const CUtensorMap &tmap, 
 }
 
 // grid: the number of CTAs the plan's static tile lists were laid out for (slot j of CTA b is record
-// j * grid + b); CTAs beyond the tiles still help with the combine units.
+// b, the rest of its list is chained through TileRec::next); CTAs beyond the tiles still help with the combine units.
 cudaError_t launch_decode_kvt(const DecodeParams &p, const void *tmap, int rows_per_page, int grid, int max_group,
                               cudaStream_t stream)
 {

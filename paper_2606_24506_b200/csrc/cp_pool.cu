@@ -167,6 +167,11 @@ struct cp_pool {
     bool last_stream_valid = false;
     cudaEvent_t ev_switch = nullptr, ev_fork = nullptr, ev_join = nullptr;
     cudaStream_t side_stream = nullptr, copy_stream = nullptr;
+    // page-table entries of GROWN requests go up on the copy stream from pinned staging (flush_tables)
+    struct TabPin { void *ptr = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; bool used = false; } tab_pin[4];
+    int tab_next = 0;
+    cudaEvent_t ev_tab = nullptr;
+    bool tab_recorded = false;
     int kind_ctas[2] = {0, 0};           // CTAs each attention kind of the cached plan was planned for
 
     // counters
@@ -299,6 +304,10 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
     // groups, split slots (in token order: static tiles, then tail tiles), combine units
     std::vector<int> split_base(ng, 0);
     kp.groups.reserve(ng);
+    // what all tile records of a group share, filled once per group (a rebuild sits between two decode steps of a
+    // serving loop: cfg5 rebuilds at 4 of 5 steps), and where the group's page ids are
+    std::vector<TileRec> rec_of(ng);
+    std::vector<const int32_t *> pages_of(ng);
     for (int g = 0; g < ng; ++g) {
         const GInfo &G = gi[g];
         const Request &r = pool->reqs[ids[G.b]];
@@ -319,58 +328,60 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
             ws += (uint64_t)part_group_floats(rows, ns, m.head_dim_v);
             const int zl = ns <= 8 ? 0 : (ns <= 32 ? 3 : (ns <= 128 ? 4 : 5));
             const int cols = 128 >> zl;
+            CombineUnit cu;
+            std::memset(&cu, 0, sizeof(cu));
+            cu.split_stride = cols;
+            cu.n_splits = ns;
+            cu.zl_log2 = zl;
+            cu.want = ns * 4;                               // one arrival per epilogue warp and tile
+            cu.group = g;
             for (int h = 0; h < rows; ++h) {
                 kp.combines.push_back(Combine{g, h});
                 // row (t, hh) of the group is row t * Hq + hh of the request's output (q_len = 1: row h)
                 const int64_t orow = (int64_t)(h / hpk) * m.n_q_heads + h % hpk;
+                cu.ml_off = gr.part_off + part_ml_off(rows, h, 0, ns, m.head_dim_v);
                 for (int c0 = 0; c0 < m.head_dim_v; c0 += cols) {
-                    CombineUnit cu;
-                    std::memset(&cu, 0, sizeof(cu));
                     // partial layout of this kernel: [h][c0 / cols][s][cols] (the unit's 512-byte reads are contiguous)
                     cu.part_off = gr.part_off + (int64_t)h * ns * m.head_dim_v + (int64_t)(c0 / cols) * ns * cols;
-                    cu.ml_off = gr.part_off + part_ml_off(rows, h, 0, ns, m.head_dim_v);
                     cu.out_off = gr.out_off + orow * m.head_dim_v + c0;
                     cu.lse_off = c0 == 0 ? gr.lse_off + orow : -1;
-                    cu.split_stride = cols;
-                    cu.n_splits = ns;
-                    cu.zl_log2 = zl;
-                    cu.want = ns * 4;                       // one arrival per epilogue warp and tile
-                    cu.group = g;
                     kp.cunits.push_back(cu);
                 }
             }
         }
         kp.groups.push_back(gr);
+        TileRec &t = rec_of[g];
+        std::memset(&t, 0, sizeof(t));
+        t.group = g; t.req = gr.req; t.kv_head = gr.kv_head; t.n_kv_heads = m.n_kv_heads;
+        t.n_splits = ns;
+        t.gsize = rows; t.n_q_heads = m.n_q_heads;
+        t.scale_log2 = (float)((double)m.softmax_scale * 1.4426950408889634);
+        t.q_off = gr.q_off; t.out_off = gr.out_off; t.lse_off = gr.lse_off; t.part_off = gr.part_off;
+        t.pad = (ns <= 8 ? 0 : (ns <= 32 ? 3 : (ns <= 128 ? 4 : 5))) << 8;   // bits 8..15: partial layout (zl of the group's units)
+        // (one new row per kv head and request: the packed k_new / v_new of a step stay far below 2^31 elements)
+        t.app_k_off = (int32_t)(pool->app_k_off[G.b] + (int64_t)gr.kv_head * m.head_dim_qk);
+        t.app_v_off = (int32_t)(pool->app_v_off[G.b] + (int64_t)gr.kv_head * m.head_dim_v);
+        pages_of[g] = r.pages.data() + gr.kv_head;        // page j of the group at [j * n_kv_heads]
     }
-    auto zl_of = [](int ns) { return ns <= 8 ? 0 : (ns <= 32 ? 3 : (ns <= 128 ? 4 : 5)); };
     auto make_rec = [&](const T &t, int split) {
         const GInfo &G = gi[t.g];
-        const Group &gr = kp.groups[t.g];
-        const cp_model_cfg &m = pool->models[gr.model];
-        TileRec r;
-        std::memset(&r, 0, sizeof(r));
-        r.group = t.g; r.req = gr.req; r.kv_head = gr.kv_head; r.n_kv_heads = m.n_kv_heads;
+        TileRec r = rec_of[t.g];
         r.page_begin = t.sl0 * pps; r.n_pages = std::min(t.sl1 * pps, G.n_lp) - r.page_begin;
-        r.split = split; r.n_splits = gr.n_splits;
-        r.gsize = m.n_q_heads / m.n_kv_heads * pool->qlen; r.n_q_heads = m.n_q_heads;
-        r.scale_log2 = (float)((double)m.softmax_scale * 1.4426950408889634);
-        r.q_off = gr.q_off; r.out_off = gr.out_off; r.lse_off = gr.lse_off; r.part_off = gr.part_off;
-        r.pad = zl_of(gr.n_splits) << 8;               // bits 8..15: partial layout; bit 0 (set below): another static slot follows
-        if (r.page_begin + r.n_pages == G.n_lp) r.pad |= 2;      // the group's last planned page is in this tile
-        r.app_k_off = pool->app_k_off[G.b] + (int64_t)gr.kv_head * m.head_dim_qk;
-        r.app_v_off = pool->app_v_off[G.b] + (int64_t)gr.kv_head * m.head_dim_v;
-        {
-            const Request &rq = pool->reqs[gr.req];
-            for (int i = 0; i < 8 && i < r.n_pages && i < pps; ++i)
-                r.first_pid[i] = rq.pages[(size_t)(r.page_begin + i) * m.n_kv_heads + gr.kv_head];
-        }
+        r.split = split;
+        // bit 0 of pad (set by the caller): another static record of the CTA follows; bit 1: the group's last planned page is here
+        if (r.page_begin + r.n_pages == G.n_lp) r.pad |= 2;
+        const int32_t *pg = pages_of[t.g] + (size_t)r.page_begin * r.n_kv_heads;
+        for (int i = 0; i < 8 && i < r.n_pages && i < pps; ++i) r.first_pid[i] = pg[(size_t)i * r.n_kv_heads];
         return r;
     };
     // split index of a tile = its rank inside the group by position (tl is in that order per group)
     std::vector<int> split_of(tl.size());
     for (size_t i = 0; i < tl.size(); ++i) split_of[i] = split_base[tl[i].g]++;
 
-    // device order: the CTAs' static lists interleaved (slot j of CTA b at j * grid + b), then the tail tiles, longest first
+    // device order: record b < grid = the first tile of CTA b's static list (n_pages = 0: it has none), then the rest of
+    // every CTA's list, contiguous and chained through TileRec::next (a list of lists would leave the array as sparse
+    // as its longest list: 2220 records for 523 tiles on cfg5, all of it cleared, copied and uploaded at every rebuild),
+    // then the tail tiles, longest first
     const int64_t n_pieces_used = n_static_tiles ? tl[n_static_tiles - 1].piece + 1 : 0;
     int grid = (int)std::min<int64_t>(n_ctas, std::max<int64_t>(std::max<int64_t>(n_pieces_used, 1),
                                                                  ((int64_t)kp.cunits.size() + KT_COMBINE_WARPS - 1) / KT_COMBINE_WARPS));
@@ -378,15 +389,19 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
     // (tl holds the static tiles in piece order, so CTA b's list is b's tiles in tl order: two counting passes)
     std::vector<int> cnt(grid, 0), slot_of(n_static_tiles);
     for (int i = 0; i < n_static_tiles; ++i) slot_of[i] = cnt[tl[i].piece % grid]++;
-    size_t rounds = 0;
-    for (int b = 0; b < grid; ++b) rounds = std::max(rounds, (size_t)cnt[b]);
-    kp.tile_recs.resize(rounds * (size_t)grid + (tl.size() - n_static_tiles));
-    std::memset(kp.tile_recs.data(), 0, kp.tile_recs.size() * sizeof(TileRec));
+    std::vector<int> cont(grid, 0);                  // where the rest of CTA b's list starts
+    size_t n_static_recs = n_static_tiles ? (size_t)grid : 0;
+    for (int b = 0; b < grid; ++b) { cont[b] = (int)n_static_recs; n_static_recs += (size_t)std::max(cnt[b] - 1, 0); }
+    kp.tile_recs.resize(n_static_recs + (tl.size() - n_static_tiles));
+    if (n_static_tiles)
+        for (int b = 0; b < grid; ++b)
+            if (cnt[b] == 0) std::memset(&kp.tile_recs[b], 0, sizeof(TileRec));
     for (int i = 0; i < n_static_tiles; ++i) {
         const int b = tl[i].piece % grid, j = slot_of[i];
-        TileRec &r = kp.tile_recs[(size_t)j * grid + b];
+        const int idx = j == 0 ? b : cont[b] + j - 1;
+        TileRec &r = kp.tile_recs[idx];
         r = make_rec(tl[i], split_of[i]);
-        r.pad |= j + 1 < cnt[b] ? 1 : 0;
+        if (j + 1 < cnt[b]) { r.pad |= 1; r.next = j == 0 ? cont[b] : idx + 1; }
     }
     std::vector<int> tails;
     for (size_t i = n_static_tiles; i < tl.size(); ++i) tails.push_back((int)i);
@@ -394,13 +409,13 @@ void build_plan_kvt(cp_pool *pool, const int32_t *ids, int n, KindPlan &kp, uint
         return (tl[a].sl1 - tl[a].sl0) > (tl[b].sl1 - tl[b].sl0);
     });
     for (size_t t = 0; t < tails.size(); ++t)
-        kp.tile_recs[rounds * (size_t)grid + t] = make_rec(tl[tails[t]], split_of[tails[t]]);
+        kp.tile_recs[n_static_recs + t] = make_rec(tl[tails[t]], split_of[tails[t]]);
     // the real tiles in device order (reporting: cp_decode_plan)
     kp.tiles.reserve(tl.size());
     for (const TileRec &r : kp.tile_recs)
         if (r.n_pages > 0) kp.tiles.push_back(Tile{r.group, r.split, r.page_begin, r.page_begin + r.n_pages});
     kp.grid = grid;
-    kp.n_static_slots = (int)(rounds * (size_t)grid);
+    kp.n_static_slots = (int)n_static_recs;
 }
 
 // ----------------------------------------------------------------------------- planner
@@ -577,8 +592,8 @@ void build_plan(cp_pool *pool, const int32_t *ids, int n)
             r.pad = pool->qlen > 1 ? m.n_q_heads / m.n_kv_heads : 0;
             r.scale_log2 = (float)((double)m.softmax_scale * 1.4426950408889634);
             r.q_off = gr.q_off; r.out_off = gr.out_off; r.lse_off = gr.lse_off; r.part_off = gr.part_off;
-            r.app_k_off = pool->app_k_off[gr.batch_index] + (int64_t)gr.kv_head * m.head_dim_qk;
-            r.app_v_off = pool->app_v_off[gr.batch_index] + (int64_t)gr.kv_head * m.head_dim_v;
+            r.app_k_off = (int32_t)(pool->app_k_off[gr.batch_index] + (int64_t)gr.kv_head * m.head_dim_qk);
+            r.app_v_off = (int32_t)(pool->app_v_off[gr.batch_index] + (int64_t)gr.kv_head * m.head_dim_v);
         }
         std::vector<int> last_pos(kp.groups.size(), 0);
         for (size_t i = 0; i < kp.tiles.size(); ++i) last_pos[kp.tiles[i].group] = (int)i;
@@ -715,7 +730,55 @@ cp_status adopt_stream(cp_pool *pool, cudaStream_t s)
 // Upload page-table rows and context lengths that changed since the last device call.
 cp_status flush_tables(cp_pool *pool, cudaStream_t stream)
 {
+    // Entries a request GAINED (r.uploaded > 0: the request's earlier entries are on the device) lie beyond every page
+    // a launch already enqueued reads, so they need no ordering behind those launches: they go up on the copy stream
+    // from pinned staging while the previous step's kernel still runs, and `stream` only waits for an event.  Measured:
+    // the same few bytes as a copy on the caller's stream in front of the kernel cost a decode loop 10-15 us of device
+    // time per page boundary (cfg5: 138 us per iteration against 126 for the attention alone).  A request's FIRST upload
+    // (or its re-upload after unmap + map) may overwrite entries that enqueued launches read: caller's stream, after
+    // everything the copy stream was given.
+    size_t grown = 0;
+    bool first = false;
     for (int rid = 0; rid < pool->max_requests; ++rid) {
+        const Request &r = pool->reqs[rid];
+        if (!r.live || r.uploaded >= r.pages.size()) continue;
+        if (r.uploaded > 0) grown += r.pages.size() - r.uploaded;
+        else first = true;
+    }
+    if (first && pool->tab_recorded && cudaStreamWaitEvent(stream, pool->ev_tab, 0) != cudaSuccess) return CP_ERR_CUDA;
+    if (grown) {
+        if (!pool->copy_stream && cudaStreamCreateWithFlags(&pool->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+        if (!pool->ev_tab && cudaEventCreateWithFlags(&pool->ev_tab, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+        cp_pool::TabPin &pb = pool->tab_pin[pool->tab_next++ % 4];
+        if (pb.used && cudaEventSynchronize(pb.ev) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+        if (pb.cap < grown * 4) {
+            if (pb.ptr) cudaFreeHost(pb.ptr);
+            pb.ptr = nullptr; pb.cap = 0;
+            const size_t want = (grown * 4 * 2 + 4095) & ~(size_t)4095;
+            if (cudaHostAlloc(&pb.ptr, want, cudaHostAllocDefault) != cudaSuccess) { cudaGetLastError(); pb.ptr = nullptr; return CP_ERR_CUDA; }
+            pb.cap = want;
+        }
+        if (!pb.ev && cudaEventCreateWithFlags(&pb.ev, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
+        size_t off = 0;
+        for (int rid = 0; rid < pool->max_requests; ++rid) {
+            Request &r = pool->reqs[rid];
+            if (!r.live || r.uploaded >= r.pages.size() || r.uploaded == 0) continue;
+            const size_t n = r.pages.size() - r.uploaded;
+            int32_t *src = (int32_t *)pb.ptr + off;
+            std::memcpy(src, r.pages.data() + r.uploaded, n * 4);
+            int32_t *dst = (int32_t *)pool->d_page_table.ptr + (size_t)rid * pool->max_ppr + r.uploaded;
+            if (cudaMemcpyAsync(dst, src, n * 4, cudaMemcpyHostToDevice, pool->copy_stream) != cudaSuccess) return CP_ERR_CUDA;
+            pool->n_h2d_bytes += n * 4;
+            r.uploaded = r.pages.size();
+            off += n;
+        }
+        if (cudaEventRecord(pb.ev, pool->copy_stream) != cudaSuccess || cudaEventRecord(pool->ev_tab, pool->copy_stream) != cudaSuccess ||
+            cudaStreamWaitEvent(stream, pool->ev_tab, 0) != cudaSuccess)
+            return CP_ERR_CUDA;
+        pb.used = true;
+        pool->tab_recorded = true;
+    }
+    for (int rid = 0; first && rid < pool->max_requests; ++rid) {
         Request &r = pool->reqs[rid];
         if (!r.live || r.uploaded >= r.pages.size()) continue;
         const size_t n = r.pages.size() - r.uploaded;
@@ -908,6 +971,8 @@ cp_status cp_pool_free(cp_pool *pool)
     if (pool->ev_join) cudaEventDestroy(pool->ev_join);
     if (pool->side_stream) cudaStreamDestroy(pool->side_stream);
     if (pool->copy_stream) cudaStreamDestroy(pool->copy_stream);
+    if (pool->ev_tab) cudaEventDestroy(pool->ev_tab);
+    for (auto &pb : pool->tab_pin) { if (pb.ptr) cudaFreeHost(pb.ptr); if (pb.ev) cudaEventDestroy(pb.ev); }
     pool->d_page_table.release(); pool->d_ctx.release(); pool->d_models.release(); pool->d_append.release(); pool->d_timeline.release();
     for (int k = 0; k < 2; ++k) {
         pool->plan[k].d_pack2[0].release(); pool->plan[k].d_pack2[1].release(); pool->plan[k].d_counters2[0].release(); pool->plan[k].d_counters2[1].release();
