@@ -53,8 +53,9 @@ constexpr int M2_SMEM_Q = 0;
 constexpr int M2_SMEM_STAGE = M2_Q_BYTES;                    // value ring
 constexpr int M2_SMEM_SRING = M2_SMEM_STAGE + M2_STAGES * M2_STAGE_BYTES;
 constexpr int M2_SMEM_P = M2_SMEM_SRING + M2_SR * M2_SPAIR;
-constexpr int M2_SMEM_XPOSE = M2_SMEM_P + 2 * M2_P_BYTES;   // epilogue transpose scratch: 4 warps x [32 rows][16 + 4 floats]
-constexpr int M2_SMEM_MISC = M2_SMEM_XPOSE + 4 * 2560;
+constexpr int M2_XPOSE_WARP = 32 * 36 * 4;                  // 4608: [32 rows][32 + 4 floats]
+constexpr int M2_SMEM_XPOSE = M2_SMEM_P + 2 * M2_P_BYTES;   // epilogue transpose scratch of the 4 softmax warps
+constexpr int M2_SMEM_MISC = M2_SMEM_XPOSE + 4 * M2_XPOSE_WARP;
 constexpr int M2_SMEM_BYTES = M2_SMEM_MISC + 2048;
 static_assert(M2_SMEM_BYTES <= 232448, "MLA pair kernel exceeds the 227 KB shared-memory limit");
 constexpr uint32_t M2_TMEM_COLS = 512;
@@ -119,49 +120,80 @@ __device__ __forceinline__ M2Item m2_item(const DecodeParams &p, int tile_idx)
 // kernel).  Same arithmetic and summation order as combine_units().
 static __device__ __noinline__ void m2_combine(const DecodeParams &p, int w, const int stride, float *wsm, const int lane)
 {
+    constexpr int NPF = 12;                                // value rows requested before the weights are known
     const int n = p.n_combine_units >> 1;
     int done_group = -1;
     for (; w < n; w += stride) {
         const CombineUnit cu = load_combine_unit<false>(p.cunits, 2 * w);
         const int ns = cu.n_splits;
         if (cu.group != done_group) {
-            if (lane == 0) wait_group(p.group_counters, cu.group, cu.want);
+            // relaxed polling with a short back-off, then one acquire fence (as kt_combine of the K/V kernel)
+            if (lane == 0) {
+                const int32_t *c = p.group_counters + (size_t)cu.group * kCounterStride;
+                unsigned nsl = 32;
+                while (ld_relaxed(c) < cu.want) {
+                    __nanosleep(nsl);
+                    if (nsl < 256) nsl <<= 1;
+                }
+                __threadfence();
+            }
             __syncwarp();
             done_group = cu.group;
         }
         const float2 *mlp = reinterpret_cast<const float2 *>(p.workspace + cu.ml_off);
         const float *src = p.workspace + cu.part_off + lane * 4;
         const int ss = cu.split_stride;
-        // the first value rows travel with the (m, l) pairs
-        float4 va[4], vb[4];
+        // ONE round trip for the (m, l) pairs (splits lane, lane + 32, ... stay in registers) and the first NPF value rows
+        float2 ml[8];
+        const bool small = ns <= 256;
+        if (small) {
 #pragma unroll
-        for (int s = 0; s < 4; ++s) {
+            for (int k = 0; k < 8; ++k) {
+                ml[k] = make_float2(-INFINITY, 0.f);
+                if (lane + 32 * k < ns) ml[k] = __ldcg(mlp + lane + 32 * k);
+            }
+        }
+        float4 va[NPF], vb[NPF];
+#pragma unroll
+        for (int s = 0; s < NPF; ++s) {
             va[s] = vb[s] = make_float4(0.f, 0.f, 0.f, 0.f);
             if (s < ns) { va[s] = ld_cg_f4(src + s * ss); vb[s] = ld_cg_f4(src + s * ss + 128); }
         }
         float M = -INFINITY, L = 0.f;
+        if (small) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) M = fmaxf(M, ml[k].x);
+            for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const float wgt = ex2_ftz(ml[k].x - M);            // 0 for absent splits (m = -inf)
+                if (lane + 32 * k < ns) wsm[lane + 32 * k] = wgt;
+                L += wgt * ml[k].y;
+            }
+        } else {
 #pragma unroll 8
-        for (int s = lane; s < ns; s += 32) M = fmaxf(M, __ldcg(mlp + s).x);
-        for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+            for (int s = lane; s < ns; s += 32) M = fmaxf(M, __ldcg(mlp + s).x);
+            for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
 #pragma unroll 8
-        for (int s = lane; s < ns; s += 32) {
-            const float2 ml = __ldcg(mlp + s);
-            const float wgt = ex2_ftz(ml.x - M);
-            wsm[s] = wgt;
-            L += wgt * ml.y;
+            for (int s = lane; s < ns; s += 32) {
+                const float2 x = __ldcg(mlp + s);
+                const float wgt = ex2_ftz(x.x - M);
+                wsm[s] = wgt;
+                L += wgt * x.y;
+            }
         }
         for (int o = 16; o > 0; o >>= 1) L += __shfl_xor_sync(0xffffffffu, L, o);
         __syncwarp();
         float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
 #pragma unroll
-        for (int s = 0; s < 4; ++s)
+        for (int s = 0; s < NPF; ++s)
             if (s < ns) {
                 const float wgt = wsm[s];
                 a.x += wgt * va[s].x; a.y += wgt * va[s].y; a.z += wgt * va[s].z; a.w += wgt * va[s].w;
                 b.x += wgt * vb[s].x; b.y += wgt * vb[s].y; b.z += wgt * vb[s].z; b.w += wgt * vb[s].w;
             }
 #pragma unroll 16
-        for (int s = 4; s < ns; ++s) {
+        for (int s = NPF; s < ns; ++s) {
             const float4 x = ld_cg_f4(src + s * ss), y = ld_cg_f4(src + s * ss + 128);
             const float wgt = wsm[s];
             a.x += wgt * x.x; a.y += wgt * x.y; a.z += wgt * x.z; a.w += wgt * x.w;
@@ -573,26 +605,29 @@ cp_decode_mla2_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap 
                 const int64_t rstride = final_out ? M2_DV : (int64_t)it.n_splits * M2_DV;
                 float *row0 = final_out ? p.out + it.out_off + (int64_t)head0 * M2_DV
                                         : p.workspace + it.part_off + part_o_off(head0, it.split, it.n_splits, M2_DV);
-                const uint32_t scr = smem_u32(smem + M2_SMEM_XPOSE) + (uint32_t)(warp - 2) * 2560;   // [32 rows][16 floats + 4 pad]
-                for (int c = 0; c < 256; c += 16) {
-                    uint32_t o[16];
-                    tmem_ld16(tl + c, o);
+                const uint32_t scr = smem_u32(smem + M2_SMEM_XPOSE) + (uint32_t)(warp - 2) * M2_XPOSE_WARP;   // [32 rows][32 floats + 4 pad]
+                for (int c = 0; c < 256; c += 32) {
+                    // 32 columns per pass (two tcgen05.ld in flight, one wait): a pass is a chain of dependent TMEM,
+                    // shared-memory and global accesses, and 16 passes of 16 columns took 3.4 us without any store
+                    uint32_t o[32];
+                    tmem_ld16(tl + c, *reinterpret_cast<uint32_t (*)[16]>(&o[0]));
+                    tmem_ld16(tl + c + 16, *reinterpret_cast<uint32_t (*)[16]>(&o[16]));
                     tmem_wait_ld();
-                    __syncwarp();                                            // previous chunk fully read back
+                    __syncwarp();                                            // previous pass fully read back
 #pragma unroll
-                    for (int j = 0; j < 16; j += 4)
-                        asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(scr + lane * 80 + j * 4),
+                    for (int j = 0; j < 32; j += 4)
+                        asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(scr + lane * 144 + j * 4),
                                      "f"(__uint_as_float(o[j]) * inv), "f"(__uint_as_float(o[j + 1]) * inv),
                                      "f"(__uint_as_float(o[j + 2]) * inv), "f"(__uint_as_float(o[j + 3]) * inv) : "memory");
                     __syncwarp();
                     // TMEM column c of MMA jj = c / 128 holds value column 256 jj + 128 th + c % 128
-                    const int col = 256 * (c >> 7) + 128 * th + (c & 127) + (lane & 3) * 4;
+                    const int col = 256 * (c >> 7) + 128 * th + (c & 127) + (lane & 7) * 4;
 #pragma unroll
-                    for (int r8 = 0; r8 < 4; ++r8) {
-                        const int r = r8 * 8 + (lane >> 2);
+                    for (int r4 = 0; r4 < 8; ++r4) {
+                        const int r = r4 * 4 + (lane >> 3);                   // a store instruction: 4 rows x 128 contiguous bytes
                         float4 v;
                         asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
-                                     : "r"(scr + r * 80 + (lane & 3) * 16) : "memory");
+                                     : "r"(scr + r * 144 + (lane & 7) * 16) : "memory");
                         if (head0 + r < it.n_heads) __stcg(reinterpret_cast<float4 *>(row0 + r * rstride + col), v);
                     }
                 }
