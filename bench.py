@@ -32,8 +32,8 @@ import numpy as np
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the decode kernel, from the committed `ncu --set full`
 # captures profiles/r2_ncu_full_cfg{2,3,4,5}.txt (cfg1, 0.66 MB, has no capture: its launch is latency, not traffic)
-NCU_TRAFFIC_BYTES = {2: 344.69e6 + 7.29e6, 3: 293.11e6 + 16.33e6, 4: 135.82e6 + 7.27e6, 5: 806.47e6 + 7.09e6}
-NCU_TENSOR_PIPE_PCT = {3: 47.9}       # sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active
+NCU_TRAFFIC_BYTES = {2: 344.69e6 + 7.29e6, 3: 293.33e6 + 16.32e6, 4: 135.82e6 + 7.27e6, 5: 806.47e6 + 7.09e6}
+NCU_TENSOR_PIPE_PCT = {3: 47.2}       # sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active
 
 METRIC = "paged decode-attention KV GB/s"
 UNIT = "GB/s"
