@@ -108,6 +108,7 @@ struct KtMisc {
     uint64_t q_full[2];                          // query buffers: the tile's rows have landed (cp.async of the scheduler warp)
     uint64_t tq_full[KT_TQ], tq_empty[KT_TQ];    // tile descriptors: scheduler -> MMA, softmax, epilogue warps
     uint64_t meta_full[KT_MQ], meta_empty[KT_MQ];   // tile records: scheduler -> producer
+    uint64_t app_done[KT_MQ];                    // the tile's LAST page may be requested (a fused append's row is in memory)
     KtDesc tq[KT_TQ];
     KtMeta meta[KT_MQ];
     uint32_t tmem_base;
@@ -368,7 +369,10 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             mbar_init(smem_u32(&mi->o_done[i]), 1); mbar_init(smem_u32(&mi->e_full[i]), 4); mbar_init(smem_u32(&mi->o_free[i]), 4);
         }
         for (int i = 0; i < KT_TQ; ++i) { mbar_init(smem_u32(&mi->tq_full[i]), 1); mbar_init(smem_u32(&mi->tq_empty[i]), 9); }
-        for (int i = 0; i < KT_MQ; ++i) { mbar_init(smem_u32(&mi->meta_full[i]), 1); mbar_init(smem_u32(&mi->meta_empty[i]), 1); }
+        for (int i = 0; i < KT_MQ; ++i) {
+            mbar_init(smem_u32(&mi->meta_full[i]), 1); mbar_init(smem_u32(&mi->meta_empty[i]), 1);
+            mbar_init(smem_u32(&mi->app_done[i]), 1);
+        }
         asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmap)) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_proxy_async();
@@ -401,9 +405,8 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             const int req = mt->req, hkv = mt->n_kv_heads, kvh = mt->kv_head, pb = mt->page_begin, npg = mt->n_pages;
             const int nf = min(pps, npg);                    // pages of the first slice: ids came with the tile record
             int32_t pid = lane < 8 ? mt->pid[lane] : 0;
-            __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(&mi->meta_empty[ms]));
-            ++ti;
+            const uint32_t tph = (ti / KT_MQ) & 1;          // phase of this tile's use of slot ms (the slot is given back when
+            ++ti;                                            // the tile's last page is out: app_done[ms] must not lap this warp)
             // translation of the pages behind them (step a2: one page-table entry per lane, 32 at a time) is
             // requested now -- it travels while the first slice is issued -- and one batch ahead from then on
             int32_t pid_nx = 0;
@@ -416,6 +419,9 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                     const int pg = jj % pps;                 // position of the page inside its slice
                     const uint32_t slot = gs % NS;
                     if (pg == 0) mbar_wait(smem_u32(&mi->empty[slot]), ((gs / NS) & 1) ^ 1);
+                    // the tile's last page is where a fused append writes: everything before it streams while the scheduler
+                    // warp fetches and stores the row (non-append tiles: the barrier is complete at the hand-over)
+                    if (jj == npg - 1) mbar_wait(smem_u32(&mi->app_done[ms]), tph);
                     if (elect_one()) {
                         const uint32_t fb = smem_u32(&mi->full[slot]);
                         if (pg == 0) mbar_arrive_expect_tx(fb, (uint32_t)min(pps, npg - jj) * (uint32_t)P * 512u);
@@ -443,6 +449,8 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 pid_nx = 0;
                 if (j0 + 32 + lane < npg) pid_nx = page_of(p, req, (int64_t)(pb + j0 + 32 + lane) * hkv + kvh);
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&mi->meta_empty[ms]));
         }
         if (lane == 0) {
             // The next kernel of the stream, if it was launched as a programmatic dependent, may now take the SMs this
@@ -464,6 +472,10 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
         TileRec r = r_next;
         bool in_static = true;
         uint32_t ti = 0;
+        bool have_pre = false;                               // the tile's context length / append operands were requested a tile ago
+        int ctx_pre = 0;
+        int32_t pid_pre = 0;
+        uint4 row_pre = make_uint4(0u, 0u, 0u, 0u);
         for (;;) {
             if (item >= 0 && r.n_pages == 0) item = -2;      // empty static slot of this CTA: skip, go dynamic
             // ---- the tile after this one: the next static slot of this CTA, else a pop from the dynamic list
@@ -517,26 +529,45 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 if (lane == 0) mbar_arrive(smem_u32(&mi->meta_full[ms]));   // release: the producer acquires via try_wait
             };
             if (lane == 0 && ti == 0) kt_stamp(p, 15);
-            // The producer gets the tile as soon as the record is there (the first slice's page ids came with it), unless
-            // this tile writes a fused append's row, which has to be in memory before its page is requested.
-            if (!app) hand_to_producer();
+            // The producer gets the tile as soon as the record is there (the first slice's page ids came with it).  A tile
+            // that writes a fused append's row streams too: only its LAST page -- where the row goes -- waits (app_done).
+            hand_to_producer();
+            if (!app && lane == 0) mbar_arrive(smem_u32(&mi->app_done[ms]));
             // ---- one round trip: the context length (it decides only how many tokens of the tile's LAST slice are
             // valid: every planned page holds a valid token, contexts never shrink under a plan), the query rows
             // and, for a fused append, the new row and its page.  Volatile asm: issued here, not sunk to first use.
+            // (Requested one tile AHEAD where there was a tile before this one, see the end of the loop: a list of short
+            // tiles that all write an append row is otherwise bound by this warp -- round trip, store, fence: ~2 us per
+            // tile against 2.6 us of streaming for two slices -- and cfg5's fused step ended 4 us late.)
             int ctx;
-            asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(ctx) : "l"(p.req_ctx + r.req));
+            if (have_pre) ctx = ctx_pre;
+            else asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(ctx) : "l"(p.req_ctx + r.req));
             ctx += p.ctx_add;                    // a fused step reads the table of the step before (see req_ctx_next)
             // ---- fused append (cp_decode_step): the tile that holds its group's last page writes the
-            // new token's K and V rows (position ctx - 1) before the producer is told about the tile, i.e. before
+            // new token's K and V rows (position ctx - 1) before the producer may request that page (app_done), i.e. before
             // the page is requested.  Source row and the page's id travel in the same round trip.
             uint4 app_row = make_uint4(0u, 0u, 0u, 0u);
             int32_t app_pid = 0;
-            if (app) {
+            if (app && have_pre) { app_row = row_pre; app_pid = pid_pre; }
+            else if (app) {
                 const uint16_t *src = lane < 16 ? p.app_k + r.app_k_off + lane * 8 : p.app_v + r.app_v_off + (lane - 16) * 8;
                 asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(app_row.x), "=r"(app_row.y), "=r"(app_row.z), "=r"(app_row.w) : "l"(src));
                 const int64_t idx = (int64_t)(r.page_begin + r.n_pages - 1) * r.n_kv_heads + r.kv_head;
                 if (p.slot_pages > 0) app_pid = r.req * p.slot_pages + (int32_t)idx;
                 else asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(app_pid) : "l"(p.page_table + (int64_t)r.req * p.max_ppr + idx));
+            }
+            if (app) {
+                // the row goes in and the producer gets the tile BEFORE this warp waits for a free query buffer below:
+                // with lists of short tiles that wait is what bounds the warp's lead over the producer
+                const int slot = (ctx - 1) % P;
+                uint8_t *dst = const_cast<uint8_t *>(p.arena) + (size_t)app_pid * p.page_bytes + (size_t)slot * (KT_D * 2) +
+                               (lane < 16 ? (size_t)lane * 16 : (size_t)P * (KT_D * 2) + (size_t)(lane - 16) * 16);
+                *reinterpret_cast<uint4 *>(dst) = app_row;
+                // the row is read by TMA (async proxy) that another thread issues after the hand-over below
+                __threadfence();
+                fence_proxy_async_all();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&mi->app_done[ms]));      // release: the producer acquires via try_wait
             }
             // ---- the tile's query rows -> buffer (ti & 1), asynchronously: two K-major [N x 64] blocks, 128-byte
             // swizzle (16-B chunk index ^ (row & 7)); rows beyond the group are zero-filled.  The buffer is free
@@ -559,17 +590,6 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
                 asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(&mi->q_full[ti & 1])) : "memory");
             }
             resolve_next();
-            if (app) {
-                const int slot = (ctx - 1) % P;
-                uint8_t *dst = const_cast<uint8_t *>(p.arena) + (size_t)app_pid * p.page_bytes + (size_t)slot * (KT_D * 2) +
-                               (lane < 16 ? (size_t)lane * 16 : (size_t)P * (KT_D * 2) + (size_t)(lane - 16) * 16);
-                *reinterpret_cast<uint4 *>(dst) = app_row;
-                // the row is read by TMA (async proxy) that another thread issues after the hand-over below
-                __threadfence();
-                fence_proxy_async_all();
-                __syncwarp();
-            }
-            if (app) hand_to_producer();
             mbar_wait(smem_u32(&mi->tq_empty[qs]), ((ti / KT_TQ) & 1) ^ 1);
             if (lane == 0) {
                 const int t_begin = r.page_begin * P;
@@ -587,6 +607,20 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
             }
             __syncwarp();
             ++ti;
+            // ---- the NEXT tile's context length (and append operands) are requested now: they travel while this warp
+            // waits for queue slots, and the next round starts with them in registers
+            have_pre = false;
+            if (item_next >= 0 && r_next.n_pages > 0) {
+                asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(ctx_pre) : "l"(p.req_ctx + r_next.req));
+                if (p.app_k != nullptr && (r_next.pad & 2)) {
+                    const uint16_t *src = lane < 16 ? p.app_k + r_next.app_k_off + lane * 8 : p.app_v + r_next.app_v_off + (lane - 16) * 8;
+                    asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(row_pre.x), "=r"(row_pre.y), "=r"(row_pre.z), "=r"(row_pre.w) : "l"(src));
+                    const int64_t idx = (int64_t)(r_next.page_begin + r_next.n_pages - 1) * r_next.n_kv_heads + r_next.kv_head;
+                    if (p.slot_pages > 0) pid_pre = r_next.req * p.slot_pages + (int32_t)idx;
+                    else asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(pid_pre) : "l"(p.page_table + (int64_t)r_next.req * p.max_ppr + idx));
+                }
+                have_pre = true;
+            }
             item = item_next; r = r_next;
         }
     } else if (warp == 1) {
