@@ -32,8 +32,8 @@ import numpy as np
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the decode kernel, from the committed `ncu --set full`
 # captures profiles/r2_ncu_full_cfg{2,3,4,5}.txt (cfg1, 0.66 MB, has no capture: its launch is latency, not traffic)
-NCU_TRAFFIC_BYTES = {2: 344.69e6 + 7.29e6, 3: 293.33e6 + 16.32e6, 4: 135.82e6 + 7.27e6, 5: 806.47e6 + 7.09e6}
-NCU_TENSOR_PIPE_PCT = {3: 47.2}       # sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active
+NCU_TRAFFIC_BYTES = {2: 344.68e6 + 7.64e6, 3: 293.21e6 + 16.84e6, 4: 135.82e6 + 7.35e6, 5: 806.45e6 + 7.51e6}
+NCU_TENSOR_PIPE_PCT = {3: 47.0}       # sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active
 
 METRIC = "paged decode-attention KV GB/s"
 UNIT = "GB/s"
@@ -830,9 +830,33 @@ def main():
                     "launches_per_iteration": (c1["kernel_launches"] - c0["kernel_launches"]) / steps,
                     "plan_builds": c1["plan_builds"] - c0["plan_builds"]}
         loop(True, 4)
+
+        def single_step_device_us(reps=8):
+            """Kernel duration on the device (first CTA entry to last CTA done, CP_OPT_TIMELINE) of single steps, one at a
+            time, no flush: the plain step and the fused step alternate, so both see the same cache state."""
+            dw.pool.set_option(cp.CP_OPT_TIMELINE, 1)
+            res = {"plain": [], "fused": []}
+            try:
+                for _ in range(reps):
+                    for name in ("plain", "fused"):
+                        if name == "plain":
+                            dw.pool.decode_attention(dw.ids, dw.q, dw.out, dw.lse, wsl, wsl.numel(), dw.stream())
+                        else:
+                            dw.pool.decode_step(dw.ids, k_new, v_new, dw.q, dw.out, dw.lse, wsl, wsl.numel(), dw.stream())
+                        torch.cuda.synchronize()
+                        t = dw.pool.read_timeline().astype(np.int64)
+                        t = t[t[:, 0] > 0]
+                        if t.size == 0 or t[:, 7].max() == 0:
+                            return None              # a kernel that does not stamp (MLA, generic)
+                        res[name].append((t[:, 7].max() - t[:, 0].min()) / 1e3)
+            finally:
+                dw.pool.set_option(cp.CP_OPT_TIMELINE, 0)
+            return {k: float(np.median(v)) for k, v in res.items()}
+        dev_cmp = single_step_device_us()
         append["decode_loop"] = {"iterations": n_loop,
                                  "fused_cp_decode_step": loop(True, n_loop),
                                  "append_then_attention": loop(False, n_loop),
+                                 "single_step_kernel_us_on_device": dev_cmp,
                                  "plain_step_cached_plan_us": back_to_back_us,
                                  "note": "a free-running loop (no device-side spin in front): us_per_iteration is wall clock from the "
                                          "first enqueue to the final synchronise, i.e. max(host, device); every request crosses a "
