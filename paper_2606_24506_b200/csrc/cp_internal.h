@@ -219,8 +219,6 @@ struct DecodeParams {
     const Combine *combines;
     const CombineUnit *cunits;     // [n_combine_units] (tensor-core kernels)
     int32_t n_tiles;
-    const uint32_t *plan_flag;     // tcgen05 K/V kernel, first launch after a plan upload: the plan (and the page-table entries
-    uint32_t plan_version;         // uploaded before it) may be read once *plan_flag == plan_version (nullptr: nothing to wait for)
     int32_t n_static_slots;        // tcgen05 K/V kernel: records [0, n_static_slots) are the CTAs' static lists (slot j of CTA b
                                    // at index b < gridDim.x, TileRec::pad bit 0 = another one follows at TileRec::next), the rest is popped
     int32_t n_combines;            // work items after the tiles (CTA-sized combine items)

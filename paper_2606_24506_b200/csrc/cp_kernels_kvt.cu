@@ -171,20 +171,6 @@ __device__ __forceinline__ float col_reduce(float (&v)[CN], const int lane, Op o
     return v[0];
 }
 
-// First launch after a plan upload: the host did not make the stream wait for the copy stream (that would cost the
-// overlap of this kernel's set-up with the previous kernel's tail); whoever reads plan data or page-table entries
-// first waits here until the copy stream has set the flag word behind the plan.  Acquire loads; a flag that never
-// comes (a host-side bug) ends in a trap, not in a hang.
-__device__ __forceinline__ void kt_wait_plan(const DecodeParams &p)
-{
-    if (p.plan_flag == nullptr) return;
-    const unsigned long long t0 = global_timer_ns();
-    while ((uint32_t)ld_acquire(reinterpret_cast<const int32_t *>(p.plan_flag)) != p.plan_version) {
-        __nanosleep(64);
-        if (global_timer_ns() - t0 > 2000000000ull) __trap();
-    }
-}
-
 __device__ __forceinline__ TileRec load_tile_rec(const TileRec *recs, int item)
 {
     TileRec r;
@@ -364,8 +350,7 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
     bool has_next = false;
     if (warp == KT_WARPS - 1) {
         has_next = (int)blockIdx.x < p.n_static_slots;
-        // (first launch after a plan upload: the record may still be on its way, see kt_wait_plan below)
-        if (has_next && p.plan_flag == nullptr) r_next = load_tile_rec(p.tile_recs, blockIdx.x);
+        if (has_next) r_next = load_tile_rec(p.tile_recs, blockIdx.x);
     }
     if (tid == 0) {
         kt_stamp(p, 0);
@@ -483,10 +468,6 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
         // hands the tile to the producer (meta ring) and to the MMA / softmax / epilogue warps (tile queue),
         // up to KT_MQ tiles ahead of the producer -- a dependent global load takes microseconds while 148 SMs
         // stream at full rate, and none of them is on the producer's path.
-        if (p.plan_flag != nullptr) {
-            kt_wait_plan(p);
-            if (has_next) r_next = load_tile_rec(p.tile_recs, blockIdx.x);
-        }
         int item = has_next ? (int)blockIdx.x : -3;          // -3: no static slot at all, start with the dynamic list
         TileRec r = r_next;
         bool in_static = true;
@@ -897,7 +878,6 @@ cp_decode_kvt_kernel(const DecodeParams p, const __grid_constant__ CUtensorMap t
         // the next launch.  (2) Fused decode step: the context table of the launches that follow is filled -- every
         // entry copied, then the batch's requests set to + ctx_add (no launch reads the table it writes).
         if (warp == 9 && blockIdx.x == gridDim.x - 1) {
-            kt_wait_plan(p);                                 // the counters were cleared by the copy stream, before the flag
             for (int i = lane; i < p.n_groups; i += 32) p.reset_counters[32 + (size_t)i * kCounterStride] = 0;
             if (lane < 4) p.reset_counters[lane] = 0;
             if (p.req_ctx_next != nullptr) {

@@ -78,12 +78,6 @@ struct KindPlan {
     cudaEvent_t ev_copied = nullptr;                // the copy stream has finished the current plan's upload
     void *p_counters = nullptr;
     bool users_recorded[2] = {false, false};
-    // tcgen05 K/V plans: the launch that follows an upload does not wait for the copy stream's event (a stream wait
-    // between two kernels costs the programmatic overlap and ~5 us); its scheduler warp polls a flag word behind the
-    // pack, which the copy stream sets to `version` after the copy and the counter memset
-    uint32_t version = 0;
-    const uint32_t *p_flag = nullptr;
-    bool flag_pending = false;           // the next launch of this plan must wait for the flag
     // pinned staging, a ring of four: a pageable source would make cudaMemcpyAsync wait for the stream (the copy is
     // staged chunk by chunk behind the work already queued), i.e. synchronise host and device on every new plan
     struct PinBuf { void *ptr = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; bool used = false; } pin[4];
@@ -178,7 +172,6 @@ struct cp_pool {
     int tab_next = 0;
     cudaEvent_t ev_tab = nullptr;
     bool tab_recorded = false;
-    bool tab_wait_pending = false;       // grown entries are on their way on the copy stream and no stream waits for them yet
     int kind_ctas[2] = {0, 0};           // CTAs each attention kind of the cached plan was planned for
 
     // counters
@@ -735,7 +728,7 @@ cp_status adopt_stream(cp_pool *pool, cudaStream_t s)
 }
 
 // Upload page-table rows and context lengths that changed since the last device call.
-cp_status flush_tables(cp_pool *pool, cudaStream_t stream, bool defer_wait = false)
+cp_status flush_tables(cp_pool *pool, cudaStream_t stream)
 {
     // Entries a request GAINED (r.uploaded > 0: the request's earlier entries are on the device) lie beyond every page
     // a launch already enqueued reads, so they need no ordering behind those launches: they go up on the copy stream
@@ -744,10 +737,6 @@ cp_status flush_tables(cp_pool *pool, cudaStream_t stream, bool defer_wait = fal
     // time per page boundary (cfg5: 138 us per iteration against 126 for the attention alone).  A request's FIRST upload
     // (or its re-upload after unmap + map) may overwrite entries that enqueued launches read: caller's stream, after
     // everything the copy stream was given.
-    if (!defer_wait && pool->tab_wait_pending) {           // left over by a call whose launch did not happen
-        if (cudaStreamWaitEvent(stream, pool->ev_tab, 0) != cudaSuccess) return CP_ERR_CUDA;
-        pool->tab_wait_pending = false;
-    }
     size_t grown = 0;
     bool first = false;
     for (int rid = 0; rid < pool->max_requests; ++rid) {
@@ -783,12 +772,9 @@ cp_status flush_tables(cp_pool *pool, cudaStream_t stream, bool defer_wait = fal
             r.uploaded = r.pages.size();
             off += n;
         }
-        if (cudaEventRecord(pb.ev, pool->copy_stream) != cudaSuccess || cudaEventRecord(pool->ev_tab, pool->copy_stream) != cudaSuccess)
+        if (cudaEventRecord(pb.ev, pool->copy_stream) != cudaSuccess || cudaEventRecord(pool->ev_tab, pool->copy_stream) != cudaSuccess ||
+            cudaStreamWaitEvent(stream, pool->ev_tab, 0) != cudaSuccess)
             return CP_ERR_CUDA;
-        // (defer_wait: a decode launch follows in this call; if it waits for its plan on the flag word -- set by the copy
-        // stream after these copies -- the stream needs no wait at all, else the launch code makes it wait: tab_wait_pending)
-        if (defer_wait) pool->tab_wait_pending = true;
-        else if (cudaStreamWaitEvent(stream, pool->ev_tab, 0) != cudaSuccess) return CP_ERR_CUDA;
         pb.used = true;
         pool->tab_recorded = true;
     }
@@ -823,8 +809,6 @@ cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
     size_t off[5], total = 0;
     for (int i = 0; i < 5; ++i) { off[i] = total; total += (bytes[i] + 255) & ~(size_t)255; }
     total = std::max(total, (size_t)256);
-    const size_t flag_off = total;            // the flag word (device) / its new value (staging) live behind the pack
-    total += 256;
     const int t = 1 - kp.buf;                 // target pair: not the one the stream's queued launches read
     if (kp.d_pack2[t].ensure(total) != cudaSuccess || kp.d_counters2[t].ensure(nb) != cudaSuccess) {
         cudaGetLastError();
@@ -846,31 +830,25 @@ cp_status upload_plan(cp_pool *pool, KindPlan &kp, cudaStream_t stream)
     if (!pb.ev && cudaEventCreateWithFlags(&pb.ev, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
     for (int i = 0; i < 5; ++i)
         if (bytes[i]) std::memcpy((uint8_t *)pb.ptr + off[i], src[i], bytes[i]);
-    const uint32_t version = ++kp.version;
-    std::memcpy((uint8_t *)pb.ptr + flag_off, &version, 4);
     // copy stream: wait for the launches that read pair t (all enqueued before the plan moved to the other pair: ev_users[t]
     // was recorded then), copy, clear the counters (two sets for alternate launches; a new plan starts from zero)
     cudaStream_t cs = pool->copy_stream;
     if ((kp.users_recorded[t] && cudaStreamWaitEvent(cs, kp.ev_users[t], 0) != cudaSuccess) ||
-        cudaMemcpyAsync(kp.d_pack2[t].ptr, pb.ptr, flag_off, cudaMemcpyHostToDevice, cs) != cudaSuccess ||
-        cudaMemsetAsync(kp.d_counters2[t].ptr, 0, kp.d_counters2[t].cap, cs) != cudaSuccess ||
-        cudaMemcpyAsync((uint8_t *)kp.d_pack2[t].ptr + flag_off, (uint8_t *)pb.ptr + flag_off, 4, cudaMemcpyHostToDevice, cs) != cudaSuccess ||
+        cudaMemcpyAsync(kp.d_pack2[t].ptr, pb.ptr, total, cudaMemcpyHostToDevice, cs) != cudaSuccess ||
         cudaEventRecord(pb.ev, cs) != cudaSuccess ||
+        cudaMemsetAsync(kp.d_counters2[t].ptr, 0, kp.d_counters2[t].cap, cs) != cudaSuccess ||
         cudaEventRecord(kp.ev_copied, cs) != cudaSuccess)
         return CP_ERR_CUDA;
     pb.used = true;
-    // caller's stream: everything enqueued so far may read the old pair; the launches that follow wait for the copy --
-    // by a stream wait, or (tcgen05 K/V plans) inside the kernel on the flag word
-    if (cudaEventRecord(kp.ev_users[kp.buf], stream) != cudaSuccess) return CP_ERR_CUDA;
-    kp.flag_pending = kp.use_kvt;
-    if (!kp.use_kvt && cudaStreamWaitEvent(stream, kp.ev_copied, 0) != cudaSuccess) return CP_ERR_CUDA;
+    // caller's stream: everything enqueued so far may read the old pair; the launches that follow wait for the copy
+    if (cudaEventRecord(kp.ev_users[kp.buf], stream) != cudaSuccess || cudaStreamWaitEvent(stream, kp.ev_copied, 0) != cudaSuccess)
+        return CP_ERR_CUDA;
     kp.users_recorded[kp.buf] = true;
     kp.buf = t;
     uint8_t *base = (uint8_t *)kp.d_pack2[t].ptr;
     kp.p_groups = base + off[0]; kp.p_tiles = base + off[1]; kp.p_tile_recs = base + off[2];
     kp.p_combines = base + off[3]; kp.p_cunits = base + off[4];
     kp.p_counters = kp.d_counters2[t].ptr;
-    kp.p_flag = (const uint32_t *)(base + flag_off);
     kp.counter_set = 0;
     pool->n_h2d_bytes += total;
     kp.uploaded = true;
@@ -1396,25 +1374,17 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
     cudaStream_t s = (cudaStream_t)stream;
     st = adopt_stream(pool, s);
     if (st != CP_OK) return st;
-    st = flush_tables(pool, s, true);
+    st = flush_tables(pool, s);
     if (st != CP_OK) return st;
 
     // A batch with both attention kinds: everything either launch reads is uploaded on the caller's stream first;
     // then the second kind's kernel runs beside the first on a stream of the pool's own (fork here, join below).
     const bool both_kinds = !pool->plan[0].tiles.empty() && !pool->plan[1].tiles.empty();
     cudaStream_t s_main = s;
-    bool all_on_flag = true;                   // every launch of this call waits for its plan on the flag word
     for (int k = 0; k < 2; ++k) {
         if (pool->plan[k].tiles.empty()) continue;
         st = upload_plan(pool, pool->plan[k], s_main);
         if (st != CP_OK) return st;
-        if (!(pool->plan[k].use_kvt && pool->plan[k].flag_pending && pool->kv_tmap_ok)) all_on_flag = false;
-    }
-    if (pool->tab_wait_pending) {
-        // page-table entries of grown requests are on the copy stream: in front of the plan copy and its flag, so a
-        // launch that waits on the flag has them; any other launch gets a stream wait
-        if (!all_on_flag && cudaStreamWaitEvent(s_main, pool->ev_tab, 0) != cudaSuccess) { cudaGetLastError(); return CP_ERR_CUDA; }
-        pool->tab_wait_pending = false;
     }
     if (pool->opt_timeline) {
         const size_t tb = (size_t)pool->n_sm * kTimelineSlots * sizeof(unsigned long long);
@@ -1475,7 +1445,6 @@ cp_status cp_decode_attention(cp_pool *pool, const int32_t *request_ids_host, in
         const int n_ctas = pool->kind_ctas[k];
         cudaError_t e;
         if (k == CP_KIND_KV && kp.use_kvt && pool->kv_tmap_ok) {
-            if (kp.flag_pending) { prm.plan_flag = kp.p_flag; prm.plan_version = kp.version; kp.flag_pending = false; }
             prm.n_combine_units = (int)kp.cunits.size();
             prm.n_tiles = (int)kp.tile_recs.size();          // static slots (some empty) + dynamic tiles
             prm.n_static_slots = kp.n_static_slots;
@@ -1548,7 +1517,7 @@ cp_status cp_decode_step(cp_pool *pool, const int32_t *request_ids_host, int32_t
     // one for later launches), so a decode iteration uploads nothing but the ids of newly opened pages.
     const bool ctx_on_device = fused_kv && sep.empty() && pool->plan[CP_KIND_MLA].tiles.empty();
     if (ctx_on_device) { pool->ctx_dirty_lo = INT32_MAX; pool->ctx_dirty_hi = -1; }     // the only dirty entries are this step's
-    st = flush_tables(pool, s, sep.empty());    // (no append kernel in front: the decode launch below settles the wait)
+    st = flush_tables(pool, s);
     if (st != CP_OK) return st;
     st = launch_append_recs(pool, sep, k_new_dev, v_new_dev, s);
     if (st != CP_OK) return st;
